@@ -1,0 +1,233 @@
+"""ctypes binding of the CPU fp64 oracle (oracle/m3dk_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+``--impl reference`` legs.  Never imported by paper_2107_13663_b200 (the product path), and it imports
+nothing from it.  ``build()`` compiles the C file in-tree with gcc -O2 -ffp-contract=off -fopenmp.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "m3dk_oracle.c")
+_SO = os.path.join(_HERE, "libm3dk_oracle.so")
+_lib = None
+
+c_dp = C.POINTER(C.c_double)
+c_ip = C.POINTER(C.c_int)
+c_lp = C.POINTER(C.c_long)
+
+
+class Analytic(C.Structure):
+    _fields_ = [("R0", C.c_double), ("a", C.c_double), ("B0", C.c_double), ("qkind", C.c_int),
+                ("qc", C.c_double * 3), ("kappa", C.c_double), ("pA", C.c_double), ("prc", C.c_double),
+                ("pwd", C.c_double), ("pomega", C.c_double), ("pn", C.c_int), ("pm", C.c_int)]
+
+
+class Species(C.Structure):
+    _fields_ = [("charge", C.c_double), ("mass", C.c_double), ("f0kind", C.c_int), ("f0par", C.c_double * 5)]
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-Wall", "-o", _SO, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _SO
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.orc_mesh_create.restype = C.c_void_p
+        L.orc_mesh_create.argtypes = [C.c_int, c_dp, C.c_int, c_ip, c_dp, C.c_int, c_ip, c_dp, c_dp]
+        L.orc_mesh_free.argtypes = [C.c_void_p]
+        L.orc_locate.argtypes = [C.c_void_p, C.c_long, c_dp, c_dp, c_ip, C.c_int]
+        L.orc_eval_fe.argtypes = [C.c_void_p, C.c_long, c_dp, c_dp, c_dp, C.c_double, c_ip, c_dp]
+        L.orc_eval_analytic.argtypes = [C.POINTER(Analytic), C.c_long, c_dp, c_dp, c_dp, C.c_double, c_dp, c_dp]
+        L.orc_push_fe.restype = C.c_long
+        L.orc_push_fe.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_ip, C.c_int, C.c_double,
+                                  C.c_double, C.c_long, C.c_int, C.c_int]
+        L.orc_push_analytic.restype = C.c_long
+        L.orc_push_analytic.argtypes = [C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 8 + [
+            C.c_int, C.c_double, C.c_double, C.c_long, C.c_int]
+        L.orc_trace.restype = C.c_long
+        L.orc_trace.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_long, C.c_double,
+                                C.c_double, C.c_long, c_dp]
+        L.orc_push_uniform.argtypes = [C.c_long] + [c_dp] * 6 + [c_dp, c_dp, C.c_double, C.c_double, C.c_long, C.c_double]
+        L.orc_eq6.argtypes = [c_dp, c_dp, c_dp, C.c_double, c_dp]
+        L.orc_weight_rhs.restype = C.c_double
+        L.orc_weight_rhs.argtypes = [c_dp, C.POINTER(Species), C.c_double, c_dp, C.c_double]
+        L.orc_sort_perm.argtypes = [C.c_long, c_ip, C.c_int, c_lp]
+        L.orc_max_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(c_dp)
+
+
+def _i(a):
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, a.ctypes.data_as(c_ip)
+
+
+def species(charge, mass, f0kind=0, T=1.0, v_c=0.3, Lambda0=0.75, dLambda=0.2, B_axis=1.0) -> Species:
+    s = Species()
+    s.charge, s.mass, s.f0kind = float(charge), float(mass), int(f0kind)
+    for k, v in enumerate((T, v_c, Lambda0, dLambda, B_axis)):
+        s.f0par[k] = float(v)
+    return s
+
+
+def species_of(workload) -> Species:
+    f = workload.f0
+    return species(workload.charge, workload.mass, f.kind, f.T, f.v_c, f.Lambda0, f.dLambda, f.B_axis)
+
+
+def analytic_of(eq, kappa=0.0, pA=0.0, prc=0.5, pwd=0.1, pomega=0.0, pn=0, pm=0) -> Analytic:
+    a = Analytic()
+    a.R0, a.a, a.B0, a.qkind = eq.R0, eq.a, eq.B0, eq.qkind
+    for k in range(3):
+        a.qc[k] = eq.qc[k]
+    a.kappa, a.pA, a.prc, a.pwd, a.pomega, a.pn, a.pm = kappa, pA, prc, pwd, pomega, pn, pm
+    return a
+
+
+class Mesh:
+    """Finite-element tables in the layouts include/m3dk.h documents; arrays are kept alive here."""
+
+    def __init__(self, node_RZ, tri, eq_coef, pert_coef=None, n_tor=None, omega=None):
+        self.node_RZ, p_nodes = _d(node_RZ)
+        self.tri, p_tri = _i(tri)
+        self.eq_coef, p_eq = _d(eq_coef)
+        self.n_elems = self.tri.shape[0]
+        n_modes = 0 if n_tor is None else len(n_tor)
+        self.n_modes = n_modes
+        self.pert_coef, p_pc = _d(pert_coef if n_modes else np.zeros(1))
+        self.n_tor, p_nt = _i(n_tor if n_modes else np.zeros(1, dtype=np.int32))
+        self.omega, p_om = _d(omega if n_modes else np.zeros(1))
+        assert self.eq_coef.shape == (self.n_elems, 4, 21)
+        if n_modes:
+            assert self.pert_coef.shape == (n_modes, self.n_elems, 7, 2, 21)
+        self.h = lib().orc_mesh_create(self.node_RZ.shape[0], p_nodes, self.n_elems, p_tri, p_eq, n_modes, p_nt, p_om, p_pc)
+
+    @classmethod
+    def of(cls, w):
+        return cls(w.node_RZ, w.tri, w.eq_coef, w.pert_coef, w.n_tor, w.omega)
+
+    def __del__(self):
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.orc_mesh_free(self.h)
+            self.h = None
+
+    def locate(self, R, Z, brute=False):
+        R, pR = _d(R)
+        Z, pZ = _d(Z)
+        out = np.empty(R.shape[0], dtype=np.int32)
+        lib().orc_locate(self.h, R.shape[0], pR, pZ, out.ctypes.data_as(c_ip), int(brute))
+        return out
+
+    def eval(self, R, phi, Z, t=0.0):
+        R, pR = _d(R)
+        phi, pP = _d(phi)
+        Z, pZ = _d(Z)
+        n = R.shape[0]
+        elem = np.empty(n, dtype=np.int32)
+        out = np.full((n, 18), np.nan)
+        lib().orc_eval_fe(self.h, n, pR, pP, pZ, float(t), elem.ctypes.data_as(c_ip), out.ctypes.data_as(c_dp))
+        return elem, out
+
+
+FIELD_COLS = ("psi_R", "psi_Z", "Bm", "Bm_R", "Bm_Z", "F", "kappa", "E1_R", "E1_phi", "E1_Z", "B1_R", "B1_phi",
+              "B1_Z", "gB1p_R", "gB1p_phi", "gB1p_Z", "dtB1p", "B1p")
+
+
+def eval_analytic(an: Analytic, R, phi, Z, t=0.0):
+    R, pR = _d(R)
+    phi, pP = _d(phi)
+    Z, pZ = _d(Z)
+    n = R.shape[0]
+    out = np.empty((n, 18))
+    psi = np.empty(n)
+    lib().orc_eval_analytic(C.byref(an), n, pR, pP, pZ, float(t), out.ctypes.data_as(c_dp), psi.ctypes.data_as(c_dp))
+    return out, psi
+
+
+def _state(m):
+    keys = ("x", "y", "z", "vx", "vy", "vz", "mu", "w")
+    arrs = [np.array(m[k], dtype=np.float64, copy=True, order="C") for k in keys]
+    return dict(zip(keys, arrs)), [a.ctypes.data_as(c_dp) for a in arrs]
+
+
+def push_fe(mesh: Mesh, sp: Species, markers: dict, nsteps: int, dt: float, t0: float = 0.0, step0: int = 0,
+            brute: bool = False, nthreads: int = 0, elem: Optional[np.ndarray] = None):
+    """Returns (new marker dict, elem, n_lost).  Input arrays are not modified."""
+    st, ptrs = _state(markers)
+    n = st["x"].shape[0]
+    e = np.full(n, -2, dtype=np.int32) if elem is None else np.array(elem, dtype=np.int32, copy=True)
+    lost = lib().orc_push_fe(mesh.h, C.byref(sp), n, *ptrs, e.ctypes.data_as(c_ip), int(nsteps), float(dt), float(t0),
+                             int(step0), int(brute), int(nthreads))
+    return st, e, int(lost)
+
+
+def push_analytic(an: Analytic, sp: Species, markers: dict, nsteps: int, dt: float, t0: float = 0.0, step0: int = 0,
+                  nthreads: int = 0):
+    st, ptrs = _state(markers)
+    n = st["x"].shape[0]
+    lib().orc_push_analytic(C.byref(an), C.byref(sp), n, *ptrs, int(nsteps), float(dt), float(t0), int(step0), int(nthreads))
+    return st
+
+
+def trace(sp: Species, state8, nsteps: int, dt: float, *, mesh: Optional[Mesh] = None, an: Optional[Analytic] = None,
+          t0: float = 0.0, stride: int = 1):
+    """Trajectory of one marker: rows (x_l[3], v_l[3], w_{l+1/2}, t_l) every ``stride`` steps."""
+    s = np.array(state8, dtype=np.float64, copy=True)
+    nout = (nsteps + stride - 1) // stride
+    out = np.empty((nout, 8))
+    k = lib().orc_trace(mesh.h if mesh is not None else None, C.byref(an) if an is not None else None, C.byref(sp),
+                        s.ctypes.data_as(c_dp), int(nsteps), float(dt), float(t0), int(stride), out.ctypes.data_as(c_dp))
+    return out[:k], s
+
+
+def push_uniform(x, v, B, E, charge, mass, nsteps, dt):
+    xs = [np.array(x[..., k], dtype=np.float64, copy=True, order="C").ravel() for k in range(3)]
+    vs = [np.array(v[..., k], dtype=np.float64, copy=True, order="C").ravel() for k in range(3)]
+    B, pB = _d(B)
+    E, pE = _d(E)
+    lib().orc_push_uniform(xs[0].shape[0], *[a.ctypes.data_as(c_dp) for a in xs + vs], pB, pE, float(charge), float(mass),
+                           int(nsteps), float(dt))
+    return np.stack(xs, -1), np.stack(vs, -1)
+
+
+def eq6(vm, E, B, h):
+    vm, p1 = _d(vm)
+    E, p2 = _d(E)
+    B, p3 = _d(B)
+    out = np.empty(3)
+    lib().orc_eq6(p1, p2, p3, float(h), out.ctypes.data_as(c_dp))
+    return out
+
+
+def weight_rhs(fields18, sp: Species, R, vl_cyl, mu):
+    f, p1 = _d(fields18)
+    v, p2 = _d(vl_cyl)
+    return float(lib().orc_weight_rhs(p1, C.byref(sp), float(R), p2, float(mu)))
+
+
+def sort_perm(elem, n_elems):
+    e, pe = _i(elem)
+    perm = np.empty(e.shape[0], dtype=np.int64)
+    lib().orc_sort_perm(e.shape[0], pe, int(n_elems), perm.ctypes.data_as(c_lp))
+    return perm
+
+
+def max_threads() -> int:
+    return int(lib().orc_max_threads())

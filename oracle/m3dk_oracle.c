@@ -1,0 +1,597 @@
+/*
+ * m3dk_oracle.c -- CPU fp64 ORACLE for the M3D-C1-K energetic-particle push.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call this file.  It shares no code with the CUDA path
+ * (paper_2107_13663_b200/csrc) and neither includes the other.  Compile: gcc -O2 -ffp-contract=off -fopenmp.
+ *
+ * What it is: the method of PAPER.md sections 2-3 written out step by step, one marker at a time,
+ * scalar loops, in the paper's order and notation (the method is a time integrator, so the oracle is
+ * the algorithm itself):
+ *
+ *   per marker, per step l, state (x_l, v_{l-1/2}, mu, w_{l-1/2}), time t_l = t0 + l*dt
+ *    1. (R, phi, Z) from Cartesian x                          [tokamak geometry; reading G3]
+ *    2. element containing (R, Z)                              [whole mesh visible; reading G11]
+ *    3. fields = per-element polynomials, first derivatives    [PAPER.md:86; readings G4, G10]
+ *       |B| is its own scalar field, grad|B| from its first derivatives [PAPER.md:86]
+ *    4. perturbed fields Re[C(R,Z) exp(i(n phi - omega t))]    [PAPER.md:130; reading G8]
+ *    5. E-dagger = E - (mu/q) grad|B|  (linear mode: E = 0, B = B0)    [PAPER.md:78, :108; reading G2]
+ *    6. Eq. (6) solved for v_{l+1/2} as a 3x3 linear system    [PAPER.md:75-78]
+ *    7. v_l = (v_{l-1/2}+v_{l+1/2})/2, weight RHS Eqs. (8)-(13) with (1-w) -> 1   [PAPER.md:106-130, :140; G5-G7, G9]
+ *    8. Eq. (5): x_{l+1} = x_l + dt v_{l+1/2}                  [PAPER.md:73]
+ *   mu is never modified [PAPER.md:114].
+ *
+ * Deliberately different routes from the CUDA path where the mathematics allows (so that agreement means
+ * something): naive monomial sums instead of Horner, libm atan2/cos/sin instead of complex powers,
+ * Gaussian elimination of the 3x3 system instead of the Boris t/s vectors, brute-force / full-list element
+ * search instead of the prioritised bucket search.
+ *
+ * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1-P15 of SURVEY.md 8(c); see DESIGN.md section 3.
+ * Unpinned by the paper (fixed by DESIGN.md readings, parity unpinned): the kappa_E model (G7),
+ * the construction of the synthetic perturbations (G19), rho* (G17).
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define NCOEF 21
+#define DEG 5
+#define N_EQ 4
+#define N_PERT 7
+
+/* ------------------------------------------------------------------------------------------------ */
+/* field values at one point, cylindrical components (R, phi, Z)                                      */
+typedef struct {
+    double psi_R, psi_Z;   /* d psi0/dR, d psi0/dZ                    */
+    double Bm, Bm_R, Bm_Z; /* |B|0 (its own scalar field) and gradient */
+    double F;              /* R B_phi0                                 */
+    double kappa;          /* d ln f0 / d psi                          */
+    double E1[3], B1[3];   /* perturbed E, B                           */
+    double gB1p[3];        /* grad B1par (phi component = (1/R) d/dphi) */
+    double dtB1p;          /* d B1par / dt                             */
+    double B1p;            /* B1par itself (diagnostic)                */
+} orc_fields;
+
+typedef struct {
+    int n_nodes, n_elems, n_modes;
+    const double *node_RZ; /* [n_nodes][2]                    */
+    const int *tri;        /* [n_elems][3] CCW                */
+    const double *eq_coef; /* [n_elems][4][21]                */
+    const double *pert_coef; /* [n_modes][n_elems][7][2][21]  */
+    const int *n_tor;
+    const double *omega;
+    /* background grid for the assisted search (own construction, bbox lists, ascending ids) */
+    int gx, gz;
+    double Rmin, Rmax, Zmin, Zmax, hx, hz;
+    int *start; /* [gx*gz+1] */
+    int *cand;
+} orc_mesh;
+
+/* analytic large-aspect-ratio circular tokamak (reading G18) + optional electrostatic harmonic */
+typedef struct {
+    double R0, a, B0;
+    int qkind;          /* 0: q = qc0 + qc1 u ; 1: q = qc0 + qc1 (u-qc2)^2 ; u=(r/a)^2, frozen for u>1 */
+    double qc[3];
+    double kappa;       /* constant d ln f0 / d psi used by the analytic back-end */
+    /* electrostatic perturbation Phi = A exp(-((r-rc)/wd)^2) cos(n phi - m theta - omega t); A = 0: none */
+    double pA, prc, pwd, pomega;
+    int pn, pm;
+} orc_analytic;
+
+typedef struct {
+    double charge, mass;
+    int f0kind;        /* 0 Maxwellian, 1 slowing-down, 2 beam pitch (reading G7) */
+    double f0par[5];   /* T, v_c, Lambda0, dLambda, B_axis */
+} orc_species;
+
+/* ------------------------------------------------------------------------------------------------ */
+/* 2. element search (reading G11): smallest element index whose three edge functions
+ *    (x_b-x_a)(Z-z_a) - (z_b-z_a)(R-r_a), evaluated in exactly this order without FMA, are all >= 0.     */
+static int tri_contains(const orc_mesh *m, int e, double R, double Z)
+{
+    const int *t = m->tri + 3 * e;
+    for (int k = 0; k < 3; ++k) {
+        const double *pa = m->node_RZ + 2 * t[k];
+        const double *pb = m->node_RZ + 2 * t[(k + 1) % 3];
+        double ra = pa[0], za = pa[1], rb = pb[0], zb = pb[1];
+        double ef = (rb - ra) * (Z - za) - (zb - za) * (R - ra);
+        if (!(ef >= 0.0)) return 0;
+    }
+    return 1;
+}
+
+static int locate_brute(const orc_mesh *m, double R, double Z)
+{
+    for (int e = 0; e < m->n_elems; ++e)
+        if (tri_contains(m, e, R, Z)) return e;
+    return -1;
+}
+
+static int locate_grid(const orc_mesh *m, double R, double Z)
+{
+    if (!(R >= m->Rmin && R <= m->Rmax && Z >= m->Zmin && Z <= m->Zmax)) return -1;
+    int ix = (int)floor((R - m->Rmin) / m->hx);
+    int iz = (int)floor((Z - m->Zmin) / m->hz);
+    if (ix < 0) ix = 0;
+    if (ix >= m->gx) ix = m->gx - 1;
+    if (iz < 0) iz = 0;
+    if (iz >= m->gz) iz = m->gz - 1;
+    int b = iz * m->gx + ix;
+    for (int k = m->start[b]; k < m->start[b + 1]; ++k) /* ascending ids: first hit = smallest index */
+        if (tri_contains(m, m->cand[k], R, Z)) return m->cand[k];
+    return -1;
+}
+
+static void build_grid(orc_mesh *m)
+{
+    double Rmin = 1e300, Rmax = -1e300, Zmin = 1e300, Zmax = -1e300;
+    for (int i = 0; i < m->n_nodes; ++i) {
+        double r = m->node_RZ[2 * i], z = m->node_RZ[2 * i + 1];
+        if (r < Rmin) Rmin = r;
+        if (r > Rmax) Rmax = r;
+        if (z < Zmin) Zmin = z;
+        if (z > Zmax) Zmax = z;
+    }
+    int g = (int)floor(sqrt(0.5 * (double)m->n_elems));
+    if (g < 1) g = 1;
+    m->gx = m->gz = g;
+    m->Rmin = Rmin; m->Rmax = Rmax; m->Zmin = Zmin; m->Zmax = Zmax;
+    m->hx = (Rmax - Rmin) / g;
+    m->hz = (Zmax - Zmin) / g;
+    const double infl = 1e-6; /* buckets, inflated: conservative against rounding of the bucket index */
+    int nb = g * g;
+    m->start = (int *)calloc((size_t)nb + 1, sizeof(int));
+    for (int pass = 0; pass < 2; ++pass) {
+        int *fill = NULL;
+        if (pass == 1) {
+            int acc = 0;
+            for (int b = 0; b < nb; ++b) { int c = m->start[b]; m->start[b] = acc; acc += c; }
+            m->start[nb] = acc;
+            m->cand = (int *)malloc(sizeof(int) * (size_t)(acc > 0 ? acc : 1));
+            fill = (int *)malloc(sizeof(int) * (size_t)nb);
+            memcpy(fill, m->start, sizeof(int) * (size_t)nb);
+        }
+        for (int e = 0; e < m->n_elems; ++e) {
+            const int *t = m->tri + 3 * e;
+            double r0 = 1e300, r1 = -1e300, z0 = 1e300, z1 = -1e300;
+            for (int k = 0; k < 3; ++k) {
+                double r = m->node_RZ[2 * t[k]], z = m->node_RZ[2 * t[k] + 1];
+                if (r < r0) r0 = r;
+                if (r > r1) r1 = r;
+                if (z < z0) z0 = z;
+                if (z > z1) z1 = z;
+            }
+            int ix0 = (int)floor((r0 - Rmin) / m->hx - infl), ix1 = (int)floor((r1 - Rmin) / m->hx + infl);
+            int iz0 = (int)floor((z0 - Zmin) / m->hz - infl), iz1 = (int)floor((z1 - Zmin) / m->hz + infl);
+            if (ix0 < 0) ix0 = 0;
+            if (iz0 < 0) iz0 = 0;
+            if (ix1 >= g) ix1 = g - 1;
+            if (iz1 >= g) iz1 = g - 1;
+            for (int iz = iz0; iz <= iz1; ++iz)
+                for (int ix = ix0; ix <= ix1; ++ix) {
+                    int b = iz * g + ix;
+                    if (pass == 0) m->start[b]++;
+                    else m->cand[fill[b]++] = e;
+                }
+        }
+        if (fill) free(fill);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------ */
+/* 3. naive polynomial evaluation (reading G10): sum_k c_k xi^i eta^j, k <-> (i,j), j outer, i inner     */
+static void poly_eval(const double *c, double xi, double eta, double *val, double *dxi, double *deta)
+{
+    double xp[DEG + 1], ep[DEG + 1];
+    xp[0] = 1.0; ep[0] = 1.0;
+    for (int p = 1; p <= DEG; ++p) { xp[p] = xp[p - 1] * xi; ep[p] = ep[p - 1] * eta; }
+    double v = 0.0, dx = 0.0, de = 0.0;
+    int k = 0;
+    for (int j = 0; j <= DEG; ++j)
+        for (int i = 0; i <= DEG - j; ++i, ++k) {
+            v += c[k] * (xp[i] * ep[j]);
+            if (i > 0) dx += c[k] * ((double)i * (xp[i - 1] * ep[j]));
+            if (j > 0) de += c[k] * ((double)j * (xp[i] * ep[j - 1]));
+        }
+    *val = v; *dxi = dx; *deta = de;
+}
+
+static void elem_frame(const orc_mesh *m, int e, double *Rc, double *Zc, double *s)
+{
+    const int *t = m->tri + 3 * e;
+    const double *a = m->node_RZ + 2 * t[0], *b = m->node_RZ + 2 * t[1], *c = m->node_RZ + 2 * t[2];
+    *Rc = (a[0] + b[0] + c[0]) / 3.0;
+    *Zc = (a[1] + b[1] + c[1]) / 3.0;
+    double l0 = sqrt((b[0] - a[0]) * (b[0] - a[0]) + (b[1] - a[1]) * (b[1] - a[1]));
+    double l1 = sqrt((c[0] - b[0]) * (c[0] - b[0]) + (c[1] - b[1]) * (c[1] - b[1]));
+    double l2 = sqrt((a[0] - c[0]) * (a[0] - c[0]) + (a[1] - c[1]) * (a[1] - c[1]));
+    double L = l0 > l1 ? l0 : l1;
+    if (l2 > L) L = l2;
+    *s = 1.0 / L;
+}
+
+/* steps 3-4 on the finite-element tables */
+static void fe_fields(const orc_mesh *m, int e, double R, double phi, double Z, double t, orc_fields *f)
+{
+    double Rc, Zc, s;
+    elem_frame(m, e, &Rc, &Zc, &s);
+    double xi = (R - Rc) * s, eta = (Z - Zc) * s;
+    const double *ce = m->eq_coef + (size_t)e * N_EQ * NCOEF;
+    double v, dx, de;
+    poly_eval(ce + 0 * NCOEF, xi, eta, &v, &dx, &de);
+    f->psi_R = dx * s; f->psi_Z = de * s;
+    poly_eval(ce + 1 * NCOEF, xi, eta, &v, &dx, &de);
+    f->Bm = v; f->Bm_R = dx * s; f->Bm_Z = de * s;
+    poly_eval(ce + 2 * NCOEF, xi, eta, &v, &dx, &de);
+    f->F = v;
+    poly_eval(ce + 3 * NCOEF, xi, eta, &v, &dx, &de);
+    f->kappa = v;
+    for (int k = 0; k < 3; ++k) { f->E1[k] = 0.0; f->B1[k] = 0.0; f->gB1p[k] = 0.0; }
+    f->dtB1p = 0.0; f->B1p = 0.0;
+    for (int md = 0; md < m->n_modes; ++md) {
+        const double *cp = m->pert_coef + ((size_t)md * m->n_elems + e) * (N_PERT * 2 * NCOEF);
+        double n = (double)m->n_tor[md], om = m->omega[md];
+        double th = n * phi - om * t;
+        double cth = cos(th), sth = sin(th);
+        double re[N_PERT], im[N_PERT], reR = 0, imR = 0, reZ = 0, imZ = 0;
+        for (int q = 0; q < N_PERT; ++q) {
+            double a, b, c2, d;
+            poly_eval(cp + (2 * q + 0) * NCOEF, xi, eta, &re[q], &a, &b);
+            poly_eval(cp + (2 * q + 1) * NCOEF, xi, eta, &im[q], &c2, &d);
+            if (q == 6) { reR = a * s; reZ = b * s; imR = c2 * s; imZ = d * s; }
+        }
+        /* Re[C e^{i th}] = Cr cos - Ci sin ; d/dphi -> Re[i n C e^{i th}] = -n (Cr sin + Ci cos) ;
+           d/dt -> Re[-i om C e^{i th}] = om (Cr sin + Ci cos)                                       */
+        for (int k = 0; k < 3; ++k) {
+            f->E1[k] += re[k] * cth - im[k] * sth;
+            f->B1[k] += re[3 + k] * cth - im[3 + k] * sth;
+        }
+        double qd = re[6] * sth + im[6] * cth;
+        f->B1p += re[6] * cth - im[6] * sth;
+        f->gB1p[0] += reR * cth - imR * sth;
+        f->gB1p[1] += -n * qd / R;
+        f->gB1p[2] += reZ * cth - imZ * sth;
+        f->dtB1p += om * qd;
+    }
+}
+
+/* analytic back-end: the same quantities from closed forms */
+static double an_q(const orc_analytic *a, double u, double *dqdu)
+{
+    if (u > 1.0) { u = 1.0; if (dqdu) *dqdu = 0.0; dqdu = NULL; }
+    if (a->qkind == 0) { if (dqdu) *dqdu = a->qc[1]; return a->qc[0] + a->qc[1] * u; }
+    if (dqdu) *dqdu = 2.0 * a->qc[1] * (u - a->qc[2]);
+    return a->qc[0] + a->qc[1] * (u - a->qc[2]) * (u - a->qc[2]);
+}
+
+static double an_psi(const orc_analytic *a, double r)
+{
+    double u = (r / a->a) * (r / a->a), ui = u > 1.0 ? 1.0 : u, p;
+    if (a->qkind == 0) p = a->B0 * a->a * a->a / (2.0 * a->qc[1]) * log1p(a->qc[1] * ui / a->qc[0]);
+    else {
+        double s = sqrt(a->qc[1] / a->qc[0]);
+        p = a->B0 * a->a * a->a / (2.0 * sqrt(a->qc[0] * a->qc[1])) * (atan(s * (ui - a->qc[2])) + atan(s * a->qc[2]));
+    }
+    if (u > 1.0) p += a->B0 * (r * r - a->a * a->a) / (2.0 * an_q(a, 1.0, NULL));
+    return p;
+}
+
+static void an_fields(const orc_analytic *a, double R, double phi, double Z, double t, orc_fields *f)
+{
+    double dR = R - a->R0, r2 = dR * dR + Z * Z, u = r2 / (a->a * a->a);
+    double dqdu, q = an_q(a, u, &dqdu);
+    double g = a->B0 / q;                                  /* (dpsi/dr)/r                    */
+    double gp_over_r = -a->B0 / (q * q) * dqdu * 2.0 / (a->a * a->a); /* (dg/dr)/r          */
+    double F = a->B0 * a->R0;
+    f->psi_R = g * dR; f->psi_Z = g * Z; f->F = F; f->kappa = a->kappa;
+    double S = g * g * r2 + F * F, sq = sqrt(S);           /* |B| = sqrt(S)/R                */
+    double Sr_over_r = 2.0 * g * gp_over_r * r2 + 2.0 * g * g;
+    f->Bm = sq / R;
+    f->Bm_R = Sr_over_r * dR / (2.0 * sq * R) - sq / (R * R);
+    f->Bm_Z = Sr_over_r * Z / (2.0 * sq * R);
+    for (int k = 0; k < 3; ++k) { f->E1[k] = 0.0; f->B1[k] = 0.0; f->gB1p[k] = 0.0; }
+    f->dtB1p = 0.0; f->B1p = 0.0;
+    if (a->pA != 0.0) {
+        double r = sqrt(r2), th = atan2(Z, dR);
+        double arg = (r - a->prc) / a->pwd, G = a->pA * exp(-arg * arg), dG = -2.0 * arg / a->pwd * G;
+        double ang = a->pn * phi - a->pm * th - a->pomega * t, ca = cos(ang), sa = sin(ang);
+        double ct = dR / r, st = Z / r;
+        /* Phi = G cos(ang); dang/dR = +m sin(th)/r, dang/dZ = -m cos(th)/r ; E = -grad Phi */
+        double PhiR = dG * ct * ca - G * sa * (a->pm * st / r);
+        double PhiZ = dG * st * ca - G * sa * (-a->pm * ct / r);
+        f->E1[0] = -PhiR;
+        f->E1[1] = (double)a->pn * G * sa / R;
+        f->E1[2] = -PhiZ;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------ */
+/* 6. Eq. (6): (m/q)(v+ - v-)/dt = E + (v+ + v-)/2 x B.  With h = q dt/(2m) and (v x B) = M v,
+ *    (I - h M) v+ = (I + h M) v- + 2 h E : solved by Gaussian elimination with partial pivoting.          */
+static void eq6_solve(const double vm[3], const double E[3], const double B[3], double h, double vp[3])
+{
+    double M[3][3] = {{0.0, B[2], -B[1]}, {-B[2], 0.0, B[0]}, {B[1], -B[0], 0.0}};
+    double A[3][4];
+    for (int i = 0; i < 3; ++i) {
+        double Mv = M[i][0] * vm[0] + M[i][1] * vm[1] + M[i][2] * vm[2];
+        for (int j = 0; j < 3; ++j) A[i][j] = (i == j ? 1.0 : 0.0) - h * M[i][j];
+        A[i][3] = vm[i] + h * Mv + 2.0 * h * E[i];
+    }
+    for (int c = 0; c < 3; ++c) {
+        int p = c;
+        for (int i = c + 1; i < 3; ++i)
+            if (fabs(A[i][c]) > fabs(A[p][c])) p = i;
+        if (p != c)
+            for (int j = 0; j < 4; ++j) { double tmp = A[c][j]; A[c][j] = A[p][j]; A[p][j] = tmp; }
+        for (int i = c + 1; i < 3; ++i) {
+            double l = A[i][c] / A[c][c];
+            for (int j = c; j < 4; ++j) A[i][j] -= l * A[c][j];
+        }
+    }
+    for (int i = 2; i >= 0; --i) {
+        double sacc = A[i][3];
+        for (int j = i + 1; j < 3; ++j) sacc -= A[i][j] * vp[j];
+        vp[i] = sacc / A[i][i];
+    }
+}
+
+/* 7. weight RHS, Eqs. (8)-(13) in linear form (readings G5, G6, G7); all vectors cylindrical        */
+static double weight_rhs(const orc_fields *f, const orc_species *sp, double R, const double vl[3], double mu)
+{
+    double q = sp->charge, m = sp->mass;
+    double B0[3] = {-f->psi_Z / R, f->F / R, f->psi_R / R};            /* reading G4 */
+    double B0n = sqrt(B0[0] * B0[0] + B0[1] * B0[1] + B0[2] * B0[2]);
+    double b0[3] = {B0[0] / B0n, B0[1] / B0n, B0[2] / B0n};
+    double vpar = vl[0] * b0[0] + vl[1] * b0[1] + vl[2] * b0[2];
+    const double *E1 = f->E1, *B1 = f->B1;
+    /* Eq. (12): (dX/dt)_1 = E1 x B0 / B0^2 + vpar B1 / B0 */
+    double ExB[3] = {E1[1] * B0[2] - E1[2] * B0[1], E1[2] * B0[0] - E1[0] * B0[2], E1[0] * B0[1] - E1[1] * B0[0]};
+    double dX[3];
+    for (int k = 0; k < 3; ++k) dX[k] = ExB[k] / (B0n * B0n) + vpar * B1[k] / B0n;
+    /* Eq. (13) (G5): m (dvpar/dt)_1 = q E1.b0 - mu b0.grad B1par */
+    double Fpar = q * (E1[0] * b0[0] + E1[1] * b0[1] + E1[2] * b0[2])
+                - mu * (b0[0] * f->gB1p[0] + b0[1] * f->gB1p[1] + b0[2] * f->gB1p[2]);
+    /* Eq. (10) (G5): dPphi/dt = q (dX/dt)_1 . grad psi0 + m (dvpar/dt)_1 R Bphi0 / B0 */
+    double dPphi = q * (dX[0] * f->psi_R + dX[2] * f->psi_Z) + Fpar * f->F / B0n;
+    /* Eq. (11) (G6): dE/dt = q v_l . E1 + mu dB1par/dt */
+    double dE = q * (vl[0] * E1[0] + vl[1] * E1[1] + vl[2] * E1[2]) + mu * f->dtB1p;
+    /* d ln f0 / dE at fixed (Pphi, mu) (G7) */
+    double v2 = vl[0] * vl[0] + vl[1] * vl[1] + vl[2] * vl[2];
+    double Ekin = 0.5 * m * v2 + mu * f->Bm;
+    double kE;
+    if (sp->f0kind == 0) kE = -1.0 / sp->f0par[0];
+    else {
+        double v = sqrt(2.0 * Ekin / m), vc = sp->f0par[1];
+        kE = -3.0 * v / (m * (v * v * v + vc * vc * vc));
+        if (sp->f0kind == 2) {
+            double Lam = mu * sp->f0par[4] / Ekin, L0 = sp->f0par[2], dL = sp->f0par[3];
+            kE += 2.0 * (Lam - L0) * Lam / (dL * dL * Ekin);
+        }
+    }
+    /* Eqs. (8)-(9), (1-w) -> 1:  dw/dt = -[ (kappa/q) dPphi/dt + kE dE/dt ] */
+    return -((f->kappa / q) * dPphi + kE * dE);
+}
+
+typedef struct {
+    int kind;               /* 0: FE tables, 1: analytic */
+    const orc_mesh *mesh;
+    const orc_analytic *an;
+    int brute;
+} provider;
+
+/* one full step of one marker.  s = {x,y,z,vx,vy,vz,mu,w}.  Returns element (FE), 0 (analytic) or -1 = lost
+ * (reading G12: a lost marker is frozen).  vl_out (optional) receives the Cartesian v_l.                  */
+static int step_marker(const provider *pv, const orc_species *sp, double *s, double t, double dt, double *vl_out)
+{
+    double x = s[0], y = s[1], z = s[2];
+    /* 1 */
+    double R = sqrt(x * x + y * y), phi = atan2(y, x), Z = z;
+    double c = x / R, sn = y / R;
+    orc_fields f;
+    int e = 0;
+    if (pv->kind == 0) {
+        /* 2 */
+        e = pv->brute ? locate_brute(pv->mesh, R, Z) : locate_grid(pv->mesh, R, Z);
+        if (e < 0) return -1;
+        /* 3, 4 */
+        fe_fields(pv->mesh, e, R, phi, Z, t, &f);
+    } else {
+        an_fields(pv->an, R, phi, Z, t, &f);
+    }
+    /* 5: linear mode, trajectory in the equilibrium field only */
+    double mu = s[6], q = sp->charge, m = sp->mass;
+    double BR = -f.psi_Z / R, BP = f.F / R, BZ = f.psi_R / R;
+    double ER = -(mu / q) * f.Bm_R, EZ = -(mu / q) * f.Bm_Z;
+    double B[3] = {BR * c - BP * sn, BR * sn + BP * c, BZ};
+    double E[3] = {ER * c, ER * sn, EZ};
+    /* 6 */
+    double vm[3] = {s[3], s[4], s[5]}, vp[3];
+    double h = q * dt / (2.0 * m);
+    eq6_solve(vm, E, B, h, vp);
+    /* 7 */
+    double vl[3] = {0.5 * (vm[0] + vp[0]), 0.5 * (vm[1] + vp[1]), 0.5 * (vm[2] + vp[2])};
+    double vlc[3] = {vl[0] * c + vl[1] * sn, -vl[0] * sn + vl[1] * c, vl[2]};
+    double wdot = weight_rhs(&f, sp, R, vlc, mu);
+    s[7] = s[7] + dt * wdot;
+    /* 8 */
+    s[0] = x + dt * vp[0]; s[1] = y + dt * vp[1]; s[2] = z + dt * vp[2];
+    s[3] = vp[0]; s[4] = vp[1]; s[5] = vp[2];
+    if (vl_out) { vl_out[0] = vl[0]; vl_out[1] = vl[1]; vl_out[2] = vl[2]; }
+    return e;
+}
+
+/* ================================================================================================ */
+/* exported entry points (ctypes)                                                                    */
+
+orc_mesh *orc_mesh_create(int n_nodes, const double *node_RZ, int n_elems, const int *tri, const double *eq_coef,
+                          int n_modes, const int *n_tor, const double *omega, const double *pert_coef)
+{
+    orc_mesh *m = (orc_mesh *)calloc(1, sizeof(orc_mesh));
+    m->n_nodes = n_nodes; m->node_RZ = node_RZ; m->n_elems = n_elems; m->tri = tri; m->eq_coef = eq_coef;
+    m->n_modes = n_modes; m->n_tor = n_tor; m->omega = omega; m->pert_coef = pert_coef;
+    build_grid(m);
+    return m;
+}
+
+void orc_mesh_free(orc_mesh *m)
+{
+    if (!m) return;
+    free(m->start); free(m->cand); free(m);
+}
+
+void orc_locate(const orc_mesh *m, long n, const double *R, const double *Z, int *elem, int brute)
+{
+#pragma omp parallel for schedule(dynamic, 256)
+    for (long i = 0; i < n; ++i) elem[i] = brute ? locate_brute(m, R[i], Z[i]) : locate_grid(m, R[i], Z[i]);
+}
+
+/* out[i][0..17] = psi_R psi_Z Bm Bm_R Bm_Z F kappa E1(3) B1(3) gB1p(3) dtB1p B1p ; elem[i] = -1: row untouched */
+void orc_eval_fe(const orc_mesh *m, long n, const double *R, const double *phi, const double *Z, double t,
+                 int *elem, double *out)
+{
+    for (long i = 0; i < n; ++i) {
+        int e = locate_grid(m, R[i], Z[i]);
+        elem[i] = e;
+        if (e < 0) continue;
+        orc_fields f;
+        fe_fields(m, e, R[i], phi[i], Z[i], t, &f);
+        double *o = out + 18 * i;
+        o[0] = f.psi_R; o[1] = f.psi_Z; o[2] = f.Bm; o[3] = f.Bm_R; o[4] = f.Bm_Z; o[5] = f.F; o[6] = f.kappa;
+        for (int k = 0; k < 3; ++k) { o[7 + k] = f.E1[k]; o[10 + k] = f.B1[k]; o[13 + k] = f.gB1p[k]; }
+        o[16] = f.dtB1p; o[17] = f.B1p;
+    }
+}
+
+void orc_eval_analytic(const orc_analytic *a, long n, const double *R, const double *phi, const double *Z, double t,
+                       double *out, double *psi)
+{
+    for (long i = 0; i < n; ++i) {
+        orc_fields f;
+        an_fields(a, R[i], phi[i], Z[i], t, &f);
+        double *o = out + 18 * i;
+        o[0] = f.psi_R; o[1] = f.psi_Z; o[2] = f.Bm; o[3] = f.Bm_R; o[4] = f.Bm_Z; o[5] = f.F; o[6] = f.kappa;
+        for (int k = 0; k < 3; ++k) { o[7 + k] = f.E1[k]; o[10 + k] = f.B1[k]; o[13 + k] = f.gB1p[k]; }
+        o[16] = f.dtB1p; o[17] = f.B1p;
+        double dR = R[i] - a->R0;
+        if (psi) psi[i] = an_psi(a, sqrt(dR * dR + Z[i] * Z[i]));
+    }
+}
+
+static void set_threads(int nthreads)
+{
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+}
+
+int orc_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* push n markers nsteps steps; step counter starts at step0 (t_l = t0 + (step0+l) dt).
+ * elem (optional, in/out): -1 on input = lost in an earlier call (stays frozen; pass -2 for "unknown");
+ * on return the element of the last evaluated position x_l of the final step, or -1 if lost.
+ * Returns the number of lost markers.                                                                  */
+static long push_generic(const provider *pv, const orc_species *sp, long n, double *x, double *y, double *z,
+                         double *vx, double *vy, double *vz, const double *mu, double *w, int *elem,
+                         int nsteps, double dt, double t0, long step0, int nthreads)
+{
+    long lost = 0;
+    set_threads(nthreads);
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : lost)
+    for (long i = 0; i < n; ++i) {
+        double s[8] = {x[i], y[i], z[i], vx[i], vy[i], vz[i], mu[i], w[i]};
+        int e = 0, dead = (elem && elem[i] == -1) ? 1 : 0; /* -1 on input: lost earlier, stays frozen */
+        for (int l = 0; l < nsteps && !dead; ++l) {
+            double t = t0 + (double)(step0 + l) * dt;
+            e = step_marker(pv, sp, s, t, dt, NULL);
+            if (e < 0) dead = 1;
+        }
+        if (dead) { lost++; e = -1; }
+        x[i] = s[0]; y[i] = s[1]; z[i] = s[2]; vx[i] = s[3]; vy[i] = s[4]; vz[i] = s[5]; w[i] = s[7];
+        if (elem) elem[i] = e;
+    }
+    return lost;
+}
+
+long orc_push_fe(const orc_mesh *m, const orc_species *sp, long n, double *x, double *y, double *z, double *vx,
+                 double *vy, double *vz, const double *mu, double *w, int *elem, int nsteps, double dt, double t0,
+                 long step0, int brute, int nthreads)
+{
+    provider pv = {0, m, NULL, brute};
+    return push_generic(&pv, sp, n, x, y, z, vx, vy, vz, mu, w, elem, nsteps, dt, t0, step0, nthreads);
+}
+
+long orc_push_analytic(const orc_analytic *a, const orc_species *sp, long n, double *x, double *y, double *z,
+                       double *vx, double *vy, double *vz, const double *mu, double *w, int nsteps, double dt,
+                       double t0, long step0, int nthreads)
+{
+    provider pv = {1, NULL, a, 0};
+    return push_generic(&pv, sp, n, x, y, z, vx, vy, vz, mu, w, NULL, nsteps, dt, t0, step0, nthreads);
+}
+
+/* trajectory of ONE marker: every `stride` steps store (x_l, v_l, w_{l+1/2}, t_l) -> out[k][8].
+ * s[8] is updated in place.  mesh == NULL: analytic back-end.  Returns samples written.                  */
+long orc_trace(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, double *s, long nsteps, double dt,
+               double t0, long stride, double *out)
+{
+    provider pv = {m ? 0 : 1, m, a, 0};
+    long k = 0;
+    for (long l = 0; l < nsteps; ++l) {
+        double t = t0 + (double)l * dt, xl[3] = {s[0], s[1], s[2]}, vl[3];
+        int e = step_marker(&pv, sp, s, t, dt, vl);
+        if (e < 0) break;
+        if (l % stride == 0) {
+            double *o = out + 8 * k++;
+            o[0] = xl[0]; o[1] = xl[1]; o[2] = xl[2]; o[3] = vl[0]; o[4] = vl[1]; o[5] = vl[2]; o[6] = s[7]; o[7] = t;
+        }
+    }
+    return k;
+}
+
+/* Eq. (5)-(6) in uniform Cartesian fields (pins P1, P2) */
+void orc_push_uniform(long n, double *x, double *y, double *z, double *vx, double *vy, double *vz, const double *B,
+                      const double *E, double charge, double mass, long nsteps, double dt)
+{
+    double h = charge * dt / (2.0 * mass);
+    for (long i = 0; i < n; ++i)
+        for (long l = 0; l < nsteps; ++l) {
+            double vm[3] = {vx[i], vy[i], vz[i]}, vp[3];
+            eq6_solve(vm, E, B, h, vp);
+            x[i] += dt * vp[0]; y[i] += dt * vp[1]; z[i] += dt * vp[2];
+            vx[i] = vp[0]; vy[i] = vp[1]; vz[i] = vp[2];
+        }
+}
+
+void orc_eq6(const double *vm, const double *E, const double *B, double h, double *vp) { eq6_solve(vm, E, B, h, vp); }
+
+double orc_weight_rhs(const double *fields18, const orc_species *sp, double R, const double *vl_cyl, double mu)
+{
+    orc_fields f;
+    const double *o = fields18;
+    f.psi_R = o[0]; f.psi_Z = o[1]; f.Bm = o[2]; f.Bm_R = o[3]; f.Bm_Z = o[4]; f.F = o[5]; f.kappa = o[6];
+    for (int k = 0; k < 3; ++k) { f.E1[k] = o[7 + k]; f.B1[k] = o[10 + k]; f.gB1p[k] = o[13 + k]; }
+    f.dtB1p = o[16]; f.B1p = o[17];
+    return weight_rhs(&f, sp, R, vl_cyl, mu);
+}
+
+/* reference counting sort by element key (lost markers, key -1, last): returns a permutation.  Any
+ * permutation with non-decreasing keys is valid (SURVEY.md 8(c) "Sort oracle"); this one is stable.   */
+void orc_sort_perm(long n, const int *elem, int n_elems, long *perm)
+{
+    long *count = (long *)calloc((size_t)n_elems + 2, sizeof(long));
+    for (long i = 0; i < n; ++i) count[(elem[i] < 0 ? n_elems : elem[i]) + 1]++;
+    for (int k = 0; k <= n_elems; ++k) count[k + 1] += count[k];
+    for (long i = 0; i < n; ++i) perm[count[elem[i] < 0 ? n_elems : elem[i]]++] = i;
+    free(count);
+}
