@@ -1,0 +1,302 @@
+#!/usr/bin/env python
+"""bench.py -- particle-steps/s of the libm3dk hot path on synthetic tokamak workloads (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the whole hot path over all markers of the workload: field evaluation + slow-manifold Boris
+push + delta-f weight (rows a1-a10 of DESIGN.md section 1) and the marker sort by element (row a11) at the configured
+interval.  Default workload: BASELINE.json configs[3] (RSAE, 2^24 markers, 256x256 mesh), the configuration the metric
+is quoted on ("16M markers on one B200").  Markers shard across ranks with no exchange, so N GPUs
+run N shards of the same size: weak scaling, no data-path collective.
+
+Prints ONE JSON line (rank 0).  --impl reference times the CPU oracle (oracle/) on a bounded sample instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particle-steps/sec (fp64 push+field eval+delta-f weight)"
+UNIT = "particle-steps/s"
+HBM_FALLBACK_GBS = 6650.0           # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA lanes x 2 flop x clocks.max.sm
+
+
+# ---- algorithmic work per marker-step (DESIGN.md section 7 derives these) ---------------------------------------------
+def algorithmic_flops(n_modes: int) -> float:
+    """FMA = 2, add/mul = 1, div = sqrt = 1 (minimal-multiplication Horner, recounted in DESIGN.md)."""
+    eq = 78 + 78 + 40 + 40                    # psi0 (value, d/dR, d/dZ), |B|0 (same), F0, kappa
+    geom, locate, boris = 45, 30, 56
+    if n_modes == 0:
+        return eq + geom + locate + boris
+    pert = 5 * 2 * 40 + 2 * 78                # E_R E_phi E_Z B_R B_Z (re, im) values; B_par (re, im) value + gradient
+    return eq + n_modes * (pert + 60) + geom + locate + boris + 130
+
+
+def algorithmic_bytes_push(n_modes: int) -> float:
+    """HBM bytes per marker per push-kernel pass: 8 fp64 read, 7 written (mu is read-only; w only with modes),
+    element key read + written; coefficient tiles are counted as on-chip (shared by the markers of an element)."""
+    return 64 + (56 if n_modes else 48) + 4 + 4
+
+
+def algorithmic_bytes_sort() -> float:
+    """Per marker per sort: key read (histogram) + rank written/read + 72 B record read and written."""
+    return 4 + 8 + 2 * 72
+
+
+# ---- helpers -----------------------------------------------------------------------------------------------------------
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", float(d.get("sm_max_mhz", 1965.0))
+    return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)", 1965.0
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for (ts, r) in self.rows if t0 <= ts <= t1 + 0.1] or [r for (_, r) in self.rows[-3:]]
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample_rate(w, sample_stride: int, nsteps: int, nthreads: int = 0):
+    """The oracle as it stands, FE back-end, OpenMP over markers, on the id = 0 (mod stride) sub-sample."""
+    import oracle
+    idx = slice(0, None, sample_stride)
+    mk = {k: np.ascontiguousarray(v[idx]) for k, v in w.markers.items()}
+    mesh, sp = oracle.Mesh.of(w), oracle.species_of(w)
+    oracle.push_fe(mesh, sp, {k: v[:256] for k, v in mk.items()}, 1, w.dt)      # touch code and tables
+    t0 = time.perf_counter()
+    oracle.push_fe(mesh, sp, mk, nsteps, w.dt, nthreads=nthreads)
+    dt = time.perf_counter() - t0
+    n = mk["x"].shape[0]
+    return n * nsteps / dt, n, dt, oracle.max_threads() if nthreads == 0 else nthreads
+
+
+def build_workload(args, rank: int):
+    import synth
+    n = args.n_markers
+    # every rank draws its own shard (seed offset by rank): independent markers, same tables
+    w = synth.make_config(args.config, n_markers=n, nx=args.nx, dt_gyro=args.dt_gyro,
+                          seed=None if rank == 0 else 1000 + args.config + 7919 * rank)
+    return w
+
+
+def config_dict(args, w, sort_interval, world):
+    return {"workload": f"BASELINE.json configs[{args.config}] ({w.name})", "n_markers_per_gpu": w.n_markers,
+            "mesh": f"{w.nx}x{w.nx} cells, {w.n_elems} triangles", "n_modes": w.n_modes, "dt": w.dt,
+            "sort_interval": sort_interval, "parallelism": f"{world} independent marker shard(s), no collective",
+            "l2": "inputs larger than L2 (marker state %.0f MB + tables %.0f MB per GPU)" % (
+                w.n_markers * 64 / 1e6, (w.eq_coef.nbytes + w.pert_coef.nbytes) / 1e6)}
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle, as it stands, on the box's host cores, on a bounded sample of the workload."""
+    if rank != 0:
+        return
+    w = build_workload(args, 0)
+    stride = max(1, w.n_markers // args.ref_sample)
+    for _ in range(max(0, min(args.warmup, 1))):
+        oracle_sample_rate(w, stride * 8, 1)
+    rate, n, secs, cores = oracle_sample_rate(w, stride, args.steps)
+    line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(args, w, 0, world),
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{n} markers (every {stride}-th of the workload) x {args.steps} steps, {secs:.1f} s"},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    import paper_2107_13663_b200 as m3dk
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libm3dk has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    m3dk.build_all()
+    w = build_workload(args, rank)
+    si = w.sort_interval if args.sort_interval is None else args.sort_interval
+    N, K, W = w.n_markers, args.steps, args.warmup
+
+    p = m3dk.Pusher(device=local_rank, verify=False)
+    p.fields_create(w.node_RZ, w.tri, w.eq_coef, w.n_tor if w.n_modes else None, w.omega if w.n_modes else None,
+                    w.pert_coef if w.n_modes else None)
+    p.particles_init(w.markers, w.charge, w.mass, w.f0)
+    p.set_options(sort_interval=si, t0=0.0)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident leg: W warm-up steps, then exactly K timed steps ---------------------------------------
+    p.push(W, w.dt)
+    p.set_profiling(True)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    wall0 = time.time()
+    e0.record(p.stream)
+    p.push(K, w.dt)
+    e1.record(p.stream)
+    barrier()
+    wall1 = time.time()
+    ms = e0.elapsed_time(e1)
+    tm = p.timing()
+    st = p.stats()
+    clocks = sampler.stop(wall0, wall1) if sampler else None
+    p.set_profiling(False)
+
+    # ---- end-to-end leg: host buffers through the C ABI, copies inside the timed region ----------------------------
+    host = {k: torch.from_numpy(np.ascontiguousarray(w.markers[k])).pin_memory() for k in m3dk.STATE_KEYS}
+    out = {k: torch.empty(N, dtype=torch.float64).pin_memory() for k in m3dk.STATE_KEYS}
+    Ke = K
+    p.upload(host); p.set_options(sort_interval=si, t0=0.0); p.push(1, w.dt); p.download(out)      # warm the path
+    barrier()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record(p.stream)
+    p.upload(host)
+    p.set_options(sort_interval=si, t0=0.0)
+    p.push(Ke, w.dt)
+    p.download(out)
+    f1.record(p.stream)
+    barrier()
+    ms_e2e = f0.elapsed_time(f1)
+
+    t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, ms_e2e = float(t[0]), float(t[1])
+    if rank != 0:
+        return
+
+    hbm_gbs, hbm_src, _ = measured_peaks()
+    fp64_meas = p.fp64_peak_tflops()
+    flops = algorithmic_flops(w.n_modes) * N
+    bytes_push = algorithmic_bytes_push(w.n_modes) * N
+    push_ms = tm["push_ms"] / max(1, tm["push_launches"])
+    t_alu, t_hbm = flops / (FP64_NOMINAL_TFLOPS * 1e12), bytes_push / (hbm_gbs * 1e9)
+    if t_alu >= t_hbm:
+        roof = {"bound": "alu", "achieved": flops / (push_ms * 1e-3) / 1e12, "peak": FP64_NOMINAL_TFLOPS,
+                "unit": "TFLOP/s", "peak_source": "nominal fp64: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md 7)"}
+    else:
+        roof = {"bound": "hbm", "achieved": bytes_push / (push_ms * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                "peak_source": hbm_src}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof.update({"kernel": "push kernel (a1-a10)", "launch_ms": push_ms, "launches": tm["push_launches"],
+                 "share_of_step": tm["push_ms"] / ms, "traffic": None,
+                 "fp64_peak_measured_tflops": fp64_meas,
+                 "flops_per_marker_step": algorithmic_flops(w.n_modes),
+                 "hbm_bytes_per_marker_step": algorithmic_bytes_push(w.n_modes),
+                 "sort_ms_per_sort": tm["sort_ms"] / max(1, tm["sort_launches"]), "sorts": tm["sort_launches"]})
+    # whole-step roofline: the binding one of (all flops / fp64 peak) and (all HBM bytes incl. sorts / HBM bandwidth)
+    step_bytes = bytes_push + algorithmic_bytes_sort() * N * tm["sort_launches"] / K
+    t_bind = max(t_alu, step_bytes / (hbm_gbs * 1e9))
+    roof["step_frac_of_binding_roofline"] = t_bind / (ms / K * 1e-3)
+
+    line = {"metric": METRIC, "value": world * N * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+            "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": config_dict(args, w, si, world),
+            "clocks": clocks, "gpu_launches": tm["kernel_launches"],
+            "e2e": {"value": world * N * Ke / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 64 * N / Ke,
+                    "d2h_bytes_per_step": 64 * N / Ke, "note": f"one upload + {Ke} steps + one download (PAPER.md:237)"},
+            "roofline": roof, "n_lost": st["n_lost"]}
+    if world == 1 and not args.no_cpu_baseline:
+        stride = max(1, N // args.ref_sample)
+        rate, n, secs, cores = oracle_sample_rate(w, stride, args.ref_steps)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"{n} markers (every {stride}-th of the workload) x {args.ref_steps} steps, {secs:.1f} s"}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--n-markers", type=int, default=None)
+    ap.add_argument("--nx", type=int, default=None)
+    ap.add_argument("--dt-gyro", type=float, default=None)
+    ap.add_argument("--sort-interval", type=int, default=None)
+    ap.add_argument("--ref-sample", type=int, default=65536, help="markers in the oracle's bounded sample")
+    ap.add_argument("--ref-steps", type=int, default=100)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=__import__("torch").device("cuda", local_rank))
+    try:
+        run_ours(args, rank, world, local_rank)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

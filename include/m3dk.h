@@ -1,0 +1,173 @@
+/*
+ * m3dk.h -- C ABI of libm3dk: the energetic-particle push of M3D-C1-K (arXiv 2107.13663) for NVIDIA B200 (sm_100a).
+ *
+ * One thing is behind this boundary: the data-parallel hot path of the paper's kinetic module.  Each marker is a
+ * classical Pauli particle advanced by the slow-manifold Boris scheme (Eqs. 5-6) with the mirror force
+ * -mu grad|B| folded into an effective electric field; each step evaluates the equilibrium and perturbed
+ * finite-element fields at the marker (per-element polynomials, first derivatives only, |B| as its own scalar field,
+ * PAPER.md:86) and advances the delta-f weight (Eqs. 8-13, linear form; v_l averaging PAPER.md:140).
+ * The fields are static while the markers are sub-cycled and the whole mesh is visible to every thread
+ * (PAPER.md:235).  The marker sort by element is not in the paper ("improving the coalesce of the GPU memory access" is
+ * listed as future work); it exists so that the threads of a warp evaluate the same element.
+ *
+ * Conventions
+ *   - Plain C, no exceptions cross the boundary.  Every call returns an m3dk_status (0 = OK, negative = error); the
+ *     text of the last error of a context is m3dk_last_error(ctx) (context-owned storage, never freed by the caller).
+ *   - HOST pointers: the mesh and coefficient tables of m3dk_fields_create, option structs, outputs of *_bytes / stats,
+ *     and the buffers of m3dk_particles_upload / _download.
+ *     DEVICE pointers: every marker array and every workspace.  The library never allocates device memory: the caller
+ *     (PyTorch in this repository) owns all of it and lends it until m3dk_destroy or the next *_create / *_init call.
+ *   - All kernels are enqueued on the stream given to m3dk_create; calls are asynchronous unless stated otherwise.
+ *     Asynchronous CUDA errors surface on the next synchronising call (m3dk_stats, m3dk_particles_download).
+ *   - One context per stream; a context is not re-entrant.
+ *   - Units: any consistent system in which m dv/dt = q (E + v x B).  Right-handed cylindrical (R, phi, Z) for the
+ *     fields, Cartesian (x, y, z) with R = sqrt(x^2 + y^2), phi = atan2(y, x), Z = z for the marker state.
+ *   - Time staggering: the caller supplies (x_l, v_{l-1/2}, w_{l-1/2}); after m3dk_push(k, dt) the arrays hold
+ *     (x_{l+k}, v_{l+k-1/2}, w_{l+k-1/2}).  mu is never modified by a push.
+ *   - There is no CPU fallback anywhere in this library.
+ */
+#ifndef M3DK_H
+#define M3DK_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define M3DK_NCOEF 21     /* monomials xi^i eta^j, i + j <= 5; storage order: j outer 0..5, i inner 0..5-j            */
+#define M3DK_N_EQ 4       /* equilibrium scalar fields per element: psi0, |B|0, F0 = R B_phi0, kappa = dlnf0/dpsi      */
+#define M3DK_N_PERT 7     /* complex perturbed amplitudes per element and mode: E_R E_phi E_Z B_R B_phi B_Z B_par      */
+#define M3DK_MAX_MODES 4  /* toroidal modes per field set                                                              */
+
+typedef struct m3dk_ctx m3dk_ctx; /* opaque; host-side bookkeeping only */
+
+typedef enum {
+    M3DK_OK = 0,
+    M3DK_EINVAL = -1,     /* bad argument (null pointer, negative size, unknown enum, non-CCW or degenerate triangle)   */
+    M3DK_ESTATE = -2,     /* call out of order (push before fields_create / particles_init, sort without workspace)   */
+    M3DK_EWORKSPACE = -3, /* workspace too small or misaligned (256-byte alignment required)                           */
+    M3DK_ECUDA = -4       /* a CUDA runtime call or an earlier kernel failed; see m3dk_last_error                      */
+} m3dk_status;
+
+typedef enum { M3DK_F0_MAXWELLIAN = 0, M3DK_F0_SLOWING_DOWN = 1, M3DK_F0_BEAM_PITCH = 2 } m3dk_f0_kind;
+
+/* Equilibrium distribution used by the weight equation, d ln f0 / dE at fixed (P_phi, mu) ("calculated
+ * from the analytical expression of f0 using the chain rule"; reading G7):
+ *   MAXWELLIAN    f0 ~ exp(-E/T)                                   -> -1/T
+ *   SLOWING_DOWN  f0 ~ 1/(v^3 + v_c^3), v = sqrt(2E/m) (Eq. 29)    -> -3 v / (m (v^3 + v_c^3))
+ *   BEAM_PITCH    slowing-down times exp(-((Lambda-Lambda0)/dLambda)^2), Lambda = mu B_axis / E
+ *                                                                  -> the above + 2 (Lambda-Lambda0) Lambda / (dLambda^2 E)
+ * with E = m |v_l|^2 / 2 + mu |B|0.  d ln f0 / d P_phi = kappa / q with kappa the 4th equilibrium table.             */
+typedef struct {
+    int kind;       /* m3dk_f0_kind */
+    double T;       /* MAXWELLIAN */
+    double v_c;     /* SLOWING_DOWN, BEAM_PITCH */
+    double Lambda0; /* BEAM_PITCH */
+    double dLambda; /* BEAM_PITCH */
+    double B_axis;  /* BEAM_PITCH */
+} m3dk_f0_params;
+
+typedef struct {
+    long n_markers;
+    long n_lost;     /* markers outside every triangle: frozen, element -1, sorted last (reading G12)                  */
+    long steps_done; /* since the last m3dk_set_options / m3dk_particles_init                                          */
+    long n_sorts;    /* sorts executed (explicit + internal)                                                           */
+    double t;        /* t0 + steps_done * dt of the last push                                                          */
+} m3dk_stats_t;
+
+int m3dk_version(void);
+
+/* Context bound to CUDA device `device` and to `stream` (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream;
+ * NULL = the legacy default stream).  Fails with M3DK_ECUDA when there is no usable CUDA device.                      */
+int m3dk_create(m3dk_ctx **out, int device, void *stream);
+int m3dk_destroy(m3dk_ctx *ctx);
+const char *m3dk_last_error(const m3dk_ctx *ctx); /* ctx may be NULL: returns the last error of m3dk_create           */
+
+/* ---- fields: poloidal triangle mesh + per-element polynomial coefficients per field + toroidal mode structure ----
+ * (PAPER.md:86, :165 "high order polynomials"; :235 whole-mesh replica on the device.)
+ *
+ * node_RZ   [n_nodes][2]  (R, Z) of the mesh nodes.
+ * tri       [n_elems][3]  node indices, counter-clockwise.
+ * eq_coef   [n_elems][M3DK_N_EQ][21]   psi0, |B|0, F0, kappa.  B0 = grad psi0 x grad phi + F0 grad phi, i.e.
+ *           B_R = -dpsi0/dZ / R, B_Z = +dpsi0/dR / R, B_phi = F0 / R (reading G4).
+ * n_tor, omega [n_modes]; pert_coef [n_modes][n_elems][M3DK_N_PERT][2][21]: (re, im) parts of the complex amplitudes C;
+ *           the physical field is Re[C(R,Z) exp(i (n_tor phi - omega t))] (readings G8, G19).
+ * Polynomials (reading G10): sum_k c_k xi^i eta^j with xi = (R - R_c) s_e, eta = (Z - Z_c) s_e, (R_c, Z_c) the centroid
+ * (sum of the three nodes / 3) and s_e = 1 / (longest edge).  d/dR = s_e d/dxi.
+ *
+ * All table pointers are HOST pointers, read during the call only.  The call repacks them into `dev_workspace`
+ * (DEVICE, 256-byte aligned, at least m3dk_fields_workspace_bytes(...) bytes), which the context then borrows:
+ * per-element coefficient tiles, per-element edge records and a bucket grid for the element search.  The call
+ * synchronises the stream before returning (the staging buffers are freed).  n_modes may be 0 (equilibrium only).    */
+int m3dk_fields_workspace_bytes(int n_nodes, int n_elems, int n_modes, size_t *bytes);
+int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node_RZ, int n_elems, const int *tri,
+                       const double *eq_coef, int n_modes, const int *n_tor, const double *omega,
+                       const double *pert_coef, void *dev_workspace, size_t workspace_bytes);
+
+/* ---- markers: SoA fp64 x, v, mu, w; species charge / mass -------------------------------------
+ * x..w: DEVICE arrays of n doubles, caller-owned, updated in place by push and permuted by sort.
+ * elem: DEVICE int[n], library-managed: the element of each marker's current position (-1 = lost).
+ * id:   DEVICE int[n]; the library fills 0..n-1 here and sorts carry it, so id[i] is the original index of slot i.
+ * The call locates every marker (one kernel).  Call it again whenever the caller has rewritten positions.            */
+int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, double *z, double *vx, double *vy, double *vz,
+                        double *mu, double *w, int *elem, int *id, double charge, double mass,
+                        const m3dk_f0_params *f0);
+
+/* sort_interval: 0 = m3dk_push never sorts; k > 0 = m3dk_push sorts before every k-th step (needs a sort workspace).
+ * mode: 0 = linear delta-f (trajectories in the equilibrium field, (1 - w) -> 1); others reserved.
+ * t0: time of the next step's x_l.  Resets steps_done to 0.                                                          */
+int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, double t0);
+
+/* Sort workspace (DEVICE, 256-byte aligned) for m3dk_sort and for the sorts inside m3dk_push; borrowed until replaced. */
+int m3dk_sort_workspace_bytes(long n_markers, int n_elems, size_t *bytes);
+int m3dk_set_sort_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes);
+
+/* nsteps slow-manifold Boris steps of size dt with field evaluation and weight update, Eqs. (5), (6), (8)-(13).
+ * Asynchronous; t advances by nsteps * dt.  A lost marker is frozen.  On return (stream order) the caller's arrays hold
+ * the new state; if sorts ran, slots are permuted and id[] says who is where.                                         */
+int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt);
+
+/* Counting sort of all marker arrays (x..w, elem, id) by element, lost markers last.  The order inside one element is
+ * unspecified.  dev_workspace may be NULL to use the workspace given to m3dk_set_sort_workspace.                      */
+int m3dk_sort(m3dk_ctx *ctx, void *dev_workspace, size_t bytes);
+
+/* Synchronises the stream, reports asynchronous errors, fills *out. */
+int m3dk_stats(m3dk_ctx *ctx, m3dk_stats_t *out);
+
+/* Host-buffer path (what a caller without device arrays uses; bench.py's e2e leg): copy the 8 state arrays between
+ * HOST buffers (pinned for full speed) and the device arrays registered by m3dk_particles_init.  upload re-locates the
+ * markers and resets id to 0..n-1.  download synchronises; host_id / host_elem may be NULL.                            */
+int m3dk_particles_upload(m3dk_ctx *ctx, const double *hx, const double *hy, const double *hz, const double *hvx,
+                          const double *hvy, const double *hvz, const double *hmu, const double *hw);
+int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, double *hz, double *hvx, double *hvy, double *hvz,
+                            double *hmu, double *hw, int *host_id, int *host_elem);
+
+/* Diagnostics for tests and the roofline: fields at arbitrary points through the same device code as the push.
+ * R, phi, Z: DEVICE [n]; elem_out: DEVICE int[n]; out: DEVICE [n][18] =
+ * psi_R psi_Z |B| |B|_R |B|_Z F kappa E1(R,phi,Z) B1(R,phi,Z) gradB1par(R,phi,Z) dB1par/dt B1par.                     */
+int m3dk_eval_fields(m3dk_ctx *ctx, long n, const double *R, const double *phi, const double *Z, double t,
+                     int *elem_out, double *out);
+
+/* Measured FP64 FMA throughput of the device (register-resident DFMA chains, all SMs), in TFLOP/s (FMA = 2 flop).
+ * Synchronous.  Used as the measured denominator of the FP64 roofline.                                                */
+int m3dk_fp64_peak_tflops(m3dk_ctx *ctx, double *tflops);
+
+/* Per-kernel timing for the roofline report.  With profiling on, the library brackets every push-kernel launch and
+ * every sort (its kernels as one group) with CUDA events on the context's stream.  m3dk_timing synchronises the stream,
+ * adds the elapsed times since the last call to the totals and returns them; m3dk_set_profiling(ctx, 1) zeroes the
+ * totals.  kernel_launches counts every kernel the library enqueued since then (profiling on or off).                */
+typedef struct {
+    double push_ms;       /* sum of push-kernel durations                                                              */
+    double sort_ms;       /* sum of sort durations (histogram + scan + scatter / permutation kernels)                  */
+    long push_launches;
+    long sort_launches;   /* number of sorts timed                                                                     */
+    long kernel_launches; /* all kernels enqueued by the library                                                       */
+} m3dk_timing_t;
+int m3dk_set_profiling(m3dk_ctx *ctx, int on);
+int m3dk_timing(m3dk_ctx *ctx, m3dk_timing_t *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* M3DK_H */

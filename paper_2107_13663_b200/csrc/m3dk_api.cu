@@ -1,0 +1,451 @@
+// m3dk_api.cu -- the C ABI of libm3dk (include/m3dk.h): argument checks, table repacking, launch logic.
+// Host code only; the kernels are in m3dk_push.cu and m3dk_sort.cu.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "m3dk_internal.h"
+
+using namespace m3dk;
+
+static std::string g_create_error;
+
+static int fail(m3dk_ctx *c, int code, const std::string &msg) {
+    if (c) c->err = msg; else g_create_error = msg;
+    return code;
+}
+static int cuda_fail(m3dk_ctx *c, cudaError_t e, const char *what) {
+    return fail(c, M3DK_ECUDA, std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")");
+}
+#define CU(call, what)                                        \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, what); \
+    } while (0)
+
+static inline size_t up256(size_t b) { return (b + 255) / 256 * 256; }
+
+// profiling brackets: a pair of events around a launch group, kept until m3dk_timing collects them
+struct EvScope {
+    m3dk_ctx *c; std::vector<std::pair<cudaEvent_t, cudaEvent_t>> *v; cudaEvent_t a = nullptr, b = nullptr;
+    EvScope(m3dk_ctx *ctx, std::vector<std::pair<cudaEvent_t, cudaEvent_t>> *vec) : c(ctx), v(vec) {
+        if (!c->profiling) return;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { a = b = nullptr; return; }
+        cudaEventRecord(a, c->stream);
+    }
+    ~EvScope() {
+        if (!a) return;
+        cudaEventRecord(b, c->stream);
+        v->emplace_back(a, b);
+    }
+};
+static void drop_events(std::vector<std::pair<cudaEvent_t, cudaEvent_t>> &v, double *acc, long *cnt) {
+    for (auto &p : v) {
+        float ms = 0.f;
+        if (acc && cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) { *acc += ms; ++*cnt; }
+        cudaEventDestroy(p.first); cudaEventDestroy(p.second);
+    }
+    v.clear();
+}
+
+extern "C" int m3dk_version(void) { return 100; }
+
+extern "C" const char *m3dk_last_error(const m3dk_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+extern "C" int m3dk_create(m3dk_ctx **out, int device, void *stream) {
+    m3dk_ctx *ctx = nullptr;
+    if (!out) return fail(nullptr, M3DK_EINVAL, "m3dk_create: out is NULL");
+    *out = nullptr;
+    int ndev = 0;
+    CU(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount (libm3dk has no CPU fallback)");
+    if (device < 0 || device >= ndev) return fail(nullptr, M3DK_EINVAL, "m3dk_create: no such CUDA device");
+    CU(cudaSetDevice(device), "cudaSetDevice");
+    ctx = new m3dk_ctx();
+    ctx->device = device;
+    ctx->stream = static_cast<cudaStream_t>(stream);
+    *out = ctx;
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_destroy(m3dk_ctx *ctx) {
+    if (!ctx) return M3DK_EINVAL;
+    drop_events(ctx->ev_push, nullptr, nullptr);
+    drop_events(ctx->ev_sort, nullptr, nullptr);
+    delete ctx;
+    return M3DK_OK;
+}
+
+// ---- fields --------------------------------------------------------------------------------------------------------
+// workspace: [control block 256 B][tiles][edge records][bstart][bcand (<= kCandPerElem * n_elems)]
+static constexpr int kCandPerElem = 24;
+
+static int grid_dim(int n_elems) {
+    int g = (int)ceil(sqrt(0.5 * (double)n_elems));
+    return g < 1 ? 1 : g;
+}
+
+extern "C" int m3dk_fields_workspace_bytes(int n_nodes, int n_elems, int n_modes, size_t *bytes) {
+    if (!bytes || n_nodes < 3 || n_elems < 1 || n_modes < 0 || n_modes > M3DK_MAX_MODES) return M3DK_EINVAL;
+    const int g = grid_dim(n_elems);
+    size_t b = 256;
+    b += up256((size_t)n_elems * tile_stride_doubles(n_modes) * sizeof(double));
+    b += up256((size_t)n_elems * kEdgeRec * sizeof(double));
+    b += up256(((size_t)g * g + 1) * sizeof(int));
+    b += up256((size_t)kCandPerElem * n_elems * sizeof(int) + 1024);
+    *bytes = b;
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node_RZ, int n_elems, const int *tri,
+                                  const double *eq_coef, int n_modes, const int *n_tor, const double *omega,
+                                  const double *pert_coef, void *dev_workspace, size_t workspace_bytes) {
+    if (!ctx) return M3DK_EINVAL;
+    size_t need = 0;
+    if (m3dk_fields_workspace_bytes(n_nodes, n_elems, n_modes, &need) != M3DK_OK || !node_RZ || !tri || !eq_coef ||
+        (n_modes > 0 && (!n_tor || !omega || !pert_coef)))
+        return fail(ctx, M3DK_EINVAL, "m3dk_fields_create: bad sizes or NULL table pointer");
+    if (!dev_workspace || workspace_bytes < need || ((uintptr_t)dev_workspace & 255))
+        return fail(ctx, M3DK_EWORKSPACE, "m3dk_fields_create: workspace NULL, misaligned or smaller than m3dk_fields_workspace_bytes");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    ctx->have_fields = false;
+
+    const int stride = tile_stride_doubles(n_modes);
+    std::vector<double> tiles((size_t)n_elems * stride, 0.0), edges((size_t)n_elems * kEdgeRec, 0.0);
+    double Rmin = 1e300, Rmax = -1e300, Zmin = 1e300, Zmax = -1e300;
+    for (int i = 0; i < n_nodes; ++i) {
+        const double r = node_RZ[2 * i], z = node_RZ[2 * i + 1];
+        if (!(r == r) || !(z == z)) return fail(ctx, M3DK_EINVAL, "m3dk_fields_create: NaN node coordinate");
+        Rmin = std::min(Rmin, r); Rmax = std::max(Rmax, r); Zmin = std::min(Zmin, z); Zmax = std::max(Zmax, z);
+    }
+    if (!(Rmin > 0.0)) return fail(ctx, M3DK_EINVAL, "m3dk_fields_create: nodes must have R > 0");
+
+    // per-element header, edge records, interleaved coefficient pairs
+    for (int e = 0; e < n_elems; ++e) {
+        double pr[3], pz[3];
+        for (int k = 0; k < 3; ++k) {
+            const int nd = tri[3 * e + k];
+            if (nd < 0 || nd >= n_nodes) return fail(ctx, M3DK_EINVAL, "m3dk_fields_create: node index out of range");
+            pr[k] = node_RZ[2 * nd]; pz[k] = node_RZ[2 * nd + 1];
+        }
+        const double area2 = (pr[1] - pr[0]) * (pz[2] - pz[0]) - (pz[1] - pz[0]) * (pr[2] - pr[0]);
+        if (!(area2 > 0.0)) return fail(ctx, M3DK_EINVAL, "m3dk_fields_create: triangle is degenerate or not counter-clockwise");
+        double L = 0.0;
+        double *er = &edges[(size_t)e * kEdgeRec];
+        for (int k = 0; k < 3; ++k) {
+            const int kb = (k + 1) % 3;
+            const double dx = pr[kb] - pr[k], dz = pz[kb] - pz[k];
+            er[4 * k + 0] = pr[k]; er[4 * k + 1] = pz[k]; er[4 * k + 2] = dx; er[4 * k + 3] = dz;
+            L = std::max(L, sqrt(dx * dx + dz * dz));
+        }
+        er[12] = 1e-9 * L * L;  // strict-interior tolerance: far above the rounding of an edge function, far below its size
+        double *t = &tiles[(size_t)e * stride];
+        t[0] = (pr[0] + pr[1] + pr[2]) / 3.0;   // centroid and scale exactly as reading G10 defines them
+        t[1] = (pz[0] + pz[1] + pz[2]) / 3.0;
+        t[2] = 1.0 / L;
+        const double *ce = eq_coef + (size_t)e * M3DK_N_EQ * M3DK_NCOEF;
+        double *pa = t + kTileHeader, *pb = pa + kPair;
+        for (int k = 0; k < M3DK_NCOEF; ++k) {
+            pa[2 * k] = ce[0 * M3DK_NCOEF + k]; pa[2 * k + 1] = ce[1 * M3DK_NCOEF + k];
+            pb[2 * k] = ce[2 * M3DK_NCOEF + k]; pb[2 * k + 1] = ce[3 * M3DK_NCOEF + k];
+        }
+        for (int md = 0; md < n_modes; ++md) {
+            const double *cp = pert_coef + ((size_t)md * n_elems + e) * (M3DK_N_PERT * 2 * M3DK_NCOEF);
+            double *pm = t + kTileHeader + kTileEq + (size_t)kTileMode * md;
+            for (int q = 0; q < M3DK_N_PERT; ++q)
+                for (int k = 0; k < M3DK_NCOEF; ++k) {
+                    pm[q * kPair + 2 * k] = cp[(2 * q + 0) * M3DK_NCOEF + k];
+                    pm[q * kPair + 2 * k + 1] = cp[(2 * q + 1) * M3DK_NCOEF + k];
+                }
+        }
+    }
+
+    // bucket grid: every element whose triangle touches the (slightly inflated) bucket, best bbox overlap first
+    const int g = grid_dim(n_elems);
+    const double hx = (Rmax - Rmin) / g, hz = (Zmax - Zmin) / g;
+    const double tolx = 1e-7 * hx, tolz = 1e-7 * hz;
+    struct Cand { int b, e; double ov; };
+    std::vector<Cand> cands;
+    cands.reserve((size_t)n_elems * 10);
+    for (int e = 0; e < n_elems; ++e) {
+        const double *er = &edges[(size_t)e * kEdgeRec];
+        double r0 = std::min({er[0], er[4], er[8]}), r1 = std::max({er[0], er[4], er[8]});
+        double z0 = std::min({er[1], er[5], er[9]}), z1 = std::max({er[1], er[5], er[9]});
+        int ix0 = std::max(0, (int)floor((r0 - tolx - Rmin) / hx)), ix1 = std::min(g - 1, (int)floor((r1 + tolx - Rmin) / hx));
+        int iz0 = std::max(0, (int)floor((z0 - tolz - Zmin) / hz)), iz1 = std::min(g - 1, (int)floor((z1 + tolz - Zmin) / hz));
+        for (int iz = iz0; iz <= iz1; ++iz)
+            for (int ix = ix0; ix <= ix1; ++ix) {
+                const double bx0 = Rmin + ix * hx - tolx, bx1 = Rmin + (ix + 1) * hx + tolx;
+                const double bz0 = Zmin + iz * hz - tolz, bz1 = Zmin + (iz + 1) * hz + tolz;
+                // separating-axis test against the three edge normals (the bbox axes are covered by the loop bounds)
+                bool sep = false;
+                for (int k = 0; k < 3 && !sep; ++k) {
+                    const double ra = er[4 * k], za = er[4 * k + 1], dx = er[4 * k + 2], dz = er[4 * k + 3];
+                    const double cx = dz > 0 ? bx0 : bx1;   // corner that maximises dx (Z - za) - dz (R - ra)
+                    const double cz = dx > 0 ? bz1 : bz0;
+                    if (dx * (cz - za) - dz * (cx - ra) < 0.0) sep = true;
+                }
+                if (sep) continue;
+                const double ox = std::min(r1, bx1) - std::max(r0, bx0), oz = std::min(z1, bz1) - std::max(z0, bz0);
+                cands.push_back({iz * g + ix, e, std::max(ox, 0.0) * std::max(oz, 0.0)});
+            }
+    }
+    if (cands.size() > (size_t)kCandPerElem * n_elems)
+        return fail(ctx, M3DK_EWORKSPACE, "m3dk_fields_create: search grid needs more candidate slots than the workspace bound");
+    std::sort(cands.begin(), cands.end(), [](const Cand &a, const Cand &b) {
+        if (a.b != b.b) return a.b < b.b;
+        if (a.ov != b.ov) return a.ov > b.ov;
+        return a.e < b.e;
+    });
+    std::vector<int> bstart((size_t)g * g + 1, 0), bcand(cands.size() + 1, 0);
+    for (size_t k = 0; k < cands.size(); ++k) { bstart[cands[k].b + 1]++; bcand[k] = cands[k].e; }
+    for (int b = 0; b < g * g; ++b) bstart[b + 1] += bstart[b];
+
+    // carve and upload
+    char *p = static_cast<char *>(dev_workspace);
+    ctx->d_count = reinterpret_cast<int *>(p); p += 256;
+    double *d_tiles = reinterpret_cast<double *>(p); p += up256(tiles.size() * sizeof(double));
+    double *d_edges = reinterpret_cast<double *>(p); p += up256(edges.size() * sizeof(double));
+    int *d_bstart = reinterpret_cast<int *>(p); p += up256(bstart.size() * sizeof(int));
+    int *d_bcand = reinterpret_cast<int *>(p);
+    CU(cudaMemsetAsync(ctx->d_count, 0, 256, ctx->stream), "memset control block");
+    CU(cudaMemcpyAsync(d_tiles, tiles.data(), tiles.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "upload tiles");
+    CU(cudaMemcpyAsync(d_edges, edges.data(), edges.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "upload edge records");
+    CU(cudaMemcpyAsync(d_bstart, bstart.data(), bstart.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream), "upload grid");
+    CU(cudaMemcpyAsync(d_bcand, bcand.data(), bcand.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream), "upload grid candidates");
+    CU(cudaStreamSynchronize(ctx->stream), "fields upload");
+
+    FieldParams &f = ctx->f;
+    f = FieldParams{};
+    f.tiles = d_tiles; f.tile_stride = stride; f.n_elems = n_elems; f.n_modes = n_modes;
+    for (int k = 0; k < n_modes; ++k) { f.n_tor[k] = n_tor[k]; f.omega[k] = omega[k]; }
+    f.grid.Rmin = Rmin; f.grid.Rmax = Rmax; f.grid.Zmin = Zmin; f.grid.Zmax = Zmax;
+    f.grid.inv_hx = 1.0 / hx; f.grid.inv_hz = 1.0 / hz; f.grid.gx = g; f.grid.gz = g;
+    f.grid.bstart = d_bstart; f.grid.bcand = d_bcand; f.grid.edges = d_edges;
+    ctx->have_fields = true;
+    ctx->have_markers = false;   // cached elements refer to the old mesh
+    return M3DK_OK;
+}
+
+// ---- markers -------------------------------------------------------------------------------------------------------
+extern "C" int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, double *z, double *vx, double *vy,
+                                   double *vz, double *mu, double *w, int *elem, int *id, double charge, double mass,
+                                   const m3dk_f0_params *f0) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_fields) return fail(ctx, M3DK_ESTATE, "m3dk_particles_init: call m3dk_fields_create first");
+    if (n < 0 || n > 0x7fffffffL || (n > 0 && (!x || !y || !z || !vx || !vy || !vz || !mu || !w || !elem || !id)) || !f0)
+        return fail(ctx, M3DK_EINVAL, "m3dk_particles_init: bad n or NULL array");
+    if (!(charge != 0.0) || !(mass > 0.0)) return fail(ctx, M3DK_EINVAL, "m3dk_particles_init: charge must be non-zero and mass positive");
+    if (f0->kind < 0 || f0->kind > 2 || (f0->kind == M3DK_F0_MAXWELLIAN && !(f0->T > 0.0)) ||
+        (f0->kind != M3DK_F0_MAXWELLIAN && !(f0->v_c > 0.0)) || (f0->kind == M3DK_F0_BEAM_PITCH && !(f0->dLambda > 0.0)))
+        return fail(ctx, M3DK_EINVAL, "m3dk_particles_init: bad f0 parameters");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    ctx->n = n;
+    ctx->user = MarkerArrays{x, y, z, vx, vy, vz, mu, w, elem, id};
+    ctx->cur = 0;
+    ctx->q = charge; ctx->m = mass; ctx->f0 = *f0;
+    ctx->steps_done = 0; ctx->n_sorts = 0;
+    ctx->steps_since_sort = ctx->sort_interval;   // the first push sorts first when sorting is on
+    ctx->have_markers = true;
+    if (ctx->have_sortws && ctx->sb.bytes) {      // an older workspace may be too small for the new n
+        if (sort_workspace_bytes(n, ctx->f.n_elems) > ctx->sb.bytes) ctx->have_sortws = false;
+    }
+    CU(launch_locate(ctx, ctx->user, n, true), "locate kernel");
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, double t0) {
+    if (!ctx) return M3DK_EINVAL;
+    if (sort_interval < 0) return fail(ctx, M3DK_EINVAL, "m3dk_set_options: sort_interval < 0");
+    if (mode != 0) return fail(ctx, M3DK_EINVAL, "m3dk_set_options: only mode 0 (linear delta-f) exists");
+    ctx->sort_interval = sort_interval; ctx->mode = mode; ctx->t0 = t0;
+    ctx->steps_done = 0;
+    ctx->steps_since_sort = sort_interval;
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_sort_workspace_bytes(long n_markers, int n_elems, size_t *bytes) {
+    if (!bytes || n_markers < 0 || n_elems < 1) return M3DK_EINVAL;
+    *bytes = sort_workspace_bytes(n_markers, n_elems);
+    return M3DK_OK;
+}
+
+static int bind_sort_ws(m3dk_ctx *ctx, void *ws, size_t bytes, const char *who) {
+    if (!ctx->have_markers) return fail(ctx, M3DK_ESTATE, std::string(who) + ": call m3dk_particles_init first");
+    if (!ws || ((uintptr_t)ws & 255) || bytes < sort_workspace_bytes(ctx->n, ctx->f.n_elems))
+        return fail(ctx, M3DK_EWORKSPACE, std::string(who) + ": workspace NULL, misaligned or smaller than m3dk_sort_workspace_bytes");
+    carve_sort_workspace(ws, ctx->n, ctx->f.n_elems, &ctx->sb);
+    ctx->sb.bytes = bytes;
+    ctx->have_sortws = true;
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_set_sort_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes) {
+    if (!ctx) return M3DK_EINVAL;
+    return bind_sort_ws(ctx, dev_workspace, bytes, "m3dk_set_sort_workspace");
+}
+
+static const MarkerArrays &cur_arrays(m3dk_ctx *ctx) { return ctx->cur ? ctx->sb.alt : ctx->user; }
+
+static int sort_flip(m3dk_ctx *ctx) {   // sort current -> other, other becomes current
+    const MarkerArrays &src = cur_arrays(ctx);
+    const MarkerArrays &dst = ctx->cur ? ctx->user : ctx->sb.alt;
+    {
+        EvScope ev(ctx, &ctx->ev_sort);
+        CU(launch_sort(ctx, src, dst, ctx->n), "sort kernels");
+    }
+    ctx->cur ^= 1;
+    ctx->n_sorts++;
+    ctx->steps_since_sort = 0;
+    return M3DK_OK;
+}
+
+static int settle(m3dk_ctx *ctx) {      // make the caller's arrays current again
+    if (!ctx->cur) return M3DK_OK;
+    const MarkerArrays &s = ctx->sb.alt, &d = ctx->user;
+    const size_t nd = (size_t)ctx->n * sizeof(double), ni = (size_t)ctx->n * sizeof(int);
+    double *const sd[8] = {s.x, s.y, s.z, s.vx, s.vy, s.vz, s.mu, s.w};
+    double *const dd[8] = {d.x, d.y, d.z, d.vx, d.vy, d.vz, d.mu, d.w};
+    for (int k = 0; k < 8; ++k) CU(cudaMemcpyAsync(dd[k], sd[k], nd, cudaMemcpyDeviceToDevice, ctx->stream), "copy back");
+    CU(cudaMemcpyAsync(d.elem, s.elem, ni, cudaMemcpyDeviceToDevice, ctx->stream), "copy back");
+    CU(cudaMemcpyAsync(d.id, s.id, ni, cudaMemcpyDeviceToDevice, ctx->stream), "copy back");
+    ctx->cur = 0;
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_sort(m3dk_ctx *ctx, void *dev_workspace, size_t bytes) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_sort: call m3dk_particles_init first");
+    if (dev_workspace) {
+        int rc = bind_sort_ws(ctx, dev_workspace, bytes, "m3dk_sort");
+        if (rc != M3DK_OK) return rc;
+    } else if (!ctx->have_sortws) {
+        return fail(ctx, M3DK_ESTATE, "m3dk_sort: no workspace (pass one or call m3dk_set_sort_workspace)");
+    }
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (ctx->n == 0) return M3DK_OK;
+    int rc = sort_flip(ctx);
+    if (rc != M3DK_OK) return rc;
+    return settle(ctx);
+}
+
+extern "C" int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_push: fields and markers must be set first");
+    if (nsteps < 0 || !(dt == dt)) return fail(ctx, M3DK_EINVAL, "m3dk_push: nsteps < 0 or dt is NaN");
+    if (ctx->sort_interval > 0 && !ctx->have_sortws)
+        return fail(ctx, M3DK_ESTATE, "m3dk_push: sort_interval > 0 needs m3dk_set_sort_workspace");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    ctx->last_dt = dt;
+    for (int l = 0; l < nsteps; ++l) {
+        if (ctx->sort_interval > 0 && ctx->steps_since_sort >= ctx->sort_interval && ctx->n > 0) {
+            int rc = sort_flip(ctx);
+            if (rc != M3DK_OK) return rc;
+        }
+        const double t = ctx->t0 + (double)ctx->steps_done * dt;   // t_l of this step's x_l
+        {
+            EvScope ev(ctx, &ctx->ev_push);
+            CU(launch_push(ctx, cur_arrays(ctx), ctx->n, dt, t), "push kernel");
+        }
+        ctx->steps_done++;
+        ctx->steps_since_sort++;
+    }
+    return settle(ctx);
+}
+
+extern "C" int m3dk_stats(m3dk_ctx *ctx, m3dk_stats_t *out) {
+    if (!ctx || !out) return M3DK_EINVAL;
+    memset(out, 0, sizeof(*out));
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    int lost = 0;
+    if (ctx->have_markers) {
+        CU(launch_count_lost(ctx, ctx->user, ctx->n, ctx->d_count), "count kernel");
+        CU(cudaMemcpyAsync(&lost, ctx->d_count, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream), "read counter");
+    }
+    CU(cudaStreamSynchronize(ctx->stream), "stream synchronize (an earlier kernel may have failed)");
+    out->n_markers = ctx->have_markers ? ctx->n : 0;
+    out->n_lost = lost;
+    out->steps_done = ctx->steps_done;
+    out->n_sorts = ctx->n_sorts;
+    out->t = ctx->t0 + (double)ctx->steps_done * ctx->last_dt;
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_particles_upload(m3dk_ctx *ctx, const double *hx, const double *hy, const double *hz,
+                                     const double *hvx, const double *hvy, const double *hvz, const double *hmu,
+                                     const double *hw) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_particles_upload: call m3dk_particles_init first");
+    if (!hx || !hy || !hz || !hvx || !hvy || !hvz || !hmu || !hw) return fail(ctx, M3DK_EINVAL, "m3dk_particles_upload: NULL buffer");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    const MarkerArrays &d = ctx->user;
+    const size_t nd = (size_t)ctx->n * sizeof(double);
+    const double *const hs[8] = {hx, hy, hz, hvx, hvy, hvz, hmu, hw};
+    double *const dd[8] = {d.x, d.y, d.z, d.vx, d.vy, d.vz, d.mu, d.w};
+    for (int k = 0; k < 8; ++k) CU(cudaMemcpyAsync(dd[k], hs[k], nd, cudaMemcpyHostToDevice, ctx->stream), "upload markers");
+    ctx->cur = 0;
+    ctx->steps_since_sort = ctx->sort_interval;
+    CU(launch_locate(ctx, ctx->user, ctx->n, true), "locate kernel");
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, double *hz, double *hvx, double *hvy,
+                                       double *hvz, double *hmu, double *hw, int *host_id, int *host_elem) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_particles_download: call m3dk_particles_init first");
+    if (!hx || !hy || !hz || !hvx || !hvy || !hvz || !hmu || !hw) return fail(ctx, M3DK_EINVAL, "m3dk_particles_download: NULL buffer");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    const MarkerArrays &d = ctx->user;
+    const size_t nd = (size_t)ctx->n * sizeof(double), ni = (size_t)ctx->n * sizeof(int);
+    double *const hs[8] = {hx, hy, hz, hvx, hvy, hvz, hmu, hw};
+    const double *const dd[8] = {d.x, d.y, d.z, d.vx, d.vy, d.vz, d.mu, d.w};
+    for (int k = 0; k < 8; ++k) CU(cudaMemcpyAsync(hs[k], dd[k], nd, cudaMemcpyDeviceToHost, ctx->stream), "download markers");
+    if (host_id) CU(cudaMemcpyAsync(host_id, d.id, ni, cudaMemcpyDeviceToHost, ctx->stream), "download id");
+    if (host_elem) CU(cudaMemcpyAsync(host_elem, d.elem, ni, cudaMemcpyDeviceToHost, ctx->stream), "download elem");
+    CU(cudaStreamSynchronize(ctx->stream), "stream synchronize (an earlier kernel may have failed)");
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_eval_fields(m3dk_ctx *ctx, long n, const double *R, const double *phi, const double *Z, double t,
+                                int *elem_out, double *out) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_fields) return fail(ctx, M3DK_ESTATE, "m3dk_eval_fields: call m3dk_fields_create first");
+    if (n < 0 || (n > 0 && (!R || !phi || !Z || !elem_out || !out))) return fail(ctx, M3DK_EINVAL, "m3dk_eval_fields: bad argument");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CU(launch_eval_fields(ctx, n, R, phi, Z, t, elem_out, out), "eval kernel");
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_fp64_peak_tflops(m3dk_ctx *ctx, double *tflops) {
+    if (!ctx || !tflops) return M3DK_EINVAL;
+    if (!ctx->have_fields) return fail(ctx, M3DK_ESTATE, "m3dk_fp64_peak_tflops: call m3dk_fields_create first (uses its control block)");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CU(fp64_probe(ctx, tflops), "fp64 probe");
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_set_profiling(m3dk_ctx *ctx, int on) {
+    if (!ctx) return M3DK_EINVAL;
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CU(cudaStreamSynchronize(ctx->stream), "stream synchronize");
+    drop_events(ctx->ev_push, nullptr, nullptr);
+    drop_events(ctx->ev_sort, nullptr, nullptr);
+    ctx->profiling = on != 0;
+    ctx->push_ms = ctx->sort_ms = 0.0;
+    ctx->push_launches = ctx->sort_launches = ctx->kernel_launches = 0;
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_timing(m3dk_ctx *ctx, m3dk_timing_t *out) {
+    if (!ctx || !out) return M3DK_EINVAL;
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CU(cudaStreamSynchronize(ctx->stream), "stream synchronize (an earlier kernel may have failed)");
+    drop_events(ctx->ev_push, &ctx->push_ms, &ctx->push_launches);
+    drop_events(ctx->ev_sort, &ctx->sort_ms, &ctx->sort_launches);
+    out->push_ms = ctx->push_ms; out->sort_ms = ctx->sort_ms;
+    out->push_launches = ctx->push_launches; out->sort_launches = ctx->sort_launches;
+    out->kernel_launches = ctx->kernel_launches;
+    return M3DK_OK;
+}

@@ -1,0 +1,92 @@
+// m3dk_sort.cu -- counting sort of the markers by element.
+// key = element of the marker's current position (cached by the push), lost markers (-1) get key n_elems (last).
+// histogram with returned ranks (one atomic per marker) -> exclusive scan -> scatter of the 8 fp64 arrays + elem + id.
+#include "m3dk_internal.h"
+
+namespace m3dk {
+
+static inline size_t up256(size_t b) { return (b + 255) / 256 * 256; }
+
+size_t sort_workspace_bytes(long n, int n_elems) {
+    const size_t nd = up256((size_t)n * sizeof(double)), ni = up256((size_t)n * sizeof(int));
+    const size_t nh = up256((size_t)(n_elems + 2) * sizeof(int));
+    return 8 * nd + 3 * ni + 2 * nh;
+}
+
+void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb) {
+    char *p = static_cast<char *>(ws);
+    const size_t nd = up256((size_t)n * sizeof(double)), ni = up256((size_t)n * sizeof(int));
+    const size_t nh = up256((size_t)(n_elems + 2) * sizeof(int));
+    double **d[8] = {&sb->alt.x, &sb->alt.y, &sb->alt.z, &sb->alt.vx, &sb->alt.vy, &sb->alt.vz, &sb->alt.mu, &sb->alt.w};
+    for (auto q : d) { *q = reinterpret_cast<double *>(p); p += nd; }
+    sb->alt.elem = reinterpret_cast<int *>(p); p += ni;
+    sb->alt.id = reinterpret_cast<int *>(p); p += ni;
+    sb->rank = reinterpret_cast<int *>(p); p += ni;
+    sb->hist = reinterpret_cast<int *>(p); p += nh;
+    sb->offs = reinterpret_cast<int *>(p); p += nh;
+    sb->bytes = (size_t)(p - static_cast<char *>(ws));
+}
+
+__global__ void __launch_bounds__(256) hist_rank_kernel(const int *__restrict__ elem, long n, int n_elems,
+                                                        int *__restrict__ hist, int *__restrict__ rank) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned live = __ballot_sync(0xffffffffu, i < n);
+    if (i >= n) return;
+    const int e = elem[i];
+    const int key = e < 0 ? n_elems : e;
+    // warp-aggregated: lanes with the same key elect a leader that does one atomic for the group
+    const unsigned peers = __match_any_sync(live, key);
+    const int lane = threadIdx.x & 31;
+    const int leader = __ffs(peers) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(hist + key, __popc(peers));
+    base = __shfl_sync(peers, base, leader);
+    rank[i] = base + __popc(peers & ((1u << lane) - 1u));
+}
+
+// exclusive scan of hist[0..m) into offs[0..m], one block (m <= a few 1e5 bins: microseconds)
+__global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist, int m, int *__restrict__ offs) {
+    __shared__ int part[1024];
+    const int t = threadIdx.x, per = (m + 1023) / 1024;
+    const int b = t * per, e = min(b + per, m);
+    int s = 0;
+    for (int k = b; k < e; ++k) s += hist[k];
+    part[t] = s;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+        int v = t >= o ? part[t - o] : 0;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    int run = t ? part[t - 1] : 0;
+    for (int k = b; k < e; ++k) { offs[k] = run; run += hist[k]; }
+    if (t == 1023) offs[m] = part[1023];
+}
+
+__global__ void __launch_bounds__(256) scatter_kernel(MarkerArrays s, MarkerArrays d, long n, int n_elems,
+                                                      const int *__restrict__ offs, const int *__restrict__ rank) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int e = s.elem[i];
+    const long j = (long)offs[e < 0 ? n_elems : e] + rank[i];
+    d.x[j] = s.x[i]; d.y[j] = s.y[i]; d.z[j] = s.z[i];
+    d.vx[j] = s.vx[i]; d.vy[j] = s.vy[i]; d.vz[j] = s.vz[i];
+    d.mu[j] = s.mu[i]; d.w[j] = s.w[i];
+    d.elem[j] = e; d.id[j] = s.id[i];
+}
+
+cudaError_t launch_sort(m3dk_ctx *c, const MarkerArrays &src, const MarkerArrays &dst, long n) {
+    if (n == 0) return cudaSuccess;
+    const int m = c->f.n_elems + 1;
+    cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)m * sizeof(int), c->stream);
+    if (e != cudaSuccess) return e;
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    c->kernel_launches += 3;
+    hist_rank_kernel<<<grid, 256, 0, c->stream>>>(src.elem, n, c->f.n_elems, c->sb.hist, c->sb.rank);
+    scan_kernel<<<1, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs);
+    scatter_kernel<<<grid, 256, 0, c->stream>>>(src, dst, n, c->f.n_elems, c->sb.offs, c->sb.rank);
+    return cudaGetLastError();
+}
+
+}  // namespace m3dk
