@@ -80,7 +80,14 @@ extern "C" int m3dk_destroy(m3dk_ctx *ctx) {
 
 // ---- fields --------------------------------------------------------------------------------------------------------
 // workspace: [control block 256 B][tiles][edge records][bstart][bcand (<= kCandPerElem * n_elems)]
+//            [fast grid: first records gf*gf][overflow records kFastOvfPerElem * n_elems]
 static constexpr int kCandPerElem = 24;
+static constexpr int kFastOvfPerElem = 12;
+
+static int fast_grid_dim(int n_elems) {
+    int g = (int)ceil(sqrt(2.0 * (double)n_elems));
+    return g < 1 ? 1 : g;
+}
 
 static int grid_dim(int n_elems) {
     int g = (int)ceil(sqrt(0.5 * (double)n_elems));
@@ -95,6 +102,9 @@ extern "C" int m3dk_fields_workspace_bytes(int n_nodes, int n_elems, int n_modes
     b += up256((size_t)n_elems * kEdgeRec * sizeof(double));
     b += up256(((size_t)g * g + 1) * sizeof(int));
     b += up256((size_t)kCandPerElem * n_elems * sizeof(int) + 1024);
+    const int gf = fast_grid_dim(n_elems);
+    b += up256((size_t)gf * gf * sizeof(FastRec));
+    b += up256((size_t)kFastOvfPerElem * n_elems * sizeof(FastRec) + 1024);
     *bytes = b;
     return M3DK_OK;
 }
@@ -146,19 +156,16 @@ extern "C" int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node
         t[1] = (pz[0] + pz[1] + pz[2]) / 3.0;
         t[2] = 1.0 / L;
         const double *ce = eq_coef + (size_t)e * M3DK_N_EQ * M3DK_NCOEF;
-        double *pa = t + kTileHeader, *pb = pa + kPair;
-        for (int k = 0; k < M3DK_NCOEF; ++k) {
-            pa[2 * k] = ce[0 * M3DK_NCOEF + k]; pa[2 * k + 1] = ce[1 * M3DK_NCOEF + k];
-            pb[2 * k] = ce[2 * M3DK_NCOEF + k]; pb[2 * k + 1] = ce[3 * M3DK_NCOEF + k];
-        }
+        double *pq = t + kTileHeader;
+        for (int k = 0; k < M3DK_NCOEF; ++k)
+            for (int q = 0; q < 4; ++q) pq[4 * k + q] = ce[q * M3DK_NCOEF + k];
         for (int md = 0; md < n_modes; ++md) {
+            // caller's order: [7 amplitudes][re, im][21]; amplitude a, part p is polynomial 2 a + p and goes to
+            // quad (2 a + p) / 4, slot (2 a + p) % 4 (B_par: quad 3, slots 0 and 1; slots 2 and 3 stay zero)
             const double *cp = pert_coef + ((size_t)md * n_elems + e) * (M3DK_N_PERT * 2 * M3DK_NCOEF);
             double *pm = t + kTileHeader + kTileEq + (size_t)kTileMode * md;
-            for (int q = 0; q < M3DK_N_PERT; ++q)
-                for (int k = 0; k < M3DK_NCOEF; ++k) {
-                    pm[q * kPair + 2 * k] = cp[(2 * q + 0) * M3DK_NCOEF + k];
-                    pm[q * kPair + 2 * k + 1] = cp[(2 * q + 1) * M3DK_NCOEF + k];
-                }
+            for (int pl = 0; pl < 2 * M3DK_N_PERT; ++pl)
+                for (int k = 0; k < M3DK_NCOEF; ++k) pm[(pl / 4) * kQuad + 4 * k + (pl % 4)] = cp[pl * M3DK_NCOEF + k];
         }
     }
 
@@ -203,18 +210,113 @@ extern "C" int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node
     for (size_t k = 0; k < cands.size(); ++k) { bstart[cands[k].b + 1]++; bcand[k] = cands[k].e; }
     for (int b = 0; b < g * g; ++b) bstart[b + 1] += bstart[b];
 
+    // fast search grid (fp32 records in bucket-local coordinates; see m3dk_internal.h).  Candidates of a bucket: the
+    // triangles that touch it, largest overlap area first, at most 4 (the device loop's bound); a bucket with a
+    // candidate too large for the fp32 error bound, or with none, sends its points to the exact search (id = -1).
+    const int gf = fast_grid_dim(n_elems);
+    const double fhx = (Rmax - Rmin) / gf, fhz = (Zmax - Zmin) / gf;
+    const double finv_hx = 1.0 / fhx, finv_hz = 1.0 / fhz;
+    struct FCand { int b, e; double area; float c[6]; bool big; };
+    std::vector<FCand> fc;
+    fc.reserve((size_t)n_elems * 10);
+    for (int e = 0; e < n_elems; ++e) {
+        const double *er = &edges[(size_t)e * kEdgeRec];
+        double gx_[3], gz_[3];
+        for (int k = 0; k < 3; ++k) { gx_[k] = (er[4 * k] - Rmin) * finv_hx; gz_[k] = (er[4 * k + 1] - Zmin) * finv_hz; }
+        const double x0 = std::min({gx_[0], gx_[1], gx_[2]}), x1 = std::max({gx_[0], gx_[1], gx_[2]});
+        const double z0 = std::min({gz_[0], gz_[1], gz_[2]}), z1 = std::max({gz_[0], gz_[1], gz_[2]});
+        const double ftol = 1e-6;
+        const int ix0 = std::max(0, (int)floor(x0 - ftol)), ix1 = std::min(gf - 1, (int)floor(x1 + ftol));
+        const int iz0 = std::max(0, (int)floor(z0 - ftol)), iz1 = std::min(gf - 1, (int)floor(z1 + ftol));
+        for (int iz = iz0; iz <= iz1; ++iz)
+            for (int ix = ix0; ix <= ix1; ++ix) {
+                double lx[3], lz[3];
+                bool big = false;
+                for (int k = 0; k < 3; ++k) {
+                    lx[k] = gx_[k] - ix; lz[k] = gz_[k] - iz;
+                    if (lx[k] < -(kFastCmax - 1.0) || lx[k] > kFastCmax || lz[k] < -(kFastCmax - 1.0) || lz[k] > kFastCmax) big = true;
+                }
+                // separating-axis test of the triangle against the inflated unit square
+                bool sep = false;
+                for (int k = 0; k < 3 && !sep; ++k) {
+                    const int kb = (k + 1) % 3;
+                    const double dx = lx[kb] - lx[k], dz = lz[kb] - lz[k];
+                    const double cx = dz > 0 ? -ftol : 1.0 + ftol, cz = dx > 0 ? 1.0 + ftol : -ftol;
+                    if (dx * (cz - lz[k]) - dz * (cx - lx[k]) < 0.0) sep = true;
+                }
+                if (sep) continue;
+                // overlap area: the triangle clipped to the unit square (Sutherland-Hodgman), shoelace formula
+                double px[16], pz[16], qx[16], qz[16];
+                int np = 3;
+                for (int k = 0; k < 3; ++k) { px[k] = lx[k]; pz[k] = lz[k]; }
+                for (int side = 0; side < 4 && np > 0; ++side) {
+                    int nq = 0;
+                    for (int k = 0; k < np; ++k) {
+                        const int kb = (k + 1) % np;
+                        const double ax = px[k], az = pz[k], bx = px[kb], bz = pz[kb];
+                        const double da = side == 0 ? ax : side == 1 ? 1.0 - ax : side == 2 ? az : 1.0 - az;
+                        const double db = side == 0 ? bx : side == 1 ? 1.0 - bx : side == 2 ? bz : 1.0 - bz;
+                        if (da >= 0.0) { qx[nq] = ax; qz[nq] = az; ++nq; }
+                        if ((da >= 0.0) != (db >= 0.0)) {
+                            const double tt = da / (da - db);
+                            qx[nq] = ax + tt * (bx - ax); qz[nq] = az + tt * (bz - az); ++nq;
+                        }
+                    }
+                    np = nq;
+                    for (int k = 0; k < np; ++k) { px[k] = qx[k]; pz[k] = qz[k]; }
+                }
+                double area = 0.0;
+                for (int k = 0; k < np; ++k) { const int kb = (k + 1) % np; area += px[k] * pz[kb] - px[kb] * pz[k]; }
+                FCand cnd{iz * gf + ix, e, 0.5 * fabs(area), {(float)lx[0], (float)lz[0], (float)lx[1], (float)lz[1], (float)lx[2], (float)lz[2]}, big};
+                fc.push_back(cnd);
+            }
+    }
+    std::sort(fc.begin(), fc.end(), [](const FCand &a, const FCand &b) {
+        if (a.b != b.b) return a.b < b.b;
+        if (a.area != b.area) return a.area > b.area;
+        return a.e < b.e;
+    });
+    const size_t ovf_cap = (size_t)kFastOvfPerElem * n_elems;
+    std::vector<FastRec> ffirst((size_t)gf * gf, FastRec{0.f, 0.f, 0.f, 0.f, 0.f, 0.f, -1, -1}), fovf;
+    fovf.reserve(std::min(ovf_cap, fc.size()));
+    for (size_t k = 0; k < fc.size();) {
+        size_t k1 = k;
+        bool big = false;
+        while (k1 < fc.size() && fc[k1].b == fc[k].b) { big = big || fc[k1].big; ++k1; }
+        if (!big) {
+            FastRec *prev = nullptr;
+            for (size_t j = k; j < k1 && j < k + 4; ++j) {
+                const FCand &cn = fc[j];
+                FastRec r{cn.c[0], cn.c[1], cn.c[2], cn.c[3], cn.c[4], cn.c[5], cn.e, -1};
+                if (j == k) { ffirst[cn.b] = r; prev = &ffirst[cn.b]; }
+                else {
+                    if (fovf.size() >= ovf_cap) break;
+                    prev->next = (int)fovf.size();
+                    fovf.push_back(r);         // reserve() above keeps `prev` valid: no reallocation below capacity
+                    prev = &fovf.back();
+                }
+            }
+        }
+        k = k1;
+    }
+    if (fovf.empty()) fovf.push_back(FastRec{0.f, 0.f, 0.f, 0.f, 0.f, 0.f, -1, -1});
+
     // carve and upload
     char *p = static_cast<char *>(dev_workspace);
     ctx->d_count = reinterpret_cast<int *>(p); p += 256;
     double *d_tiles = reinterpret_cast<double *>(p); p += up256(tiles.size() * sizeof(double));
     double *d_edges = reinterpret_cast<double *>(p); p += up256(edges.size() * sizeof(double));
     int *d_bstart = reinterpret_cast<int *>(p); p += up256(bstart.size() * sizeof(int));
-    int *d_bcand = reinterpret_cast<int *>(p);
+    int *d_bcand = reinterpret_cast<int *>(p); p += up256((size_t)kCandPerElem * n_elems * sizeof(int) + 1024);
+    FastRec *d_ffirst = reinterpret_cast<FastRec *>(p); p += up256(ffirst.size() * sizeof(FastRec));
+    FastRec *d_fovf = reinterpret_cast<FastRec *>(p);
     CU(cudaMemsetAsync(ctx->d_count, 0, 256, ctx->stream), "memset control block");
     CU(cudaMemcpyAsync(d_tiles, tiles.data(), tiles.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "upload tiles");
     CU(cudaMemcpyAsync(d_edges, edges.data(), edges.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "upload edge records");
     CU(cudaMemcpyAsync(d_bstart, bstart.data(), bstart.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream), "upload grid");
     CU(cudaMemcpyAsync(d_bcand, bcand.data(), bcand.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream), "upload grid candidates");
+    CU(cudaMemcpyAsync(d_ffirst, ffirst.data(), ffirst.size() * sizeof(FastRec), cudaMemcpyHostToDevice, ctx->stream), "upload fast grid");
+    CU(cudaMemcpyAsync(d_fovf, fovf.data(), fovf.size() * sizeof(FastRec), cudaMemcpyHostToDevice, ctx->stream), "upload fast grid overflow");
     CU(cudaStreamSynchronize(ctx->stream), "fields upload");
 
     FieldParams &f = ctx->f;
@@ -224,6 +326,8 @@ extern "C" int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node
     f.grid.Rmin = Rmin; f.grid.Rmax = Rmax; f.grid.Zmin = Zmin; f.grid.Zmax = Zmax;
     f.grid.inv_hx = 1.0 / hx; f.grid.inv_hz = 1.0 / hz; f.grid.gx = g; f.grid.gz = g;
     f.grid.bstart = d_bstart; f.grid.bcand = d_bcand; f.grid.edges = d_edges;
+    f.fast.Rmin = Rmin; f.fast.Zmin = Zmin; f.fast.inv_hx = finv_hx; f.fast.inv_hz = finv_hz;
+    f.fast.gx = gf; f.fast.gz = gf; f.fast.first = d_ffirst; f.fast.ovf = d_fovf;
     ctx->have_fields = true;
     ctx->have_markers = false;   // cached elements refer to the old mesh
     return M3DK_OK;
@@ -249,6 +353,7 @@ extern "C" int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, 
     ctx->steps_done = 0; ctx->n_sorts = 0;
     ctx->steps_since_sort = ctx->sort_interval;   // the first push sorts first when sorting is on
     ctx->have_markers = true;
+    ctx->hist_valid = false;
     if (ctx->have_sortws && ctx->sb.bytes) {      // an older workspace may be too small for the new n
         if (sort_workspace_bytes(n, ctx->f.n_elems) > ctx->sb.bytes) ctx->have_sortws = false;
     }
@@ -277,6 +382,7 @@ static int bind_sort_ws(m3dk_ctx *ctx, void *ws, size_t bytes, const char *who) 
     if (!ws || ((uintptr_t)ws & 255) || bytes < sort_workspace_bytes(ctx->n, ctx->f.n_elems))
         return fail(ctx, M3DK_EWORKSPACE, std::string(who) + ": workspace NULL, misaligned or smaller than m3dk_sort_workspace_bytes");
     carve_sort_workspace(ws, ctx->n, ctx->f.n_elems, &ctx->sb);
+    ctx->hist_valid = false;
     ctx->sb.bytes = bytes;
     ctx->have_sortws = true;
     return M3DK_OK;
@@ -294,8 +400,9 @@ static int sort_flip(m3dk_ctx *ctx) {   // sort current -> other, other becomes 
     const MarkerArrays &dst = ctx->cur ? ctx->user : ctx->sb.alt;
     {
         EvScope ev(ctx, &ctx->ev_sort);
-        CU(launch_sort(ctx, src, dst, ctx->n), "sort kernels");
+        CU(launch_sort(ctx, src, dst, ctx->n, ctx->hist_valid), "sort kernels");
     }
+    ctx->hist_valid = false;
     ctx->cur ^= 1;
     ctx->n_sorts++;
     ctx->steps_since_sort = 0;
@@ -346,8 +453,11 @@ extern "C" int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt) {
         }
         const double t = ctx->t0 + (double)ctx->steps_done * dt;   // t_l of this step's x_l
         {
+            // when the next step starts with a sort, this push also histograms its new keys (a11 fused into a10)
+            const bool with_hist = ctx->sort_interval > 0 && ctx->steps_since_sort + 1 >= ctx->sort_interval && ctx->n > 0;
             EvScope ev(ctx, &ctx->ev_push);
-            CU(launch_push(ctx, cur_arrays(ctx), ctx->n, dt, t), "push kernel");
+            CU(launch_push(ctx, cur_arrays(ctx), ctx->n, dt, t, with_hist), "push kernel");
+            ctx->hist_valid = with_hist;
         }
         ctx->steps_done++;
         ctx->steps_since_sort++;
@@ -386,6 +496,7 @@ extern "C" int m3dk_particles_upload(m3dk_ctx *ctx, const double *hx, const doub
     double *const dd[8] = {d.x, d.y, d.z, d.vx, d.vy, d.vz, d.mu, d.w};
     for (int k = 0; k < 8; ++k) CU(cudaMemcpyAsync(dd[k], hs[k], nd, cudaMemcpyHostToDevice, ctx->stream), "upload markers");
     ctx->cur = 0;
+    ctx->hist_valid = false;
     ctx->steps_since_sort = ctx->sort_interval;
     CU(launch_locate(ctx, ctx->user, ctx->n, true), "locate kernel");
     return M3DK_OK;

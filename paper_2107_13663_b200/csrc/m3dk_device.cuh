@@ -24,58 +24,50 @@ struct Fields {
 
 __device__ __forceinline__ double2 ldc(const double2 *p) { return __ldg(p); }
 
-// ---- polynomial pairs (G10: monomials xi^i eta^j, j outer, i inner; row j starts at kRow[j], has 6 - j terms) -----
-// c[k] = (a_k, b_k): two quintics evaluated together, Horner in xi inside a row, Horner in eta across rows.
-// value only: 15 + 5 FMA per polynomial.
-__device__ __forceinline__ void pair_v(const double2 *__restrict__ c, double xi, double eta, double &va, double &vb) {
-    constexpr int kRow[6] = {0, 6, 11, 15, 18, 20};
-    double a = 0.0, b = 0.0;
-#pragma unroll
-    for (int j = 5; j >= 0; --j) {
-        const int L = 6 - j;
-        double2 t = ldc(c + kRow[j] + L - 1);
-        double pa = t.x, pb = t.y;
-#pragma unroll
-        for (int i = L - 2; i >= 0; --i) {
-            t = ldc(c + kRow[j] + i);
-            pa = M3DK_FMA(pa, xi, t.x);
-            pb = M3DK_FMA(pb, xi, t.y);
-        }
-        if (j == 5) { a = pa; b = pb; }
-        else { a = M3DK_FMA(a, eta, pa); b = M3DK_FMA(b, eta, pb); }
-    }
-    va = a; vb = b;
+// One 32-byte read-only load (LDG.E.256.CONSTANT, sm_100): four interleaved coefficients.  Not volatile: the tables
+// are immutable for the lifetime of a kernel, so the compiler may hoist and reorder these freely.
+struct Quad { double a, b, c, d; };
+__device__ __forceinline__ Quad ldq(const double *p) {
+    Quad q;
+    asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(q.a), "=d"(q.b), "=d"(q.c), "=d"(q.d) : "l"(p));
+    return q;
 }
 
-// value, d/dxi, d/deta: 38 FMA per polynomial.
-__device__ __forceinline__ void pair_vd(const double2 *__restrict__ c, double xi, double eta, double &va, double &dxa,
-                                        double &dea, double &vb, double &dxb, double &deb) {
+// ---- polynomial quads (G10: monomials xi^i eta^j, j outer, i inner; row j starts at kRow[j], has 6 - j terms) -----
+// c[4 k + s]: coefficient k of slot s.  Horner in xi inside a row, Horner in eta across rows; value, d/dxi, d/deta of
+// all four slots: 38 FMA per slot.  Callers ignore the outputs they do not need; after full unrolling the unused
+// chains are dead code and disappear (value only: 20 FMA per slot).
+__device__ __forceinline__ void quad_vd(const double *__restrict__ c, double xi, double eta, double (&v)[4],
+                                        double (&dx)[4], double (&de)[4]) {
     constexpr int kRow[6] = {0, 6, 11, 15, 18, 20};
-    double a = 0.0, b = 0.0, ax = 0.0, bx = 0.0, ae = 0.0, be = 0.0;
+    double a[4], ax[4], ae[4];
 #pragma unroll
     for (int j = 5; j >= 0; --j) {
         const int L = 6 - j;
-        double2 t = ldc(c + kRow[j] + L - 1);
-        double pa = t.x, pb = t.y, da = 0.0, db = 0.0;
+        const Quad t = ldq(c + 4 * (kRow[j] + L - 1));
+        double p[4] = {t.a, t.b, t.c, t.d}, d[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
         for (int i = L - 2; i >= 0; --i) {
-            if (i == L - 2) { da = pa; db = pb; }
-            else { da = M3DK_FMA(da, xi, pa); db = M3DK_FMA(db, xi, pb); }
-            t = ldc(c + kRow[j] + i);
-            pa = M3DK_FMA(pa, xi, t.x);
-            pb = M3DK_FMA(pb, xi, t.y);
-        }
-        if (j == 5) { a = pa; b = pb; }
-        else {
-            if (j == 4) { ae = a; be = b; ax = da; bx = db; }
-            else {
-                ae = M3DK_FMA(ae, eta, a); be = M3DK_FMA(be, eta, b);
-                ax = M3DK_FMA(ax, eta, da); bx = M3DK_FMA(bx, eta, db);
+            const Quad u = ldq(c + 4 * (kRow[j] + i));
+            const double uu[4] = {u.a, u.b, u.c, u.d};
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                d[s] = (i == L - 2) ? p[s] : M3DK_FMA(d[s], xi, p[s]);
+                p[s] = M3DK_FMA(p[s], xi, uu[s]);
             }
-            a = M3DK_FMA(a, eta, pa); b = M3DK_FMA(b, eta, pb);
+        }
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            if (j == 5) { a[s] = p[s]; ax[s] = 0.0; ae[s] = 0.0; }
+            else {
+                if (j == 4) { ae[s] = a[s]; ax[s] = d[s]; }
+                else { ae[s] = M3DK_FMA(ae[s], eta, a[s]); ax[s] = M3DK_FMA(ax[s], eta, d[s]); }
+                a[s] = M3DK_FMA(a[s], eta, p[s]);
+            }
         }
     }
-    va = a; vb = b; dxa = ax; dxb = bx; dea = ae; deb = be;
+#pragma unroll
+    for (int s = 0; s < 4; ++s) { v[s] = a[s]; dx[s] = ax[s]; de[s] = ae[s]; }
 }
 
 // ---- element search (G11) ------------------------------------------------------------------------------------------
@@ -114,20 +106,61 @@ __device__ __forceinline__ int locate(const GridParams &g, double R, double Z) {
     return best == 0x7fffffff ? -1 : best;
 }
 
+// ---- fast element search: fp32 edge functions in bucket-local coordinates, conservative ---------------------------
+// Returns the element when the point is strictly inside a candidate by more than the fp32 error bound (then rule G11
+// yields the same element), otherwise -2: the caller falls back to the exact search `locate`.
+__device__ __forceinline__ FastRec ldrec(const FastRec *p) {
+    unsigned r[8];
+    asm("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "l"(p));
+    FastRec q;
+    q.x0 = __uint_as_float(r[0]); q.y0 = __uint_as_float(r[1]); q.x1 = __uint_as_float(r[2]);
+    q.y1 = __uint_as_float(r[3]); q.x2 = __uint_as_float(r[4]); q.y2 = __uint_as_float(r[5]);
+    q.id = (int)r[6]; q.next = (int)r[7];
+    return q;
+}
+
+// The asm loads are not volatile, so the compiler may hoist them above the range checks: every address is therefore
+// clamped into its table first and the checks only decide whether the loaded record is used.
+__device__ __forceinline__ int locate_fast(const FastGrid &g, double R, double Z) {
+    const double fx = (R - g.Rmin) * g.inv_hx, fz = (Z - g.Zmin) * g.inv_hz;
+    const bool inside = fx >= 0.0 && fx < (double)g.gx && fz >= 0.0 && fz < (double)g.gz;
+    const int ix = inside ? (int)fx : 0, iz = inside ? (int)fz : 0;
+    const float u = (float)(fx - (double)ix), v = (float)(fz - (double)iz);
+    FastRec r = ldrec(g.first + (size_t)(iz * g.gx + ix));
+    int found = -2;
+    bool open = inside;
+#pragma unroll 1
+    for (int it = 0; it < 4 && open; ++it) {
+        const float e0 = __fmul_rn(r.x1 - r.x0, v - r.y0) - __fmul_rn(r.y1 - r.y0, u - r.x0);
+        const float e1 = __fmul_rn(r.x2 - r.x1, v - r.y1) - __fmul_rn(r.y2 - r.y1, u - r.x1);
+        const float e2 = __fmul_rn(r.x0 - r.x2, v - r.y2) - __fmul_rn(r.y0 - r.y2, u - r.x2);
+        if (r.id >= 0 && e0 > kFastMargin && e1 > kFastMargin && e2 > kFastMargin) { found = r.id; open = false; }
+        else if (r.id < 0 || r.next < 0) open = false;
+        else r = ldrec(g.ovf + max(r.next, 0));
+    }
+    return found;
+}
+
+__device__ __forceinline__ int locate_any(const FieldParams &f, double R, double Z) {
+    const int e = locate_fast(f.fast, R, Z);
+    return e != -2 ? e : locate(f.grid, R, Z);
+}
+
 // ---- fields at (R, phi, Z) in element e -----------------------------------------------------
-// cph, sph = cos phi, sin phi; rinv = 1/R; cwt/swt = cos / sin(omega_k t).  NM: number of toroidal modes to evaluate.
+// cph, sph = cos phi, sin phi; rinv = 1/R; cwt/swt = cos / sin(omega_k t).  When all lanes of a warp pass the same e
+// every load below is a one-wavefront broadcast.
 __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double R, double Z, double cph, double sph,
                                             double rinv, const double *cwt, const double *swt, Fields &o) {
-    const double *tile = f.tiles + (size_t)e * f.tile_stride;
-    const double2 *t2 = reinterpret_cast<const double2 *>(tile);
-    const double2 h0 = ldc(t2), h1 = ldc(t2 + 1);
-    const double Rc = h0.x, Zc = h0.y, se = h1.x;
+    const double *tile = f.tiles + (size_t)max(e, 0) * f.tile_stride;   // clamped: the loads may be speculated
+    const Quad h = ldq(tile);
+    const double Rc = h.a, Zc = h.b, se = h.c;
     const double xi = (R - Rc) * se, eta = (Z - Zc) * se;
-    double v0, dx0, de0, v1, dx1, de1;
-    pair_vd(t2 + kTileHeader / 2, xi, eta, v0, dx0, de0, v1, dx1, de1);
-    o.psi_R = dx0 * se; o.psi_Z = de0 * se;
-    o.Bm = v1; o.Bm_R = dx1 * se; o.Bm_Z = de1 * se;
-    pair_v(t2 + (kTileHeader + kPair) / 2, xi, eta, o.F, o.kappa);
+    double v[4], dx[4], de[4];
+    quad_vd(tile + kTileHeader, xi, eta, v, dx, de);          // (psi0, |B|0, F0, kappa)
+    o.psi_R = dx[0] * se; o.psi_Z = de[0] * se;
+    o.Bm = v[1]; o.Bm_R = dx[1] * se; o.Bm_Z = de[1] * se;
+    o.F = v[2]; o.kappa = v[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) { o.E1[k] = 0.0; o.B1[k] = 0.0; o.gB[k] = 0.0; }
     o.dtB = 0.0; o.B1p = 0.0;
@@ -143,27 +176,24 @@ __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double 
         if (n < 0) sn = -sn;
         const double cth = cn * cwt[md] + sn * swt[md];      // cos(n phi - omega t)
         const double sth = sn * cwt[md] - cn * swt[md];      // sin(n phi - omega t)
-        const double2 *pm = t2 + (kTileHeader + kTileEq + kTileMode * md) / 2;
+        const double *pm = tile + kTileHeader + kTileEq + kTileMode * md;
         // Re[C e^{i th}] = Cr cos th - Ci sin th
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            double re, im;
-            pair_v(pm + q * M3DK_NCOEF, xi, eta, re, im);
-            o.E1[q] += re * cth - im * sth;
-        }
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            double re, im;
-            pair_v(pm + (3 + q) * M3DK_NCOEF, xi, eta, re, im);
-            o.B1[q] += re * cth - im * sth;
-        }
-        double re, reX, reE, im, imX, imE;
-        pair_vd(pm + 6 * M3DK_NCOEF, xi, eta, re, reX, reE, im, imX, imE);
+        quad_vd(pm, xi, eta, v, dx, de);                      // E_R, E_phi
+        o.E1[0] += v[0] * cth - v[1] * sth;
+        o.E1[1] += v[2] * cth - v[3] * sth;
+        quad_vd(pm + kQuad, xi, eta, v, dx, de);              // E_Z, B_R
+        o.E1[2] += v[0] * cth - v[1] * sth;
+        o.B1[0] += v[2] * cth - v[3] * sth;
+        quad_vd(pm + 2 * kQuad, xi, eta, v, dx, de);          // B_phi, B_Z
+        o.B1[1] += v[0] * cth - v[1] * sth;
+        o.B1[2] += v[2] * cth - v[3] * sth;
+        quad_vd(pm + 3 * kQuad, xi, eta, v, dx, de);          // B_par with gradient (slots 2, 3 are padding)
+        const double re = v[0], im = v[1];
         const double qd = re * sth + im * cth;               // -Im-part combination: d/dphi -> -n qd, d/dt -> omega qd
         o.B1p += re * cth - im * sth;
-        o.gB[0] += (reX * se) * cth - (imX * se) * sth;
+        o.gB[0] += (dx[0] * se) * cth - (dx[1] * se) * sth;
         o.gB[1] += -(double)n * qd * rinv;
-        o.gB[2] += (reE * se) * cth - (imE * se) * sth;
+        o.gB[2] += (de[0] * se) * cth - (de[1] * se) * sth;
         o.dtB += f.omega[md] * qd;
     }
 }
@@ -184,13 +214,17 @@ __device__ __forceinline__ double kappa_E(const PushParams &P, double Ekin, doub
 // state in: (x_l, v_{l-1/2}, mu, w_{l-1/2}) with e = element of x_l;  out: (x_{l+1}, v_{l+1/2}, w_{l+1/2}).
 struct Marker { double x, y, z, vx, vy, vz, mu, w; };
 
-__device__ __forceinline__ void step_marker(const PushParams &P, int e, Marker &s) {
-    // cylindrical map (G3)
-    const double R = sqrt(s.x * s.x + s.y * s.y);
-    const double rinv = 1.0 / R;
-    const double cph = s.x * rinv, sph = s.y * rinv;
-    Fields f;
-    eval_fields(P.f, e, R, s.z, cph, sph, rinv, P.cwt, P.swt, f);
+struct StepGeom { double R, rinv, cph, sph; };
+
+// cylindrical map (G3)
+__device__ __forceinline__ void step_geometry(const Marker &s, StepGeom &g) {
+    g.R = sqrt(s.x * s.x + s.y * s.y);
+    g.rinv = 1.0 / g.R;
+    g.cph = s.x * g.rinv; g.sph = s.y * g.rinv;
+}
+
+__device__ __forceinline__ void step_marker(const PushParams &P, const StepGeom &g, const Fields &f, Marker &s) {
+    const double rinv = g.rinv, cph = g.cph, sph = g.sph;
     // B0 = grad psi0 x grad phi + F0 grad phi (G4); E-dagger = -(mu/q) grad|B|0 (G2)
     const double BR = -f.psi_Z * rinv, BP = f.F * rinv, BZ = f.psi_R * rinv;
     const double muq = s.mu * P.inv_q;
@@ -233,8 +267,8 @@ __device__ __forceinline__ void step_marker(const PushParams &P, int e, Marker &
     s.vx = nvx; s.vy = nvy; s.vz = nvz;
 }
 
-__device__ __forceinline__ int locate_xyz(const GridParams &g, double x, double y, double z) {
-    return locate(g, sqrt(x * x + y * y), z);
+__device__ __forceinline__ int locate_xyz(const FieldParams &f, double x, double y, double z) {
+    return locate_any(f, sqrt(x * x + y * y), z);
 }
 
 }  // namespace m3dk

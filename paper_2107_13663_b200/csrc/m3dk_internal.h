@@ -15,22 +15,42 @@
 namespace m3dk {
 
 // ---- device data layout -------------------------------------------------------------------
-// Element tile, `tile_stride` doubles, 128-byte aligned:
-//   [0..15]   header: R_c, Z_c, s_e, 13 x pad
-//   [16..57]  pair A: (psi0_k, |B|0_k) k = 0..20   interleaved so that one 16-byte load feeds two Horner chains
-//   [58..99]  pair B: (F0_k, kappa_k)
-//   per mode m: 7 pairs (re_k, im_k) of E_R E_phi E_Z B_R B_phi B_Z B_par, 42 doubles each (294 per mode)
-constexpr int kTileHeader = 16;
-constexpr int kPair = 2 * M3DK_NCOEF;                 // 42
-constexpr int kTileEq = 2 * kPair;                    // 84
-constexpr int kTileMode = M3DK_N_PERT * kPair;        // 294
+// Element tile, `tile_stride` doubles, 128-byte aligned.  Four polynomials are interleaved coefficient by coefficient
+// ("quad"), so that one 32-byte load (LDG.E.256) feeds four independent Horner chains:
+//   [0..3]    header: R_c, Z_c, s_e, pad
+//   [4..87]   quad EQ: (psi0_k, |B|0_k, F0_k, kappa_k), k = 0..20
+//   per mode m, 4 quads of 84 doubles (336 per mode), (re, im) parts of the complex amplitudes:
+//     quad 0: (E_R re, E_R im, E_phi re, E_phi im)     quad 1: (E_Z re, E_Z im, B_R re, B_R im)
+//     quad 2: (B_phi re, B_phi im, B_Z re, B_Z im)     quad 3: (B_par re, B_par im, 0, 0)
+constexpr int kTileHeader = 4;
+constexpr int kQuad = 4 * M3DK_NCOEF;                 // 84
+constexpr int kTileEq = kQuad;                        // 84
+constexpr int kTileMode = 4 * kQuad;                  // 336
 inline int tile_stride_doubles(int n_modes) {
     int n = kTileHeader + kTileEq + kTileMode * n_modes;
     return (n + 15) / 16 * 16;
 }
-// Edge record of one element for the search, 16 doubles = one 128-byte line:
+// Edge record of one element for the exact search, 16 doubles = one 128-byte line:
 //   3 x (r_a, z_a, r_b - r_a, z_b - z_a), strict-interior tolerance, 3 x pad
 constexpr int kEdgeRec = 16;
+
+// Fast search grid (fp32, conservative): one 32-byte record per (bucket, candidate triangle):
+//   x0 y0 x1 y1 x2 y2  vertices in bucket-local units (bucket = [0,1)^2), all within [-kFastCmax+1, kFastCmax]
+//   id                  element index, -1 = "use the exact search for this bucket"
+//   next                index of the next candidate's record in the overflow array, -1 = none
+// A point whose three fp32 edge functions exceed kFastMargin is strictly inside that triangle in exact arithmetic
+// (error bound 720 * 2^-24 = 4.3e-5 for coordinates bounded by kFastCmax), so the exact rule G11 gives the same element.
+constexpr float kFastMargin = 1.0e-4f;
+constexpr double kFastCmax = 5.0;
+struct FastRec { float x0, y0, x1, y1, x2, y2; int id, next; };
+static_assert(sizeof(FastRec) == 32, "FastRec must be one 32-byte sector");
+
+struct FastGrid {
+    double Rmin, Zmin, inv_hx, inv_hz;
+    int gx, gz;
+    const FastRec *first;    // [gx*gz]
+    const FastRec *ovf;      // overflow records
+};
 
 struct GridParams {          // bucket grid of the element search
     double Rmin, Rmax, Zmin, Zmax, inv_hx, inv_hz;
@@ -48,6 +68,7 @@ struct FieldParams {
     int n_tor[M3DK_MAX_MODES];
     double omega[M3DK_MAX_MODES];
     GridParams grid;
+    FastGrid fast;
 };
 
 struct MarkerArrays {
@@ -64,6 +85,7 @@ struct PushParams {
     int f0kind;
     double f0T_inv, f0vc3, f0L0, f0dL2_inv, f0Bax;
     double cwt[M3DK_MAX_MODES], swt[M3DK_MAX_MODES];   // cos / sin (omega_k t_l) of this step
+    int *hist, *rank;        // fused sort histogram of the new keys (push_kernel<true>), else unused
 };
 
 struct SortBuffers {         // carved from the sort workspace
@@ -100,6 +122,7 @@ struct m3dk_ctx {
     double last_dt = 0.0;
     // sort workspace
     bool have_sortws = false;
+    bool hist_valid = false;     // sb.hist / sb.rank describe the keys of the current arrays (filled by the last push)
     m3dk::SortBuffers sb{};
     int *d_count = nullptr;      // small device scratch inside the fields workspace (lost counter etc.)
     // profiling (m3dk_set_profiling / m3dk_timing)
@@ -113,11 +136,11 @@ namespace m3dk {
 
 // launchers (defined in push.cu / sort.cu); all enqueue on ctx->stream and return cudaGetLastError()
 cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_id);
-cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t);
+cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t, bool with_hist);
 cudaError_t launch_eval_fields(m3dk_ctx *c, long n, const double *R, const double *phi, const double *Z, double t,
                                int *elem_out, double *out);
 cudaError_t launch_count_lost(m3dk_ctx *c, const MarkerArrays &a, long n, int *d_count);
-cudaError_t launch_sort(m3dk_ctx *c, const MarkerArrays &src, const MarkerArrays &dst, long n);
+cudaError_t launch_sort(m3dk_ctx *c, const MarkerArrays &src, const MarkerArrays &dst, long n, bool have_hist);
 cudaError_t fp64_probe(m3dk_ctx *c, double *tflops);
 
 size_t sort_workspace_bytes(long n, int n_elems);

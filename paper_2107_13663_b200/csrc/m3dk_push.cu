@@ -8,30 +8,76 @@ namespace m3dk {
 constexpr int kPushThreads = 128;
 
 // ---- element of every marker (particles_init / upload) ------------------------------------------------------------
-__global__ void __launch_bounds__(256) locate_kernel(GridParams g, MarkerArrays a, long n, int fill_id) {
+__global__ void __launch_bounds__(256) locate_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, long n,
+                                                     int fill_id) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    a.elem[i] = locate_xyz(g, a.x[i], a.y[i], a.z[i]);
+    a.elem[i] = locate_xyz(f, a.x[i], a.y[i], a.z[i]);
     if (fill_id) a.id[i] = (int)i;
+}
+
+// Warp-aggregated histogram with returned ranks: lanes with the same key elect a leader that does one atomic.
+__device__ __forceinline__ int hist_rank(int *hist, int key, bool on) {
+    const unsigned live = __ballot_sync(0xffffffffu, on);
+    int r = 0;
+    if (on) {
+        const unsigned peers = __match_any_sync(live, key);
+        const int lane = threadIdx.x & 31;
+        const int leader = __ffs(peers) - 1;
+        int base = 0;
+        if (lane == leader) base = atomicAdd(hist + key, __popc(peers));
+        base = __shfl_sync(peers, base, leader);
+        r = base + __popc(peers & ((1u << lane) - 1u));
+    }
+    return r;
 }
 
 // ---- generic push: one marker per thread, any marker order -----------------------------------------------------------
 // a1 load, a2 cylindrical map, a4-a6 tile fetch + Horner evaluation, a7 assemble, a8 Boris, a9 weight, a10 drift + store
 // and a3 for the NEW position (the element is cached for the next step and is the sort key).
-__global__ void __launch_bounds__(kPushThreads) push_generic_kernel(const __grid_constant__ PushParams P) {
+// The element loop makes the tile address warp-uniform: the lanes that share the leader's element evaluate together and
+// every coefficient load is a one-wavefront broadcast.  On an element-sorted marker stream a warp needs one or two
+// passes; on an unsorted stream up to 32 (the loop is still correct, only slower).
+template <bool kHist>
+__global__ void __launch_bounds__(kPushThreads) push_kernel(const __grid_constant__ PushParams P) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.n) return;
-    const int e = P.a.elem[i];
-    if (e < 0) return;  // lost markers are frozen (G12)
+    const bool valid = i < P.n;
+    const int e = valid ? P.a.elem[i] : -1;
+    const bool active = e >= 0;             // lost markers are frozen (G12)
     Marker s;
-    s.x = P.a.x[i]; s.y = P.a.y[i]; s.z = P.a.z[i];
-    s.vx = P.a.vx[i]; s.vy = P.a.vy[i]; s.vz = P.a.vz[i];
-    s.mu = P.a.mu[i]; s.w = P.a.w[i];
-    step_marker(P, e, s);
-    P.a.x[i] = s.x; P.a.y[i] = s.y; P.a.z[i] = s.z;
-    P.a.vx[i] = s.vx; P.a.vy[i] = s.vy; P.a.vz[i] = s.vz;
-    if (P.f.n_modes > 0) P.a.w[i] = s.w;
-    P.a.elem[i] = locate_xyz(P.f.grid, s.x, s.y, s.z);
+    if (active) {
+        s.x = P.a.x[i]; s.y = P.a.y[i]; s.z = P.a.z[i];
+        s.vx = P.a.vx[i]; s.vy = P.a.vy[i]; s.vz = P.a.vz[i];
+        s.mu = P.a.mu[i]; s.w = P.a.w[i];
+    } else {
+        s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
+    }
+    StepGeom gm;
+    step_geometry(s, gm);
+    Fields f;
+    // NB the compiler proves e == ke inside the branch, addresses the tile with the lane's own e and hoists the loads
+    // out of the loop (they run for inactive lanes too): the element used for addressing is clamped to a valid one.
+    const int es = max(e, 0);
+    unsigned todo = __ballot_sync(0xffffffffu, active);
+    while (todo) {
+        const int ke = __shfl_sync(0xffffffffu, es, __ffs(todo) - 1);
+        const bool mine = active && es == ke;
+        if (mine) eval_fields(P.f, ke, gm.R, s.z, gm.cph, gm.sph, gm.rinv, P.cwt, P.swt, f);
+        todo &= ~__ballot_sync(0xffffffffu, mine);
+    }
+    int ne = e;
+    if (active) {
+        step_marker(P, gm, f, s);
+        P.a.x[i] = s.x; P.a.y[i] = s.y; P.a.z[i] = s.z;
+        P.a.vx[i] = s.vx; P.a.vy[i] = s.vy; P.a.vz[i] = s.vz;
+        if (P.f.n_modes > 0) P.a.w[i] = s.w;
+        ne = locate_xyz(P.f, s.x, s.y, s.z);
+        P.a.elem[i] = ne;
+    }
+    if (kHist) {   // histogram of the NEW keys and each marker's rank inside its key: the sort then needs no key pass
+        const int r = hist_rank(P.hist, ne < 0 ? P.f.n_elems : ne, valid);
+        if (valid) P.rank[i] = r;
+    }
 }
 
 // ---- diagnostics ---------------------------------------------------------------------------------------------------
@@ -40,7 +86,7 @@ __global__ void __launch_bounds__(128) eval_fields_kernel(FieldParams f, long n,
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const double r = R[i], z = Z[i];
-    const int e = locate(f.grid, r, z);
+    const int e = locate_any(f, r, z);
     elem_out[i] = e;
     if (e < 0) return;
     double cwt[M3DK_MAX_MODES], swt[M3DK_MAX_MODES];
@@ -101,16 +147,23 @@ cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_
     if (n == 0) return cudaSuccess;
     const unsigned grid = (unsigned)((n + 255) / 256);
     c->kernel_launches += 1;
-    locate_kernel<<<grid, 256, 0, c->stream>>>(c->f.grid, a, n, fill_id ? 1 : 0);
+    locate_kernel<<<grid, 256, 0, c->stream>>>(c->f, a, n, fill_id ? 1 : 0);
     return cudaGetLastError();
 }
 
-cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t) {
+cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t, bool with_hist) {
     if (n == 0) return cudaSuccess;
-    const PushParams P = make_params(c, a, n, dt, t);
+    PushParams P = make_params(c, a, n, dt, t);
     const unsigned grid = (unsigned)((n + kPushThreads - 1) / kPushThreads);
     c->kernel_launches += 1;
-    push_generic_kernel<<<grid, kPushThreads, 0, c->stream>>>(P);
+    if (with_hist) {
+        P.hist = c->sb.hist; P.rank = c->sb.rank;
+        cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
+        if (e != cudaSuccess) return e;
+        push_kernel<true><<<grid, kPushThreads, 0, c->stream>>>(P);
+    } else {
+        push_kernel<false><<<grid, kPushThreads, 0, c->stream>>>(P);
+    }
     return cudaGetLastError();
 }
 

@@ -44,24 +44,50 @@ __global__ void __launch_bounds__(256) hist_rank_kernel(const int *__restrict__ 
     rank[i] = base + __popc(peers & ((1u << lane) - 1u));
 }
 
-// exclusive scan of hist[0..m) into offs[0..m], one block (m <= a few 1e5 bins: microseconds)
+// exclusive scan of hist[0..m) into offs[0..m] (offs[m] = total): one CTA, coalesced chunks of 1024 x 4 bins, warp
+// shuffles inside a chunk, a running carry across chunks (m is a few 1e5 bins: ~30 chunk iterations).
 __global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist, int m, int *__restrict__ offs) {
-    __shared__ int part[1024];
-    const int t = threadIdx.x, per = (m + 1023) / 1024;
-    const int b = t * per, e = min(b + per, m);
-    int s = 0;
-    for (int k = b; k < e; ++k) s += hist[k];
-    part[t] = s;
+    __shared__ int wsum[32];
+    __shared__ int carry_s;
+    const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+    if (t == 0) carry_s = 0;
     __syncthreads();
-    for (int o = 1; o < 1024; o <<= 1) {
-        int v = t >= o ? part[t - o] : 0;
+    for (int base = 0; base < m; base += 4096) {
+        const int k = base + 4 * t;
+        int v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) v[q] = k + q < m ? hist[k + q] : 0;
+        const int mine = v[0] + v[1] + v[2] + v[3];
+        int inc = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int u = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += u;
+        }
+        if (lane == 31) wsum[wid] = inc;
         __syncthreads();
-        part[t] += v;
+        if (wid == 0) {
+            int w = wsum[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int u = __shfl_up_sync(0xffffffffu, w, o);
+                if (lane >= o) w += u;
+            }
+            wsum[lane] = w;      // inclusive over warps
+        }
+        __syncthreads();
+        const int carry = carry_s;
+        int run = carry + (wid ? wsum[wid - 1] : 0) + inc - mine;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (k + q < m) offs[k + q] = run;
+            run += v[q];
+        }
+        __syncthreads();
+        if (t == 1023) carry_s = carry + wsum[31];
         __syncthreads();
     }
-    int run = t ? part[t - 1] : 0;
-    for (int k = b; k < e; ++k) { offs[k] = run; run += hist[k]; }
-    if (t == 1023) offs[m] = part[1023];
+    if (t == 0) offs[m] = carry_s;
 }
 
 __global__ void __launch_bounds__(256) scatter_kernel(MarkerArrays s, MarkerArrays d, long n, int n_elems,
@@ -76,14 +102,17 @@ __global__ void __launch_bounds__(256) scatter_kernel(MarkerArrays s, MarkerArra
     d.elem[j] = e; d.id[j] = s.id[i];
 }
 
-cudaError_t launch_sort(m3dk_ctx *c, const MarkerArrays &src, const MarkerArrays &dst, long n) {
+cudaError_t launch_sort(m3dk_ctx *c, const MarkerArrays &src, const MarkerArrays &dst, long n, bool have_hist) {
     if (n == 0) return cudaSuccess;
     const int m = c->f.n_elems + 1;
-    cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)m * sizeof(int), c->stream);
-    if (e != cudaSuccess) return e;
     const unsigned grid = (unsigned)((n + 255) / 256);
-    c->kernel_launches += 3;
-    hist_rank_kernel<<<grid, 256, 0, c->stream>>>(src.elem, n, c->f.n_elems, c->sb.hist, c->sb.rank);
+    if (!have_hist) {   // otherwise the push kernel that produced these keys has filled hist and rank already
+        cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)m * sizeof(int), c->stream);
+        if (e != cudaSuccess) return e;
+        c->kernel_launches += 1;
+        hist_rank_kernel<<<grid, 256, 0, c->stream>>>(src.elem, n, c->f.n_elems, c->sb.hist, c->sb.rank);
+    }
+    c->kernel_launches += 2;
     scan_kernel<<<1, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs);
     scatter_kernel<<<grid, 256, 0, c->stream>>>(src, dst, n, c->f.n_elems, c->sb.offs, c->sb.rank);
     return cudaGetLastError();
