@@ -66,6 +66,8 @@ extern "C" int m3dk_create(m3dk_ctx **out, int device, void *stream) {
     ctx = new m3dk_ctx();
     ctx->device = device;
     ctx->stream = static_cast<cudaStream_t>(stream);
+    if (cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || ctx->sm_count < 1)
+        ctx->sm_count = 148;
     *out = ctx;
     return M3DK_OK;
 }
@@ -354,6 +356,7 @@ extern "C" int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, 
     ctx->steps_since_sort = ctx->sort_interval;   // the first push sorts first when sorting is on
     ctx->have_markers = true;
     ctx->hist_valid = false;
+    ctx->items_valid = false;
     if (ctx->have_sortws && ctx->sb.bytes) {      // an older workspace may be too small for the new n
         if (sort_workspace_bytes(n, ctx->f.n_elems) > ctx->sb.bytes) ctx->have_sortws = false;
     }
@@ -383,6 +386,7 @@ static int bind_sort_ws(m3dk_ctx *ctx, void *ws, size_t bytes, const char *who) 
         return fail(ctx, M3DK_EWORKSPACE, std::string(who) + ": workspace NULL, misaligned or smaller than m3dk_sort_workspace_bytes");
     carve_sort_workspace(ws, ctx->n, ctx->f.n_elems, &ctx->sb);
     ctx->hist_valid = false;
+    ctx->items_valid = false;
     ctx->sb.bytes = bytes;
     ctx->have_sortws = true;
     return M3DK_OK;
@@ -403,6 +407,7 @@ static int sort_flip(m3dk_ctx *ctx) {   // sort current -> other, other becomes 
         CU(launch_sort(ctx, src, dst, ctx->n, ctx->hist_valid), "sort kernels");
     }
     ctx->hist_valid = false;
+    ctx->items_valid = true;     // the arrays that are current now are sorted and sb.items cut them by element
     ctx->cur ^= 1;
     ctx->n_sorts++;
     ctx->steps_since_sort = 0;
@@ -456,8 +461,9 @@ extern "C" int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt) {
             // when the next step starts with a sort, this push also histograms its new keys (a11 fused into a10)
             const bool with_hist = ctx->sort_interval > 0 && ctx->steps_since_sort + 1 >= ctx->sort_interval && ctx->n > 0;
             EvScope ev(ctx, &ctx->ev_push);
-            CU(launch_push(ctx, cur_arrays(ctx), ctx->n, dt, t, with_hist), "push kernel");
+            CU(launch_push(ctx, cur_arrays(ctx), ctx->n, dt, t, with_hist, ctx->items_valid), "push kernel");
             ctx->hist_valid = with_hist;
+            ctx->items_valid = false;    // the markers have moved: the order is stale until the next sort
         }
         ctx->steps_done++;
         ctx->steps_since_sort++;
@@ -497,6 +503,7 @@ extern "C" int m3dk_particles_upload(m3dk_ctx *ctx, const double *hx, const doub
     for (int k = 0; k < 8; ++k) CU(cudaMemcpyAsync(dd[k], hs[k], nd, cudaMemcpyHostToDevice, ctx->stream), "upload markers");
     ctx->cur = 0;
     ctx->hist_valid = false;
+    ctx->items_valid = false;
     ctx->steps_since_sort = ctx->sort_interval;
     CU(launch_locate(ctx, ctx->user, ctx->n, true), "locate kernel");
     return M3DK_OK;

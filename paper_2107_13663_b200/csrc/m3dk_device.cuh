@@ -37,37 +37,51 @@ __device__ __forceinline__ Quad ldq(const double *p) {
 // c[4 k + s]: coefficient k of slot s.  Horner in xi inside a row, Horner in eta across rows; value, d/dxi, d/deta of
 // all four slots: 38 FMA per slot.  Callers ignore the outputs they do not need; after full unrolling the unused
 // chains are dead code and disappear (value only: 20 FMA per slot).
-__device__ __forceinline__ void quad_vd(const double *__restrict__ c, double xi, double eta, double (&v)[4],
-                                        double (&dx)[4], double (&de)[4]) {
+// R markers per thread share every coefficient load (all R sit in the same element): one 32-byte load feeds up to
+// 8 R FMAs, which is what takes the L1 -> register-file path (128 B/clk/SM) off the critical path.
+template <int R>
+__device__ __forceinline__ void quad_vd(const double *__restrict__ c, const double (&xi)[R], const double (&eta)[R],
+                                        double (&v)[R][4], double (&dx)[R][4], double (&de)[R][4]) {
     constexpr int kRow[6] = {0, 6, 11, 15, 18, 20};
-    double a[4], ax[4], ae[4];
+    double a[R][4], ax[R][4], ae[R][4];
 #pragma unroll
     for (int j = 5; j >= 0; --j) {
         const int L = 6 - j;
         const Quad t = ldq(c + 4 * (kRow[j] + L - 1));
-        double p[4] = {t.a, t.b, t.c, t.d}, d[4] = {0.0, 0.0, 0.0, 0.0};
+        double p[R][4], d[R][4];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            p[r][0] = t.a; p[r][1] = t.b; p[r][2] = t.c; p[r][3] = t.d;
+            d[r][0] = d[r][1] = d[r][2] = d[r][3] = 0.0;
+        }
 #pragma unroll
         for (int i = L - 2; i >= 0; --i) {
             const Quad u = ldq(c + 4 * (kRow[j] + i));
             const double uu[4] = {u.a, u.b, u.c, u.d};
 #pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                d[s] = (i == L - 2) ? p[s] : M3DK_FMA(d[s], xi, p[s]);
-                p[s] = M3DK_FMA(p[s], xi, uu[s]);
-            }
+            for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    d[r][s] = (i == L - 2) ? p[r][s] : M3DK_FMA(d[r][s], xi[r], p[r][s]);
+                    p[r][s] = M3DK_FMA(p[r][s], xi[r], uu[s]);
+                }
         }
 #pragma unroll
-        for (int s = 0; s < 4; ++s) {
-            if (j == 5) { a[s] = p[s]; ax[s] = 0.0; ae[s] = 0.0; }
-            else {
-                if (j == 4) { ae[s] = a[s]; ax[s] = d[s]; }
-                else { ae[s] = M3DK_FMA(ae[s], eta, a[s]); ax[s] = M3DK_FMA(ax[s], eta, d[s]); }
-                a[s] = M3DK_FMA(a[s], eta, p[s]);
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                if (j == 5) { a[r][s] = p[r][s]; ax[r][s] = 0.0; ae[r][s] = 0.0; }
+                else {
+                    if (j == 4) { ae[r][s] = a[r][s]; ax[r][s] = d[r][s]; }
+                    else { ae[r][s] = M3DK_FMA(ae[r][s], eta[r], a[r][s]); ax[r][s] = M3DK_FMA(ax[r][s], eta[r], d[r][s]); }
+                    a[r][s] = M3DK_FMA(a[r][s], eta[r], p[r][s]);
+                }
             }
-        }
     }
 #pragma unroll
-    for (int s = 0; s < 4; ++s) { v[s] = a[s]; dx[s] = ax[s]; de[s] = ae[s]; }
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int s = 0; s < 4; ++s) { v[r][s] = a[r][s]; dx[r][s] = ax[r][s]; de[r][s] = ae[r][s]; }
 }
 
 // ---- element search (G11) ------------------------------------------------------------------------------------------
@@ -86,7 +100,7 @@ __device__ __forceinline__ void edge_fn(const double *__restrict__ rec, double R
 // Two phases over the bucket's candidate list (a superset of every element touching the bucket, priority order):
 // a candidate that contains the point strictly (all edge functions above its tolerance) is the only one that can
 // contain it, so it is returned at once; otherwise (the point is within rounding of an edge) take the minimum index.
-__device__ __forceinline__ int locate(const GridParams &g, double R, double Z) {
+__device__ __noinline__ int locate(const GridParams &g, double R, double Z) {
     if (!(R >= g.Rmin && R <= g.Rmax && Z >= g.Zmin && Z <= g.Zmax)) return -1;
     int ix = (int)((R - g.Rmin) * g.inv_hx), iz = (int)((Z - g.Zmin) * g.inv_hz);
     ix = min(max(ix, 0), g.gx - 1);
@@ -142,6 +156,14 @@ __device__ __forceinline__ int locate_fast(const FastGrid &g, double R, double Z
     return found;
 }
 
+// first record of the bucket of (R, Z): one line into L1 (the search itself runs later)
+__device__ __forceinline__ void locate_prefetch(const FastGrid &g, double R, double Z) {
+    const double fx = (R - g.Rmin) * g.inv_hx, fz = (Z - g.Zmin) * g.inv_hz;
+    const bool inside = fx >= 0.0 && fx < (double)g.gx && fz >= 0.0 && fz < (double)g.gz;
+    const int ix = inside ? (int)fx : 0, iz = inside ? (int)fz : 0;
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(g.first + (size_t)(iz * g.gx + ix)));
+}
+
 __device__ __forceinline__ int locate_any(const FieldParams &f, double R, double Z) {
     const int e = locate_fast(f.fast, R, Z);
     return e != -2 ? e : locate(f.grid, R, Z);
@@ -155,9 +177,10 @@ __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double 
     const double *tile = f.tiles + (size_t)max(e, 0) * f.tile_stride;   // clamped: the loads may be speculated
     const Quad h = ldq(tile);
     const double Rc = h.a, Zc = h.b, se = h.c;
-    const double xi = (R - Rc) * se, eta = (Z - Zc) * se;
-    double v[4], dx[4], de[4];
-    quad_vd(tile + kTileHeader, xi, eta, v, dx, de);          // (psi0, |B|0, F0, kappa)
+    const double xi1[1] = {(R - Rc) * se}, eta1[1] = {(Z - Zc) * se};
+    double vv[1][4], dxx[1][4], dee[1][4];
+    double (&v)[4] = vv[0], (&dx)[4] = dxx[0], (&de)[4] = dee[0];
+    quad_vd<1>(tile + kTileHeader, xi1, eta1, vv, dxx, dee);  // (psi0, |B|0, F0, kappa)
     o.psi_R = dx[0] * se; o.psi_Z = de[0] * se;
     o.Bm = v[1]; o.Bm_R = dx[1] * se; o.Bm_Z = de[1] * se;
     o.F = v[2]; o.kappa = v[3];
@@ -178,16 +201,16 @@ __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double 
         const double sth = sn * cwt[md] - cn * swt[md];      // sin(n phi - omega t)
         const double *pm = tile + kTileHeader + kTileEq + kTileMode * md;
         // Re[C e^{i th}] = Cr cos th - Ci sin th
-        quad_vd(pm, xi, eta, v, dx, de);                      // E_R, E_phi
+        quad_vd<1>(pm, xi1, eta1, vv, dxx, dee);                     // E_R, E_phi
         o.E1[0] += v[0] * cth - v[1] * sth;
         o.E1[1] += v[2] * cth - v[3] * sth;
-        quad_vd(pm + kQuad, xi, eta, v, dx, de);              // E_Z, B_R
+        quad_vd<1>(pm + kQuad, xi1, eta1, vv, dxx, dee);             // E_Z, B_R
         o.E1[2] += v[0] * cth - v[1] * sth;
         o.B1[0] += v[2] * cth - v[3] * sth;
-        quad_vd(pm + 2 * kQuad, xi, eta, v, dx, de);          // B_phi, B_Z
+        quad_vd<1>(pm + 2 * kQuad, xi1, eta1, vv, dxx, dee);         // B_phi, B_Z
         o.B1[1] += v[0] * cth - v[1] * sth;
         o.B1[2] += v[2] * cth - v[3] * sth;
-        quad_vd(pm + 3 * kQuad, xi, eta, v, dx, de);          // B_par with gradient (slots 2, 3 are padding)
+        quad_vd<1>(pm + 3 * kQuad, xi1, eta1, vv, dxx, dee);         // B_par with gradient (slots 2, 3 are padding)
         const double re = v[0], im = v[1];
         const double qd = re * sth + im * cth;               // -Im-part combination: d/dphi -> -n qd, d/dt -> omega qd
         o.B1p += re * cth - im * sth;
@@ -201,11 +224,12 @@ __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double 
 // d ln f0 / dE at fixed (P_phi, mu) (G7)
 __device__ __forceinline__ double kappa_E(const PushParams &P, double Ekin, double mu) {
     if (P.f0kind == M3DK_F0_MAXWELLIAN) return -P.f0T_inv;
-    const double v = sqrt(2.0 * Ekin / P.m);
-    double kE = -3.0 * v / (P.m * (v * v * v + P.f0vc3));
+    const double v = __dsqrt_rn(__ddiv_rn(__dmul_rn(2.0, Ekin), P.m));
+    const double v3 = __dmul_rn(__dmul_rn(v, v), v);
+    double kE = __ddiv_rn(__dmul_rn(-3.0, v), __dmul_rn(P.m, __dadd_rn(v3, P.f0vc3)));
     if (P.f0kind == M3DK_F0_BEAM_PITCH) {
-        const double Lam = mu * P.f0Bax / Ekin;
-        kE += 2.0 * (Lam - P.f0L0) * Lam * P.f0dL2_inv / Ekin;
+        const double Lam = __ddiv_rn(__dmul_rn(mu, P.f0Bax), Ekin);
+        kE = __dadd_rn(kE, __ddiv_rn(__dmul_rn(__dmul_rn(__dmul_rn(2.0, __dsub_rn(Lam, P.f0L0)), Lam), P.f0dL2_inv), Ekin));
     }
     return kE;
 }
@@ -218,57 +242,114 @@ struct StepGeom { double R, rinv, cph, sph; };
 
 // cylindrical map (G3)
 __device__ __forceinline__ void step_geometry(const Marker &s, StepGeom &g) {
-    g.R = sqrt(s.x * s.x + s.y * s.y);
-    g.rinv = 1.0 / g.R;
-    g.cph = s.x * g.rinv; g.sph = s.y * g.rinv;
+    g.R = __dsqrt_rn(M3DK_FMA(s.x, s.x, __dmul_rn(s.y, s.y)));
+    g.rinv = __ddiv_rn(1.0, g.R);
+    g.cph = __dmul_rn(s.x, g.rinv); g.sph = __dmul_rn(s.y, g.rinv);
 }
 
-__device__ __forceinline__ void step_marker(const PushParams &P, const StepGeom &g, const Fields &f, Marker &s) {
+// Equilibrium fields of one marker and the weights with which the perturbed fields enter dw/dt.
+struct EqOut { double psi_R, psi_Z, Bm, Bm_R, Bm_Z, F, kappa; };
+struct PertW { double aER, aEP, aEZ, bBR, bBZ, gR, gP, gZ, dT; };
+
+// Phase A of a step, after the equilibrium quad: Eq. (6) (Boris) and Eq. (5) (drift) on s.{x..vz}; then, with modes,
+// the linear delta-f equation (Eqs. 8-13 at (x_l, v_l), v_l = (v_{l-1/2} + v_{l+1/2}) / 2) is written as
+//   dw/dt = aER E1_R + aEP E1_phi + aEZ E1_Z + bBR B1_R + bBZ B1_Z + gR dB1par/dR + gP (1/R) dB1par/dphi
+//           + gZ dB1par/dZ + dT dB1par/dt
+// (it is linear in the perturbed fields; B1_phi does not enter), so that the perturbed polynomials can be folded into
+// one scalar per marker as they are evaluated (phase B) instead of being kept in registers:
+//   K = kappa/q, G = F/|B0|, b = B0/|B0|, v_par = v_l . b
+//   Eq. (12)+(10): dP/dt = q (dX_1 . grad psi0) + F_par1 G, dX_1 = E1 x B0 / B0^2 + v_par B1 / |B0|
+//   Eq. (13) x m (G5): F_par1 = q E1 . b - mu b . grad B1par;  Eq. (11) (G6): dE/dt = q v_l . E1 + mu dB1par/dt
+//   Eqs. (8)-(9), (1 - w) -> 1: dw/dt = -(K dP/dt + kE dE/dt)
+// Every operation below is written out (DM/DA/DS/M3DK_FMA: no contraction left to the compiler), so that every kernel
+// that inlines this code produces the same bits for the same marker (pin P13: results do not depend on the order).
+#define DM(a, b) __dmul_rn((a), (b))
+#define DA(a, b) __dadd_rn((a), (b))
+#define DS(a, b) __dsub_rn((a), (b))
+__device__ __forceinline__ void push_eq(const PushParams &P, const StepGeom &g, const EqOut &f, Marker &s, PertW &W) {
     const double rinv = g.rinv, cph = g.cph, sph = g.sph;
     // B0 = grad psi0 x grad phi + F0 grad phi (G4); E-dagger = -(mu/q) grad|B|0 (G2)
-    const double BR = -f.psi_Z * rinv, BP = f.F * rinv, BZ = f.psi_R * rinv;
-    const double muq = s.mu * P.inv_q;
-    const double ER = -muq * f.Bm_R, EZ = -muq * f.Bm_Z;
-    const double Bx = BR * cph - BP * sph, By = BR * sph + BP * cph, Bz = BZ;
-    const double Ex = ER * cph, Ey = ER * sph, Ez = EZ;
+    const double BR = -DM(f.psi_Z, rinv), BP = DM(f.F, rinv), BZ = DM(f.psi_R, rinv);
+    const double muq = DM(s.mu, P.inv_q);
+    const double ER = -DM(muq, f.Bm_R), EZ = -DM(muq, f.Bm_Z);
+    const double Bx = M3DK_FMA(BR, cph, -DM(BP, sph)), By = M3DK_FMA(BR, sph, DM(BP, cph)), Bz = BZ;
+    const double Ex = DM(ER, cph), Ey = DM(ER, sph), Ez = EZ;
     // Eq. (6) in the explicit Boris form: half kick, rotation t = h B, s = 2 t / (1 + t^2), half kick
     const double h = P.h;
-    const double ux = s.vx + h * Ex, uy = s.vy + h * Ey, uz = s.vz + h * Ez;
-    const double tx = h * Bx, ty = h * By, tz = h * Bz;
-    const double sc = 2.0 / (1.0 + (tx * tx + ty * ty + tz * tz));
-    const double px = ux + (uy * tz - uz * ty), py = uy + (uz * tx - ux * tz), pz = uz + (ux * ty - uy * tx);
-    const double wx = ux + sc * (py * tz - pz * ty), wy = uy + sc * (pz * tx - px * tz), wz = uz + sc * (px * ty - py * tx);
-    const double nvx = wx + h * Ex, nvy = wy + h * Ey, nvz = wz + h * Ez;
-    // weight, Eqs. (8)-(13) at (x_l, v_l), v_l = (v_{l-1/2} + v_{l+1/2}) / 2; skipped without modes
+    const double ux = M3DK_FMA(h, Ex, s.vx), uy = M3DK_FMA(h, Ey, s.vy), uz = M3DK_FMA(h, Ez, s.vz);
+    const double tx = DM(h, Bx), ty = DM(h, By), tz = DM(h, Bz);
+    const double sc = __ddiv_rn(2.0, DA(1.0, M3DK_FMA(tx, tx, M3DK_FMA(ty, ty, DM(tz, tz)))));
+    const double px = DA(ux, M3DK_FMA(uy, tz, -DM(uz, ty))), py = DA(uy, M3DK_FMA(uz, tx, -DM(ux, tz))),
+                 pz = DA(uz, M3DK_FMA(ux, ty, -DM(uy, tx)));
+    const double wx = M3DK_FMA(sc, M3DK_FMA(py, tz, -DM(pz, ty)), ux), wy = M3DK_FMA(sc, M3DK_FMA(pz, tx, -DM(px, tz)), uy),
+                 wz = M3DK_FMA(sc, M3DK_FMA(px, ty, -DM(py, tx)), uz);
+    const double nvx = M3DK_FMA(h, Ex, wx), nvy = M3DK_FMA(h, Ey, wy), nvz = M3DK_FMA(h, Ez, wz);
     if (P.f.n_modes > 0) {
-        const double vlx = 0.5 * (s.vx + nvx), vly = 0.5 * (s.vy + nvy), vlz = 0.5 * (s.vz + nvz);
-        const double vR = vlx * cph + vly * sph, vP = vly * cph - vlx * sph, vZ = vlz;
-        const double B2 = BR * BR + BP * BP + BZ * BZ;
-        const double binv = 1.0 / sqrt(B2);
-        const double bR = BR * binv, bP = BP * binv, bZ = BZ * binv;
-        const double vpar = vR * bR + vP * bP + vZ * bZ;
-        // Eq. (12): (dX/dt)_1 = E1 x B0 / B0^2 + v_par B1 / B0 ; only its (R, Z) components meet grad psi0
-        const double cR = f.E1[1] * BZ - f.E1[2] * BP, cZ = f.E1[0] * BP - f.E1[1] * BR;
-        const double b2inv = binv * binv;
-        const double dXR = cR * b2inv + vpar * f.B1[0] * binv, dXZ = cZ * b2inv + vpar * f.B1[2] * binv;
-        // Eq. (13) x m (G5)
-        const double Fpar = P.q * (f.E1[0] * bR + f.E1[1] * bP + f.E1[2] * bZ) - s.mu * (bR * f.gB[0] + bP * f.gB[1] + bZ * f.gB[2]);
-        // Eq. (10) (G5), Eq. (11) (G6)
-        const double dP = P.q * (dXR * f.psi_R + dXZ * f.psi_Z) + Fpar * f.F * binv;
-        const double dE = P.q * (vR * f.E1[0] + vP * f.E1[1] + vZ * f.E1[2]) + s.mu * f.dtB;
-        const double Ekin = 0.5 * P.m * (vlx * vlx + vly * vly + vlz * vlz) + s.mu * f.Bm;
+        const double vlx = DM(0.5, DA(s.vx, nvx)), vly = DM(0.5, DA(s.vy, nvy)), vlz = DM(0.5, DA(s.vz, nvz));
+        const double vR = M3DK_FMA(vlx, cph, DM(vly, sph)), vP = M3DK_FMA(vly, cph, -DM(vlx, sph)), vZ = vlz;
+        const double B2 = M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, DM(BZ, BZ)));
+        const double binv = __ddiv_rn(1.0, __dsqrt_rn(B2));
+        const double b2inv = DM(binv, binv);
+        const double bR = DM(BR, binv), bP = DM(BP, binv), bZ = DM(BZ, binv);
+        const double vpar = M3DK_FMA(vR, bR, M3DK_FMA(vP, bP, DM(vZ, bZ)));
+        const double v2 = M3DK_FMA(vlx, vlx, M3DK_FMA(vly, vly, DM(vlz, vlz)));
+        const double Ekin = M3DK_FMA(DM(0.5, P.m), v2, DM(s.mu, f.Bm));
         const double kE = kappa_E(P, Ekin, s.mu);
-        // Eqs. (8)-(9) with (1 - w) -> 1; explicit midpoint on the staggered grid (G9)
-        const double wdot = -((f.kappa * P.inv_q) * dP + kE * dE);
-        s.w = s.w + P.dt * wdot;
+        const double K = DM(f.kappa, P.inv_q), G = DM(f.F, binv);
+        const double Kq = DM(K, P.q), kEq = DM(kE, P.q);
+        W.aER = -M3DK_FMA(Kq, M3DK_FMA(DM(f.psi_Z, BP), b2inv, DM(bR, G)), DM(kEq, vR));
+        W.aEP = -M3DK_FMA(Kq, M3DK_FMA(M3DK_FMA(f.psi_R, BZ, -DM(f.psi_Z, BR)), b2inv, DM(bP, G)), DM(kEq, vP));
+        W.aEZ = -M3DK_FMA(Kq, M3DK_FMA(-DM(f.psi_R, BP), b2inv, DM(bZ, G)), DM(kEq, vZ));
+        const double Kv = -DM(DM(Kq, vpar), binv);
+        W.bBR = DM(Kv, f.psi_R);
+        W.bBZ = DM(Kv, f.psi_Z);
+        const double Kg = DM(DM(K, s.mu), G);
+        W.gR = DM(Kg, bR); W.gP = DM(Kg, bP); W.gZ = DM(Kg, bZ);
+        W.dT = -DM(kE, s.mu);
     }
     // Eq. (5)
-    s.x = s.x + P.dt * nvx; s.y = s.y + P.dt * nvy; s.z = s.z + P.dt * nvz;
+    s.x = M3DK_FMA(P.dt, nvx, s.x); s.y = M3DK_FMA(P.dt, nvy, s.y); s.z = M3DK_FMA(P.dt, nvz, s.z);
     s.vx = nvx; s.vy = nvy; s.vz = nvz;
 }
 
+// cos / sin of (n phi - omega t): exp(i n phi) by complex powers of (cos phi + i sin phi), exp(-i omega t) from the host
+__device__ __forceinline__ void mode_phase(int n, double cph, double sph, double cwt, double swt, double &cth,
+                                           double &sth) {
+    double cn = 1.0, sn = 0.0;
+    for (int k = 0; k < abs(n); ++k) {
+        const double c2 = M3DK_FMA(cn, cph, -__dmul_rn(sn, sph));
+        sn = M3DK_FMA(cn, sph, __dmul_rn(sn, cph));
+        cn = c2;
+    }
+    if (n < 0) sn = -sn;
+    cth = M3DK_FMA(cn, cwt, __dmul_rn(sn, swt));
+    sth = M3DK_FMA(sn, cwt, -__dmul_rn(cn, swt));
+}
+
+// Phase B: fold quad Q of a mode into dw/dt.  Re[C e^{i th}] = Cr cos th - Ci sin th; every operation is written out
+// (no contraction left to the compiler) so that all kernels that call this produce the same bits.
+__device__ __forceinline__ double re_part(double cr, double ci, double cth, double sth) {
+    return M3DK_FMA(cr, cth, -__dmul_rn(ci, sth));
+}
+// value-only quad: two complex amplitudes (v0 + i v1), (v2 + i v3) with weights wa, wb
+__device__ __forceinline__ double pert_fold_v(double wsum, const double (&v)[4], double wa, double wb, double cth,
+                                              double sth) {
+    wsum = M3DK_FMA(wa, re_part(v[0], v[1], cth, sth), wsum);
+    return M3DK_FMA(wb, re_part(v[2], v[3], cth, sth), wsum);
+}
+// B_par quad: gradient and time derivative; d/dphi -> -n qd, d/dt -> omega qd
+__device__ __forceinline__ double pert_fold_par(double wsum, const double (&v)[4], const double (&dx)[4],
+                                                const double (&de)[4], const PertW &W, double cth, double sth, double se,
+                                                double n_rinv, double omega) {
+    const double qd = M3DK_FMA(v[0], sth, __dmul_rn(v[1], cth));
+    wsum = M3DK_FMA(W.gR, re_part(__dmul_rn(dx[0], se), __dmul_rn(dx[1], se), cth, sth), wsum);
+    wsum = M3DK_FMA(W.gP, -__dmul_rn(n_rinv, qd), wsum);
+    wsum = M3DK_FMA(W.gZ, re_part(__dmul_rn(de[0], se), __dmul_rn(de[1], se), cth, sth), wsum);
+    return M3DK_FMA(W.dT, __dmul_rn(omega, qd), wsum);
+}
+
 __device__ __forceinline__ int locate_xyz(const FieldParams &f, double x, double y, double z) {
-    return locate_any(f, sqrt(x * x + y * y), z);
+    return locate_any(f, __dsqrt_rn(M3DK_FMA(x, x, __dmul_rn(y, y))), z);
 }
 
 }  // namespace m3dk

@@ -85,14 +85,25 @@ struct PushParams {
     int f0kind;
     double f0T_inv, f0vc3, f0L0, f0dL2_inv, f0Bax;
     double cwt[M3DK_MAX_MODES], swt[M3DK_MAX_MODES];   // cos / sin (omega_k t_l) of this step
-    int *hist, *rank;        // fused sort histogram of the new keys (push_kernel<true>), else unused
+    int *hist, *rank;        // fused sort histogram of the new keys (kHist kernels), else unused
+    const int4 *items;       // work items of the element-ordered kernel: (element, first slot, count, -)
+    const int *n_items;      // device: number of items
+    int *item_counter;       // device: next item to hand out (zeroed before the launch)
 };
+
+#ifndef M3DK_ITEM_R
+#define M3DK_ITEM_R 2
+#endif
+constexpr int kItemR = M3DK_ITEM_R;              // markers per lane in the element-ordered push
+constexpr int kItemMarkers = 32 * kItemR;        // markers per work item
 
 struct SortBuffers {         // carved from the sort workspace
     MarkerArrays alt;        // second set of marker arrays (ping-pong partner of the caller's)
     int *rank;               // [n]
     int *hist;               // [n_elems + 2]
     int *offs;               // [n_elems + 2]
+    int *ioffs;              // [n_elems + 2] first work item of each element; ioffs[n_elems + 1] = number of items
+    int4 *items;             // [n / kItemMarkers + n_elems + 2]
     size_t bytes;
 };
 
@@ -100,6 +111,7 @@ struct SortBuffers {         // carved from the sort workspace
 
 struct m3dk_ctx {
     int device = 0;
+    int sm_count = 148;
     cudaStream_t stream = nullptr;
     std::string err;
     // fields
@@ -122,6 +134,7 @@ struct m3dk_ctx {
     double last_dt = 0.0;
     // sort workspace
     bool have_sortws = false;
+    bool items_valid = false;    // sb.items cut the CURRENT arrays, which are sorted by element (set by a sort, cleared by a push)
     bool hist_valid = false;     // sb.hist / sb.rank describe the keys of the current arrays (filled by the last push)
     m3dk::SortBuffers sb{};
     int *d_count = nullptr;      // small device scratch inside the fields workspace (lost counter etc.)
@@ -136,7 +149,7 @@ namespace m3dk {
 
 // launchers (defined in push.cu / sort.cu); all enqueue on ctx->stream and return cudaGetLastError()
 cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_id);
-cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t, bool with_hist);
+cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t, bool with_hist, bool use_items);
 cudaError_t launch_eval_fields(m3dk_ctx *c, long n, const double *R, const double *phi, const double *Z, double t,
                                int *elem_out, double *out);
 cudaError_t launch_count_lost(m3dk_ctx *c, const MarkerArrays &a, long n, int *d_count);

@@ -5,7 +5,13 @@
 
 namespace m3dk {
 
-constexpr int kPushThreads = 128;
+#ifndef M3DK_PUSH_THREADS
+#define M3DK_PUSH_THREADS 128
+#endif
+#ifndef M3DK_PUSH_MINBLOCKS
+#define M3DK_PUSH_MINBLOCKS 4
+#endif
+constexpr int kPushThreads = M3DK_PUSH_THREADS;
 
 // ---- element of every marker (particles_init / upload) ------------------------------------------------------------
 __global__ void __launch_bounds__(256) locate_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, long n,
@@ -32,51 +38,183 @@ __device__ __forceinline__ int hist_rank(int *hist, int key, bool on) {
     return r;
 }
 
-// ---- generic push: one marker per thread, any marker order -----------------------------------------------------------
-// a1 load, a2 cylindrical map, a4-a6 tile fetch + Horner evaluation, a7 assemble, a8 Boris, a9 weight, a10 drift + store
-// and a3 for the NEW position (the element is cached for the next step and is the sort key).
-// The element loop makes the tile address warp-uniform: the lanes that share the leader's element evaluate together and
-// every coefficient load is a one-wavefront broadcast.  On an element-sorted marker stream a warp needs one or two
-// passes; on an unsorted stream up to 32 (the loop is still correct, only slower).
+// Lane l touches line l of the element's tile (27 lines for one mode): the whole tile is in flight with one instruction
+// per lane, long before the Horner chains ask for it.
+__device__ __forceinline__ void prefetch_tile(const FieldParams &f, int e) {
+    const int lane = threadIdx.x & 31;
+    const int nlines = f.tile_stride >> 4;
+    const double *tile = f.tiles + (size_t)e * f.tile_stride;
+    for (int l = lane; l < nlines; l += 32) asm volatile("prefetch.global.L1 [%0];" ::"l"(tile + 16 * l));
+}
+
+// ---- one step of R markers of one thread that sit in the same element e (rows a1-a10) -------------------------------
+// m[r]: slot of marker r in the SoA arrays, on[r]: marker r exists.  Phase A: a1 load, a2 cylindrical map, a4-a5
+// equilibrium quad (every coefficient load shared by the R markers), a7 assemble, a8 Boris, a10 drift + store, a3 for
+// the NEW position (cached for the next step; it is the sort key) and, with kHist, the sort histogram of the new keys.
+// Phase B: a6 perturbed quads folded into dw/dt as they are evaluated, a9 weight update.
+template <int R, bool kHist>
+__device__ __forceinline__ void step_R(const PushParams &P, int e, const long (&m)[R], const bool (&on)[R]) {
+    // the loads below may be speculated above the `on` tests: e is clamped to a valid element for addressing
+    const double *tile = P.f.tiles + (size_t)max(e, 0) * P.f.tile_stride;
+    Marker s[R];
+    StepGeom g[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (on[r]) { s[r].x = P.a.x[m[r]]; s[r].y = P.a.y[m[r]]; s[r].z = P.a.z[m[r]]; }
+        else { s[r].x = 1.0; s[r].y = 0.0; s[r].z = 0.0; }
+    }
+    const Quad hd = ldq(tile);
+    const double Rc = hd.a, Zc = hd.b, se = hd.c;
+    double xi[R], eta[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        step_geometry(s[r], g[r]);
+        xi[r] = __dmul_rn(__dsub_rn(g[r].R, Rc), se); eta[r] = __dmul_rn(__dsub_rn(s[r].z, Zc), se);
+    }
+    double v[R][4], dx[R][4], de[R][4];
+    quad_vd<R>(tile + kTileHeader, xi, eta, v, dx, de);          // (psi0, |B|0, F0, kappa)
+    PertW W[R];
+    double Rn[R], Zn[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        EqOut f;
+        f.psi_R = __dmul_rn(dx[r][0], se); f.psi_Z = __dmul_rn(de[r][0], se);
+        f.Bm = v[r][1]; f.Bm_R = __dmul_rn(dx[r][1], se); f.Bm_Z = __dmul_rn(de[r][1], se);
+        f.F = v[r][2]; f.kappa = v[r][3];
+        if (on[r]) {
+            s[r].vx = P.a.vx[m[r]]; s[r].vy = P.a.vy[m[r]]; s[r].vz = P.a.vz[m[r]]; s[r].mu = P.a.mu[m[r]];
+        } else { s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
+        push_eq(P, g[r], f, s[r], W[r]);
+        if (on[r]) {
+            P.a.x[m[r]] = s[r].x; P.a.y[m[r]] = s[r].y; P.a.z[m[r]] = s[r].z;
+            P.a.vx[m[r]] = s[r].vx; P.a.vy[m[r]] = s[r].vy; P.a.vz[m[r]] = s[r].vz;
+        }
+        // the element search of the new position runs after phase B; its first record starts travelling now
+        Rn[r] = __dsqrt_rn(M3DK_FMA(s[r].x, s[r].x, __dmul_rn(s[r].y, s[r].y)));
+        Zn[r] = s[r].z;
+        locate_prefetch(P.f.fast, Rn[r], Zn[r]);
+    }
+    if (P.f.n_modes > 0) {
+        double wsum[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) wsum[r] = 0.0;
+        for (int md = 0; md < P.f.n_modes; ++md) {
+            const int n = P.f.n_tor[md];
+            const double om = P.f.omega[md];
+            double cth[R], sth[R], nri[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                mode_phase(n, g[r].cph, g[r].sph, P.cwt[md], P.swt[md], cth[r], sth[r]);
+                nri[r] = __dmul_rn((double)n, g[r].rinv);
+            }
+            const double *pm = tile + kTileHeader + kTileEq + kTileMode * md;
+            // the three value-only quads share one copy of the Horner code (rolled: the kernel must fit the 32 KB
+            // instruction cache); the weights of quad q are picked by selects
+#pragma unroll 1
+            for (int q = 0; q < 3; ++q) {
+                quad_vd<R>(pm + q * kQuad, xi, eta, v, dx, de);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const double wa = q == 0 ? W[r].aER : (q == 1 ? W[r].aEZ : 0.0);     // B_phi does not enter
+                    const double wb = q == 0 ? W[r].aEP : (q == 1 ? W[r].bBR : W[r].bBZ);
+                    wsum[r] = pert_fold_v(wsum[r], v[r], wa, wb, cth[r], sth[r]);
+                }
+            }
+            quad_vd<R>(pm + 3 * kQuad, xi, eta, v, dx, de);
+#pragma unroll
+            for (int r = 0; r < R; ++r) wsum[r] = pert_fold_par(wsum[r], v[r], dx[r], de[r], W[r], cth[r], sth[r], se, nri[r], om);
+        }
+        // Eqs. (8)-(9): explicit midpoint on the staggered grid (G9)
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (on[r]) P.a.w[m[r]] = M3DK_FMA(P.dt, wsum[r], P.a.w[m[r]]);
+    }
+    // a3 for the NEW position (the key of the next sort) and, with kHist, the sort histogram of the new keys with each
+    // marker's rank inside its key: the sort then needs no pass over the keys
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        int ne = -1;
+        if (on[r]) {
+            ne = locate_any(P.f, Rn[r], Zn[r]);
+            P.a.elem[m[r]] = ne;
+        }
+        if (kHist) {
+            const int rk = hist_rank(P.hist, ne < 0 ? P.f.n_elems : ne, on[r]);
+            if (on[r]) P.rank[m[r]] = rk;
+        }
+    }
+}
+
+// ---- generic push: one marker per thread, any marker order (every thread gathers its own element's tile) ------------
 template <bool kHist>
-__global__ void __launch_bounds__(kPushThreads) push_kernel(const __grid_constant__ PushParams P) {
+__global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant__ PushParams P) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < P.n;
     const int e = valid ? P.a.elem[i] : -1;
-    const bool active = e >= 0;             // lost markers are frozen (G12)
-    Marker s;
-    if (active) {
-        s.x = P.a.x[i]; s.y = P.a.y[i]; s.z = P.a.z[i];
-        s.vx = P.a.vx[i]; s.vy = P.a.vy[i]; s.vz = P.a.vz[i];
-        s.mu = P.a.mu[i]; s.w = P.a.w[i];
-    } else {
-        s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
+    const long m[1] = {i};
+    const bool on[1] = {e >= 0};             // lost markers are frozen (G12)
+    if (__any_sync(0xffffffffu, on[0])) step_R<1, false>(P, e, m, on);
+    if (kHist) {
+        const int ne = valid ? P.a.elem[i] : -1;
+        const int rk = hist_rank(P.hist, ne < 0 ? P.f.n_elems : ne, valid);
+        if (valid) P.rank[i] = rk;
     }
-    StepGeom gm;
-    step_geometry(s, gm);
-    Fields f;
-    // NB the compiler proves e == ke inside the branch, addresses the tile with the lane's own e and hoists the loads
-    // out of the loop (they run for inactive lanes too): the element used for addressing is clamped to a valid one.
-    const int es = max(e, 0);
-    unsigned todo = __ballot_sync(0xffffffffu, active);
-    while (todo) {
-        const int ke = __shfl_sync(0xffffffffu, es, __ffs(todo) - 1);
-        const bool mine = active && es == ke;
-        if (mine) eval_fields(P.f, ke, gm.R, s.z, gm.cph, gm.sph, gm.rinv, P.cwt, P.swt, f);
-        todo &= ~__ballot_sync(0xffffffffu, mine);
-    }
-    int ne = e;
-    if (active) {
-        step_marker(P, gm, f, s);
-        P.a.x[i] = s.x; P.a.y[i] = s.y; P.a.z[i] = s.z;
-        P.a.vx[i] = s.vx; P.a.vy[i] = s.vy; P.a.vz[i] = s.vz;
-        if (P.f.n_modes > 0) P.a.w[i] = s.w;
-        ne = locate_xyz(P.f, s.x, s.y, s.z);
-        P.a.elem[i] = ne;
-    }
-    if (kHist) {   // histogram of the NEW keys and each marker's rank inside its key: the sort then needs no key pass
-        const int r = hist_rank(P.hist, ne < 0 ? P.f.n_elems : ne, valid);
-        if (valid) P.rank[i] = r;
+}
+
+// ---- element-ordered push: the marker stream is sorted by element and cut into work items --------------------------
+// A work item is up to kItemMarkers = 32 kItemR consecutive markers of ONE element; a warp takes an item, every lane up to
+// kItemR of its markers (slots lane, lane + 32, ...), so that each 32-byte coefficient load is a one-wavefront broadcast
+// that feeds kItemR markers per lane.  Persistent warps draw items from an atomic counter.  Items of the pseudo-element n_elems hold the lost
+// markers: they are frozen and only enter the histogram.
+template <int R, bool kHist>
+__device__ __forceinline__ void item_R(const PushParams &P, int e, int start, int count) {
+    const int lane = threadIdx.x & 31;
+    long m[R];
+    bool on[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { m[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count; }
+    step_R<R, kHist>(P, e, m, on);
+}
+
+// Lines of the next item's marker state (8 arrays x at most 5 lines of 128 B) and of its coefficient tile, one
+// prefetch per lane: they travel while the current item computes.
+__device__ __forceinline__ void prefetch_item(const PushParams &P, int e, int start) {
+    const int lane = threadIdx.x & 31;
+    const double *const arr[8] = {P.a.x, P.a.y, P.a.z, P.a.vx, P.a.vy, P.a.vz, P.a.mu, P.a.w};
+    const double *base = arr[lane >> 2] + (start & ~15);
+    constexpr int kLines = (kItemMarkers * 8 + 127) / 128 + 1;
+#pragma unroll
+    for (int j = 0; j < (kLines + 3) / 4; ++j)
+        if (4 * j + (lane & 3) < kLines) asm volatile("prefetch.global.L1 [%0];" ::"l"(base + 16 * (4 * j + (lane & 3))));
+    if (e < P.f.n_elems) prefetch_tile(P.f, e);
+}
+
+template <bool kHist>
+__global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_kernel(const __grid_constant__ PushParams P) {
+    const int lane = threadIdx.x & 31;
+    const int total = *P.n_items;
+    // static assignment: the warps of a CTA take consecutive items (mostly the same element: shared L1 lines)
+    constexpr int kWarps = kPushThreads / 32;
+    const int stride = gridDim.x * kWarps;
+    int it = blockIdx.x * kWarps + (threadIdx.x >> 5);
+    int4 w = make_int4(P.f.n_elems, 0, 0, 0);
+    if (it < total) { w = __ldg(P.items + it); prefetch_item(P, w.x, w.y); }
+    while (it < total) {
+        const int e = w.x, start = w.y, count = w.z;   // (element, first slot, count, -)
+        it += stride;
+        if (it < total) { w = __ldg(P.items + it); prefetch_item(P, w.x, w.y); }
+        if (e >= P.f.n_elems) {                        // lost markers: frozen (G12), counted for the next sort
+            if (kHist) {
+#pragma unroll 1
+                for (int k = lane; k < ((count + 31) & ~31); k += 32) {
+                    const bool onk = k < count;
+                    const int rk = hist_rank(P.hist, P.f.n_elems, onk);
+                    if (onk) P.rank[start + k] = rk;
+                }
+            }
+            continue;
+        }
+        item_R<kItemR, kHist>(P, e, start, count);
     }
 }
 
@@ -151,18 +289,26 @@ cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_
     return cudaGetLastError();
 }
 
-cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t, bool with_hist) {
+cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t, bool with_hist, bool use_items) {
     if (n == 0) return cudaSuccess;
     PushParams P = make_params(c, a, n, dt, t);
-    const unsigned grid = (unsigned)((n + kPushThreads - 1) / kPushThreads);
     c->kernel_launches += 1;
     if (with_hist) {
         P.hist = c->sb.hist; P.rank = c->sb.rank;
         cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
         if (e != cudaSuccess) return e;
-        push_kernel<true><<<grid, kPushThreads, 0, c->stream>>>(P);
+    }
+    if (use_items) {
+        P.items = c->sb.items; P.n_items = c->sb.ioffs + c->f.n_elems + 1; P.item_counter = c->d_count + 1;
+        cudaError_t e = cudaMemsetAsync(c->d_count + 1, 0, sizeof(int), c->stream);
+        if (e != cudaSuccess) return e;
+        const unsigned grid = (unsigned)(c->sm_count * M3DK_PUSH_MINBLOCKS);
+        if (with_hist) push_items_kernel<true><<<grid, kPushThreads, 0, c->stream>>>(P);
+        else push_items_kernel<false><<<grid, kPushThreads, 0, c->stream>>>(P);
     } else {
-        push_kernel<false><<<grid, kPushThreads, 0, c->stream>>>(P);
+        const unsigned grid = (unsigned)((n + 127) / 128);
+        if (with_hist) push_generic_kernel<true><<<grid, 128, 0, c->stream>>>(P);
+        else push_generic_kernel<false><<<grid, 128, 0, c->stream>>>(P);
     }
     return cudaGetLastError();
 }

@@ -10,7 +10,8 @@ static inline size_t up256(size_t b) { return (b + 255) / 256 * 256; }
 size_t sort_workspace_bytes(long n, int n_elems) {
     const size_t nd = up256((size_t)n * sizeof(double)), ni = up256((size_t)n * sizeof(int));
     const size_t nh = up256((size_t)(n_elems + 2) * sizeof(int));
-    return 8 * nd + 3 * ni + 2 * nh;
+    const size_t nit = up256(((size_t)n / kItemMarkers + n_elems + 2) * sizeof(int4));
+    return 8 * nd + 3 * ni + 3 * nh + nit;
 }
 
 void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb) {
@@ -24,6 +25,8 @@ void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb) {
     sb->rank = reinterpret_cast<int *>(p); p += ni;
     sb->hist = reinterpret_cast<int *>(p); p += nh;
     sb->offs = reinterpret_cast<int *>(p); p += nh;
+    sb->ioffs = reinterpret_cast<int *>(p); p += nh;
+    sb->items = reinterpret_cast<int4 *>(p); p += up256(((size_t)n / kItemMarkers + n_elems + 2) * sizeof(int4));
     sb->bytes = (size_t)(p - static_cast<char *>(ws));
 }
 
@@ -44,50 +47,67 @@ __global__ void __launch_bounds__(256) hist_rank_kernel(const int *__restrict__ 
     rank[i] = base + __popc(peers & ((1u << lane) - 1u));
 }
 
-// exclusive scan of hist[0..m) into offs[0..m] (offs[m] = total): one CTA, coalesced chunks of 1024 x 4 bins, warp
-// shuffles inside a chunk, a running carry across chunks (m is a few 1e5 bins: ~30 chunk iterations).
-__global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist, int m, int *__restrict__ offs) {
-    __shared__ int wsum[32];
-    __shared__ int carry_s;
+// exclusive scan of hist[0..m) into offs[0..m] (offs[m] = total) and, in the same sweep, of the work-item counts
+// ceil(hist[k] / kItemMarkers) into ioffs[0..m]: one CTA, coalesced chunks of 1024 x 4 bins, warp shuffles inside a
+// chunk, running carries across chunks (m is a few 1e5 bins: ~30 chunk iterations).
+__global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist, int m, int *__restrict__ offs,
+                                                    int *__restrict__ ioffs) {
+    __shared__ int2 wsum[32];
+    __shared__ int2 carry_s;
     const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
-    if (t == 0) carry_s = 0;
+    if (t == 0) carry_s = make_int2(0, 0);
     __syncthreads();
     for (int base = 0; base < m; base += 4096) {
         const int k = base + 4 * t;
-        int v[4];
+        int v[4], it[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) v[q] = k + q < m ? hist[k + q] : 0;
-        const int mine = v[0] + v[1] + v[2] + v[3];
-        int inc = mine;
+        for (int q = 0; q < 4; ++q) {
+            v[q] = k + q < m ? hist[k + q] : 0;
+            it[q] = (v[q] + kItemMarkers - 1) / kItemMarkers;
+        }
+        const int2 mine = make_int2(v[0] + v[1] + v[2] + v[3], it[0] + it[1] + it[2] + it[3]);
+        int2 inc = mine;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const int u = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += u;
+            const int ux = __shfl_up_sync(0xffffffffu, inc.x, o), uy = __shfl_up_sync(0xffffffffu, inc.y, o);
+            if (lane >= o) { inc.x += ux; inc.y += uy; }
         }
         if (lane == 31) wsum[wid] = inc;
         __syncthreads();
         if (wid == 0) {
-            int w = wsum[lane];
+            int2 w = wsum[lane];
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
-                const int u = __shfl_up_sync(0xffffffffu, w, o);
-                if (lane >= o) w += u;
+                const int ux = __shfl_up_sync(0xffffffffu, w.x, o), uy = __shfl_up_sync(0xffffffffu, w.y, o);
+                if (lane >= o) { w.x += ux; w.y += uy; }
             }
             wsum[lane] = w;      // inclusive over warps
         }
         __syncthreads();
-        const int carry = carry_s;
-        int run = carry + (wid ? wsum[wid - 1] : 0) + inc - mine;
+        const int2 carry = carry_s;
+        const int2 wprev = wid ? wsum[wid - 1] : make_int2(0, 0);
+        int run = carry.x + wprev.x + inc.x - mine.x, irun = carry.y + wprev.y + inc.y - mine.y;
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            if (k + q < m) offs[k + q] = run;
-            run += v[q];
+            if (k + q < m) { offs[k + q] = run; ioffs[k + q] = irun; }
+            run += v[q]; irun += it[q];
         }
         __syncthreads();
-        if (t == 1023) carry_s = carry + wsum[31];
+        if (t == 1023) carry_s = make_int2(carry.x + wsum[31].x, carry.y + wsum[31].y);
         __syncthreads();
     }
-    if (t == 0) offs[m] = carry_s;
+    if (t == 0) { offs[m] = carry_s.x; ioffs[m] = carry_s.y; }
+}
+
+// work items of the element-ordered push: element k's sorted segment [offs[k], offs[k+1]) cut into pieces of at most
+// kItemMarkers markers; k = n_elems is the pseudo-element of the lost markers
+__global__ void __launch_bounds__(256) items_kernel(const int *__restrict__ offs, const int *__restrict__ ioffs, int m,
+                                                    int4 *__restrict__ items) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m) return;
+    const int b = offs[k], cnt = offs[k + 1] - b;
+    int j = ioffs[k];
+    for (int c = 0; c < cnt; c += kItemMarkers, ++j) items[j] = make_int4(k, b + c, min(kItemMarkers, cnt - c), 0);
 }
 
 __global__ void __launch_bounds__(256) scatter_kernel(MarkerArrays s, MarkerArrays d, long n, int n_elems,
@@ -113,7 +133,9 @@ cudaError_t launch_sort(m3dk_ctx *c, const MarkerArrays &src, const MarkerArrays
         hist_rank_kernel<<<grid, 256, 0, c->stream>>>(src.elem, n, c->f.n_elems, c->sb.hist, c->sb.rank);
     }
     c->kernel_launches += 2;
-    scan_kernel<<<1, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs);
+    scan_kernel<<<1, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs, c->sb.ioffs);
+    c->kernel_launches += 1;
+    items_kernel<<<(m + 255) / 256, 256, 0, c->stream>>>(c->sb.offs, c->sb.ioffs, m, c->sb.items);
     scatter_kernel<<<grid, 256, 0, c->stream>>>(src, dst, n, c->f.n_elems, c->sb.offs, c->sb.rank);
     return cudaGetLastError();
 }
