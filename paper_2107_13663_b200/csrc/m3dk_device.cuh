@@ -33,37 +33,63 @@ __device__ __forceinline__ Quad ldq(const double *p) {
     return q;
 }
 
+// The same four coefficients from a tile staged in shared memory (two LDS.128, warp-uniform address: broadcast).
+template <bool kSmem>
+__device__ __forceinline__ Quad ldq_t(const double *p) {
+    if (kSmem) {
+        const double2 lo = reinterpret_cast<const double2 *>(p)[0], hi = reinterpret_cast<const double2 *>(p)[1];
+        Quad q; q.a = lo.x; q.b = lo.y; q.c = hi.x; q.d = hi.y;
+        return q;
+    }
+    return ldq(p);
+}
+
 // ---- polynomial quads (G10: monomials xi^i eta^j, j outer, i inner; row j starts at kRow[j], has 6 - j terms) -----
 // c[4 k + s]: coefficient k of slot s.  Horner in xi inside a row, Horner in eta across rows; value, d/dxi, d/deta of
 // all four slots: 38 FMA per slot.  Callers ignore the outputs they do not need; after full unrolling the unused
 // chains are dead code and disappear (value only: 20 FMA per slot).
 // R markers per thread share every coefficient load (all R sit in the same element): one 32-byte load feeds up to
 // 8 R FMAs, which is what takes the L1 -> register-file path (128 B/clk/SM) off the critical path.
-template <int R>
-__device__ __forceinline__ void quad_vd(const double *__restrict__ c, const double (&xi)[R], const double (&eta)[R],
-                                        double (&v)[R][4], double (&dx)[R][4], double (&de)[R][4]) {
+// The Horner scheme consumes the 21 coefficient quads of a block in descending order k = 20 .. 0, so the loads are
+// software-pipelined through a ring of kRing quads: `ring` holds k = 20 .. 20 - kRing + 1 on entry; while quad k is
+// consumed quad k - kRing is loaded, and on exit `ring` holds the first kRing quads of the block `nxt` (the block the
+// caller evaluates next: the blocks of a tile are consumed back to back), so an L1 hit is never waited for.
+constexpr int kRing = 3;   // must divide 21 so that the ring slots line up from one block to the next
+static_assert(21 % kRing == 0, "kRing must divide the 21 coefficients of a block");
+struct Ring { Quad q[kRing]; };
+template <bool kSmem>
+__device__ __forceinline__ void ring_fill(Ring &ring, const double *__restrict__ c) {
+#pragma unroll
+    for (int i = 0; i < kRing; ++i) ring.q[i] = ldq_t<kSmem>(c + 4 * (20 - i));
+}
+
+template <int R, bool kSmem>
+__device__ __forceinline__ void quad_vd(const double *__restrict__ c, const double *__restrict__ nxt, Ring &ring,
+                                        const double (&xi)[R], const double (&eta)[R], double (&v)[R][4],
+                                        double (&dx)[R][4], double (&de)[R][4]) {
     constexpr int kRow[6] = {0, 6, 11, 15, 18, 20};
     double a[R][4], ax[R][4], ae[R][4];
+    int n = 0;   // quads consumed so far: quad k = 20 - n sits in ring slot n % kRing
 #pragma unroll
     for (int j = 5; j >= 0; --j) {
         const int L = 6 - j;
-        const Quad t = ldq(c + 4 * (kRow[j] + L - 1));
         double p[R][4], d[R][4];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            p[r][0] = t.a; p[r][1] = t.b; p[r][2] = t.c; p[r][3] = t.d;
-            d[r][0] = d[r][1] = d[r][2] = d[r][3] = 0.0;
-        }
-#pragma unroll
-        for (int i = L - 2; i >= 0; --i) {
-            const Quad u = ldq(c + 4 * (kRow[j] + i));
+        for (int i = L - 1; i >= 0; --i) {
+            const int k = kRow[j] + i;                 // == 20 - n
+            const Quad u = ring.q[n % kRing];
+            ring.q[n % kRing] = k - kRing >= 0 ? ldq_t<kSmem>(c + 4 * (k - kRing)) : ldq_t<kSmem>(nxt + 4 * (k - kRing + 21));
+            ++n;
             const double uu[4] = {u.a, u.b, u.c, u.d};
 #pragma unroll
             for (int r = 0; r < R; ++r)
 #pragma unroll
                 for (int s = 0; s < 4; ++s) {
-                    d[r][s] = (i == L - 2) ? p[r][s] : M3DK_FMA(d[r][s], xi[r], p[r][s]);
-                    p[r][s] = M3DK_FMA(p[r][s], xi[r], uu[s]);
+                    if (i == L - 1) { p[r][s] = uu[s]; d[r][s] = 0.0; }
+                    else {
+                        d[r][s] = (i == L - 2) ? p[r][s] : M3DK_FMA(d[r][s], xi[r], p[r][s]);
+                        p[r][s] = M3DK_FMA(p[r][s], xi[r], uu[s]);
+                    }
                 }
         }
 #pragma unroll
@@ -136,12 +162,17 @@ __device__ __forceinline__ FastRec ldrec(const FastRec *p) {
 
 // The asm loads are not volatile, so the compiler may hoist them above the range checks: every address is therefore
 // clamped into its table first and the checks only decide whether the loaded record is used.
-__device__ __forceinline__ int locate_fast(const FastGrid &g, double R, double Z) {
+__device__ __forceinline__ FastRec locate_first(const FastGrid &g, double R, double Z) {
+    const double fx = (R - g.Rmin) * g.inv_hx, fz = (Z - g.Zmin) * g.inv_hz;
+    const bool inside = fx >= 0.0 && fx < (double)g.gx && fz >= 0.0 && fz < (double)g.gz;
+    const int ix = inside ? (int)fx : 0, iz = inside ? (int)fz : 0;
+    return ldrec(g.first + (size_t)(iz * g.gx + ix));
+}
+__device__ __forceinline__ int locate_fast_from(const FastGrid &g, FastRec r, double R, double Z) {
     const double fx = (R - g.Rmin) * g.inv_hx, fz = (Z - g.Zmin) * g.inv_hz;
     const bool inside = fx >= 0.0 && fx < (double)g.gx && fz >= 0.0 && fz < (double)g.gz;
     const int ix = inside ? (int)fx : 0, iz = inside ? (int)fz : 0;
     const float u = (float)(fx - (double)ix), v = (float)(fz - (double)iz);
-    FastRec r = ldrec(g.first + (size_t)(iz * g.gx + ix));
     int found = -2;
     bool open = inside;
 #pragma unroll 1
@@ -155,6 +186,9 @@ __device__ __forceinline__ int locate_fast(const FastGrid &g, double R, double Z
     }
     return found;
 }
+__device__ __forceinline__ int locate_fast(const FastGrid &g, double R, double Z) {
+    return locate_fast_from(g, locate_first(g, R, Z), R, Z);
+}
 
 // first record of the bucket of (R, Z): one line into L1 (the search itself runs later)
 __device__ __forceinline__ void locate_prefetch(const FastGrid &g, double R, double Z) {
@@ -162,6 +196,11 @@ __device__ __forceinline__ void locate_prefetch(const FastGrid &g, double R, dou
     const bool inside = fx >= 0.0 && fx < (double)g.gx && fz >= 0.0 && fz < (double)g.gz;
     const int ix = inside ? (int)fx : 0, iz = inside ? (int)fz : 0;
     asm volatile("prefetch.global.L1 [%0];" ::"l"(g.first + (size_t)(iz * g.gx + ix)));
+}
+
+__device__ __forceinline__ int locate_finish(const FieldParams &f, const FastRec &first, double R, double Z) {
+    const int e = locate_fast_from(f.fast, first, R, Z);
+    return e != -2 ? e : locate(f.grid, R, Z);
 }
 
 __device__ __forceinline__ int locate_any(const FieldParams &f, double R, double Z) {
@@ -180,7 +219,9 @@ __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double 
     const double xi1[1] = {(R - Rc) * se}, eta1[1] = {(Z - Zc) * se};
     double vv[1][4], dxx[1][4], dee[1][4];
     double (&v)[4] = vv[0], (&dx)[4] = dxx[0], (&de)[4] = dee[0];
-    quad_vd<1>(tile + kTileHeader, xi1, eta1, vv, dxx, dee);  // (psi0, |B|0, F0, kappa)
+    Ring ring;
+    ring_fill<false>(ring, tile + kTileHeader);
+    quad_vd<1, false>(tile + kTileHeader, tile + kTileHeader, ring, xi1, eta1, vv, dxx, dee);  // (psi0, |B|0, F0, kappa)
     o.psi_R = dx[0] * se; o.psi_Z = de[0] * se;
     o.Bm = v[1]; o.Bm_R = dx[1] * se; o.Bm_Z = de[1] * se;
     o.F = v[2]; o.kappa = v[3];
@@ -201,16 +242,17 @@ __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double 
         const double sth = sn * cwt[md] - cn * swt[md];      // sin(n phi - omega t)
         const double *pm = tile + kTileHeader + kTileEq + kTileMode * md;
         // Re[C e^{i th}] = Cr cos th - Ci sin th
-        quad_vd<1>(pm, xi1, eta1, vv, dxx, dee);                     // E_R, E_phi
+        ring_fill<false>(ring, pm);
+        quad_vd<1, false>(pm, pm + kQuad, ring, xi1, eta1, vv, dxx, dee);                  // E_R, E_phi
         o.E1[0] += v[0] * cth - v[1] * sth;
         o.E1[1] += v[2] * cth - v[3] * sth;
-        quad_vd<1>(pm + kQuad, xi1, eta1, vv, dxx, dee);             // E_Z, B_R
+        quad_vd<1, false>(pm + kQuad, pm + 2 * kQuad, ring, xi1, eta1, vv, dxx, dee);         // E_Z, B_R
         o.E1[2] += v[0] * cth - v[1] * sth;
         o.B1[0] += v[2] * cth - v[3] * sth;
-        quad_vd<1>(pm + 2 * kQuad, xi1, eta1, vv, dxx, dee);         // B_phi, B_Z
+        quad_vd<1, false>(pm + 2 * kQuad, pm + 3 * kQuad, ring, xi1, eta1, vv, dxx, dee);         // B_phi, B_Z
         o.B1[1] += v[0] * cth - v[1] * sth;
         o.B1[2] += v[2] * cth - v[3] * sth;
-        quad_vd<1>(pm + 3 * kQuad, xi1, eta1, vv, dxx, dee);         // B_par with gradient (slots 2, 3 are padding)
+        quad_vd<1, false>(pm + 3 * kQuad, pm, ring, xi1, eta1, vv, dxx, dee);         // B_par with gradient (slots 2, 3 are padding)
         const double re = v[0], im = v[1];
         const double qd = re * sth + im * cth;               // -Im-part combination: d/dphi -> -n qd, d/dt -> omega qd
         o.B1p += re * cth - im * sth;

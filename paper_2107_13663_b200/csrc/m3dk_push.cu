@@ -38,13 +38,28 @@ __device__ __forceinline__ int hist_rank(int *hist, int key, bool on) {
     return r;
 }
 
-// Lane l touches line l of the element's tile (27 lines for one mode): the whole tile is in flight with one instruction
-// per lane, long before the Horner chains ask for it.
-__device__ __forceinline__ void prefetch_tile(const FieldParams &f, int e) {
+// The same for R keys per lane: all atomics are issued before the first returned value is needed.
+template <int R>
+__device__ __forceinline__ void hist_rank_R(int *hist, int *rank, const int (&key)[R], const long (&m)[R],
+                                            const bool (&on)[R]) {
     const int lane = threadIdx.x & 31;
-    const int nlines = f.tile_stride >> 4;
-    const double *tile = f.tiles + (size_t)e * f.tile_stride;
-    for (int l = lane; l < nlines; l += 32) asm volatile("prefetch.global.L1 [%0];" ::"l"(tile + 16 * l));
+    unsigned peers[R];
+    int base[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const unsigned live = __ballot_sync(0xffffffffu, on[r]);
+        peers[r] = 0u; base[r] = 0;
+        if (on[r]) {
+            peers[r] = __match_any_sync(live, key[r]);
+            if (lane == __ffs(peers[r]) - 1) base[r] = atomicAdd(hist + key[r], __popc(peers[r]));
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+        if (on[r]) {
+            const int b = __shfl_sync(peers[r], base[r], __ffs(peers[r]) - 1);
+            rank[m[r]] = b + __popc(peers[r] & ((1u << lane) - 1u));
+        }
 }
 
 // ---- one step of R markers of one thread that sit in the same element e (rows a1-a10) -------------------------------
@@ -52,10 +67,10 @@ __device__ __forceinline__ void prefetch_tile(const FieldParams &f, int e) {
 // equilibrium quad (every coefficient load shared by the R markers), a7 assemble, a8 Boris, a10 drift + store, a3 for
 // the NEW position (cached for the next step; it is the sort key) and, with kHist, the sort histogram of the new keys.
 // Phase B: a6 perturbed quads folded into dw/dt as they are evaluated, a9 weight update.
-template <int R, bool kHist>
-__device__ __forceinline__ void step_R(const PushParams &P, int e, const long (&m)[R], const bool (&on)[R]) {
-    // the loads below may be speculated above the `on` tests: e is clamped to a valid element for addressing
-    const double *tile = P.f.tiles + (size_t)max(e, 0) * P.f.tile_stride;
+// tile: the element's coefficient tile, in global memory (kSmem = false) or staged in shared memory (kSmem = true).
+template <int R, bool kHist, bool kSmem>
+__device__ __forceinline__ void step_R(const PushParams &P, const double *__restrict__ tile, const long (&m)[R],
+                                       const bool (&on)[R]) {
     Marker s[R];
     StepGeom g[R];
 #pragma unroll
@@ -63,7 +78,7 @@ __device__ __forceinline__ void step_R(const PushParams &P, int e, const long (&
         if (on[r]) { s[r].x = P.a.x[m[r]]; s[r].y = P.a.y[m[r]]; s[r].z = P.a.z[m[r]]; }
         else { s[r].x = 1.0; s[r].y = 0.0; s[r].z = 0.0; }
     }
-    const Quad hd = ldq(tile);
+    const Quad hd = ldq_t<kSmem>(tile);
     const double Rc = hd.a, Zc = hd.b, se = hd.c;
     double xi[R], eta[R];
 #pragma unroll
@@ -72,7 +87,9 @@ __device__ __forceinline__ void step_R(const PushParams &P, int e, const long (&
         xi[r] = __dmul_rn(__dsub_rn(g[r].R, Rc), se); eta[r] = __dmul_rn(__dsub_rn(s[r].z, Zc), se);
     }
     double v[R][4], dx[R][4], de[R][4];
-    quad_vd<R>(tile + kTileHeader, xi, eta, v, dx, de);          // (psi0, |B|0, F0, kappa)
+    Ring ring;
+    ring_fill<kSmem>(ring, tile + kTileHeader);
+    quad_vd<R, kSmem>(tile + kTileHeader, tile + kTileHeader, ring, xi, eta, v, dx, de);   // (psi0, |B|0, F0, kappa)
     PertW W[R];
     double Rn[R], Zn[R];
 #pragma unroll
@@ -95,9 +112,9 @@ __device__ __forceinline__ void step_R(const PushParams &P, int e, const long (&
         locate_prefetch(P.f.fast, Rn[r], Zn[r]);
     }
     if (P.f.n_modes > 0) {
-        double wsum[R];
+        double wsum[R], w0[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) wsum[r] = 0.0;
+        for (int r = 0; r < R; ++r) { wsum[r] = 0.0; w0[r] = on[r] ? P.a.w[m[r]] : 0.0; }
         for (int md = 0; md < P.f.n_modes; ++md) {
             const int n = P.f.n_tor[md];
             const double om = P.f.omega[md];
@@ -108,11 +125,12 @@ __device__ __forceinline__ void step_R(const PushParams &P, int e, const long (&
                 nri[r] = __dmul_rn((double)n, g[r].rinv);
             }
             const double *pm = tile + kTileHeader + kTileEq + kTileMode * md;
+            ring_fill<kSmem>(ring, pm);
             // the three value-only quads share one copy of the Horner code (rolled: the kernel must fit the 32 KB
             // instruction cache); the weights of quad q are picked by selects
 #pragma unroll 1
             for (int q = 0; q < 3; ++q) {
-                quad_vd<R>(pm + q * kQuad, xi, eta, v, dx, de);
+                quad_vd<R, kSmem>(pm + q * kQuad, pm + (q + 1) * kQuad, ring, xi, eta, v, dx, de);
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const double wa = q == 0 ? W[r].aER : (q == 1 ? W[r].aEZ : 0.0);     // B_phi does not enter
@@ -120,29 +138,31 @@ __device__ __forceinline__ void step_R(const PushParams &P, int e, const long (&
                     wsum[r] = pert_fold_v(wsum[r], v[r], wa, wb, cth[r], sth[r]);
                 }
             }
-            quad_vd<R>(pm + 3 * kQuad, xi, eta, v, dx, de);
+            quad_vd<R, kSmem>(pm + 3 * kQuad, pm, ring, xi, eta, v, dx, de);
 #pragma unroll
             for (int r = 0; r < R; ++r) wsum[r] = pert_fold_par(wsum[r], v[r], dx[r], de[r], W[r], cth[r], sth[r], se, nri[r], om);
         }
         // Eqs. (8)-(9): explicit midpoint on the staggered grid (G9)
 #pragma unroll
         for (int r = 0; r < R; ++r)
-            if (on[r]) P.a.w[m[r]] = M3DK_FMA(P.dt, wsum[r], P.a.w[m[r]]);
+            if (on[r]) P.a.w[m[r]] = M3DK_FMA(P.dt, wsum[r], w0[r]);
     }
     // a3 for the NEW position (the key of the next sort) and, with kHist, the sort histogram of the new keys with each
     // marker's rank inside its key: the sort then needs no pass over the keys
+    FastRec rec[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);   // all first records in flight together
+    int key[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         int ne = -1;
         if (on[r]) {
-            ne = locate_any(P.f, Rn[r], Zn[r]);
+            ne = locate_finish(P.f, rec[r], Rn[r], Zn[r]);
             P.a.elem[m[r]] = ne;
         }
-        if (kHist) {
-            const int rk = hist_rank(P.hist, ne < 0 ? P.f.n_elems : ne, on[r]);
-            if (on[r]) P.rank[m[r]] = rk;
-        }
+        key[r] = ne < 0 ? P.f.n_elems : ne;
     }
+    if (kHist) hist_rank_R<R>(P.hist, P.rank, key, m, on);
 }
 
 // ---- generic push: one marker per thread, any marker order (every thread gathers its own element's tile) ------------
@@ -153,7 +173,8 @@ __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant
     const int e = valid ? P.a.elem[i] : -1;
     const long m[1] = {i};
     const bool on[1] = {e >= 0};             // lost markers are frozen (G12)
-    if (__any_sync(0xffffffffu, on[0])) step_R<1, false>(P, e, m, on);
+    // the tile loads may be speculated above the `on` tests: e is clamped to a valid element for addressing
+    if (__any_sync(0xffffffffu, on[0])) step_R<1, false, false>(P, P.f.tiles + (size_t)max(e, 0) * P.f.tile_stride, m, on);
     if (kHist) {
         const int ne = valid ? P.a.elem[i] : -1;
         const int rk = hist_rank(P.hist, ne < 0 ? P.f.n_elems : ne, valid);
@@ -166,43 +187,73 @@ __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant
 // kItemR of its markers (slots lane, lane + 32, ...), so that each 32-byte coefficient load is a one-wavefront broadcast
 // that feeds kItemR markers per lane.  Persistent warps draw items from an atomic counter.  Items of the pseudo-element n_elems hold the lost
 // markers: they are frozen and only enter the histogram.
-template <int R, bool kHist>
-__device__ __forceinline__ void item_R(const PushParams &P, int e, int start, int count) {
-    const int lane = threadIdx.x & 31;
-    long m[R];
-    bool on[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) { m[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count; }
-    step_R<R, kHist>(P, e, m, on);
+// ---- tile staging: one bulk copy (TMA, cp.async.bulk) per item into the warp's double buffer, mbarrier completion --
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tile_copy_issue(unsigned dst, const double *src, unsigned bytes, unsigned bar) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile("{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @!p bra WAIT_%=;\n}"
+                 ::"r"(bar), "r"(parity) : "memory");
 }
 
-// Lines of the next item's marker state (8 arrays x at most 5 lines of 128 B) and of its coefficient tile, one
-// prefetch per lane: they travel while the current item computes.
-__device__ __forceinline__ void prefetch_item(const PushParams &P, int e, int start) {
+// Lines of the next item's marker state (8 arrays x at most 5 lines of 128 B), one L2 prefetch per lane: they travel
+// while the current item computes.
+__device__ __forceinline__ void prefetch_state(const PushParams &P, int start) {
     const int lane = threadIdx.x & 31;
     const double *const arr[8] = {P.a.x, P.a.y, P.a.z, P.a.vx, P.a.vy, P.a.vz, P.a.mu, P.a.w};
     const double *base = arr[lane >> 2] + (start & ~15);
     constexpr int kLines = (kItemMarkers * 8 + 127) / 128 + 1;
 #pragma unroll
     for (int j = 0; j < (kLines + 3) / 4; ++j)
-        if (4 * j + (lane & 3) < kLines) asm volatile("prefetch.global.L1 [%0];" ::"l"(base + 16 * (4 * j + (lane & 3))));
-    if (e < P.f.n_elems) prefetch_tile(P.f, e);
+        if (4 * j + (lane & 3) < kLines) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + 16 * (4 * j + (lane & 3))));
 }
 
+// ---- element-ordered push: the marker stream is sorted by element and cut into work items --------------------------
+// A work item is up to kItemMarkers = 32 kItemR consecutive markers of ONE element; a warp takes an item, every lane up to
+// kItemR of its markers (slots lane, lane + 32, ...).  The element's coefficient tile is staged in shared memory by one
+// bulk copy per item (double-buffered per warp: the next item's tile travels while this one computes), and every
+// coefficient read is a broadcast LDS that feeds kItemR markers per lane.  Static assignment: the warps of a CTA take
+// consecutive items.  Items of the pseudo-element n_elems hold the lost markers: frozen, they only enter the histogram.
 template <bool kHist>
 __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_kernel(const __grid_constant__ PushParams P) {
-    const int lane = threadIdx.x & 31;
-    const int total = *P.n_items;
-    // static assignment: the warps of a CTA take consecutive items (mostly the same element: shared L1 lines)
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int kWarps = kPushThreads / 32;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int stride_d = P.f.tile_stride;
+    const unsigned tile_bytes = (unsigned)stride_d * 8u;
+    double *const tbuf = reinterpret_cast<double *>(smem_raw) + (size_t)warp * 2 * stride_d;
+    unsigned long long *const bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)kWarps * 2 * tile_bytes) + warp * 2;
+    const unsigned bar0 = smem_u32(bars), buf0 = smem_u32(tbuf);
+    if (lane == 0) {
+        mbar_init(bar0); mbar_init(bar0 + 8);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    const int total = *P.n_items;
     const int stride = gridDim.x * kWarps;
-    int it = blockIdx.x * kWarps + (threadIdx.x >> 5);
+    int it = blockIdx.x * kWarps + warp;
     int4 w = make_int4(P.f.n_elems, 0, 0, 0);
-    if (it < total) { w = __ldg(P.items + it); prefetch_item(P, w.x, w.y); }
+    unsigned b = 0, phase = 0;   // buffer of the current item; bit k of phase: parity to wait for on buffer k
+    if (it < total) {
+        w = __ldg(P.items + it);
+        if (w.x < P.f.n_elems && lane == 0) tile_copy_issue(buf0, P.f.tiles + (size_t)w.x * stride_d, tile_bytes, bar0);
+    }
     while (it < total) {
         const int e = w.x, start = w.y, count = w.z;   // (element, first slot, count, -)
         it += stride;
-        if (it < total) { w = __ldg(P.items + it); prefetch_item(P, w.x, w.y); }
+        if (it < total) {
+            w = __ldg(P.items + it);
+            __syncwarp();                              // every lane has finished reading buffer b ^ 1 (previous item)
+            if (w.x < P.f.n_elems && lane == 0)
+                tile_copy_issue(buf0 + (b ^ 1) * tile_bytes, P.f.tiles + (size_t)w.x * stride_d, tile_bytes, bar0 + (b ^ 1) * 8);
+            prefetch_state(P, w.y);
+        }
         if (e >= P.f.n_elems) {                        // lost markers: frozen (G12), counted for the next sort
             if (kHist) {
 #pragma unroll 1
@@ -212,9 +263,16 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
                     if (onk) P.rank[start + k] = rk;
                 }
             }
-            continue;
+        } else {
+            long m[kItemR];
+            bool on[kItemR];
+#pragma unroll
+            for (int r = 0; r < kItemR; ++r) { m[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count; }
+            mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
+            phase ^= 1u << b;
+            step_R<kItemR, kHist, true>(P, tbuf + (size_t)b * stride_d, m, on);
         }
-        item_R<kItemR, kHist>(P, e, start, count);
+        b ^= 1;
     }
 }
 
@@ -303,8 +361,11 @@ cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, d
         cudaError_t e = cudaMemsetAsync(c->d_count + 1, 0, sizeof(int), c->stream);
         if (e != cudaSuccess) return e;
         const unsigned grid = (unsigned)(c->sm_count * M3DK_PUSH_MINBLOCKS);
-        if (with_hist) push_items_kernel<true><<<grid, kPushThreads, 0, c->stream>>>(P);
-        else push_items_kernel<false><<<grid, kPushThreads, 0, c->stream>>>(P);
+        const size_t smem = (size_t)(kPushThreads / 32) * 2 * (c->f.tile_stride * 8 + 8);
+        auto kern = with_hist ? push_items_kernel<true> : push_items_kernel<false>;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        kern<<<grid, kPushThreads, smem, c->stream>>>(P);
     } else {
         const unsigned grid = (unsigned)((n + 127) / 128);
         if (with_hist) push_generic_kernel<true><<<grid, 128, 0, c->stream>>>(P);
