@@ -350,13 +350,10 @@ extern "C" int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, 
     CU(cudaSetDevice(ctx->device), "cudaSetDevice");
     ctx->n = n;
     ctx->user = MarkerArrays{x, y, z, vx, vy, vz, mu, w, elem, id};
-    ctx->cur = 0;
     ctx->q = charge; ctx->m = mass; ctx->f0 = *f0;
     ctx->steps_done = 0; ctx->n_sorts = 0;
     ctx->steps_since_sort = ctx->sort_interval;   // the first push sorts first when sorting is on
     ctx->have_markers = true;
-    ctx->hist_valid = false;
-    ctx->items_valid = false;
     if (ctx->have_sortws && ctx->sb.bytes) {      // an older workspace may be too small for the new n
         if (sort_workspace_bytes(n, ctx->f.n_elems) > ctx->sb.bytes) ctx->have_sortws = false;
     }
@@ -385,8 +382,6 @@ static int bind_sort_ws(m3dk_ctx *ctx, void *ws, size_t bytes, const char *who) 
     if (!ws || ((uintptr_t)ws & 255) || bytes < sort_workspace_bytes(ctx->n, ctx->f.n_elems))
         return fail(ctx, M3DK_EWORKSPACE, std::string(who) + ": workspace NULL, misaligned or smaller than m3dk_sort_workspace_bytes");
     carve_sort_workspace(ws, ctx->n, ctx->f.n_elems, &ctx->sb);
-    ctx->hist_valid = false;
-    ctx->items_valid = false;
     ctx->sb.bytes = bytes;
     ctx->have_sortws = true;
     return M3DK_OK;
@@ -397,36 +392,13 @@ extern "C" int m3dk_set_sort_workspace(m3dk_ctx *ctx, void *dev_workspace, size_
     return bind_sort_ws(ctx, dev_workspace, bytes, "m3dk_set_sort_workspace");
 }
 
-static const MarkerArrays &cur_arrays(m3dk_ctx *ctx) { return ctx->cur ? ctx->sb.alt : ctx->user; }
-
-static int sort_flip(m3dk_ctx *ctx) {   // sort current -> other, other becomes current
-    const MarkerArrays &src = cur_arrays(ctx);
-    const MarkerArrays &dst = ctx->cur ? ctx->user : ctx->sb.alt;
-    {
-        EvScope ev(ctx, &ctx->ev_sort);
-        CU(launch_sort(ctx, src, dst, ctx->n, ctx->hist_valid), "sort kernels");
-    }
-    ctx->hist_valid = false;
-    ctx->items_valid = true;     // the arrays that are current now are sorted and sb.items cut them by element
-    ctx->cur ^= 1;
-    ctx->n_sorts++;
-    ctx->steps_since_sort = 0;
-    return M3DK_OK;
-}
-
-static int settle(m3dk_ctx *ctx) {      // make the caller's arrays current again
-    if (!ctx->cur) return M3DK_OK;
-    const MarkerArrays &s = ctx->sb.alt, &d = ctx->user;
-    const size_t nd = (size_t)ctx->n * sizeof(double), ni = (size_t)ctx->n * sizeof(int);
-    double *const sd[8] = {s.x, s.y, s.z, s.vx, s.vy, s.vz, s.mu, s.w};
-    double *const dd[8] = {d.x, d.y, d.z, d.vx, d.vy, d.vz, d.mu, d.w};
-    for (int k = 0; k < 8; ++k) CU(cudaMemcpyAsync(dd[k], sd[k], nd, cudaMemcpyDeviceToDevice, ctx->stream), "copy back");
-    CU(cudaMemcpyAsync(d.elem, s.elem, ni, cudaMemcpyDeviceToDevice, ctx->stream), "copy back");
-    CU(cudaMemcpyAsync(d.id, s.id, ni, cudaMemcpyDeviceToDevice, ctx->stream), "copy back");
-    ctx->cur = 0;
-    return M3DK_OK;
-}
-
+// ---- sort and push ---------------------------------------------------------------------------------------------------
+// sort_interval = 0: the caller's SoA arrays are pushed in place, in whatever order they are (one marker per thread,
+// every thread gathers its own element's coefficients).
+// sort_interval = k >= 1: ordered pipeline.  At the start of the call the markers are packed into 64-byte records in
+// element order (a sort); every k-th step is followed by a re-ordering (histogram fused into the push, scan, work-item
+// cut, order list) and the step after an ordering runs the element-ordered kernel, the others the in-place kernel;
+// at the end of the call the records are unpacked into the caller's arrays (permuted; id[] says who is where).
 extern "C" int m3dk_sort(m3dk_ctx *ctx, void *dev_workspace, size_t bytes) {
     if (!ctx) return M3DK_EINVAL;
     if (!ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_sort: call m3dk_particles_init first");
@@ -438,9 +410,14 @@ extern "C" int m3dk_sort(m3dk_ctx *ctx, void *dev_workspace, size_t bytes) {
     }
     CU(cudaSetDevice(ctx->device), "cudaSetDevice");
     if (ctx->n == 0) return M3DK_OK;
-    int rc = sort_flip(ctx);
-    if (rc != M3DK_OK) return rc;
-    return settle(ctx);
+    {
+        EvScope ev(ctx, &ctx->ev_sort);
+        CU(launch_pack_sorted(ctx, ctx->n), "sort kernels (pack)");
+        CU(launch_unpack(ctx, ctx->n), "sort kernels (unpack)");
+    }
+    ctx->n_sorts++;
+    ctx->steps_since_sort = 0;
+    return M3DK_OK;
 }
 
 extern "C" int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt) {
@@ -451,24 +428,46 @@ extern "C" int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt) {
         return fail(ctx, M3DK_ESTATE, "m3dk_push: sort_interval > 0 needs m3dk_set_sort_workspace");
     CU(cudaSetDevice(ctx->device), "cudaSetDevice");
     ctx->last_dt = dt;
-    for (int l = 0; l < nsteps; ++l) {
-        if (ctx->sort_interval > 0 && ctx->steps_since_sort >= ctx->sort_interval && ctx->n > 0) {
-            int rc = sort_flip(ctx);
-            if (rc != M3DK_OK) return rc;
-        }
-        const double t = ctx->t0 + (double)ctx->steps_done * dt;   // t_l of this step's x_l
-        {
-            // when the next step starts with a sort, this push also histograms its new keys (a11 fused into a10)
-            const bool with_hist = ctx->sort_interval > 0 && ctx->steps_since_sort + 1 >= ctx->sort_interval && ctx->n > 0;
+    const int k = ctx->sort_interval;
+    if (k == 0 || ctx->n == 0 || nsteps == 0) {
+        for (int l = 0; l < nsteps; ++l) {
+            const double t = ctx->t0 + (double)ctx->steps_done * dt;   // t_l of this step's x_l
             EvScope ev(ctx, &ctx->ev_push);
-            CU(launch_push(ctx, cur_arrays(ctx), ctx->n, dt, t, with_hist, ctx->items_valid), "push kernel");
-            ctx->hist_valid = with_hist;
-            ctx->items_valid = false;    // the markers have moved: the order is stale until the next sort
+            CU(launch_push_soa(ctx, ctx->n, dt, t), "push kernel");
+            ctx->steps_done++;
         }
+        return M3DK_OK;
+    }
+    {
+        EvScope ev(ctx, &ctx->ev_sort);
+        CU(launch_pack_sorted(ctx, ctx->n), "sort kernels (pack)");
+    }
+    ctx->n_sorts++;
+    ctx->steps_since_sort = 0;
+    bool ordered = true;     // the records are in element order and sb.items cut them
+    for (int l = 0; l < nsteps; ++l) {
+        const double t = ctx->t0 + (double)ctx->steps_done * dt;
+        const bool reorder_after = l + 1 < nsteps && ctx->steps_since_sort + 1 >= k;
+        {
+            EvScope ev(ctx, &ctx->ev_push);
+            CU(launch_push_rec(ctx, ctx->n, dt, t, reorder_after, ordered), "push kernel");
+        }
+        ordered = false;     // the markers have moved
         ctx->steps_done++;
         ctx->steps_since_sort++;
+        if (reorder_after) {
+            EvScope ev(ctx, &ctx->ev_sort);
+            CU(launch_reorder(ctx, ctx->n), "sort kernels (reorder)");
+            ctx->n_sorts++;
+            ctx->steps_since_sort = 0;
+            ordered = true;
+        }
     }
-    return settle(ctx);
+    {
+        EvScope ev(ctx, &ctx->ev_sort);
+        CU(launch_unpack(ctx, ctx->n), "sort kernels (unpack)");
+    }
+    return M3DK_OK;
 }
 
 extern "C" int m3dk_stats(m3dk_ctx *ctx, m3dk_stats_t *out) {
@@ -501,9 +500,6 @@ extern "C" int m3dk_particles_upload(m3dk_ctx *ctx, const double *hx, const doub
     const double *const hs[8] = {hx, hy, hz, hvx, hvy, hvz, hmu, hw};
     double *const dd[8] = {d.x, d.y, d.z, d.vx, d.vy, d.vz, d.mu, d.w};
     for (int k = 0; k < 8; ++k) CU(cudaMemcpyAsync(dd[k], hs[k], nd, cudaMemcpyHostToDevice, ctx->stream), "upload markers");
-    ctx->cur = 0;
-    ctx->hist_valid = false;
-    ctx->items_valid = false;
     ctx->steps_since_sort = ctx->sort_interval;
     CU(launch_locate(ctx, ctx->user, ctx->n, true), "locate kernel");
     return M3DK_OK;

@@ -76,9 +76,22 @@ struct MarkerArrays {
     int *elem, *id;
 };
 
+// Marker record of the ordered pipeline: 64 bytes = two 32-byte sectors, fields (x, y, z, w | vx, vy, vz, mu).
+// Records are gathered / written with 256-bit accesses: a marker is two full sectors wherever it lands, which is what
+// makes re-ordering every step affordable (an 8-byte SoA scatter costs a 32-byte sector and an L1 wavefront per field).
+constexpr int kRecDoubles = 8;
+
+struct RecArrays {            // ordered pipeline, carved from the sort workspace
+    const double *in;        // records of this step's input  [n][8]
+    double *out;             // records of this step's output [n][8] (== in for the in-place generic kernel)
+    const int2 *order;       // [n] (src, id): output slot d takes the input record src; id = caller's marker index
+    int *key;                // [n] element of the NEW position of output slot d (n_elems = lost)
+};
+
 struct PushParams {
     long n;
-    MarkerArrays a;
+    MarkerArrays a;          // SoA path (sort_interval = 0)
+    RecArrays rc;            // record path (sort_interval >= 1)
     FieldParams f;
     double dt, h;            // h = q dt / (2 m)
     double q, m, inv_q;
@@ -88,7 +101,6 @@ struct PushParams {
     int *hist, *rank;        // fused sort histogram of the new keys (kHist kernels), else unused
     const int4 *items;       // work items of the element-ordered kernel: (element, first slot, count, -)
     const int *n_items;      // device: number of items
-    int *item_counter;       // device: next item to hand out (zeroed before the launch)
 };
 
 #ifndef M3DK_ITEM_R
@@ -98,7 +110,9 @@ constexpr int kItemR = M3DK_ITEM_R;              // markers per lane in the elem
 constexpr int kItemMarkers = 32 * kItemR;        // markers per work item
 
 struct SortBuffers {         // carved from the sort workspace
-    MarkerArrays alt;        // second set of marker arrays (ping-pong partner of the caller's)
+    double *rec[2];          // [n][8] record ping-pong
+    int2 *order[2];          // [n] (src, id) ping-pong: order[k][d].y is also the id of the record in slot d
+    int *key;                // [n]
     int *rank;               // [n]
     int *hist;               // [n_elems + 2]
     int *offs;               // [n_elems + 2]
@@ -120,8 +134,9 @@ struct m3dk_ctx {
     // markers
     bool have_markers = false;
     long n = 0;
-    m3dk::MarkerArrays user{};   // caller's arrays
-    int cur = 0;                 // 0: state lives in `user`, 1: in sb.alt (only transiently inside push / sort)
+    m3dk::MarkerArrays user{};   // caller's arrays (the state lives here between calls)
+    int cur = 0;                 // record buffer that holds the state inside an ordered push / sort
+    int ocur = 0;                // order buffer whose .y are the ids of the records in sb.rec[cur]
     double q = 1.0, m = 1.0;
     m3dk_f0_params f0{};
     // options / clock
@@ -134,8 +149,6 @@ struct m3dk_ctx {
     double last_dt = 0.0;
     // sort workspace
     bool have_sortws = false;
-    bool items_valid = false;    // sb.items cut the CURRENT arrays, which are sorted by element (set by a sort, cleared by a push)
-    bool hist_valid = false;     // sb.hist / sb.rank describe the keys of the current arrays (filled by the last push)
     m3dk::SortBuffers sb{};
     int *d_count = nullptr;      // small device scratch inside the fields workspace (lost counter etc.)
     // profiling (m3dk_set_profiling / m3dk_timing)
@@ -149,11 +162,14 @@ namespace m3dk {
 
 // launchers (defined in push.cu / sort.cu); all enqueue on ctx->stream and return cudaGetLastError()
 cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_id);
-cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t, bool with_hist, bool use_items);
+cudaError_t launch_push_soa(m3dk_ctx *c, long n, double dt, double t);                           // caller's arrays, any order
+cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_hist, bool use_items);   // records
 cudaError_t launch_eval_fields(m3dk_ctx *c, long n, const double *R, const double *phi, const double *Z, double t,
                                int *elem_out, double *out);
 cudaError_t launch_count_lost(m3dk_ctx *c, const MarkerArrays &a, long n, int *d_count);
-cudaError_t launch_sort(m3dk_ctx *c, const MarkerArrays &src, const MarkerArrays &dst, long n, bool have_hist);
+cudaError_t launch_pack_sorted(m3dk_ctx *c, long n);     // caller's arrays -> records in element order, items cut
+cudaError_t launch_reorder(m3dk_ctx *c, long n);         // histogram of the last push -> offsets, items, next order
+cudaError_t launch_unpack(m3dk_ctx *c, long n);          // records -> caller's arrays (+ elem, id)
 cudaError_t fp64_probe(m3dk_ctx *c, double *tflops);
 
 size_t sort_workspace_bytes(long n, int n_elems);

@@ -62,21 +62,69 @@ __device__ __forceinline__ void hist_rank_R(int *hist, int *rank, const int (&ke
         }
 }
 
-// ---- one step of R markers of one thread that sit in the same element e (rows a1-a10) -------------------------------
-// m[r]: slot of marker r in the SoA arrays, on[r]: marker r exists.  Phase A: a1 load, a2 cylindrical map, a4-a5
-// equilibrium quad (every coefficient load shared by the R markers), a7 assemble, a8 Boris, a10 drift + store, a3 for
-// the NEW position (cached for the next step; it is the sort key) and, with kHist, the sort histogram of the new keys.
-// Phase B: a6 perturbed quads folded into dw/dt as they are evaluated, a9 weight update.
+// ---- marker state access: the caller's SoA arrays (any order, in place) or 64-byte records (ordered pipeline) -------
+__device__ __forceinline__ void ldrec256(const double *p, double &a, double &b, double &c, double &d) {
+    asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void strec256(double *p, double a, double b, double c, double d) {
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
+struct SoAIO {
+    MarkerArrays a;
+    int n_elems;
+    __device__ __forceinline__ void load_pos(long i, double &x, double &y, double &z, double &w) const {
+        x = a.x[i]; y = a.y[i]; z = a.z[i]; w = a.w[i];
+    }
+    __device__ __forceinline__ void load_vel(long i, double &vx, double &vy, double &vz, double &mu) const {
+        vx = a.vx[i]; vy = a.vy[i]; vz = a.vz[i]; mu = a.mu[i];
+    }
+    __device__ __forceinline__ void store_pos(long o, double x, double y, double z, double) const {
+        a.x[o] = x; a.y[o] = y; a.z[o] = z;
+    }
+    __device__ __forceinline__ void store_vel(long o, double vx, double vy, double vz, double) const {
+        a.vx[o] = vx; a.vy[o] = vy; a.vz[o] = vz;          // mu is never written
+    }
+    __device__ __forceinline__ void store_w(long o, double w) const { a.w[o] = w; }
+    __device__ __forceinline__ void store_key(long o, int ne) const { a.elem[o] = ne; }
+};
+
+struct RecIO {   // record = (x, y, z, w | vx, vy, vz, mu): two 32-byte sectors, each moved by one 256-bit access
+    const double *in;
+    double *out;
+    int *key;
+    int n_elems;
+    __device__ __forceinline__ void load_pos(long i, double &x, double &y, double &z, double &w) const {
+        ldrec256(in + kRecDoubles * i, x, y, z, w);
+    }
+    __device__ __forceinline__ void load_vel(long i, double &vx, double &vy, double &vz, double &mu) const {
+        ldrec256(in + kRecDoubles * i + 4, vx, vy, vz, mu);
+    }
+    __device__ __forceinline__ void store_pos(long o, double x, double y, double z, double w_old) const {
+        strec256(out + kRecDoubles * o, x, y, z, w_old);      // w is patched by store_w once phase B has it
+    }
+    __device__ __forceinline__ void store_vel(long o, double vx, double vy, double vz, double mu) const {
+        strec256(out + kRecDoubles * o + 4, vx, vy, vz, mu);
+    }
+    __device__ __forceinline__ void store_w(long o, double w) const { out[kRecDoubles * o + 3] = w; }
+    __device__ __forceinline__ void store_key(long o, int ne) const { key[o] = ne < 0 ? n_elems : ne; }
+};
+
+// ---- one step of R markers of one thread that sit in the same element (rows a1-a10) ------------------------------
+// mi[r] / mo[r]: input / output slot of marker r, on[r]: marker r exists.  Phase A: a1 load, a2 cylindrical map, a4-a5
+// equilibrium quad (every coefficient load shared by the R markers), a7 assemble, a8 Boris, a10 drift + store.
+// Phase B: a6 perturbed quads folded into dw/dt as they are evaluated, a9 weight update.  Then a3 for the NEW position
+// (cached for the next step; it is the sort key) and, with kHist, the sort histogram of the new keys.
 // tile: the element's coefficient tile, in global memory (kSmem = false) or staged in shared memory (kSmem = true).
-template <int R, bool kHist, bool kSmem>
-__device__ __forceinline__ void step_R(const PushParams &P, const double *__restrict__ tile, const long (&m)[R],
-                                       const bool (&on)[R]) {
+template <int R, bool kHist, bool kSmem, class IO>
+__device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const double *__restrict__ tile,
+                                       const long (&mi)[R], const long (&mo)[R], const bool (&on)[R]) {
     Marker s[R];
     StepGeom g[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        if (on[r]) { s[r].x = P.a.x[m[r]]; s[r].y = P.a.y[m[r]]; s[r].z = P.a.z[m[r]]; }
-        else { s[r].x = 1.0; s[r].y = 0.0; s[r].z = 0.0; }
+        if (on[r]) io.load_pos(mi[r], s[r].x, s[r].y, s[r].z, s[r].w);
+        else { s[r].x = 1.0; s[r].y = 0.0; s[r].z = 0.0; s[r].w = 0.0; }
     }
     const Quad hd = ldq_t<kSmem>(tile);
     const double Rc = hd.a, Zc = hd.b, se = hd.c;
@@ -98,13 +146,12 @@ __device__ __forceinline__ void step_R(const PushParams &P, const double *__rest
         f.psi_R = __dmul_rn(dx[r][0], se); f.psi_Z = __dmul_rn(de[r][0], se);
         f.Bm = v[r][1]; f.Bm_R = __dmul_rn(dx[r][1], se); f.Bm_Z = __dmul_rn(de[r][1], se);
         f.F = v[r][2]; f.kappa = v[r][3];
-        if (on[r]) {
-            s[r].vx = P.a.vx[m[r]]; s[r].vy = P.a.vy[m[r]]; s[r].vz = P.a.vz[m[r]]; s[r].mu = P.a.mu[m[r]];
-        } else { s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
+        if (on[r]) io.load_vel(mi[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
+        else { s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
         push_eq(P, g[r], f, s[r], W[r]);
         if (on[r]) {
-            P.a.x[m[r]] = s[r].x; P.a.y[m[r]] = s[r].y; P.a.z[m[r]] = s[r].z;
-            P.a.vx[m[r]] = s[r].vx; P.a.vy[m[r]] = s[r].vy; P.a.vz[m[r]] = s[r].vz;
+            io.store_pos(mo[r], s[r].x, s[r].y, s[r].z, s[r].w);
+            io.store_vel(mo[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
         }
         // the element search of the new position runs after phase B; its first record starts travelling now
         Rn[r] = __dsqrt_rn(M3DK_FMA(s[r].x, s[r].x, __dmul_rn(s[r].y, s[r].y)));
@@ -112,9 +159,9 @@ __device__ __forceinline__ void step_R(const PushParams &P, const double *__rest
         locate_prefetch(P.f.fast, Rn[r], Zn[r]);
     }
     if (P.f.n_modes > 0) {
-        double wsum[R], w0[R];
+        double wsum[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) { wsum[r] = 0.0; w0[r] = on[r] ? P.a.w[m[r]] : 0.0; }
+        for (int r = 0; r < R; ++r) wsum[r] = 0.0;
         for (int md = 0; md < P.f.n_modes; ++md) {
             const int n = P.f.n_tor[md];
             const double om = P.f.omega[md];
@@ -145,7 +192,7 @@ __device__ __forceinline__ void step_R(const PushParams &P, const double *__rest
         // Eqs. (8)-(9): explicit midpoint on the staggered grid (G9)
 #pragma unroll
         for (int r = 0; r < R; ++r)
-            if (on[r]) P.a.w[m[r]] = M3DK_FMA(P.dt, wsum[r], w0[r]);
+            if (on[r]) io.store_w(mo[r], M3DK_FMA(P.dt, wsum[r], s[r].w));
     }
     // a3 for the NEW position (the key of the next sort) and, with kHist, the sort histogram of the new keys with each
     // marker's rank inside its key: the sort then needs no pass over the keys
@@ -158,35 +205,37 @@ __device__ __forceinline__ void step_R(const PushParams &P, const double *__rest
         int ne = -1;
         if (on[r]) {
             ne = locate_finish(P.f, rec[r], Rn[r], Zn[r]);
-            P.a.elem[m[r]] = ne;
+            io.store_key(mo[r], ne);
         }
         key[r] = ne < 0 ? P.f.n_elems : ne;
     }
-    if (kHist) hist_rank_R<R>(P.hist, P.rank, key, m, on);
+    if (kHist) hist_rank_R<R>(P.hist, P.rank, key, mo, on);
 }
 
 // ---- generic push: one marker per thread, any marker order (every thread gathers its own element's tile) ------------
-template <bool kHist>
+// kRec = false: the caller's SoA arrays in place (sort_interval = 0).  kRec = true: the records of the ordered pipeline
+// in place, for the steps between two sorts when sort_interval > 1.
+template <bool kRec, bool kHist>
 __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant__ PushParams P) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < P.n;
-    const int e = valid ? P.a.elem[i] : -1;
+    int e = -1;
+    if (valid) { e = kRec ? P.rc.key[i] : P.a.elem[i]; if (kRec && e >= P.f.n_elems) e = -1; }
     const long m[1] = {i};
     const bool on[1] = {e >= 0};             // lost markers are frozen (G12)
     // the tile loads may be speculated above the `on` tests: e is clamped to a valid element for addressing
-    if (__any_sync(0xffffffffu, on[0])) step_R<1, false, false>(P, P.f.tiles + (size_t)max(e, 0) * P.f.tile_stride, m, on);
+    const double *tile = P.f.tiles + (size_t)max(e, 0) * P.f.tile_stride;
+    if (__any_sync(0xffffffffu, on[0])) {
+        if (kRec) { const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems}; step_R<1, false, false>(P, io, tile, m, m, on); }
+        else { const SoAIO io{P.a, P.f.n_elems}; step_R<1, false, false>(P, io, tile, m, m, on); }
+    }
     if (kHist) {
-        const int ne = valid ? P.a.elem[i] : -1;
-        const int rk = hist_rank(P.hist, ne < 0 ? P.f.n_elems : ne, valid);
+        const int k = valid ? P.rc.key[i] : 0;
+        const int rk = hist_rank(P.hist, k, valid);
         if (valid) P.rank[i] = rk;
     }
 }
 
-// ---- element-ordered push: the marker stream is sorted by element and cut into work items --------------------------
-// A work item is up to kItemMarkers = 32 kItemR consecutive markers of ONE element; a warp takes an item, every lane up to
-// kItemR of its markers (slots lane, lane + 32, ...), so that each 32-byte coefficient load is a one-wavefront broadcast
-// that feeds kItemR markers per lane.  Persistent warps draw items from an atomic counter.  Items of the pseudo-element n_elems hold the lost
-// markers: they are frozen and only enter the histogram.
 // ---- tile staging: one bulk copy (TMA, cp.async.bulk) per item into the warp's double buffer, mbarrier completion --
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned bar) {
@@ -200,18 +249,6 @@ __device__ __forceinline__ void tile_copy_issue(unsigned dst, const double *src,
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
     asm volatile("{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @!p bra WAIT_%=;\n}"
                  ::"r"(bar), "r"(parity) : "memory");
-}
-
-// Lines of the next item's marker state (8 arrays x at most 5 lines of 128 B), one L2 prefetch per lane: they travel
-// while the current item computes.
-__device__ __forceinline__ void prefetch_state(const PushParams &P, int start) {
-    const int lane = threadIdx.x & 31;
-    const double *const arr[8] = {P.a.x, P.a.y, P.a.z, P.a.vx, P.a.vy, P.a.vz, P.a.mu, P.a.w};
-    const double *base = arr[lane >> 2] + (start & ~15);
-    constexpr int kLines = (kItemMarkers * 8 + 127) / 128 + 1;
-#pragma unroll
-    for (int j = 0; j < (kLines + 3) / 4; ++j)
-        if (4 * j + (lane & 3) < kLines) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + 16 * (4 * j + (lane & 3))));
 }
 
 // ---- element-ordered push: the marker stream is sorted by element and cut into work items --------------------------
@@ -252,25 +289,32 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
             __syncwarp();                              // every lane has finished reading buffer b ^ 1 (previous item)
             if (w.x < P.f.n_elems && lane == 0)
                 tile_copy_issue(buf0 + (b ^ 1) * tile_bytes, P.f.tiles + (size_t)w.x * stride_d, tile_bytes, bar0 + (b ^ 1) * 8);
-            prefetch_state(P, w.y);
         }
-        if (e >= P.f.n_elems) {                        // lost markers: frozen (G12), counted for the next sort
-            if (kHist) {
-#pragma unroll 1
-                for (int k = lane; k < ((count + 31) & ~31); k += 32) {
-                    const bool onk = k < count;
-                    const int rk = hist_rank(P.hist, P.f.n_elems, onk);
-                    if (onk) P.rank[start + k] = rk;
+        long mi[kItemR], mo[kItemR];
+        bool on[kItemR];
+#pragma unroll
+        for (int r = 0; r < kItemR; ++r) {
+            mo[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count;
+            mi[r] = on[r] ? P.rc.order[mo[r]].x : 0;   // the record that belongs in this slot
+        }
+        const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems};
+        if (e >= P.f.n_elems) {                        // lost markers: frozen (G12), moved along and counted for the next sort
+            int key[kItemR];
+#pragma unroll
+            for (int r = 0; r < kItemR; ++r) {
+                key[r] = P.f.n_elems;
+                if (on[r]) {
+                    double a0, a1, a2, a3, b0, b1, b2, b3;
+                    io.load_pos(mi[r], a0, a1, a2, a3); io.load_vel(mi[r], b0, b1, b2, b3);
+                    io.store_pos(mo[r], a0, a1, a2, a3); io.store_vel(mo[r], b0, b1, b2, b3);
+                    io.store_key(mo[r], -1);
                 }
             }
+            if (kHist) hist_rank_R<kItemR>(P.hist, P.rank, key, mo, on);
         } else {
-            long m[kItemR];
-            bool on[kItemR];
-#pragma unroll
-            for (int r = 0; r < kItemR; ++r) { m[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count; }
             mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
             phase ^= 1u << b;
-            step_R<kItemR, kHist, true>(P, tbuf + (size_t)b * stride_d, m, on);
+            step_R<kItemR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
         }
         b ^= 1;
     }
@@ -347,29 +391,42 @@ cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_
     return cudaGetLastError();
 }
 
-cudaError_t launch_push(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t, bool with_hist, bool use_items) {
+cudaError_t launch_push_soa(m3dk_ctx *c, long n, double dt, double t) {
     if (n == 0) return cudaSuccess;
-    PushParams P = make_params(c, a, n, dt, t);
+    PushParams P = make_params(c, c->user, n, dt, t);
     c->kernel_launches += 1;
+    push_generic_kernel<false, false><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
+    return cudaGetLastError();
+}
+
+// One step on the records: element-ordered (use_items: sb.rec[cur] gathered through sb.order[ocur] into sb.rec[cur ^ 1],
+// which becomes current) or in place.  with_hist: also histogram the new keys for the reorder that follows.
+cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_hist, bool use_items) {
+    if (n == 0) return cudaSuccess;
+    PushParams P = make_params(c, c->user, n, dt, t);
+    c->kernel_launches += 1;
+    P.hist = c->sb.hist; P.rank = c->sb.rank;
+    P.rc.key = c->sb.key; P.rc.order = c->sb.order[c->ocur];
+    P.rc.in = c->sb.rec[c->cur];
     if (with_hist) {
-        P.hist = c->sb.hist; P.rank = c->sb.rank;
         cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
         if (e != cudaSuccess) return e;
     }
     if (use_items) {
-        P.items = c->sb.items; P.n_items = c->sb.ioffs + c->f.n_elems + 1; P.item_counter = c->d_count + 1;
-        cudaError_t e = cudaMemsetAsync(c->d_count + 1, 0, sizeof(int), c->stream);
-        if (e != cudaSuccess) return e;
+        P.rc.out = c->sb.rec[c->cur ^ 1];
+        P.items = c->sb.items; P.n_items = c->sb.ioffs + c->f.n_elems + 1;
         const unsigned grid = (unsigned)(c->sm_count * M3DK_PUSH_MINBLOCKS);
         const size_t smem = (size_t)(kPushThreads / 32) * 2 * (c->f.tile_stride * 8 + 8);
         auto kern = with_hist ? push_items_kernel<true> : push_items_kernel<false>;
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         kern<<<grid, kPushThreads, smem, c->stream>>>(P);
+        c->cur ^= 1;
     } else {
+        P.rc.out = c->sb.rec[c->cur];
         const unsigned grid = (unsigned)((n + 127) / 128);
-        if (with_hist) push_generic_kernel<true><<<grid, 128, 0, c->stream>>>(P);
-        else push_generic_kernel<false><<<grid, 128, 0, c->stream>>>(P);
+        if (with_hist) push_generic_kernel<true, true><<<grid, 128, 0, c->stream>>>(P);
+        else push_generic_kernel<true, false><<<grid, 128, 0, c->stream>>>(P);
     }
     return cudaGetLastError();
 }

@@ -1,6 +1,9 @@
-// m3dk_sort.cu -- counting sort of the markers by element.
+// m3dk_sort.cu -- ordering of the markers by element and the record pipeline around it.
 // key = element of the marker's current position (cached by the push), lost markers (-1) get key n_elems (last).
-// histogram with returned ranks (one atomic per marker) -> exclusive scan -> scatter of the 8 fp64 arrays + elem + id.
+// Counting sort: histogram with returned ranks (one warp-aggregated atomic per marker; normally fused into the push
+// kernel that produced the keys) -> exclusive scan (+ work-item cut) -> placement.  The placement never moves SoA
+// pieces: markers travel as 64-byte records (two full sectors), and inside a push the records are not moved by a sort
+// pass at all -- the next push gathers them through the (src, id) order list written here.
 #include "m3dk_internal.h"
 
 namespace m3dk {
@@ -8,20 +11,19 @@ namespace m3dk {
 static inline size_t up256(size_t b) { return (b + 255) / 256 * 256; }
 
 size_t sort_workspace_bytes(long n, int n_elems) {
-    const size_t nd = up256((size_t)n * sizeof(double)), ni = up256((size_t)n * sizeof(int));
-    const size_t nh = up256((size_t)(n_elems + 2) * sizeof(int));
+    const size_t nr = up256((size_t)n * kRecDoubles * sizeof(double)), no = up256((size_t)n * sizeof(int2));
+    const size_t ni = up256((size_t)n * sizeof(int)), nh = up256((size_t)(n_elems + 2) * sizeof(int));
     const size_t nit = up256(((size_t)n / kItemMarkers + n_elems + 2) * sizeof(int4));
-    return 8 * nd + 3 * ni + 3 * nh + nit;
+    return 2 * nr + 2 * no + 2 * ni + 3 * nh + nit;
 }
 
 void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb) {
     char *p = static_cast<char *>(ws);
-    const size_t nd = up256((size_t)n * sizeof(double)), ni = up256((size_t)n * sizeof(int));
-    const size_t nh = up256((size_t)(n_elems + 2) * sizeof(int));
-    double **d[8] = {&sb->alt.x, &sb->alt.y, &sb->alt.z, &sb->alt.vx, &sb->alt.vy, &sb->alt.vz, &sb->alt.mu, &sb->alt.w};
-    for (auto q : d) { *q = reinterpret_cast<double *>(p); p += nd; }
-    sb->alt.elem = reinterpret_cast<int *>(p); p += ni;
-    sb->alt.id = reinterpret_cast<int *>(p); p += ni;
+    const size_t nr = up256((size_t)n * kRecDoubles * sizeof(double)), no = up256((size_t)n * sizeof(int2));
+    const size_t ni = up256((size_t)n * sizeof(int)), nh = up256((size_t)(n_elems + 2) * sizeof(int));
+    for (int k = 0; k < 2; ++k) { sb->rec[k] = reinterpret_cast<double *>(p); p += nr; }
+    for (int k = 0; k < 2; ++k) { sb->order[k] = reinterpret_cast<int2 *>(p); p += no; }
+    sb->key = reinterpret_cast<int *>(p); p += ni;
     sb->rank = reinterpret_cast<int *>(p); p += ni;
     sb->hist = reinterpret_cast<int *>(p); p += nh;
     sb->offs = reinterpret_cast<int *>(p); p += nh;
@@ -110,33 +112,94 @@ __global__ void __launch_bounds__(256) items_kernel(const int *__restrict__ offs
     for (int c = 0; c < cnt; c += kItemMarkers, ++j) items[j] = make_int4(k, b + c, min(kItemMarkers, cnt - c), 0);
 }
 
-__global__ void __launch_bounds__(256) scatter_kernel(MarkerArrays s, MarkerArrays d, long n, int n_elems,
-                                                      const int *__restrict__ offs, const int *__restrict__ rank) {
-    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const int e = s.elem[i];
-    const long j = (long)offs[e < 0 ? n_elems : e] + rank[i];
-    d.x[j] = s.x[i]; d.y[j] = s.y[i]; d.z[j] = s.z[i];
-    d.vx[j] = s.vx[i]; d.vy[j] = s.vy[i]; d.vz[j] = s.vz[i];
-    d.mu[j] = s.mu[i]; d.w[j] = s.w[i];
-    d.elem[j] = e; d.id[j] = s.id[i];
+__device__ __forceinline__ void st256(double *p, double a, double b, double c, double d) {
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+__device__ __forceinline__ void ld256(const double *p, double &a, double &b, double &c, double &d) {
+    asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p) : "memory");
 }
 
-cudaError_t launch_sort(m3dk_ctx *c, const MarkerArrays &src, const MarkerArrays &dst, long n, bool have_hist) {
+// caller's SoA arrays -> records in element order: slot d = offs[key] + rank; order[d] = (d, id): the first push of the
+// call reads its records in place
+__global__ void __launch_bounds__(256) pack_kernel(MarkerArrays a, long n, int n_elems, const int *__restrict__ offs,
+                                                   const int *__restrict__ rank, double *__restrict__ rec,
+                                                   int2 *__restrict__ order, int *__restrict__ key) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int e = a.elem[i];
+    const int k = e < 0 ? n_elems : e;
+    const long d = (long)offs[k] + rank[i];
+    st256(rec + kRecDoubles * d, a.x[i], a.y[i], a.z[i], a.w[i]);
+    st256(rec + kRecDoubles * d + 4, a.vx[i], a.vy[i], a.vz[i], a.mu[i]);
+    order[d] = make_int2((int)d, a.id[i]);
+    key[d] = k;
+}
+
+// next order list: the record in slot j goes to slot d = offs[key[j]] + rank[j] of the next element-ordered push
+__global__ void __launch_bounds__(256) invert_kernel(long n, const int *__restrict__ key, const int *__restrict__ offs,
+                                                     const int *__restrict__ rank, const int2 *__restrict__ order_cur,
+                                                     int2 *__restrict__ order_next) {
+    const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const long d = (long)offs[key[j]] + rank[j];
+    order_next[d] = make_int2((int)j, order_cur[j].y);
+}
+
+// records -> caller's SoA arrays, slot by slot (the caller's arrays end up in the record order; id says who is where)
+__global__ void __launch_bounds__(256) unpack_kernel(MarkerArrays a, long n, int n_elems, const double *__restrict__ rec,
+                                                     const int2 *__restrict__ order, const int *__restrict__ key) {
+    const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    double x, y, z, w, vx, vy, vz, mu;
+    ld256(rec + kRecDoubles * j, x, y, z, w);
+    ld256(rec + kRecDoubles * j + 4, vx, vy, vz, mu);
+    a.x[j] = x; a.y[j] = y; a.z[j] = z; a.w[j] = w;
+    a.vx[j] = vx; a.vy[j] = vy; a.vz[j] = vz; a.mu[j] = mu;
+    a.id[j] = order[j].y;
+    const int k = key[j];
+    a.elem[j] = k >= n_elems ? -1 : k;
+}
+
+static cudaError_t scan_and_cut(m3dk_ctx *c) {
+    const int m = c->f.n_elems + 1;
+    c->kernel_launches += 2;
+    scan_kernel<<<1, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs, c->sb.ioffs);
+    items_kernel<<<(m + 255) / 256, 256, 0, c->stream>>>(c->sb.offs, c->sb.ioffs, m, c->sb.items);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pack_sorted(m3dk_ctx *c, long n) {
     if (n == 0) return cudaSuccess;
     const int m = c->f.n_elems + 1;
     const unsigned grid = (unsigned)((n + 255) / 256);
-    if (!have_hist) {   // otherwise the push kernel that produced these keys has filled hist and rank already
-        cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)m * sizeof(int), c->stream);
-        if (e != cudaSuccess) return e;
-        c->kernel_launches += 1;
-        hist_rank_kernel<<<grid, 256, 0, c->stream>>>(src.elem, n, c->f.n_elems, c->sb.hist, c->sb.rank);
-    }
+    cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)m * sizeof(int), c->stream);
+    if (e != cudaSuccess) return e;
     c->kernel_launches += 2;
-    scan_kernel<<<1, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs, c->sb.ioffs);
+    hist_rank_kernel<<<grid, 256, 0, c->stream>>>(c->user.elem, n, c->f.n_elems, c->sb.hist, c->sb.rank);
+    e = scan_and_cut(c);
+    if (e != cudaSuccess) return e;
+    c->cur = 0; c->ocur = 0;
+    pack_kernel<<<grid, 256, 0, c->stream>>>(c->user, n, c->f.n_elems, c->sb.offs, c->sb.rank, c->sb.rec[0], c->sb.order[0],
+                                            c->sb.key);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_reorder(m3dk_ctx *c, long n) {
+    if (n == 0) return cudaSuccess;
+    cudaError_t e = scan_and_cut(c);
+    if (e != cudaSuccess) return e;
     c->kernel_launches += 1;
-    items_kernel<<<(m + 255) / 256, 256, 0, c->stream>>>(c->sb.offs, c->sb.ioffs, m, c->sb.items);
-    scatter_kernel<<<grid, 256, 0, c->stream>>>(src, dst, n, c->f.n_elems, c->sb.offs, c->sb.rank);
+    invert_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, c->sb.key, c->sb.offs, c->sb.rank,
+                                                                       c->sb.order[c->ocur], c->sb.order[c->ocur ^ 1]);
+    c->ocur ^= 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_unpack(m3dk_ctx *c, long n) {
+    if (n == 0) return cudaSuccess;
+    c->kernel_launches += 1;
+    unpack_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->user, n, c->f.n_elems, c->sb.rec[c->cur],
+                                                                       c->sb.order[c->ocur], c->sb.key);
     return cudaGetLastError();
 }
 
