@@ -13,6 +13,35 @@ namespace m3dk {
 #define M3DK_FMA(a, b, c) fma((a), (b), (c))
 #endif
 
+// ---- reciprocal, reciprocal square root, square root: hardware seed (MUFU.RCP64H / RSQ64H, ~20 bits) + two Newton
+// steps, ~1 ulp.  fp64 division and square root have no hardware unit; the IEEE-rounded library sequences cost about
+// three times as many FP64-pipe instructions plus a slow-path branch, and a step has seven of them.  The parity bar is
+// 1e-12, four orders above the difference.  Arguments are positive and normal wherever these are used (R >= R_min > 0,
+// |B|^2 > 0, 1 + t^2 >= 1, v^3 + v_c^3 > 0); m3dk_sqrt also accepts 0.
+__device__ __forceinline__ double m3dk_rcp(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = M3DK_FMA(-x, y, 1.0);
+    y = M3DK_FMA(y, e, y);
+    e = M3DK_FMA(-x, y, 1.0);
+    return M3DK_FMA(y, e, y);
+}
+__device__ __forceinline__ double m3dk_rsqrt(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double hx = __dmul_rn(0.5, x);
+    double e = M3DK_FMA(-__dmul_rn(hx, y), y, 0.5);
+    y = M3DK_FMA(y, e, y);
+    e = M3DK_FMA(-__dmul_rn(hx, y), y, 0.5);
+    return M3DK_FMA(y, e, y);
+}
+__device__ __forceinline__ double m3dk_sqrt(double x) {
+    const double y = m3dk_rsqrt(x);
+    const double s = __dmul_rn(x, y);
+    const double r = M3DK_FMA(M3DK_FMA(-s, s, x), __dmul_rn(0.5, y), s);
+    return x > 0.0 ? r : 0.0;
+}
+
 struct Fields {
     double psi_R, psi_Z;        // d psi0/dR, d psi0/dZ
     double Bm, Bm_R, Bm_Z;      // |B|0 as its own scalar field and its gradient
@@ -266,12 +295,13 @@ __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double 
 // d ln f0 / dE at fixed (P_phi, mu) (G7)
 __device__ __forceinline__ double kappa_E(const PushParams &P, double Ekin, double mu) {
     if (P.f0kind == M3DK_F0_MAXWELLIAN) return -P.f0T_inv;
-    const double v = __dsqrt_rn(__ddiv_rn(__dmul_rn(2.0, Ekin), P.m));
+    const double v = m3dk_sqrt(__dmul_rn(__dmul_rn(2.0, Ekin), P.inv_m));
     const double v3 = __dmul_rn(__dmul_rn(v, v), v);
-    double kE = __ddiv_rn(__dmul_rn(-3.0, v), __dmul_rn(P.m, __dadd_rn(v3, P.f0vc3)));
+    double kE = __dmul_rn(__dmul_rn(-3.0, v), m3dk_rcp(__dmul_rn(P.m, __dadd_rn(v3, P.f0vc3))));
     if (P.f0kind == M3DK_F0_BEAM_PITCH) {
-        const double Lam = __ddiv_rn(__dmul_rn(mu, P.f0Bax), Ekin);
-        kE = __dadd_rn(kE, __ddiv_rn(__dmul_rn(__dmul_rn(__dmul_rn(2.0, __dsub_rn(Lam, P.f0L0)), Lam), P.f0dL2_inv), Ekin));
+        const double Einv = m3dk_rcp(Ekin);
+        const double Lam = __dmul_rn(__dmul_rn(mu, P.f0Bax), Einv);
+        kE = __dadd_rn(kE, __dmul_rn(__dmul_rn(__dmul_rn(__dmul_rn(2.0, __dsub_rn(Lam, P.f0L0)), Lam), P.f0dL2_inv), Einv));
     }
     return kE;
 }
@@ -284,8 +314,9 @@ struct StepGeom { double R, rinv, cph, sph; };
 
 // cylindrical map (G3)
 __device__ __forceinline__ void step_geometry(const Marker &s, StepGeom &g) {
-    g.R = __dsqrt_rn(M3DK_FMA(s.x, s.x, __dmul_rn(s.y, s.y)));
-    g.rinv = __ddiv_rn(1.0, g.R);
+    const double r2 = M3DK_FMA(s.x, s.x, __dmul_rn(s.y, s.y));
+    g.rinv = m3dk_rsqrt(r2);
+    g.R = __dmul_rn(r2, g.rinv);
     g.cph = __dmul_rn(s.x, g.rinv); g.sph = __dmul_rn(s.y, g.rinv);
 }
 
@@ -320,7 +351,7 @@ __device__ __forceinline__ void push_eq(const PushParams &P, const StepGeom &g, 
     const double h = P.h;
     const double ux = M3DK_FMA(h, Ex, s.vx), uy = M3DK_FMA(h, Ey, s.vy), uz = M3DK_FMA(h, Ez, s.vz);
     const double tx = DM(h, Bx), ty = DM(h, By), tz = DM(h, Bz);
-    const double sc = __ddiv_rn(2.0, DA(1.0, M3DK_FMA(tx, tx, M3DK_FMA(ty, ty, DM(tz, tz)))));
+    const double sc = DM(2.0, m3dk_rcp(DA(1.0, M3DK_FMA(tx, tx, M3DK_FMA(ty, ty, DM(tz, tz))))));
     const double px = DA(ux, M3DK_FMA(uy, tz, -DM(uz, ty))), py = DA(uy, M3DK_FMA(uz, tx, -DM(ux, tz))),
                  pz = DA(uz, M3DK_FMA(ux, ty, -DM(uy, tx)));
     const double wx = M3DK_FMA(sc, M3DK_FMA(py, tz, -DM(pz, ty)), ux), wy = M3DK_FMA(sc, M3DK_FMA(pz, tx, -DM(px, tz)), uy),
@@ -330,7 +361,7 @@ __device__ __forceinline__ void push_eq(const PushParams &P, const StepGeom &g, 
         const double vlx = DM(0.5, DA(s.vx, nvx)), vly = DM(0.5, DA(s.vy, nvy)), vlz = DM(0.5, DA(s.vz, nvz));
         const double vR = M3DK_FMA(vlx, cph, DM(vly, sph)), vP = M3DK_FMA(vly, cph, -DM(vlx, sph)), vZ = vlz;
         const double B2 = M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, DM(BZ, BZ)));
-        const double binv = __ddiv_rn(1.0, __dsqrt_rn(B2));
+        const double binv = m3dk_rsqrt(B2);
         const double b2inv = DM(binv, binv);
         const double bR = DM(BR, binv), bP = DM(BP, binv), bZ = DM(BZ, binv);
         const double vpar = M3DK_FMA(vR, bR, M3DK_FMA(vP, bP, DM(vZ, bZ)));
@@ -391,7 +422,7 @@ __device__ __forceinline__ double pert_fold_par(double wsum, const double (&v)[4
 }
 
 __device__ __forceinline__ int locate_xyz(const FieldParams &f, double x, double y, double z) {
-    return locate_any(f, __dsqrt_rn(M3DK_FMA(x, x, __dmul_rn(y, y))), z);
+    return locate_any(f, m3dk_sqrt(M3DK_FMA(x, x, __dmul_rn(y, y))), z);
 }
 
 }  // namespace m3dk

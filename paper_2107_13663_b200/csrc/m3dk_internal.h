@@ -94,7 +94,7 @@ struct PushParams {
     RecArrays rc;            // record path (sort_interval >= 1)
     FieldParams f;
     double dt, h;            // h = q dt / (2 m)
-    double q, m, inv_q;
+    double q, m, inv_q, inv_m;
     int f0kind;
     double f0T_inv, f0vc3, f0L0, f0dL2_inv, f0Bax;
     double cwt[M3DK_MAX_MODES], swt[M3DK_MAX_MODES];   // cos / sin (omega_k t_l) of this step

@@ -5,11 +5,14 @@
 
 namespace m3dk {
 
+#ifndef M3DK_EARLY_LOCATE
+#define M3DK_EARLY_LOCATE 1
+#endif
 #ifndef M3DK_PUSH_THREADS
 #define M3DK_PUSH_THREADS 128
 #endif
 #ifndef M3DK_PUSH_MINBLOCKS
-#define M3DK_PUSH_MINBLOCKS 4
+#define M3DK_PUSH_MINBLOCKS 3
 #endif
 constexpr int kPushThreads = M3DK_PUSH_THREADS;
 
@@ -140,6 +143,7 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
     quad_vd<R, kSmem>(tile + kTileHeader, tile + kTileHeader, ring, xi, eta, v, dx, de);   // (psi0, |B|0, F0, kappa)
     PertW W[R];
     double Rn[R], Zn[R];
+    FastRec rec[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         EqOut f;
@@ -154,9 +158,13 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
             io.store_vel(mo[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
         }
         // the element search of the new position runs after phase B; its first record starts travelling now
-        Rn[r] = __dsqrt_rn(M3DK_FMA(s[r].x, s[r].x, __dmul_rn(s[r].y, s[r].y)));
+        Rn[r] = m3dk_sqrt(M3DK_FMA(s[r].x, s[r].x, __dmul_rn(s[r].y, s[r].y)));
         Zn[r] = s[r].z;
+#if M3DK_EARLY_LOCATE
+        rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);
+#else
         locate_prefetch(P.f.fast, Rn[r], Zn[r]);
+#endif
     }
     if (P.f.n_modes > 0) {
         double wsum[R];
@@ -196,9 +204,10 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
     }
     // a3 for the NEW position (the key of the next sort) and, with kHist, the sort histogram of the new keys with each
     // marker's rank inside its key: the sort then needs no pass over the keys
-    FastRec rec[R];
+#if !M3DK_EARLY_LOCATE
 #pragma unroll
     for (int r = 0; r < R; ++r) rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);   // all first records in flight together
+#endif
     int key[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -368,7 +377,7 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double *sink, int iters
 static PushParams make_params(m3dk_ctx *c, const MarkerArrays &a, long n, double dt, double t) {
     PushParams P{};
     P.n = n; P.a = a; P.f = c->f;
-    P.dt = dt; P.q = c->q; P.m = c->m; P.inv_q = 1.0 / c->q;
+    P.dt = dt; P.q = c->q; P.m = c->m; P.inv_q = 1.0 / c->q; P.inv_m = 1.0 / c->m;
     P.h = c->q * dt / (2.0 * c->m);
     P.f0kind = c->f0.kind;
     P.f0T_inv = c->f0.kind == M3DK_F0_MAXWELLIAN ? 1.0 / c->f0.T : 0.0;
