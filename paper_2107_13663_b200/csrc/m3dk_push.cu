@@ -8,6 +8,12 @@ namespace m3dk {
 #ifndef M3DK_EARLY_LOCATE
 #define M3DK_EARLY_LOCATE 1
 #endif
+#ifndef M3DK_MID_LOCATE
+#define M3DK_MID_LOCATE 0
+#endif
+#ifndef M3DK_PREFETCH_REC
+#define M3DK_PREFETCH_REC 1
+#endif
 #ifndef M3DK_PUSH_THREADS
 #define M3DK_PUSH_THREADS 128
 #endif
@@ -41,13 +47,12 @@ __device__ __forceinline__ int hist_rank(int *hist, int key, bool on) {
     return r;
 }
 
-// The same for R keys per lane: all atomics are issued before the first returned value is needed.
+// The same for R keys per lane, in two halves: the atomics are issued as soon as the new keys exist, the returned
+// values are consumed (rank_finish) only after the next block of arithmetic, so their round trip to L2 is never waited for.
 template <int R>
-__device__ __forceinline__ void hist_rank_R(int *hist, int *rank, const int (&key)[R], const long (&m)[R],
-                                            const bool (&on)[R]) {
+__device__ __forceinline__ void hist_issue(int *hist, const int (&key)[R], const bool (&on)[R], unsigned (&peers)[R],
+                                           int (&base)[R]) {
     const int lane = threadIdx.x & 31;
-    unsigned peers[R];
-    int base[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const unsigned live = __ballot_sync(0xffffffffu, on[r]);
@@ -57,6 +62,11 @@ __device__ __forceinline__ void hist_rank_R(int *hist, int *rank, const int (&ke
             if (lane == __ffs(peers[r]) - 1) base[r] = atomicAdd(hist + key[r], __popc(peers[r]));
         }
     }
+}
+template <int R>
+__device__ __forceinline__ void rank_finish(int *rank, const long (&m)[R], const bool (&on)[R], const unsigned (&peers)[R],
+                                            const int (&base)[R]) {
+    const int lane = threadIdx.x & 31;
 #pragma unroll
     for (int r = 0; r < R; ++r)
         if (on[r]) {
@@ -166,6 +176,29 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
         locate_prefetch(P.f.fast, Rn[r], Zn[r]);
 #endif
     }
+    // a3 for the NEW position (the key of the next sort) and, with kHist, the sort histogram of the new keys with each
+    // marker's rank inside its key (the sort then needs no pass over the keys).  With modes this sits between the value
+    // quads and the B_par quad of the last mode: the search record has arrived by then and the atomics' round trip is
+    // covered by the B_par quad.
+    unsigned peers[R];
+    int base[R];
+    auto locate_and_count = [&]() {
+#if !M3DK_EARLY_LOCATE
+#pragma unroll
+        for (int r = 0; r < R; ++r) rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);
+#endif
+        int key[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            int ne = -1;
+            if (on[r]) {
+                ne = locate_finish(P.f, rec[r], Rn[r], Zn[r]);
+                io.store_key(mo[r], ne);
+            }
+            key[r] = ne < 0 ? P.f.n_elems : ne;
+        }
+        if (kHist) hist_issue<R>(P.hist, key, on, peers, base);
+    };
     if (P.f.n_modes > 0) {
         double wsum[R];
 #pragma unroll
@@ -193,6 +226,9 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
                     wsum[r] = pert_fold_v(wsum[r], v[r], wa, wb, cth[r], sth[r]);
                 }
             }
+#if M3DK_MID_LOCATE
+            if (md == P.f.n_modes - 1) locate_and_count();
+#endif
             quad_vd<R, kSmem>(pm + 3 * kQuad, pm, ring, xi, eta, v, dx, de);
 #pragma unroll
             for (int r = 0; r < R; ++r) wsum[r] = pert_fold_par(wsum[r], v[r], dx[r], de[r], W[r], cth[r], sth[r], se, nri[r], om);
@@ -201,24 +237,13 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
 #pragma unroll
         for (int r = 0; r < R; ++r)
             if (on[r]) io.store_w(mo[r], M3DK_FMA(P.dt, wsum[r], s[r].w));
-    }
-    // a3 for the NEW position (the key of the next sort) and, with kHist, the sort histogram of the new keys with each
-    // marker's rank inside its key: the sort then needs no pass over the keys
-#if !M3DK_EARLY_LOCATE
-#pragma unroll
-    for (int r = 0; r < R; ++r) rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);   // all first records in flight together
+#if !M3DK_MID_LOCATE
+        locate_and_count();
 #endif
-    int key[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        int ne = -1;
-        if (on[r]) {
-            ne = locate_finish(P.f, rec[r], Rn[r], Zn[r]);
-            io.store_key(mo[r], ne);
-        }
-        key[r] = ne < 0 ? P.f.n_elems : ne;
+    } else {
+        locate_and_count();
     }
-    if (kHist) hist_rank_R<R>(P.hist, P.rank, key, mo, on);
+    if (kHist) rank_finish<R>(P.rank, mo, on, peers, base);
 }
 
 // ---- generic push: one marker per thread, any marker order (every thread gathers its own element's tile) ------------
@@ -283,29 +308,41 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
     __syncwarp();
     const int total = *P.n_items;
     const int stride = gridDim.x * kWarps;
+    // Software pipeline over this warp's items (static assignment: the warps of a CTA take consecutive items):
+    //   item descriptors are read two items ahead, the order entries (which record goes to which slot) one item ahead,
+    //   and at the start of an item the NEXT item's records are prefetched into L2 and its tile copy is issued,
+    // so that an item starts with its tile in shared memory and its records one L2 hit away.
+    const int4 none = make_int4(P.f.n_elems, 0, 0, 0);
     int it = blockIdx.x * kWarps + warp;
-    int4 w = make_int4(P.f.n_elems, 0, 0, 0);
-    unsigned b = 0, phase = 0;   // buffer of the current item; bit k of phase: parity to wait for on buffer k
-    if (it < total) {
-        w = __ldg(P.items + it);
-        if (w.x < P.f.n_elems && lane == 0) tile_copy_issue(buf0, P.f.tiles + (size_t)w.x * stride_d, tile_bytes, bar0);
+    int4 w0 = it < total ? __ldg(P.items + it) : none;
+    int4 w1 = it + stride < total ? __ldg(P.items + it + stride) : none;
+    int src0[kItemR], src1[kItemR];
+#pragma unroll
+    for (int r = 0; r < kItemR; ++r) {
+        src0[r] = 32 * r + lane < w0.z ? P.rc.order[w0.y + 32 * r + lane].x : 0;
+        src1[r] = 32 * r + lane < w1.z ? P.rc.order[w1.y + 32 * r + lane].x : 0;
     }
+    unsigned b = 0, phase = 0;   // buffer of the current item; bit k of phase: parity to wait for on buffer k
+    if (w0.x < P.f.n_elems && lane == 0) tile_copy_issue(buf0, P.f.tiles + (size_t)w0.x * stride_d, tile_bytes, bar0);
     while (it < total) {
-        const int e = w.x, start = w.y, count = w.z;   // (element, first slot, count, -)
-        it += stride;
-        if (it < total) {
-            w = __ldg(P.items + it);
-            __syncwarp();                              // every lane has finished reading buffer b ^ 1 (previous item)
-            if (w.x < P.f.n_elems && lane == 0)
-                tile_copy_issue(buf0 + (b ^ 1) * tile_bytes, P.f.tiles + (size_t)w.x * stride_d, tile_bytes, bar0 + (b ^ 1) * 8);
+        const int e = w0.x, start = w0.y, count = w0.z;   // (element, first slot, count, -)
+        const int4 w2 = it + 2 * stride < total ? __ldg(P.items + it + 2 * stride) : none;
+        __syncwarp();                                  // every lane has finished reading buffer b ^ 1 (previous item)
+        if (w1.x < P.f.n_elems && lane == 0)
+            tile_copy_issue(buf0 + (b ^ 1) * tile_bytes, P.f.tiles + (size_t)w1.x * stride_d, tile_bytes, bar0 + (b ^ 1) * 8);
+        int src2[kItemR];
+#pragma unroll
+        for (int r = 0; r < kItemR; ++r) {
+            if (M3DK_PREFETCH_REC && 32 * r + lane < w1.z) {
+                const double *rp = P.rc.in + (size_t)kRecDoubles * src1[r];
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(rp));
+            }
+            src2[r] = 32 * r + lane < w2.z ? P.rc.order[w2.y + 32 * r + lane].x : 0;
         }
         long mi[kItemR], mo[kItemR];
         bool on[kItemR];
 #pragma unroll
-        for (int r = 0; r < kItemR; ++r) {
-            mo[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count;
-            mi[r] = on[r] ? P.rc.order[mo[r]].x : 0;   // the record that belongs in this slot
-        }
+        for (int r = 0; r < kItemR; ++r) { mo[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count; mi[r] = src0[r]; }
         const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems};
         if (e >= P.f.n_elems) {                        // lost markers: frozen (G12), moved along and counted for the next sort
             int key[kItemR];
@@ -319,13 +356,22 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
                     io.store_key(mo[r], -1);
                 }
             }
-            if (kHist) hist_rank_R<kItemR>(P.hist, P.rank, key, mo, on);
+            if (kHist) {
+                unsigned peers[kItemR];
+                int base[kItemR];
+                hist_issue<kItemR>(P.hist, key, on, peers, base);
+                rank_finish<kItemR>(P.rank, mo, on, peers, base);
+            }
         } else {
             mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
             phase ^= 1u << b;
             step_R<kItemR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
         }
         b ^= 1;
+        it += stride;
+        w0 = w1; w1 = w2;
+#pragma unroll
+        for (int r = 0; r < kItemR; ++r) { src0[r] = src1[r]; src1[r] = src2[r]; }
     }
 }
 
