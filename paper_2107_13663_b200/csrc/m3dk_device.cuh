@@ -83,7 +83,10 @@ __device__ __forceinline__ Quad ldq_t(const double *p) {
 // software-pipelined through a ring of kRing quads: `ring` holds k = 20 .. 20 - kRing + 1 on entry; while quad k is
 // consumed quad k - kRing is loaded, and on exit `ring` holds the first kRing quads of the block `nxt` (the block the
 // caller evaluates next: the blocks of a tile are consumed back to back), so an L1 hit is never waited for.
-constexpr int kRing = 3;   // must divide 21 so that the ring slots line up from one block to the next
+#ifndef M3DK_RING
+#define M3DK_RING 3
+#endif
+constexpr int kRing = M3DK_RING;   // must divide 21 so that the ring slots line up from one block to the next
 static_assert(21 % kRing == 0, "kRing must divide the 21 coefficients of a block");
 struct Ring { Quad q[kRing]; };
 template <bool kSmem>

@@ -77,10 +77,12 @@ __device__ __forceinline__ void rank_finish(int *rank, const long (&m)[R], const
 
 // ---- marker state access: the caller's SoA arrays (any order, in place) or 64-byte records (ordered pipeline) -------
 __device__ __forceinline__ void ldrec256(const double *p, double &a, double &b, double &c, double &d) {
-    asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p) : "memory");
+    // not volatile, no memory clobber: a thread only ever writes a record after it has read it, and every value it
+    // stores depends on the values loaded here, so the data dependences already order the accesses
+    asm("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
 }
 __device__ __forceinline__ void strec256(double *p, double a, double b, double c, double d) {
-    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d));
 }
 
 struct SoAIO {
@@ -154,22 +156,30 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
     PertW W[R];
     double Rn[R], Zn[R];
     FastRec rec[R];
+    // three separate loops (loads, arithmetic, stores): the arithmetic of the R markers sits in one block with no
+    // memory operation in between, so that the scheduler interleaves the R dependent chains (DFMA latency 8 cycles)
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (on[r]) io.load_vel(mi[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
+        else { s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
+    }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         EqOut f;
         f.psi_R = __dmul_rn(dx[r][0], se); f.psi_Z = __dmul_rn(de[r][0], se);
         f.Bm = v[r][1]; f.Bm_R = __dmul_rn(dx[r][1], se); f.Bm_Z = __dmul_rn(de[r][1], se);
         f.F = v[r][2]; f.kappa = v[r][3];
-        if (on[r]) io.load_vel(mi[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
-        else { s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
         push_eq(P, g[r], f, s[r], W[r]);
+        Rn[r] = m3dk_sqrt(M3DK_FMA(s[r].x, s[r].x, __dmul_rn(s[r].y, s[r].y)));
+        Zn[r] = s[r].z;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
         if (on[r]) {
             io.store_pos(mo[r], s[r].x, s[r].y, s[r].z, s[r].w);
             io.store_vel(mo[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
         }
         // the element search of the new position runs after phase B; its first record starts travelling now
-        Rn[r] = m3dk_sqrt(M3DK_FMA(s[r].x, s[r].x, __dmul_rn(s[r].y, s[r].y)));
-        Zn[r] = s[r].z;
 #if M3DK_EARLY_LOCATE
         rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);
 #else
