@@ -46,15 +46,19 @@ def algorithmic_flops(n_modes: int) -> float:
     return eq + n_modes * (pert + 60) + geom + locate + boris + 130
 
 
-def algorithmic_bytes_push(n_modes: int) -> float:
-    """HBM bytes per marker per push-kernel pass: 8 fp64 read, 7 written (mu is read-only; w only with modes),
-    element key read + written; coefficient tiles are counted as on-chip (shared by the markers of an element)."""
+def algorithmic_bytes_push(n_modes: int, ordered: bool = True) -> float:
+    """HBM bytes per marker per push-kernel pass.  Ordered pipeline: 64 B record read + 8 B order
+    entry read, 64 B record + 4 B key + 4 B rank written.  SoA path (sort_interval 0): 8 fp64 read, 7 written (mu is
+    read-only; w only with modes), element key read + written.  Coefficient tiles are counted as on-chip (shared by the
+    markers of an element; about 13 B per marker-step at config 3 if every tile is fetched once per step)."""
+    if ordered:
+        return 64 + 8 + 64 + 4 + 4
     return 64 + (56 if n_modes else 48) + 4 + 4
 
 
 def algorithmic_bytes_sort() -> float:
-    """Per marker per sort: key read (histogram) + rank written/read + 72 B record read and written."""
-    return 4 + 8 + 2 * 72
+    """Per marker per re-ordering (scan, work-item cut, order list): key + rank + order entry read, order entry written."""
+    return 4 + 4 + 8 + 8
 
 
 # ---- helpers -----------------------------------------------------------------------------------------------------------
@@ -65,6 +69,18 @@ def measured_peaks():
             d = json.load(fh)
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", float(d.get("sm_max_mhz", 1965.0))
     return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)", 1965.0
+
+
+def ncu_traffic(config: int, sort_interval: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the push kernel, per launch, from the committed ncu --set full
+    capture of this workload (profiles/push_traffic.json, written by hand from the capture named there); None when no
+    capture of this configuration is committed."""
+    p = os.path.join(ROOT, "profiles", "push_traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as fh:
+        d = json.load(fh)
+    return d.get(f"config{config}_si{sort_interval}", {}).get("dram_bytes_per_launch")
 
 
 class ClockSampler:
@@ -227,7 +243,7 @@ def run_ours(args, rank, world, local_rank):
     hbm_gbs, hbm_src, _ = measured_peaks()
     fp64_meas = p.fp64_peak_tflops()
     flops = algorithmic_flops(w.n_modes) * N
-    bytes_push = algorithmic_bytes_push(w.n_modes) * N
+    bytes_push = algorithmic_bytes_push(w.n_modes, ordered=si > 0) * N
     push_ms = tm["push_ms"] / max(1, tm["push_launches"])
     t_alu, t_hbm = flops / (FP64_NOMINAL_TFLOPS * 1e12), bytes_push / (hbm_gbs * 1e9)
     if t_alu >= t_hbm:
@@ -238,10 +254,10 @@ def run_ours(args, rank, world, local_rank):
                 "peak_source": hbm_src}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof.update({"kernel": "push kernel (a1-a10)", "launch_ms": push_ms, "launches": tm["push_launches"],
-                 "share_of_step": tm["push_ms"] / ms, "traffic": None,
+                 "share_of_step": tm["push_ms"] / ms, "traffic": ncu_traffic(args.config, si),
                  "fp64_peak_measured_tflops": fp64_meas,
                  "flops_per_marker_step": algorithmic_flops(w.n_modes),
-                 "hbm_bytes_per_marker_step": algorithmic_bytes_push(w.n_modes),
+                 "hbm_bytes_per_marker_step": algorithmic_bytes_push(w.n_modes, ordered=si > 0),
                  "sort_ms_per_sort": tm["sort_ms"] / max(1, tm["sort_launches"]), "sorts": tm["sort_launches"]})
     # whole-step roofline: the binding one of (all flops / fp64 peak) and (all HBM bytes incl. sorts / HBM bandwidth)
     step_bytes = bytes_push + algorithmic_bytes_sort() * N * tm["sort_launches"] / K

@@ -162,12 +162,17 @@ extern "C" int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node
         for (int k = 0; k < M3DK_NCOEF; ++k)
             for (int q = 0; q < 4; ++q) pq[4 * k + q] = ce[q * M3DK_NCOEF + k];
         for (int md = 0; md < n_modes; ++md) {
-            // caller's order: [7 amplitudes][re, im][21]; amplitude a, part p is polynomial 2 a + p and goes to
-            // quad (2 a + p) / 4, slot (2 a + p) % 4 (B_par: quad 3, slots 0 and 1; slots 2 and 3 stay zero)
+            // caller's order: [7 amplitudes][re, im][21], amplitudes E_R E_phi E_Z B_R B_phi B_Z B_par; tile order:
+            // quad 0 (E_R, E_phi), quad 1 (E_Z, B_R), quad 2 (B_par, B_Z), quad 3 (B_phi, zero padding)
+            static const int kSlotOf[M3DK_N_PERT] = {0, 2, 4, 6, 12, 10, 8};   // first of the amplitude's two slots
             const double *cp = pert_coef + ((size_t)md * n_elems + e) * (M3DK_N_PERT * 2 * M3DK_NCOEF);
             double *pm = t + kTileHeader + kTileEq + (size_t)kTileMode * md;
-            for (int pl = 0; pl < 2 * M3DK_N_PERT; ++pl)
-                for (int k = 0; k < M3DK_NCOEF; ++k) pm[(pl / 4) * kQuad + 4 * k + (pl % 4)] = cp[pl * M3DK_NCOEF + k];
+            for (int a = 0; a < M3DK_N_PERT; ++a)
+                for (int part = 0; part < 2; ++part) {
+                    const int pl = kSlotOf[a] + part;
+                    for (int k = 0; k < M3DK_NCOEF; ++k)
+                        pm[(pl / 4) * kQuad + 4 * k + (pl % 4)] = cp[(2 * a + part) * M3DK_NCOEF + k];
+                }
         }
     }
 

@@ -281,16 +281,16 @@ __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double 
         quad_vd<1, false>(pm + kQuad, pm + 2 * kQuad, ring, xi1, eta1, vv, dxx, dee);         // E_Z, B_R
         o.E1[2] += v[0] * cth - v[1] * sth;
         o.B1[0] += v[2] * cth - v[3] * sth;
-        quad_vd<1, false>(pm + 2 * kQuad, pm + 3 * kQuad, ring, xi1, eta1, vv, dxx, dee);         // B_phi, B_Z
-        o.B1[1] += v[0] * cth - v[1] * sth;
+        quad_vd<1, false>(pm + 2 * kQuad, pm + 3 * kQuad, ring, xi1, eta1, vv, dxx, dee);   // B_par with gradient, B_Z
         o.B1[2] += v[2] * cth - v[3] * sth;
-        quad_vd<1, false>(pm + 3 * kQuad, pm, ring, xi1, eta1, vv, dxx, dee);         // B_par with gradient (slots 2, 3 are padding)
         const double re = v[0], im = v[1];
         const double qd = re * sth + im * cth;               // -Im-part combination: d/dphi -> -n qd, d/dt -> omega qd
         o.B1p += re * cth - im * sth;
         o.gB[0] += (dx[0] * se) * cth - (dx[1] * se) * sth;
         o.gB[1] += -(double)n * qd * rinv;
         o.gB[2] += (de[0] * se) * cth - (de[1] * se) * sth;
+        quad_vd<1, false>(pm + 3 * kQuad, pm, ring, xi1, eta1, vv, dxx, dee);                // B_phi (slots 2, 3 are padding)
+        o.B1[1] += v[0] * cth - v[1] * sth;
         o.dtB += f.omega[md] * qd;
     }
 }
@@ -413,10 +413,11 @@ __device__ __forceinline__ double pert_fold_v(double wsum, const double (&v)[4],
     wsum = M3DK_FMA(wa, re_part(v[0], v[1], cth, sth), wsum);
     return M3DK_FMA(wb, re_part(v[2], v[3], cth, sth), wsum);
 }
-// B_par quad: gradient and time derivative; d/dphi -> -n qd, d/dt -> omega qd
+// (B_par, B_Z) quad: gradient and time derivative of B_par (d/dphi -> -n qd, d/dt -> omega qd), value of B_Z
 __device__ __forceinline__ double pert_fold_par(double wsum, const double (&v)[4], const double (&dx)[4],
                                                 const double (&de)[4], const PertW &W, double cth, double sth, double se,
                                                 double n_rinv, double omega) {
+    wsum = M3DK_FMA(W.bBZ, re_part(v[2], v[3], cth, sth), wsum);
     const double qd = M3DK_FMA(v[0], sth, __dmul_rn(v[1], cth));
     wsum = M3DK_FMA(W.gR, re_part(__dmul_rn(dx[0], se), __dmul_rn(dx[1], se), cth, sth), wsum);
     wsum = M3DK_FMA(W.gP, -__dmul_rn(n_rinv, qd), wsum);

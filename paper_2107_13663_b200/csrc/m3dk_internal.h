@@ -21,7 +21,8 @@ namespace m3dk {
 //   [4..87]   quad EQ: (psi0_k, |B|0_k, F0_k, kappa_k), k = 0..20
 //   per mode m, 4 quads of 84 doubles (336 per mode), (re, im) parts of the complex amplitudes:
 //     quad 0: (E_R re, E_R im, E_phi re, E_phi im)     quad 1: (E_Z re, E_Z im, B_R re, B_R im)
-//     quad 2: (B_phi re, B_phi im, B_Z re, B_Z im)     quad 3: (B_par re, B_par im, 0, 0)
+//     quad 2: (B_par re, B_par im, B_Z re, B_Z im)     quad 3: (B_phi re, B_phi im, 0, 0)
+//   B_phi does not enter the linear delta-f weight equation: the push never reads quad 3 (m3dk_eval_fields does).
 constexpr int kTileHeader = 4;
 constexpr int kQuad = 4 * M3DK_NCOEF;                 // 84
 constexpr int kTileEq = kQuad;                        // 84

@@ -6,13 +6,16 @@
 namespace m3dk {
 
 #ifndef M3DK_EARLY_LOCATE
-#define M3DK_EARLY_LOCATE 1
+#define M3DK_EARLY_LOCATE 0
 #endif
 #ifndef M3DK_MID_LOCATE
 #define M3DK_MID_LOCATE 0
 #endif
 #ifndef M3DK_PREFETCH_REC
 #define M3DK_PREFETCH_REC 1
+#endif
+#ifndef M3DK_UNROLL_Q
+#define M3DK_UNROLL_Q 0
 #endif
 #ifndef M3DK_PUSH_THREADS
 #define M3DK_PUSH_THREADS 128
@@ -224,22 +227,26 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
             }
             const double *pm = tile + kTileHeader + kTileEq + kTileMode * md;
             ring_fill<kSmem>(ring, pm);
-            // the three value-only quads share one copy of the Horner code (rolled: the kernel must fit the 32 KB
+            // the two value-only quads share one copy of the Horner code (rolled: the kernel must fit the 32 KB
             // instruction cache); the weights of quad q are picked by selects
+#if M3DK_UNROLL_Q
+#pragma unroll
+#else
 #pragma unroll 1
-            for (int q = 0; q < 3; ++q) {
+#endif
+            for (int q = 0; q < 2; ++q) {
                 quad_vd<R, kSmem>(pm + q * kQuad, pm + (q + 1) * kQuad, ring, xi, eta, v, dx, de);
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const double wa = q == 0 ? W[r].aER : (q == 1 ? W[r].aEZ : 0.0);     // B_phi does not enter
-                    const double wb = q == 0 ? W[r].aEP : (q == 1 ? W[r].bBR : W[r].bBZ);
+                    const double wa = q == 0 ? W[r].aER : W[r].aEZ;
+                    const double wb = q == 0 ? W[r].aEP : W[r].bBR;
                     wsum[r] = pert_fold_v(wsum[r], v[r], wa, wb, cth[r], sth[r]);
                 }
             }
 #if M3DK_MID_LOCATE
             if (md == P.f.n_modes - 1) locate_and_count();
 #endif
-            quad_vd<R, kSmem>(pm + 3 * kQuad, pm, ring, xi, eta, v, dx, de);
+            quad_vd<R, kSmem>(pm + 2 * kQuad, pm, ring, xi, eta, v, dx, de);   // (B_par, B_Z); quad 3 (B_phi) is not needed
 #pragma unroll
             for (int r = 0; r < R; ++r) wsum[r] = pert_fold_par(wsum[r], v[r], dx[r], de[r], W[r], cth[r], sth[r], se, nri[r], om);
         }
