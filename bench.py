@@ -37,13 +37,17 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA lanes 
 
 # ---- algorithmic work per marker-step (DESIGN.md section 7 derives these) ---------------------------------------------
 def algorithmic_flops(n_modes: int) -> float:
-    """FMA = 2, add/mul = 1, div = sqrt = 1 (minimal-multiplication Horner, recounted in DESIGN.md)."""
-    eq = 78 + 78 + 40 + 40                    # psi0 (value, d/dR, d/dZ), |B|0 (same), F0, kappa
-    geom, locate, boris = 45, 30, 56
+    """fp64 operations per marker-step counted from the kernel's formulas: FMA = 2, add / mul = 1,
+    reciprocal / rsqrt / sqrt = 1 each (their Newton steps are not counted); minimal-multiplication Horner: value of a
+    21-term quintic = 20 FMA, value + d/dxi + d/deta = 38 FMA.  The fp32 arithmetic of the element search is not counted."""
+    eq = 2 * (38 + 38 + 20 + 20)              # psi0 and |B|0 with gradients, F0, kappa
+    common = 11 + 4 + 68 + 6 + 7              # cylindrical map + local coordinates, scaling, B / E-dagger / Boris, drift, R of x_{l+1}
     if n_modes == 0:
-        return eq + geom + locate + boris
-    pert = 5 * 2 * 40 + 2 * 78                # E_R E_phi E_Z B_R B_Z (re, im) values; B_par (re, im) value + gradient
-    return eq + n_modes * (pert + 60) + geom + locate + boris + 130
+        return eq + common
+    pert = 2 * (10 * 20 + 2 * 38)             # E_R E_phi E_Z B_R B_Z (re, im) values; B_par (re, im) value + gradient
+    fold = 25 + 25 + 23                       # phase exp(i(n phi - omega t)) for n = 3, folding 5 + 1 complex fields into dw/dt
+    weight = 86 + 2                           # coefficients of dw/dt (Eqs. 8-13 incl. kappa_E), w update
+    return eq + common + weight + n_modes * (pert + fold)
 
 
 def algorithmic_bytes_push(n_modes: int, ordered: bool = True) -> float:
