@@ -143,11 +143,10 @@ def oracle_sample_rate(w, sample_stride: int, nsteps: int, nthreads: int = 0):
 
 def build_workload(args, rank: int):
     import synth
-    n = args.n_markers
-    # every rank draws its own shard (seed offset by rank): independent markers, same tables
-    w = synth.make_config(args.config, n_markers=n, nx=args.nx, dt_gyro=args.dt_gyro,
-                          seed=None if rank == 0 else 1000 + args.config + 7919 * rank)
-    return w
+    from paper_2107_13663_b200 import shard
+    # every rank draws its own shard (seed offset by rank): independent markers, same tables (DESIGN.md section 9)
+    return synth.make_config(args.config, n_markers=args.n_markers, nx=args.nx, dt_gyro=args.dt_gyro,
+                             seed=shard.shard_seed(args.config, rank))
 
 
 def config_dict(args, w, sort_interval, world):
@@ -237,10 +236,8 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     ms_e2e = f0.elapsed_time(f1)
 
-    t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e = float(t[0]), float(t[1])
+    from paper_2107_13663_b200 import shard
+    ms, ms_e2e = shard.max_over_ranks([ms, ms_e2e], dist if world > 1 else None, device=dev)
     if rank != 0:
         return
 
@@ -268,11 +265,11 @@ def run_ours(args, rank, world, local_rank):
     t_bind = max(t_alu, step_bytes / (hbm_gbs * 1e9))
     roof["step_frac_of_binding_roofline"] = t_bind / (ms / K * 1e-3)
 
-    line = {"metric": METRIC, "value": world * N * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+    line = {"metric": METRIC, "value": shard.whole_job_rate([N] * world, K, ms), "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": config_dict(args, w, si, world),
             "clocks": clocks, "gpu_launches": tm["kernel_launches"],
-            "e2e": {"value": world * N * Ke / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 64 * N / Ke,
+            "e2e": {"value": shard.whole_job_rate([N] * world, Ke, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": 64 * N / Ke,
                     "d2h_bytes_per_step": 64 * N / Ke, "note": f"one upload + {Ke} steps + one download (PAPER.md:237)"},
             "roofline": roof, "n_lost": st["n_lost"]}
     if world == 1 and not args.no_cpu_baseline:
@@ -295,7 +292,7 @@ def main():
     ap.add_argument("--dt-gyro", type=float, default=None)
     ap.add_argument("--sort-interval", type=int, default=None)
     ap.add_argument("--ref-sample", type=int, default=65536, help="markers in the oracle's bounded sample")
-    ap.add_argument("--ref-steps", type=int, default=100)
+    ap.add_argument("--ref-steps", type=int, default=400)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

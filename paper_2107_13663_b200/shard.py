@@ -1,0 +1,40 @@
+"""Marker sharding across ranks: independent shards, no data-path collective.
+
+Markers are independent and the paper runs every GPU with the whole field table and no traffic during
+the push, so rank r of N simply owns its own shard of markers.  This module holds the bookkeeping that
+``bench.py`` uses under torchrun: the per-rank seed, the per-rank slice of a global id range, and the reduction of the
+per-rank timings to the whole-job figure (max over ranks).  No arithmetic of the method lives here.
+"""
+from __future__ import annotations
+
+from typing import Sequence, Tuple
+
+
+def shard_seed(config: int, rank: int) -> int:
+    """Seed of rank's shard: rank 0 draws the documented seed 1000 + config."""
+    return 1000 + int(config) + 7919 * int(rank)
+
+
+def shard_range(n_global: int, rank: int, world: int) -> Tuple[int, int]:
+    """[begin, end) of the global marker ids owned by `rank` when n_global markers are split over `world` ranks
+    (contiguous blocks, the first n_global % world ranks get one more)."""
+    if world < 1 or not 0 <= rank < world or n_global < 0:
+        raise ValueError("bad shard arguments")
+    base, extra = divmod(int(n_global), int(world))
+    begin = rank * base + min(rank, extra)
+    return begin, begin + base + (1 if rank < extra else 0)
+
+
+def whole_job_rate(markers_per_rank: Sequence[int], steps: int, ms_max_over_ranks: float) -> float:
+    """particle-steps/s of the whole job: all markers of all ranks x steps / the slowest rank's device time."""
+    return float(sum(int(m) for m in markers_per_rank)) * steps / (ms_max_over_ranks * 1e-3)
+
+
+def max_over_ranks(values, dist=None, device=None):
+    """Element-wise maximum of a list of floats over the ranks of torch.distributed (identity without a group)."""
+    import torch
+
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None and dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
