@@ -127,6 +127,16 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def oracle_bounded_sample(w, n_sample: int, target_s: float = 15.0):
+    """The oracle on a bounded sample sized for about target_s seconds of CPU work on this box: a short calibration run
+    (every 1024-th marker, 20 steps) fixes the number of steps for the id = 0 (mod stride) sub-sample."""
+    stride = max(1, w.n_markers // n_sample)
+    rate, n, secs, cores = oracle_sample_rate(w, max(stride, min(1024, w.n_markers // 1024 or 1)), 20)
+    n_s = len(range(0, w.n_markers, stride))
+    steps = int(min(2000, max(20, target_s * rate / n_s)))
+    return oracle_sample_rate(w, stride, steps) + (stride, steps)
+
+
 def oracle_sample_rate(w, sample_stride: int, nsteps: int, nthreads: int = 0):
     """The oracle as it stands, FE back-end, OpenMP over markers, on the id = 0 (mod stride) sub-sample."""
     import oracle
@@ -187,7 +197,9 @@ def run_ours(args, rank, world, local_rank):
     dev = torch.device("cuda", local_rank)
     m3dk.build_all()
     w = build_workload(args, rank)
-    si = w.sort_interval if args.sort_interval is None else args.sort_interval
+    # decision D-c: the ordering interval is a tuning knob with bit-identical results; workloads
+    # that sort at all run the fused ordering every step unless --sort-interval says otherwise
+    si = (1 if w.sort_interval > 0 else 0) if args.sort_interval is None else args.sort_interval
     N, K, W = w.n_markers, args.steps, args.warmup
 
     p = m3dk.Pusher(device=local_rank, verify=False)
@@ -273,10 +285,9 @@ def run_ours(args, rank, world, local_rank):
                     "d2h_bytes_per_step": 64 * N / Ke, "note": f"one upload + {Ke} steps + one download (PAPER.md:237)"},
             "roofline": roof, "n_lost": st["n_lost"]}
     if world == 1 and not args.no_cpu_baseline:
-        stride = max(1, N // args.ref_sample)
-        rate, n, secs, cores = oracle_sample_rate(w, stride, args.ref_steps)
+        rate, n, secs, cores, stride, rsteps = oracle_bounded_sample(w, args.ref_sample)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"{n} markers (every {stride}-th of the workload) x {args.ref_steps} steps, {secs:.1f} s"}
+                                "sample": f"{n} markers (every {stride}-th of the workload) x {rsteps} steps, {secs:.1f} s"}
     print(json.dumps(line), flush=True)
 
 
@@ -292,7 +303,6 @@ def main():
     ap.add_argument("--dt-gyro", type=float, default=None)
     ap.add_argument("--sort-interval", type=int, default=None)
     ap.add_argument("--ref-sample", type=int, default=65536, help="markers in the oracle's bounded sample")
-    ap.add_argument("--ref-steps", type=int, default=400)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

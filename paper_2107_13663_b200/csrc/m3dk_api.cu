@@ -387,6 +387,7 @@ static int bind_sort_ws(m3dk_ctx *ctx, void *ws, size_t bytes, const char *who) 
     if (!ws || ((uintptr_t)ws & 255) || bytes < sort_workspace_bytes(ctx->n, ctx->f.n_elems))
         return fail(ctx, M3DK_EWORKSPACE, std::string(who) + ": workspace NULL, misaligned or smaller than m3dk_sort_workspace_bytes");
     carve_sort_workspace(ws, ctx->n, ctx->f.n_elems, &ctx->sb);
+
     ctx->sb.bytes = bytes;
     ctx->have_sortws = true;
     return M3DK_OK;

@@ -119,6 +119,7 @@ struct SortBuffers {         // carved from the sort workspace
     int *offs;               // [n_elems + 2]
     int *ioffs;              // [n_elems + 2] first work item of each element; ioffs[n_elems + 1] = number of items
     int4 *items;             // [n / kItemMarkers + n_elems + 2]
+    unsigned long long *scan_state;   // ticket + per-chunk totals of the single-pass scan
     size_t bytes;
 };
 
@@ -137,7 +138,8 @@ struct m3dk_ctx {
     long n = 0;
     m3dk::MarkerArrays user{};   // caller's arrays (the state lives here between calls)
     int cur = 0;                 // record buffer that holds the state inside an ordered push / sort
-    int ocur = 0;                // order buffer whose .y are the ids of the records in sb.rec[cur]
+    int ocur = 0;
+    unsigned scan_epoch = 0;     // tag of the current scan launch (decoupled look-back without clearing)                // order buffer whose .y are the ids of the records in sb.rec[cur]
     double q = 1.0, m = 1.0;
     m3dk_f0_params f0{};
     // options / clock

@@ -14,7 +14,8 @@ size_t sort_workspace_bytes(long n, int n_elems) {
     const size_t nr = up256((size_t)n * kRecDoubles * sizeof(double)), no = up256((size_t)n * sizeof(int2));
     const size_t ni = up256((size_t)n * sizeof(int)), nh = up256((size_t)(n_elems + 2) * sizeof(int));
     const size_t nit = up256(((size_t)n / kItemMarkers + n_elems + 2) * sizeof(int4));
-    return 2 * nr + 2 * no + 2 * ni + 3 * nh + nit;
+    const size_t nst = up256(((size_t)(n_elems + 1) / 4096 + 4) * sizeof(unsigned long long));
+    return 2 * nr + 2 * no + 2 * ni + 3 * nh + nit + nst;
 }
 
 void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb) {
@@ -29,6 +30,7 @@ void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb) {
     sb->offs = reinterpret_cast<int *>(p); p += nh;
     sb->ioffs = reinterpret_cast<int *>(p); p += nh;
     sb->items = reinterpret_cast<int4 *>(p); p += up256(((size_t)n / kItemMarkers + n_elems + 2) * sizeof(int4));
+    sb->scan_state = reinterpret_cast<unsigned long long *>(p); p += up256(((size_t)(n_elems + 1) / 4096 + 4) * sizeof(unsigned long long));
     sb->bytes = (size_t)(p - static_cast<char *>(ws));
 }
 
@@ -50,55 +52,78 @@ __global__ void __launch_bounds__(256) hist_rank_kernel(const int *__restrict__ 
 }
 
 // exclusive scan of hist[0..m) into offs[0..m] (offs[m] = total) and, in the same sweep, of the work-item counts
-// ceil(hist[k] / kItemMarkers) into ioffs[0..m]: one CTA, coalesced chunks of 1024 x 4 bins, warp shuffles inside a
-// chunk, running carries across chunks (m is a few 1e5 bins: ~30 chunk iterations).
+// ceil(hist[k] / kItemMarkers) into ioffs[0..m].  Single pass, decoupled look-back: a CTA takes a chunk of 4096 bins by
+// ticket, publishes the chunk's totals at once, then sums the totals of the chunks before it (which were taken earlier,
+// so they are running: no deadlock) while it scans its own bins.  state[0] = ticket counter, state[2 + c] = totals of
+// chunk c with a ready tag in the upper bits; the launcher clears the state (a few hundred bytes) before each launch.
+// word = tag << 56 | items << 31 | markers   (markers < 2^31, items < 2^25)
+constexpr int kScanChunk = 4096;
 __global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist, int m, int *__restrict__ offs,
-                                                    int *__restrict__ ioffs) {
+                                                    int *__restrict__ ioffs, unsigned long long *state,
+                                                    unsigned epoch) {
     __shared__ int2 wsum[32];
-    __shared__ int2 carry_s;
+    __shared__ int2 prefix_s;
+    __shared__ int chunk_s;
     const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
-    if (t == 0) carry_s = make_int2(0, 0);
+    if (t == 0) chunk_s = (int)atomicAdd(state, 1ull);
     __syncthreads();
-    for (int base = 0; base < m; base += 4096) {
-        const int k = base + 4 * t;
-        int v[4], it[4];
+    const int chunk = chunk_s;
+    const int nchunks = (m + kScanChunk - 1) / kScanChunk;
+    if (chunk >= nchunks) return;
+    const int k = chunk * kScanChunk + 4 * t;
+    int v[4], it[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            v[q] = k + q < m ? hist[k + q] : 0;
-            it[q] = (v[q] + kItemMarkers - 1) / kItemMarkers;
-        }
-        const int2 mine = make_int2(v[0] + v[1] + v[2] + v[3], it[0] + it[1] + it[2] + it[3]);
-        int2 inc = mine;
+    for (int q = 0; q < 4; ++q) {
+        v[q] = k + q < m ? hist[k + q] : 0;
+        it[q] = (v[q] + kItemMarkers - 1) / kItemMarkers;
+    }
+    const int2 mine = make_int2(v[0] + v[1] + v[2] + v[3], it[0] + it[1] + it[2] + it[3]);
+    int2 inc = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int ux = __shfl_up_sync(0xffffffffu, inc.x, o), uy = __shfl_up_sync(0xffffffffu, inc.y, o);
+        if (lane >= o) { inc.x += ux; inc.y += uy; }
+    }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        int2 w = wsum[lane];
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const int ux = __shfl_up_sync(0xffffffffu, inc.x, o), uy = __shfl_up_sync(0xffffffffu, inc.y, o);
-            if (lane >= o) { inc.x += ux; inc.y += uy; }
+            const int ux = __shfl_up_sync(0xffffffffu, w.x, o), uy = __shfl_up_sync(0xffffffffu, w.y, o);
+            if (lane >= o) { w.x += ux; w.y += uy; }
         }
-        if (lane == 31) wsum[wid] = inc;
-        __syncthreads();
-        if (wid == 0) {
-            int2 w = wsum[lane];
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int ux = __shfl_up_sync(0xffffffffu, w.x, o), uy = __shfl_up_sync(0xffffffffu, w.y, o);
-                if (lane >= o) { w.x += ux; w.y += uy; }
+        wsum[lane] = w;      // inclusive over warps; lane 31 holds the chunk's totals
+        const unsigned long long tag = (unsigned long long)(epoch & 0xffu) << 56;
+        if (lane == 31) {
+            const unsigned long long word = tag | ((unsigned long long)(unsigned)w.y << 31) | (unsigned long long)(unsigned)w.x;
+            atomicExch(state + 2 + chunk, word);
+        }
+        // look back over the chunks before this one, 32 at a time
+        long long px = 0, py = 0;
+        for (int c0 = chunk - 1; c0 >= 0; c0 -= 32) {
+            const int c = c0 - lane;
+            unsigned long long word = 0ull;
+            if (c >= 0) {
+                do { word = *reinterpret_cast<volatile unsigned long long *>(state + 2 + c); } while ((word >> 56) != (tag >> 56));
+                px += (long long)(word & 0x7fffffffull);
+                py += (long long)((word >> 31) & 0x1ffffffull);
             }
-            wsum[lane] = w;      // inclusive over warps
         }
-        __syncthreads();
-        const int2 carry = carry_s;
-        const int2 wprev = wid ? wsum[wid - 1] : make_int2(0, 0);
-        int run = carry.x + wprev.x + inc.x - mine.x, irun = carry.y + wprev.y + inc.y - mine.y;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            if (k + q < m) { offs[k + q] = run; ioffs[k + q] = irun; }
-            run += v[q]; irun += it[q];
-        }
-        __syncthreads();
-        if (t == 1023) carry_s = make_int2(carry.x + wsum[31].x, carry.y + wsum[31].y);
-        __syncthreads();
+        for (int o = 16; o > 0; o >>= 1) { px += __shfl_xor_sync(0xffffffffu, px, o); py += __shfl_xor_sync(0xffffffffu, py, o); }
+        if (lane == 0) prefix_s = make_int2((int)px, (int)py);
     }
-    if (t == 0) { offs[m] = carry_s.x; ioffs[m] = carry_s.y; }
+    __syncthreads();
+    const int2 carry = prefix_s;
+    const int2 wprev = wid ? wsum[wid - 1] : make_int2(0, 0);
+    int run = carry.x + wprev.x + inc.x - mine.x, irun = carry.y + wprev.y + inc.y - mine.y;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        if (k + q < m) { offs[k + q] = run; ioffs[k + q] = irun; }
+        run += v[q]; irun += it[q];
+    }
+    if (chunk == nchunks - 1 && t == 1023) { offs[m] = carry.x + wsum[31].x; ioffs[m] = carry.y + wsum[31].y; }
 }
 
 // work items of the element-ordered push: element k's sorted segment [offs[k], offs[k+1]) cut into pieces of at most
@@ -163,7 +188,11 @@ __global__ void __launch_bounds__(256) unpack_kernel(MarkerArrays a, long n, int
 static cudaError_t scan_and_cut(m3dk_ctx *c) {
     const int m = c->f.n_elems + 1;
     c->kernel_launches += 2;
-    scan_kernel<<<1, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs, c->sb.ioffs);
+    const int nchunks = (m + kScanChunk - 1) / kScanChunk;
+    // ticket and per-chunk words cleared together (a few hundred bytes): a word is ready when its tag is set
+    cudaError_t e = cudaMemsetAsync(c->sb.scan_state, 0, (size_t)(nchunks + 2) * sizeof(unsigned long long), c->stream);
+    if (e != cudaSuccess) return e;
+    scan_kernel<<<nchunks, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs, c->sb.ioffs, c->sb.scan_state, 1u);
     items_kernel<<<(m + 255) / 256, 256, 0, c->stream>>>(c->sb.offs, c->sb.ioffs, m, c->sb.items);
     return cudaGetLastError();
 }
