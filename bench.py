@@ -291,6 +291,49 @@ def run_ours(args, rank, world, local_rank):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: marker count x dt x ordering interval on the config-3 equilibrium and perturbation; one
+    JSON line per point (particle-steps/s and the fraction of the binding roofline), single GPU, device-resident timing.
+    Not the driver's contract line: a table generator for BASELINE.md."""
+    import torch
+    import synth
+    import paper_2107_13663_b200 as m3dk
+
+    torch.cuda.set_device(0)
+    m3dk.build_all()
+    hbm_gbs, _, _ = measured_peaks()
+    K, W = args.steps, args.warmup
+    for n in args.sweep_n:
+        for dtg in args.sweep_dt:
+            w = synth.make_config(4, n_markers=n, dt_gyro=dtg)
+            for si in args.sweep_si:
+                p = m3dk.Pusher(device=0, verify=False)
+                p.fields_create(w.node_RZ, w.tri, w.eq_coef, w.n_tor, w.omega, w.pert_coef)
+                p.particles_init(w.markers, w.charge, w.mass, w.f0)
+                p.set_options(sort_interval=si, t0=0.0)
+                p.push(W, w.dt)
+                p.set_profiling(True)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record(p.stream)
+                p.push(K, w.dt)
+                e1.record(p.stream)
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1) / K
+                tm = p.timing()
+                t_alu = algorithmic_flops(w.n_modes) * n / (FP64_NOMINAL_TFLOPS * 1e12)
+                t_hbm = (algorithmic_bytes_push(w.n_modes, ordered=si > 0) + algorithmic_bytes_sort() * tm["sort_launches"] / K) * n / (hbm_gbs * 1e9)
+                print(json.dumps({"sweep_point": {"n_markers": n, "dt_gyro": dtg, "sort_interval": si},
+                                  "value": n / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms,
+                                  "push_ms": tm["push_ms"] / max(1, tm["push_launches"]),
+                                  "binding": "alu" if t_alu >= t_hbm else "hbm",
+                                  "frac_of_binding_roofline": max(t_alu, t_hbm) / (ms * 1e-3),
+                                  "n_lost": p.stats()["n_lost"]}), flush=True)
+                p.close()
+                del p
+                torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -304,6 +347,10 @@ def main():
     ap.add_argument("--sort-interval", type=int, default=None)
     ap.add_argument("--ref-sample", type=int, default=65536, help="markers in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="configs[4] sweep: one JSON line per (n, dt, sort interval)")
+    ap.add_argument("--sweep-n", type=int, nargs="+", default=[1 << 20, 1 << 22, 1 << 24, 1 << 26])
+    ap.add_argument("--sweep-dt", type=float, nargs="+", default=[1.0, 4.0, 16.0])
+    ap.add_argument("--sweep-si", type=int, nargs="+", default=[1, 10, 0])
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -312,6 +359,10 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+        return
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
         return
     if world > 1:
         import torch.distributed as dist
