@@ -30,7 +30,8 @@ class Analytic(C.Structure):
 
 
 class Species(C.Structure):
-    _fields_ = [("charge", C.c_double), ("mass", C.c_double), ("f0kind", C.c_int), ("f0par", C.c_double * 5)]
+    _fields_ = [("charge", C.c_double), ("mass", C.c_double), ("f0kind", C.c_int), ("f0par", C.c_double * 5),
+                ("mode", C.c_int)]
 
 
 def build(force: bool = False) -> str:
@@ -79,17 +80,18 @@ def _i(a):
     return a, a.ctypes.data_as(c_ip)
 
 
-def species(charge, mass, f0kind=0, T=1.0, v_c=0.3, Lambda0=0.75, dLambda=0.2, B_axis=1.0) -> Species:
+def species(charge, mass, f0kind=0, T=1.0, v_c=0.3, Lambda0=0.75, dLambda=0.2, B_axis=1.0, mode=0) -> Species:
+    """mode 0: linear delta-f; 1: non-linear trajectories with (1 - w) kept (reading G21)."""
     s = Species()
-    s.charge, s.mass, s.f0kind = float(charge), float(mass), int(f0kind)
+    s.charge, s.mass, s.f0kind, s.mode = float(charge), float(mass), int(f0kind), int(mode)
     for k, v in enumerate((T, v_c, Lambda0, dLambda, B_axis)):
         s.f0par[k] = float(v)
     return s
 
 
-def species_of(workload) -> Species:
+def species_of(workload, mode=0) -> Species:
     f = workload.f0
-    return species(workload.charge, workload.mass, f.kind, f.T, f.v_c, f.Lambda0, f.dLambda, f.B_axis)
+    return species(workload.charge, workload.mass, f.kind, f.T, f.v_c, f.Lambda0, f.dLambda, f.B_axis, mode=mode)
 
 
 def analytic_of(eq, kappa=0.0, pA=0.0, prc=0.5, pwd=0.1, pomega=0.0, pn=0, pm=0) -> Analytic:

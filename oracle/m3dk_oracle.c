@@ -85,6 +85,7 @@ typedef struct {
     double charge, mass;
     int f0kind;        /* 0 Maxwellian, 1 slowing-down, 2 beam pitch (reading G7) */
     double f0par[5];   /* T, v_c, Lambda0, dLambda, B_axis */
+    int mode;          /* 0: linear delta-f; 1: non-linear trajectories, (1 - w) kept (reading G21) */
 } orc_species;
 
 /* ------------------------------------------------------------------------------------------------ */
@@ -401,12 +402,20 @@ static int step_marker(const provider *pv, const orc_species *sp, double *s, dou
     } else {
         an_fields(pv->an, R, phi, Z, t, &f);
     }
-    /* 5: linear mode, trajectory in the equilibrium field only */
+    /* 5: linear mode: trajectory in the equilibrium field only.  Non-linear mode (reading G21):
+     *    "the particle trajectories are calculated using the total fields": B = B0 + B1,
+     *    E-dagger = E1 - (mu/q) grad(|B|0 + B1par), the mirror force of the total field strength.   */
     double mu = s[6], q = sp->charge, m = sp->mass;
     double BR = -f.psi_Z / R, BP = f.F / R, BZ = f.psi_R / R;
-    double ER = -(mu / q) * f.Bm_R, EZ = -(mu / q) * f.Bm_Z;
+    double ER = -(mu / q) * f.Bm_R, EP = 0.0, EZ = -(mu / q) * f.Bm_Z;
+    if (sp->mode == 1) {
+        BR += f.B1[0]; BP += f.B1[1]; BZ += f.B1[2];
+        ER = f.E1[0] - (mu / q) * (f.Bm_R + f.gB1p[0]);
+        EP = f.E1[1] - (mu / q) * f.gB1p[1];
+        EZ = f.E1[2] - (mu / q) * (f.Bm_Z + f.gB1p[2]);
+    }
     double B[3] = {BR * c - BP * sn, BR * sn + BP * c, BZ};
-    double E[3] = {ER * c, ER * sn, EZ};
+    double E[3] = {ER * c - EP * sn, ER * sn + EP * c, EZ};
     /* 6 */
     double vm[3] = {s[3], s[4], s[5]}, vp[3];
     double h = q * dt / (2.0 * m);
@@ -415,6 +424,9 @@ static int step_marker(const provider *pv, const orc_species *sp, double *s, dou
     double vl[3] = {0.5 * (vm[0] + vp[0]), 0.5 * (vm[1] + vp[1]), 0.5 * (vm[2] + vp[2])};
     double vlc[3] = {vl[0] * c + vl[1] * sn, -vl[0] * sn + vl[1] * c, vl[2]};
     double wdot = weight_rhs(&f, sp, R, vlc, mu);
+    /* Eq. (8): dw/dt = -(1 - w) (1/f0) df0/dt; the linear mode takes (1 - w) -> 1, the non-linear mode
+     * keeps the factor, explicit in w on the staggered grid (readings G9, G21)                                    */
+    if (sp->mode == 1) wdot *= (1.0 - s[7]);
     s[7] = s[7] + dt * wdot;
     /* 8 */
     s[0] = x + dt * vp[0]; s[1] = y + dt * vp[1]; s[2] = z + dt * vp[2];
