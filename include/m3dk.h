@@ -115,7 +115,10 @@ int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, double *z, 
                         const m3dk_f0_params *f0);
 
 /* sort_interval: 0 = m3dk_push never sorts; k > 0 = m3dk_push sorts before every k-th step (needs a sort workspace).
- * mode: 0 = linear delta-f (trajectories in the equilibrium field, (1 - w) -> 1); others reserved.
+ * mode: 0 = linear delta-f (trajectories in the equilibrium field, (1 - w) -> 1);
+ *       1 = non-linear trajectories (reading G21): the marker moves in the total fields,
+ *           B = B0 + B1 and E-dagger = E1 - (mu/q) grad(|B|0 + B1par), and Eq. (8) keeps its factor (1 - w):
+ *           w_{l+1/2} = w_{l-1/2} + dt (1 - w_{l-1/2}) dw/dt|linear(x_l, v_l, t_l).
  * t0: time of the next step's x_l.  Resets steps_done to 0.                                                          */
 int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, double t0);
 

@@ -342,6 +342,34 @@ struct PertW { double aER, aEP, aEZ, bBR, bBZ, gR, gP, gZ, dT; };
 #define DM(a, b) __dmul_rn((a), (b))
 #define DA(a, b) __dadd_rn((a), (b))
 #define DS(a, b) __dsub_rn((a), (b))
+// Coefficients of dw/dt in the perturbed fields (see push_eq): (BR, BP, BZ) is the EQUILIBRIUM field B0, s holds
+// v_{l-1/2}, (nvx, nvy, nvz) = v_{l+1/2}.
+__device__ __forceinline__ void weight_coeffs(const PushParams &P, const StepGeom &g, const EqOut &f, double BR, double BP,
+                                              double BZ, const Marker &s, double nvx, double nvy, double nvz, PertW &W) {
+    const double cph = g.cph, sph = g.sph;
+    const double vlx = DM(0.5, DA(s.vx, nvx)), vly = DM(0.5, DA(s.vy, nvy)), vlz = DM(0.5, DA(s.vz, nvz));
+    const double vR = M3DK_FMA(vlx, cph, DM(vly, sph)), vP = M3DK_FMA(vly, cph, -DM(vlx, sph)), vZ = vlz;
+    const double B2 = M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, DM(BZ, BZ)));
+    const double binv = m3dk_rsqrt(B2);
+    const double b2inv = DM(binv, binv);
+    const double bR = DM(BR, binv), bP = DM(BP, binv), bZ = DM(BZ, binv);
+    const double vpar = M3DK_FMA(vR, bR, M3DK_FMA(vP, bP, DM(vZ, bZ)));
+    const double v2 = M3DK_FMA(vlx, vlx, M3DK_FMA(vly, vly, DM(vlz, vlz)));
+    const double Ekin = M3DK_FMA(DM(0.5, P.m), v2, DM(s.mu, f.Bm));
+    const double kE = kappa_E(P, Ekin, s.mu);
+    const double K = DM(f.kappa, P.inv_q), G = DM(f.F, binv);
+    const double Kq = DM(K, P.q), kEq = DM(kE, P.q);
+    W.aER = -M3DK_FMA(Kq, M3DK_FMA(DM(f.psi_Z, BP), b2inv, DM(bR, G)), DM(kEq, vR));
+    W.aEP = -M3DK_FMA(Kq, M3DK_FMA(M3DK_FMA(f.psi_R, BZ, -DM(f.psi_Z, BR)), b2inv, DM(bP, G)), DM(kEq, vP));
+    W.aEZ = -M3DK_FMA(Kq, M3DK_FMA(-DM(f.psi_R, BP), b2inv, DM(bZ, G)), DM(kEq, vZ));
+    const double Kv = -DM(DM(Kq, vpar), binv);
+    W.bBR = DM(Kv, f.psi_R);
+    W.bBZ = DM(Kv, f.psi_Z);
+    const double Kg = DM(DM(K, s.mu), G);
+    W.gR = DM(Kg, bR); W.gP = DM(Kg, bP); W.gZ = DM(Kg, bZ);
+    W.dT = -DM(kE, s.mu);
+}
+
 __device__ __forceinline__ void push_eq(const PushParams &P, const StepGeom &g, const EqOut &f, Marker &s, PertW &W) {
     const double rinv = g.rinv, cph = g.cph, sph = g.sph;
     // B0 = grad psi0 x grad phi + F0 grad phi (G4); E-dagger = -(mu/q) grad|B|0 (G2)
@@ -361,29 +389,46 @@ __device__ __forceinline__ void push_eq(const PushParams &P, const StepGeom &g, 
                  wz = M3DK_FMA(sc, M3DK_FMA(px, ty, -DM(py, tx)), uz);
     const double nvx = M3DK_FMA(h, Ex, wx), nvy = M3DK_FMA(h, Ey, wy), nvz = M3DK_FMA(h, Ez, wz);
     if (P.f.n_modes > 0) {
-        const double vlx = DM(0.5, DA(s.vx, nvx)), vly = DM(0.5, DA(s.vy, nvy)), vlz = DM(0.5, DA(s.vz, nvz));
-        const double vR = M3DK_FMA(vlx, cph, DM(vly, sph)), vP = M3DK_FMA(vly, cph, -DM(vlx, sph)), vZ = vlz;
-        const double B2 = M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, DM(BZ, BZ)));
-        const double binv = m3dk_rsqrt(B2);
-        const double b2inv = DM(binv, binv);
-        const double bR = DM(BR, binv), bP = DM(BP, binv), bZ = DM(BZ, binv);
-        const double vpar = M3DK_FMA(vR, bR, M3DK_FMA(vP, bP, DM(vZ, bZ)));
-        const double v2 = M3DK_FMA(vlx, vlx, M3DK_FMA(vly, vly, DM(vlz, vlz)));
-        const double Ekin = M3DK_FMA(DM(0.5, P.m), v2, DM(s.mu, f.Bm));
-        const double kE = kappa_E(P, Ekin, s.mu);
-        const double K = DM(f.kappa, P.inv_q), G = DM(f.F, binv);
-        const double Kq = DM(K, P.q), kEq = DM(kE, P.q);
-        W.aER = -M3DK_FMA(Kq, M3DK_FMA(DM(f.psi_Z, BP), b2inv, DM(bR, G)), DM(kEq, vR));
-        W.aEP = -M3DK_FMA(Kq, M3DK_FMA(M3DK_FMA(f.psi_R, BZ, -DM(f.psi_Z, BR)), b2inv, DM(bP, G)), DM(kEq, vP));
-        W.aEZ = -M3DK_FMA(Kq, M3DK_FMA(-DM(f.psi_R, BP), b2inv, DM(bZ, G)), DM(kEq, vZ));
-        const double Kv = -DM(DM(Kq, vpar), binv);
-        W.bBR = DM(Kv, f.psi_R);
-        W.bBZ = DM(Kv, f.psi_Z);
-        const double Kg = DM(DM(K, s.mu), G);
-        W.gR = DM(Kg, bR); W.gP = DM(Kg, bP); W.gZ = DM(Kg, bZ);
-        W.dT = -DM(kE, s.mu);
+        weight_coeffs(P, g, f, BR, BP, BZ, s, nvx, nvy, nvz, W);
     }
     // Eq. (5)
+    s.x = M3DK_FMA(P.dt, nvx, s.x); s.y = M3DK_FMA(P.dt, nvy, s.y); s.z = M3DK_FMA(P.dt, nvz, s.z);
+    s.vx = nvx; s.vy = nvy; s.vz = nvz;
+}
+
+// ---- non-linear trajectory mode (mode 1; reading G21) ----------------------------------------
+// Perturbed fields of one marker, cylindrical components, summed over the toroidal modes.
+struct PertF { double ER, EP, EZ, BR, BP, BZ, gR, gP, gZ, dT; };
+
+// The marker moves in the total fields: B = B0 + B1, E-dagger = E1 - (mu/q) grad(|B|0 + B1par) (PAPER.md:78 with the
+// total field strength).  The weight equation keeps its linear right-hand side (Eqs. 10-13 with the equilibrium b0,
+// evaluated at (x_l, v_l)); wdot returns it and the caller applies the factor (1 - w) of Eq. (8).
+__device__ __forceinline__ void push_eq_nl(const PushParams &P, const StepGeom &g, const EqOut &f, const PertF &p,
+                                           Marker &s, double &wdot) {
+    const double rinv = g.rinv, cph = g.cph, sph = g.sph;
+    const double B0R = -DM(f.psi_Z, rinv), B0P = DM(f.F, rinv), B0Z = DM(f.psi_R, rinv);
+    const double BR = DA(B0R, p.BR), BP = DA(B0P, p.BP), BZ = DA(B0Z, p.BZ);
+    const double muq = DM(s.mu, P.inv_q);
+    const double ER = M3DK_FMA(-muq, DA(f.Bm_R, p.gR), p.ER), EP = M3DK_FMA(-muq, p.gP, p.EP),
+                 EZ = M3DK_FMA(-muq, DA(f.Bm_Z, p.gZ), p.EZ);
+    const double Bx = M3DK_FMA(BR, cph, -DM(BP, sph)), By = M3DK_FMA(BR, sph, DM(BP, cph)), Bz = BZ;
+    const double Ex = M3DK_FMA(ER, cph, -DM(EP, sph)), Ey = M3DK_FMA(ER, sph, DM(EP, cph)), Ez = EZ;
+    const double h = P.h;
+    const double ux = M3DK_FMA(h, Ex, s.vx), uy = M3DK_FMA(h, Ey, s.vy), uz = M3DK_FMA(h, Ez, s.vz);
+    const double tx = DM(h, Bx), ty = DM(h, By), tz = DM(h, Bz);
+    const double sc = DM(2.0, m3dk_rcp(DA(1.0, M3DK_FMA(tx, tx, M3DK_FMA(ty, ty, DM(tz, tz))))));
+    const double px = DA(ux, M3DK_FMA(uy, tz, -DM(uz, ty))), py = DA(uy, M3DK_FMA(uz, tx, -DM(ux, tz))),
+                 pz = DA(uz, M3DK_FMA(ux, ty, -DM(uy, tx)));
+    const double wx = M3DK_FMA(sc, M3DK_FMA(py, tz, -DM(pz, ty)), ux), wy = M3DK_FMA(sc, M3DK_FMA(pz, tx, -DM(px, tz)), uy),
+                 wz = M3DK_FMA(sc, M3DK_FMA(px, ty, -DM(py, tx)), uz);
+    const double nvx = M3DK_FMA(h, Ex, wx), nvy = M3DK_FMA(h, Ey, wy), nvz = M3DK_FMA(h, Ez, wz);
+    PertW W;
+    weight_coeffs(P, g, f, B0R, B0P, B0Z, s, nvx, nvy, nvz, W);
+    double a = DM(W.aER, p.ER);
+    a = M3DK_FMA(W.aEP, p.EP, a); a = M3DK_FMA(W.aEZ, p.EZ, a);
+    a = M3DK_FMA(W.bBR, p.BR, a); a = M3DK_FMA(W.bBZ, p.BZ, a);
+    a = M3DK_FMA(W.gR, p.gR, a); a = M3DK_FMA(W.gP, p.gP, a); a = M3DK_FMA(W.gZ, p.gZ, a);
+    wdot = M3DK_FMA(W.dT, p.dT, a);
     s.x = M3DK_FMA(P.dt, nvx, s.x); s.y = M3DK_FMA(P.dt, nvy, s.y); s.z = M3DK_FMA(P.dt, nvz, s.z);
     s.vx = nvx; s.vy = nvy; s.vz = nvz;
 }

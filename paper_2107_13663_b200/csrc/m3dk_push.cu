@@ -263,10 +263,113 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
     if (kHist) rank_finish<R>(P.rank, mo, on, peers, base);
 }
 
+// ---- the same step in the non-linear trajectory mode (mode 1: PAPER.md:108, :130; reading G21) ------------------------
+// All perturbed fields are needed BEFORE the velocity update (the marker moves in the total fields), so they are
+// accumulated per marker (10 values) and the folding trick of the linear mode does not apply; B1_phi (quad 3) enters.
+template <int R, bool kHist, bool kSmem, class IO>
+__device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, const double *__restrict__ tile,
+                                          const long (&mi)[R], const long (&mo)[R], const bool (&on)[R]) {
+    Marker s[R];
+    StepGeom g[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (on[r]) { io.load_pos(mi[r], s[r].x, s[r].y, s[r].z, s[r].w); io.load_vel(mi[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu); }
+        else { s[r].x = 1.0; s[r].y = 0.0; s[r].z = 0.0; s[r].w = 0.0; s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
+    }
+    const Quad hd = ldq_t<kSmem>(tile);
+    const double Rc = hd.a, Zc = hd.b, se = hd.c;
+    double xi[R], eta[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        step_geometry(s[r], g[r]);
+        xi[r] = __dmul_rn(__dsub_rn(g[r].R, Rc), se); eta[r] = __dmul_rn(__dsub_rn(s[r].z, Zc), se);
+    }
+    double v[R][4], dx[R][4], de[R][4];
+    Ring ring;
+    ring_fill<kSmem>(ring, tile + kTileHeader);
+    quad_vd<R, kSmem>(tile + kTileHeader, tile + kTileHeader, ring, xi, eta, v, dx, de);   // (psi0, |B|0, F0, kappa)
+    EqOut f[R];
+    PertF pf[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        f[r].psi_R = __dmul_rn(dx[r][0], se); f[r].psi_Z = __dmul_rn(de[r][0], se);
+        f[r].Bm = v[r][1]; f[r].Bm_R = __dmul_rn(dx[r][1], se); f[r].Bm_Z = __dmul_rn(de[r][1], se);
+        f[r].F = v[r][2]; f[r].kappa = v[r][3];
+        pf[r].ER = pf[r].EP = pf[r].EZ = pf[r].BR = pf[r].BP = pf[r].BZ = pf[r].gR = pf[r].gP = pf[r].gZ = pf[r].dT = 0.0;
+    }
+    for (int md = 0; md < P.f.n_modes; ++md) {
+        const int n = P.f.n_tor[md];
+        const double om = P.f.omega[md];
+        double cth[R], sth[R], nri[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            mode_phase(n, g[r].cph, g[r].sph, P.cwt[md], P.swt[md], cth[r], sth[r]);
+            nri[r] = __dmul_rn((double)n, g[r].rinv);
+        }
+        const double *pm = tile + kTileHeader + kTileEq + kTileMode * md;
+        ring_fill<kSmem>(ring, pm);
+        quad_vd<R, kSmem>(pm, pm + kQuad, ring, xi, eta, v, dx, de);                          // E_R, E_phi
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            pf[r].ER = __dadd_rn(pf[r].ER, re_part(v[r][0], v[r][1], cth[r], sth[r]));
+            pf[r].EP = __dadd_rn(pf[r].EP, re_part(v[r][2], v[r][3], cth[r], sth[r]));
+        }
+        quad_vd<R, kSmem>(pm + kQuad, pm + 2 * kQuad, ring, xi, eta, v, dx, de);             // E_Z, B_R
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            pf[r].EZ = __dadd_rn(pf[r].EZ, re_part(v[r][0], v[r][1], cth[r], sth[r]));
+            pf[r].BR = __dadd_rn(pf[r].BR, re_part(v[r][2], v[r][3], cth[r], sth[r]));
+        }
+        quad_vd<R, kSmem>(pm + 2 * kQuad, pm + 3 * kQuad, ring, xi, eta, v, dx, de);         // B_par (+ gradient), B_Z
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            pf[r].BZ = __dadd_rn(pf[r].BZ, re_part(v[r][2], v[r][3], cth[r], sth[r]));
+            const double qd = M3DK_FMA(v[r][0], sth[r], __dmul_rn(v[r][1], cth[r]));   // d/dphi -> -n qd, d/dt -> omega qd
+            pf[r].gR = __dadd_rn(pf[r].gR, re_part(__dmul_rn(dx[r][0], se), __dmul_rn(dx[r][1], se), cth[r], sth[r]));
+            pf[r].gP = __dsub_rn(pf[r].gP, __dmul_rn(nri[r], qd));
+            pf[r].gZ = __dadd_rn(pf[r].gZ, re_part(__dmul_rn(de[r][0], se), __dmul_rn(de[r][1], se), cth[r], sth[r]));
+            pf[r].dT = M3DK_FMA(om, qd, pf[r].dT);
+        }
+        quad_vd<R, kSmem>(pm + 3 * kQuad, pm, ring, xi, eta, v, dx, de);                      // B_phi
+#pragma unroll
+        for (int r = 0; r < R; ++r) pf[r].BP = __dadd_rn(pf[r].BP, re_part(v[r][0], v[r][1], cth[r], sth[r]));
+    }
+    double Rn[R], Zn[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const double w_old = s[r].w;
+        double wdot;
+        push_eq_nl(P, g[r], f[r], pf[r], s[r], wdot);
+        // Eq. (8) with (1 - w) kept, explicit on the staggered grid (readings G9, G21)
+        if (P.f.n_modes > 0) s[r].w = M3DK_FMA(P.dt, __dmul_rn(__dsub_rn(1.0, w_old), wdot), w_old);
+        Rn[r] = m3dk_sqrt(M3DK_FMA(s[r].x, s[r].x, __dmul_rn(s[r].y, s[r].y)));
+        Zn[r] = s[r].z;
+    }
+    int key[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        int ne = -1;
+        if (on[r]) {
+            io.store_pos(mo[r], s[r].x, s[r].y, s[r].z, s[r].w);
+            io.store_vel(mo[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
+            if (P.f.n_modes > 0) io.store_w(mo[r], s[r].w);
+            ne = locate_any(P.f, Rn[r], Zn[r]);
+            io.store_key(mo[r], ne);
+        }
+        key[r] = ne < 0 ? P.f.n_elems : ne;
+    }
+    if (kHist) {
+        unsigned peers[R];
+        int base[R];
+        hist_issue<R>(P.hist, key, on, peers, base);
+        rank_finish<R>(P.rank, mo, on, peers, base);
+    }
+}
+
 // ---- generic push: one marker per thread, any marker order (every thread gathers its own element's tile) ------------
 // kRec = false: the caller's SoA arrays in place (sort_interval = 0).  kRec = true: the records of the ordered pipeline
 // in place, for the steps between two sorts when sort_interval > 1.
-template <bool kRec, bool kHist>
+template <bool kRec, bool kHist, int kMode>
 __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant__ PushParams P) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < P.n;
@@ -277,8 +380,15 @@ __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant
     // the tile loads may be speculated above the `on` tests: e is clamped to a valid element for addressing
     const double *tile = P.f.tiles + (size_t)max(e, 0) * P.f.tile_stride;
     if (__any_sync(0xffffffffu, on[0])) {
-        if (kRec) { const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems}; step_R<1, false, false>(P, io, tile, m, m, on); }
-        else { const SoAIO io{P.a, P.f.n_elems}; step_R<1, false, false>(P, io, tile, m, m, on); }
+        if (kRec) {
+            const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems};
+            if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on);
+            else step_R<1, false, false>(P, io, tile, m, m, on);
+        } else {
+            const SoAIO io{P.a, P.f.n_elems};
+            if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on);
+            else step_R<1, false, false>(P, io, tile, m, m, on);
+        }
     }
     if (kHist) {
         const int k = valid ? P.rc.key[i] : 0;
@@ -308,7 +418,7 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
 // bulk copy per item (double-buffered per warp: the next item's tile travels while this one computes), and every
 // coefficient read is a broadcast LDS that feeds kItemR markers per lane.  Static assignment: the warps of a CTA take
 // consecutive items.  Items of the pseudo-element n_elems hold the lost markers: frozen, they only enter the histogram.
-template <bool kHist>
+template <bool kHist, int kMode>
 __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_kernel(const __grid_constant__ PushParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int kWarps = kPushThreads / 32;
@@ -382,7 +492,8 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
         } else {
             mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
             phase ^= 1u << b;
-            step_R<kItemR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
+            if (kMode == 1) step_R_nl<kItemR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
+            else step_R<kItemR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
         }
         b ^= 1;
         it += stride;
@@ -467,7 +578,8 @@ cudaError_t launch_push_soa(m3dk_ctx *c, long n, double dt, double t) {
     if (n == 0) return cudaSuccess;
     PushParams P = make_params(c, c->user, n, dt, t);
     c->kernel_launches += 1;
-    push_generic_kernel<false, false><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
+    if (c->mode == 1) push_generic_kernel<false, false, 1><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
+    else push_generic_kernel<false, false, 0><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
     return cudaGetLastError();
 }
 
@@ -489,7 +601,8 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
         P.items = c->sb.items; P.n_items = c->sb.ioffs + c->f.n_elems + 1;
         const unsigned grid = (unsigned)(c->sm_count * M3DK_PUSH_MINBLOCKS);
         const size_t smem = (size_t)(kPushThreads / 32) * 2 * (c->f.tile_stride * 8 + 8);
-        auto kern = with_hist ? push_items_kernel<true> : push_items_kernel<false>;
+        auto kern = c->mode == 1 ? (with_hist ? push_items_kernel<true, 1> : push_items_kernel<false, 1>)
+                                 : (with_hist ? push_items_kernel<true, 0> : push_items_kernel<false, 0>);
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         kern<<<grid, kPushThreads, smem, c->stream>>>(P);
@@ -497,8 +610,9 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
     } else {
         P.rc.out = c->sb.rec[c->cur];
         const unsigned grid = (unsigned)((n + 127) / 128);
-        if (with_hist) push_generic_kernel<true, true><<<grid, 128, 0, c->stream>>>(P);
-        else push_generic_kernel<true, false><<<grid, 128, 0, c->stream>>>(P);
+        auto kern = c->mode == 1 ? (with_hist ? push_generic_kernel<true, true, 1> : push_generic_kernel<true, false, 1>)
+                                 : (with_hist ? push_generic_kernel<true, true, 0> : push_generic_kernel<true, false, 0>);
+        kern<<<grid, 128, 0, c->stream>>>(P);
     }
     return cudaGetLastError();
 }

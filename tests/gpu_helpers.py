@@ -27,17 +27,17 @@ def take(markers: dict, idx):
     return {k: np.ascontiguousarray(markers[k][idx]) for k in KEYS}
 
 
-def make_pusher(w, verify=True, markers=None, sort_interval=0, t0=0.0):
+def make_pusher(w, verify=True, markers=None, sort_interval=0, t0=0.0, mode=0):
     p = m3dk.Pusher(device=0, verify=verify)
     p.fields_create(w.node_RZ, w.tri, w.eq_coef, w.n_tor if w.n_modes else None, w.omega if w.n_modes else None,
                     w.pert_coef if w.n_modes else None)
     p.particles_init(w.markers if markers is None else markers, w.charge, w.mass, w.f0)
-    p.set_options(sort_interval=sort_interval, t0=t0)
+    p.set_options(sort_interval=sort_interval, mode=mode, t0=t0)
     return p
 
 
-def oracle_of(w):
-    return oracle.Mesh.of(w), oracle.species_of(w)
+def oracle_of(w, mode=0):
+    return oracle.Mesh.of(w), oracle.species_of(w, mode=mode)
 
 
 def oracle_push(mesh, sp, markers, nsteps, dt, t0=0.0, step0=0, elem=None):
