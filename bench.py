@@ -36,7 +36,7 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA lanes 
 
 
 # ---- algorithmic work per marker-step (DESIGN.md section 7 derives these) ---------------------------------------------
-def algorithmic_flops(n_modes: int) -> float:
+def algorithmic_flops(n_modes: int, mode: int = 0) -> float:
     """fp64 operations per marker-step counted from the kernel's formulas: FMA = 2, add / mul = 1,
     reciprocal / rsqrt / sqrt = 1 each (their Newton steps are not counted); minimal-multiplication Horner: value of a
     21-term quintic = 20 FMA, value + d/dxi + d/deta = 38 FMA.  The fp32 arithmetic of the element search is not counted."""
@@ -47,6 +47,8 @@ def algorithmic_flops(n_modes: int) -> float:
     pert = 2 * (10 * 20 + 2 * 38)             # E_R E_phi E_Z B_R B_Z (re, im) values; B_par (re, im) value + gradient
     fold = 25 + 25 + 23                       # phase exp(i(n phi - omega t)) for n = 3, folding 5 + 1 complex fields into dw/dt
     weight = 86 + 2                           # coefficients of dw/dt (Eqs. 8-13 incl. kappa_E), w update
+    if mode == 1:                             # non-linear trajectories: + B_phi (re, im), total fields, (1 - w)
+        return eq + common + weight + 30 + n_modes * (pert + 2 * 2 * 20 + fold + 5)
     return eq + common + weight + n_modes * (pert + fold)
 
 
@@ -127,6 +129,9 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+ORACLE_MODE = [0]     # set from --mode: the oracle is timed in the same mode as the CUDA path
+
+
 def oracle_bounded_sample(w, n_sample: int, target_s: float = 15.0):
     """The oracle on a bounded sample sized for about target_s seconds of CPU work on this box: a short calibration run
     (every 1024-th marker, 20 steps) fixes the number of steps for the id = 0 (mod stride) sub-sample."""
@@ -142,7 +147,7 @@ def oracle_sample_rate(w, sample_stride: int, nsteps: int, nthreads: int = 0):
     import oracle
     idx = slice(0, None, sample_stride)
     mk = {k: np.ascontiguousarray(v[idx]) for k, v in w.markers.items()}
-    mesh, sp = oracle.Mesh.of(w), oracle.species_of(w)
+    mesh, sp = oracle.Mesh.of(w), oracle.species_of(w, mode=ORACLE_MODE[0])
     oracle.push_fe(mesh, sp, {k: v[:256] for k, v in mk.items()}, 1, w.dt)      # touch code and tables
     t0 = time.perf_counter()
     oracle.push_fe(mesh, sp, mk, nsteps, w.dt, nthreads=nthreads)
@@ -162,7 +167,8 @@ def build_workload(args, rank: int):
 def config_dict(args, w, sort_interval, world):
     return {"workload": f"BASELINE.json configs[{args.config}] ({w.name})", "n_markers_per_gpu": w.n_markers,
             "mesh": f"{w.nx}x{w.nx} cells, {w.n_elems} triangles", "n_modes": w.n_modes, "dt": w.dt,
-            "sort_interval": sort_interval, "parallelism": f"{world} independent marker shard(s), no collective",
+            "sort_interval": sort_interval, "mode": "linear delta-f" if args.mode == 0 else "non-linear trajectories",
+            "parallelism": f"{world} independent marker shard(s), no collective",
             "l2": "inputs larger than L2 (marker state %.0f MB + tables %.0f MB per GPU)" % (
                 w.n_markers * 64 / 1e6, (w.eq_coef.nbytes + w.pert_coef.nbytes) / 1e6)}
 
@@ -206,7 +212,7 @@ def run_ours(args, rank, world, local_rank):
     p.fields_create(w.node_RZ, w.tri, w.eq_coef, w.n_tor if w.n_modes else None, w.omega if w.n_modes else None,
                     w.pert_coef if w.n_modes else None)
     p.particles_init(w.markers, w.charge, w.mass, w.f0)
-    p.set_options(sort_interval=si, t0=0.0)
+    p.set_options(sort_interval=si, mode=args.mode, t0=0.0)
 
     def barrier():
         if world > 1:
@@ -236,12 +242,12 @@ def run_ours(args, rank, world, local_rank):
     host = {k: torch.from_numpy(np.ascontiguousarray(w.markers[k])).pin_memory() for k in m3dk.STATE_KEYS}
     out = {k: torch.empty(N, dtype=torch.float64).pin_memory() for k in m3dk.STATE_KEYS}
     Ke = K
-    p.upload(host); p.set_options(sort_interval=si, t0=0.0); p.push(1, w.dt); p.download(out)      # warm the path
+    p.upload(host); p.set_options(sort_interval=si, mode=args.mode, t0=0.0); p.push(1, w.dt); p.download(out)      # warm the path
     barrier()
     f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     f0.record(p.stream)
     p.upload(host)
-    p.set_options(sort_interval=si, t0=0.0)
+    p.set_options(sort_interval=si, mode=args.mode, t0=0.0)
     p.push(Ke, w.dt)
     p.download(out)
     f1.record(p.stream)
@@ -255,7 +261,7 @@ def run_ours(args, rank, world, local_rank):
 
     hbm_gbs, hbm_src, _ = measured_peaks()
     fp64_meas = p.fp64_peak_tflops()
-    flops = algorithmic_flops(w.n_modes) * N
+    flops = algorithmic_flops(w.n_modes, args.mode) * N
     bytes_push = algorithmic_bytes_push(w.n_modes, ordered=si > 0) * N
     push_ms = tm["push_ms"] / max(1, tm["push_launches"])
     t_alu, t_hbm = flops / (FP64_NOMINAL_TFLOPS * 1e12), bytes_push / (hbm_gbs * 1e9)
@@ -269,7 +275,7 @@ def run_ours(args, rank, world, local_rank):
     roof.update({"kernel": "push kernel (a1-a10)", "launch_ms": push_ms, "launches": tm["push_launches"],
                  "share_of_step": tm["push_ms"] / ms, "traffic": ncu_traffic(args.config, si),
                  "fp64_peak_measured_tflops": fp64_meas,
-                 "flops_per_marker_step": algorithmic_flops(w.n_modes),
+                 "flops_per_marker_step": algorithmic_flops(w.n_modes, args.mode),
                  "hbm_bytes_per_marker_step": algorithmic_bytes_push(w.n_modes, ordered=si > 0),
                  "sort_ms_per_sort": tm["sort_ms"] / max(1, tm["sort_launches"]), "sorts": tm["sort_launches"]})
     # whole-step roofline: the binding one of (all flops / fp64 peak) and (all HBM bytes incl. sorts / HBM bandwidth)
@@ -346,6 +352,8 @@ def main():
     ap.add_argument("--dt-gyro", type=float, default=None)
     ap.add_argument("--sort-interval", type=int, default=None)
     ap.add_argument("--ref-sample", type=int, default=65536, help="markers in the oracle's bounded sample")
+    ap.add_argument("--mode", type=int, default=0, choices=[0, 1],
+                    help="0: linear delta-f (the headline); 1: non-linear trajectories (SURVEY.md 8(f)-1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4] sweep: one JSON line per (n, dt, sort interval)")
     ap.add_argument("--sweep-n", type=int, nargs="+", default=[1 << 20, 1 << 22, 1 << 24, 1 << 26])
@@ -354,6 +362,7 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
+    ORACLE_MODE[0] = args.mode
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
