@@ -26,7 +26,10 @@
  * Gaussian elimination of the 3x3 system instead of the Boris t/s vectors, brute-force / full-list element
  * search instead of the prioritised bucket search.
  *
- * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1-P15 of SURVEY.md 8(c); see DESIGN.md section 3.
+ * Mode 1 (non-linear trajectories; reading G21): step 5 uses the total fields,
+ * B = B0 + B1 and E-dagger = E1 - (mu/q) grad(|B|0 + B1par), and step 7 keeps the factor (1 - w) of Eq. (8).
+ *
+ * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1-P15 of SURVEY.md 8(c) and P16-P19 for mode 1; see DESIGN.md section 4.
  * Unpinned by the paper (fixed by DESIGN.md readings, parity unpinned): the kappa_E model (G7),
  * the construction of the synthetic perturbations (G19), rho* (G17).
  */
