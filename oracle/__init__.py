@@ -57,6 +57,8 @@ def lib():
         L.orc_push_analytic.restype = C.c_long
         L.orc_push_analytic.argtypes = [C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 8 + [
             C.c_int, C.c_double, C.c_double, C.c_long, C.c_int]
+        L.orc_deposit.restype = C.c_long
+        L.orc_deposit.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_dp]
         L.orc_trace.restype = C.c_long
         L.orc_trace.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_long, C.c_double,
                                 C.c_double, C.c_long, c_dp]
@@ -186,6 +188,16 @@ def push_analytic(an: Analytic, sp: Species, markers: dict, nsteps: int, dt: flo
     n = st["x"].shape[0]
     lib().orc_push_analytic(C.byref(an), C.byref(sp), n, *ptrs, int(nsteps), float(dt), float(t0), int(step0), int(nthreads))
     return st
+
+
+def deposit(mesh: "Mesh", sp: Species, markers: dict):
+    """Right-hand sides of Eqs. (17)-(18) with a delta-function shape: rhs[n_elems][2][1 + 2 n_modes][21], n_lost."""
+    st, ptrs = _state(markers)
+    n = st["x"].shape[0]
+    H = 1 + 2 * mesh.n_modes
+    rhs = np.zeros((mesh.n_elems, 2, H, 21), dtype=np.float64)
+    lost = lib().orc_deposit(mesh.h, C.byref(sp), n, *ptrs, rhs.ctypes.data_as(c_dp))
+    return rhs, int(lost)
 
 
 def trace(sp: Species, state8, nsteps: int, dt: float, *, mesh: Optional[Mesh] = None, an: Optional[Analytic] = None,

@@ -600,6 +600,56 @@ double orc_weight_rhs(const double *fields18, const orc_species *sp, double R, c
     return weight_rhs(&f, sp, R, vl_cyl, mu);
 }
 
+/* ================================================================================================ */
+/* Moment deposition: right-hand sides of the Galerkin projection of the pressure moments with a
+ * delta-function particle shape, Eqs. (17)-(18):
+ *     rhs_par [e][h][k] = sum over markers p in element e of  w_p m v_par,p^2    nu_k(x_p) T_h(phi_p)
+ *     rhs_perp[e][h][k] = sum over markers p in element e of  w_p mu_p |B|0(x_p) nu_k(x_p) T_h(phi_p)
+ * nu_k = xi^i eta^j: the element's own polynomial basis (reading G10); T_0 = 1, T_{2m+1} = cos(n_m phi),
+ * T_{2m+2} = sin(n_m phi) for the toroidal modes of the field set (reading G22: the delta function is normalised in
+ * physical volume, so the Jacobian J of Eq. (17) is absorbed by it; v_par = v . B0/|B0| with the marker's v as stored).
+ * rhs[n_elems][2][1 + 2 n_modes][21], zero-filled here.  Lost markers (outside every triangle) deposit nothing.
+ * Plain loops, one marker at a time, in marker order.                                                             */
+long orc_deposit(const orc_mesh *m, const orc_species *sp, long n, const double *x, const double *y, const double *z,
+                 const double *vx, const double *vy, const double *vz, const double *mu, const double *w, double *rhs)
+{
+    const int H = 1 + 2 * m->n_modes;
+    long lost = 0;
+    memset(rhs, 0, (size_t)m->n_elems * 2 * H * NCOEF * sizeof(double));
+    for (long p = 0; p < n; ++p) {
+        double R = sqrt(x[p] * x[p] + y[p] * y[p]), phi = atan2(y[p], x[p]), Z = z[p];
+        int e = locate_grid(m, R, Z);
+        if (e < 0) { lost++; continue; }
+        orc_fields f;
+        fe_fields(m, e, R, phi, Z, 0.0, &f);
+        double B0[3] = {-f.psi_Z / R, f.F / R, f.psi_R / R};
+        double B0n = sqrt(B0[0] * B0[0] + B0[1] * B0[1] + B0[2] * B0[2]);
+        double c = x[p] / R, sn = y[p] / R;
+        double vc[3] = {vx[p] * c + vy[p] * sn, -vx[p] * sn + vy[p] * c, vz[p]};
+        double vpar = (vc[0] * B0[0] + vc[1] * B0[1] + vc[2] * B0[2]) / B0n;
+        double a[2] = {w[p] * sp->mass * vpar * vpar, w[p] * mu[p] * f.Bm};
+        double Rc, Zc, s;
+        elem_frame(m, e, &Rc, &Zc, &s);
+        double xi = (R - Rc) * s, eta = (Z - Zc) * s;
+        double xp[DEG + 1], ep[DEG + 1];
+        xp[0] = 1.0; ep[0] = 1.0;
+        for (int q = 1; q <= DEG; ++q) { xp[q] = xp[q - 1] * xi; ep[q] = ep[q - 1] * eta; }
+        for (int mom = 0; mom < 2; ++mom)
+            for (int h = 0; h < H; ++h) {
+                double T = 1.0;
+                if (h > 0) {
+                    double nn = (double)m->n_tor[(h - 1) / 2];
+                    T = ((h - 1) % 2 == 0) ? cos(nn * phi) : sin(nn * phi);
+                }
+                double *out = rhs + (((size_t)e * 2 + mom) * H + h) * NCOEF;
+                int k = 0;
+                for (int j = 0; j <= DEG; ++j)
+                    for (int i = 0; i <= DEG - j; ++i, ++k) out[k] += a[mom] * T * (xp[i] * ep[j]);
+            }
+    }
+    return lost;
+}
+
 /* reference counting sort by element key (lost markers, key -1, last): returns a permutation.  Any
  * permutation with non-decreasing keys is valid (SURVEY.md 8(c) "Sort oracle"); this one is stable.   */
 void orc_sort_perm(long n, const int *elem, int n_elems, long *perm)

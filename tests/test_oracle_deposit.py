@@ -1,0 +1,126 @@
+"""Pins of the oracle's moment deposition (Eqs. 17-18 with a delta-function shape;
+readings G10, G22).  Checked against what the mathematics fixes, never against itself: sums that must equal totals
+computed from the ANALYTIC equilibrium, the closed-form integrals of monomials over a triangle (Monte Carlo limit),
+the orthogonality of the toroidal harmonics, linearity.  CPU only."""
+from math import factorial
+
+import numpy as np
+import pytest
+
+import synth
+from synth.mesh import element_frames, monomial_exponents
+
+
+@pytest.fixture(scope="module")
+def wl():
+    return synth.make_config(1, n_markers=20000, nx=16)
+
+
+def _weights(w, seed=3):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    mk = {k: v.copy() for k, v in w.markers.items()}
+    mk["w"] = rng.normal(size=w.n_markers) * 1e-3
+    return mk
+
+
+def test_d1_unit_test_function_sums_to_the_analytic_totals(orc, wl):
+    """nu_0 = 1, T_0 = 1: summing the k = 0, h = 0 entries over the elements must give sum_p w m v_par^2 and
+    sum_p w mu |B|, here with v_par and |B| from the ANALYTIC equilibrium (the tables are quintic fits of it: agreement to
+    the fit error pins b0, |B|0, the element assignment and the indexing of the two moments)."""
+    mk = _weights(wl)
+    rhs, lost = orc.deposit(orc.Mesh.of(wl), orc.species_of(wl), mk)
+    assert lost == 0 and rhs.shape == (wl.n_elems, 2, 3, 21)
+    eq = wl.eq
+    R = np.hypot(mk["x"], mk["y"])
+    BR, BP, BZ = eq.B_cyl(R, mk["z"])
+    Bn = np.sqrt(BR ** 2 + BP ** 2 + BZ ** 2)
+    c, s = mk["x"] / R, mk["y"] / R
+    vpar = ((mk["vx"] * c + mk["vy"] * s) * BR + (-mk["vx"] * s + mk["vy"] * c) * BP + mk["vz"] * BZ) / Bn
+    par, perp = mk["w"] * wl.mass * vpar ** 2, mk["w"] * mk["mu"] * Bn
+    for mom, a in ((0, par), (1, perp)):
+        tot, ref = rhs[:, mom, 0, 0].sum(), a.sum()
+        assert abs(tot - ref) < 2e-5 * np.abs(a).sum(), (mom, tot, ref)
+    # per element, and the first moments: sum_p a_p xi_p = s_e (sum_p a_p R_p - R_c sum_p a_p) (frame of reading G10)
+    mesh = orc.Mesh.of(wl)
+    elem = mesh.locate(R, mk["z"])
+    cen, se = element_frames(wl.node_RZ, wl.tri)
+    for mom, a in ((0, par), (1, perp)):
+        s0 = np.bincount(elem, weights=a, minlength=wl.n_elems)
+        sR = np.bincount(elem, weights=a * R, minlength=wl.n_elems)
+        sZ = np.bincount(elem, weights=a * mk["z"], minlength=wl.n_elems)
+        scale = np.abs(s0).max()
+        assert np.abs(rhs[:, mom, 0, 0] - s0).max() < 2e-5 * scale
+        assert np.abs(rhs[:, mom, 0, 1] - se * (sR - cen[:, 0] * s0)).max() < 2e-5 * scale       # k = 1: xi
+        assert np.abs(rhs[:, mom, 0, 6] - se * (sZ - cen[:, 1] * s0)).max() < 2e-5 * scale       # k = 6: eta
+
+
+def test_d2_monte_carlo_limit_is_the_integral_of_the_monomials_over_the_triangle(orc):
+    """Markers uniform in ONE triangle, identical w mu |B| up to the slow variation of |B|: rhs_perp[k] / rhs_perp[0] ->
+    (1/A) int_T xi^i eta^j dA, which has the closed form 2A a! b! c! / (a + b + c + 2)! in barycentric monomials; here the
+    expectation is computed exactly by expanding xi^i eta^j in the vertices' local coordinates."""
+    w = synth.make_config(1, n_markers=8, nx=8)
+    e = 70
+    P = w.node_RZ[w.tri[e]]
+    rng = np.random.Generator(np.random.PCG64(12))
+    N = 400000
+    u = rng.random((N, 2))
+    flip = u.sum(1) > 1
+    u[flip] = 1 - u[flip]
+    lam = np.stack([1 - u[:, 0] - u[:, 1], u[:, 0], u[:, 1]], 1)
+    RZ = lam @ P
+    phi = rng.uniform(0, 2 * np.pi, N)
+    eqB = np.sqrt(sum(b ** 2 for b in w.eq.B_cyl(RZ[:, 0], RZ[:, 1])))
+    mk = dict(x=RZ[:, 0] * np.cos(phi), y=RZ[:, 0] * np.sin(phi), z=RZ[:, 1], vx=np.zeros(N), vy=np.zeros(N), vz=np.zeros(N),
+              mu=1.0 / eqB, w=np.ones(N))                   # w mu |B| = 1 for every marker (up to the fit error)
+    rhs, lost = orc.deposit(orc.Mesh.of(w), orc.species_of(w), mk)
+    assert lost == 0
+    got = rhs[e, 1, 0] / N
+    assert np.abs(rhs[np.arange(w.n_elems) != e]).max() == 0.0          # nothing leaks into other elements
+    cen, se = element_frames(w.node_RZ, w.tri)
+    V = (P - cen[e]) * se[e]                                            # vertices in the local frame: xi = sum_v lam_v V_v0
+
+    def bary_integral(a, b, c):                                         # (1/A) int lam1^a lam2^b lam3^c dA
+        return 2.0 * factorial(a) * factorial(b) * factorial(c) / factorial(a + b + c + 2)
+
+    from itertools import product
+    loc = (RZ - cen[e]) * se[e]                                          # the samples in the local frame (for the error bar only)
+    for k, (i, j) in enumerate(monomial_exponents()):
+        # expand (sum_v lam_v x_v)^i (sum_v lam_v y_v)^j by brute-force multinomial enumeration
+        exp = 0.0
+        for pick in product(range(3), repeat=int(i + j)):
+            coef = np.prod([V[v, 0] for v in pick[:i]]) * np.prod([V[v, 1] for v in pick[i:]])
+            exp += coef * bary_integral(pick.count(0), pick.count(1), pick.count(2))
+        sigma = np.std(loc[:, 0] ** i * loc[:, 1] ** j) / np.sqrt(N)       # Monte Carlo standard error of this mean
+        assert abs(got[k] - exp) < 6.0 * sigma + 3e-6 * max(abs(exp), 1e-3), (k, i, j, got[k], exp, sigma)
+
+
+def test_d3_toroidal_harmonics_are_orthogonal_projections(orc):
+    """Markers at ONE poloidal point, evenly spaced in phi, weights w = A + B cos(n phi) + C sin(n phi) (n the mode of the
+    field set): T_0 picks N A, the cos harmonic N B / 2, the sin harmonic N C / 2 (discrete orthogonality)."""
+    w = synth.make_config(3, n_markers=8, nx=8)             # n = 3
+    n = int(w.n_tor[0])
+    N = 360
+    phi = 2 * np.pi * np.arange(N) / N
+    R0, Z0 = 3.37, 0.21
+    A, Bc, Cs = 0.7, -0.4, 0.25
+    Bm = np.sqrt(sum(b ** 2 for b in w.eq.B_cyl(np.array([R0]), np.array([Z0]))))[0]
+    mk = dict(x=R0 * np.cos(phi), y=R0 * np.sin(phi), z=np.full(N, Z0), vx=np.zeros(N), vy=np.zeros(N), vz=np.zeros(N),
+              mu=np.full(N, 1.0 / Bm), w=A + Bc * np.cos(n * phi) + Cs * np.sin(n * phi))
+    rhs, _ = orc.deposit(orc.Mesh.of(w), orc.species_of(w), mk)
+    e = int(orc.Mesh.of(w).locate(np.array([R0]), np.array([Z0]))[0])
+    got = rhs[e, 1, :, 0]
+    assert np.allclose(got, [N * A, N * Bc / 2, N * Cs / 2], rtol=2e-5, atol=1e-9), got
+    assert np.abs(rhs[e, 0]).max() == 0.0                   # v = 0: no parallel pressure
+
+
+def test_d4_linear_in_w_and_independent_of_marker_order(orc, wl):
+    mk = _weights(wl)
+    mesh, sp = orc.Mesh.of(wl), orc.species_of(wl)
+    a, _ = orc.deposit(mesh, sp, mk)
+    mk2 = dict(mk)
+    mk2["w"] = 3.0 * mk["w"]
+    b, _ = orc.deposit(mesh, sp, mk2)
+    assert np.abs(b - 3.0 * a).max() <= 1e-13 * np.abs(a).max()
+    perm = np.random.Generator(np.random.PCG64(1)).permutation(wl.n_markers)
+    c, _ = orc.deposit(mesh, sp, {k: v[perm] for k, v in mk.items()})
+    assert np.abs(c - a).max() <= 1e-12 * np.abs(a).max()
