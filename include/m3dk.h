@@ -152,6 +152,20 @@ int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, double *hz, d
 int m3dk_eval_fields(m3dk_ctx *ctx, long n, const double *R, const double *phi, const double *Z, double t,
                      int *elem_out, double *out);
 
+/* Moment deposition: right-hand sides of the Galerkin projection of the energetic-particle pressure
+ * moments with a delta-function particle shape, Eqs. (17)-(18) (readings G10, G22):
+ *   rhs[e][0][h][k] = sum over the markers p in element e of  w_p m v_par,p^2    nu_k(x_p) T_h(phi_p)     (parallel)
+ *   rhs[e][1][h][k] = sum over the markers p in element e of  w_p mu_p |B|0(x_p) nu_k(x_p) T_h(phi_p)     (perpendicular)
+ * nu_k = xi^i eta^j, the element's polynomial basis in its local frame (same order as the coefficient tables);
+ * T_0 = 1, T_{2m+1} = cos(n_tor[m] phi), T_{2m+2} = sin(n_tor[m] phi); v_par = v . B0/|B0| with the stored v (v_{l-1/2}).
+ * The delta function is normalised in physical volume, so no Jacobian factor appears (G22); the mass-matrix solve that
+ * turns these sums into pressure coefficients belongs to the MHD code and is out of scope.  Lost markers deposit nothing.
+ * rhs: DEVICE, m3dk_deposit_bytes() bytes = [n_elems][2][1 + 2 n_modes][21] doubles, overwritten.  Asynchronous.  Works on
+ * the caller's arrays in whatever order they are; fastest when they are element-ordered (after m3dk_sort or a push with
+ * sort_interval >= 1).  Sums are accumulated with fp64 atomics: the order of addition, hence the last bits, may vary.   */
+int m3dk_deposit_bytes(const m3dk_ctx *ctx, size_t *bytes);
+int m3dk_deposit(m3dk_ctx *ctx, double *rhs);
+
 /* Measured FP64 FMA throughput of the device (register-resident DFMA chains, all SMs), in TFLOP/s (FMA = 2 flop).
  * Synchronous.  Used as the measured denominator of the FP64 roofline.                                                */
 int m3dk_fp64_peak_tflops(m3dk_ctx *ctx, double *tflops);

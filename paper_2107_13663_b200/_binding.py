@@ -78,6 +78,8 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_particles_upload": ([vp] + [vp] * 8, i),
         "m3dk_particles_download": ([vp] + [vp] * 10, i),
         "m3dk_eval_fields": ([vp, lng, vp, vp, vp, dbl, vp, vp], i),
+        "m3dk_deposit_bytes": ([vp, C.POINTER(sz)], i),
+        "m3dk_deposit": ([vp, vp], i),
         "m3dk_fp64_peak_tflops": ([vp, _c_dp], i),
         "m3dk_set_profiling": ([vp, i], i),
         "m3dk_timing": ([vp, C.POINTER(_Timing)], i),
@@ -303,6 +305,16 @@ class Pusher:
                                          self._p(out)))
         self.stats()
         return elem.cpu().numpy(), out.cpu().numpy()
+
+    def deposit(self):
+        """m3dk_deposit into a fresh device tensor; returns it as numpy [n_elems][2][1 + 2 n_modes][21] (synchronises)."""
+        need = C.c_size_t()
+        self._ck(self.L.m3dk_deposit_bytes(self.h, C.byref(need)))
+        rhs = self.torch.empty(need.value // 8, dtype=self.torch.float64, device=self.device)
+        self._ck(self.L.m3dk_deposit(self.h, self._p(rhs)))
+        self.stats()
+        self._keep["rhs"] = rhs
+        return rhs.cpu().numpy().reshape(self.n_elems, 2, 1 + 2 * self.n_modes, 21)
 
     def fp64_peak_tflops(self) -> float:
         v = C.c_double()

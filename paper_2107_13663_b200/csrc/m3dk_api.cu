@@ -539,6 +539,22 @@ extern "C" int m3dk_eval_fields(m3dk_ctx *ctx, long n, const double *R, const do
     return M3DK_OK;
 }
 
+extern "C" int m3dk_deposit_bytes(const m3dk_ctx *ctx, size_t *bytes) {
+    if (!ctx || !bytes) return M3DK_EINVAL;
+    if (!ctx->have_fields) return M3DK_ESTATE;
+    *bytes = (size_t)ctx->f.n_elems * 2 * (1 + 2 * ctx->f.n_modes) * M3DK_NCOEF * sizeof(double);
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_deposit(m3dk_ctx *ctx, double *rhs) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_deposit: fields and markers must be set first");
+    if (!rhs) return fail(ctx, M3DK_EINVAL, "m3dk_deposit: rhs is NULL");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CU(launch_deposit(ctx, ctx->n, rhs), "deposit kernel");
+    return M3DK_OK;
+}
+
 extern "C" int m3dk_fp64_peak_tflops(m3dk_ctx *ctx, double *tflops) {
     if (!ctx || !tflops) return M3DK_EINVAL;
     if (!ctx->have_fields) return fail(ctx, M3DK_ESTATE, "m3dk_fp64_peak_tflops: call m3dk_fields_create first (uses its control block)");

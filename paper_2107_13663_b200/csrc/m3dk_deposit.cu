@@ -1,0 +1,88 @@
+// m3dk_deposit.cu -- moment deposition: right-hand sides of the Galerkin projection of the pressure
+// moments with a delta-function particle shape, Eqs. (17)-(18) (readings G10, G22):
+//     rhs[e][0][h][k] = sum over markers p in element e of  w_p m v_par,p^2    nu_k(x_p) T_h(phi_p)
+//     rhs[e][1][h][k] = sum over markers p in element e of  w_p mu_p |B|0(x_p) nu_k(x_p) T_h(phi_p)
+// nu_k = xi^i eta^j (the element's own basis), T_0 = 1, T_{2m+1} = cos(n_m phi), T_{2m+2} = sin(n_m phi).
+// One marker per lane; the lanes of a warp that sit in the same element are reduced with shuffles and their sum enters the
+// table with ONE fp64 atomic per entry, so on an element-ordered marker stream (what m3dk_push leaves behind when
+// sort_interval >= 1) a warp makes one or two passes and an element's 42 (1 + 2 n_modes) sums receive a few atomics each.
+#include "m3dk_device.cuh"
+
+namespace m3dk {
+
+constexpr int kDepHarmMax = 1 + 2 * M3DK_MAX_MODES;
+
+__global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, long n,
+                                                      double mass, double *__restrict__ rhs) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const bool valid = i < n;
+    const int e = valid ? a.elem[i] : -1;
+    const bool active = e >= 0;                      // lost markers deposit nothing
+    const int H = 1 + 2 * f.n_modes;
+    Marker s;
+    if (active) {
+        s.x = a.x[i]; s.y = a.y[i]; s.z = a.z[i]; s.vx = a.vx[i]; s.vy = a.vy[i]; s.vz = a.vz[i]; s.mu = a.mu[i]; s.w = a.w[i];
+    } else {
+        s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
+    }
+    StepGeom g;
+    step_geometry(s, g);
+    // equilibrium quad at the marker: B0 = grad psi0 x grad phi + F0 grad phi (G4), |B|0 from its own table
+    const double *tile = f.tiles + (size_t)max(e, 0) * f.tile_stride;     // clamped: the loads may be speculated
+    const Quad hd = ldq(tile);
+    const double se = hd.c;
+    const double xi1[1] = {__dmul_rn(__dsub_rn(g.R, hd.a), se)}, eta1[1] = {__dmul_rn(__dsub_rn(s.z, hd.b), se)};
+    double v[1][4], dx[1][4], de[1][4];
+    Ring ring;
+    ring_fill<false>(ring, tile + kTileHeader);
+    quad_vd<1, false>(tile + kTileHeader, tile + kTileHeader, ring, xi1, eta1, v, dx, de);
+    const double BR = -__dmul_rn(__dmul_rn(de[0][0], se), g.rinv), BP = __dmul_rn(v[0][2], g.rinv),
+                 BZ = __dmul_rn(__dmul_rn(dx[0][0], se), g.rinv);
+    const double binv = m3dk_rsqrt(M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, __dmul_rn(BZ, BZ))));
+    const double vR = M3DK_FMA(s.vx, g.cph, __dmul_rn(s.vy, g.sph)), vP = M3DK_FMA(s.vy, g.cph, -__dmul_rn(s.vx, g.sph));
+    const double vpar = __dmul_rn(M3DK_FMA(vR, BR, M3DK_FMA(vP, BP, __dmul_rn(s.vz, BZ))), binv);
+    const double amp[2] = {__dmul_rn(__dmul_rn(s.w, mass), __dmul_rn(vpar, vpar)), __dmul_rn(__dmul_rn(s.w, s.mu), v[0][1])};
+    // toroidal factors by complex powers of (cos phi + i sin phi)
+    double T[kDepHarmMax];
+    T[0] = 1.0;
+    for (int md = 0; md < f.n_modes; ++md) mode_phase(f.n_tor[md], g.cph, g.sph, 1.0, 0.0, T[1 + 2 * md], T[2 + 2 * md]);
+    double xp[6], ep[6];
+    xp[0] = 1.0; ep[0] = 1.0;
+#pragma unroll
+    for (int q = 1; q < 6; ++q) { xp[q] = __dmul_rn(xp[q - 1], xi1[0]); ep[q] = __dmul_rn(ep[q - 1], eta1[0]); }
+    const size_t stride_e = (size_t)2 * H * M3DK_NCOEF;
+    unsigned todo = __ballot_sync(0xffffffffu, active);
+    while (todo) {
+        const int ke = __shfl_sync(0xffffffffu, e, __ffs(todo) - 1);
+        const bool mine = active && e == ke;
+        double *out = rhs + (size_t)ke * stride_e;
+        for (int mom = 0; mom < 2; ++mom)
+            for (int h = 0; h < H; ++h) {
+                const double ah = mine ? __dmul_rn(amp[mom], T[h]) : 0.0;
+                double *o = out + ((size_t)mom * H + h) * M3DK_NCOEF;
+                int k = 0;
+#pragma unroll
+                for (int j = 0; j < 6; ++j)
+#pragma unroll
+                    for (int ii = 0; ii < 6 - j; ++ii, ++k) {
+                        double val = __dmul_rn(ah, __dmul_rn(xp[ii], ep[j]));
+#pragma unroll
+                        for (int sft = 16; sft > 0; sft >>= 1) val += __shfl_xor_sync(0xffffffffu, val, sft);
+                        if (lane == 0) atomicAdd(o + k, val);
+                    }
+            }
+        todo &= ~__ballot_sync(0xffffffffu, mine);
+    }
+}
+
+cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs) {
+    const size_t bytes = (size_t)c->f.n_elems * 2 * (1 + 2 * c->f.n_modes) * M3DK_NCOEF * sizeof(double);
+    cudaError_t e = cudaMemsetAsync(rhs, 0, bytes, c->stream);
+    if (e != cudaSuccess || n == 0) return e;
+    c->kernel_launches += 1;
+    deposit_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, c->user, n, c->m, rhs);
+    return cudaGetLastError();
+}
+
+}  // namespace m3dk

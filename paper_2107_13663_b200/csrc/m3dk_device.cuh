@@ -158,7 +158,7 @@ __device__ __forceinline__ void edge_fn(const double *__restrict__ rec, double R
 // Two phases over the bucket's candidate list (a superset of every element touching the bucket, priority order):
 // a candidate that contains the point strictly (all edge functions above its tolerance) is the only one that can
 // contain it, so it is returned at once; otherwise (the point is within rounding of an edge) take the minimum index.
-__device__ __noinline__ int locate(const GridParams &g, double R, double Z) {
+static __device__ __noinline__ int locate(const GridParams &g, double R, double Z) {
     if (!(R >= g.Rmin && R <= g.Rmax && Z >= g.Zmin && Z <= g.Zmax)) return -1;
     int ix = (int)((R - g.Rmin) * g.inv_hx), iz = (int)((Z - g.Zmin) * g.inv_hz);
     ix = min(max(ix, 0), g.gx - 1);

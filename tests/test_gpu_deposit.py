@@ -1,0 +1,73 @@
+"""GPU parity of m3dk_deposit (Eqs. 17-18 with a delta-function shape) against the oracle's deposition
+(pinned by tests/test_oracle_deposit.py), through the C ABI.  The GPU accumulates with fp64 atomics, so the order of
+addition is free: entries are compared within 1e-12 of the sum of the ABSOLUTE contributions to that element and moment
+(the monomials and toroidal factors are bounded by 1 in the element's frame)."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from gpu_helpers import KEYS, make_pusher, oracle_of
+from test_gpu_ordered import _unstructured
+
+pytestmark = pytest.mark.gpu
+
+
+def _check(w, markers, p):
+    mesh, sp = oracle_of(w)
+    ref, lost = oracle.deposit(mesh, sp, markers)
+    absw = dict(markers)
+    absw["w"] = np.abs(markers["w"])
+    scale, _ = oracle.deposit(mesh, sp, absw)
+    S = scale[:, :, 0, 0][:, :, None, None]                     # sum of |a_p| per element and moment
+    got = p.deposit()
+    assert got.shape == ref.shape
+    err = np.abs(got - ref)
+    assert (err <= 1e-12 * S + 1e-300).all(), float((err / (S + 1e-300)).max())
+    assert np.abs(ref).max() > 0
+    return got, ref, lost
+
+
+@pytest.mark.parametrize("si", [0, 1])
+def test_deposit_matches_oracle_after_a_push(si):
+    """Weights produced by the push itself (config 3 shape), arrays in caller order (si = 0) and element order (si = 1)."""
+    w = synth.make_config(3, n_markers=1 << 16, nx=32)
+    p = make_pusher(w, verify=False, sort_interval=si)
+    p.push(12, w.dt)
+    raw, elem, ids = p.state(by_id=False)                       # exactly the arrays the library deposits from
+    got, ref, lost = _check(w, raw, p)
+    assert lost == int((elem < 0).sum())
+    # order independence: the same markers deposited from id order give the same table within the tolerance
+    by_id, _, _ = p.state()
+    ref2, _ = oracle.deposit(*oracle_of(w), by_id)
+    assert np.abs(ref2 - ref).max() <= 1e-12 * np.abs(ref).max() * 50
+
+
+def test_deposit_two_modes_unstructured_mesh_with_lost_markers():
+    w0 = _unstructured(two_modes=True)
+    rng = np.random.Generator(np.random.PCG64(4))
+    mk = {k: v.copy() for k, v in w0.markers.items()}
+    mk["w"] = rng.normal(size=w0.n_markers)
+    mk["x"][:11] = 40.0                                         # outside the mesh: must deposit nothing
+    w = dataclasses.replace(w0, markers=mk)
+    p = make_pusher(w, verify=True)
+    got, ref, lost = _check(w, mk, p)
+    assert lost == 11 and got.shape[2] == 5                     # harmonics 1, cos / sin of both modes
+    # the rows of the lost markers' would-be elements are not polluted: total of the unit test function
+    live = np.ones(w.n_markers, dtype=bool)
+    live[:11] = False
+    assert abs(got[:, 1, 0, 0].sum() - ref[:, 1, 0, 0].sum()) <= 1e-9 * np.abs(mk["w"][live]).sum()
+
+
+def test_deposit_equilibrium_only_and_empty():
+    w = synth.make_config(0, n_markers=4096, nx=32)             # no modes: a single harmonic
+    mk = {k: v.copy() for k, v in w.markers.items()}
+    mk["w"] = np.linspace(-1.0, 1.0, w.n_markers)
+    p = make_pusher(dataclasses.replace(w, markers=mk), verify=False)
+    got, ref, _ = _check(w, mk, p)
+    assert got.shape == (w.n_elems, 2, 1, 21)
+    empty = {k: np.zeros(0) for k in KEYS}
+    p2 = make_pusher(dataclasses.replace(w, markers=empty), verify=False)
+    assert np.abs(p2.deposit()).max() == 0.0
