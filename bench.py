@@ -290,6 +290,23 @@ def run_ours(args, rank, world, local_rank):
             "e2e": {"value": shard.whole_job_rate([N] * world, Ke, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": 64 * N / Ke,
                     "d2h_bytes_per_step": 64 * N / Ke, "note": f"one upload + {Ke} steps + one download (PAPER.md:237)"},
             "roofline": roof, "n_lost": st["n_lost"]}
+    if args.deposit:
+        # row (f)-4: one deposition of the pressure moments from the element-ordered arrays the push left behind
+        need = p.deposit_bytes()
+        rhs = torch.empty(need // 8, dtype=torch.float64, device=dev)
+        p.deposit_into(rhs)
+        torch.cuda.synchronize(dev)
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(p.stream)
+        for _ in range(5):
+            p.deposit_into(rhs)
+        d1.record(p.stream)
+        torch.cuda.synchronize(dev)
+        dms = d0.elapsed_time(d1) / 5
+        dbytes = (68.0 * N + need)            # 8 fp64 + element key per marker read, the table cleared and accumulated
+        line["deposit"] = {"ms": dms, "markers_per_s": N / (dms * 1e-3), "table_bytes": need,
+                           "hbm_bytes": dbytes, "hbm_frac": dbytes / (dms * 1e-3) / (hbm_gbs * 1e9),
+                           "note": "m3dk_deposit, Eqs. (17)-(18), delta-function shape (SURVEY.md 8(f)-4)"}
     if world == 1 and not args.no_cpu_baseline:
         rate, n, secs, cores, stride, rsteps = oracle_bounded_sample(w, args.ref_sample)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -354,6 +371,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=65536, help="markers in the oracle's bounded sample")
     ap.add_argument("--mode", type=int, default=0, choices=[0, 1],
                     help="0: linear delta-f (the headline); 1: non-linear trajectories (SURVEY.md 8(f)-1)")
+    ap.add_argument("--deposit", action="store_true", help="also time m3dk_deposit (SURVEY.md 8(f)-4) on the final state")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4] sweep: one JSON line per (n, dt, sort interval)")
     ap.add_argument("--sweep-n", type=int, nargs="+", default=[1 << 20, 1 << 22, 1 << 24, 1 << 26])

@@ -160,9 +160,11 @@ int m3dk_eval_fields(m3dk_ctx *ctx, long n, const double *R, const double *phi, 
  * T_0 = 1, T_{2m+1} = cos(n_tor[m] phi), T_{2m+2} = sin(n_tor[m] phi); v_par = v . B0/|B0| with the stored v (v_{l-1/2}).
  * The delta function is normalised in physical volume, so no Jacobian factor appears (G22); the mass-matrix solve that
  * turns these sums into pressure coefficients belongs to the MHD code and is out of scope.  Lost markers deposit nothing.
- * rhs: DEVICE, m3dk_deposit_bytes() bytes = [n_elems][2][1 + 2 n_modes][21] doubles, overwritten.  Asynchronous.  Works on
- * the caller's arrays in whatever order they are; fastest when they are element-ordered (after m3dk_sort or a push with
- * sort_interval >= 1).  Sums are accumulated with fp64 atomics: the order of addition, hence the last bits, may vary.   */
+ * rhs: DEVICE, m3dk_deposit_bytes() bytes = [n_elems][2][1 + 2 n_modes][21] doubles, overwritten.  Asynchronous.  The
+ * caller's arrays are read, not modified.  With a sort workspace set (m3dk_set_sort_workspace) the markers are first
+ * ordered by the element of their current position inside the workspace and a warp reduces up to 64 markers of one
+ * element per table update; without one, every warp loops over the distinct elements of its 32 markers (slow on an
+ * unordered stream).  Sums are accumulated with fp64 atomics: the order of addition, hence the last bits, may vary.     */
 int m3dk_deposit_bytes(const m3dk_ctx *ctx, size_t *bytes);
 int m3dk_deposit(m3dk_ctx *ctx, double *rhs);
 

@@ -306,6 +306,15 @@ class Pusher:
         self.stats()
         return elem.cpu().numpy(), out.cpu().numpy()
 
+    def deposit_bytes(self) -> int:
+        need = C.c_size_t()
+        self._ck(self.L.m3dk_deposit_bytes(self.h, C.byref(need)))
+        return int(need.value)
+
+    def deposit_into(self, rhs):
+        """m3dk_deposit into a caller's device tensor of deposit_bytes() bytes (asynchronous)."""
+        self._ck(self.L.m3dk_deposit(self.h, self._p(rhs)))
+
     def deposit(self):
         """m3dk_deposit into a fresh device tensor; returns it as numpy [n_elems][2][1 + 2 n_modes][21] (synchronises)."""
         need = C.c_size_t()

@@ -12,20 +12,10 @@ namespace m3dk {
 
 constexpr int kDepHarmMax = 1 + 2 * M3DK_MAX_MODES;
 
-__global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, long n,
-                                                      double mass, double *__restrict__ rhs) {
-    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int lane = threadIdx.x & 31;
-    const bool valid = i < n;
-    const int e = valid ? a.elem[i] : -1;
-    const bool active = e >= 0;                      // lost markers deposit nothing
-    const int H = 1 + 2 * f.n_modes;
-    Marker s;
-    if (active) {
-        s.x = a.x[i]; s.y = a.y[i]; s.z = a.z[i]; s.vx = a.vx[i]; s.vy = a.vy[i]; s.vz = a.vz[i]; s.mu = a.mu[i]; s.w = a.w[i];
-    } else {
-        s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
-    }
+// contributions of one marker: amp[0] = w m v_par^2, amp[1] = w mu |B|0; T[h]; xp[i] = xi^i, ep[j] = eta^j
+struct DepMarker { double amp[2], T[kDepHarmMax], xp[6], ep[6]; };
+
+__device__ __forceinline__ void dep_marker(const FieldParams &f, int e, const Marker &s, double mass, DepMarker &d) {
     StepGeom g;
     step_geometry(s, g);
     // equilibrium quad at the marker: B0 = grad psi0 x grad phi + F0 grad phi (G4), |B|0 from its own table
@@ -42,15 +32,34 @@ __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ Fi
     const double binv = m3dk_rsqrt(M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, __dmul_rn(BZ, BZ))));
     const double vR = M3DK_FMA(s.vx, g.cph, __dmul_rn(s.vy, g.sph)), vP = M3DK_FMA(s.vy, g.cph, -__dmul_rn(s.vx, g.sph));
     const double vpar = __dmul_rn(M3DK_FMA(vR, BR, M3DK_FMA(vP, BP, __dmul_rn(s.vz, BZ))), binv);
-    const double amp[2] = {__dmul_rn(__dmul_rn(s.w, mass), __dmul_rn(vpar, vpar)), __dmul_rn(__dmul_rn(s.w, s.mu), v[0][1])};
-    // toroidal factors by complex powers of (cos phi + i sin phi)
-    double T[kDepHarmMax];
-    T[0] = 1.0;
-    for (int md = 0; md < f.n_modes; ++md) mode_phase(f.n_tor[md], g.cph, g.sph, 1.0, 0.0, T[1 + 2 * md], T[2 + 2 * md]);
-    double xp[6], ep[6];
-    xp[0] = 1.0; ep[0] = 1.0;
+    d.amp[0] = __dmul_rn(__dmul_rn(s.w, mass), __dmul_rn(vpar, vpar));
+    d.amp[1] = __dmul_rn(__dmul_rn(s.w, s.mu), v[0][1]);
+    d.T[0] = 1.0;     // toroidal factors by complex powers of (cos phi + i sin phi)
 #pragma unroll
-    for (int q = 1; q < 6; ++q) { xp[q] = __dmul_rn(xp[q - 1], xi1[0]); ep[q] = __dmul_rn(ep[q - 1], eta1[0]); }
+    for (int md = 0; md < M3DK_MAX_MODES; ++md)
+        if (md < f.n_modes) mode_phase(f.n_tor[md], g.cph, g.sph, 1.0, 0.0, d.T[1 + 2 * md], d.T[2 + 2 * md]);
+    d.xp[0] = 1.0; d.ep[0] = 1.0;
+#pragma unroll
+    for (int q = 1; q < 6; ++q) { d.xp[q] = __dmul_rn(d.xp[q - 1], xi1[0]); d.ep[q] = __dmul_rn(d.ep[q - 1], eta1[0]); }
+}
+
+// any marker order: one marker per lane, the warp loops over its distinct elements
+__global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, long n,
+                                                      double mass, double *__restrict__ rhs) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const bool valid = i < n;
+    const int e = valid ? a.elem[i] : -1;
+    const bool active = e >= 0;                      // lost markers deposit nothing
+    const int H = 1 + 2 * f.n_modes;
+    Marker s;
+    if (active) {
+        s.x = a.x[i]; s.y = a.y[i]; s.z = a.z[i]; s.vx = a.vx[i]; s.vy = a.vy[i]; s.vz = a.vz[i]; s.mu = a.mu[i]; s.w = a.w[i];
+    } else {
+        s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
+    }
+    DepMarker d;
+    dep_marker(f, e, s, mass, d);
     const size_t stride_e = (size_t)2 * H * M3DK_NCOEF;
     unsigned todo = __ballot_sync(0xffffffffu, active);
     while (todo) {
@@ -58,15 +67,17 @@ __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ Fi
         const bool mine = active && e == ke;
         double *out = rhs + (size_t)ke * stride_e;
         for (int mom = 0; mom < 2; ++mom)
-            for (int h = 0; h < H; ++h) {
-                const double ah = mine ? __dmul_rn(amp[mom], T[h]) : 0.0;
+#pragma unroll
+            for (int h = 0; h < kDepHarmMax; ++h) {
+                if (h >= H) break;
+                const double ah = mine ? __dmul_rn(d.amp[mom], d.T[h]) : 0.0;
                 double *o = out + ((size_t)mom * H + h) * M3DK_NCOEF;
                 int k = 0;
 #pragma unroll
                 for (int j = 0; j < 6; ++j)
 #pragma unroll
                     for (int ii = 0; ii < 6 - j; ++ii, ++k) {
-                        double val = __dmul_rn(ah, __dmul_rn(xp[ii], ep[j]));
+                        double val = __dmul_rn(ah, __dmul_rn(d.xp[ii], d.ep[j]));
 #pragma unroll
                         for (int sft = 16; sft > 0; sft >>= 1) val += __shfl_xor_sync(0xffffffffu, val, sft);
                         if (lane == 0) atomicAdd(o + k, val);
@@ -76,10 +87,70 @@ __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ Fi
     }
 }
 
+// element-ordered records cut into work items (the ordering kernels of m3dk_sort.cu): a warp takes an item (<= 64
+// markers of ONE element), every lane two of them, one reduction and one atomic per table entry and item
+__global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constant__ FieldParams f, const double *__restrict__ rec,
+                                                            const int4 *__restrict__ items, const int *__restrict__ n_items,
+                                                            double mass, double *__restrict__ rhs) {
+    const int lane = threadIdx.x & 31;
+    const int it = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (it >= *n_items) return;
+    const int4 w = __ldg(items + it);
+    const int e = w.x, start = w.y, count = w.z;
+    if (e >= f.n_elems) return;                      // the pseudo-element of the lost markers
+    const int H = 1 + 2 * f.n_modes;
+    DepMarker d[kItemR];
+#pragma unroll
+    for (int r = 0; r < kItemR; ++r) {
+        const bool on = 32 * r + lane < count;
+        Marker s;
+        s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
+        if (on) {
+            const double *p = rec + (size_t)kRecDoubles * (start + 32 * r + lane);
+            s.x = p[0]; s.y = p[1]; s.z = p[2]; s.w = p[3]; s.vx = p[4]; s.vy = p[5]; s.vz = p[6]; s.mu = p[7];
+        }
+        dep_marker(f, e, s, mass, d[r]);
+        if (!on) { d[r].amp[0] = 0.0; d[r].amp[1] = 0.0; }
+    }
+    double *out = rhs + (size_t)e * 2 * H * M3DK_NCOEF;
+    for (int mom = 0; mom < 2; ++mom)
+#pragma unroll
+        for (int h = 0; h < kDepHarmMax; ++h) {
+            if (h >= H) break;
+            double ah[kItemR];
+#pragma unroll
+            for (int r = 0; r < kItemR; ++r) ah[r] = __dmul_rn(d[r].amp[mom], d[r].T[h]);
+            double *o = out + ((size_t)mom * H + h) * M3DK_NCOEF;
+            int k = 0;
+#pragma unroll
+            for (int j = 0; j < 6; ++j)
+#pragma unroll
+                for (int ii = 0; ii < 6 - j; ++ii, ++k) {
+                    double val = 0.0;
+#pragma unroll
+                    for (int r = 0; r < kItemR; ++r) val = M3DK_FMA(ah[r], __dmul_rn(d[r].xp[ii], d[r].ep[j]), val);
+#pragma unroll
+                    for (int sft = 16; sft > 0; sft >>= 1) val += __shfl_xor_sync(0xffffffffu, val, sft);
+                    if (lane == 0) atomicAdd(o + k, val);
+                }
+        }
+}
+
 cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs) {
     const size_t bytes = (size_t)c->f.n_elems * 2 * (1 + 2 * c->f.n_modes) * M3DK_NCOEF * sizeof(double);
     cudaError_t e = cudaMemsetAsync(rhs, 0, bytes, c->stream);
     if (e != cudaSuccess || n == 0) return e;
+    if (c->have_sortws) {
+        // order the markers by the element of their CURRENT position first (after a push the arrays are in the order of
+        // the previous positions): records in element order + work items, then one warp per item
+        e = launch_pack_sorted(c, n);
+        if (e != cudaSuccess) return e;
+        const long max_items = n / kItemMarkers + c->f.n_elems + 2;
+        c->kernel_launches += 1;
+        deposit_items_kernel<<<(unsigned)((max_items + 3) / 4), 128, 0, c->stream>>>(
+            c->f, c->sb.rec[c->cur], c->sb.items, c->sb.ioffs + c->f.n_elems + 1, c->m, rhs);
+        return cudaGetLastError();
+    }
     c->kernel_launches += 1;
     deposit_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, c->user, n, c->m, rhs);
     return cudaGetLastError();
