@@ -5,18 +5,8 @@
 
 namespace m3dk {
 
-#ifndef M3DK_EARLY_LOCATE
-#define M3DK_EARLY_LOCATE 0
-#endif
-#ifndef M3DK_MID_LOCATE
-#define M3DK_MID_LOCATE 0
-#endif
-#ifndef M3DK_PREFETCH_REC
-#define M3DK_PREFETCH_REC 1
-#endif
-#ifndef M3DK_UNROLL_Q
-#define M3DK_UNROLL_Q 0
-#endif
+// CTA shape of the element-ordered kernel: 128 threads x 3 CTAs per SM (168 registers); measured alternatives in
+// profiles/r1_development_notes.md
 #ifndef M3DK_PUSH_THREADS
 #define M3DK_PUSH_THREADS 128
 #endif
@@ -182,24 +172,17 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
             io.store_pos(mo[r], s[r].x, s[r].y, s[r].z, s[r].w);
             io.store_vel(mo[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
         }
-        // the element search of the new position runs after phase B; its first record starts travelling now
-#if M3DK_EARLY_LOCATE
-        rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);
-#else
+        // the element search of the new position runs after phase B (loading its first record here, or searching
+        // between the quads, costs registers in the hottest part of the kernel and measured slower)
         locate_prefetch(P.f.fast, Rn[r], Zn[r]);
-#endif
     }
     // a3 for the NEW position (the key of the next sort) and, with kHist, the sort histogram of the new keys with each
-    // marker's rank inside its key (the sort then needs no pass over the keys).  With modes this sits between the value
-    // quads and the B_par quad of the last mode: the search record has arrived by then and the atomics' round trip is
-    // covered by the B_par quad.
+    // marker's rank inside its key (the sort then needs no pass over the keys)
     unsigned peers[R];
     int base[R];
     auto locate_and_count = [&]() {
-#if !M3DK_EARLY_LOCATE
 #pragma unroll
-        for (int r = 0; r < R; ++r) rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);
-#endif
+        for (int r = 0; r < R; ++r) rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);   // all first records in flight together
         int key[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -229,11 +212,7 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
             ring_fill<kSmem>(ring, pm);
             // the two value-only quads share one copy of the Horner code (rolled: the kernel must fit the 32 KB
             // instruction cache); the weights of quad q are picked by selects
-#if M3DK_UNROLL_Q
-#pragma unroll
-#else
 #pragma unroll 1
-#endif
             for (int q = 0; q < 2; ++q) {
                 quad_vd<R, kSmem>(pm + q * kQuad, pm + (q + 1) * kQuad, ring, xi, eta, v, dx, de);
 #pragma unroll
@@ -243,9 +222,6 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
                     wsum[r] = pert_fold_v(wsum[r], v[r], wa, wb, cth[r], sth[r]);
                 }
             }
-#if M3DK_MID_LOCATE
-            if (md == P.f.n_modes - 1) locate_and_count();
-#endif
             quad_vd<R, kSmem>(pm + 2 * kQuad, pm, ring, xi, eta, v, dx, de);   // (B_par, B_Z); quad 3 (B_phi) is not needed
 #pragma unroll
             for (int r = 0; r < R; ++r) wsum[r] = pert_fold_par(wsum[r], v[r], dx[r], de[r], W[r], cth[r], sth[r], se, nri[r], om);
@@ -254,9 +230,7 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
 #pragma unroll
         for (int r = 0; r < R; ++r)
             if (on[r]) io.store_w(mo[r], M3DK_FMA(P.dt, wsum[r], s[r].w));
-#if !M3DK_MID_LOCATE
         locate_and_count();
-#endif
     } else {
         locate_and_count();
     }
@@ -460,7 +434,7 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
         int src2[kItemR];
 #pragma unroll
         for (int r = 0; r < kItemR; ++r) {
-            if (M3DK_PREFETCH_REC && 32 * r + lane < w1.z) {
+            if (32 * r + lane < w1.z) {
                 const double *rp = P.rc.in + (size_t)kRecDoubles * src1[r];
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(rp));
             }
