@@ -148,3 +148,31 @@ def test_full_size_bench_configuration_on_sampled_markers():
     assert max(ex.max(), ev.max(), ew.max()) <= 3 * TOL_STEP, (ex.max(), ev.max(), ew.max())
     st = p.stats()
     assert st["steps_done"] == nsteps and st["n_markers"] == w.n_markers
+
+
+def test_four_modes_including_axisymmetric_and_negative_n():
+    """M3DK_MAX_MODES toroidal modes at once (n = 1, -2, 0, 5): the largest tile (11.5 KB, staged by TMA), the n = 0 phase
+    (no complex power at all) and a negative n, linear and non-linear mode, ordered and SoA path, against the oracle."""
+    w0 = synth.make_config(1, n_markers=3000 + 5, nx=24)
+    eq = w0.eq
+    perts = list(w0.perts)
+    for n, m, rc, om in ((-2, 3, 0.45, 0.013), (0, 2, 0.35, 0.004), (5, 6, 0.3, 0.021)):
+        p = synth.Perturbation(eq, n=n, omega=om, harmonics=[synth.Harmonic(m, sc.gaussian_radial(m, rc, 0.1))])
+        perts.append(p.normalise(0.6e-4 * eq.B0))
+    pc, n_tor, omega = pert_tables(perts, w0.node_RZ, w0.tri)
+    w = dataclasses.replace(w0, pert_coef=pc, n_tor=n_tor, omega=omega, perts=perts)
+    assert w.n_modes == 4 and 0 in list(n_tor) and min(n_tor) < 0
+    for mode in (0, 1):
+        mesh, sp = oracle_of(w, mode=mode)
+        ref, e_ref, _ = oracle_push(mesh, sp, w.markers, 4, w.dt, t0=0.3)
+        out = {}
+        for si in (0, 1):
+            p = make_pusher(w, verify=True, sort_interval=si, t0=0.3, mode=mode)
+            p.push(4, w.dt)
+            out[si], _, _ = p.state()
+            live = e_ref >= 0
+            wrms = np.sqrt(np.mean(ref["w"][live] ** 2))
+            ex, ev, ew = g16_errors(take(out[si], live), take(ref, live), w_floor=wrms)
+            assert max(ex.max(), ev.max(), ew.max()) <= 4 * TOL_STEP, (mode, si, ex.max(), ev.max(), ew.max())
+        for k in KEYS:
+            assert np.array_equal(out[0][k], out[1][k]), (mode, k)
