@@ -57,6 +57,8 @@ def lib():
         L.orc_push_analytic.restype = C.c_long
         L.orc_push_analytic.argtypes = [C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 8 + [
             C.c_int, C.c_double, C.c_double, C.c_long, C.c_int]
+        L.orc_gyro_ring.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_double, c_dp]
+        L.orc_flr_fields.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_double, C.c_double, c_dp]
         L.orc_deposit.restype = C.c_long
         L.orc_deposit.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_dp]
         L.orc_trace.restype = C.c_long
@@ -83,7 +85,8 @@ def _i(a):
 
 
 def species(charge, mass, f0kind=0, T=1.0, v_c=0.3, Lambda0=0.75, dLambda=0.2, B_axis=1.0, mode=0) -> Species:
-    """mode 0: linear delta-f; 1: non-linear trajectories with (1 - w) kept (reading G21)."""
+    """mode 0: linear delta-f; 1: non-linear trajectories with (1 - w) kept (reading G21); 2: linear delta-f with the
+    4-point gyro-average of the perturbed fields (reading G23)."""
     s = Species()
     s.charge, s.mass, s.f0kind, s.mode = float(charge), float(mass), int(f0kind), int(mode)
     for k, v in enumerate((T, v_c, Lambda0, dLambda, B_axis)):
@@ -188,6 +191,24 @@ def push_analytic(an: Analytic, sp: Species, markers: dict, nsteps: int, dt: flo
     n = st["x"].shape[0]
     lib().orc_push_analytic(C.byref(an), C.byref(sp), n, *ptrs, int(nsteps), float(dt), float(t0), int(step0), int(nthreads))
     return st
+
+
+def gyro_ring(sp: Species, X, mu: float, *, mesh=None, an=None):
+    """The four gyro-ring points X + rho_L,j of reading G23 (Cartesian, shape (4, 3)); None when X is outside the mesh."""
+    X = np.ascontiguousarray(X, dtype=np.float64)
+    pts = np.empty((4, 3))
+    ok = lib().orc_gyro_ring(mesh.h if mesh is not None else None, C.byref(an) if an is not None else None, C.byref(sp),
+                             X.ctypes.data_as(c_dp), float(mu), pts.ctypes.data_as(c_dp))
+    return pts if ok else None
+
+
+def flr_fields(sp: Species, X, mu: float, t: float = 0.0, *, mesh=None, an=None):
+    """Gyro-averaged perturbed fields of Eq. (14) at X in the marker's cylindrical frame: <E1>, <B1>, <grad B1par>, <dB1par/dt>."""
+    X = np.ascontiguousarray(X, dtype=np.float64)
+    out = np.empty(10)
+    ok = lib().orc_flr_fields(mesh.h if mesh is not None else None, C.byref(an) if an is not None else None, C.byref(sp),
+                              X.ctypes.data_as(c_dp), float(mu), float(t), out.ctypes.data_as(c_dp))
+    return out if ok else None
 
 
 def deposit(mesh: "Mesh", sp: Species, markers: dict):

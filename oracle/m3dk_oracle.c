@@ -91,7 +91,8 @@ typedef struct {
     double charge, mass;
     int f0kind;        /* 0 Maxwellian, 1 slowing-down, 2 beam pitch (reading G7) */
     double f0par[5];   /* T, v_c, Lambda0, dLambda, B_axis */
-    int mode;          /* 0: linear delta-f; 1: non-linear trajectories, (1 - w) kept (reading G21) */
+    int mode;          /* 0: linear delta-f; 1: non-linear trajectories, (1 - w) kept (reading G21);
+                          2: linear delta-f with 4-point gyro-averaged perturbed fields (Eq. 14; reading G23) */
 } orc_species;
 
 /* ------------------------------------------------------------------------------------------------ */
@@ -389,6 +390,73 @@ typedef struct {
     int brute;
 } provider;
 
+/* fields of either back-end at (R, phi, Z); returns 0 when the point is outside the mesh (FE back-end) */
+static int provider_fields(const provider *pv, double R, double phi, double Z, double t, orc_fields *f)
+{
+    if (pv->kind == 0) {
+        int e = pv->brute ? locate_brute(pv->mesh, R, Z) : locate_grid(pv->mesh, R, Z);
+        if (e < 0) return 0;
+        fe_fields(pv->mesh, e, R, phi, Z, t, f);
+    } else {
+        an_fields(pv->an, R, phi, Z, t, f);
+    }
+    return 1;
+}
+
+/* Finite Larmor radius (Eq. 14; reading G23): the four gyro-ring points
+ * X + rho_L,j, |rho_L| = m v_perp / (|q| B) with v_perp = sqrt(2 mu B / m) "calculated from mu", uniformly spaced in
+ * the gyro-angle in the plane perpendicular to b0: +-rho e1, +-rho e2 with e1 = the major-radius direction made
+ * perpendicular to b0 and e2 = b0 x e1.  B0c = equilibrium field at X in cylindrical components, (c, sn) = cos / sin of
+ * the marker's phi.  pts[4][3] Cartesian.                                                                          */
+static void gyro_ring(const double X[3], const double B0c[3], double c, double sn, double mu, double q, double m,
+                      double pts[4][3])
+{
+    double Bn = sqrt(B0c[0] * B0c[0] + B0c[1] * B0c[1] + B0c[2] * B0c[2]);
+    double b[3] = {B0c[0] / Bn, B0c[1] / Bn, B0c[2] / Bn};
+    double rho = sqrt(2.0 * m * mu / Bn) / fabs(q);
+    double e1[3] = {1.0 - b[0] * b[0], -b[0] * b[1], -b[0] * b[2]};      /* R-hat - (R-hat . b) b, cylindrical */
+    double n1 = sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+    for (int k = 0; k < 3; ++k) e1[k] /= n1;
+    double e2[3] = {b[1] * e1[2] - b[2] * e1[1], b[2] * e1[0] - b[0] * e1[2], b[0] * e1[1] - b[1] * e1[0]};
+    /* cylindrical (R, phi, Z) components at the marker -> Cartesian */
+    double e1c[3] = {e1[0] * c - e1[1] * sn, e1[0] * sn + e1[1] * c, e1[2]};
+    double e2c[3] = {e2[0] * c - e2[1] * sn, e2[0] * sn + e2[1] * c, e2[2]};
+    for (int k = 0; k < 3; ++k) {
+        pts[0][k] = X[k] + rho * e1c[k]; pts[1][k] = X[k] + rho * e2c[k];
+        pts[2][k] = X[k] - rho * e1c[k]; pts[3][k] = X[k] - rho * e2c[k];
+    }
+}
+
+/* Eq. (14): <E1>, <B1>, <grad B1par>, <dB1par/dt> = quarter of the sum over the four ring points, vectors averaged in
+ * Cartesian components and returned in the marker's cylindrical frame.  A ring point outside the mesh contributes zero. */
+static void flr_average(const provider *pv, const double pts[4][3], double c, double sn, double t, orc_fields *f)
+{
+    double E[3] = {0, 0, 0}, B[3] = {0, 0, 0}, G[3] = {0, 0, 0}, dT = 0.0, Bp = 0.0;
+    for (int j = 0; j < 4; ++j) {
+        double x = pts[j][0], y = pts[j][1], z = pts[j][2];
+        double R = sqrt(x * x + y * y), phi = atan2(y, x);
+        orc_fields fj;
+        if (!provider_fields(pv, R, phi, z, t, &fj)) continue;
+        double cj = x / R, sj = y / R;
+        const double *src[3] = {fj.E1, fj.B1, fj.gB1p};
+        double *dst[3] = {E, B, G};
+        for (int v = 0; v < 3; ++v) {
+            dst[v][0] += src[v][0] * cj - src[v][1] * sj;
+            dst[v][1] += src[v][0] * sj + src[v][1] * cj;
+            dst[v][2] += src[v][2];
+        }
+        dT += fj.dtB1p; Bp += fj.B1p;
+    }
+    double *dst[3] = {f->E1, f->B1, f->gB1p};
+    const double *src[3] = {E, B, G};
+    for (int v = 0; v < 3; ++v) {
+        dst[v][0] = 0.25 * (src[v][0] * c + src[v][1] * sn);
+        dst[v][1] = 0.25 * (-src[v][0] * sn + src[v][1] * c);
+        dst[v][2] = 0.25 * src[v][2];
+    }
+    f->dtB1p = 0.25 * dT; f->B1p = 0.25 * Bp;
+}
+
 /* one full step of one marker.  s = {x,y,z,vx,vy,vz,mu,w}.  Returns element (FE), 0 (analytic) or -1 = lost
  * (reading G12: a lost marker is frozen).  vl_out (optional) receives the Cartesian v_l.                  */
 static int step_marker(const provider *pv, const orc_species *sp, double *s, double t, double dt, double *vl_out)
@@ -419,6 +487,11 @@ static int step_marker(const provider *pv, const orc_species *sp, double *s, dou
         ER = f.E1[0] - (mu / q) * (f.Bm_R + f.gB1p[0]);
         EP = f.E1[1] - (mu / q) * f.gB1p[1];
         EZ = f.E1[2] - (mu / q) * (f.Bm_Z + f.gB1p[2]);
+    }
+    if (sp->mode == 2) {   /* linear delta-f with the 4-point gyro-average of the perturbed fields (Eq. 14, reading G23) */
+        double X[3] = {x, y, z}, B0c[3] = {BR, BP, BZ}, pts[4][3];
+        gyro_ring(X, B0c, c, sn, mu, q, m, pts);
+        flr_average(pv, pts, c, sn, t, &f);
     }
     double B[3] = {BR * c - BP * sn, BR * sn + BP * c, BZ};
     double E[3] = {ER * c - EP * sn, ER * sn + EP * c, EZ};
@@ -589,6 +662,35 @@ void orc_push_uniform(long n, double *x, double *y, double *z, double *vx, doubl
             x[i] += dt * vp[0]; y[i] += dt * vp[1]; z[i] += dt * vp[2];
             vx[i] = vp[0]; vy[i] = vp[1]; vz[i] = vp[2];
         }
+}
+
+/* gyro ring of one marker at Cartesian X with magnetic moment mu (pins of reading G23); analytic back-end when m == NULL */
+int orc_gyro_ring(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, const double *X, double mu, double *pts12)
+{
+    provider pv = {m ? 0 : 1, m, a, 0};
+    double R = sqrt(X[0] * X[0] + X[1] * X[1]), phi = atan2(X[1], X[0]);
+    orc_fields f;
+    if (!provider_fields(&pv, R, phi, X[2], 0.0, &f)) return 0;
+    double B0c[3] = {-f.psi_Z / R, f.F / R, f.psi_R / R}, pts[4][3];
+    gyro_ring(X, B0c, X[0] / R, X[1] / R, mu, sp->charge, sp->mass, pts);
+    memcpy(pts12, pts, sizeof(pts));
+    return 1;
+}
+
+/* gyro-averaged perturbed fields at X (marker frame): out10 = <E1>(3), <B1>(3), <grad B1par>(3), <dB1par/dt> */
+int orc_flr_fields(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, const double *X, double mu, double t,
+                   double *out10)
+{
+    provider pv = {m ? 0 : 1, m, a, 0};
+    double R = sqrt(X[0] * X[0] + X[1] * X[1]), phi = atan2(X[1], X[0]);
+    orc_fields f;
+    if (!provider_fields(&pv, R, phi, X[2], t, &f)) return 0;
+    double B0c[3] = {-f.psi_Z / R, f.F / R, f.psi_R / R}, pts[4][3];
+    gyro_ring(X, B0c, X[0] / R, X[1] / R, mu, sp->charge, sp->mass, pts);
+    flr_average(&pv, pts, X[0] / R, X[1] / R, t, &f);
+    for (int k = 0; k < 3; ++k) { out10[k] = f.E1[k]; out10[3 + k] = f.B1[k]; out10[6 + k] = f.gB1p[k]; }
+    out10[9] = f.dtB1p;
+    return 1;
 }
 
 void orc_eq6(const double *vm, const double *E, const double *B, double h, double *vp) { eq6_solve(vm, E, B, h, vp); }
