@@ -119,6 +119,10 @@ int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, double *z, 
  *       1 = non-linear trajectories (reading G21): the marker moves in the total fields,
  *           B = B0 + B1 and E-dagger = E1 - (mu/q) grad(|B|0 + B1par), and Eq. (8) keeps its factor (1 - w):
  *           w_{l+1/2} = w_{l-1/2} + dt (1 - w_{l-1/2}) dw/dt|linear(x_l, v_l, t_l).
+ *       2 = linear delta-f with finite-Larmor-radius averaging (Eq. 14; reading G23): E1, B1,
+ *           grad B1par and dB1par/dt of the weight equation are replaced by the quarter sum over the four gyro-ring
+ *           points x_l +- rho e1, x_l +- rho e2, rho = m v_perp / (|q| B0), v_perp = sqrt(2 mu B0 / m), e1 = the
+ *           major-radius direction made perpendicular to b0, e2 = b0 x e1; a ring point outside the mesh contributes 0.
  * t0: time of the next step's x_l.  Resets steps_done to 0.                                                          */
 int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, double t0);
 

@@ -369,8 +369,8 @@ extern "C" int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, 
 extern "C" int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, double t0) {
     if (!ctx) return M3DK_EINVAL;
     if (sort_interval < 0) return fail(ctx, M3DK_EINVAL, "m3dk_set_options: sort_interval < 0");
-    if (mode != 0 && mode != 1)
-        return fail(ctx, M3DK_EINVAL, "m3dk_set_options: mode must be 0 (linear delta-f) or 1 (non-linear trajectories)");
+    if (mode < 0 || mode > 2)
+        return fail(ctx, M3DK_EINVAL, "m3dk_set_options: mode must be 0 (linear delta-f), 1 (non-linear trajectories) or 2 (linear + FLR)");
     ctx->sort_interval = sort_interval; ctx->mode = mode; ctx->t0 = t0;
     ctx->steps_done = 0;
     ctx->steps_since_sort = sort_interval;

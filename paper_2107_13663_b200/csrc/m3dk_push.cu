@@ -124,7 +124,11 @@ struct RecIO {   // record = (x, y, z, w | vx, vy, vz, mu): two 32-byte sectors,
 // Phase B: a6 perturbed quads folded into dw/dt as they are evaluated, a9 weight update.  Then a3 for the NEW position
 // (cached for the next step; it is the sort key) and, with kHist, the sort histogram of the new keys.
 // tile: the element's coefficient tile, in global memory (kSmem = false) or staged in shared memory (kSmem = true).
-template <int R, bool kHist, bool kSmem, class IO>
+__device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
+                                           const PertW &W);
+
+// kFlr (mode 2): phase B is replaced by the 4-point gyro-average of the perturbed fields (flr_wdot).
+template <int R, bool kHist, bool kSmem, class IO, bool kFlr = false>
 __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const double *__restrict__ tile,
                                        const long (&mi)[R], const long (&mo)[R], const bool (&on)[R]) {
     Marker s[R];
@@ -156,12 +160,15 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
         if (on[r]) io.load_vel(mi[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
         else { s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
     }
+    EqOut fe[kFlr ? R : 1];   // kept for the gyro ring (mode 2)
+    double zl[kFlr ? R : 1];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         EqOut f;
         f.psi_R = __dmul_rn(dx[r][0], se); f.psi_Z = __dmul_rn(de[r][0], se);
         f.Bm = v[r][1]; f.Bm_R = __dmul_rn(dx[r][1], se); f.Bm_Z = __dmul_rn(de[r][1], se);
         f.F = v[r][2]; f.kappa = v[r][3];
+        if (kFlr) { fe[r] = f; zl[r] = s[r].z; }
         push_eq(P, g[r], f, s[r], W[r]);
         Rn[r] = m3dk_sqrt(M3DK_FMA(s[r].x, s[r].x, __dmul_rn(s[r].y, s[r].y)));
         Zn[r] = s[r].z;
@@ -195,7 +202,14 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
         }
         if (kHist) hist_issue<R>(P.hist, key, on, peers, base);
     };
-    if (P.f.n_modes > 0) {
+    if (kFlr && P.f.n_modes > 0) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double wdot = flr_wdot(P, fe[kFlr ? r : 0], g[r], zl[kFlr ? r : 0], s[r].mu, W[r]);
+            if (on[r]) io.store_w(mo[r], M3DK_FMA(P.dt, wdot, s[r].w));
+        }
+        locate_and_count();
+    } else if (P.f.n_modes > 0) {
         double wsum[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) wsum[r] = 0.0;
@@ -237,40 +251,13 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
     if (kHist) rank_finish<R>(P.rank, mo, on, peers, base);
 }
 
-// ---- the same step in the non-linear trajectory mode (mode 1: PAPER.md:108, :130; reading G21) ------------------------
-// All perturbed fields are needed BEFORE the velocity update (the marker moves in the total fields), so they are
-// accumulated per marker (10 values) and the folding trick of the linear mode does not apply; B1_phi (quad 3) enters.
-template <int R, bool kHist, bool kSmem, class IO>
-__device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, const double *__restrict__ tile,
-                                          const long (&mi)[R], const long (&mo)[R], const bool (&on)[R]) {
-    Marker s[R];
-    StepGeom g[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        if (on[r]) { io.load_pos(mi[r], s[r].x, s[r].y, s[r].z, s[r].w); io.load_vel(mi[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu); }
-        else { s[r].x = 1.0; s[r].y = 0.0; s[r].z = 0.0; s[r].w = 0.0; s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
-    }
-    const Quad hd = ldq_t<kSmem>(tile);
-    const double Rc = hd.a, Zc = hd.b, se = hd.c;
-    double xi[R], eta[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        step_geometry(s[r], g[r]);
-        xi[r] = __dmul_rn(__dsub_rn(g[r].R, Rc), se); eta[r] = __dmul_rn(__dsub_rn(s[r].z, Zc), se);
-    }
+// Perturbed fields of R markers of one element, summed over the toroidal modes, in each marker's own cylindrical frame
+// (all four quads of every mode: E_R E_phi | E_Z B_R | B_par with gradient, B_Z | B_phi).  pf must be zeroed by the caller.
+template <int R, bool kSmem>
+__device__ __forceinline__ void pert_fields(const PushParams &P, const double *__restrict__ tile, const double (&xi)[R],
+                                            const double (&eta)[R], const StepGeom (&g)[R], double se, PertF (&pf)[R]) {
     double v[R][4], dx[R][4], de[R][4];
     Ring ring;
-    ring_fill<kSmem>(ring, tile + kTileHeader);
-    quad_vd<R, kSmem>(tile + kTileHeader, tile + kTileHeader, ring, xi, eta, v, dx, de);   // (psi0, |B|0, F0, kappa)
-    EqOut f[R];
-    PertF pf[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        f[r].psi_R = __dmul_rn(dx[r][0], se); f[r].psi_Z = __dmul_rn(de[r][0], se);
-        f[r].Bm = v[r][1]; f[r].Bm_R = __dmul_rn(dx[r][1], se); f[r].Bm_Z = __dmul_rn(de[r][1], se);
-        f[r].F = v[r][2]; f[r].kappa = v[r][3];
-        pf[r].ER = pf[r].EP = pf[r].EZ = pf[r].BR = pf[r].BP = pf[r].BZ = pf[r].gR = pf[r].gP = pf[r].gZ = pf[r].dT = 0.0;
-    }
     for (int md = 0; md < P.f.n_modes; ++md) {
         const int n = P.f.n_tor[md];
         const double om = P.f.omega[md];
@@ -308,6 +295,104 @@ __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, con
 #pragma unroll
         for (int r = 0; r < R; ++r) pf[r].BP = __dadd_rn(pf[r].BP, re_part(v[r][0], v[r][1], cth[r], sth[r]));
     }
+}
+
+// ---- finite Larmor radius (mode 2; Eq. 14; reading G23) ------------------------------------------
+// dw/dt of one marker with the perturbed fields replaced by the quarter sum over the four gyro-ring points
+// X +- rho e1, X +- rho e2 (rho = m v_perp / (|q| B), v_perp = sqrt(2 mu B / m); e1 = the major-radius direction made
+// perpendicular to b0, e2 = b0 x e1).  Each point is searched and evaluated on its own element's tile (global memory:
+// the ring leaves the marker's element), vectors are summed in Cartesian components and returned to the marker's
+// cylindrical frame.  A point outside the mesh contributes zero.  (g, zl) = cylindrical map and z of x_l.
+__device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
+                                           const PertW &W) {
+    const double BR = -__dmul_rn(f.psi_Z, g.rinv), BP = __dmul_rn(f.F, g.rinv), BZ = __dmul_rn(f.psi_R, g.rinv);
+    const double binv = m3dk_rsqrt(M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, __dmul_rn(BZ, BZ))));
+    const double bR = __dmul_rn(BR, binv), bP = __dmul_rn(BP, binv), bZ = __dmul_rn(BZ, binv);
+    const double rho = __dmul_rn(m3dk_sqrt(__dmul_rn(__dmul_rn(__dmul_rn(2.0, P.m), mu), binv)), fabs(P.inv_q));
+    // e1 = R-hat - (R-hat . b) b, normalised; e2 = b x e1 (cylindrical components at the marker)
+    double e1R = M3DK_FMA(-bR, bR, 1.0), e1P = -__dmul_rn(bR, bP), e1Z = -__dmul_rn(bR, bZ);
+    const double n1 = m3dk_rsqrt(M3DK_FMA(e1R, e1R, M3DK_FMA(e1P, e1P, __dmul_rn(e1Z, e1Z))));
+    e1R = __dmul_rn(e1R, n1); e1P = __dmul_rn(e1P, n1); e1Z = __dmul_rn(e1Z, n1);
+    const double e2R = M3DK_FMA(bP, e1Z, -__dmul_rn(bZ, e1P)), e2P = M3DK_FMA(bZ, e1R, -__dmul_rn(bR, e1Z)),
+                 e2Z = M3DK_FMA(bR, e1P, -__dmul_rn(bP, e1R));
+    const double c = g.cph, sn = g.sph;
+    const double ex[2] = {M3DK_FMA(e1R, c, -__dmul_rn(e1P, sn)), M3DK_FMA(e2R, c, -__dmul_rn(e2P, sn))};
+    const double ey[2] = {M3DK_FMA(e1R, sn, __dmul_rn(e1P, c)), M3DK_FMA(e2R, sn, __dmul_rn(e2P, c))};
+    const double ez[2] = {e1Z, e2Z};
+    const double X = __dmul_rn(g.R, c), Y = __dmul_rn(g.R, sn);
+    double Ex = 0.0, Ey = 0.0, Ez = 0.0, Bx = 0.0, By = 0.0, Bz = 0.0, Gx = 0.0, Gy = 0.0, Gz = 0.0, dT = 0.0;
+#pragma unroll 1
+    for (int j = 0; j < 4; ++j) {
+        const double sg = j < 2 ? rho : -rho;
+        const double x = M3DK_FMA(sg, ex[j & 1], X), y = M3DK_FMA(sg, ey[j & 1], Y), z = M3DK_FMA(sg, ez[j & 1], zl);
+        Marker sp;
+        sp.x = x; sp.y = y; sp.z = z;
+        StepGeom gj[1];
+        step_geometry(sp, gj[0]);
+        const int ej = locate_any(P.f, gj[0].R, z);
+        if (ej < 0) continue;
+        const double *tile = P.f.tiles + (size_t)ej * P.f.tile_stride;
+        const Quad hd = ldq(tile);
+        const double se = hd.c;
+        const double xi[1] = {__dmul_rn(__dsub_rn(gj[0].R, hd.a), se)}, eta[1] = {__dmul_rn(__dsub_rn(z, hd.b), se)};
+        PertF pf[1];
+        pf[0].ER = pf[0].EP = pf[0].EZ = pf[0].BR = pf[0].BP = pf[0].BZ = pf[0].gR = pf[0].gP = pf[0].gZ = pf[0].dT = 0.0;
+        pert_fields<1, false>(P, tile, xi, eta, gj, se, pf);
+        const double cj = gj[0].cph, sj = gj[0].sph;
+        Ex = __dadd_rn(Ex, M3DK_FMA(pf[0].ER, cj, -__dmul_rn(pf[0].EP, sj))); Ey = __dadd_rn(Ey, M3DK_FMA(pf[0].ER, sj, __dmul_rn(pf[0].EP, cj)));
+        Ez = __dadd_rn(Ez, pf[0].EZ);
+        Bx = __dadd_rn(Bx, M3DK_FMA(pf[0].BR, cj, -__dmul_rn(pf[0].BP, sj))); By = __dadd_rn(By, M3DK_FMA(pf[0].BR, sj, __dmul_rn(pf[0].BP, cj)));
+        Bz = __dadd_rn(Bz, pf[0].BZ);
+        Gx = __dadd_rn(Gx, M3DK_FMA(pf[0].gR, cj, -__dmul_rn(pf[0].gP, sj))); Gy = __dadd_rn(Gy, M3DK_FMA(pf[0].gR, sj, __dmul_rn(pf[0].gP, cj)));
+        Gz = __dadd_rn(Gz, pf[0].gZ);
+        dT = __dadd_rn(dT, pf[0].dT);
+    }
+    // back to the marker's frame, quarter sum (Eq. 14), then the linear right-hand side of Eqs. (8)-(13)
+    const double ER = __dmul_rn(0.25, M3DK_FMA(Ex, c, __dmul_rn(Ey, sn))), EP = __dmul_rn(0.25, M3DK_FMA(Ey, c, -__dmul_rn(Ex, sn)));
+    const double B1R = __dmul_rn(0.25, M3DK_FMA(Bx, c, __dmul_rn(By, sn)));
+    const double gR = __dmul_rn(0.25, M3DK_FMA(Gx, c, __dmul_rn(Gy, sn))), gP = __dmul_rn(0.25, M3DK_FMA(Gy, c, -__dmul_rn(Gx, sn)));
+    double a = __dmul_rn(W.aER, ER);
+    a = M3DK_FMA(W.aEP, EP, a); a = M3DK_FMA(W.aEZ, __dmul_rn(0.25, Ez), a);
+    a = M3DK_FMA(W.bBR, B1R, a); a = M3DK_FMA(W.bBZ, __dmul_rn(0.25, Bz), a);
+    a = M3DK_FMA(W.gR, gR, a); a = M3DK_FMA(W.gP, gP, a); a = M3DK_FMA(W.gZ, __dmul_rn(0.25, Gz), a);
+    return M3DK_FMA(W.dT, __dmul_rn(0.25, dT), a);
+}
+
+// ---- the same step in the non-linear trajectory mode (mode 1: PAPER.md:108, :130; reading G21) ------------------------
+// All perturbed fields are needed BEFORE the velocity update (the marker moves in the total fields), so they are
+// accumulated per marker (10 values) and the folding trick of the linear mode does not apply; B1_phi (quad 3) enters.
+template <int R, bool kHist, bool kSmem, class IO>
+__device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, const double *__restrict__ tile,
+                                          const long (&mi)[R], const long (&mo)[R], const bool (&on)[R]) {
+    Marker s[R];
+    StepGeom g[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (on[r]) { io.load_pos(mi[r], s[r].x, s[r].y, s[r].z, s[r].w); io.load_vel(mi[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu); }
+        else { s[r].x = 1.0; s[r].y = 0.0; s[r].z = 0.0; s[r].w = 0.0; s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
+    }
+    const Quad hd = ldq_t<kSmem>(tile);
+    const double Rc = hd.a, Zc = hd.b, se = hd.c;
+    double xi[R], eta[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        step_geometry(s[r], g[r]);
+        xi[r] = __dmul_rn(__dsub_rn(g[r].R, Rc), se); eta[r] = __dmul_rn(__dsub_rn(s[r].z, Zc), se);
+    }
+    double v[R][4], dx[R][4], de[R][4];
+    Ring ring;
+    ring_fill<kSmem>(ring, tile + kTileHeader);
+    quad_vd<R, kSmem>(tile + kTileHeader, tile + kTileHeader, ring, xi, eta, v, dx, de);   // (psi0, |B|0, F0, kappa)
+    EqOut f[R];
+    PertF pf[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        f[r].psi_R = __dmul_rn(dx[r][0], se); f[r].psi_Z = __dmul_rn(de[r][0], se);
+        f[r].Bm = v[r][1]; f[r].Bm_R = __dmul_rn(dx[r][1], se); f[r].Bm_Z = __dmul_rn(de[r][1], se);
+        f[r].F = v[r][2]; f[r].kappa = v[r][3];
+        pf[r].ER = pf[r].EP = pf[r].EZ = pf[r].BR = pf[r].BP = pf[r].BZ = pf[r].gR = pf[r].gP = pf[r].gZ = pf[r].dT = 0.0;
+    }
+    pert_fields<R, kSmem>(P, tile, xi, eta, g, se, pf);
     double Rn[R], Zn[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -357,11 +442,11 @@ __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant
         if (kRec) {
             const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems};
             if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on);
-            else step_R<1, false, false>(P, io, tile, m, m, on);
+            else step_R<1, false, false, RecIO, kMode == 2>(P, io, tile, m, m, on);
         } else {
             const SoAIO io{P.a, P.f.n_elems};
             if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on);
-            else step_R<1, false, false>(P, io, tile, m, m, on);
+            else step_R<1, false, false, SoAIO, kMode == 2>(P, io, tile, m, m, on);
         }
     }
     if (kHist) {
@@ -467,7 +552,7 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
             mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
             phase ^= 1u << b;
             if (kMode == 1) step_R_nl<kItemR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
-            else step_R<kItemR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
+            else step_R<kItemR, kHist, true, RecIO, kMode == 2>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
         }
         b ^= 1;
         it += stride;
@@ -553,6 +638,7 @@ cudaError_t launch_push_soa(m3dk_ctx *c, long n, double dt, double t) {
     PushParams P = make_params(c, c->user, n, dt, t);
     c->kernel_launches += 1;
     if (c->mode == 1) push_generic_kernel<false, false, 1><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
+    else if (c->mode == 2) push_generic_kernel<false, false, 2><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
     else push_generic_kernel<false, false, 0><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
     return cudaGetLastError();
 }
@@ -575,8 +661,9 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
         P.items = c->sb.items; P.n_items = c->sb.ioffs + c->f.n_elems + 1;
         const unsigned grid = (unsigned)(c->sm_count * M3DK_PUSH_MINBLOCKS);
         const size_t smem = (size_t)(kPushThreads / 32) * 2 * (c->f.tile_stride * 8 + 8);
-        auto kern = c->mode == 1 ? (with_hist ? push_items_kernel<true, 1> : push_items_kernel<false, 1>)
-                                 : (with_hist ? push_items_kernel<true, 0> : push_items_kernel<false, 0>);
+        auto kern = c->mode == 1   ? (with_hist ? push_items_kernel<true, 1> : push_items_kernel<false, 1>)
+                    : c->mode == 2 ? (with_hist ? push_items_kernel<true, 2> : push_items_kernel<false, 2>)
+                                   : (with_hist ? push_items_kernel<true, 0> : push_items_kernel<false, 0>);
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         kern<<<grid, kPushThreads, smem, c->stream>>>(P);
@@ -584,8 +671,9 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
     } else {
         P.rc.out = c->sb.rec[c->cur];
         const unsigned grid = (unsigned)((n + 127) / 128);
-        auto kern = c->mode == 1 ? (with_hist ? push_generic_kernel<true, true, 1> : push_generic_kernel<true, false, 1>)
-                                 : (with_hist ? push_generic_kernel<true, true, 0> : push_generic_kernel<true, false, 0>);
+        auto kern = c->mode == 1   ? (with_hist ? push_generic_kernel<true, true, 1> : push_generic_kernel<true, false, 1>)
+                    : c->mode == 2 ? (with_hist ? push_generic_kernel<true, true, 2> : push_generic_kernel<true, false, 2>)
+                                   : (with_hist ? push_generic_kernel<true, true, 0> : push_generic_kernel<true, false, 0>);
         kern<<<grid, 128, 0, c->stream>>>(P);
     }
     return cudaGetLastError();

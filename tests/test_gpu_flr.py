@@ -1,0 +1,67 @@
+"""GPU parity of the finite-Larmor-radius mode (m3dk_set_options mode = 2, Eq. 14,
+reading G23) against the oracle's mode 2 (pinned by tests/test_oracle_flr.py), through the C ABI."""
+import numpy as np
+import pytest
+
+import synth
+from gpu_helpers import KEYS, g16_errors, make_pusher, oracle_of, oracle_push, take
+from test_gpu_ordered import _unstructured
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = 1.0e-12
+SMALL = {1: dict(n_markers=5000 + 37, nx=32), 2: dict(n_markers=5000 + 37, nx=48), 3: dict(n_markers=5000 + 37, nx=64)}
+
+
+@pytest.mark.parametrize("verify", [True, False])
+@pytest.mark.parametrize("idx", [1, 2, 3])
+def test_per_step_parity_flr(idx, verify):
+    w = synth.make_config(idx, **SMALL[idx])
+    mesh, sp = oracle_of(w, mode=2)
+    p = make_pusher(w, verify=verify, mode=2)
+    state = {k: w.markers[k].copy() for k in KEYS}
+    done, worst = 0, np.zeros(3)
+    for s in (0, 1, 10, 40):
+        if s > done:
+            state, _, _ = oracle_push(mesh, sp, state, s - done, w.dt, t0=0.0, step0=done)
+            done = s
+        ref, e_ref, _ = oracle_push(mesh, sp, state, 1, w.dt, t0=0.0, step0=s)
+        p.set_state(state)
+        p.set_options(sort_interval=0, mode=2, t0=s * w.dt)
+        p.push(1, w.dt)
+        got, _, _ = p.state()
+        live = e_ref >= 0
+        assert live.sum() > 0.9 * live.size
+        wrms = np.sqrt(np.mean(ref["w"][live] ** 2))
+        ex, ev, ew = g16_errors(take(got, live), take(ref, live), w_floor=wrms)
+        worst = np.maximum(worst, [ex.max(), ev.max(), ew.max()])
+    assert worst.max() <= TOL_STEP, worst
+    # the averaging does something: the weights differ from the linear mode's on the same orbits
+    lin, _, _ = oracle_push(oracle_of(w)[0], oracle_of(w)[1], w.markers, 20, w.dt)
+    flr, _, _ = oracle_push(mesh, sp, w.markers, 20, w.dt)
+    assert np.array_equal(lin["x"], flr["x"])
+    assert np.abs(lin["w"] - flr["w"]).max() > 1e-3 * np.sqrt(np.mean(lin["w"] ** 2))
+
+
+@pytest.mark.parametrize("two_modes", [False, True])
+def test_flr_ordered_pipeline_and_bitwise_order_independence(two_modes):
+    """Mode 2 through the element-ordered path on an unstructured mesh (ring points land in other, arbitrary elements and
+    some fall outside the mesh), against the oracle, and the same bits for sort_interval 0, 1 and 3."""
+    w = _unstructured(two_modes=two_modes)
+    mesh, sp = oracle_of(w, mode=2)
+    nsteps = 5
+    ref, e_ref, _ = oracle_push(mesh, sp, w.markers, nsteps, w.dt)
+    res = {}
+    for si in (0, 1, 3):
+        p = make_pusher(w, verify=True, sort_interval=si, mode=2)
+        p.push(nsteps, w.dt)
+        got, elem, ids = p.state()
+        assert np.array_equal(np.sort(ids), np.arange(w.n_markers))
+        res[si] = got
+        live = e_ref >= 0
+        wrms = np.sqrt(np.mean(ref["w"][live] ** 2))
+        ex, ev, ew = g16_errors(take(got, live), take(ref, live), w_floor=wrms)
+        assert max(ex.max(), ev.max(), ew.max()) <= 5 * TOL_STEP, (si, ex.max(), ev.max(), ew.max())
+    for si in (1, 3):
+        for k in KEYS:
+            assert np.array_equal(res[si][k], res[0][k]), (si, k)
