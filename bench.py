@@ -49,6 +49,8 @@ def algorithmic_flops(n_modes: int, mode: int = 0) -> float:
     weight = 86 + 2                           # coefficients of dw/dt (Eqs. 8-13 incl. kappa_E), w update
     if mode == 1:                             # non-linear trajectories: + B_phi (re, im), total fields, (1 - w)
         return eq + common + weight + 30 + n_modes * (pert + 2 * 2 * 20 + fold + 5)
+    if mode == 2:                             # FLR: ring geometry, then 4 x (map, local coordinates, all 14 polynomials, rotation)
+        return eq + common + weight + 60 + 4 * (11 + 4 + 30 + n_modes * (pert + 2 * 2 * 20 + fold)) + 30
     return eq + common + weight + n_modes * (pert + fold)
 
 
@@ -167,7 +169,7 @@ def build_workload(args, rank: int):
 def config_dict(args, w, sort_interval, world):
     return {"workload": f"BASELINE.json configs[{args.config}] ({w.name})", "n_markers_per_gpu": w.n_markers,
             "mesh": f"{w.nx}x{w.nx} cells, {w.n_elems} triangles", "n_modes": w.n_modes, "dt": w.dt,
-            "sort_interval": sort_interval, "mode": "linear delta-f" if args.mode == 0 else "non-linear trajectories",
+            "sort_interval": sort_interval, "mode": ("linear delta-f", "non-linear trajectories", "linear delta-f + FLR 4-point average")[args.mode],
             "parallelism": f"{world} independent marker shard(s), no collective",
             "l2": "inputs larger than L2 (marker state %.0f MB + tables %.0f MB per GPU)" % (
                 w.n_markers * 64 / 1e6, (w.eq_coef.nbytes + w.pert_coef.nbytes) / 1e6)}
@@ -369,8 +371,9 @@ def main():
     ap.add_argument("--dt-gyro", type=float, default=None)
     ap.add_argument("--sort-interval", type=int, default=None)
     ap.add_argument("--ref-sample", type=int, default=65536, help="markers in the oracle's bounded sample")
-    ap.add_argument("--mode", type=int, default=0, choices=[0, 1],
-                    help="0: linear delta-f (the headline); 1: non-linear trajectories (SURVEY.md 8(f)-1)")
+    ap.add_argument("--mode", type=int, default=0, choices=[0, 1, 2],
+                    help="0: linear delta-f (the headline); 1: non-linear trajectories (SURVEY.md 8(f)-1); "
+                         "2: linear delta-f with the 4-point gyro-average (8(f)-2)")
     ap.add_argument("--deposit", action="store_true", help="also time m3dk_deposit (SURVEY.md 8(f)-4) on the final state")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4] sweep: one JSON line per (n, dt, sort interval)")

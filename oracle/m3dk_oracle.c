@@ -29,6 +29,9 @@
  * Mode 1 (non-linear trajectories; reading G21): step 5 uses the total fields,
  * B = B0 + B1 and E-dagger = E1 - (mu/q) grad(|B|0 + B1par), and step 7 keeps the factor (1 - w) of Eq. (8).
  *
+ * Mode 2 (finite Larmor radius; Eq. 14; reading G23): step 7 uses the quarter sum of the
+ * perturbed fields over the four gyro-ring points (gyro_ring, flr_average); pins F1-F4.
+ *
  * orc_deposit: right-hand sides of Eqs. (17)-(18) with a delta-function shape (readings G10, G22).
  *
  * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1-P15 of SURVEY.md 8(c), P16-P19 for mode 1, D1-D4 for the
