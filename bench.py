@@ -81,14 +81,17 @@ def measured_peaks():
 
 def ncu_traffic(config: int, sort_interval: int):
     """dram__bytes_read.sum + dram__bytes_write.sum of the push kernel, per launch, from the committed ncu --set full
-    capture of this workload (profiles/push_traffic.json, written by hand from the capture named there); None when no
-    capture of this configuration is committed."""
-    p = os.path.join(ROOT, "profiles", "push_traffic.json")
+    capture of this workload (profiles/push_traffic.csv, copied by hand from the capture named in the .md beside it);
+    None when no capture of this configuration is committed."""
+    p = os.path.join(ROOT, "profiles", "push_traffic.csv")
     if not os.path.exists(p):
         return None
     with open(p) as fh:
-        d = json.load(fh)
-    return d.get(f"config{config}_si{sort_interval}", {}).get("dram_bytes_per_launch")
+        for line in fh:
+            cols = [c.strip() for c in line.split(",")]
+            if len(cols) >= 3 and cols[0] == f"config{config}" and cols[1] == f"si{sort_interval}":
+                return float(cols[2])
+    return None
 
 
 class ClockSampler:
