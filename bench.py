@@ -143,7 +143,7 @@ def oracle_bounded_sample(w, n_sample: int, target_s: float = 15.0):
     stride = max(1, w.n_markers // n_sample)
     rate, n, secs, cores = oracle_sample_rate(w, max(stride, min(1024, w.n_markers // 1024 or 1)), 20)
     n_s = len(range(0, w.n_markers, stride))
-    steps = int(min(2000, max(20, target_s * rate / n_s)))
+    steps = int(min(6000, max(20, target_s * rate / n_s)))
     return oracle_sample_rate(w, stride, steps) + (stride, steps)
 
 

@@ -222,14 +222,6 @@ __device__ __forceinline__ int locate_fast(const FastGrid &g, double R, double Z
     return locate_fast_from(g, locate_first(g, R, Z), R, Z);
 }
 
-// first record of the bucket of (R, Z): one line into L1 (the search itself runs later)
-__device__ __forceinline__ void locate_prefetch(const FastGrid &g, double R, double Z) {
-    const double fx = (R - g.Rmin) * g.inv_hx, fz = (Z - g.Zmin) * g.inv_hz;
-    const bool inside = fx >= 0.0 && fx < (double)g.gx && fz >= 0.0 && fz < (double)g.gz;
-    const int ix = inside ? (int)fx : 0, iz = inside ? (int)fz : 0;
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(g.first + (size_t)(iz * g.gx + ix)));
-}
-
 __device__ __forceinline__ int locate_finish(const FieldParams &f, const FastRec &first, double R, double Z) {
     const int e = locate_fast_from(f.fast, first, R, Z);
     return e != -2 ? e : locate(f.grid, R, Z);

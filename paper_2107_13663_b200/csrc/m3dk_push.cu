@@ -180,8 +180,8 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
             io.store_vel(mo[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
         }
         // the element search of the new position runs after phase B (loading its first record here, or searching
-        // between the quads, costs registers in the hottest part of the kernel and measured slower)
-        locate_prefetch(P.f.fast, Rn[r], Zn[r]);
+        // between the quads, costs registers in the hottest part of the kernel and measured slower; an L1 prefetch of
+        // the record measured no gain)
     }
     // a3 for the NEW position (the key of the next sort) and, with kHist, the sort histogram of the new keys with each
     // marker's rank inside its key (the sort then needs no pass over the keys)
