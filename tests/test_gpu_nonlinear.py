@@ -89,3 +89,27 @@ def test_nonlinear_zero_amplitude_equals_linear_mode_on_gpu():
     for k in ("x", "y", "z", "vx", "vy", "vz"):
         d = np.abs(out[1][k] - out[0][k]).max()
         assert d <= 1e-13, (k, d)
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_300_step_parity_on_non_chaotic_orbits(mode):
+    """The long-run bar of BASELINE.json (<= 1e-8 on non-chaotic orbits, filter of reading G15 from the oracle alone) for the
+    non-linear and the FLR mode, through the ordered pipeline."""
+    w0 = synth.make_config(3, n_markers=600 + 7, nx=48)
+    w = dataclasses.replace(w0, pert_coef=w0.pert_coef * (20.0 if mode == 1 else 1.0))
+    mesh, sp = oracle_of(w, mode=mode)
+    nsteps = 300
+    a, ea, _ = oracle_push(mesh, sp, w.markers, nsteps, w.dt)
+    twin = {k: w.markers[k].copy() for k in KEYS}
+    for k in ("x", "y", "z"):
+        twin[k] *= (1.0 + 1.0e-13)
+    b, eb, _ = oracle_push(mesh, sp, twin, nsteps, w.dt)
+    ex, ev, _ = g16_errors(b, a)
+    keep = (ex < 1e-9) & (ev < 1e-9) & (ea == eb) & (ea >= 0)
+    assert keep.mean() > 0.5
+    p = make_pusher(w, verify=True, sort_interval=1, mode=mode)
+    p.push(nsteps, w.dt)
+    got, _, _ = p.state()
+    wrms = np.sqrt(np.mean(a["w"][keep] ** 2))
+    ex, ev, ew = g16_errors(take(got, keep), take(a, keep), w_floor=wrms)
+    assert max(ex.max(), ev.max(), ew.max()) <= 1.0e-8, (ex.max(), ev.max(), ew.max(), keep.mean())
