@@ -59,6 +59,10 @@ def lib():
             C.c_int, C.c_double, C.c_double, C.c_long, C.c_int]
         L.orc_gyro_ring.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_double, c_dp]
         L.orc_flr_fields.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_double, C.c_double, c_dp]
+        L.orc_gc_push.restype = C.c_long
+        L.orc_gc_push.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5 + [c_ip, C.c_int,
+                                  C.c_double, C.c_int]
+        L.orc_gc_rhs.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5
         L.orc_deposit.restype = C.c_long
         L.orc_deposit.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_dp]
         L.orc_trace.restype = C.c_long
@@ -191,6 +195,28 @@ def push_analytic(an: Analytic, sp: Species, markers: dict, nsteps: int, dt: flo
     n = st["x"].shape[0]
     lib().orc_push_analytic(C.byref(an), C.byref(sp), n, *ptrs, int(nsteps), float(dt), float(t0), int(step0), int(nthreads))
     return st
+
+
+def gc_push(sp: Species, x, y, z, vpar, mu, nsteps: int, dt: float, *, mesh=None, an=None, nthreads: int = 0):
+    """RK4 on the guiding-centre equations (Eqs. 1-4, equilibrium fields; reading G24).  Returns (x, y, z, vpar, elem, lost)."""
+    arrs = [np.array(a, dtype=np.float64, copy=True, order="C") for a in (x, y, z, vpar)]
+    mu = np.ascontiguousarray(mu, dtype=np.float64)
+    n = arrs[0].shape[0]
+    e = np.zeros(n, dtype=np.int32)
+    lost = lib().orc_gc_push(mesh.h if mesh is not None else None, C.byref(an) if an is not None else None, C.byref(sp), n,
+                             *[a.ctypes.data_as(c_dp) for a in arrs], mu.ctypes.data_as(c_dp), e.ctypes.data_as(c_ip),
+                             int(nsteps), float(dt), int(nthreads))
+    return arrs[0], arrs[1], arrs[2], arrs[3], e, int(lost)
+
+
+def gc_rhs(sp: Species, R, Z, vpar, mu, *, mesh=None, an=None):
+    """Right-hand sides of Eqs. (1)-(2): rows (dR/dt, R dphi/dt, dZ/dt, dv_par/dt)."""
+    R, Z, vpar, mu = (np.ascontiguousarray(a, dtype=np.float64) for a in (R, Z, vpar, mu))
+    out = np.zeros((R.shape[0], 4))
+    lib().orc_gc_rhs(mesh.h if mesh is not None else None, C.byref(an) if an is not None else None, C.byref(sp), R.shape[0],
+                     R.ctypes.data_as(c_dp), Z.ctypes.data_as(c_dp), vpar.ctypes.data_as(c_dp), mu.ctypes.data_as(c_dp),
+                     out.ctypes.data_as(c_dp))
+    return out
 
 
 def gyro_ring(sp: Species, X, mu: float, *, mesh=None, an=None):

@@ -709,6 +709,150 @@ double orc_weight_rhs(const double *fields18, const orc_species *sp, double R, c
 }
 
 /* ================================================================================================ */
+/* Guiding-centre equations with RK4 (Eqs. 1-4: the comparator pusher of Fig. 1 and the
+ * "(dX/dt)_0 using only the equilibrium fields" of PAPER.md:130), equilibrium fields only (E = 0; reading G24):
+ *     dX/dt      = (1/B*par) [ v_par B* + (mu/q) b x grad|B| ]            Eq. (1) with E = 0
+ *     m dv_par/dt = -(mu/B*par) B* . grad|B|                               Eq. (2) with E = 0
+ *     B* = B + (m v_par/q) curl b,   B*par = B* . b                        Eqs. (3), (4)
+ * b = B/|B| with B = grad psi x grad phi + F grad phi (G4); grad|B| from the |B| table; curl b needs the
+ * second derivatives of psi and the first of F -- the cost the paper's profile points at.
+ * Axisymmetric: (curl b)_R = -d b_phi/dZ, (curl b)_phi = d b_R/dZ - d b_Z/dR, (curl b)_Z = (1/R) d(R b_phi)/dR.   */
+typedef struct {
+    double psi_R, psi_Z, psi_RR, psi_RZ, psi_ZZ, F, F_R, F_Z, Bm, Bm_R, Bm_Z;
+} orc_gcf;
+
+static void poly_eval2(const double *c, double xi, double eta, double *dxx, double *dxe, double *dee)
+{
+    double xp[DEG + 1], ep[DEG + 1];
+    xp[0] = 1.0; ep[0] = 1.0;
+    for (int p = 1; p <= DEG; ++p) { xp[p] = xp[p - 1] * xi; ep[p] = ep[p - 1] * eta; }
+    double a = 0.0, b = 0.0, d = 0.0;
+    int k = 0;
+    for (int j = 0; j <= DEG; ++j)
+        for (int i = 0; i <= DEG - j; ++i, ++k) {
+            if (i > 1) a += c[k] * ((double)(i * (i - 1)) * (xp[i - 2] * ep[j]));
+            if (i > 0 && j > 0) b += c[k] * ((double)(i * j) * (xp[i - 1] * ep[j - 1]));
+            if (j > 1) d += c[k] * ((double)(j * (j - 1)) * (xp[i] * ep[j - 2]));
+        }
+    *dxx = a; *dxe = b; *dee = d;
+}
+
+static int gc_fields(const provider *pv, double R, double Z, orc_gcf *g)
+{
+    if (pv->kind == 0) {
+        const orc_mesh *m = pv->mesh;
+        int e = pv->brute ? locate_brute(m, R, Z) : locate_grid(m, R, Z);
+        if (e < 0) return -1;
+        double Rc, Zc, s;
+        elem_frame(m, e, &Rc, &Zc, &s);
+        double xi = (R - Rc) * s, eta = (Z - Zc) * s;
+        const double *ce = m->eq_coef + (size_t)e * N_EQ * NCOEF;
+        double v, dx, de, a, b, d;
+        poly_eval(ce, xi, eta, &v, &dx, &de);
+        poly_eval2(ce, xi, eta, &a, &b, &d);
+        g->psi_R = dx * s; g->psi_Z = de * s; g->psi_RR = a * s * s; g->psi_RZ = b * s * s; g->psi_ZZ = d * s * s;
+        poly_eval(ce + NCOEF, xi, eta, &v, &dx, &de);
+        g->Bm = v; g->Bm_R = dx * s; g->Bm_Z = de * s;
+        poly_eval(ce + 2 * NCOEF, xi, eta, &v, &dx, &de);
+        g->F = v; g->F_R = dx * s; g->F_Z = de * s;
+        return e;
+    }
+    const orc_analytic *a = pv->an;
+    double dR = R - a->R0, r2 = dR * dR + Z * Z, u = r2 / (a->a * a->a);
+    double dqdu, q = an_q(a, u, &dqdu);
+    double gq = a->B0 / q, gp_over_r = -a->B0 / (q * q) * dqdu * 2.0 / (a->a * a->a);
+    orc_fields f;
+    an_fields(a, R, 0.0, Z, 0.0, &f);
+    g->psi_R = f.psi_R; g->psi_Z = f.psi_Z; g->F = f.F; g->F_R = 0.0; g->F_Z = 0.0;
+    g->Bm = f.Bm; g->Bm_R = f.Bm_R; g->Bm_Z = f.Bm_Z;
+    g->psi_RR = gq + gp_over_r * dR * dR; g->psi_RZ = gp_over_r * dR * Z; g->psi_ZZ = gq + gp_over_r * Z * Z;
+    return 0;
+}
+
+/* right-hand side of Eqs. (1)-(2) at (R, Z, v_par): dX/dt in cylindrical components, dv_par/dt.  Returns -1 outside. */
+static int gc_rhs(const provider *pv, const orc_species *sp, double R, double Z, double vpar, double mu, double dX[3],
+                  double *dvpar)
+{
+    orc_gcf g;
+    int e = gc_fields(pv, R, Z, &g);
+    if (e < 0) return -1;
+    double q = sp->charge, m = sp->mass;
+    double B[3] = {-g.psi_Z / R, g.F / R, g.psi_R / R};
+    /* b = B / |B| with |B| from its own table; derivatives of b's components by the quotient rule */
+    double BR_R = -g.psi_RZ / R + g.psi_Z / (R * R), BR_Z = -g.psi_ZZ / R;
+    double BP_R = g.F_R / R - g.F / (R * R), BP_Z = g.F_Z / R;
+    double BZ_R = g.psi_RR / R - g.psi_R / (R * R), BZ_Z = g.psi_RZ / R;
+    double Bm = g.Bm;
+    double b[3] = {B[0] / Bm, B[1] / Bm, B[2] / Bm};
+    double bR_Z = (BR_Z - b[0] * g.Bm_Z) / Bm;
+    double bP_R = (BP_R - b[1] * g.Bm_R) / Bm, bP_Z = (BP_Z - b[1] * g.Bm_Z) / Bm;
+    double bZ_R = (BZ_R - b[2] * g.Bm_R) / Bm;
+    (void)BR_R; (void)BZ_Z;
+    double curlb[3] = {-bP_Z, bR_Z - bZ_R, b[1] / R + bP_R};
+    double Bs[3], Bspar = 0.0;
+    for (int k = 0; k < 3; ++k) { Bs[k] = B[k] + (m * vpar / q) * curlb[k]; Bspar += Bs[k] * b[k]; }
+    double gB[3] = {g.Bm_R, 0.0, g.Bm_Z};
+    double bxg[3] = {b[1] * gB[2] - b[2] * gB[1], b[2] * gB[0] - b[0] * gB[2], b[0] * gB[1] - b[1] * gB[0]};
+    for (int k = 0; k < 3; ++k) dX[k] = (vpar * Bs[k] + (mu / q) * bxg[k]) / Bspar;
+    *dvpar = -(mu / m) * (Bs[0] * gB[0] + Bs[1] * gB[1] + Bs[2] * gB[2]) / Bspar;
+    return e;
+}
+
+/* RK4 on y = (x, y, z, v_par) in Cartesian position; returns the element of the first stage (-1: lost, state frozen) */
+static int gc_step(const provider *pv, const orc_species *sp, double y[4], double mu, double dt)
+{
+    double k[4][4], yy[4];
+    int e0 = 0;
+    static const double cs[4] = {0.0, 0.5, 0.5, 1.0};
+    for (int st = 0; st < 4; ++st) {
+        for (int i = 0; i < 4; ++i) yy[i] = y[i] + (st ? cs[st] * dt * k[st - 1][i] : 0.0);
+        double R = sqrt(yy[0] * yy[0] + yy[1] * yy[1]), c = yy[0] / R, sn = yy[1] / R;
+        double dX[3], dv;
+        int e = gc_rhs(pv, sp, R, yy[2], yy[3], mu, dX, &dv);
+        if (e < 0) return -1;
+        if (st == 0) e0 = e;
+        k[st][0] = dX[0] * c - dX[1] * sn; k[st][1] = dX[0] * sn + dX[1] * c; k[st][2] = dX[2]; k[st][3] = dv;
+    }
+    for (int i = 0; i < 4; ++i) y[i] += dt / 6.0 * (k[0][i] + 2.0 * k[1][i] + 2.0 * k[2][i] + k[3][i]);
+    return e0;
+}
+
+/* n guiding centres nsteps RK4 steps; elem (optional out): element of the last step's first stage or -1 (lost, frozen) */
+long orc_gc_push(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, long n, double *x, double *y, double *z,
+                 double *vpar, const double *mu, int *elem, int nsteps, double dt, int nthreads)
+{
+    provider pv = {m ? 0 : 1, m, a, 0};
+    long lost = 0;
+    set_threads(nthreads);
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : lost)
+    for (long i = 0; i < n; ++i) {
+        double s[4] = {x[i], y[i], z[i], vpar[i]};
+        int e = 0, dead = 0;
+        for (int l = 0; l < nsteps && !dead; ++l) {
+            double keep[4] = {s[0], s[1], s[2], s[3]};
+            e = gc_step(&pv, sp, s, mu[i], dt);
+            if (e < 0) { dead = 1; for (int q = 0; q < 4; ++q) s[q] = keep[q]; }
+        }
+        if (dead) { lost++; e = -1; }
+        x[i] = s[0]; y[i] = s[1]; z[i] = s[2]; vpar[i] = s[3];
+        if (elem) elem[i] = e;
+    }
+    return lost;
+}
+
+/* right-hand side at given points, for the pins: out[n][4] = dX/dt (R, phi, Z components), dv_par/dt */
+void orc_gc_rhs(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, long n, const double *R, const double *Z,
+                const double *vpar, const double *mu, double *out)
+{
+    provider pv = {m ? 0 : 1, m, a, 0};
+    for (long i = 0; i < n; ++i) {
+        double dX[3] = {0, 0, 0}, dv = 0.0;
+        gc_rhs(&pv, sp, R[i], Z[i], vpar[i], mu[i], dX, &dv);
+        out[4 * i] = dX[0]; out[4 * i + 1] = dX[1]; out[4 * i + 2] = dX[2]; out[4 * i + 3] = dv;
+    }
+}
+
+/* ================================================================================================ */
 /* Moment deposition: right-hand sides of the Galerkin projection of the pressure moments with a
  * delta-function particle shape, Eqs. (17)-(18):
  *     rhs_par [e][h][k] = sum over markers p in element e of  w_p m v_par,p^2    nu_k(x_p) T_h(phi_p)

@@ -1,0 +1,125 @@
+"""Pins of the oracle's RK4 guiding-centre pusher (Eqs. 1-4; reading G24).  Against the
+exact invariants of the continuous equations (which involve curl b), the order of the integrator, the paper's qualitative
+claim of Fig. 1 (RK4 errors accumulate, slow-manifold Boris errors stay bounded) and the slow-manifold orbit itself.  CPU."""
+import numpy as np
+import pytest
+
+import synth
+from synth.configs import CHARGE, MASS
+
+from helpers import gc_start, invariants, trend_and_swing
+
+EQ = synth.CircularTokamak()
+TG = EQ.gyro_period_axis(CHARGE, MASS)
+
+
+def _bphi_R(R, Z):
+    BR, BP, BZ = EQ.B_cyl(R, Z)
+    return R * BP / np.sqrt(BR ** 2 + BP ** 2 + BZ ** 2)
+
+
+def test_g1_rhs_conserves_energy_and_pphi_pointwise(orc):
+    """dE/dt = m v_par dv_par/dt + mu grad|B| . dX/dt = 0 and dP_phi/dt = q grad psi . dX/dt + m d(v_par R b_phi)/dt = 0 hold
+    identically for Eqs. (1)-(4) in an axisymmetric field -- the second only if curl b is right.  grad|B| and grad(R b_phi)
+    are taken from the ANALYTIC equilibrium by central differences, independently of the oracle's own derivatives."""
+    an = orc.analytic_of(EQ)
+    sp = orc.species(CHARGE, MASS)
+    rng = np.random.Generator(np.random.PCG64(5))
+    n = 200
+    R, Z = rng.uniform(2.3, 3.7, n), rng.uniform(-0.6, 0.6, n)
+    vpar, mu = rng.uniform(-1.0, 1.0, n), rng.uniform(0.0, 0.01, n)
+    out = orc.gc_rhs(sp, R, Z, vpar, mu, an=an)
+    dR, dZ, dv = out[:, 0], out[:, 2], out[:, 3]
+    h = 1e-5
+    Bm = lambda r, z: np.sqrt(sum(b ** 2 for b in EQ.B_cyl(r, z)))
+    gBR, gBZ = (Bm(R + h, Z) - Bm(R - h, Z)) / (2 * h), (Bm(R, Z + h) - Bm(R, Z - h)) / (2 * h)
+    dE = MASS * vpar * dv + mu * (gBR * dR + gBZ * dZ)
+    scaleE = np.abs(MASS * vpar * dv) + np.abs(mu * gBR * dR) + np.abs(mu * gBZ * dZ) + 1e-12
+    assert (np.abs(dE) / scaleE).max() < 1e-7
+    pR, pZ = EQ.grad_psi(R, Z)
+    gR = (_bphi_R(R + h, Z) - _bphi_R(R - h, Z)) / (2 * h)
+    gZ = (_bphi_R(R, Z + h) - _bphi_R(R, Z - h)) / (2 * h)
+    dP = CHARGE * (pR * dR + pZ * dZ) + MASS * dv * _bphi_R(R, Z) + MASS * vpar * (gR * dR + gZ * dZ)
+    scaleP = np.abs(CHARGE * pR * dR) + np.abs(CHARGE * pZ * dZ) + np.abs(MASS * dv * _bphi_R(R, Z)) + 1e-12
+    assert (np.abs(dP) / scaleP).max() < 1e-6
+    # and the leading behaviour: parallel streaming along B plus a vertical grad-B / curvature drift of order rho* v
+    BR, BP, BZ = EQ.B_cyl(R, Z)
+    assert np.allclose(out[:, 1], vpar * BP / Bm(R, Z), rtol=0.05, atol=2e-3)
+
+
+def test_g2_fourth_order_convergence(orc):
+    an = orc.analytic_of(EQ)
+    sp = orc.species(CHARGE, MASS)
+    s = gc_start(EQ, 0.3, 0.6, 0.0, CHARGE, MASS)
+    R0 = np.hypot(s[0], s[1])
+    Bm = float(np.sqrt(sum(np.asarray(b) ** 2 for b in EQ.B_cyl(np.array([R0]), np.array([s[2]])))).reshape(-1)[0])
+    vpar0, mu = 0.6, MASS * (1 - 0.36) / (2 * Bm)
+    T = 60.0
+
+    def err(dt):
+        n = int(round(T / dt))
+        x, y, z, vp, e, lost = orc.gc_push(sp, [s[0]], [s[1]], [s[2]], [vpar0], [mu], n, T / n, an=an)
+        R = np.hypot(x, y)
+        B = np.sqrt(sum(np.asarray(b) ** 2 for b in EQ.B_cyl(R, z)))
+        return abs(0.5 * MASS * vp[0] ** 2 + mu * B[0] - (0.5 * MASS * vpar0 ** 2 + mu * Bm))
+    e1, e2, e3 = err(1.0), err(0.5), err(0.25)
+    assert 10.0 < e1 / e2 < 24.0 and 10.0 < e2 / e3 < 24.0, (e1, e2, e3)
+
+
+@pytest.mark.parametrize("lam", [0.8, 0.2])
+def test_g3_rk4_errors_accumulate_while_boris_errors_stay_bounded(orc, lam):
+    """PAPER.md:84, :92 (Fig. 1): with dt of several gyro-periods the energy error of the RK4 guiding-centre orbit
+    accumulates (a secular trend that dominates its oscillation), that of the slow-manifold Boris orbit at a quarter of the
+    step stays bounded (trend far below the oscillation)."""
+    an = orc.analytic_of(EQ)
+    sp = orc.species(CHARGE, MASS)
+    dt = 5.0 * TG
+    s = gc_start(EQ, 0.3, lam, dt / 4, CHARGE, MASS)
+    R0 = np.hypot(s[0], s[1])
+    Bm = float(np.sqrt(sum(np.asarray(b) ** 2 for b in EQ.B_cyl(np.array([R0]), np.array([s[2]])))).reshape(-1)[0])
+    mu = MASS * (1 - lam ** 2) / (2 * Bm)
+    nblk, per = 60, 200
+    x, y, z, vp = np.array([s[0]]), np.array([s[1]]), np.array([s[2]]), np.array([lam])
+    E = []
+    for _ in range(nblk):
+        x, y, z, vp, _, lost = orc.gc_push(sp, x, y, z, vp, [mu], per, dt, an=an)
+        assert lost == 0
+        B = np.sqrt(sum(np.asarray(b) ** 2 for b in EQ.B_cyl(np.hypot(x, y), z)))
+        E.append(0.5 * MASS * vp[0] ** 2 + mu * B[0])
+    E = np.array(E)
+    t = np.arange(nblk) * per * dt
+    drift = abs(E[-1] - E[0]) / abs(E[0])
+    trend, swing = trend_and_swing(t, E)
+    assert trend > 0.5 * swing and drift > 1e-8, (trend, swing, drift)          # RK4: the error is a trend
+    tr, _ = orc.trace(sp, s, 4 * nblk * per, dt / 4, an=an, stride=4 * per)
+    Eb, _ = invariants(orc, an, tr, s[6], CHARGE, MASS)
+    trend_b, swing_b = trend_and_swing(tr[:, 7], Eb)
+    assert trend_b < 0.2 * swing_b, (trend_b, swing_b)                           # Boris: bounded
+    assert trend / swing > 3.0 * trend_b / swing_b
+
+
+def test_g4_guiding_centre_orbit_lies_on_the_slow_manifold_orbit(orc):
+    """The slow-manifold Boris marker follows the guiding-centre orbit: same radial excursion (banana /
+    drift-surface shift) and the same poloidal transit time to a few per cent at rho* = 0.02."""
+    an = orc.analytic_of(EQ)
+    sp = orc.species(CHARGE, MASS)
+    lam = 0.75
+    dt = 0.5 * TG
+    s = gc_start(EQ, 0.3, lam, dt, CHARGE, MASS)
+    n = int(260 / dt)
+    tr, _ = orc.trace(sp, s, n, dt, an=an, stride=8)
+    rb = np.hypot(np.hypot(tr[:, 0], tr[:, 1]) - EQ.R0, tr[:, 2])
+    thb = np.unwrap(np.arctan2(tr[:, 2], np.hypot(tr[:, 0], tr[:, 1]) - EQ.R0))
+    R0 = np.hypot(s[0], s[1])
+    Bm = float(np.sqrt(sum(np.asarray(b) ** 2 for b in EQ.B_cyl(np.array([R0]), np.array([s[2]])))).reshape(-1)[0])
+    mu = s[6]
+    BR, BP, BZ = (float(np.asarray(b).reshape(-1)[0]) for b in EQ.B_cyl(np.array([R0]), np.array([s[2]])))
+    vpar0 = (s[3] * BR + s[4] * BP + s[5] * BZ) / Bm                              # phi = 0 at the start: (vx, vy, vz) = (vR, vphi, vZ)
+    x, y, z, vp = np.array([s[0]]), np.array([s[1]]), np.array([s[2]]), np.array([vpar0])
+    rg, thg = [], []
+    for _ in range(len(tr)):
+        rg.append(np.hypot(np.hypot(x[0], y[0]) - EQ.R0, z[0])); thg.append(np.arctan2(z[0], np.hypot(x[0], y[0]) - EQ.R0))
+        x, y, z, vp, _, _ = orc.gc_push(sp, x, y, z, vp, [mu], 8, dt, an=an)
+    rg, thg = np.array(rg), np.unwrap(np.array(thg))
+    assert abs((rg.max() - rg.min()) - (rb.max() - rb.min())) < 0.1 * (rb.max() - rb.min()) + 2e-3
+    assert abs(thg[-1] - thb[-1]) < 0.05 * abs(thb[-1])
