@@ -156,6 +156,15 @@ int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, double *hz, d
 int m3dk_eval_fields(m3dk_ctx *ctx, long n, const double *R, const double *phi, const double *Z, double t,
                      int *elem_out, double *out);
 
+/* RK4 guiding-centre pusher (Eqs. 1-4; reading G24): the paper's comparator
+ * (Fig. 1) and the equilibrium guiding-centre motion "(dX/dt)_0" of PAPER.md:130.  Equilibrium fields only (E = 0):
+ *   dX/dt = (1/B*par)[v_par B* + (mu/q) b x grad|B|],  m dv_par/dt = -(mu/B*par) B* . grad|B|,
+ *   B* = B + (m v_par/q) curl b,  B*par = B* . b;  curl b from the second derivatives of psi0 and the first of F0.
+ * The registered arrays x, y, z are read and written as the guiding-centre position X (Cartesian), mu is read, elem is
+ * kept up to date; vx, vy, vz, w are not touched.  vpar: DEVICE [n], in/out.  nsteps classical RK4 steps of size dt.  A
+ * guiding centre one of whose stages leaves the mesh is lost: state of the step before, elem = -1, frozen.  Asynchronous. */
+int m3dk_gc_push(m3dk_ctx *ctx, int nsteps, double dt, double *vpar);
+
 /* Moment deposition: right-hand sides of the Galerkin projection of the energetic-particle pressure
  * moments with a delta-function particle shape, Eqs. (17)-(18) (readings G10, G22):
  *   rhs[e][0][h][k] = sum over the markers p in element e of  w_p m v_par,p^2    nu_k(x_p) T_h(phi_p)     (parallel)

@@ -78,6 +78,7 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_particles_upload": ([vp] + [vp] * 8, i),
         "m3dk_particles_download": ([vp] + [vp] * 10, i),
         "m3dk_eval_fields": ([vp, lng, vp, vp, vp, dbl, vp, vp], i),
+        "m3dk_gc_push": ([vp, i, dbl, vp], i),
         "m3dk_deposit_bytes": ([vp, C.POINTER(sz)], i),
         "m3dk_deposit": ([vp, vp], i),
         "m3dk_fp64_peak_tflops": ([vp, _c_dp], i),
@@ -305,6 +306,17 @@ class Pusher:
                                          self._p(out)))
         self.stats()
         return elem.cpu().numpy(), out.cpu().numpy()
+
+    def gc_push(self, nsteps: int, dt: float, vpar):
+        """m3dk_gc_push: RK4 guiding-centre steps; vpar is a numpy array (copied to the device and back).  Returns
+        (x, y, z, vpar, elem) as numpy arrays in slot order (synchronises)."""
+        t = self.torch
+        vp = t.from_numpy(_np_d(vpar).copy()).to(self.device)
+        self._ck(self.L.m3dk_gc_push(self.h, int(nsteps), float(dt), self._p(vp)))
+        self.stats()
+        self._keep["vpar"] = vp
+        return (self.state_t["x"].cpu().numpy(), self.state_t["y"].cpu().numpy(), self.state_t["z"].cpu().numpy(),
+                vp.cpu().numpy(), self.elem_t.cpu().numpy())
 
     def deposit_bytes(self) -> int:
         need = C.c_size_t()

@@ -539,6 +539,15 @@ extern "C" int m3dk_eval_fields(m3dk_ctx *ctx, long n, const double *R, const do
     return M3DK_OK;
 }
 
+extern "C" int m3dk_gc_push(m3dk_ctx *ctx, int nsteps, double dt, double *vpar) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_gc_push: fields and markers must be set first");
+    if (nsteps < 0 || !(dt == dt) || (ctx->n > 0 && !vpar)) return fail(ctx, M3DK_EINVAL, "m3dk_gc_push: nsteps < 0, dt is NaN or vpar is NULL");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CU(launch_gc_push(ctx, ctx->n, vpar, nsteps, dt), "guiding-centre kernel");
+    return M3DK_OK;
+}
+
 extern "C" int m3dk_deposit_bytes(const m3dk_ctx *ctx, size_t *bytes) {
     if (!ctx || !bytes) return M3DK_EINVAL;
     if (!ctx->have_fields) return M3DK_ESTATE;

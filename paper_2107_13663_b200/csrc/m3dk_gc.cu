@@ -1,0 +1,134 @@
+// m3dk_gc.cu -- RK4 guiding-centre pusher (Eqs. 1-4; reading G24): the paper's comparator
+// pusher (Fig. 1) and the "(dX/dt)_0 using only the equilibrium fields" of PAPER.md:130.  Equilibrium fields only (E = 0):
+//     dX/dt       = (1/B*par) [ v_par B* + (mu/q) b x grad|B| ]      B* = B + (m v_par/q) curl b,  B*par = B* . b
+//     m dv_par/dt = -(mu/B*par) B* . grad|B|
+// curl b needs the SECOND derivatives of psi0 and the first of F0 (the cost that made the authors prefer the
+// Boris scheme); |B| and its gradient come from the |B| table.  One guiding centre per thread, four stages per step, each
+// with its own element search and tile gather (the stages leave the element): the one-marker-per-thread regime.
+#include "m3dk_device.cuh"
+
+namespace m3dk {
+
+// value, first and second derivatives of the four polynomials of a quad at (xi, eta): nested Horner.  Row j of the
+// triangle is a polynomial in xi (value r, r', r''/2 by the three-term Horner recurrence); the rows are then combined by
+// the same recurrence in eta.  out[s] = {f, f_xi, f_eta, f_xixi, f_xieta, f_etaeta}.
+__device__ __forceinline__ void quad_d2(const double *__restrict__ c, double xi, double eta, double (&out)[4][6]) {
+    constexpr int kRow[6] = {0, 6, 11, 15, 18, 20};
+    double V[4], Ve[4], Vee[4], X[4], Xe[4], XX[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) V[s] = Ve[s] = Vee[s] = X[s] = Xe[s] = XX[s] = 0.0;
+#pragma unroll
+    for (int j = 5; j >= 0; --j) {
+        const int L = 6 - j;
+        double r[4] = {0.0, 0.0, 0.0, 0.0}, r1[4] = {0.0, 0.0, 0.0, 0.0}, r2[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+        for (int i = L - 1; i >= 0; --i) {
+            const Quad u = ldq(c + 4 * (kRow[j] + i));
+            const double uu[4] = {u.a, u.b, u.c, u.d};
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                r2[s] = M3DK_FMA(r2[s], xi, r1[s]);
+                r1[s] = M3DK_FMA(r1[s], xi, r[s]);
+                r[s] = M3DK_FMA(r[s], xi, uu[s]);
+            }
+        }
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            Vee[s] = M3DK_FMA(Vee[s], eta, Ve[s]);
+            Ve[s] = M3DK_FMA(Ve[s], eta, V[s]);
+            V[s] = M3DK_FMA(V[s], eta, r[s]);
+            Xe[s] = M3DK_FMA(Xe[s], eta, X[s]);
+            X[s] = M3DK_FMA(X[s], eta, r1[s]);
+            XX[s] = M3DK_FMA(XX[s], eta, r2[s]);
+        }
+    }
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+        out[s][0] = V[s]; out[s][1] = X[s]; out[s][2] = Ve[s];
+        out[s][3] = __dmul_rn(2.0, XX[s]); out[s][4] = Xe[s]; out[s][5] = __dmul_rn(2.0, Vee[s]);
+    }
+}
+
+// right-hand side of Eqs. (1)-(2) at (R, Z, v_par): dX/dt in cylindrical components, dv_par/dt; false outside the mesh
+__device__ __forceinline__ bool gc_rhs(const FieldParams &f, double q, double m, double R, double Z, double vpar, double mu,
+                                       double (&dX)[3], double &dv, int &elem) {
+    const int e = locate_any(f, R, Z);
+    elem = e;
+    if (e < 0) return false;
+    const double *tile = f.tiles + (size_t)e * f.tile_stride;
+    const Quad hd = ldq(tile);
+    const double se = hd.c, xi = (R - hd.a) * se, eta = (Z - hd.b) * se;
+    double d[4][6];
+    quad_d2(tile + kTileHeader, xi, eta, d);                     // slots: psi0, |B|0, F0, kappa
+    const double s2 = se * se, rinv = m3dk_rcp(R), rinv2 = rinv * rinv;
+    const double psi_R = d[0][1] * se, psi_Z = d[0][2] * se, psi_RR = d[0][3] * s2, psi_RZ = d[0][4] * s2, psi_ZZ = d[0][5] * s2;
+    const double Bm = d[1][0], Bm_R = d[1][1] * se, Bm_Z = d[1][2] * se;
+    const double F = d[2][0], F_R = d[2][1] * se, F_Z = d[2][2] * se;
+    const double B[3] = {-psi_Z * rinv, F * rinv, psi_R * rinv};
+    const double BR_Z = -psi_ZZ * rinv;
+    const double BP_R = F_R * rinv - F * rinv2, BP_Z = F_Z * rinv;
+    const double BZ_R = psi_RR * rinv - psi_R * rinv2;
+    (void)psi_RZ;
+    const double binv = m3dk_rcp(Bm);
+    const double b[3] = {B[0] * binv, B[1] * binv, B[2] * binv};
+    const double bR_Z = (BR_Z - b[0] * Bm_Z) * binv;
+    const double bP_R = (BP_R - b[1] * Bm_R) * binv, bP_Z = (BP_Z - b[1] * Bm_Z) * binv;
+    const double bZ_R = (BZ_R - b[2] * Bm_R) * binv;
+    const double curlb[3] = {-bP_Z, bR_Z - bZ_R, b[1] * rinv + bP_R};
+    const double mvq = m * vpar / q;
+    const double Bs[3] = {B[0] + mvq * curlb[0], B[1] + mvq * curlb[1], B[2] + mvq * curlb[2]};
+    const double Bspar = Bs[0] * b[0] + Bs[1] * b[1] + Bs[2] * b[2];
+    const double bsinv = m3dk_rcp(Bspar);
+    const double muq = mu / q;
+    const double bxg[3] = {b[1] * Bm_Z, b[2] * Bm_R - b[0] * Bm_Z, -b[1] * Bm_R};     // b x grad|B|, grad|B| = (Bm_R, 0, Bm_Z)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) dX[k] = (vpar * Bs[k] + muq * bxg[k]) * bsinv;
+    dv = -(mu / m) * (Bs[0] * Bm_R + Bs[2] * Bm_Z) * bsinv;
+    return true;
+}
+
+// nsteps RK4 steps of y = (x, y, z, v_par); a guiding centre one of whose stages leaves the mesh is lost: its state is
+// the one before that step, elem = -1, frozen from then on (reading G12)
+__global__ void __launch_bounds__(128) gc_push_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, double *vpar,
+                                                      long n, double q, double m, double dt, int nsteps) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int e = a.elem[i];
+    if (e < 0) return;
+    double y[4] = {a.x[i], a.y[i], a.z[i], vpar[i]};
+    const double mu = a.mu[i];
+    for (int l = 0; l < nsteps; ++l) {
+        double k[4][4], yy[4];
+        bool ok = true;
+        int e0 = e;
+#pragma unroll
+        for (int st = 0; st < 4; ++st) {
+            const double cs = st == 0 ? 0.0 : (st == 3 ? 1.0 : 0.5);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) yy[c] = st ? y[c] + cs * dt * k[st > 0 ? st - 1 : 0][c] : y[c];
+            const double r2 = yy[0] * yy[0] + yy[1] * yy[1];
+            const double rinv = m3dk_rsqrt(r2), R = r2 * rinv, c = yy[0] * rinv, sn = yy[1] * rinv;
+            double dX[3], dv;
+            int es;
+            if (ok && !gc_rhs(f, q, m, R, yy[2], yy[3], mu, dX, dv, es)) ok = false;
+            if (!ok) { dX[0] = dX[1] = dX[2] = 0.0; dv = 0.0; es = -1; }
+            if (st == 0) e0 = es;
+            k[st][0] = dX[0] * c - dX[1] * sn; k[st][1] = dX[0] * sn + dX[1] * c; k[st][2] = dX[2]; k[st][3] = dv;
+        }
+        if (!ok) { e = -1; break; }
+        e = e0;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) y[c] += dt / 6.0 * (k[0][c] + 2.0 * k[1][c] + 2.0 * k[2][c] + k[3][c]);
+    }
+    a.x[i] = y[0]; a.y[i] = y[1]; a.z[i] = y[2]; vpar[i] = y[3];
+    a.elem[i] = e;
+}
+
+cudaError_t launch_gc_push(m3dk_ctx *c, long n, double *vpar, int nsteps, double dt) {
+    if (n == 0 || nsteps == 0) return cudaSuccess;
+    c->kernel_launches += 1;
+    gc_push_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, c->user, vpar, n, c->q, c->m, dt, nsteps);
+    return cudaGetLastError();
+}
+
+}  // namespace m3dk

@@ -1,0 +1,72 @@
+"""GPU parity of m3dk_gc_push (RK4 guiding-centre pusher, Eqs. 1-4, reading G24) against the oracle's
+gc_push on the same finite-element tables (pinned by tests/test_oracle_gc.py), through the C ABI."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from gpu_helpers import make_pusher
+
+pytestmark = pytest.mark.gpu
+
+
+def _vpar(w):
+    """v . b0 of the workload's markers from the analytic equilibrium (an input, not method arithmetic)."""
+    mk = w.markers
+    R = np.hypot(mk["x"], mk["y"])
+    BR, BP, BZ = w.eq.B_cyl(R, mk["z"])
+    Bn = np.sqrt(BR ** 2 + BP ** 2 + BZ ** 2)
+    c, s = mk["x"] / R, mk["y"] / R
+    return ((mk["vx"] * c + mk["vy"] * s) * BR + (-mk["vx"] * s + mk["vy"] * c) * BP + mk["vz"] * BZ) / Bn
+
+
+def _err(got, ref, live):
+    gx, gy, gz, gv = got
+    rx, ry, rz, rv = ref
+    dx = np.sqrt((gx - rx) ** 2 + (gy - ry) ** 2 + (gz - rz) ** 2) / np.sqrt(rx ** 2 + ry ** 2 + rz ** 2)
+    dv = np.abs(gv - rv) / np.maximum(np.abs(rv), np.sqrt(np.mean(rv[live] ** 2)))
+    return float(dx[live].max()), float(dv[live].max())
+
+
+@pytest.mark.parametrize("verify", [True, False])
+@pytest.mark.parametrize("idx,nx", [(0, 32), (3, 64)])
+def test_gc_push_matches_oracle(idx, nx, verify):
+    w = synth.make_config(idx, n_markers=5000 + 13, nx=nx)
+    mesh, sp = oracle.Mesh.of(w), oracle.species_of(w)
+    mk, vp0 = w.markers, _vpar(w)
+    dt = 2.0 * w.dt
+    for nsteps, tol in ((1, 1e-12), (40, 1e-9)):
+        rx, ry, rz, rv, e_ref, lost = oracle.gc_push(sp, mk["x"], mk["y"], mk["z"], vp0, mk["mu"], nsteps, dt, mesh=mesh)
+        p = make_pusher(w, verify=verify)
+        gx, gy, gz, gv, e_gpu = p.gc_push(nsteps, dt, vp0)
+        live = e_ref >= 0
+        assert live.mean() > 0.9
+        assert np.array_equal(e_gpu < 0, e_ref < 0)
+        if nsteps == 1:
+            assert np.array_equal(e_gpu, e_ref)            # element of the step's first stage
+        ex, ev = _err((gx, gy, gz, gv), (rx, ry, rz, rv), live)
+        assert max(ex, ev) <= tol, (nsteps, ex, ev)
+        st, _, _ = p.state(by_id=False)
+        assert np.array_equal(st["mu"], mk["mu"]) and np.array_equal(st["vx"], mk["vx"])      # untouched arrays
+
+
+def test_gc_lost_guiding_centres_are_frozen():
+    w = synth.make_config(0, n_markers=400, nx=16)
+    mk = {k: v.copy() for k, v in w.markers.items()}
+    vp = _vpar(w)
+    mk["x"][:5] = 60.0                                  # outside from the start
+    mk["z"][5:25] = 1.0995                              # next to the upper edge: drift / streaming takes some of them out
+    w2 = dataclasses.replace(w, markers=mk)
+    mesh, sp = oracle.Mesh.of(w2), oracle.species_of(w2)
+    rx, ry, rz, rv, e_ref, lost = oracle.gc_push(sp, mk["x"], mk["y"], mk["z"], vp, mk["mu"], 30, 4.0 * w.dt, mesh=mesh)
+    p = make_pusher(w2, verify=True)
+    gx, gy, gz, gv, e_gpu = p.gc_push(30, 4.0 * w.dt, vp)
+    assert lost >= 6 and np.array_equal(e_gpu < 0, e_ref < 0)
+    assert np.array_equal(gx[:5], mk["x"][:5]) and np.array_equal(gv[:5], vp[:5])
+    dead = e_ref < 0
+    # a lost guiding centre keeps the state it had before the step that left the mesh: same as the oracle's
+    assert np.allclose(gx[dead], rx[dead], rtol=1e-9) and np.allclose(gz[dead], rz[dead], rtol=1e-9, atol=1e-12)
+    ex, ev = _err((gx, gy, gz, gv), (rx, ry, rz, rv), ~dead)
+    assert max(ex, ev) <= 1e-9
