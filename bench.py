@@ -295,6 +295,19 @@ def run_ours(args, rank, world, local_rank):
             "e2e": {"value": shard.whole_job_rate([N] * world, Ke, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": 64 * N / Ke,
                     "d2h_bytes_per_step": 64 * N / Ke, "note": f"one upload + {Ke} steps + one download (PAPER.md:237)"},
             "roofline": roof, "n_lost": st["n_lost"]}
+    if args.gc:
+        # row (f)-3: RK4 guiding-centre steps on the same markers (x, y, z as X; v_par = 0.5 for every marker)
+        vpar = torch.full((N,), 0.5, dtype=torch.float64, device=dev)
+        p.gc_push_into(3, w.dt, vpar)
+        torch.cuda.synchronize(dev)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record(p.stream)
+        p.gc_push_into(10, w.dt, vpar)
+        g1.record(p.stream)
+        torch.cuda.synchronize(dev)
+        gms = g0.elapsed_time(g1) / 10
+        line["gc"] = {"ms_per_step": gms, "particle_steps_per_s": N / (gms * 1e-3),
+                      "note": "m3dk_gc_push, RK4 on Eqs. (1)-(4), equilibrium fields (SURVEY.md 8(f)-3); 4 field evaluations per step"}
     if args.deposit:
         # row (f)-4: one deposition of the pressure moments from the element-ordered arrays the push left behind
         need = p.deposit_bytes()
@@ -377,6 +390,7 @@ def main():
     ap.add_argument("--mode", type=int, default=0, choices=[0, 1, 2],
                     help="0: linear delta-f (the headline); 1: non-linear trajectories (SURVEY.md 8(f)-1); "
                          "2: linear delta-f with the 4-point gyro-average (8(f)-2)")
+    ap.add_argument("--gc", action="store_true", help="also time m3dk_gc_push (SURVEY.md 8(f)-3) on the final state")
     ap.add_argument("--deposit", action="store_true", help="also time m3dk_deposit (SURVEY.md 8(f)-4) on the final state")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4] sweep: one JSON line per (n, dt, sort interval)")

@@ -32,6 +32,8 @@
  * Mode 2 (finite Larmor radius; Eq. 14; reading G23): step 7 uses the quarter sum of the
  * perturbed fields over the four gyro-ring points (gyro_ring, flr_average); pins F1-F4.
  *
+ * orc_gc_push: RK4 on the guiding-centre equations (1)-(4), equilibrium fields (reading G24); pins G1-G4.
+ *
  * orc_deposit: right-hand sides of Eqs. (17)-(18) with a delta-function shape (readings G10, G22).
  *
  * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1-P15 of SURVEY.md 8(c), P16-P19 for mode 1, D1-D4 for the

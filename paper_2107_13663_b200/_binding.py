@@ -318,6 +318,10 @@ class Pusher:
         return (self.state_t["x"].cpu().numpy(), self.state_t["y"].cpu().numpy(), self.state_t["z"].cpu().numpy(),
                 vp.cpu().numpy(), self.elem_t.cpu().numpy())
 
+    def gc_push_into(self, nsteps: int, dt: float, vpar_t):
+        """m3dk_gc_push on a caller's device tensor vpar [n] (asynchronous)."""
+        self._ck(self.L.m3dk_gc_push(self.h, int(nsteps), float(dt), self._p(vpar_t)))
+
     def deposit_bytes(self) -> int:
         need = C.c_size_t()
         self._ck(self.L.m3dk_deposit_bytes(self.h, C.byref(need)))
