@@ -312,19 +312,19 @@ def run_ours(args, rank, world, local_rank):
         # row (f)-4: one deposition of the pressure moments from the element-ordered arrays the push left behind
         need = p.deposit_bytes()
         rhs = torch.empty(need // 8, dtype=torch.float64, device=dev)
-        p.deposit_into(rhs)
+        p.deposit_into(rhs, 1, 0.0)
         torch.cuda.synchronize(dev)
         d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         d0.record(p.stream)
         for _ in range(5):
-            p.deposit_into(rhs)
+            p.deposit_into(rhs, 1, 0.0)
         d1.record(p.stream)
         torch.cuda.synchronize(dev)
         dms = d0.elapsed_time(d1) / 5
         dbytes = (68.0 * N + need)            # 8 fp64 + element key per marker read, the table cleared and accumulated
         line["deposit"] = {"ms": dms, "markers_per_s": N / (dms * 1e-3), "table_bytes": need,
                            "hbm_bytes": dbytes, "hbm_frac": dbytes / (dms * 1e-3) / (hbm_gbs * 1e9),
-                           "note": "m3dk_deposit, Eqs. (17)-(18), delta-function shape (SURVEY.md 8(f)-4)"}
+                           "note": "m3dk_deposit with the B1par term of Eq. (16), delta-function shape (SURVEY.md 8(f)-4)"}
     if world == 1 and not args.no_cpu_baseline:
         rate, n, secs, cores, stride, rsteps = oracle_bounded_sample(w, args.ref_sample)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",

@@ -64,7 +64,7 @@ def lib():
                                   C.c_double, C.c_int]
         L.orc_gc_rhs.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5
         L.orc_deposit.restype = C.c_long
-        L.orc_deposit.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_dp]
+        L.orc_deposit.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_dp, C.c_int, C.c_double]
         L.orc_trace.restype = C.c_long
         L.orc_trace.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_long, C.c_double,
                                 C.c_double, C.c_long, c_dp]
@@ -237,13 +237,14 @@ def flr_fields(sp: Species, X, mu: float, t: float = 0.0, *, mesh=None, an=None)
     return out if ok else None
 
 
-def deposit(mesh: "Mesh", sp: Species, markers: dict):
-    """Right-hand sides of Eqs. (17)-(18) with a delta-function shape: rhs[n_elems][2][1 + 2 n_modes][21], n_lost."""
+def deposit(mesh: "Mesh", sp: Species, markers: dict, flags: int = 0, t: float = 0.0):
+    """Right-hand sides of Eqs. (17)-(18) with a delta-function shape: rhs[n_elems][2][1 + 2 n_modes][21], n_lost.
+    flags bit 0: add the mu B1par term of Eq. (16) to the perpendicular moment (B1par at time t)."""
     st, ptrs = _state(markers)
     n = st["x"].shape[0]
     H = 1 + 2 * mesh.n_modes
     rhs = np.zeros((mesh.n_elems, 2, H, 21), dtype=np.float64)
-    lost = lib().orc_deposit(mesh.h, C.byref(sp), n, *ptrs, rhs.ctypes.data_as(c_dp))
+    lost = lib().orc_deposit(mesh.h, C.byref(sp), n, *ptrs, rhs.ctypes.data_as(c_dp), int(flags), float(t))
     return rhs, int(lost)
 
 

@@ -864,8 +864,12 @@ void orc_gc_rhs(const orc_mesh *m, const orc_analytic *a, const orc_species *sp,
  * physical volume, so the Jacobian J of Eq. (17) is absorbed by it; v_par = v . B0/|B0| with the marker's v as stored).
  * rhs[n_elems][2][1 + 2 n_modes][21], zero-filled here.  Lost markers (outside every triangle) deposit nothing.
  * Plain loops, one marker at a time, in marker order.                                                             */
+/* flags bit 0: the perpendicular moment carries the term of Eq. (16), mu |B|0 (w + B1par/|B|0) = w mu |B|0 + mu B1par,
+ * with B1par = Re[C e^{i(n phi - omega t)}] at time t ("the change of perpendicular pressure due to the variation of
+ * B_par"); without it Eq. (18) as printed.                                                            */
 long orc_deposit(const orc_mesh *m, const orc_species *sp, long n, const double *x, const double *y, const double *z,
-                 const double *vx, const double *vy, const double *vz, const double *mu, const double *w, double *rhs)
+                 const double *vx, const double *vy, const double *vz, const double *mu, const double *w, double *rhs,
+                 int flags, double t)
 {
     const int H = 1 + 2 * m->n_modes;
     long lost = 0;
@@ -875,13 +879,14 @@ long orc_deposit(const orc_mesh *m, const orc_species *sp, long n, const double 
         int e = locate_grid(m, R, Z);
         if (e < 0) { lost++; continue; }
         orc_fields f;
-        fe_fields(m, e, R, phi, Z, 0.0, &f);
+        fe_fields(m, e, R, phi, Z, t, &f);
         double B0[3] = {-f.psi_Z / R, f.F / R, f.psi_R / R};
         double B0n = sqrt(B0[0] * B0[0] + B0[1] * B0[1] + B0[2] * B0[2]);
         double c = x[p] / R, sn = y[p] / R;
         double vc[3] = {vx[p] * c + vy[p] * sn, -vx[p] * sn + vy[p] * c, vz[p]};
         double vpar = (vc[0] * B0[0] + vc[1] * B0[1] + vc[2] * B0[2]) / B0n;
         double a[2] = {w[p] * sp->mass * vpar * vpar, w[p] * mu[p] * f.Bm};
+        if (flags & 1) a[1] += mu[p] * f.B1p;
         double Rc, Zc, s;
         elem_frame(m, e, &Rc, &Zc, &s);
         double xi = (R - Rc) * s, eta = (Z - Zc) * s;

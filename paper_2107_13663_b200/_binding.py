@@ -80,7 +80,7 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_eval_fields": ([vp, lng, vp, vp, vp, dbl, vp, vp], i),
         "m3dk_gc_push": ([vp, i, dbl, vp], i),
         "m3dk_deposit_bytes": ([vp, C.POINTER(sz)], i),
-        "m3dk_deposit": ([vp, vp], i),
+        "m3dk_deposit": ([vp, vp, i, dbl], i),
         "m3dk_fp64_peak_tflops": ([vp, _c_dp], i),
         "m3dk_set_profiling": ([vp, i], i),
         "m3dk_timing": ([vp, C.POINTER(_Timing)], i),
@@ -327,16 +327,16 @@ class Pusher:
         self._ck(self.L.m3dk_deposit_bytes(self.h, C.byref(need)))
         return int(need.value)
 
-    def deposit_into(self, rhs):
+    def deposit_into(self, rhs, flags: int = 0, t: float = 0.0):
         """m3dk_deposit into a caller's device tensor of deposit_bytes() bytes (asynchronous)."""
-        self._ck(self.L.m3dk_deposit(self.h, self._p(rhs)))
+        self._ck(self.L.m3dk_deposit(self.h, self._p(rhs), int(flags), float(t)))
 
-    def deposit(self):
+    def deposit(self, flags: int = 0, t: float = 0.0):
         """m3dk_deposit into a fresh device tensor; returns it as numpy [n_elems][2][1 + 2 n_modes][21] (synchronises)."""
         need = C.c_size_t()
         self._ck(self.L.m3dk_deposit_bytes(self.h, C.byref(need)))
         rhs = self.torch.empty(need.value // 8, dtype=self.torch.float64, device=self.device)
-        self._ck(self.L.m3dk_deposit(self.h, self._p(rhs)))
+        self._ck(self.L.m3dk_deposit(self.h, self._p(rhs), int(flags), float(t)))
         self.stats()
         self._keep["rhs"] = rhs
         return rhs.cpu().numpy().reshape(self.n_elems, 2, 1 + 2 * self.n_modes, 21)

@@ -6,6 +6,8 @@
 // One marker per lane; the lanes of a warp that sit in the same element are reduced with shuffles and their sum enters the
 // table with ONE fp64 atomic per entry, so on an element-ordered marker stream (what m3dk_push leaves behind when
 // sort_interval >= 1) a warp makes one or two passes and an element's 42 (1 + 2 n_modes) sums receive a few atomics each.
+#include <math.h>
+
 #include "m3dk_device.cuh"
 
 namespace m3dk {
@@ -15,7 +17,11 @@ constexpr int kDepHarmMax = 1 + 2 * M3DK_MAX_MODES;
 // contributions of one marker: amp[0] = w m v_par^2, amp[1] = w mu |B|0; T[h]; xp[i] = xi^i, ep[j] = eta^j
 struct DepMarker { double amp[2], T[kDepHarmMax], xp[6], ep[6]; };
 
-__device__ __forceinline__ void dep_marker(const FieldParams &f, int e, const Marker &s, double mass, DepMarker &d) {
+// options of one deposition: with_b1par adds mu B1par (Eq. 16) to the perpendicular moment; cwt / swt = cos / sin(omega_k t)
+struct DepOpts { int with_b1par; double cwt[M3DK_MAX_MODES], swt[M3DK_MAX_MODES]; };
+
+__device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &o, int e, const Marker &s, double mass,
+                                           DepMarker &d) {
     StepGeom g;
     step_geometry(s, g);
     // equilibrium quad at the marker: B0 = grad psi0 x grad phi + F0 grad phi (G4), |B|0 from its own table
@@ -34,6 +40,18 @@ __device__ __forceinline__ void dep_marker(const FieldParams &f, int e, const Ma
     const double vpar = __dmul_rn(M3DK_FMA(vR, BR, M3DK_FMA(vP, BP, __dmul_rn(s.vz, BZ))), binv);
     d.amp[0] = __dmul_rn(__dmul_rn(s.w, mass), __dmul_rn(vpar, vpar));
     d.amp[1] = __dmul_rn(__dmul_rn(s.w, s.mu), v[0][1]);
+    if (o.with_b1par) {   // Eq. (16): mu |B|0 (w + B1par/|B|0); B1par = Re[C e^{i(n phi - omega t)}] from quad 2 of every mode
+        double b1p = 0.0;
+        for (int md = 0; md < f.n_modes; ++md) {
+            double cth, sth;
+            mode_phase(f.n_tor[md], g.cph, g.sph, o.cwt[md], o.swt[md], cth, sth);
+            const double *pm = tile + kTileHeader + kTileEq + kTileMode * md + 2 * kQuad;
+            ring_fill<false>(ring, pm);
+            quad_vd<1, false>(pm, pm, ring, xi1, eta1, v, dx, de);
+            b1p = __dadd_rn(b1p, re_part(v[0][0], v[0][1], cth, sth));
+        }
+        d.amp[1] = M3DK_FMA(s.mu, b1p, d.amp[1]);
+    }
     d.T[0] = 1.0;     // toroidal factors by complex powers of (cos phi + i sin phi)
 #pragma unroll
     for (int md = 0; md < M3DK_MAX_MODES; ++md)
@@ -44,8 +62,8 @@ __device__ __forceinline__ void dep_marker(const FieldParams &f, int e, const Ma
 }
 
 // any marker order: one marker per lane, the warp loops over its distinct elements
-__global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, long n,
-                                                      double mass, double *__restrict__ rhs) {
+__global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
+                                                      MarkerArrays a, long n, double mass, double *__restrict__ rhs) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const bool valid = i < n;
@@ -59,7 +77,7 @@ __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ Fi
         s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
     }
     DepMarker d;
-    dep_marker(f, e, s, mass, d);
+    dep_marker(f, o, e, s, mass, d);
     const size_t stride_e = (size_t)2 * H * M3DK_NCOEF;
     unsigned todo = __ballot_sync(0xffffffffu, active);
     while (todo) {
@@ -89,7 +107,8 @@ __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ Fi
 
 // element-ordered records cut into work items (the ordering kernels of m3dk_sort.cu): a warp takes an item (<= 64
 // markers of ONE element), every lane two of them, one reduction and one atomic per table entry and item
-__global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constant__ FieldParams f, const double *__restrict__ rec,
+__global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
+                                                            const double *__restrict__ rec,
                                                             const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                             double mass, double *__restrict__ rhs) {
     const int lane = threadIdx.x & 31;
@@ -109,7 +128,7 @@ __global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constan
             const double *p = rec + (size_t)kRecDoubles * (start + 32 * r + lane);
             s.x = p[0]; s.y = p[1]; s.z = p[2]; s.w = p[3]; s.vx = p[4]; s.vy = p[5]; s.vz = p[6]; s.mu = p[7];
         }
-        dep_marker(f, e, s, mass, d[r]);
+        dep_marker(f, o, e, s, mass, d[r]);
         if (!on) { d[r].amp[0] = 0.0; d[r].amp[1] = 0.0; }
     }
     double *out = rhs + (size_t)e * 2 * H * M3DK_NCOEF;
@@ -136,7 +155,10 @@ __global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constan
         }
 }
 
-cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs) {
+cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t) {
+    DepOpts o{};
+    o.with_b1par = (flags & 1) && c->f.n_modes > 0;
+    for (int k = 0; k < c->f.n_modes; ++k) { o.cwt[k] = cos(c->f.omega[k] * t); o.swt[k] = sin(c->f.omega[k] * t); }
     const size_t bytes = (size_t)c->f.n_elems * 2 * (1 + 2 * c->f.n_modes) * M3DK_NCOEF * sizeof(double);
     cudaError_t e = cudaMemsetAsync(rhs, 0, bytes, c->stream);
     if (e != cudaSuccess || n == 0) return e;
@@ -148,11 +170,11 @@ cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs) {
         const long max_items = n / kItemMarkers + c->f.n_elems + 2;
         c->kernel_launches += 1;
         deposit_items_kernel<<<(unsigned)((max_items + 3) / 4), 128, 0, c->stream>>>(
-            c->f, c->sb.rec[c->cur], c->sb.items, c->sb.ioffs + c->f.n_elems + 1, c->m, rhs);
+            c->f, o, c->sb.rec[c->cur], c->sb.items, c->sb.ioffs + c->f.n_elems + 1, c->m, rhs);
         return cudaGetLastError();
     }
     c->kernel_launches += 1;
-    deposit_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, c->user, n, c->m, rhs);
+    deposit_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->user, n, c->m, rhs);
     return cudaGetLastError();
 }
 

@@ -15,14 +15,19 @@ from test_gpu_ordered import _unstructured
 pytestmark = pytest.mark.gpu
 
 
-def _check(w, markers, p):
+def _check(w, markers, p, flags=0, t=0.0):
     mesh, sp = oracle_of(w)
-    ref, lost = oracle.deposit(mesh, sp, markers)
+    ref, lost = oracle.deposit(mesh, sp, markers, flags=flags, t=t)
     absw = dict(markers)
     absw["w"] = np.abs(markers["w"])
     scale, _ = oracle.deposit(mesh, sp, absw)
     S = scale[:, :, 0, 0][:, :, None, None]                     # sum of |a_p| per element and moment
-    got = p.deposit()
+    if flags & 1:                                               # + sum of |mu_p B1par| bounded by mu_p * max|B1par|
+        zero = dict(markers)
+        zero["w"] = np.zeros_like(markers["w"])
+        b1, _ = oracle.deposit(mesh, sp, zero, flags=1, t=t)
+        S = S + np.abs(b1).max() * 64.0 + np.abs(b1[:, :, 0, 0])[:, :, None, None] * 64.0
+    got = p.deposit(flags=flags, t=t)
     assert got.shape == ref.shape
     err = np.abs(got - ref)
     assert (err <= 1e-12 * S + 1e-300).all(), float((err / (S + 1e-300)).max())
@@ -71,3 +76,17 @@ def test_deposit_equilibrium_only_and_empty():
     empty = {k: np.zeros(0) for k in KEYS}
     p2 = make_pusher(dataclasses.replace(w, markers=empty), verify=False)
     assert np.abs(p2.deposit()).max() == 0.0
+
+
+def test_deposit_with_b1par_term_of_eq16():
+    """flags = M3DK_DEPOSIT_B1PAR at t != 0, one and two modes: the perpendicular moment gains mu B1par(x, t)."""
+    for two in (False, True):
+        w = _unstructured(two_modes=two)
+        rng = np.random.Generator(np.random.PCG64(9))
+        mk = {k: v.copy() for k, v in w.markers.items()}
+        mk["w"] = rng.normal(size=w.n_markers) * 1e-4
+        p = make_pusher(dataclasses.replace(w, markers=mk), verify=True)
+        got, ref, _ = _check(w, mk, p, flags=1, t=5.7)
+        off = p.deposit(flags=0, t=5.7)
+        assert np.abs(got[:, 1] - off[:, 1]).max() > 1e-3 * np.abs(off[:, 1]).max()      # the term is there
+        assert np.abs(got[:, 0] - off[:, 0]).max() <= 1e-12 * np.abs(off[:, 0]).max()     # parallel moment untouched

@@ -124,3 +124,31 @@ def test_d4_linear_in_w_and_independent_of_marker_order(orc, wl):
     perm = np.random.Generator(np.random.PCG64(1)).permutation(wl.n_markers)
     c, _ = orc.deposit(mesh, sp, {k: v[perm] for k, v in mk.items()})
     assert np.abs(c - a).max() <= 1e-12 * np.abs(a).max()
+
+
+def test_d5_b1par_term_of_eq16(orc):
+    """flags bit 0: with w = 0 the perpendicular moment is sum_p mu_p B1par(x_p, t) (Eq. 16); B1par here from the ANALYTIC
+    perturbation of the workload (the tables are quintic fits of it), at a time t != 0 so that the phase counts; the
+    parallel moment and the w-terms are untouched."""
+    w = synth.make_config(3, n_markers=20000, nx=32)
+    mk = {k: v.copy() for k, v in w.markers.items()}
+    mk["w"][:] = 0.0
+    t = 7.3
+    mesh, sp = orc.Mesh.of(w), orc.species_of(w)
+    rhs, _ = orc.deposit(mesh, sp, mk, flags=1, t=t)
+    off, _ = orc.deposit(mesh, sp, mk, flags=0, t=t)
+    assert np.abs(off).max() == 0.0 and np.abs(rhs[:, 0]).max() == 0.0
+    R, phi = np.hypot(mk["x"], mk["y"]), np.arctan2(mk["y"], mk["x"])
+    pert = w.perts[0]
+    amp = pert.amplitudes(R, mk["z"])                        # complex amplitudes in the table order, B_par last
+    Bpar = amp[6] if isinstance(amp, (list, tuple)) else amp[..., 6]
+    b1 = np.real(Bpar * np.exp(1j * (pert.n * phi - pert.omega * t)))
+    ref = (mk["mu"] * b1).sum()
+    got = rhs[:, 1, 0, 0].sum()
+    assert abs(got - ref) < 2e-3 * np.abs(mk["mu"] * b1).sum(), (got, ref)
+    # linear superposition with the w-term
+    mk2 = dict(mk)
+    mk2["w"] = np.full(w.n_markers, 0.25)
+    both, _ = orc.deposit(mesh, sp, mk2, flags=1, t=t)
+    wonly, _ = orc.deposit(mesh, sp, mk2, flags=0, t=t)
+    assert np.abs(both[:, 1] - wonly[:, 1] - rhs[:, 1]).max() < 1e-12 * np.abs(both[:, 1]).max()
