@@ -887,24 +887,40 @@ long orc_deposit(const orc_mesh *m, const orc_species *sp, long n, const double 
         double vpar = (vc[0] * B0[0] + vc[1] * B0[1] + vc[2] * B0[2]) / B0n;
         double a[2] = {w[p] * sp->mass * vpar * vpar, w[p] * mu[p] * f.Bm};
         if (flags & 1) a[1] += mu[p] * f.B1p;
-        double Rc, Zc, s;
-        elem_frame(m, e, &Rc, &Zc, &s);
-        double xi = (R - Rc) * s, eta = (Z - Zc) * s;
-        double xp[DEG + 1], ep[DEG + 1];
-        xp[0] = 1.0; ep[0] = 1.0;
-        for (int q = 1; q <= DEG; ++q) { xp[q] = xp[q - 1] * xi; ep[q] = ep[q - 1] * eta; }
-        for (int mom = 0; mom < 2; ++mom)
-            for (int h = 0; h < H; ++h) {
-                double T = 1.0;
-                if (h > 0) {
-                    double nn = (double)m->n_tor[(h - 1) / 2];
-                    T = ((h - 1) % 2 == 0) ? cos(nn * phi) : sin(nn * phi);
+        /* deposition points: the marker itself, or (flags bit 1) the four gyro-ring points of reading G23
+         * with a quarter of the amplitude each; a ring point outside the mesh deposits nothing                         */
+        double pts[4][3], wgt = 1.0;
+        int npts = 1;
+        pts[0][0] = x[p]; pts[0][1] = y[p]; pts[0][2] = z[p];
+        if (flags & 2) {
+            double X[3] = {x[p], y[p], z[p]};
+            gyro_ring(X, B0, c, sn, mu[p], sp->charge, sp->mass, pts);
+            npts = 4; wgt = 0.25;
+        }
+        for (int jp = 0; jp < npts; ++jp) {
+            double Rj = sqrt(pts[jp][0] * pts[jp][0] + pts[jp][1] * pts[jp][1]), phij = atan2(pts[jp][1], pts[jp][0]);
+            double Zj = pts[jp][2];
+            int ej = (flags & 2) ? locate_grid(m, Rj, Zj) : e;
+            if (ej < 0) continue;
+            double Rc, Zc, s;
+            elem_frame(m, ej, &Rc, &Zc, &s);
+            double xi = (Rj - Rc) * s, eta = (Zj - Zc) * s;
+            double xp[DEG + 1], ep[DEG + 1];
+            xp[0] = 1.0; ep[0] = 1.0;
+            for (int q = 1; q <= DEG; ++q) { xp[q] = xp[q - 1] * xi; ep[q] = ep[q - 1] * eta; }
+            for (int mom = 0; mom < 2; ++mom)
+                for (int h = 0; h < H; ++h) {
+                    double T = 1.0;
+                    if (h > 0) {
+                        double nn = (double)m->n_tor[(h - 1) / 2];
+                        T = ((h - 1) % 2 == 0) ? cos(nn * phij) : sin(nn * phij);
+                    }
+                    double *out = rhs + (((size_t)ej * 2 + mom) * H + h) * NCOEF;
+                    int k = 0;
+                    for (int j = 0; j <= DEG; ++j)
+                        for (int i = 0; i <= DEG - j; ++i, ++k) out[k] += wgt * a[mom] * T * (xp[i] * ep[j]);
                 }
-                double *out = rhs + (((size_t)e * 2 + mom) * H + h) * NCOEF;
-                int k = 0;
-                for (int j = 0; j <= DEG; ++j)
-                    for (int i = 0; i <= DEG - j; ++i, ++k) out[k] += a[mom] * T * (xp[i] * ep[j]);
-            }
+        }
     }
     return lost;
 }

@@ -152,3 +152,39 @@ def test_d5_b1par_term_of_eq16(orc):
     both, _ = orc.deposit(mesh, sp, mk2, flags=1, t=t)
     wonly, _ = orc.deposit(mesh, sp, mk2, flags=0, t=t)
     assert np.abs(both[:, 1] - wonly[:, 1] - rhs[:, 1]).max() < 1e-12 * np.abs(both[:, 1]).max()
+
+
+def test_d6_four_point_flr_deposition(orc):
+    """flags bit 1: each marker deposits a quarter of its amplitude at each of its four gyro-ring points.
+    One marker with a gyro-radius of a few elements: exactly the four elements that contain the ring points (ring from the
+    pinned gyro_ring, elements from the pinned search) receive a quarter each; over many markers the total of the unit test
+    function is unchanged and so is the total first moment in z (the ring is centred on the marker and z is linear)."""
+    from synth.mesh import element_frames
+    w = synth.make_config(1, n_markers=4000, nx=32)
+    mesh, sp = orc.Mesh.of(w), orc.species_of(w)
+    X = np.array([3.31, 0.0, 0.12])
+    BR, BP, BZ = (float(np.asarray(b).reshape(-1)[0]) for b in w.eq.B_cyl(np.array([X[0]]), np.array([X[2]])))
+    Bn = np.sqrt(BR ** 2 + BP ** 2 + BZ ** 2)
+    mu = 0.02 * 4.0                                         # rho = sqrt(2 m mu / B) / q ~ 0.1: several elements of size 0.07
+    one = dict(x=X[:1], y=X[1:2], z=X[2:], vx=np.zeros(1), vy=np.zeros(1), vz=np.zeros(1), mu=np.array([mu]), w=np.array([2.0]))
+    rhs, _ = orc.deposit(mesh, sp, one, flags=2)
+    pts = orc.gyro_ring(sp, X, mu, mesh=mesh)
+    el = mesh.locate(np.hypot(pts[:, 0], pts[:, 1]), pts[:, 2])
+    assert len(set(el.tolist())) == 4 and (el >= 0).all()
+    a_perp = 2.0 * mu * Bn
+    hit = np.flatnonzero(np.abs(rhs[:, 1, 0, 0]) > 0)
+    assert sorted(hit.tolist()) == sorted(el.tolist())
+    assert np.allclose(rhs[el, 1, 0, 0], 0.25 * a_perp, rtol=1e-5)
+    # many markers: totals and the z-moment are those of the plain deposition
+    rng = np.random.Generator(np.random.PCG64(3))
+    mk = {k: v.copy() for k, v in w.markers.items()}
+    mk["w"] = rng.normal(size=w.n_markers)
+    plain, _ = orc.deposit(mesh, sp, mk, flags=0)
+    flr, _ = orc.deposit(mesh, sp, mk, flags=2)
+    cen, se = element_frames(w.node_RZ, w.tri)
+    for mom in (0, 1):
+        scale = np.abs(plain[:, mom, 0, 0]).sum()
+        assert abs(flr[:, mom, 0, 0].sum() - plain[:, mom, 0, 0].sum()) < 1e-11 * scale
+        zmom = lambda r: (r[:, mom, 0, 6] / se + cen[:, 1] * r[:, mom, 0, 0]).sum()
+        assert abs(zmom(flr) - zmom(plain)) < 1e-10 * scale
+    assert np.abs(flr[:, 1, 0, 0] - plain[:, 1, 0, 0]).max() > 1e-3 * np.abs(plain[:, 1, 0, 0]).max()   # but it is spread out
