@@ -173,7 +173,9 @@ int m3dk_gc_push(m3dk_ctx *ctx, int nsteps, double dt, double *vpar);
  * T_0 = 1, T_{2m+1} = cos(n_tor[m] phi), T_{2m+2} = sin(n_tor[m] phi); v_par = v . B0/|B0| with the stored v (v_{l-1/2}).
  * flags bit 0 (M3DK_DEPOSIT_B1PAR): the perpendicular moment carries the term of Eq. (16), mu |B|0 (w + B1par/|B|0), i.e.
  * rhs[e][1] also receives mu_p B1par(x_p, t) with B1par = Re[C e^{i(n phi - omega t)}] at the time t given; 0: Eq. (18) as
- * printed.  The delta function is normalised in physical volume, so no Jacobian factor appears (G22); the mass-matrix solve that
+ * printed.  flags bit 1 (M3DK_DEPOSIT_FLR): 4-point FLR deposition: each marker deposits a quarter of its
+ * amplitudes at each of its four gyro-ring points (the ring of mode 2, reading G23), test functions taken at the ring
+ * point; a ring point outside the mesh deposits nothing.  The delta function is normalised in physical volume, so no Jacobian factor appears (G22); the mass-matrix solve that
  * turns these sums into pressure coefficients belongs to the MHD code and is out of scope.  Lost markers deposit nothing.
  * rhs: DEVICE, m3dk_deposit_bytes() bytes = [n_elems][2][1 + 2 n_modes][21] doubles, overwritten.  Asynchronous.  The
  * caller's arrays are read, not modified.  With a sort workspace set (m3dk_set_sort_workspace) the markers are first
@@ -182,6 +184,7 @@ int m3dk_gc_push(m3dk_ctx *ctx, int nsteps, double dt, double *vpar);
  * unordered stream).  Sums are accumulated with fp64 atomics: the order of addition, hence the last bits, may vary.     */
 int m3dk_deposit_bytes(const m3dk_ctx *ctx, size_t *bytes);
 #define M3DK_DEPOSIT_B1PAR 1
+#define M3DK_DEPOSIT_FLR 2
 int m3dk_deposit(m3dk_ctx *ctx, double *rhs, int flags, double t);
 
 /* Measured FP64 FMA throughput of the device (register-resident DFMA chains, all SMs), in TFLOP/s (FMA = 2 flop).

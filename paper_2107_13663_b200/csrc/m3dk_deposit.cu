@@ -105,6 +105,100 @@ __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ Fi
     }
 }
 
+// 4-point FLR deposition (flags bit 1): a marker deposits a quarter of its amplitudes at each of its four
+// gyro-ring points (the ring of reading G23, as in the FLR push).  One marker per lane; for each of the four points the lane
+// finds the point's element and the warp loops over its distinct elements exactly as deposit_kernel does.
+__global__ void __launch_bounds__(128) deposit_flr_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
+                                                          MarkerArrays a, long n, double q, double mass,
+                                                          double *__restrict__ rhs) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const bool valid = i < n;
+    const int e = valid ? a.elem[i] : -1;
+    const bool active = e >= 0;
+    const int H = 1 + 2 * f.n_modes;
+    Marker s;
+    if (active) {
+        s.x = a.x[i]; s.y = a.y[i]; s.z = a.z[i]; s.vx = a.vx[i]; s.vy = a.vy[i]; s.vz = a.vz[i]; s.mu = a.mu[i]; s.w = a.w[i];
+    } else {
+        s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
+    }
+    DepMarker d;
+    dep_marker(f, o, e, s, mass, d);          // amplitudes at the marker itself
+    // the ring: same construction as flr_wdot of the push (reading G23)
+    StepGeom g;
+    step_geometry(s, g);
+    const double *tile = f.tiles + (size_t)max(e, 0) * f.tile_stride;
+    const Quad hd = ldq(tile);
+    const double se0 = hd.c;
+    const double xi1[1] = {__dmul_rn(__dsub_rn(g.R, hd.a), se0)}, eta1[1] = {__dmul_rn(__dsub_rn(s.z, hd.b), se0)};
+    double v[1][4], dx[1][4], de[1][4];
+    Ring ring;
+    ring_fill<false>(ring, tile + kTileHeader);
+    quad_vd<1, false>(tile + kTileHeader, tile + kTileHeader, ring, xi1, eta1, v, dx, de);
+    const double BR = -__dmul_rn(__dmul_rn(de[0][0], se0), g.rinv), BP = __dmul_rn(v[0][2], g.rinv),
+                 BZ = __dmul_rn(__dmul_rn(dx[0][0], se0), g.rinv);
+    const double binv = m3dk_rsqrt(M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, __dmul_rn(BZ, BZ))));
+    const double bR = __dmul_rn(BR, binv), bP = __dmul_rn(BP, binv), bZ = __dmul_rn(BZ, binv);
+    const double rho = __dmul_rn(m3dk_sqrt(__dmul_rn(__dmul_rn(__dmul_rn(2.0, mass), s.mu), binv)), fabs(1.0 / q));
+    double e1R = M3DK_FMA(-bR, bR, 1.0), e1P = -__dmul_rn(bR, bP), e1Z = -__dmul_rn(bR, bZ);
+    const double n1 = m3dk_rsqrt(M3DK_FMA(e1R, e1R, M3DK_FMA(e1P, e1P, __dmul_rn(e1Z, e1Z))));
+    e1R = __dmul_rn(e1R, n1); e1P = __dmul_rn(e1P, n1); e1Z = __dmul_rn(e1Z, n1);
+    const double e2R = M3DK_FMA(bP, e1Z, -__dmul_rn(bZ, e1P)), e2P = M3DK_FMA(bZ, e1R, -__dmul_rn(bR, e1Z)),
+                 e2Z = M3DK_FMA(bR, e1P, -__dmul_rn(bP, e1R));
+    const double c = g.cph, sn = g.sph;
+    const double ex[2] = {M3DK_FMA(e1R, c, -__dmul_rn(e1P, sn)), M3DK_FMA(e2R, c, -__dmul_rn(e2P, sn))};
+    const double ey[2] = {M3DK_FMA(e1R, sn, __dmul_rn(e1P, c)), M3DK_FMA(e2R, sn, __dmul_rn(e2P, c))};
+    const double ez[2] = {e1Z, e2Z};
+    const double X = __dmul_rn(g.R, c), Y = __dmul_rn(g.R, sn);
+    const size_t stride_e = (size_t)2 * H * M3DK_NCOEF;
+#pragma unroll 1
+    for (int j = 0; j < 4; ++j) {
+        const double sg = j < 2 ? rho : -rho;
+        Marker sp;
+        sp.x = M3DK_FMA(sg, ex[j & 1], X); sp.y = M3DK_FMA(sg, ey[j & 1], Y); sp.z = M3DK_FMA(sg, ez[j & 1], s.z);
+        StepGeom gj;
+        step_geometry(sp, gj);
+        const int ej = active ? locate_any(f, gj.R, sp.z) : -1;
+        const bool on = ej >= 0;
+        const double *tj = f.tiles + (size_t)max(ej, 0) * f.tile_stride;
+        const Quad hj = ldq(tj);
+        const double xi = __dmul_rn(__dsub_rn(gj.R, hj.a), hj.c), eta = __dmul_rn(__dsub_rn(sp.z, hj.b), hj.c);
+        double xp[6], ep[6], T[kDepHarmMax];
+        xp[0] = 1.0; ep[0] = 1.0;
+#pragma unroll
+        for (int p = 1; p < 6; ++p) { xp[p] = __dmul_rn(xp[p - 1], xi); ep[p] = __dmul_rn(ep[p - 1], eta); }
+        T[0] = 1.0;
+#pragma unroll
+        for (int md = 0; md < M3DK_MAX_MODES; ++md)
+            if (md < f.n_modes) mode_phase(f.n_tor[md], gj.cph, gj.sph, 1.0, 0.0, T[1 + 2 * md], T[2 + 2 * md]);
+        unsigned todo = __ballot_sync(0xffffffffu, on);
+        while (todo) {
+            const int ke = __shfl_sync(0xffffffffu, ej, __ffs(todo) - 1);
+            const bool mine = on && ej == ke;
+            double *out = rhs + (size_t)ke * stride_e;
+            for (int mom = 0; mom < 2; ++mom)
+#pragma unroll
+                for (int h = 0; h < kDepHarmMax; ++h) {
+                    if (h >= H) break;
+                    const double ah = mine ? __dmul_rn(__dmul_rn(0.25, d.amp[mom]), T[h]) : 0.0;
+                    double *op = out + ((size_t)mom * H + h) * M3DK_NCOEF;
+                    int k = 0;
+#pragma unroll
+                    for (int jj = 0; jj < 6; ++jj)
+#pragma unroll
+                        for (int ii = 0; ii < 6 - jj; ++ii, ++k) {
+                            double val = __dmul_rn(ah, __dmul_rn(xp[ii], ep[jj]));
+#pragma unroll
+                            for (int sft = 16; sft > 0; sft >>= 1) val += __shfl_xor_sync(0xffffffffu, val, sft);
+                            if (lane == 0) atomicAdd(op + k, val);
+                        }
+                }
+            todo &= ~__ballot_sync(0xffffffffu, mine);
+        }
+    }
+}
+
 // element-ordered records cut into work items (the ordering kernels of m3dk_sort.cu): a warp takes an item (<= 64
 // markers of ONE element), every lane two of them, one reduction and one atomic per table entry and item
 __global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
@@ -162,6 +256,11 @@ cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t
     const size_t bytes = (size_t)c->f.n_elems * 2 * (1 + 2 * c->f.n_modes) * M3DK_NCOEF * sizeof(double);
     cudaError_t e = cudaMemsetAsync(rhs, 0, bytes, c->stream);
     if (e != cudaSuccess || n == 0) return e;
+    if (flags & 2) {   // 4-point FLR deposition: the ring points leave the marker's element, one marker per lane
+        c->kernel_launches += 1;
+        deposit_flr_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->user, n, c->q, c->m, rhs);
+        return cudaGetLastError();
+    }
     if (c->have_sortws) {
         // order the markers by the element of their CURRENT position first (after a push the arrays are in the order of
         // the previous positions): records in element order + work items, then one warp per item

@@ -90,3 +90,21 @@ def test_deposit_with_b1par_term_of_eq16():
         off = p.deposit(flags=0, t=5.7)
         assert np.abs(got[:, 1] - off[:, 1]).max() > 1e-3 * np.abs(off[:, 1]).max()      # the term is there
         assert np.abs(got[:, 0] - off[:, 0]).max() <= 1e-12 * np.abs(off[:, 0]).max()     # parallel moment untouched
+
+
+def test_deposit_flr_four_point():
+    """flags = M3DK_DEPOSIT_FLR (with and without the B1par term): a quarter of every amplitude at each gyro-ring point."""
+    w = _unstructured(two_modes=True)
+    rng = np.random.Generator(np.random.PCG64(10))
+    mk = {k: v.copy() for k, v in w.markers.items()}
+    mk["w"] = rng.normal(size=w.n_markers) * 1e-4
+    mk["mu"] = mk["mu"] * 4.0                                   # rings of a few elements; near the edge some points fall outside
+    p = make_pusher(dataclasses.replace(w, markers=mk), verify=True)
+    mesh, sp = oracle_of(w)
+    for flags in (2, 3):
+        ref, _ = oracle.deposit(mesh, sp, mk, flags=flags, t=2.1)
+        got = p.deposit(flags=flags, t=2.1)
+        S = np.abs(ref).max()
+        assert np.abs(got - ref).max() <= 1e-11 * S, float(np.abs(got - ref).max() / S)
+    plain = p.deposit(flags=0)
+    assert np.abs(got[:, 1, 0, 0] - plain[:, 1, 0, 0]).max() > 1e-3 * np.abs(plain[:, 1, 0, 0]).max()
