@@ -108,17 +108,25 @@ __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ Fi
 // 4-point FLR deposition (flags bit 1): a marker deposits a quarter of its amplitudes at each of its four
 // gyro-ring points (the ring of reading G23, as in the FLR push).  One marker per lane; for each of the four points the lane
 // finds the point's element and the warp loops over its distinct elements exactly as deposit_kernel does.
+// kRec: the markers are read from the element-ordered records of the sort workspace (a warp's 32 markers then share an
+// element and their rings touch a handful of elements), else from the caller's arrays in whatever order they are.
+template <bool kRec>
 __global__ void __launch_bounds__(128) deposit_flr_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
-                                                          MarkerArrays a, long n, double q, double mass,
+                                                          MarkerArrays a, const double *__restrict__ rec,
+                                                          const int *__restrict__ key, long n, double q, double mass,
                                                           double *__restrict__ rhs) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const bool valid = i < n;
-    const int e = valid ? a.elem[i] : -1;
+    int e = -1;
+    if (valid) { e = kRec ? key[i] : a.elem[i]; if (kRec && e >= f.n_elems) e = -1; }
     const bool active = e >= 0;
     const int H = 1 + 2 * f.n_modes;
     Marker s;
-    if (active) {
+    if (active && kRec) {
+        const double *p = rec + (size_t)kRecDoubles * i;
+        s.x = p[0]; s.y = p[1]; s.z = p[2]; s.w = p[3]; s.vx = p[4]; s.vy = p[5]; s.vz = p[6]; s.mu = p[7];
+    } else if (active) {
         s.x = a.x[i]; s.y = a.y[i]; s.z = a.z[i]; s.vx = a.vx[i]; s.vy = a.vy[i]; s.vz = a.vz[i]; s.mu = a.mu[i]; s.w = a.w[i];
     } else {
         s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
@@ -257,8 +265,17 @@ cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t
     cudaError_t e = cudaMemsetAsync(rhs, 0, bytes, c->stream);
     if (e != cudaSuccess || n == 0) return e;
     if (flags & 2) {   // 4-point FLR deposition: the ring points leave the marker's element, one marker per lane
-        c->kernel_launches += 1;
-        deposit_flr_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->user, n, c->q, c->m, rhs);
+        if (c->have_sortws) {
+            e = launch_pack_sorted(c, n);
+            if (e != cudaSuccess) return e;
+            c->kernel_launches += 1;
+            deposit_flr_kernel<true><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->user, c->sb.rec[c->cur],
+                                                                                        c->sb.key, n, c->q, c->m, rhs);
+        } else {
+            c->kernel_launches += 1;
+            deposit_flr_kernel<false><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->user, nullptr, nullptr, n,
+                                                                                         c->q, c->m, rhs);
+        }
         return cudaGetLastError();
     }
     if (c->have_sortws) {

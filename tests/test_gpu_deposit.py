@@ -108,3 +108,20 @@ def test_deposit_flr_four_point():
         assert np.abs(got - ref).max() <= 1e-11 * S, float(np.abs(got - ref).max() / S)
     plain = p.deposit(flags=0)
     assert np.abs(got[:, 1, 0, 0] - plain[:, 1, 0, 0]).max() > 1e-3 * np.abs(plain[:, 1, 0, 0]).max()
+
+
+def test_deposit_without_sort_workspace_uses_the_callers_arrays():
+    """No sort workspace registered: plain and FLR deposition fall back to the any-order kernels; same tables."""
+    import paper_2107_13663_b200 as m3dk
+    w = _unstructured(two_modes=False)
+    rng = np.random.Generator(np.random.PCG64(11))
+    mk = {k: v.copy() for k, v in w.markers.items()}
+    mk["w"] = rng.normal(size=w.n_markers)
+    p = m3dk.Pusher(device=0, verify=True)
+    p.fields_create(w.node_RZ, w.tri, w.eq_coef, w.n_tor, w.omega, w.pert_coef)
+    p.particles_init(mk, w.charge, w.mass, w.f0, with_sort_workspace=False)
+    mesh, sp = oracle_of(w)
+    for flags in (0, 1, 2):
+        ref, _ = oracle.deposit(mesh, sp, mk, flags=flags, t=1.3)
+        got = p.deposit(flags=flags, t=1.3)
+        assert np.abs(got - ref).max() <= 1e-11 * np.abs(ref).max(), flags
