@@ -113,3 +113,19 @@ def test_300_step_parity_on_non_chaotic_orbits(mode):
     wrms = np.sqrt(np.mean(a["w"][keep] ** 2))
     ex, ev, ew = g16_errors(take(got, keep), take(a, keep), w_floor=wrms)
     assert max(ex.max(), ev.max(), ew.max()) <= 1.0e-8, (ex.max(), ev.max(), ew.max(), keep.mean())
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_modes_without_any_perturbation_table(mode):
+    """n_modes = 0 (config 0): both modes reduce to the equilibrium push, w is never written, parity with the oracle."""
+    w = synth.make_config(0, n_markers=2000 + 3, nx=32)
+    mesh, sp = oracle_of(w, mode=mode)
+    ref, e_ref, _ = oracle_push(mesh, sp, w.markers, 5, w.dt)
+    for si in (0, 1):
+        p = make_pusher(w, verify=True, sort_interval=si, mode=mode)
+        p.push(5, w.dt)
+        got, _, _ = p.state()
+        live = e_ref >= 0
+        ex, ev, _ = g16_errors(take(got, live), take(ref, live), w_floor=1.0)
+        assert max(ex.max(), ev.max()) <= 5 * TOL_STEP
+        assert np.array_equal(got["w"], w.markers["w"])
