@@ -283,10 +283,12 @@ cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t
         // the previous positions): records in element order + work items, then one warp per item
         e = launch_pack_sorted(c, n);
         if (e != cudaSuccess) return e;
-        const long max_items = n / kItemMarkers + c->f.n_elems + 2;
-        c->kernel_launches += 1;
+        const long max_items = n / kItemMarkers + c->f.n_elems + 2, max_small = c->f.n_elems + 2;
+        c->kernel_launches += 2;
         deposit_items_kernel<<<(unsigned)((max_items + 3) / 4), 128, 0, c->stream>>>(
             c->f, o, c->sb.rec[c->cur], c->sb.items, c->sb.ioffs + c->f.n_elems + 1, c->m, rhs);
+        deposit_items_kernel<<<(unsigned)((max_small + 3) / 4), 128, 0, c->stream>>>(          // the small items
+            c->f, o, c->sb.rec[c->cur], c->sb.items_small, reinterpret_cast<const int *>(c->sb.scan_state + 1), c->m, rhs);
         return cudaGetLastError();
     }
     c->kernel_launches += 1;

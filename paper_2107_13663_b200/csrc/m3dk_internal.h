@@ -119,7 +119,8 @@ struct SortBuffers {         // carved from the sort workspace
     int *offs;               // [n_elems + 2]
     int *ioffs;              // [n_elems + 2] first work item of each element; ioffs[n_elems + 1] = number of items
     int4 *items;             // [n / kItemMarkers + n_elems + 2]
-    unsigned long long *scan_state;   // ticket + per-chunk totals of the single-pass scan
+    int4 *items_small;       // [n_elems + 2] items of 1..32 markers (one marker per lane); their count is scan_state[1]
+    unsigned long long *scan_state;   // ticket, small-item counter, per-chunk totals of the single-pass scan
     size_t bytes;
 };
 

@@ -477,7 +477,8 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
 // bulk copy per item (double-buffered per warp: the next item's tile travels while this one computes), and every
 // coefficient read is a broadcast LDS that feeds kItemR markers per lane.  Static assignment: the warps of a CTA take
 // consecutive items.  Items of the pseudo-element n_elems hold the lost markers: frozen, they only enter the histogram.
-template <bool kHist, int kMode>
+// kR = 2: the items of up to 64 markers; kR = 1: the small items (a remainder of 1..32 markers of an element).
+template <bool kHist, int kMode, int kR>
 __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_kernel(const __grid_constant__ PushParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int kWarps = kPushThreads / 32;
@@ -502,9 +503,9 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
     int it = blockIdx.x * kWarps + warp;
     int4 w0 = it < total ? __ldg(P.items + it) : none;
     int4 w1 = it + stride < total ? __ldg(P.items + it + stride) : none;
-    int src0[kItemR], src1[kItemR];
+    int src0[kR], src1[kR];
 #pragma unroll
-    for (int r = 0; r < kItemR; ++r) {
+    for (int r = 0; r < kR; ++r) {
         src0[r] = 32 * r + lane < w0.z ? P.rc.order[w0.y + 32 * r + lane].x : 0;
         src1[r] = 32 * r + lane < w1.z ? P.rc.order[w1.y + 32 * r + lane].x : 0;
     }
@@ -516,24 +517,24 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
         __syncwarp();                                  // every lane has finished reading buffer b ^ 1 (previous item)
         if (w1.x < P.f.n_elems && lane == 0)
             tile_copy_issue(buf0 + (b ^ 1) * tile_bytes, P.f.tiles + (size_t)w1.x * stride_d, tile_bytes, bar0 + (b ^ 1) * 8);
-        int src2[kItemR];
+        int src2[kR];
 #pragma unroll
-        for (int r = 0; r < kItemR; ++r) {
+        for (int r = 0; r < kR; ++r) {
             if (32 * r + lane < w1.z) {
                 const double *rp = P.rc.in + (size_t)kRecDoubles * src1[r];
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(rp));
             }
             src2[r] = 32 * r + lane < w2.z ? P.rc.order[w2.y + 32 * r + lane].x : 0;
         }
-        long mi[kItemR], mo[kItemR];
-        bool on[kItemR];
+        long mi[kR], mo[kR];
+        bool on[kR];
 #pragma unroll
-        for (int r = 0; r < kItemR; ++r) { mo[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count; mi[r] = src0[r]; }
+        for (int r = 0; r < kR; ++r) { mo[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count; mi[r] = src0[r]; }
         const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems};
         if (e >= P.f.n_elems) {                        // lost markers: frozen (G12), moved along and counted for the next sort
-            int key[kItemR];
+            int key[kR];
 #pragma unroll
-            for (int r = 0; r < kItemR; ++r) {
+            for (int r = 0; r < kR; ++r) {
                 key[r] = P.f.n_elems;
                 if (on[r]) {
                     double a0, a1, a2, a3, b0, b1, b2, b3;
@@ -543,22 +544,22 @@ __global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_
                 }
             }
             if (kHist) {
-                unsigned peers[kItemR];
-                int base[kItemR];
-                hist_issue<kItemR>(P.hist, key, on, peers, base);
-                rank_finish<kItemR>(P.rank, mo, on, peers, base);
+                unsigned peers[kR];
+                int base[kR];
+                hist_issue<kR>(P.hist, key, on, peers, base);
+                rank_finish<kR>(P.rank, mo, on, peers, base);
             }
         } else {
             mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
             phase ^= 1u << b;
-            if (kMode == 1) step_R_nl<kItemR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
-            else step_R<kItemR, kHist, true, RecIO, kMode == 2>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
+            if (kMode == 1) step_R_nl<kR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
+            else step_R<kR, kHist, true, RecIO, kMode == 2>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
         }
         b ^= 1;
         it += stride;
         w0 = w1; w1 = w2;
 #pragma unroll
-        for (int r = 0; r < kItemR; ++r) { src0[r] = src1[r]; src1[r] = src2[r]; }
+        for (int r = 0; r < kR; ++r) { src0[r] = src1[r]; src1[r] = src2[r]; }
     }
 }
 
@@ -661,12 +662,24 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
         P.items = c->sb.items; P.n_items = c->sb.ioffs + c->f.n_elems + 1;
         const unsigned grid = (unsigned)(c->sm_count * M3DK_PUSH_MINBLOCKS);
         const size_t smem = (size_t)(kPushThreads / 32) * 2 * (c->f.tile_stride * 8 + 8);
-        auto kern = c->mode == 1   ? (with_hist ? push_items_kernel<true, 1> : push_items_kernel<false, 1>)
-                    : c->mode == 2 ? (with_hist ? push_items_kernel<true, 2> : push_items_kernel<false, 2>)
-                                   : (with_hist ? push_items_kernel<true, 0> : push_items_kernel<false, 0>);
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        kern<<<grid, kPushThreads, smem, c->stream>>>(P);
+        // two launches: the items of up to 64 markers (two per lane), then the small items (one per lane)
+        for (int small = 0; small < 2; ++small) {
+            P.items = small ? c->sb.items_small : c->sb.items;
+            P.n_items = small ? reinterpret_cast<const int *>(c->sb.scan_state + 1) : c->sb.ioffs + c->f.n_elems + 1;
+            void (*kern)(PushParams);
+            if (small)
+                kern = c->mode == 1   ? (with_hist ? push_items_kernel<true, 1, 1> : push_items_kernel<false, 1, 1>)
+                       : c->mode == 2 ? (with_hist ? push_items_kernel<true, 2, 1> : push_items_kernel<false, 2, 1>)
+                                      : (with_hist ? push_items_kernel<true, 0, 1> : push_items_kernel<false, 0, 1>);
+            else
+                kern = c->mode == 1   ? (with_hist ? push_items_kernel<true, 1, 2> : push_items_kernel<false, 1, 2>)
+                       : c->mode == 2 ? (with_hist ? push_items_kernel<true, 2, 2> : push_items_kernel<false, 2, 2>)
+                                      : (with_hist ? push_items_kernel<true, 0, 2> : push_items_kernel<false, 0, 2>);
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            if (small) c->kernel_launches += 1;
+            kern<<<grid, kPushThreads, smem, c->stream>>>(P);
+        }
         c->cur ^= 1;
     } else {
         P.rc.out = c->sb.rec[c->cur];

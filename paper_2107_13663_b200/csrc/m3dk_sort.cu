@@ -15,7 +15,8 @@ size_t sort_workspace_bytes(long n, int n_elems) {
     const size_t ni = up256((size_t)n * sizeof(int)), nh = up256((size_t)(n_elems + 2) * sizeof(int));
     const size_t nit = up256(((size_t)n / kItemMarkers + n_elems + 2) * sizeof(int4));
     const size_t nst = up256(((size_t)(n_elems + 1) / 4096 + 4) * sizeof(unsigned long long));
-    return 2 * nr + 2 * no + 2 * ni + 3 * nh + nit + nst;
+    const size_t nsm = up256((size_t)(n_elems + 2) * sizeof(int4));
+    return 2 * nr + 2 * no + 2 * ni + 3 * nh + nit + nst + nsm;
 }
 
 void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb) {
@@ -31,6 +32,7 @@ void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb) {
     sb->ioffs = reinterpret_cast<int *>(p); p += nh;
     sb->items = reinterpret_cast<int4 *>(p); p += up256(((size_t)n / kItemMarkers + n_elems + 2) * sizeof(int4));
     sb->scan_state = reinterpret_cast<unsigned long long *>(p); p += up256(((size_t)(n_elems + 1) / 4096 + 4) * sizeof(unsigned long long));
+    sb->items_small = reinterpret_cast<int4 *>(p); p += up256((size_t)(n_elems + 2) * sizeof(int4));
     sb->bytes = (size_t)(p - static_cast<char *>(ws));
 }
 
@@ -57,6 +59,11 @@ __global__ void __launch_bounds__(256) hist_rank_kernel(const int *__restrict__ 
 // so they are running: no deadlock) while it scans its own bins.  state[0] = ticket counter, state[2 + c] = totals of
 // chunk c with a ready tag in the upper bits; the launcher clears the state (a few hundred bytes) before each launch.
 // word = tag << 56 | items << 31 | markers   (markers < 2^31, items < 2^25)
+// Cut of an element's run of c markers: full items of kItemMarkers, a remainder of more than 32 markers is one more item
+// of the same kind (both slots of a lane in use), a remainder of 1..32 markers becomes a SMALL item (one marker per lane),
+// pushed by the one-slot instance of the kernel: no arithmetic is issued for an empty second slot.
+__host__ __device__ inline int n_big_items(int c) { return c / kItemMarkers + ((c % kItemMarkers) > 32 ? 1 : 0); }
+
 constexpr int kScanChunk = 4096;
 __global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist, int m, int *__restrict__ offs,
                                                     int *__restrict__ ioffs, unsigned long long *state,
@@ -75,7 +82,7 @@ __global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
         v[q] = k + q < m ? hist[k + q] : 0;
-        it[q] = (v[q] + kItemMarkers - 1) / kItemMarkers;
+        it[q] = n_big_items(v[q]);
     }
     const int2 mine = make_int2(v[0] + v[1] + v[2] + v[3], it[0] + it[1] + it[2] + it[3]);
     int2 inc = mine;
@@ -126,15 +133,18 @@ __global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist
     if (chunk == nchunks - 1 && t == 1023) { offs[m] = carry.x + wsum[31].x; ioffs[m] = carry.y + wsum[31].y; }
 }
 
-// work items of the element-ordered push: element k's sorted segment [offs[k], offs[k+1]) cut into pieces of at most
-// kItemMarkers markers; k = n_elems is the pseudo-element of the lost markers
+// work items of the element-ordered push: element k's sorted segment [offs[k], offs[k+1]) cut as n_big_items() says;
+// k = n_elems is the pseudo-element of the lost markers.  Small items are appended to their own list through a counter
+// (their order does not matter: every item is independent).
 __global__ void __launch_bounds__(256) items_kernel(const int *__restrict__ offs, const int *__restrict__ ioffs, int m,
-                                                    int4 *__restrict__ items) {
+                                                    int4 *__restrict__ items, int4 *__restrict__ items_small,
+                                                    int *__restrict__ n_small) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= m) return;
     const int b = offs[k], cnt = offs[k + 1] - b;
-    int j = ioffs[k];
-    for (int c = 0; c < cnt; c += kItemMarkers, ++j) items[j] = make_int4(k, b + c, min(kItemMarkers, cnt - c), 0);
+    int j = ioffs[k], c = 0;
+    for (; cnt - c > 32; c += kItemMarkers, ++j) items[j] = make_int4(k, b + c, min(kItemMarkers, cnt - c), 0);
+    if (cnt - c > 0) items_small[atomicAdd(n_small, 1)] = make_int4(k, b + c, cnt - c, 0);
 }
 
 __device__ __forceinline__ void st256(double *p, double a, double b, double c, double d) {
@@ -193,7 +203,8 @@ static cudaError_t scan_and_cut(m3dk_ctx *c) {
     cudaError_t e = cudaMemsetAsync(c->sb.scan_state, 0, (size_t)(nchunks + 2) * sizeof(unsigned long long), c->stream);
     if (e != cudaSuccess) return e;
     scan_kernel<<<nchunks, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs, c->sb.ioffs, c->sb.scan_state, 1u);
-    items_kernel<<<(m + 255) / 256, 256, 0, c->stream>>>(c->sb.offs, c->sb.ioffs, m, c->sb.items);
+    items_kernel<<<(m + 255) / 256, 256, 0, c->stream>>>(c->sb.offs, c->sb.ioffs, m, c->sb.items, c->sb.items_small,
+                                                        reinterpret_cast<int *>(c->sb.scan_state + 1));
     return cudaGetLastError();
 }
 
