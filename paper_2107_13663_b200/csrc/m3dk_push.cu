@@ -479,7 +479,7 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
 // consecutive items.  Items of the pseudo-element n_elems hold the lost markers: frozen, they only enter the histogram.
 // kR = 2: the items of up to 64 markers; kR = 1: the small items (a remainder of 1..32 markers of an element).
 template <bool kHist, int kMode, int kR>
-__global__ void __launch_bounds__(kPushThreads, M3DK_PUSH_MINBLOCKS) push_items_kernel(const __grid_constant__ PushParams P) {
+__global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 1 : M3DK_PUSH_MINBLOCKS) push_items_kernel(const __grid_constant__ PushParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int kWarps = kPushThreads / 32;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -678,7 +678,7 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
             if (small) c->kernel_launches += 1;
-            kern<<<grid, kPushThreads, smem, c->stream>>>(P);
+            kern<<<small ? grid / M3DK_PUSH_MINBLOCKS * (M3DK_PUSH_MINBLOCKS + 1) : grid, kPushThreads, smem, c->stream>>>(P);
         }
         c->cur ^= 1;
     } else {
