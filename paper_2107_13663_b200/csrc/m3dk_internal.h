@@ -102,6 +102,7 @@ struct PushParams {
     int *hist, *rank;        // fused sort histogram of the new keys (kHist kernels), else unused
     const int4 *items;       // work items of the element-ordered kernel: (element, first slot, count, -)
     const int *n_items;      // device: number of items
+    int *ticket;             // device: next unassigned item beyond the first three rounds (cleared by the cut)
 };
 
 #ifndef M3DK_ITEM_R
@@ -120,7 +121,8 @@ struct SortBuffers {         // carved from the sort workspace
     int *ioffs;              // [n_elems + 2] first work item of each element; ioffs[n_elems + 1] = number of items
     int4 *items;             // [n / kItemMarkers + n_elems + 2]
     int4 *items_small;       // [n_elems + 2] items of 1..32 markers (one marker per lane); their count is scan_state[1]
-    unsigned long long *scan_state;   // ticket, small-item counter, per-chunk totals of the single-pass scan
+    unsigned long long *scan_state;   // ticket, small-item counter, per-chunk totals of the single-pass scan, then
+                                      // one word holding the two item tickets of the push kernels (big, small)
     size_t bytes;
 };
 

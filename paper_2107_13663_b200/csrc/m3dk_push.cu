@@ -500,9 +500,11 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
     //   and at the start of an item the NEXT item's records are prefetched into L2 and its tile copy is issued,
     // so that an item starts with its tile in shared memory and its records one L2 hit away.
     const int4 none = make_int4(P.f.n_elems, 0, 0, 0);
-    int it = blockIdx.x * kWarps + warp;
+    // The first three items of a warp are fixed (items it, it + stride, it + 2 stride); every further one is drawn from a
+    // ticket counter one item ahead of its descriptor read, so that no warp idles while another still has a queue.
+    int it = blockIdx.x * kWarps + warp, it1 = it + stride, it2 = it + 2 * stride;
     int4 w0 = it < total ? __ldg(P.items + it) : none;
-    int4 w1 = it + stride < total ? __ldg(P.items + it + stride) : none;
+    int4 w1 = it1 < total ? __ldg(P.items + it1) : none;
     int src0[kR], src1[kR];
 #pragma unroll
     for (int r = 0; r < kR; ++r) {
@@ -513,7 +515,9 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
     if (w0.x < P.f.n_elems && lane == 0) tile_copy_issue(buf0, P.f.tiles + (size_t)w0.x * stride_d, tile_bytes, bar0);
     while (it < total) {
         const int e = w0.x, start = w0.y, count = w0.z;   // (element, first slot, count, -)
-        const int4 w2 = it + 2 * stride < total ? __ldg(P.items + it + 2 * stride) : none;
+        const int4 w2 = it2 < total ? __ldg(P.items + it2) : none;
+        int ticket = 0;
+        if (lane == 0) ticket = atomicAdd(P.ticket, 1);
         __syncwarp();                                  // every lane has finished reading buffer b ^ 1 (previous item)
         if (w1.x < P.f.n_elems && lane == 0)
             tile_copy_issue(buf0 + (b ^ 1) * tile_bytes, P.f.tiles + (size_t)w1.x * stride_d, tile_bytes, bar0 + (b ^ 1) * 8);
@@ -556,7 +560,7 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
             else step_R<kR, kHist, true, RecIO, kMode == 2>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
         }
         b ^= 1;
-        it += stride;
+        it = it1; it1 = it2; it2 = 3 * stride + __shfl_sync(0xffffffffu, ticket, 0);
         w0 = w1; w1 = w2;
 #pragma unroll
         for (int r = 0; r < kR; ++r) { src0[r] = src1[r]; src1[r] = src2[r]; }
@@ -666,6 +670,7 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
         for (int small = 0; small < 2; ++small) {
             P.items = small ? c->sb.items_small : c->sb.items;
             P.n_items = small ? reinterpret_cast<const int *>(c->sb.scan_state + 1) : c->sb.ioffs + c->f.n_elems + 1;
+            P.ticket = reinterpret_cast<int *>(c->sb.scan_state + (c->f.n_elems + 1 + 4095) / 4096 + 2) + small;
             void (*kern)(PushParams);
             if (small)
                 kern = c->mode == 1   ? (with_hist ? push_items_kernel<true, 1, 1> : push_items_kernel<false, 1, 1>)

@@ -14,7 +14,7 @@ size_t sort_workspace_bytes(long n, int n_elems) {
     const size_t nr = up256((size_t)n * kRecDoubles * sizeof(double)), no = up256((size_t)n * sizeof(int2));
     const size_t ni = up256((size_t)n * sizeof(int)), nh = up256((size_t)(n_elems + 2) * sizeof(int));
     const size_t nit = up256(((size_t)n / kItemMarkers + n_elems + 2) * sizeof(int4));
-    const size_t nst = up256(((size_t)(n_elems + 1) / 4096 + 4) * sizeof(unsigned long long));
+    const size_t nst = up256(((size_t)(n_elems + 1) / 4096 + 6) * sizeof(unsigned long long));
     const size_t nsm = up256((size_t)(n_elems + 2) * sizeof(int4));
     return 2 * nr + 2 * no + 2 * ni + 3 * nh + nit + nst + nsm;
 }
@@ -31,7 +31,7 @@ void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb) {
     sb->offs = reinterpret_cast<int *>(p); p += nh;
     sb->ioffs = reinterpret_cast<int *>(p); p += nh;
     sb->items = reinterpret_cast<int4 *>(p); p += up256(((size_t)n / kItemMarkers + n_elems + 2) * sizeof(int4));
-    sb->scan_state = reinterpret_cast<unsigned long long *>(p); p += up256(((size_t)(n_elems + 1) / 4096 + 4) * sizeof(unsigned long long));
+    sb->scan_state = reinterpret_cast<unsigned long long *>(p); p += up256(((size_t)(n_elems + 1) / 4096 + 6) * sizeof(unsigned long long));
     sb->items_small = reinterpret_cast<int4 *>(p); p += up256((size_t)(n_elems + 2) * sizeof(int4));
     sb->bytes = (size_t)(p - static_cast<char *>(ws));
 }
@@ -200,7 +200,7 @@ static cudaError_t scan_and_cut(m3dk_ctx *c) {
     c->kernel_launches += 2;
     const int nchunks = (m + kScanChunk - 1) / kScanChunk;
     // ticket and per-chunk words cleared together (a few hundred bytes): a word is ready when its tag is set
-    cudaError_t e = cudaMemsetAsync(c->sb.scan_state, 0, (size_t)(nchunks + 2) * sizeof(unsigned long long), c->stream);
+    cudaError_t e = cudaMemsetAsync(c->sb.scan_state, 0, (size_t)(nchunks + 3) * sizeof(unsigned long long), c->stream);
     if (e != cudaSuccess) return e;
     scan_kernel<<<nchunks, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs, c->sb.ioffs, c->sb.scan_state, 1u);
     items_kernel<<<(m + 255) / 256, 256, 0, c->stream>>>(c->sb.offs, c->sb.ioffs, m, c->sb.items, c->sb.items_small,
