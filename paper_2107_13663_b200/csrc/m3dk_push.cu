@@ -475,8 +475,8 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
 // A work item is up to kItemMarkers = 32 kItemR consecutive markers of ONE element; a warp takes an item, every lane up to
 // kItemR of its markers (slots lane, lane + 32, ...).  The element's coefficient tile is staged in shared memory by one
 // bulk copy per item (double-buffered per warp: the next item's tile travels while this one computes), and every
-// coefficient read is a broadcast LDS that feeds kItemR markers per lane.  Static assignment: the warps of a CTA take
-// consecutive items.  Items of the pseudo-element n_elems hold the lost markers: frozen, they only enter the histogram.
+// coefficient read is a broadcast LDS that feeds kItemR markers per lane.  Items are handed out by a ticket counter after
+// a warp's first three.  Items of the pseudo-element n_elems hold the lost markers: frozen, they only enter the histogram.
 // kR = 2: the items of up to 64 markers; kR = 1: the small items (a remainder of 1..32 markers of an element).
 template <bool kHist, int kMode, int kR>
 __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 1 : M3DK_PUSH_MINBLOCKS) push_items_kernel(const __grid_constant__ PushParams P) {
@@ -495,7 +495,7 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
     __syncwarp();
     const int total = *P.n_items;
     const int stride = gridDim.x * kWarps;
-    // Software pipeline over this warp's items (static assignment: the warps of a CTA take consecutive items):
+    // Software pipeline over this warp's items:
     //   item descriptors are read two items ahead, the order entries (which record goes to which slot) one item ahead,
     //   and at the start of an item the NEXT item's records are prefetched into L2 and its tile copy is issued,
     // so that an item starts with its tile in shared memory and its records one L2 hit away.
