@@ -41,41 +41,76 @@ def build(force: bool = False) -> str:
     return _SO
 
 
+def _configure(L):
+    """Declare the argument / result types of every exported oracle function on the loaded library L."""
+    L.orc_mesh_create.restype = C.c_void_p
+    L.orc_mesh_create.argtypes = [C.c_int, c_dp, C.c_int, c_ip, c_dp, C.c_int, c_ip, c_dp, c_dp]
+    L.orc_mesh_free.argtypes = [C.c_void_p]
+    L.orc_locate.argtypes = [C.c_void_p, C.c_long, c_dp, c_dp, c_ip, C.c_int]
+    L.orc_eval_fe.argtypes = [C.c_void_p, C.c_long, c_dp, c_dp, c_dp, C.c_double, c_ip, c_dp]
+    L.orc_eval_analytic.argtypes = [C.POINTER(Analytic), C.c_long, c_dp, c_dp, c_dp, C.c_double, c_dp, c_dp]
+    L.orc_push_fe.restype = C.c_long
+    L.orc_push_fe.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_ip, C.c_int, C.c_double,
+                              C.c_double, C.c_long, C.c_int, C.c_int]
+    L.orc_push_analytic.restype = C.c_long
+    L.orc_push_analytic.argtypes = [C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 8 + [
+        C.c_int, C.c_double, C.c_double, C.c_long, C.c_int]
+    L.orc_gyro_ring.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_double, c_dp]
+    L.orc_flr_fields.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_double, C.c_double, c_dp]
+    L.orc_gc_push.restype = C.c_long
+    L.orc_gc_push.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5 + [c_ip, C.c_int,
+                              C.c_double, C.c_int]
+    L.orc_gc_rhs.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5
+    L.orc_gc_fields.argtypes = [C.c_void_p, C.POINTER(Analytic), C.c_long, c_dp, c_dp, c_ip, c_dp]
+    L.orc_deposit.restype = C.c_long
+    L.orc_deposit.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_dp, C.c_int, C.c_double]
+    L.orc_trace.restype = C.c_long
+    L.orc_trace.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_long, C.c_double,
+                            C.c_double, C.c_long, c_dp]
+    L.orc_push_uniform.argtypes = [C.c_long] + [c_dp] * 6 + [c_dp, c_dp, C.c_double, C.c_double, C.c_long, C.c_double]
+    L.orc_eq6.argtypes = [c_dp, c_dp, c_dp, C.c_double, c_dp]
+    L.orc_weight_rhs.restype = C.c_double
+    L.orc_weight_rhs.argtypes = [c_dp, C.POINTER(Species), C.c_double, c_dp, C.c_double]
+    L.orc_sort_perm.argtypes = [C.c_long, c_ip, C.c_int, c_lp]
+    L.orc_max_threads.restype = C.c_int
+    return L
+
+
 def lib():
     global _lib
     if _lib is None:
-        L = C.CDLL(build())
-        L.orc_mesh_create.restype = C.c_void_p
-        L.orc_mesh_create.argtypes = [C.c_int, c_dp, C.c_int, c_ip, c_dp, C.c_int, c_ip, c_dp, c_dp]
-        L.orc_mesh_free.argtypes = [C.c_void_p]
-        L.orc_locate.argtypes = [C.c_void_p, C.c_long, c_dp, c_dp, c_ip, C.c_int]
-        L.orc_eval_fe.argtypes = [C.c_void_p, C.c_long, c_dp, c_dp, c_dp, C.c_double, c_ip, c_dp]
-        L.orc_eval_analytic.argtypes = [C.POINTER(Analytic), C.c_long, c_dp, c_dp, c_dp, C.c_double, c_dp, c_dp]
-        L.orc_push_fe.restype = C.c_long
-        L.orc_push_fe.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_ip, C.c_int, C.c_double,
-                                  C.c_double, C.c_long, C.c_int, C.c_int]
-        L.orc_push_analytic.restype = C.c_long
-        L.orc_push_analytic.argtypes = [C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 8 + [
-            C.c_int, C.c_double, C.c_double, C.c_long, C.c_int]
-        L.orc_gyro_ring.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_double, c_dp]
-        L.orc_flr_fields.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_double, C.c_double, c_dp]
-        L.orc_gc_push.restype = C.c_long
-        L.orc_gc_push.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5 + [c_ip, C.c_int,
-                                  C.c_double, C.c_int]
-        L.orc_gc_rhs.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5
-        L.orc_deposit.restype = C.c_long
-        L.orc_deposit.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_dp, C.c_int, C.c_double]
-        L.orc_trace.restype = C.c_long
-        L.orc_trace.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_long, C.c_double,
-                                C.c_double, C.c_long, c_dp]
-        L.orc_push_uniform.argtypes = [C.c_long] + [c_dp] * 6 + [c_dp, c_dp, C.c_double, C.c_double, C.c_long, C.c_double]
-        L.orc_eq6.argtypes = [c_dp, c_dp, c_dp, C.c_double, c_dp]
-        L.orc_weight_rhs.restype = C.c_double
-        L.orc_weight_rhs.argtypes = [c_dp, C.POINTER(Species), C.c_double, c_dp, C.c_double]
-        L.orc_sort_perm.argtypes = [C.c_long, c_ip, C.c_int, c_lp]
-        L.orc_max_threads.restype = C.c_int
-        _lib = L
+        _lib = _configure(C.CDLL(build()))
     return _lib
+
+
+class variant:
+    """Context manager for the mutation checks of the pins (tests/test_oracle_mutants.py): compile a COPY of the oracle
+    source with one textual substitution into ``workdir`` and route every call of this module to it while the block runs.
+    The oracle itself is never edited; a substitution that does not apply exactly once is an error."""
+
+    def __init__(self, old: str, new: str, workdir: str, tag: str):
+        with open(_SRC) as fh:
+            src = fh.read()
+        if src.count(old) != 1:
+            raise ValueError(f"mutation {tag!r}: pattern occurs {src.count(old)} times in the oracle source, expected 1")
+        c_path = os.path.join(workdir, f"m3dk_oracle_{tag}.c")
+        self.so = os.path.join(workdir, f"libm3dk_oracle_{tag}.so")
+        with open(c_path, "w") as fh:
+            fh.write(src.replace(old, new))
+        subprocess.run(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-o", self.so, c_path, "-lm"],
+                       check=True)
+
+    def __enter__(self):
+        global _lib
+        lib()
+        self._saved = _lib
+        _lib = _configure(C.CDLL(self.so))
+        return self
+
+    def __exit__(self, *exc):
+        global _lib
+        _lib = self._saved
+        return False
 
 
 def _d(a):
@@ -217,6 +252,20 @@ def gc_rhs(sp: Species, R, Z, vpar, mu, *, mesh=None, an=None):
                      R.ctypes.data_as(c_dp), Z.ctypes.data_as(c_dp), vpar.ctypes.data_as(c_dp), mu.ctypes.data_as(c_dp),
                      out.ctypes.data_as(c_dp))
     return out
+
+
+def gc_fields(R, Z, *, mesh=None, an=None):
+    """The field values the guiding-centre right-hand side works from: (elem, out[n][11]) with columns GC_FIELD_COLS."""
+    R, Z = (np.ascontiguousarray(a, dtype=np.float64) for a in (R, Z))
+    n = R.shape[0]
+    elem = np.empty(n, dtype=np.int32)
+    out = np.full((n, 11), np.nan)
+    lib().orc_gc_fields(mesh.h if mesh is not None else None, C.byref(an) if an is not None else None, n,
+                        R.ctypes.data_as(c_dp), Z.ctypes.data_as(c_dp), elem.ctypes.data_as(c_ip), out.ctypes.data_as(c_dp))
+    return elem, out
+
+
+GC_FIELD_COLS = ("psi_R", "psi_Z", "psi_RR", "psi_RZ", "psi_ZZ", "F", "F_R", "F_Z", "Bm", "Bm_R", "Bm_Z")
 
 
 def gyro_ring(sp: Species, X, mu: float, *, mesh=None, an=None):

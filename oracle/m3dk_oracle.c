@@ -36,8 +36,10 @@
  *
  * orc_deposit: right-hand sides of Eqs. (17)-(18) with a delta-function shape (readings G10, G22).
  *
- * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1-P15 of SURVEY.md 8(c), P16-P19 for mode 1, D1-D4 for the
- * deposition; see DESIGN.md section 4.
+ * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1-P15 of SURVEY.md 8(c), P16-P19 for mode 1, M1-M3 for the
+ * magnetic terms of Eqs. (11)-(13), N1 for the total fields of the mode-1 push, Q1-Q2 for poly_eval2 and the finite-element
+ * branch of gc_fields, F1-F4 (FLR), G1-G5 (guiding centre), D1-D6 (deposition); mutation checks of M1-M3, N1, Q1, Q2, G5 in
+ * tests/test_oracle_mutants.py (they compile mutated COPIES of this file); see DESIGN.md section 4.
  * Unpinned by the paper (fixed by DESIGN.md readings, parity unpinned): the kappa_E model (G7),
  * the construction of the synthetic perturbations (G19), rho* (G17).
  */
@@ -840,6 +842,21 @@ long orc_gc_push(const orc_mesh *m, const orc_analytic *a, const orc_species *sp
         if (elem) elem[i] = e;
     }
     return lost;
+}
+
+/* the field values gc_rhs works from, at given points, for the pins of poly_eval2 and of the finite-element branch of
+ * gc_fields: out[n][11] = psi_R psi_Z psi_RR psi_RZ psi_ZZ F F_R F_Z Bm Bm_R Bm_Z; elem[i] = -1: row untouched          */
+void orc_gc_fields(const orc_mesh *m, const orc_analytic *a, long n, const double *R, const double *Z, int *elem, double *out)
+{
+    provider pv = {m ? 0 : 1, m, a, 0};
+    for (long i = 0; i < n; ++i) {
+        orc_gcf g;
+        elem[i] = gc_fields(&pv, R[i], Z[i], &g);
+        if (elem[i] < 0) continue;
+        double *o = out + 11 * i;
+        o[0] = g.psi_R; o[1] = g.psi_Z; o[2] = g.psi_RR; o[3] = g.psi_RZ; o[4] = g.psi_ZZ;
+        o[5] = g.F; o[6] = g.F_R; o[7] = g.F_Z; o[8] = g.Bm; o[9] = g.Bm_R; o[10] = g.Bm_Z;
+    }
 }
 
 /* right-hand side at given points, for the pins: out[n][4] = dX/dt (R, phi, Z components), dv_par/dt */

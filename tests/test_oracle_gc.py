@@ -123,3 +123,46 @@ def test_g4_guiding_centre_orbit_lies_on_the_slow_manifold_orbit(orc):
     rg, thg = np.array(rg), np.unwrap(np.array(thg))
     assert abs((rg.max() - rg.min()) - (rb.max() - rb.min())) < 0.1 * (rb.max() - rb.min()) + 2e-3
     assert abs(thg[-1] - thb[-1]) < 0.05 * abs(thb[-1])
+
+
+def check_g5_phase_space_volume(orc):
+    """Liouville's theorem of Eqs. (1)-(4) (the B*par of Eq. 4 is the phase-space Jacobian):
+        (1/R) d(R B*par dR/dt)/dR + d(B*par dZ/dt)/dZ + d(B*par dv_par/dt)/dv_par = 0      (axisymmetric).
+    B*par = |B| + (m v_par/q) b . curl b is computed HERE from the analytic equilibrium (curl b by central differences of
+    b), the divergence by central differences of the oracle's right-hand side.  The conservation pins G1 cannot see B*par
+    (it divides both equations alike, and (curl b)_phi enters nothing else); this one fails when any component of curl b or
+    the form of B*par in the oracle is wrong."""
+    an = orc.analytic_of(EQ)
+    sp = orc.species(CHARGE, MASS)
+    rng = np.random.Generator(np.random.PCG64(11))
+    n = 120
+    R, Z = rng.uniform(2.4, 3.6, n), rng.uniform(-0.5, 0.5, n)
+    vpar, mu = rng.uniform(-1.0, 1.0, n), rng.uniform(0.001, 0.01, n)
+    h = 2e-4
+
+    def bhat(r, z):
+        B = np.array(EQ.B_cyl(r, z))
+        return B / np.sqrt((B ** 2).sum(axis=0))
+
+    def Bspar(r, z, vp):
+        b = bhat(r, z)
+        dbR, dbZ = (bhat(r + h, z) - bhat(r - h, z)) / (2 * h), (bhat(r, z + h) - bhat(r, z - h)) / (2 * h)
+        curl = np.array([-dbZ[1], dbZ[0] - dbR[2], b[1] / r + dbR[1]])       # axisymmetric curl in (R, phi, Z)
+        Bm = np.sqrt(sum(c ** 2 for c in EQ.B_cyl(r, z)))
+        return Bm + (MASS * vp / CHARGE) * (b * curl).sum(axis=0)
+
+    def flux(r, z, vp):
+        o = orc.gc_rhs(sp, r, z, vp, mu, an=an)
+        J = Bspar(r, z, vp)
+        return r * J * o[:, 0], J * o[:, 2], J * o[:, 3]
+    d = 1e-3
+    fR = (flux(R + d, Z, vpar)[0] - flux(R - d, Z, vpar)[0]) / (2 * d) / R
+    fZ = (flux(R, Z + d, vpar)[1] - flux(R, Z - d, vpar)[1]) / (2 * d)
+    fv = (flux(R, Z, vpar + d)[2] - flux(R, Z, vpar - d)[2]) / (2 * d)
+    div = fR + fZ + fv
+    scale = np.abs(fR) + np.abs(fZ) + np.abs(fv)
+    assert (np.abs(div) / scale).max() < 2e-5, (np.abs(div) / scale).max()
+
+
+def test_g5_phase_space_volume(orc):
+    check_g5_phase_space_volume(orc)

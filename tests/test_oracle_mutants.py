@@ -1,0 +1,51 @@
+"""Mutation checks of the pins M1-M3, N1, Q1, Q2 (tests/test_oracle_magnetic.py) and G5 (tests/test_oracle_gc.py).
+
+Each case compiles a COPY of oracle/m3dk_oracle.c with one plausible mistake (a flipped sign, a dropped factor, a wrong
+index) into a temporary directory, routes the oracle binding to that copy and asserts that the named pin FAILS -- the
+evidence that the pin would catch that mistake.  The oracle itself is never modified (oracle.variant).  CPU only.
+"""
+import pytest
+
+from test_oracle_gc import check_g5_phase_space_volume
+from test_oracle_magnetic import CHECKS as _MAGNETIC
+
+CHECKS = dict(_MAGNETIC, g5=check_g5_phase_space_volume)
+
+#        pin   tag                      text in the oracle source                         mutated text
+MUTANTS = [
+    ("m1", "eq12_sign", "+ vpar * B1[k] / B0n;", "- vpar * B1[k] / B0n;"),
+    ("m1", "eq12_factor", "+ vpar * B1[k] / B0n;", "+ vpar * B1[k] / (B0n * B0n);"),
+    ("m1", "eq12_dropped", "+ vpar * B1[k] / B0n;", ";"),
+    ("m2", "eq13_sign", "- mu * (b0[0] * f->gB1p[0] + b0[1] * f->gB1p[1] + b0[2] * f->gB1p[2]);",
+     "+ mu * (b0[0] * f->gB1p[0] + b0[1] * f->gB1p[1] + b0[2] * f->gB1p[2]);"),
+    ("m2", "eq13_component", "- mu * (b0[0] * f->gB1p[0] + b0[1] * f->gB1p[1] + b0[2] * f->gB1p[2]);",
+     "- mu * (b0[0] * f->gB1p[0] + b0[2] * f->gB1p[1] + b0[1] * f->gB1p[2]);"),
+    ("m2", "eq10_factor", "+ Fpar * f->F / B0n;", "+ Fpar * f->F / (B0n * R);"),
+    ("m2", "dphi_sign", "f->gB1p[1] += -n * qd / R;", "f->gB1p[1] += n * qd / R;"),
+    ("m3", "eq11_sign", "+ mu * f->dtB1p;", "- mu * f->dtB1p;"),
+    ("m3", "eq11_dropped", "+ mu * f->dtB1p;", ";"),
+    ("m3", "dt_sign", "f->dtB1p += om * qd;", "f->dtB1p += -om * qd;"),
+    ("n1", "B1R_sign", "BR += f.B1[0];", "BR -= f.B1[0];"),
+    ("n1", "B1phi_dropped", "BP += f.B1[1];", ""),
+    ("n1", "B1Z_sign", "BZ += f.B1[2];", "BZ -= f.B1[2];"),
+    ("n1", "gradB1par_R_sign", "(f.Bm_R + f.gB1p[0])", "(f.Bm_R - f.gB1p[0])"),
+    ("n1", "gradB1par_phi_sign", "EP = f.E1[1] - (mu / q) * f.gB1p[1];", "EP = f.E1[1] + (mu / q) * f.gB1p[1];"),
+    ("n1", "gradB1par_Z_dropped", "(f.Bm_Z + f.gB1p[2])", "(f.Bm_Z)"),
+    ("q1", "dxe_factor", "(double)(i * j) *", "(double)(i + j) *"),
+    ("q1", "dxx_index", "(xp[i - 2] * ep[j])", "(xp[i - 1] * ep[j])"),
+    ("q1", "psi_RZ_scale", "g->psi_RZ = b * s * s;", "g->psi_RZ = b * s;"),
+    ("q2", "curlb_R_sign", "double curlb[3] = {-bP_Z,", "double curlb[3] = {bP_Z,"),
+    ("q2", "curlb_Z_term", "b[1] / R + bP_R};", "bP_R};"),
+    ("g5", "curlb_phi_sign", "double curlb[3] = {-bP_Z, bR_Z - bZ_R,", "double curlb[3] = {-bP_Z, bZ_R - bR_Z,"),
+    ("g5", "Bstar_par", "Bspar += Bs[k] * b[k]; }", "Bspar += B[k] * b[k]; }"),
+    ("q1", "psi_ZZ_dropped", "g->psi_ZZ = d * s * s;", "g->psi_ZZ = 0.0 * d;"),
+]
+
+
+@pytest.mark.parametrize("pin,tag,old,new", MUTANTS, ids=[f"{m[0]}-{m[1]}" for m in MUTANTS])
+def test_pin_fails_on_mutated_oracle(orc, tmp_path, pin, tag, old, new):
+    CHECKS[pin](orc)                                   # green on the oracle as it stands
+    with orc.variant(old, new, str(tmp_path), tag):
+        with pytest.raises(AssertionError):
+            CHECKS[pin](orc)
+    CHECKS[pin](orc)                                   # and the binding is back on the real oracle
