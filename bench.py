@@ -218,6 +218,7 @@ def run_ours(args, rank, world, local_rank):
                     w.pert_coef if w.n_modes else None)
     p.particles_init(w.markers, w.charge, w.mass, w.f0)
     p.set_options(sort_interval=si, mode=args.mode, t0=0.0)
+    p.set_push_variant(args.push_variant)
 
     def barrier():
         if world > 1:
@@ -393,6 +394,8 @@ def main():
     ap.add_argument("--gc", action="store_true", help="also time m3dk_gc_push (SURVEY.md 8(f)-3) on the final state")
     ap.add_argument("--deposit", action="store_true", help="also time m3dk_deposit (SURVEY.md 8(f)-4) on the final state")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--push-variant", type=int, default=0, choices=[0, 1],
+                    help="m3dk_set_push_variant: 0 = default kernel, 1 = asynchronously staged kernel (A/B comparison)")
     ap.add_argument("--sweep", action="store_true", help="configs[4] sweep: one JSON line per (n, dt, sort interval)")
     ap.add_argument("--sweep-n", type=int, nargs="+", default=[1 << 20, 1 << 22, 1 << 24, 1 << 26])
     ap.add_argument("--sweep-dt", type=float, nargs="+", default=[1.0, 4.0, 16.0])

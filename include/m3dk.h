@@ -126,6 +126,14 @@ int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, double *z, 
  * t0: time of the next step's x_l.  Resets steps_done to 0.                                                          */
 int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, double t0);
 
+/* Which kernel runs the element-ordered steps (sort_interval >= 1) of modes 0 and 1.  Results are bit-identical.
+ *   0 (default)  push_items_kernel: a warp per work item, tile staged by a bulk copy, records gathered with 256-bit loads,
+ *                search + histogram with returned ranks at the end of the item;
+ *   1            push_async_kernel: the same decomposition with every L2 / HBM access of an item requested one item ahead
+ *                (cp.async into shared memory) and the histogram without returned values (the re-ordering draws the slots).
+ *                Kept for comparison: measured 7 % slower per step at configs[3] (K1b).           */
+int m3dk_set_push_variant(m3dk_ctx *ctx, int variant);
+
 /* Sort workspace (DEVICE, 256-byte aligned) for m3dk_sort and for the sorts inside m3dk_push; borrowed until replaced. */
 int m3dk_sort_workspace_bytes(long n_markers, int n_elems, size_t *bytes);
 int m3dk_set_sort_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes);

@@ -70,6 +70,7 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_fields_create": ([vp, i, _c_dp, i, _c_ip, _c_dp, i, _c_ip, _c_dp, _c_dp, vp, sz], i),
         "m3dk_particles_init": ([vp, lng] + [vp] * 10 + [dbl, dbl, C.POINTER(_F0)], i),
         "m3dk_set_options": ([vp, i, i, dbl], i),
+        "m3dk_set_push_variant": ([vp, i], i),
         "m3dk_sort_workspace_bytes": ([lng, i, C.POINTER(sz)], i),
         "m3dk_set_sort_workspace": ([vp, vp, sz], i),
         "m3dk_push": ([vp, i, dbl], i),
@@ -231,6 +232,9 @@ class Pusher:
     # ---- options, sort ----------------------------------------------------------------------------------------
     def set_options(self, sort_interval: int = 0, mode: int = 0, t0: float = 0.0):
         self._ck(self.L.m3dk_set_options(self.h, int(sort_interval), int(mode), float(t0)))
+
+    def set_push_variant(self, variant: int):
+        self._ck(self.L.m3dk_set_push_variant(self.h, int(variant)))
 
     def sort_workspace_bytes(self) -> int:
         need = C.c_size_t()

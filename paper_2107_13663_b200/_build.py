@@ -30,31 +30,56 @@ def _stale(out: str) -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def nvcc_cmd(verify: bool, out: str, extra=()):
-    cmd = ["nvcc", "-O3", "-std=c++17", *ARCH, "-lineinfo", "-shared", "-Xcompiler", "-fPIC,-ffp-contract=off",
-           "-Xptxas", "-v", "-o", out]
+def nvcc_flags(verify: bool, extra=()):
+    flags = ["-O3", "-std=c++17", *ARCH, "-lineinfo", "-Xcompiler", "-fPIC,-ffp-contract=off", "-Xptxas", "-v"]
     if verify:
-        cmd += ["-fmad=false", "-DM3DK_NO_FMA"]
-    cmd += list(extra)
-    cmd += [os.path.join(_CSRC, s) for s in SOURCES]
-    return cmd
+        flags += ["-fmad=false", "-DM3DK_NO_FMA"]
+    return flags + list(extra)
 
 
-def build(verify: bool = False, force: bool = False, verbose: bool = False) -> str:
+def nvcc_cmd(verify: bool, out: str, extra=()):
+    """The single-command form of the build (what the object-by-object build below is equivalent to)."""
+    return ["nvcc", *nvcc_flags(verify, extra), "-shared", "-o", out] + [os.path.join(_CSRC, s) for s in SOURCES]
+
+
+def build(verify: bool = False, force: bool = False, verbose: bool = False, extra=()) -> str:
+    """Compile every source to an object (in parallel: ptxas on the push kernels takes a minute) and link the library."""
+    from concurrent.futures import ThreadPoolExecutor
+
     out = lib_path(verify)
-    if force or _stale(out):
-        r = subprocess.run(nvcc_cmd(verify, out), capture_output=True, text=True)
-        if verbose or r.returncode != 0:
-            sys.stderr.write(r.stdout + r.stderr)
-        if r.returncode != 0:
-            raise RuntimeError("nvcc failed building " + out)
-        with open(out + ".ptxas.log", "w") as fh:
-            fh.write(r.stdout + r.stderr)
+    if not (force or _stale(out)):
+        return out
+    objdir = os.path.join(_HERE, "build", "verify" if verify else "timing")
+    os.makedirs(objdir, exist_ok=True)
+
+    def compile_one(src):
+        obj = os.path.join(objdir, src.replace(".cu", ".o"))
+        r = subprocess.run(["nvcc", *nvcc_flags(verify, extra), "-c", "-o", obj, os.path.join(_CSRC, src)],
+                           capture_output=True, text=True)
+        return obj, r
+
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as pool:
+        results = list(pool.map(compile_one, SOURCES))
+    log = "".join(r.stdout + r.stderr for _, r in results)
+    if verbose or any(r.returncode != 0 for _, r in results):
+        sys.stderr.write(log)
+    if any(r.returncode != 0 for _, r in results):
+        raise RuntimeError("nvcc failed building " + out)
+    r = subprocess.run(["nvcc", *ARCH, "-shared", "-o", out] + [o for o, _ in results], capture_output=True, text=True)
+    if r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("nvcc failed linking " + out)
+    with open(out + ".ptxas.log", "w") as fh:
+        fh.write(log)
     return out
 
 
 def build_all(force: bool = False, verbose: bool = False):
-    return build(False, force, verbose), build(True, force, verbose)
+    from concurrent.futures import ThreadPoolExecutor
+
+    with ThreadPoolExecutor(max_workers=2) as pool:
+        a, b = pool.submit(build, False, force, verbose), pool.submit(build, True, force, verbose)
+        return a.result(), b.result()
 
 
 if __name__ == "__main__":

@@ -68,6 +68,9 @@ extern "C" int m3dk_create(m3dk_ctx **out, int device, void *stream) {
     ctx->stream = static_cast<cudaStream_t>(stream);
     if (cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || ctx->sm_count < 1)
         ctx->sm_count = 148;
+    int optin = 0;
+    if (cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device) == cudaSuccess && optin > 0)
+        ctx->smem_optin = (size_t)optin;
     *out = ctx;
     return M3DK_OK;
 }
@@ -82,9 +85,8 @@ extern "C" int m3dk_destroy(m3dk_ctx *ctx) {
 
 // ---- fields --------------------------------------------------------------------------------------------------------
 // workspace: [control block 256 B][tiles][edge records][bstart][bcand (<= kCandPerElem * n_elems)]
-//            [fast grid: first records gf*gf][overflow records kFastOvfPerElem * n_elems]
+//            [fast grid: first records gf*gf][overflow records: at most one per bucket, gf*gf]
 static constexpr int kCandPerElem = 24;
-static constexpr int kFastOvfPerElem = 12;
 
 static int fast_grid_dim(int n_elems) {
     int g = (int)ceil(sqrt(2.0 * (double)n_elems));
@@ -106,7 +108,7 @@ extern "C" int m3dk_fields_workspace_bytes(int n_nodes, int n_elems, int n_modes
     b += up256((size_t)kCandPerElem * n_elems * sizeof(int) + 1024);
     const int gf = fast_grid_dim(n_elems);
     b += up256((size_t)gf * gf * sizeof(FastRec));
-    b += up256((size_t)kFastOvfPerElem * n_elems * sizeof(FastRec) + 1024);
+    b += up256((size_t)gf * gf * sizeof(FastRec) + 1024);
     *bytes = b;
     return M3DK_OK;
 }
@@ -283,30 +285,35 @@ extern "C" int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node
         if (a.area != b.area) return a.area > b.area;
         return a.e < b.e;
     });
-    const size_t ovf_cap = (size_t)kFastOvfPerElem * n_elems;
-    std::vector<FastRec> ffirst((size_t)gf * gf, FastRec{0.f, 0.f, 0.f, 0.f, 0.f, 0.f, -1, -1}), fovf;
-    fovf.reserve(std::min(ovf_cap, fc.size()));
+    const size_t ovf_cap = (size_t)gf * gf;
+    FastRec empty_rec;
+    memset(&empty_rec, 0, sizeof(empty_rec));
+    empty_rec.ida = empty_rec.idb = empty_rec.next = -1;
+    std::vector<FastRec> ffirst((size_t)gf * gf, empty_rec), fovf;
+    fovf.reserve(std::min(ovf_cap, fc.size() / 2 + 1));
     for (size_t k = 0; k < fc.size();) {
         size_t k1 = k;
         bool big = false;
         while (k1 < fc.size() && fc[k1].b == fc[k].b) { big = big || fc[k1].big; ++k1; }
         if (!big) {
-            FastRec *prev = nullptr;
+            // two candidates per record, at most 4 per bucket (the device loop's bound): first record + one overflow record
+            FastRec *cur = &ffirst[fc[k].b];
             for (size_t j = k; j < k1 && j < k + 4; ++j) {
                 const FCand &cn = fc[j];
-                FastRec r{cn.c[0], cn.c[1], cn.c[2], cn.c[3], cn.c[4], cn.c[5], cn.e, -1};
-                if (j == k) { ffirst[cn.b] = r; prev = &ffirst[cn.b]; }
-                else {
+                const size_t pos = j - k;
+                if (pos == 2) {
                     if (fovf.size() >= ovf_cap) break;
-                    prev->next = (int)fovf.size();
-                    fovf.push_back(r);         // reserve() above keeps `prev` valid: no reallocation below capacity
-                    prev = &fovf.back();
+                    cur->next = (int)fovf.size();
+                    fovf.push_back(empty_rec);     // reserve() above keeps `cur` valid: no reallocation below capacity
+                    cur = &fovf.back();
                 }
+                if (pos % 2 == 0) { for (int q = 0; q < 6; ++q) cur->a[q] = cn.c[q]; cur->ida = cn.e; }
+                else { for (int q = 0; q < 6; ++q) cur->b[q] = cn.c[q]; cur->idb = cn.e; }
             }
         }
         k = k1;
     }
-    if (fovf.empty()) fovf.push_back(FastRec{0.f, 0.f, 0.f, 0.f, 0.f, 0.f, -1, -1});
+    if (fovf.empty()) fovf.push_back(empty_rec);
 
     // carve and upload
     char *p = static_cast<char *>(dev_workspace);
@@ -374,6 +381,13 @@ extern "C" int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, doub
     ctx->sort_interval = sort_interval; ctx->mode = mode; ctx->t0 = t0;
     ctx->steps_done = 0;
     ctx->steps_since_sort = sort_interval;
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_set_push_variant(m3dk_ctx *ctx, int variant) {
+    if (!ctx) return M3DK_EINVAL;
+    if (variant < 0 || variant > 1) return fail(ctx, M3DK_EINVAL, "m3dk_set_push_variant: variant must be 0 or 1");
+    ctx->push_variant = variant;
     return M3DK_OK;
 }
 

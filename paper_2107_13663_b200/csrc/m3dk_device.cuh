@@ -182,38 +182,51 @@ static __device__ __noinline__ int locate(const GridParams &g, double R, double 
 // Returns the element when the point is strictly inside a candidate by more than the fp32 error bound (then rule G11
 // yields the same element), otherwise -2: the caller falls back to the exact search `locate`.
 __device__ __forceinline__ FastRec ldrec(const FastRec *p) {
-    unsigned r[8];
+    FastRec q;
+    unsigned r[16];
     asm("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
         : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "l"(p));
-    FastRec q;
-    q.x0 = __uint_as_float(r[0]); q.y0 = __uint_as_float(r[1]); q.x1 = __uint_as_float(r[2]);
-    q.y1 = __uint_as_float(r[3]); q.x2 = __uint_as_float(r[4]); q.y2 = __uint_as_float(r[5]);
-    q.id = (int)r[6]; q.next = (int)r[7];
+    asm("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+        : "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "l"(reinterpret_cast<const char *>(p) + 32));
+#pragma unroll
+    for (int k = 0; k < 6; ++k) { q.a[k] = __uint_as_float(r[k]); q.b[k] = __uint_as_float(r[6 + k]); }
+    q.ida = (int)r[12]; q.idb = (int)r[13]; q.next = (int)r[14]; q.pad = 0;
     return q;
+}
+
+// bucket of (R, Z) in the fast grid; `inside` false: the point is outside the grid (bucket 0 is returned for addressing)
+__device__ __forceinline__ int fast_bucket(const FastGrid &g, double R, double Z, float &u, float &v, bool &inside) {
+    const double fx = (R - g.Rmin) * g.inv_hx, fz = (Z - g.Zmin) * g.inv_hz;
+    inside = fx >= 0.0 && fx < (double)g.gx && fz >= 0.0 && fz < (double)g.gz;
+    const int ix = inside ? (int)fx : 0, iz = inside ? (int)fz : 0;
+    u = (float)(fx - (double)ix); v = (float)(fz - (double)iz);
+    return iz * g.gx + ix;
 }
 
 // The asm loads are not volatile, so the compiler may hoist them above the range checks: every address is therefore
 // clamped into its table first and the checks only decide whether the loaded record is used.
 __device__ __forceinline__ FastRec locate_first(const FastGrid &g, double R, double Z) {
-    const double fx = (R - g.Rmin) * g.inv_hx, fz = (Z - g.Zmin) * g.inv_hz;
-    const bool inside = fx >= 0.0 && fx < (double)g.gx && fz >= 0.0 && fz < (double)g.gz;
-    const int ix = inside ? (int)fx : 0, iz = inside ? (int)fz : 0;
-    return ldrec(g.first + (size_t)(iz * g.gx + ix));
+    float u, v;
+    bool inside;
+    return ldrec(g.first + (size_t)fast_bucket(g, R, Z, u, v, inside));
+}
+__device__ __forceinline__ bool fast_inside(const float (&t)[6], float u, float v) {
+    const float e0 = __fmul_rn(t[2] - t[0], v - t[1]) - __fmul_rn(t[3] - t[1], u - t[0]);
+    const float e1 = __fmul_rn(t[4] - t[2], v - t[3]) - __fmul_rn(t[5] - t[3], u - t[2]);
+    const float e2 = __fmul_rn(t[0] - t[4], v - t[5]) - __fmul_rn(t[1] - t[5], u - t[4]);
+    return e0 > kFastMargin && e1 > kFastMargin && e2 > kFastMargin;
 }
 __device__ __forceinline__ int locate_fast_from(const FastGrid &g, FastRec r, double R, double Z) {
-    const double fx = (R - g.Rmin) * g.inv_hx, fz = (Z - g.Zmin) * g.inv_hz;
-    const bool inside = fx >= 0.0 && fx < (double)g.gx && fz >= 0.0 && fz < (double)g.gz;
-    const int ix = inside ? (int)fx : 0, iz = inside ? (int)fz : 0;
-    const float u = (float)(fx - (double)ix), v = (float)(fz - (double)iz);
+    float u, v;
+    bool open;
+    fast_bucket(g, R, Z, u, v, open);
     int found = -2;
-    bool open = inside;
 #pragma unroll 1
-    for (int it = 0; it < 4 && open; ++it) {
-        const float e0 = __fmul_rn(r.x1 - r.x0, v - r.y0) - __fmul_rn(r.y1 - r.y0, u - r.x0);
-        const float e1 = __fmul_rn(r.x2 - r.x1, v - r.y1) - __fmul_rn(r.y2 - r.y1, u - r.x1);
-        const float e2 = __fmul_rn(r.x0 - r.x2, v - r.y2) - __fmul_rn(r.y0 - r.y2, u - r.x2);
-        if (r.id >= 0 && e0 > kFastMargin && e1 > kFastMargin && e2 > kFastMargin) { found = r.id; open = false; }
-        else if (r.id < 0 || r.next < 0) open = false;
+    for (int it = 0; it < 2 && open; ++it) {
+        if (r.ida >= 0 && fast_inside(r.a, u, v)) { found = r.ida; open = false; }
+        else if (r.ida >= 0 && r.idb >= 0 && fast_inside(r.b, u, v)) { found = r.idb; open = false; }
+        else if (r.ida < 0 || r.next < 0) open = false;
         else r = ldrec(g.ovf + max(r.next, 0));
     }
     return found;

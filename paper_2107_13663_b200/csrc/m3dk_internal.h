@@ -35,16 +35,19 @@ inline int tile_stride_doubles(int n_modes) {
 //   3 x (r_a, z_a, r_b - r_a, z_b - z_a), strict-interior tolerance, 3 x pad
 constexpr int kEdgeRec = 16;
 
-// Fast search grid (fp32, conservative): one 32-byte record per (bucket, candidate triangle):
-//   x0 y0 x1 y1 x2 y2  vertices in bucket-local units (bucket = [0,1)^2), all within [-kFastCmax+1, kFastCmax]
-//   id                  element index, -1 = "use the exact search for this bucket"
-//   next                index of the next candidate's record in the overflow array, -1 = none
+// Fast search grid (fp32, conservative): one 64-byte record per bucket, two candidate triangles each:
+//   a[6], b[6]          vertices (x0 y0 x1 y1 x2 y2) of the two candidates in bucket-local units (bucket = [0,1)^2), all
+//                       within [-kFastCmax+1, kFastCmax]
+//   ida, idb            their element indices; ida = -1: "use the exact search for this bucket"; idb = -1: no second one
+//   next                index of a record with two more candidates in the overflow array, -1 = none
 // A point whose three fp32 edge functions exceed kFastMargin is strictly inside that triangle in exact arithmetic
 // (error bound 720 * 2^-24 = 4.3e-5 for coordinates bounded by kFastCmax), so the exact rule G11 gives the same element.
+// Two candidates per record: one 64-byte fetch settles the search for nearly every point (a bucket of the regular mesh
+// meets one or two triangles), so the record of the new position can be fetched asynchronously ahead of its use.
 constexpr float kFastMargin = 1.0e-4f;
 constexpr double kFastCmax = 5.0;
-struct FastRec { float x0, y0, x1, y1, x2, y2; int id, next; };
-static_assert(sizeof(FastRec) == 32, "FastRec must be one 32-byte sector");
+struct FastRec { float a[6], b[6]; int ida, idb, next, pad; };
+static_assert(sizeof(FastRec) == 64, "FastRec must be two 32-byte sectors");
 
 struct FastGrid {
     double Rmin, Zmin, inv_hx, inv_hz;
@@ -131,6 +134,8 @@ struct SortBuffers {         // carved from the sort workspace
 struct m3dk_ctx {
     int device = 0;
     int sm_count = 148;
+    size_t smem_optin = 0;       // cudaDevAttrMaxSharedMemoryPerBlockOptin
+    int push_variant = 0;        // m3dk_set_push_variant: 0 = push_items_kernel (default), 1 = push_async_kernel (measured slower)
     cudaStream_t stream = nullptr;
     std::string err;
     // fields
@@ -142,6 +147,7 @@ struct m3dk_ctx {
     m3dk::MarkerArrays user{};   // caller's arrays (the state lives here between calls)
     int cur = 0;                 // record buffer that holds the state inside an ordered push / sort
     int ocur = 0;
+    bool ranks_valid = true;     // the last push with a histogram also wrote rank[] (else invert_kernel draws the slots)
     unsigned scan_epoch = 0;     // tag of the current scan launch (decoupled look-back without clearing)                // order buffer whose .y are the ids of the records in sb.rec[cur]
     double q = 1.0, m = 1.0;
     m3dk_f0_params f0{};

@@ -128,9 +128,13 @@ __device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, 
                                            const PertW &W);
 
 // kFlr (mode 2): phase B is replaced by the 4-point gyro-average of the perturbed fields (flr_wdot).
-template <int R, bool kHist, bool kSmem, class IO, bool kFlr = false>
+// kPost (asynchronously staged kernel): the step ends with the new (R, Z) in Rn, Zn; search, key, histogram and rank are
+// the caller's (it runs them one item later, on data that was fetched in the meantime); io.stage_next() is called once
+// all of this lane's input has been consumed.
+template <int R, bool kHist, bool kSmem, class IO, bool kFlr = false, bool kPost = false>
 __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const double *__restrict__ tile,
-                                       const long (&mi)[R], const long (&mo)[R], const bool (&on)[R]) {
+                                       const long (&mi)[R], const long (&mo)[R], const bool (&on)[R], double (&Rn)[R],
+                                       double (&Zn)[R]) {
     Marker s[R];
     StepGeom g[R];
 #pragma unroll
@@ -151,8 +155,7 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
     ring_fill<kSmem>(ring, tile + kTileHeader);
     quad_vd<R, kSmem>(tile + kTileHeader, tile + kTileHeader, ring, xi, eta, v, dx, de);   // (psi0, |B|0, F0, kappa)
     PertW W[R];
-    double Rn[R], Zn[R];
-    FastRec rec[R];
+    FastRec rec[kPost ? 1 : R];
     // three separate loops (loads, arithmetic, stores): the arithmetic of the R markers sits in one block with no
     // memory operation in between, so that the scheduler interleaves the R dependent chains (DFMA latency 8 cycles)
 #pragma unroll
@@ -183,24 +186,27 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
         // between the quads, costs registers in the hottest part of the kernel and measured slower; an L1 prefetch of
         // the record measured no gain)
     }
+    if constexpr (kPost) io.stage_next();
     // a3 for the NEW position (the key of the next sort) and, with kHist, the sort histogram of the new keys with each
     // marker's rank inside its key (the sort then needs no pass over the keys)
     unsigned peers[R];
     int base[R];
     auto locate_and_count = [&]() {
+        if constexpr (!kPost) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);   // all first records in flight together
-        int key[R];
+            for (int r = 0; r < R; ++r) rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);   // all first records in flight together
+            int key[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            int ne = -1;
-            if (on[r]) {
-                ne = locate_finish(P.f, rec[r], Rn[r], Zn[r]);
-                io.store_key(mo[r], ne);
+            for (int r = 0; r < R; ++r) {
+                int ne = -1;
+                if (on[r]) {
+                    ne = locate_finish(P.f, rec[r], Rn[r], Zn[r]);
+                    io.store_key(mo[r], ne);
+                }
+                key[r] = ne < 0 ? P.f.n_elems : ne;
             }
-            key[r] = ne < 0 ? P.f.n_elems : ne;
+            if (kHist) hist_issue<R>(P.hist, key, on, peers, base);
         }
-        if (kHist) hist_issue<R>(P.hist, key, on, peers, base);
     };
     if (kFlr && P.f.n_modes > 0) {
 #pragma unroll
@@ -248,7 +254,7 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
     } else {
         locate_and_count();
     }
-    if (kHist) rank_finish<R>(P.rank, mo, on, peers, base);
+    if (kHist && !kPost) rank_finish<R>(P.rank, mo, on, peers, base);
 }
 
 // Perturbed fields of R markers of one element, summed over the toroidal modes, in each marker's own cylindrical frame
@@ -361,9 +367,10 @@ __device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, 
 // ---- the same step in the non-linear trajectory mode (mode 1: PAPER.md:108, :130; reading G21) ------------------------
 // All perturbed fields are needed BEFORE the velocity update (the marker moves in the total fields), so they are
 // accumulated per marker (10 values) and the folding trick of the linear mode does not apply; B1_phi (quad 3) enters.
-template <int R, bool kHist, bool kSmem, class IO>
+template <int R, bool kHist, bool kSmem, class IO, bool kPost = false>
 __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, const double *__restrict__ tile,
-                                          const long (&mi)[R], const long (&mo)[R], const bool (&on)[R]) {
+                                          const long (&mi)[R], const long (&mo)[R], const bool (&on)[R], double (&Rn)[R],
+                                          double (&Zn)[R]) {
     Marker s[R];
     StepGeom g[R];
 #pragma unroll
@@ -393,7 +400,6 @@ __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, con
         pf[r].ER = pf[r].EP = pf[r].EZ = pf[r].BR = pf[r].BP = pf[r].BZ = pf[r].gR = pf[r].gP = pf[r].gZ = pf[r].dT = 0.0;
     }
     pert_fields<R, kSmem>(P, tile, xi, eta, g, se, pf);
-    double Rn[R], Zn[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const double w_old = s[r].w;
@@ -412,12 +418,15 @@ __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, con
             io.store_pos(mo[r], s[r].x, s[r].y, s[r].z, s[r].w);
             io.store_vel(mo[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
             if (P.f.n_modes > 0) io.store_w(mo[r], s[r].w);
-            ne = locate_any(P.f, Rn[r], Zn[r]);
-            io.store_key(mo[r], ne);
+            if constexpr (!kPost) {
+                ne = locate_any(P.f, Rn[r], Zn[r]);
+                io.store_key(mo[r], ne);
+            }
         }
         key[r] = ne < 0 ? P.f.n_elems : ne;
     }
-    if (kHist) {
+    if constexpr (kPost) io.stage_next();
+    if (kHist && !kPost) {
         unsigned peers[R];
         int base[R];
         hist_issue<R>(P.hist, key, on, peers, base);
@@ -439,14 +448,15 @@ __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant
     // the tile loads may be speculated above the `on` tests: e is clamped to a valid element for addressing
     const double *tile = P.f.tiles + (size_t)max(e, 0) * P.f.tile_stride;
     if (__any_sync(0xffffffffu, on[0])) {
+        double Rn[1], Zn[1];
         if (kRec) {
             const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems};
-            if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on);
-            else step_R<1, false, false, RecIO, kMode == 2>(P, io, tile, m, m, on);
+            if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on, Rn, Zn);
+            else step_R<1, false, false, RecIO, kMode == 2>(P, io, tile, m, m, on, Rn, Zn);
         } else {
             const SoAIO io{P.a, P.f.n_elems};
-            if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on);
-            else step_R<1, false, false, SoAIO, kMode == 2>(P, io, tile, m, m, on);
+            if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on, Rn, Zn);
+            else step_R<1, false, false, SoAIO, kMode == 2>(P, io, tile, m, m, on, Rn, Zn);
         }
     }
     if (kHist) {
@@ -458,8 +468,11 @@ __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant
 
 // ---- tile staging: one bulk copy (TMA, cp.async.bulk) per item into the warp's double buffer, mbarrier completion --
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned bar) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count = 1) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar, unsigned count = 1) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
 __device__ __forceinline__ void tile_copy_issue(unsigned dst, const double *src, unsigned bytes, unsigned bar) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
@@ -556,8 +569,9 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
         } else {
             mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
             phase ^= 1u << b;
-            if (kMode == 1) step_R_nl<kR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
-            else step_R<kR, kHist, true, RecIO, kMode == 2>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
+            double Rn[kR], Zn[kR];
+            if (kMode == 1) step_R_nl<kR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
+            else step_R<kR, kHist, true, RecIO, kMode == 2>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
         }
         b ^= 1;
         it = it1; it1 = it2; it2 = 3 * stride + __shfl_sync(0xffffffffu, ticket, 0);
@@ -565,6 +579,248 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
 #pragma unroll
         for (int r = 0; r < kR; ++r) { src0[r] = src1[r]; src1[r] = src2[r]; }
     }
+}
+
+
+// ---- element-ordered push with asynchronous staging (modes 0 and 1) ---------------------------------------------------
+// The same work decomposition as push_items_kernel (a warp takes a work item of one element, a lane up to kR of its
+// markers, tile staged by one bulk copy per item, items drawn from a ticket counter), but no warp ever waits for L2 or HBM
+// inside an item: everything an item needs from memory is requested one item ahead and lands in shared memory meanwhile.
+//   records   gathered with cp.async (4 x 16 B per marker) into the warp's record box while the previous item computes;
+//   search    at the end of item k the lane writes the new (R, Z) of its markers to shared memory and requests the 64-byte
+//             record of their search bucket with cp.async; the edge tests, the key store and the histogram atomics of
+//             item k run at the end of item k + 1, the returned ranks are stored at the end of item k + 2.
+// cp.async groups are committed in the order ... records(k + 1), search(k) ...; both waits allow the most recent group
+// to be pending (wait_group 1).
+__device__ __forceinline__ void cp_async16(unsigned dst, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// record box of the staged item: [4][32 R] double2 = (x, y), (z, w), (vx, vy), (vz, mu) of the item's slots: every access of
+// a warp is conflict-free, and a lane only ever touches the slots of its own markers
+template <int R>
+struct AsyncIO {
+    double2 *box;
+    double *out;
+    const double *in;
+    const int2 *ord_next;   // order entries (src, id) of the NEXT item's slots, src = -1: none (shared memory)
+    static constexpr int n = 32 * R;
+    __device__ __forceinline__ void load_pos(long i, double &x, double &y, double &z, double &w) const {
+        const double2 a = box[i], b = box[n + i];
+        x = a.x; y = a.y; z = b.x; w = b.y;
+    }
+    __device__ __forceinline__ void load_vel(long i, double &vx, double &vy, double &vz, double &mu) const {
+        const double2 a = box[2 * n + i], b = box[3 * n + i];
+        vx = a.x; vy = a.y; vz = b.x; mu = b.y;
+    }
+    __device__ __forceinline__ void store_pos(long o, double x, double y, double z, double w_old) const {
+        strec256(out + kRecDoubles * o, x, y, z, w_old);
+    }
+    __device__ __forceinline__ void store_vel(long o, double vx, double vy, double vz, double mu) const {
+        strec256(out + kRecDoubles * o + 4, vx, vy, vz, mu);
+    }
+    __device__ __forceinline__ void store_w(long o, double w) const { out[kRecDoubles * o + 3] = w; }
+    // this lane has consumed its records: the next item's may land in the same slots
+    __device__ __forceinline__ void stage_next() const {
+        const int lane = threadIdx.x & 31;
+        const unsigned b0 = smem_u32(box) + lane * 16u;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int src = ord_next[32 * r + lane].x;
+            if (src >= 0) {
+                const double *g = in + (size_t)kRecDoubles * src;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) cp_async16(b0 + (unsigned)(q * n + 32 * r) * 16u, g + 2 * q);
+            }
+        }
+        cp_async_commit();
+    }
+};
+
+template <bool kHist, int kMode, int kR>
+__global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 1 : M3DK_PUSH_MINBLOCKS) push_async_kernel(const __grid_constant__ PushParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int kWarps = kPushThreads / 32;
+    constexpr int kSlots = 32 * kR;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int stride_d = P.f.tile_stride;
+    const unsigned tile_bytes = (unsigned)stride_d * 8u;
+    // per warp: record box | new (R, Z) | search records | order entries [2] | descriptors [16] | 2 mbarriers | tile[2]
+    constexpr unsigned kBoxBytes = 4u * kSlots * 16u, kRzBytes = kSlots * 16u, kFrBytes = 4u * kSlots * 16u;
+    constexpr unsigned kOrdBytes = 2u * kSlots * 8u, kDscBytes = 16u * 16u;
+    constexpr unsigned kFixed = kBoxBytes + kRzBytes + kFrBytes + kOrdBytes + kDscBytes + 16u;
+    const unsigned wblock = 2u * tile_bytes + kFixed;
+    // the fixed-size areas come first (constant offsets from the warp's base), the two tile buffers last
+    unsigned char *const wbase = smem_raw + (size_t)warp * wblock;
+    unsigned char *q = wbase;
+    double2 *const box = reinterpret_cast<double2 *>(q); q += kBoxBytes;
+    double2 *const rz = reinterpret_cast<double2 *>(q); q += kRzBytes;
+    uint4 *const fr = reinterpret_cast<uint4 *>(q); q += kFrBytes;
+    int2 *const ord = reinterpret_cast<int2 *>(q); q += kOrdBytes;          // [2][kSlots]: order entries of items k + 1, k + 2
+    int4 *const dsc = reinterpret_cast<int4 *>(q); q += kDscBytes;             // ring of 16 item descriptors: items k - 1 .. k + 7
+    const unsigned bar0 = smem_u32(q);
+    double *const tbuf = reinterpret_cast<double *>(q + 16);
+    const unsigned buf0 = smem_u32(tbuf);
+    if (lane == 0) {
+        mbar_init(bar0); mbar_init(bar0 + 8);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    const int total = *P.n_items;
+    const int n_elems = P.f.n_elems;
+    const int stride = gridDim.x * kWarps;
+    const int4 none = make_int4(n_elems, 0, 0, 0);
+    AsyncIO<kR> io{box, P.rc.out, P.rc.in, ord};
+
+    // ---- prologue (blocking loads, once per warp): descriptors of the first four items, order entries of the first two,
+    // records and tile of the first.
+    // Items 0..3 of a warp are fixed (global warp index + 0, 1, 2, 3 grid strides); every further one comes from the ticket
+    // counter, four at a time: a returned atomic is waited for where it is used (a value left pending across an item is
+    // spilled by the compiler, i.e. waited for at once), so one wait serves four items
+    {
+        const int it0 = blockIdx.x * kWarps + warp;
+        if (lane < 16) {
+            int4 d = none;
+            const int it = it0 + lane * stride;
+            if (lane < 4 && it < total) d = __ldg(P.items + it);
+            dsc[lane] = d;
+        }
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int4 d = dsc[j];
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const int i = 32 * r + lane;
+                ord[j * kSlots + i] = i < d.z ? P.rc.order[d.y + i] : make_int2(-1, 0);
+            }
+        }
+        const int4 d0 = dsc[0];
+        if (d0.x < n_elems && d0.z > 0 && lane == 0) tile_copy_issue(buf0, P.f.tiles + (size_t)d0.x * stride_d, tile_bytes, bar0);
+        io.stage_next();                                 // records of the first item (order slot 0)
+        cp_async_commit();                               // (stands for the search group of an item before the first)
+    }
+    unsigned phase = 0;
+
+    // a3 for item k - 1: edge tests on the search records fetched meanwhile, key store, histogram count (no returned value:
+    // invert_kernel<true> draws the slots)
+    auto search_prev = [&](int k1) {
+        if (k1 < 0) return;
+        const int4 d = dsc[k1 & 15];
+        const int cnt = d.x < n_elems ? d.z : 0;
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            const int i = 32 * r + lane;
+            const bool on = i < cnt;
+            int key = n_elems;
+            if (on) {
+                const double2 p = rz[i];
+                const uint4 q0 = fr[i], q1 = fr[kSlots + i], q2 = fr[2 * kSlots + i], q3 = fr[3 * kSlots + i];
+                FastRec f;
+                f.a[0] = __uint_as_float(q0.x); f.a[1] = __uint_as_float(q0.y); f.a[2] = __uint_as_float(q0.z); f.a[3] = __uint_as_float(q0.w);
+                f.a[4] = __uint_as_float(q1.x); f.a[5] = __uint_as_float(q1.y); f.b[0] = __uint_as_float(q1.z); f.b[1] = __uint_as_float(q1.w);
+                f.b[2] = __uint_as_float(q2.x); f.b[3] = __uint_as_float(q2.y); f.b[4] = __uint_as_float(q2.z); f.b[5] = __uint_as_float(q2.w);
+                f.ida = (int)q3.x; f.idb = (int)q3.y; f.next = (int)q3.z; f.pad = 0;
+                const int ne = locate_finish(P.f, f, p.x, p.y);
+                key = ne < 0 ? n_elems : ne;
+                P.rc.key[(long)d.y + i] = key;
+            }
+            if (kHist && on) atomicAdd(P.hist + key, 1);
+        }
+    };
+
+    int k = 0;                                           // items this warp has stepped
+    for (;; ++k) {
+        const unsigned b = k & 1;
+        // everything requested up to one item ago has landed: the records of item k, the order entries of item k + 1, the
+        // descriptor of item k + 2 (only the search records of item k - 1 may still be under way)
+        cp_async_wait<1>();
+        __syncwarp();                                  // lane 0's descriptor copies are visible; tile buffer b ^ 1 is free
+        const int4 w0 = dsc[k & 15];                   // (element, first slot, count, -)
+        if (w0.z == 0) break;                          // tickets only grow: no item left for this warp
+        const int e = w0.x, start = w0.y, count = w0.z;
+        {
+            // requests: tile of item k + 1, order entries of item k + 2, every fourth item the descriptors of items k + 4 .. k + 7
+            const int4 w1 = dsc[(k + 1) & 15], w2 = dsc[(k + 2) & 15];
+            if (lane == 0 && w1.x < n_elems && w1.z > 0)
+                tile_copy_issue(buf0 + (b ^ 1) * tile_bytes, P.f.tiles + (size_t)w1.x * stride_d, tile_bytes, bar0 + (b ^ 1) * 8);
+            if ((k & 3) == 0 && lane < 4) {
+                int tk = 0;
+                if (lane == 0) tk = atomicAdd(P.ticket, 4);
+                const int it = 4 * stride + __shfl_sync(0xfu, tk, 0) + lane;
+                if (it < total) cp_async16(smem_u32(dsc + ((k + 4 + lane) & 15)), P.items + it);
+                else dsc[(k + 4 + lane) & 15] = none;
+            }
+            int2 *const o2 = ord + ((k + 2) & 1) * kSlots;
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const int i = 32 * r + lane;
+                if (i < w2.z) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(o2 + i)), "l"(P.rc.order + w2.y + i) : "memory");
+                else o2[i] = make_int2(-1, 0);
+            }
+            cp_async_commit();
+        }
+        io.ord_next = ord + ((k + 1) & 1) * kSlots;
+        long mi[kR], mo[kR];
+        bool on[kR];
+        double Rn[kR], Zn[kR];
+#pragma unroll
+        for (int r = 0; r < kR; ++r) { mi[r] = 32 * r + lane; mo[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count; Rn[r] = 1.0; Zn[r] = 0.0; }
+        if (e >= n_elems) {                            // lost markers: frozen (G12), moved along and counted for the next sort
+            int key[kR];
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                key[r] = n_elems;
+                if (on[r]) {
+                    double a0, a1, a2, a3, b0, b1, b2, b3;
+                    io.load_pos(mi[r], a0, a1, a2, a3); io.load_vel(mi[r], b0, b1, b2, b3);
+                    io.store_pos(mo[r], a0, a1, a2, a3); io.store_vel(mo[r], b0, b1, b2, b3);
+                    P.rc.key[mo[r]] = n_elems;
+                }
+            }
+            io.stage_next();
+            if (kHist) {
+                unsigned peers[kR];
+                int base[kR];
+                hist_issue<kR>(P.hist, key, on, peers, base);
+                rank_finish<kR>(P.rank, mo, on, peers, base);
+            }
+        } else {
+            mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
+            phase ^= 1u << b;
+            if (kMode == 1) step_R_nl<kR, kHist, true, AsyncIO<kR>, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
+            else step_R<kR, kHist, true, AsyncIO<kR>, false, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
+        }
+        cp_async_wait<2>();                            // the search records of item k - 1 have landed
+        search_prev(k - 1);
+        // item k: new (R, Z) and the request for the record of their search bucket
+        if (e < n_elems) {
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const int i = 32 * r + lane;
+                if (i < count) {
+                    rz[i] = make_double2(Rn[r], Zn[r]);
+                    float u, v;
+                    bool inside;
+                    const FastRec *g = P.f.fast.first + (size_t)fast_bucket(P.f.fast, Rn[r], Zn[r], u, v, inside);
+                    const unsigned d = smem_u32(fr) + (unsigned)i * 16u;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) cp_async16(d + (unsigned)(c * kSlots) * 16u, reinterpret_cast<const char *>(g) + 16 * c);
+                }
+            }
+        }
+        cp_async_commit();
+    }
+    // drain: search and ranks of the last item
+    cp_async_wait<0>();
+    search_prev(k - 1);
+}
+
+static size_t async_smem_bytes(int tile_stride, int kR) {
+    const size_t warps = kPushThreads / 32, slots = 32 * (size_t)kR;
+    return warps * (2 * (size_t)tile_stride * 8 + slots * (64 + 16 + 64 + 16) + 16 * 16 + 16);
 }
 
 // ---- diagnostics ---------------------------------------------------------------------------------------------------
@@ -655,6 +911,7 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
     PushParams P = make_params(c, c->user, n, dt, t);
     c->kernel_launches += 1;
     P.hist = c->sb.hist; P.rank = c->sb.rank;
+    c->ranks_valid = true;
     P.rc.key = c->sb.key; P.rc.order = c->sb.order[c->ocur];
     P.rc.in = c->sb.rec[c->cur];
     if (with_hist) {
@@ -672,6 +929,25 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
             P.n_items = small ? reinterpret_cast<const int *>(c->sb.scan_state + 1) : c->sb.ioffs + c->f.n_elems + 1;
             P.ticket = reinterpret_cast<int *>(c->sb.scan_state + (c->f.n_elems + 1 + 4095) / 4096 + 2) + small;
             void (*kern)(PushParams);
+            const size_t as_smem = async_smem_bytes(c->f.tile_stride, small ? 1 : 2);
+            if (c->push_variant == 1 && c->mode != 2 && as_smem <= c->smem_optin) {
+                if (small)
+                    kern = c->mode == 1 ? (with_hist ? push_async_kernel<true, 1, 1> : push_async_kernel<false, 1, 1>)
+                                        : (with_hist ? push_async_kernel<true, 0, 1> : push_async_kernel<false, 0, 1>);
+                else
+                    kern = c->mode == 1 ? (with_hist ? push_async_kernel<true, 1, 2> : push_async_kernel<false, 1, 2>)
+                                        : (with_hist ? push_async_kernel<true, 0, 2> : push_async_kernel<false, 0, 2>);
+                cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)as_smem);
+                if (e != cudaSuccess) return e;
+                int per_sm = 0;
+                e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kPushThreads, as_smem);
+                if (e != cudaSuccess) return e;
+                if (per_sm < 1) per_sm = 1;
+                if (small) c->kernel_launches += 1;
+                kern<<<(unsigned)(c->sm_count * per_sm), kPushThreads, as_smem, c->stream>>>(P);
+                c->ranks_valid = false;      // this kernel only counts; invert_kernel draws the slots
+                continue;
+            }
             if (small)
                 kern = c->mode == 1   ? (with_hist ? push_items_kernel<true, 1, 1> : push_items_kernel<false, 1, 1>)
                        : c->mode == 2 ? (with_hist ? push_items_kernel<true, 2, 1> : push_items_kernel<false, 2, 1>)

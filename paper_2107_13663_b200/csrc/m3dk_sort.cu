@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(256) hist_rank_kernel(const int *__restrict__ 
 __host__ __device__ inline int n_big_items(int c) { return c / kItemMarkers + ((c % kItemMarkers) > 32 ? 1 : 0); }
 
 constexpr int kScanChunk = 4096;
-__global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist, int m, int *__restrict__ offs,
+__global__ void __launch_bounds__(1024) scan_kernel(int *__restrict__ hist, int m, int *__restrict__ offs,
                                                     int *__restrict__ ioffs, unsigned long long *state,
                                                     unsigned epoch) {
     __shared__ int2 wsum[32];
@@ -83,6 +83,7 @@ __global__ void __launch_bounds__(1024) scan_kernel(const int *__restrict__ hist
     for (int q = 0; q < 4; ++q) {
         v[q] = k + q < m ? hist[k + q] : 0;
         it[q] = n_big_items(v[q]);
+        if (k + q < m) hist[k + q] = 0;       // the counts are consumed: the array serves invert_kernel<true> as slot cursors
     }
     const int2 mine = make_int2(v[0] + v[1] + v[2] + v[3], it[0] + it[1] + it[2] + it[3]);
     int2 inc = mine;
@@ -170,13 +171,33 @@ __global__ void __launch_bounds__(256) pack_kernel(MarkerArrays a, long n, int n
     key[d] = k;
 }
 
-// next order list: the record in slot j goes to slot d = offs[key[j]] + rank[j] of the next element-ordered push
+// next order list: the record in slot j goes to slot d = offs[key[j]] + rank[j] of the next element-ordered push.
+// kDraw = false: rank[] was written by the push kernel (returned histogram atomics).  kDraw = true: the push kernel only
+// counted (atomics without a returned value: nothing pending in its registers); the rank inside the key is drawn here from
+// cursor[] (the histogram array, zeroed by the scan) with one warp-aggregated atomic per distinct key of a warp.  Slots
+// are in the order of the OLD elements, so neighbouring warps would hit the same few cursors at the same time: block b
+// takes the chunk (b * cstride) mod gridDim.x (cstride coprime with the grid, chosen by the launcher).
+template <bool kDraw>
 __global__ void __launch_bounds__(256) invert_kernel(long n, const int *__restrict__ key, const int *__restrict__ offs,
-                                                     const int *__restrict__ rank, const int2 *__restrict__ order_cur,
-                                                     int2 *__restrict__ order_next) {
-    const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n) return;
-    const long d = (long)offs[key[j]] + rank[j];
+                                                     const int *__restrict__ rank, int *__restrict__ cursor,
+                                                     const int2 *__restrict__ order_cur, int2 *__restrict__ order_next,
+                                                     unsigned cstride) {
+    const unsigned blk = kDraw ? (unsigned)(((unsigned long long)blockIdx.x * cstride) % gridDim.x) : blockIdx.x;
+    const long j = (long)blk * blockDim.x + threadIdx.x;
+    const bool on = j < n;
+    if (!kDraw) {
+        if (on) order_next[(long)offs[key[j]] + rank[j]] = make_int2((int)j, order_cur[j].y);
+        return;
+    }
+    const unsigned live = __ballot_sync(0xffffffffu, on);
+    if (!on) return;
+    const int k = key[j];
+    const unsigned peers = __match_any_sync(live, k);
+    const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(cursor + k, __popc(peers));
+    base = __shfl_sync(peers, base, leader);
+    const long d = (long)offs[k] + base + __popc(peers & ((1u << lane) - 1u));
     order_next[d] = make_int2((int)j, order_cur[j].y);
 }
 
@@ -229,8 +250,18 @@ cudaError_t launch_reorder(m3dk_ctx *c, long n) {
     cudaError_t e = scan_and_cut(c);
     if (e != cudaSuccess) return e;
     c->kernel_launches += 1;
-    invert_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, c->sb.key, c->sb.offs, c->sb.rank,
-                                                                       c->sb.order[c->ocur], c->sb.order[c->ocur ^ 1]);
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    if (c->ranks_valid) {
+        invert_kernel<false><<<grid, 256, 0, c->stream>>>(n, c->sb.key, c->sb.offs, c->sb.rank, c->sb.hist,
+                                                         c->sb.order[c->ocur], c->sb.order[c->ocur ^ 1], 1u);
+    } else {
+        static const unsigned primes[] = {1009u, 1013u, 1019u, 1021u, 1031u};
+        unsigned cs = 1u;
+        for (unsigned p : primes)
+            if (grid % p != 0) { cs = p; break; }
+        invert_kernel<true><<<grid, 256, 0, c->stream>>>(n, c->sb.key, c->sb.offs, c->sb.rank, c->sb.hist,
+                                                        c->sb.order[c->ocur], c->sb.order[c->ocur ^ 1], cs);
+    }
     c->ocur ^= 1;
     return cudaGetLastError();
 }
