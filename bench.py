@@ -244,18 +244,18 @@ def run_ours(args, rank, world, local_rank):
     clocks = sampler.stop(wall0, wall1) if sampler else None
     p.set_profiling(False)
 
-    # ---- end-to-end leg: host buffers through the C ABI, copies inside the timed region ----------------------------
+    # ---- end-to-end leg: host buffers through the C ABI (m3dk_push_host), copies inside the timed region ------------------
+    # One call = upload + K steps + download of all markers, pipelined by marker chunk.  The buffers are the ones a first
+    # call returned (element order, the steady state of a caller that keeps pushing the same markers): a chunk is then
+    # spatially compact and keeps the full number of markers per element.
     host = {k: torch.from_numpy(np.ascontiguousarray(w.markers[k])).pin_memory() for k in m3dk.STATE_KEYS}
-    out = {k: torch.empty(N, dtype=torch.float64).pin_memory() for k in m3dk.STATE_KEYS}
-    Ke = K
-    p.upload(host); p.set_options(sort_interval=si, mode=args.mode, t0=0.0); p.push(1, w.dt); p.download(out)      # warm the path
+    Ke, C_e2e = K, args.e2e_chunks
+    p.push_host(host, 1, w.dt, n_chunks=C_e2e)
+    p.set_options(sort_interval=si, mode=args.mode, t0=0.0)
     barrier()
     f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     f0.record(p.stream)
-    p.upload(host)
-    p.set_options(sort_interval=si, mode=args.mode, t0=0.0)
-    p.push(Ke, w.dt)
-    p.download(out)
+    p.push_host(host, Ke, w.dt, n_chunks=C_e2e)
     f1.record(p.stream)
     barrier()
     ms_e2e = f0.elapsed_time(f1)
@@ -294,7 +294,9 @@ def run_ours(args, rank, world, local_rank):
             "dtype": "f64", "data": "synthetic", "config": config_dict(args, w, si, world),
             "clocks": clocks, "gpu_launches": tm["kernel_launches"],
             "e2e": {"value": shard.whole_job_rate([N] * world, Ke, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": 64 * N / Ke,
-                    "d2h_bytes_per_step": 64 * N / Ke, "note": f"one upload + {Ke} steps + one download (PAPER.md:237)"},
+                    "d2h_bytes_per_step": 64 * N / Ke,
+                    "note": f"m3dk_push_host: one upload + {Ke} steps + one download per call (PAPER.md:237), pipelined in "
+                            f"{C_e2e} marker chunks; host buffers pinned, in the element order an earlier call returned"},
             "roofline": roof, "n_lost": st["n_lost"]}
     if args.gc:
         # row (f)-3: RK4 guiding-centre steps on the same markers (x, y, z as X; v_par = 0.5 for every marker)
@@ -394,6 +396,7 @@ def main():
     ap.add_argument("--gc", action="store_true", help="also time m3dk_gc_push (SURVEY.md 8(f)-3) on the final state")
     ap.add_argument("--deposit", action="store_true", help="also time m3dk_deposit (SURVEY.md 8(f)-4) on the final state")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-chunks", type=int, default=4, help="marker chunks of the pipelined host-buffer call (e2e leg)")
     ap.add_argument("--push-variant", type=int, default=0, choices=[0, 1],
                     help="m3dk_set_push_variant: 0 = default kernel, 1 = asynchronously staged kernel (A/B comparison)")
     ap.add_argument("--sweep", action="store_true", help="configs[4] sweep: one JSON line per (n, dt, sort interval)")

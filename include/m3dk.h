@@ -158,6 +158,20 @@ int m3dk_particles_upload(m3dk_ctx *ctx, const double *hx, const double *hy, con
 int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, double *hz, double *hvx, double *hvy, double *hvz,
                             double *hmu, double *hw, int *host_id, int *host_elem);
 
+/* The host-buffer path as ONE call, pipelined by marker chunk: equivalent to m3dk_particles_upload -> m3dk_push(nsteps, dt)
+ * -> m3dk_particles_download on the same HOST buffers (in place: on return they hold the new state), but the n markers are
+ * cut into n_chunks contiguous chunks and chunk c uploads while chunk c - 1 runs its nsteps steps and chunk c - 2
+ * downloads (markers are independent; the three run on three streams, the two copy directions concurrently).
+ * Sorts act inside a chunk: slot i of chunk c holds the marker host_id[i], with ids global (0..n-1 = the caller's order at
+ * entry).  host_id / host_elem may be NULL.  Pinned buffers are needed for the copies to overlap.  Every chunk steps from
+ * the same time; t advances by nsteps * dt once.  The call needs the device arrays of m3dk_particles_init (n markers) and,
+ * for sort_interval >= 1, the sort workspace; it synchronises before returning.  n_chunks = 1 is the unpipelined path.
+ * Chunks of a marker stream in random order see a mesh n_chunks times sparser per chunk (fewer markers per element, less
+ * sharing of coefficient tiles); buffers that come back from an earlier call are in element order, and their chunks are
+ * spatially compact.                                                                                                   */
+int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz, double *hvx, double *hvy, double *hvz, double *hmu,
+                   double *hw, int *host_id, int *host_elem, int nsteps, double dt, int n_chunks);
+
 /* Diagnostics for tests and the roofline: fields at arbitrary points through the same device code as the push.
  * R, phi, Z: DEVICE [n]; elem_out: DEVICE int[n]; out: DEVICE [n][18] =
  * psi_R psi_Z |B| |B|_R |B|_Z F kappa E1(R,phi,Z) B1(R,phi,Z) gradB1par(R,phi,Z) dB1par/dt B1par.                     */

@@ -78,6 +78,7 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_stats": ([vp, C.POINTER(_Stats)], i),
         "m3dk_particles_upload": ([vp] + [vp] * 8, i),
         "m3dk_particles_download": ([vp] + [vp] * 10, i),
+        "m3dk_push_host": ([vp] + [vp] * 10 + [i, dbl, i], i),
         "m3dk_eval_fields": ([vp, lng, vp, vp, vp, dbl, vp, vp], i),
         "m3dk_gc_push": ([vp, i, dbl, vp], i),
         "m3dk_deposit_bytes": ([vp, C.POINTER(sz)], i),
@@ -282,6 +283,17 @@ class Pusher:
         for a in (host_id, host_elem):
             ptrs.append(None if a is None else C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data))
         self._ck(self.L.m3dk_particles_download(self.h, *ptrs))
+
+    def push_host(self, host: dict, nsteps: int, dt: float, n_chunks: int = 1, host_id=None, host_elem=None):
+        """m3dk_push_host: upload, nsteps steps and download pipelined by marker chunk, in place on the (pinned) host
+        buffers of ``host`` (dict of torch CPU tensors or numpy arrays, fp64, length n).  Synchronises."""
+        ptrs = []
+        for k in STATE_KEYS:
+            a = host[k]
+            ptrs.append(C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data))
+        for a in (host_id, host_elem):
+            ptrs.append(None if a is None else C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data))
+        self._ck(self.L.m3dk_push_host(self.h, *ptrs, int(nsteps), float(dt), int(n_chunks)))
 
     # ---- results ------------------------------------------------------------------------------------------------
     def state(self, by_id: bool = True):

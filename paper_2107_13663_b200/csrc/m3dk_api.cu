@@ -11,7 +11,7 @@
 
 using namespace m3dk;
 
-static std::string g_create_error;
+static thread_local std::string g_create_error;
 
 static int fail(m3dk_ctx *c, int code, const std::string &msg) {
     if (c) c->err = msg; else g_create_error = msg;
@@ -79,6 +79,9 @@ extern "C" int m3dk_destroy(m3dk_ctx *ctx) {
     if (!ctx) return M3DK_EINVAL;
     drop_events(ctx->ev_push, nullptr, nullptr);
     drop_events(ctx->ev_sort, nullptr, nullptr);
+    for (cudaEvent_t e : ctx->ev_chunk) cudaEventDestroy(e);
+    if (ctx->s_up) cudaStreamDestroy(ctx->s_up);
+    if (ctx->s_down) cudaStreamDestroy(ctx->s_down);
     delete ctx;
     return M3DK_OK;
 }
@@ -364,10 +367,15 @@ extern "C" int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, 
     ctx->user = MarkerArrays{x, y, z, vx, vy, vz, mu, w, elem, id};
     ctx->q = charge; ctx->m = mass; ctx->f0 = *f0;
     ctx->steps_done = 0; ctx->n_sorts = 0;
+    ctx->t_base = ctx->t0; ctx->steps_at_dt = 0;
     ctx->steps_since_sort = ctx->sort_interval;   // the first push sorts first when sorting is on
     ctx->have_markers = true;
-    if (ctx->have_sortws && ctx->sb.bytes) {      // an older workspace may be too small for the new n
-        if (sort_workspace_bytes(n, ctx->f.n_elems) > ctx->sb.bytes) ctx->have_sortws = false;
+    // the sort workspace was carved for the previous n / mesh: carve it again, or drop it if it has become too small
+    ctx->have_sortws = false;
+    if (ctx->sortws_base && sort_workspace_bytes(n, ctx->f.n_elems) <= ctx->sortws_bytes) {
+        carve_sort_workspace(ctx->sortws_base, n, ctx->f.n_elems, &ctx->sb);
+        ctx->sb.bytes = ctx->sortws_bytes;
+        ctx->have_sortws = true;
     }
     CU(launch_locate(ctx, ctx->user, n, true), "locate kernel");
     return M3DK_OK;
@@ -379,6 +387,7 @@ extern "C" int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, doub
     if (mode < 0 || mode > 2)
         return fail(ctx, M3DK_EINVAL, "m3dk_set_options: mode must be 0 (linear delta-f), 1 (non-linear trajectories) or 2 (linear + FLR)");
     ctx->sort_interval = sort_interval; ctx->mode = mode; ctx->t0 = t0;
+    ctx->t_base = t0; ctx->steps_at_dt = 0;
     ctx->steps_done = 0;
     ctx->steps_since_sort = sort_interval;
     return M3DK_OK;
@@ -402,8 +411,8 @@ static int bind_sort_ws(m3dk_ctx *ctx, void *ws, size_t bytes, const char *who) 
     if (!ws || ((uintptr_t)ws & 255) || bytes < sort_workspace_bytes(ctx->n, ctx->f.n_elems))
         return fail(ctx, M3DK_EWORKSPACE, std::string(who) + ": workspace NULL, misaligned or smaller than m3dk_sort_workspace_bytes");
     carve_sort_workspace(ws, ctx->n, ctx->f.n_elems, &ctx->sb);
-
     ctx->sb.bytes = bytes;
+    ctx->sortws_base = ws; ctx->sortws_bytes = bytes;
     ctx->have_sortws = true;
     return M3DK_OK;
 }
@@ -441,21 +450,25 @@ extern "C" int m3dk_sort(m3dk_ctx *ctx, void *dev_workspace, size_t bytes) {
     return M3DK_OK;
 }
 
-extern "C" int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt) {
-    if (!ctx) return M3DK_EINVAL;
-    if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_push: fields and markers must be set first");
-    if (nsteps < 0 || !(dt == dt)) return fail(ctx, M3DK_EINVAL, "m3dk_push: nsteps < 0 or dt is NaN");
-    if (ctx->sort_interval > 0 && !ctx->have_sortws)
-        return fail(ctx, M3DK_ESTATE, "m3dk_push: sort_interval > 0 needs m3dk_set_sort_workspace");
-    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
-    ctx->last_dt = dt;
+// time of the next step's x_l: t_base + (steps taken at the current dt) * dt; a changed dt starts a new run of equal steps
+static double step_time(m3dk_ctx *ctx, double dt) {
+    if (dt != ctx->last_dt) {
+        ctx->t_base += (double)ctx->steps_at_dt * ctx->last_dt;
+        ctx->steps_at_dt = 0;
+        ctx->last_dt = dt;
+    }
+    return ctx->t_base + (double)ctx->steps_at_dt * dt;
+}
+
+// nsteps steps of the markers currently bound to the context (ctx->n, ctx->user, ctx->sb)
+static int run_steps(m3dk_ctx *ctx, int nsteps, double dt) {
     const int k = ctx->sort_interval;
     if (k == 0 || ctx->n == 0 || nsteps == 0) {
         for (int l = 0; l < nsteps; ++l) {
-            const double t = ctx->t0 + (double)ctx->steps_done * dt;   // t_l of this step's x_l
+            const double t = step_time(ctx, dt);            // t_l of this step's x_l
             EvScope ev(ctx, &ctx->ev_push);
             CU(launch_push_soa(ctx, ctx->n, dt, t), "push kernel");
-            ctx->steps_done++;
+            ctx->steps_done++; ctx->steps_at_dt++;
         }
         return M3DK_OK;
     }
@@ -467,14 +480,14 @@ extern "C" int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt) {
     ctx->steps_since_sort = 0;
     bool ordered = true;     // the records are in element order and sb.items cut them
     for (int l = 0; l < nsteps; ++l) {
-        const double t = ctx->t0 + (double)ctx->steps_done * dt;
+        const double t = step_time(ctx, dt);
         const bool reorder_after = l + 1 < nsteps && ctx->steps_since_sort + 1 >= k;
         {
             EvScope ev(ctx, &ctx->ev_push);
             CU(launch_push_rec(ctx, ctx->n, dt, t, reorder_after, ordered), "push kernel");
         }
         ordered = false;     // the markers have moved
-        ctx->steps_done++;
+        ctx->steps_done++; ctx->steps_at_dt++;
         ctx->steps_since_sort++;
         if (reorder_after) {
             EvScope ev(ctx, &ctx->ev_sort);
@@ -491,6 +504,16 @@ extern "C" int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt) {
     return M3DK_OK;
 }
 
+extern "C" int m3dk_push(m3dk_ctx *ctx, int nsteps, double dt) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_push: fields and markers must be set first");
+    if (nsteps < 0 || !(dt == dt)) return fail(ctx, M3DK_EINVAL, "m3dk_push: nsteps < 0 or dt is NaN");
+    if (ctx->sort_interval > 0 && !ctx->have_sortws)
+        return fail(ctx, M3DK_ESTATE, "m3dk_push: sort_interval > 0 needs m3dk_set_sort_workspace");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    return run_steps(ctx, nsteps, dt);
+}
+
 extern "C" int m3dk_stats(m3dk_ctx *ctx, m3dk_stats_t *out) {
     if (!ctx || !out) return M3DK_EINVAL;
     memset(out, 0, sizeof(*out));
@@ -505,7 +528,7 @@ extern "C" int m3dk_stats(m3dk_ctx *ctx, m3dk_stats_t *out) {
     out->n_lost = lost;
     out->steps_done = ctx->steps_done;
     out->n_sorts = ctx->n_sorts;
-    out->t = ctx->t0 + (double)ctx->steps_done * ctx->last_dt;
+    out->t = ctx->t_base + (double)ctx->steps_at_dt * ctx->last_dt;
     return M3DK_OK;
 }
 
@@ -540,6 +563,80 @@ extern "C" int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, do
     if (host_id) CU(cudaMemcpyAsync(host_id, d.id, ni, cudaMemcpyDeviceToHost, ctx->stream), "download id");
     if (host_elem) CU(cudaMemcpyAsync(host_elem, d.elem, ni, cudaMemcpyDeviceToHost, ctx->stream), "download elem");
     CU(cudaStreamSynchronize(ctx->stream), "stream synchronize (an earlier kernel may have failed)");
+    return M3DK_OK;
+}
+
+// Host-buffer push, pipelined by marker chunk (markers are independent): chunk c is uploaded on the upload
+// stream while chunk c - 1 runs its nsteps steps on the context's stream and chunk c - 2 is downloaded on the download
+// stream (the two copy directions run concurrently).  Every chunk goes through the same code as m3dk_push on its
+// sub-range of the registered device arrays; the sort workspace is re-carved for the chunk size and used by one chunk at
+// a time (the steps of all chunks are in stream order).
+extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz, double *hvx, double *hvy, double *hvz,
+                              double *hmu, double *hw, int *host_id, int *host_elem, int nsteps, double dt, int n_chunks) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_push_host: fields and markers must be set first");
+    if (!hx || !hy || !hz || !hvx || !hvy || !hvz || !hmu || !hw) return fail(ctx, M3DK_EINVAL, "m3dk_push_host: NULL buffer");
+    if (nsteps < 0 || !(dt == dt) || n_chunks < 1) return fail(ctx, M3DK_EINVAL, "m3dk_push_host: nsteps < 0, dt is NaN or n_chunks < 1");
+    if (ctx->sort_interval > 0 && !ctx->have_sortws)
+        return fail(ctx, M3DK_ESTATE, "m3dk_push_host: sort_interval > 0 needs m3dk_set_sort_workspace");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    const long n = ctx->n;
+    if (n == 0) return M3DK_OK;
+    if ((long)n_chunks > n) n_chunks = (int)n;
+    if (!ctx->s_up) {
+        CU(cudaStreamCreateWithFlags(&ctx->s_up, cudaStreamNonBlocking), "create upload stream");
+        CU(cudaStreamCreateWithFlags(&ctx->s_down, cudaStreamNonBlocking), "create download stream");
+    }
+    while (ctx->ev_chunk.size() < (size_t)2 * n_chunks + 1) {
+        cudaEvent_t e;
+        CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "create chunk event");
+        ctx->ev_chunk.push_back(e);
+    }
+    // the copy streams start after everything already enqueued on the context's stream (the arrays may be in use)
+    cudaEvent_t ev_start = ctx->ev_chunk[2 * n_chunks];
+    CU(cudaEventRecord(ev_start, ctx->stream), "record start");
+    CU(cudaStreamWaitEvent(ctx->s_up, ev_start, 0), "upload stream wait");
+    CU(cudaStreamWaitEvent(ctx->s_down, ev_start, 0), "download stream wait");
+
+    const MarkerArrays all = ctx->user;
+    const long steps0 = ctx->steps_done, at0 = ctx->steps_at_dt;
+    const double tb0 = ctx->t_base, ldt0 = ctx->last_dt;
+    double *const hs[8] = {hx, hy, hz, hvx, hvy, hvz, hmu, hw};
+    double *const dd[8] = {all.x, all.y, all.z, all.vx, all.vy, all.vz, all.mu, all.w};
+    int rc = M3DK_OK;
+    const long per = (n + n_chunks - 1) / n_chunks;
+    for (int c = 0; c < n_chunks && rc == M3DK_OK; ++c) {
+        const long o = (long)c * per, nc = std::min(per, n - o);
+        if (nc <= 0) break;
+        const size_t nb = (size_t)nc * sizeof(double);
+        for (int k = 0; k < 8; ++k)
+            CU(cudaMemcpyAsync(dd[k] + o, hs[k] + o, nb, cudaMemcpyHostToDevice, ctx->s_up), "upload chunk");
+        CU(cudaEventRecord(ctx->ev_chunk[2 * c], ctx->s_up), "record upload");
+        CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_chunk[2 * c], 0), "compute waits for upload");
+        // bind the chunk: same time and step counter for every chunk
+        ctx->n = nc;
+        ctx->user = MarkerArrays{all.x + o, all.y + o, all.z + o, all.vx + o, all.vy + o, all.vz + o, all.mu + o, all.w + o,
+                                 all.elem + o, all.id + o};
+        if (ctx->have_sortws) carve_sort_workspace(ctx->sortws_base, nc, ctx->f.n_elems, &ctx->sb);
+        ctx->steps_done = steps0; ctx->steps_at_dt = at0; ctx->t_base = tb0; ctx->last_dt = ldt0;
+        cudaError_t e = launch_locate(ctx, ctx->user, nc, true, (int)o);
+        if (e != cudaSuccess) { rc = cuda_fail(ctx, e, "locate kernel"); break; }
+        rc = run_steps(ctx, nsteps, dt);
+        if (rc != M3DK_OK) break;
+        CU(cudaEventRecord(ctx->ev_chunk[2 * c + 1], ctx->stream), "record compute");
+        CU(cudaStreamWaitEvent(ctx->s_down, ctx->ev_chunk[2 * c + 1], 0), "download waits for compute");
+        for (int k = 0; k < 8; ++k)                     // mu included: it travels with its marker through the sorts
+            CU(cudaMemcpyAsync(hs[k] + o, dd[k] + o, nb, cudaMemcpyDeviceToHost, ctx->s_down), "download chunk");
+        if (host_id) CU(cudaMemcpyAsync(host_id + o, all.id + o, (size_t)nc * sizeof(int), cudaMemcpyDeviceToHost, ctx->s_down), "download id");
+        if (host_elem) CU(cudaMemcpyAsync(host_elem + o, all.elem + o, (size_t)nc * sizeof(int), cudaMemcpyDeviceToHost, ctx->s_down), "download elem");
+    }
+    // restore the full binding
+    ctx->n = n; ctx->user = all;
+    if (ctx->have_sortws) carve_sort_workspace(ctx->sortws_base, n, ctx->f.n_elems, &ctx->sb);
+    ctx->sb.bytes = ctx->sortws_bytes;
+    if (rc != M3DK_OK) return rc;
+    CU(cudaStreamSynchronize(ctx->s_down), "download stream synchronize (an earlier kernel may have failed)");
+    CU(cudaStreamSynchronize(ctx->stream), "stream synchronize");
     return M3DK_OK;
 }
 

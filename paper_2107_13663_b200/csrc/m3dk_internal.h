@@ -154,7 +154,9 @@ struct m3dk_ctx {
     // options / clock
     int sort_interval = 0;
     int mode = 0;
-    double t0 = 0.0;
+    double t0 = 0.0;             // time of the first step after m3dk_set_options
+    double t_base = 0.0;         // time at which the current run of equal steps began; t = t_base + steps_at_dt * last_dt
+    long steps_at_dt = 0;
     long steps_done = 0;
     long steps_since_sort = 0;
     long n_sorts = 0;
@@ -163,6 +165,11 @@ struct m3dk_ctx {
     bool have_sortws = false;
     m3dk::SortBuffers sb{};
     int *d_count = nullptr;      // small device scratch inside the fields workspace (lost counter etc.)
+    void *sortws_base = nullptr; // the caller's sort workspace as given (re-carved when n or the mesh changes)
+    size_t sortws_bytes = 0;
+    // m3dk_push_host: copy streams and per-chunk events (created on first use)
+    cudaStream_t s_up = nullptr, s_down = nullptr;
+    std::vector<cudaEvent_t> ev_chunk;
     // profiling (m3dk_set_profiling / m3dk_timing)
     bool profiling = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_push, ev_sort;
@@ -173,7 +180,7 @@ struct m3dk_ctx {
 namespace m3dk {
 
 // launchers (defined in push.cu / sort.cu); all enqueue on ctx->stream and return cudaGetLastError()
-cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_id);
+cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_id, int id_base = 0);
 cudaError_t launch_push_soa(m3dk_ctx *c, long n, double dt, double t);                           // caller's arrays, any order
 cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_hist, bool use_items);   // records
 cudaError_t launch_eval_fields(m3dk_ctx *c, long n, const double *R, const double *phi, const double *Z, double t,

@@ -17,11 +17,11 @@ constexpr int kPushThreads = M3DK_PUSH_THREADS;
 
 // ---- element of every marker (particles_init / upload) ------------------------------------------------------------
 __global__ void __launch_bounds__(256) locate_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, long n,
-                                                     int fill_id) {
+                                                     int fill_id, int id_base) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     a.elem[i] = locate_xyz(f, a.x[i], a.y[i], a.z[i]);
-    if (fill_id) a.id[i] = (int)i;
+    if (fill_id) a.id[i] = id_base + (int)i;
 }
 
 // Warp-aggregated histogram with returned ranks: lanes with the same key elect a leader that does one atomic.
@@ -886,11 +886,11 @@ static PushParams make_params(m3dk_ctx *c, const MarkerArrays &a, long n, double
     return P;
 }
 
-cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_id) {
+cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_id, int id_base) {
     if (n == 0) return cudaSuccess;
     const unsigned grid = (unsigned)((n + 255) / 256);
     c->kernel_launches += 1;
-    locate_kernel<<<grid, 256, 0, c->stream>>>(c->f, a, n, fill_id ? 1 : 0);
+    locate_kernel<<<grid, 256, 0, c->stream>>>(c->f, a, n, fill_id ? 1 : 0, id_base);
     return cudaGetLastError();
 }
 
