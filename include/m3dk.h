@@ -72,7 +72,7 @@ typedef struct {
     long n_markers;
     long n_lost;     /* markers outside every triangle: frozen, element -1, sorted last (reading G12)                  */
     long steps_done; /* since the last m3dk_set_options / m3dk_particles_init                                          */
-    long n_sorts;    /* sorts executed (explicit + internal)                                                           */
+    long n_sorts;    /* orderings executed: m3dk_sort calls, the pack at the start of a push call, one per step after   */
     double t;        /* t0 + steps_done * dt of the last push                                                          */
 } m3dk_stats_t;
 
@@ -114,7 +114,13 @@ int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, double *z, 
                         double *mu, double *w, int *elem, int *id, double charge, double mass,
                         const m3dk_f0_params *f0);
 
-/* sort_interval: 0 = m3dk_push never sorts; k > 0 = m3dk_push sorts before every k-th step (needs a sort workspace).
+/* sort_interval: 0 = m3dk_push never sorts: the caller's SoA arrays are pushed in place, one marker per thread (every
+ *       thread gathers its own element's coefficients: seven times slower per step at configs[3]).
+ *       k >= 1 = ordered pipeline (needs a sort workspace): m3dk_push packs the markers into element-ordered 64-byte
+ *       records at the start of a call (about one step's time at 2^24 markers, so sub-cycle many steps per call,
+ *       PAPER.md:237), runs EVERY step through the element-ordered kernel, re-orders after EVERY step (the histogram is
+ *       fused into the push; a re-ordering costs a tenth of a step) and unpacks at the end of the call.  k is a request
+ *       the library exceeds: k > 1 behaves like k = 1, and results are bit-identical for every value (0 included).
  * mode: 0 = linear delta-f (trajectories in the equilibrium field, (1 - w) -> 1);
  *       1 = non-linear trajectories (reading G21): the marker moves in the total fields,
  *           B = B0 + B1 and E-dagger = E1 - (mu/q) grad(|B|0 + B1par), and Eq. (8) keeps its factor (1 - w):
@@ -183,9 +189,20 @@ int m3dk_eval_fields(m3dk_ctx *ctx, long n, const double *R, const double *phi, 
  *   dX/dt = (1/B*par)[v_par B* + (mu/q) b x grad|B|],  m dv_par/dt = -(mu/B*par) B* . grad|B|,
  *   B* = B + (m v_par/q) curl b,  B*par = B* . b;  curl b from the second derivatives of psi0 and the first of F0.
  * The registered arrays x, y, z are read and written as the guiding-centre position X (Cartesian), mu is read, elem is
- * kept up to date; vx, vy, vz, w are not touched.  vpar: DEVICE [n], in/out.  nsteps classical RK4 steps of size dt.  A
- * guiding centre one of whose stages leaves the mesh is lost: state of the step before, elem = -1, frozen.  Asynchronous. */
+ * kept at the element of the CURRENT position (a following m3dk_push / m3dk_deposit uses it as it is); vx, vy, vz, w are
+ * not touched.  vpar: DEVICE [n], in/out.  nsteps classical RK4 steps of size dt.  A guiding centre is lost (elem = -1,
+ * frozen) when a stage of a step leaves the mesh (state of the step before) or a step ends outside (state after it).
+ * Asynchronous.                                                                                                      */
 int m3dk_gc_push(m3dk_ctx *ctx, int nsteps, double dt, double *vpar);
+
+/* Bootstrap of the slow-manifold Boris scheme ("we use RK4 to advance the guiding center equations of motion
+ * from x0 to x1, and then use (x1 - x0)/dt as v_1/2 to ensure that markers stay close to the slow manifold"; :82 a marker
+ * not initialised that way jumps back and forth across it).  One RK4 guiding-centre step of size dt from the registered
+ * positions with the parallel velocities vpar (DEVICE [n], read only); then x, y, z hold x_1 and vx, vy, vz hold
+ * (x_1 - x_0)/dt: the staggered state (x_l, v_{l-1/2}) m3dk_push takes, one step later in time (advance t0 by dt).  mu, w
+ * are untouched, elem is the element of x_1.  A marker whose step leaves the mesh is lost (elem = -1, state untouched).
+ * Asynchronous.                                                                                                      */
+int m3dk_gc_bootstrap(m3dk_ctx *ctx, double dt, const double *vpar);
 
 /* Moment deposition: right-hand sides of the Galerkin projection of the energetic-particle pressure
  * moments with a delta-function particle shape, Eqs. (17)-(18) (readings G10, G22):

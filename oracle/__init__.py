@@ -61,6 +61,7 @@ def _configure(L):
     L.orc_gc_push.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5 + [c_ip, C.c_int,
                               C.c_double, C.c_int]
     L.orc_gc_rhs.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5
+    L.orc_gc_bootstrap.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5 + [C.c_double] + [c_dp] * 3 + [c_ip]
     L.orc_gc_fields.argtypes = [C.c_void_p, C.POINTER(Analytic), C.c_long, c_dp, c_dp, c_ip, c_dp]
     L.orc_deposit.restype = C.c_long
     L.orc_deposit.argtypes = [C.c_void_p, C.POINTER(Species), C.c_long] + [c_dp] * 8 + [c_dp, C.c_int, C.c_double]
@@ -242,6 +243,20 @@ def gc_push(sp: Species, x, y, z, vpar, mu, nsteps: int, dt: float, *, mesh=None
                              *[a.ctypes.data_as(c_dp) for a in arrs], mu.ctypes.data_as(c_dp), e.ctypes.data_as(c_ip),
                              int(nsteps), float(dt), int(nthreads))
     return arrs[0], arrs[1], arrs[2], arrs[3], e, int(lost)
+
+
+def gc_bootstrap(sp: Species, x, y, z, vpar, mu, dt: float, *, mesh=None, an=None):
+    """one RK4 guiding-centre step x_0 -> x_1 and v_{1/2} = (x_1 - x_0)/dt.
+    Returns (x1, y1, z1, vx, vy, vz, ok); rows with ok False keep x_0 and have v = 0."""
+    pos = [np.array(a, dtype=np.float64, copy=True, order="C") for a in (x, y, z)]
+    vpar, mu = (np.ascontiguousarray(a, dtype=np.float64) for a in (vpar, mu))
+    n = pos[0].shape[0]
+    v = [np.zeros(n) for _ in range(3)]
+    ok = np.zeros(n, dtype=np.int32)
+    lib().orc_gc_bootstrap(mesh.h if mesh is not None else None, C.byref(an) if an is not None else None, C.byref(sp), n,
+                           *[a.ctypes.data_as(c_dp) for a in pos], vpar.ctypes.data_as(c_dp), mu.ctypes.data_as(c_dp),
+                           float(dt), *[a.ctypes.data_as(c_dp) for a in v], ok.ctypes.data_as(c_ip))
+    return pos[0], pos[1], pos[2], v[0], v[1], v[2], ok.astype(bool)
 
 
 def gc_rhs(sp: Species, R, Z, vpar, mu, *, mesh=None, an=None):

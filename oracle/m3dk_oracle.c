@@ -32,7 +32,8 @@
  * Mode 2 (finite Larmor radius; Eq. 14; reading G23): step 7 uses the quarter sum of the
  * perturbed fields over the four gyro-ring points (gyro_ring, flr_average); pins F1-F4.
  *
- * orc_gc_push: RK4 on the guiding-centre equations (1)-(4), equilibrium fields (reading G24); pins G1-G4.
+ * orc_gc_push: RK4 on the guiding-centre equations (1)-(4), equilibrium fields (reading G24); pins G1-G5.
+ * orc_gc_bootstrap: v_{1/2} = (x_1 - x_0)/dt from one such step; pin G6.
  *
  * orc_deposit: right-hand sides of Eqs. (17)-(18) with a delta-function shape (readings G10, G22).
  *
@@ -802,26 +803,31 @@ static int gc_rhs(const provider *pv, const orc_species *sp, double R, double Z,
     return e;
 }
 
-/* RK4 on y = (x, y, z, v_par) in Cartesian position; returns the element of the first stage (-1: lost, state frozen) */
-static int gc_step(const provider *pv, const orc_species *sp, double y[4], double mu, double dt)
+/* RK4 on y = (x, y, z, v_par) in Cartesian position.  Returns -1 when one of the four stages lies outside the mesh (the
+ * caller keeps the state of the step before: lost), otherwise the element of the NEW position (FE back-end; 0 for the
+ * analytic one), which is -1 as well when the step itself ends outside: then the new state is kept and the guiding centre
+ * is lost from there.  *stage_lost tells the two cases apart.                                                          */
+static int gc_step(const provider *pv, const orc_species *sp, double y[4], double mu, double dt, int *stage_lost)
 {
     double k[4][4], yy[4];
-    int e0 = 0;
     static const double cs[4] = {0.0, 0.5, 0.5, 1.0};
+    *stage_lost = 0;
     for (int st = 0; st < 4; ++st) {
         for (int i = 0; i < 4; ++i) yy[i] = y[i] + (st ? cs[st] * dt * k[st - 1][i] : 0.0);
         double R = sqrt(yy[0] * yy[0] + yy[1] * yy[1]), c = yy[0] / R, sn = yy[1] / R;
         double dX[3], dv;
         int e = gc_rhs(pv, sp, R, yy[2], yy[3], mu, dX, &dv);
-        if (e < 0) return -1;
-        if (st == 0) e0 = e;
+        if (e < 0) { *stage_lost = 1; return -1; }
         k[st][0] = dX[0] * c - dX[1] * sn; k[st][1] = dX[0] * sn + dX[1] * c; k[st][2] = dX[2]; k[st][3] = dv;
     }
     for (int i = 0; i < 4; ++i) y[i] += dt / 6.0 * (k[0][i] + 2.0 * k[1][i] + 2.0 * k[2][i] + k[3][i]);
-    return e0;
+    if (pv->kind != 0) return 0;
+    double Rn = sqrt(y[0] * y[0] + y[1] * y[1]);
+    return pv->brute ? locate_brute(pv->mesh, Rn, y[2]) : locate_grid(pv->mesh, Rn, y[2]);
 }
 
-/* n guiding centres nsteps RK4 steps; elem (optional out): element of the last step's first stage or -1 (lost, frozen) */
+/* n guiding centres nsteps RK4 steps; elem (optional out): element of the CURRENT position, -1 = lost (frozen): either a
+ * stage of a step left the mesh (state of the step before) or a step ended outside (state after that step)             */
 long orc_gc_push(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, long n, double *x, double *y, double *z,
                  double *vpar, const double *mu, int *elem, int nsteps, double dt, int nthreads)
 {
@@ -832,16 +838,41 @@ long orc_gc_push(const orc_mesh *m, const orc_analytic *a, const orc_species *sp
     for (long i = 0; i < n; ++i) {
         double s[4] = {x[i], y[i], z[i], vpar[i]};
         int e = 0, dead = 0;
+        if (m) {                                           /* element of the starting position */
+            e = locate_grid(m, sqrt(s[0] * s[0] + s[1] * s[1]), s[2]);
+            if (e < 0) dead = 1;
+        }
         for (int l = 0; l < nsteps && !dead; ++l) {
             double keep[4] = {s[0], s[1], s[2], s[3]};
-            e = gc_step(&pv, sp, s, mu[i], dt);
-            if (e < 0) { dead = 1; for (int q = 0; q < 4; ++q) s[q] = keep[q]; }
+            int stage_lost;
+            e = gc_step(&pv, sp, s, mu[i], dt, &stage_lost);
+            if (e < 0) { dead = 1; if (stage_lost) for (int q = 0; q < 4; ++q) s[q] = keep[q]; }
         }
         if (dead) { lost++; e = -1; }
         x[i] = s[0]; y[i] = s[1]; z[i] = s[2]; vpar[i] = s[3];
         if (elem) elem[i] = e;
     }
     return lost;
+}
+
+/* Bootstrap of the slow-manifold Boris scheme: "we use RK4 to advance the guiding center equations of motion
+ * (Eqs. (1-4)) from x_0 to x_1, and then use (x_1 - x_0)/dt as v_{1/2}".  One RK4 guiding-centre step of size dt from
+ * (x_0, v_par) with the equilibrium fields; on return the position is x_1 and v[3] = (x_1 - x_0)/dt: the pair
+ * (x_1, v_{1/2}) is the staggered state the Boris step takes (velocity half a step behind the position).  ok[i] = 0 when
+ * the step left the mesh (nothing is written for that marker).                                                        */
+void orc_gc_bootstrap(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, long n, double *x, double *y, double *z,
+                      const double *vpar, const double *mu, double dt, double *vx, double *vy, double *vz, int *ok)
+{
+    provider pv = {m ? 0 : 1, m, a, 0};
+    for (long i = 0; i < n; ++i) {
+        double s[4] = {x[i], y[i], z[i], vpar[i]};
+        int stage_lost;
+        int e = gc_step(&pv, sp, s, mu[i], dt, &stage_lost);
+        ok[i] = e >= 0;
+        if (e < 0) continue;
+        vx[i] = (s[0] - x[i]) / dt; vy[i] = (s[1] - y[i]) / dt; vz[i] = (s[2] - z[i]) / dt;
+        x[i] = s[0]; y[i] = s[1]; z[i] = s[2];
+    }
 }
 
 /* the field values gc_rhs works from, at given points, for the pins of poly_eval2 and of the finite-element branch of

@@ -81,6 +81,7 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_push_host": ([vp] + [vp] * 10 + [i, dbl, i], i),
         "m3dk_eval_fields": ([vp, lng, vp, vp, vp, dbl, vp, vp], i),
         "m3dk_gc_push": ([vp, i, dbl, vp], i),
+        "m3dk_gc_bootstrap": ([vp, dbl, vp], i),
         "m3dk_deposit_bytes": ([vp, C.POINTER(sz)], i),
         "m3dk_deposit": ([vp, vp, i, dbl], i),
         "m3dk_fp64_peak_tflops": ([vp, _c_dp], i),
@@ -333,6 +334,12 @@ class Pusher:
         self._keep["vpar"] = vp
         return (self.state_t["x"].cpu().numpy(), self.state_t["y"].cpu().numpy(), self.state_t["z"].cpu().numpy(),
                 vp.cpu().numpy(), self.elem_t.cpu().numpy())
+
+    def gc_bootstrap(self, dt: float, vpar):
+        """m3dk_gc_bootstrap: (x, v) <- (x_1, (x_1 - x_0)/dt) from one RK4 guiding-centre step; vpar is a numpy array."""
+        vp = self.torch.from_numpy(_np_d(vpar).copy()).to(self.device)
+        self._keep["vpar_boot"] = vp
+        self._ck(self.L.m3dk_gc_bootstrap(self.h, float(dt), self._p(vp)))
 
     def gc_push_into(self, nsteps: int, dt: float, vpar_t):
         """m3dk_gc_push on a caller's device tensor vpar [n] (asynchronous)."""

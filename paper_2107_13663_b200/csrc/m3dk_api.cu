@@ -426,9 +426,9 @@ extern "C" int m3dk_set_sort_workspace(m3dk_ctx *ctx, void *dev_workspace, size_
 // sort_interval = 0: the caller's SoA arrays are pushed in place, in whatever order they are (one marker per thread,
 // every thread gathers its own element's coefficients).
 // sort_interval = k >= 1: ordered pipeline.  At the start of the call the markers are packed into 64-byte records in
-// element order (a sort); every k-th step is followed by a re-ordering (histogram fused into the push, scan, work-item
-// cut, order list) and the step after an ordering runs the element-ordered kernel, the others the in-place kernel;
-// at the end of the call the records are unpacked into the caller's arrays (permuted; id[] says who is where).
+// element order (a sort); EVERY step runs the element-ordered kernel and is followed by a re-ordering (histogram fused
+// into the push, scan, work-item cut, order list); at the end of the call the records are unpacked into the caller's
+// arrays (permuted; id[] says who is where).  k > 1 is accepted and served as k = 1 (results are bit-identical).
 extern "C" int m3dk_sort(m3dk_ctx *ctx, void *dev_workspace, size_t bytes) {
     if (!ctx) return M3DK_EINVAL;
     if (!ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_sort: call m3dk_particles_init first");
@@ -462,8 +462,7 @@ static double step_time(m3dk_ctx *ctx, double dt) {
 
 // nsteps steps of the markers currently bound to the context (ctx->n, ctx->user, ctx->sb)
 static int run_steps(m3dk_ctx *ctx, int nsteps, double dt) {
-    const int k = ctx->sort_interval;
-    if (k == 0 || ctx->n == 0 || nsteps == 0) {
+    if (ctx->sort_interval == 0 || ctx->n == 0 || nsteps == 0) {
         for (int l = 0; l < nsteps; ++l) {
             const double t = step_time(ctx, dt);            // t_l of this step's x_l
             EvScope ev(ctx, &ctx->ev_push);
@@ -478,23 +477,23 @@ static int run_steps(m3dk_ctx *ctx, int nsteps, double dt) {
     }
     ctx->n_sorts++;
     ctx->steps_since_sort = 0;
-    bool ordered = true;     // the records are in element order and sb.items cut them
+    // Every step runs the element-ordered kernel and is followed by a re-ordering, whatever k >= 1 asks for: the ordering
+    // is fused into the push (histogram) and costs a tenth of a step, while a step on a stale order costs seven times one
+    // on a fresh order (markers cross 2-18 elements per step; measured in BASELINE.md section 4).
     for (int l = 0; l < nsteps; ++l) {
         const double t = step_time(ctx, dt);
-        const bool reorder_after = l + 1 < nsteps && ctx->steps_since_sort + 1 >= k;
+        const bool reorder_after = l + 1 < nsteps;
         {
             EvScope ev(ctx, &ctx->ev_push);
-            CU(launch_push_rec(ctx, ctx->n, dt, t, reorder_after, ordered), "push kernel");
+            CU(launch_push_rec(ctx, ctx->n, dt, t, reorder_after), "push kernel");
         }
-        ordered = false;     // the markers have moved
         ctx->steps_done++; ctx->steps_at_dt++;
-        ctx->steps_since_sort++;
+        ctx->steps_since_sort = 1;
         if (reorder_after) {
             EvScope ev(ctx, &ctx->ev_sort);
             CU(launch_reorder(ctx, ctx->n), "sort kernels (reorder)");
             ctx->n_sorts++;
             ctx->steps_since_sort = 0;
-            ordered = true;
         }
     }
     {
@@ -656,6 +655,15 @@ extern "C" int m3dk_gc_push(m3dk_ctx *ctx, int nsteps, double dt, double *vpar) 
     if (nsteps < 0 || !(dt == dt) || (ctx->n > 0 && !vpar)) return fail(ctx, M3DK_EINVAL, "m3dk_gc_push: nsteps < 0, dt is NaN or vpar is NULL");
     CU(cudaSetDevice(ctx->device), "cudaSetDevice");
     CU(launch_gc_push(ctx, ctx->n, vpar, nsteps, dt), "guiding-centre kernel");
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_gc_bootstrap(m3dk_ctx *ctx, double dt, const double *vpar) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_gc_bootstrap: fields and markers must be set first");
+    if (!(dt == dt) || dt == 0.0 || (ctx->n > 0 && !vpar)) return fail(ctx, M3DK_EINVAL, "m3dk_gc_bootstrap: dt is NaN or 0, or vpar is NULL");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CU(launch_gc_bootstrap(ctx, ctx->n, vpar, dt), "guiding-centre bootstrap kernel");
     return M3DK_OK;
 }
 

@@ -87,8 +87,32 @@ __device__ __forceinline__ bool gc_rhs(const FieldParams &f, double q, double m,
     return true;
 }
 
-// nsteps RK4 steps of y = (x, y, z, v_par); a guiding centre one of whose stages leaves the mesh is lost: its state is
-// the one before that step, elem = -1, frozen from then on (reading G12)
+// One RK4 step of y = (x, y, z, v_par).  false: one of the four stages lies outside the mesh (y is left untouched).
+__device__ __forceinline__ bool gc_rk4_step(const FieldParams &f, double q, double m, double mu, double dt, double (&y)[4]) {
+    double k[4][4], yy[4];
+    bool ok = true;
+#pragma unroll
+    for (int st = 0; st < 4; ++st) {
+        const double cs = st == 0 ? 0.0 : (st == 3 ? 1.0 : 0.5);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) yy[c] = st ? y[c] + cs * dt * k[st > 0 ? st - 1 : 0][c] : y[c];
+        const double r2 = yy[0] * yy[0] + yy[1] * yy[1];
+        const double rinv = m3dk_rsqrt(r2), R = r2 * rinv, c = yy[0] * rinv, sn = yy[1] * rinv;
+        double dX[3], dv;
+        int es;
+        if (ok && !gc_rhs(f, q, m, R, yy[2], yy[3], mu, dX, dv, es)) ok = false;
+        if (!ok) { dX[0] = dX[1] = dX[2] = 0.0; dv = 0.0; }
+        k[st][0] = dX[0] * c - dX[1] * sn; k[st][1] = dX[0] * sn + dX[1] * c; k[st][2] = dX[2]; k[st][3] = dv;
+    }
+    if (!ok) return false;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) y[c] += dt / 6.0 * (k[0][c] + 2.0 * k[1][c] + 2.0 * k[2][c] + k[3][c]);
+    return true;
+}
+
+// nsteps RK4 steps.  elem is kept at the element of the CURRENT position (every other entry point trusts it).  A guiding
+// centre is lost (elem = -1, frozen; reading G12) when a stage of a step leaves the mesh (it keeps the state of the step
+// before) or when a step ends outside (it keeps that state).
 __global__ void __launch_bounds__(128) gc_push_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, double *vpar,
                                                       long n, double q, double m, double dt, int nsteps) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -97,37 +121,44 @@ __global__ void __launch_bounds__(128) gc_push_kernel(const __grid_constant__ Fi
     if (e < 0) return;
     double y[4] = {a.x[i], a.y[i], a.z[i], vpar[i]};
     const double mu = a.mu[i];
-    for (int l = 0; l < nsteps; ++l) {
-        double k[4][4], yy[4];
-        bool ok = true;
-        int e0 = e;
-#pragma unroll
-        for (int st = 0; st < 4; ++st) {
-            const double cs = st == 0 ? 0.0 : (st == 3 ? 1.0 : 0.5);
-#pragma unroll
-            for (int c = 0; c < 4; ++c) yy[c] = st ? y[c] + cs * dt * k[st > 0 ? st - 1 : 0][c] : y[c];
-            const double r2 = yy[0] * yy[0] + yy[1] * yy[1];
-            const double rinv = m3dk_rsqrt(r2), R = r2 * rinv, c = yy[0] * rinv, sn = yy[1] * rinv;
-            double dX[3], dv;
-            int es;
-            if (ok && !gc_rhs(f, q, m, R, yy[2], yy[3], mu, dX, dv, es)) ok = false;
-            if (!ok) { dX[0] = dX[1] = dX[2] = 0.0; dv = 0.0; es = -1; }
-            if (st == 0) e0 = es;
-            k[st][0] = dX[0] * c - dX[1] * sn; k[st][1] = dX[0] * sn + dX[1] * c; k[st][2] = dX[2]; k[st][3] = dv;
-        }
-        if (!ok) { e = -1; break; }
-        e = e0;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) y[c] += dt / 6.0 * (k[0][c] + 2.0 * k[1][c] + 2.0 * k[2][c] + k[3][c]);
+    for (int l = 0; l < nsteps && e >= 0; ++l) {
+        if (!gc_rk4_step(f, q, m, mu, dt, y)) { e = -1; break; }
+        e = locate_xyz(f, y[0], y[1], y[2]);
     }
     a.x[i] = y[0]; a.y[i] = y[1]; a.z[i] = y[2]; vpar[i] = y[3];
     a.elem[i] = e;
+}
+
+// Bootstrap of the slow-manifold Boris scheme: one RK4 guiding-centre step x_0 -> x_1, then
+// (x, v) <- (x_1, (x_1 - x_0)/dt): the staggered state (x_l, v_{l-1/2}) m3dk_push starts from.  A marker whose step leaves
+// the mesh (a stage or the end point) is lost: elem = -1, state untouched.
+__global__ void __launch_bounds__(128) gc_bootstrap_kernel(const __grid_constant__ FieldParams f, MarkerArrays a,
+                                                           const double *vpar, long n, double q, double m, double dt) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (a.elem[i] < 0) return;
+    const double x0 = a.x[i], y0 = a.y[i], z0 = a.z[i];
+    double y[4] = {x0, y0, z0, vpar[i]};
+    int e = -1;
+    if (gc_rk4_step(f, q, m, a.mu[i], dt, y)) e = locate_xyz(f, y[0], y[1], y[2]);
+    a.elem[i] = e;
+    if (e < 0) return;
+    const double rdt = 1.0 / dt;
+    a.vx[i] = (y[0] - x0) * rdt; a.vy[i] = (y[1] - y0) * rdt; a.vz[i] = (y[2] - z0) * rdt;
+    a.x[i] = y[0]; a.y[i] = y[1]; a.z[i] = y[2];
 }
 
 cudaError_t launch_gc_push(m3dk_ctx *c, long n, double *vpar, int nsteps, double dt) {
     if (n == 0 || nsteps == 0) return cudaSuccess;
     c->kernel_launches += 1;
     gc_push_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, c->user, vpar, n, c->q, c->m, dt, nsteps);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gc_bootstrap(m3dk_ctx *c, long n, const double *vpar, double dt) {
+    if (n == 0) return cudaSuccess;
+    c->kernel_launches += 1;
+    gc_bootstrap_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, c->user, vpar, n, c->q, c->m, dt);
     return cudaGetLastError();
 }
 

@@ -182,7 +182,7 @@ namespace m3dk {
 // launchers (defined in push.cu / sort.cu); all enqueue on ctx->stream and return cudaGetLastError()
 cudaError_t launch_locate(m3dk_ctx *c, const MarkerArrays &a, long n, bool fill_id, int id_base = 0);
 cudaError_t launch_push_soa(m3dk_ctx *c, long n, double dt, double t);                           // caller's arrays, any order
-cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_hist, bool use_items);   // records
+cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_hist);   // records, element-ordered
 cudaError_t launch_eval_fields(m3dk_ctx *c, long n, const double *R, const double *phi, const double *Z, double t,
                                int *elem_out, double *out);
 cudaError_t launch_count_lost(m3dk_ctx *c, const MarkerArrays &a, long n, int *d_count);
@@ -191,6 +191,7 @@ cudaError_t launch_reorder(m3dk_ctx *c, long n);         // histogram of the las
 cudaError_t launch_unpack(m3dk_ctx *c, long n);          // records -> caller's arrays (+ elem, id)
 cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t);   // Eqs. (17)-(18) right-hand sides from the caller's arrays
 cudaError_t launch_gc_push(m3dk_ctx *c, long n, double *vpar, int nsteps, double dt);   // RK4 guiding-centre steps
+cudaError_t launch_gc_bootstrap(m3dk_ctx *c, long n, const double *vpar, double dt);     // (x_1, v_{1/2}) from one such step
 cudaError_t fp64_probe(m3dk_ctx *c, double *tflops);
 
 size_t sort_workspace_bytes(long n, int n_elems);

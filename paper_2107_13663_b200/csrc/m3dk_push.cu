@@ -24,23 +24,8 @@ __global__ void __launch_bounds__(256) locate_kernel(const __grid_constant__ Fie
     if (fill_id) a.id[i] = id_base + (int)i;
 }
 
-// Warp-aggregated histogram with returned ranks: lanes with the same key elect a leader that does one atomic.
-__device__ __forceinline__ int hist_rank(int *hist, int key, bool on) {
-    const unsigned live = __ballot_sync(0xffffffffu, on);
-    int r = 0;
-    if (on) {
-        const unsigned peers = __match_any_sync(live, key);
-        const int lane = threadIdx.x & 31;
-        const int leader = __ffs(peers) - 1;
-        int base = 0;
-        if (lane == leader) base = atomicAdd(hist + key, __popc(peers));
-        base = __shfl_sync(peers, base, leader);
-        r = base + __popc(peers & ((1u << lane) - 1u));
-    }
-    return r;
-}
-
-// The same for R keys per lane, in two halves: the atomics are issued as soon as the new keys exist, the returned
+// Warp-aggregated histogram with returned ranks for R keys per lane (lanes with the same key elect a leader that does
+// one atomic), in two halves: the atomics are issued as soon as the new keys exist, the returned
 // values are consumed (rank_finish) only after the next block of arithmetic, so their round trip to L2 is never waited for.
 template <int R>
 __device__ __forceinline__ void hist_issue(int *hist, const int (&key)[R], const bool (&on)[R], unsigned (&peers)[R],
@@ -435,34 +420,20 @@ __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, con
 }
 
 // ---- generic push: one marker per thread, any marker order (every thread gathers its own element's tile) ------------
-// kRec = false: the caller's SoA arrays in place (sort_interval = 0).  kRec = true: the records of the ordered pipeline
-// in place, for the steps between two sorts when sort_interval > 1.
-template <bool kRec, bool kHist, int kMode>
+// The caller's SoA arrays in place: sort_interval = 0, i.e. no sort workspace.
+template <int kMode>
 __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant__ PushParams P) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool valid = i < P.n;
-    int e = -1;
-    if (valid) { e = kRec ? P.rc.key[i] : P.a.elem[i]; if (kRec && e >= P.f.n_elems) e = -1; }
+    const int e = i < P.n ? P.a.elem[i] : -1;
     const long m[1] = {i};
     const bool on[1] = {e >= 0};             // lost markers are frozen (G12)
     // the tile loads may be speculated above the `on` tests: e is clamped to a valid element for addressing
     const double *tile = P.f.tiles + (size_t)max(e, 0) * P.f.tile_stride;
     if (__any_sync(0xffffffffu, on[0])) {
         double Rn[1], Zn[1];
-        if (kRec) {
-            const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems};
-            if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on, Rn, Zn);
-            else step_R<1, false, false, RecIO, kMode == 2>(P, io, tile, m, m, on, Rn, Zn);
-        } else {
-            const SoAIO io{P.a, P.f.n_elems};
-            if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on, Rn, Zn);
-            else step_R<1, false, false, SoAIO, kMode == 2>(P, io, tile, m, m, on, Rn, Zn);
-        }
-    }
-    if (kHist) {
-        const int k = valid ? P.rc.key[i] : 0;
-        const int rk = hist_rank(P.hist, k, valid);
-        if (valid) P.rank[i] = rk;
+        const SoAIO io{P.a, P.f.n_elems};
+        if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on, Rn, Zn);
+        else step_R<1, false, false, SoAIO, kMode == 2>(P, io, tile, m, m, on, Rn, Zn);
     }
 }
 
@@ -898,15 +869,15 @@ cudaError_t launch_push_soa(m3dk_ctx *c, long n, double dt, double t) {
     if (n == 0) return cudaSuccess;
     PushParams P = make_params(c, c->user, n, dt, t);
     c->kernel_launches += 1;
-    if (c->mode == 1) push_generic_kernel<false, false, 1><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
-    else if (c->mode == 2) push_generic_kernel<false, false, 2><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
-    else push_generic_kernel<false, false, 0><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
+    if (c->mode == 1) push_generic_kernel<1><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
+    else if (c->mode == 2) push_generic_kernel<2><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
+    else push_generic_kernel<0><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
     return cudaGetLastError();
 }
 
-// One step on the records: element-ordered (use_items: sb.rec[cur] gathered through sb.order[ocur] into sb.rec[cur ^ 1],
-// which becomes current) or in place.  with_hist: also histogram the new keys for the reorder that follows.
-cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_hist, bool use_items) {
+// One element-ordered step on the records: sb.rec[cur] gathered through sb.order[ocur] into sb.rec[cur ^ 1], which becomes
+// current.  with_hist: also histogram the new keys for the reorder that follows.
+cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_hist) {
     if (n == 0) return cudaSuccess;
     PushParams P = make_params(c, c->user, n, dt, t);
     c->kernel_launches += 1;
@@ -918,7 +889,7 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
         cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
         if (e != cudaSuccess) return e;
     }
-    if (use_items) {
+    {
         P.rc.out = c->sb.rec[c->cur ^ 1];
         P.items = c->sb.items; P.n_items = c->sb.ioffs + c->f.n_elems + 1;
         const unsigned grid = (unsigned)(c->sm_count * M3DK_PUSH_MINBLOCKS);
@@ -962,13 +933,6 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
             kern<<<small ? grid / M3DK_PUSH_MINBLOCKS * (M3DK_PUSH_MINBLOCKS + 1) : grid, kPushThreads, smem, c->stream>>>(P);
         }
         c->cur ^= 1;
-    } else {
-        P.rc.out = c->sb.rec[c->cur];
-        const unsigned grid = (unsigned)((n + 127) / 128);
-        auto kern = c->mode == 1   ? (with_hist ? push_generic_kernel<true, true, 1> : push_generic_kernel<true, false, 1>)
-                    : c->mode == 2 ? (with_hist ? push_generic_kernel<true, true, 2> : push_generic_kernel<true, false, 2>)
-                                   : (with_hist ? push_generic_kernel<true, true, 0> : push_generic_kernel<true, false, 0>);
-        kern<<<grid, 128, 0, c->stream>>>(P);
     }
     return cudaGetLastError();
 }

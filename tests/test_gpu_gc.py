@@ -44,8 +44,7 @@ def test_gc_push_matches_oracle(idx, nx, verify):
         live = e_ref >= 0
         assert live.mean() > 0.9
         assert np.array_equal(e_gpu < 0, e_ref < 0)
-        if nsteps == 1:
-            assert np.array_equal(e_gpu, e_ref)            # element of the step's first stage
+        assert np.array_equal(e_gpu, e_ref)                # element of the CURRENT position, step after step
         ex, ev = _err((gx, gy, gz, gv), (rx, ry, rz, rv), live)
         assert max(ex, ev) <= tol, (nsteps, ex, ev)
         st, _, _ = p.state(by_id=False)
@@ -70,3 +69,46 @@ def test_gc_lost_guiding_centres_are_frozen():
     assert np.allclose(gx[dead], rx[dead], rtol=1e-9) and np.allclose(gz[dead], rz[dead], rtol=1e-9, atol=1e-12)
     ex, ev = _err((gx, gy, gz, gv), (rx, ry, rz, rv), ~dead)
     assert max(ex, ev) <= 1e-9
+
+
+def test_gc_bootstrap_then_push_then_deposit_matches_the_oracle_chain():
+    """PAPER.md:80 on the device: m3dk_gc_bootstrap writes (x_1, (x_1 - x_0)/dt) and the element of x_1; a following
+    m3dk_push and m3dk_deposit trust that element (it used to be one step stale).  The same chain through the
+    oracle: gc_bootstrap -> push_fe -> deposit."""
+    w = synth.make_config(3, n_markers=6000 + 7, nx=64)
+    mesh, sp = oracle.Mesh.of(w), oracle.species_of(w)
+    mk, vp0 = w.markers, _vpar(w)
+    x1, y1, z1, vx, vy, vz, ok = oracle.gc_bootstrap(sp, mk["x"], mk["y"], mk["z"], vp0, mk["mu"], w.dt, mesh=mesh)
+    assert ok.mean() > 0.99
+    start = {k: v.copy() for k, v in mk.items()}
+    for k, a in (("x", x1), ("y", y1), ("z", z1)):
+        start[k] = a
+    for k, a in (("vx", vx), ("vy", vy), ("vz", vz)):
+        start[k] = np.where(ok, a, mk[k])
+    nsteps = 3
+    ref, e_ref, _ = oracle.push_fe(mesh, sp, start, nsteps, w.dt, t0=w.dt)
+    p = make_pusher(w, verify=True, sort_interval=1, t0=w.dt)
+    p.gc_bootstrap(w.dt, vp0)
+    got0, e0, _ = p.state()
+    assert np.array_equal(e0 >= 0, ok)
+    for k in ("x", "y", "z", "vx", "vy", "vz"):
+        assert np.allclose(got0[k][ok], start[k][ok], rtol=1e-12, atol=1e-13), k
+    R1 = np.hypot(start["x"], start["y"])
+    assert np.array_equal(e0[ok], mesh.locate(R1, start["z"])[ok])          # element of x_1, not of x_0
+    p.push(nsteps, w.dt)
+    got, e_gpu, _ = p.state()
+    live = (e_ref >= 0) & ok
+    from gpu_helpers import g16_errors, take
+    wrms = np.sqrt(np.mean(ref["w"][live] ** 2))
+    ex, ev, ew = g16_errors(take(got, live), take(ref, live), w_floor=wrms)
+    assert max(ex.max(), ev.max(), ew.max()) <= 1e-11, (ex.max(), ev.max(), ew.max())
+    # deposit after a guiding-centre push: bins by the element gc_push left behind
+    q = make_pusher(w, verify=True, sort_interval=1)
+    gx, gy, gz, gv, e_gc = q.gc_push(2, w.dt, vp0)
+    rhs = q.deposit(flags=0, t=0.0)
+    mk2 = {k: v.copy() for k, v in mk.items()}
+    rx, ry, rz, rv, e_or, _ = oracle.gc_push(sp, mk["x"], mk["y"], mk["z"], vp0, mk["mu"], 2, w.dt, mesh=mesh)
+    mk2["x"], mk2["y"], mk2["z"] = rx, ry, rz
+    want, _ = oracle.deposit(mesh, sp, mk2, 0, 0.0)
+    scale = np.abs(want).max()
+    assert np.abs(rhs - want).max() <= 1e-9 * scale
