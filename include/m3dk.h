@@ -214,7 +214,10 @@ int m3dk_gc_bootstrap(m3dk_ctx *ctx, double dt, const double *vpar);
  * rhs[e][1] also receives mu_p B1par(x_p, t) with B1par = Re[C e^{i(n phi - omega t)}] at the time t given; 0: Eq. (18) as
  * printed.  flags bit 1 (M3DK_DEPOSIT_FLR): 4-point FLR deposition: each marker deposits a quarter of its
  * amplitudes at each of its four gyro-ring points (the ring of mode 2, reading G23), test functions taken at the ring
- * point; a ring point outside the mesh deposits nothing.  The delta function is normalised in physical volume, so no Jacobian factor appears (G22); the mass-matrix solve that
+ * point; a ring point outside the mesh deposits nothing.  flags bit 2 (M3DK_DEPOSIT_BSTAR): w is replaced in both moments by
+ * d = w + B1star / Bstar (the linear form: the change of the phase-space Jacobian Bstar of Eq. 4), with B1star
+ * taken as B1par at the time t given and Bstar = (B0 + (m v_par/q) curl b0) . b0 at the v_par of the marker (reading G25).
+ * The delta function is normalised in physical volume, so no Jacobian factor appears (G22); the mass-matrix solve that
  * turns these sums into pressure coefficients belongs to the MHD code and is out of scope.  Lost markers deposit nothing.
  * rhs: DEVICE, m3dk_deposit_bytes() bytes = [n_elems][2][1 + 2 n_modes][21] doubles, overwritten.  Asynchronous.  The
  * caller's arrays are read, not modified.  With a sort workspace set (m3dk_set_sort_workspace) the markers are first
@@ -224,6 +227,7 @@ int m3dk_gc_bootstrap(m3dk_ctx *ctx, double dt, const double *vpar);
 int m3dk_deposit_bytes(const m3dk_ctx *ctx, size_t *bytes);
 #define M3DK_DEPOSIT_B1PAR 1
 #define M3DK_DEPOSIT_FLR 2
+#define M3DK_DEPOSIT_BSTAR 4
 int m3dk_deposit(m3dk_ctx *ctx, double *rhs, int flags, double t);
 
 /* Measured FP64 FMA throughput of the device (register-resident DFMA chains, all SMs), in TFLOP/s (FMA = 2 flop).

@@ -774,6 +774,27 @@ static int gc_fields(const provider *pv, double R, double Z, orc_gcf *g)
     return 0;
 }
 
+/* Eqs. (3)-(4) at (R, Z, v_par) from the field values g: b = B/|B| with |B| from its own table, curl b by the quotient rule
+ * (axisymmetric), B* = B + (m v_par/q) curl b and the phase-space Jacobian B*par = B* . b.                              */
+static double bstar(const orc_gcf *g, const orc_species *sp, double R, double vpar, double Bs[3], double b[3])
+{
+    double q = sp->charge, m = sp->mass;
+    double B[3] = {-g->psi_Z / R, g->F / R, g->psi_R / R};
+    double BR_R = -g->psi_RZ / R + g->psi_Z / (R * R), BR_Z = -g->psi_ZZ / R;
+    double BP_R = g->F_R / R - g->F / (R * R), BP_Z = g->F_Z / R;
+    double BZ_R = g->psi_RR / R - g->psi_R / (R * R), BZ_Z = g->psi_RZ / R;
+    double Bm = g->Bm;
+    for (int k = 0; k < 3; ++k) b[k] = B[k] / Bm;
+    double bR_Z = (BR_Z - b[0] * g->Bm_Z) / Bm;
+    double bP_R = (BP_R - b[1] * g->Bm_R) / Bm, bP_Z = (BP_Z - b[1] * g->Bm_Z) / Bm;
+    double bZ_R = (BZ_R - b[2] * g->Bm_R) / Bm;
+    (void)BR_R; (void)BZ_Z;
+    double curlb[3] = {-bP_Z, bR_Z - bZ_R, b[1] / R + bP_R};
+    double Bspar = 0.0;
+    for (int k = 0; k < 3; ++k) { Bs[k] = B[k] + (m * vpar / q) * curlb[k]; Bspar += Bs[k] * b[k]; }
+    return Bspar;
+}
+
 /* right-hand side of Eqs. (1)-(2) at (R, Z, v_par): dX/dt in cylindrical components, dv_par/dt.  Returns -1 outside. */
 static int gc_rhs(const provider *pv, const orc_species *sp, double R, double Z, double vpar, double mu, double dX[3],
                   double *dvpar)
@@ -782,20 +803,8 @@ static int gc_rhs(const provider *pv, const orc_species *sp, double R, double Z,
     int e = gc_fields(pv, R, Z, &g);
     if (e < 0) return -1;
     double q = sp->charge, m = sp->mass;
-    double B[3] = {-g.psi_Z / R, g.F / R, g.psi_R / R};
-    /* b = B / |B| with |B| from its own table; derivatives of b's components by the quotient rule */
-    double BR_R = -g.psi_RZ / R + g.psi_Z / (R * R), BR_Z = -g.psi_ZZ / R;
-    double BP_R = g.F_R / R - g.F / (R * R), BP_Z = g.F_Z / R;
-    double BZ_R = g.psi_RR / R - g.psi_R / (R * R), BZ_Z = g.psi_RZ / R;
-    double Bm = g.Bm;
-    double b[3] = {B[0] / Bm, B[1] / Bm, B[2] / Bm};
-    double bR_Z = (BR_Z - b[0] * g.Bm_Z) / Bm;
-    double bP_R = (BP_R - b[1] * g.Bm_R) / Bm, bP_Z = (BP_Z - b[1] * g.Bm_Z) / Bm;
-    double bZ_R = (BZ_R - b[2] * g.Bm_R) / Bm;
-    (void)BR_R; (void)BZ_Z;
-    double curlb[3] = {-bP_Z, bR_Z - bZ_R, b[1] / R + bP_R};
-    double Bs[3], Bspar = 0.0;
-    for (int k = 0; k < 3; ++k) { Bs[k] = B[k] + (m * vpar / q) * curlb[k]; Bspar += Bs[k] * b[k]; }
+    double Bs[3], b[3];
+    double Bspar = bstar(&g, sp, R, vpar, Bs, b);
     double gB[3] = {g.Bm_R, 0.0, g.Bm_Z};
     double bxg[3] = {b[1] * gB[2] - b[2] * gB[1], b[2] * gB[0] - b[0] * gB[2], b[0] * gB[1] - b[1] * gB[0]};
     for (int k = 0; k < 3; ++k) dX[k] = (vpar * Bs[k] + (mu / q) * bxg[k]) / Bspar;
@@ -914,7 +923,8 @@ void orc_gc_rhs(const orc_mesh *m, const orc_analytic *a, const orc_species *sp,
  * Plain loops, one marker at a time, in marker order.                                                             */
 /* flags bit 0: the perpendicular moment carries the term of Eq. (16), mu |B|0 (w + B1par/|B|0) = w mu |B|0 + mu B1par,
  * with B1par = Re[C e^{i(n phi - omega t)}] at time t ("the change of perpendicular pressure due to the variation of
- * B_par"); without it Eq. (18) as printed.                                                            */
+ * B_par"); without it Eq. (18) as printed.  flags bit 1: 4-point FLR deposition.  flags bit 2:
+ * d = w + B1par/B*par replaces w in both moments (reading G25).                                           */
 long orc_deposit(const orc_mesh *m, const orc_species *sp, long n, const double *x, const double *y, const double *z,
                  const double *vx, const double *vy, const double *vz, const double *mu, const double *w, double *rhs,
                  int flags, double t)
@@ -933,7 +943,19 @@ long orc_deposit(const orc_mesh *m, const orc_species *sp, long n, const double 
         double c = x[p] / R, sn = y[p] / R;
         double vc[3] = {vx[p] * c + vy[p] * sn, -vx[p] * sn + vy[p] * c, vz[p]};
         double vpar = (vc[0] * B0[0] + vc[1] * B0[1] + vc[2] * B0[2]) / B0n;
-        double a[2] = {w[p] * sp->mass * vpar * vpar, w[p] * mu[p] * f.Bm};
+        /* flags bit 2: "use d = w + (1 - w) B1* / B* to replace w in the summation in Eqs. (15) and (16) ... For a
+         * linear simulation, the definition of d is d = w + B1* / B*": the change of the phase-space Jacobian B* = B*par of
+         * Eq. (4).  B1* is taken as B1par (reading G25: the (m v_par/q)(b . curl b)_1 part of B1* needs curl B1, which the
+         * field tables do not carry, and is smaller by rho*); B*par from the equilibrium with this marker's v_par.        */
+        double dd = w[p];
+        if (flags & 4) {
+            provider pv = {0, m, NULL, 0};
+            orc_gcf g;
+            gc_fields(&pv, R, Z, &g);
+            double Bs[3], bb[3];
+            dd += f.B1p / bstar(&g, sp, R, vpar, Bs, bb);
+        }
+        double a[2] = {dd * sp->mass * vpar * vpar, dd * mu[p] * f.Bm};
         if (flags & 1) a[1] += mu[p] * f.B1p;
         /* deposition points: the marker itself, or (flags bit 1) the four gyro-ring points of reading G23
          * with a quarter of the amplitude each; a ring point outside the mesh deposits nothing                         */

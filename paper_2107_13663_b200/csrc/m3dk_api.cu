@@ -677,7 +677,7 @@ extern "C" int m3dk_deposit_bytes(const m3dk_ctx *ctx, size_t *bytes) {
 extern "C" int m3dk_deposit(m3dk_ctx *ctx, double *rhs, int flags, double t) {
     if (!ctx) return M3DK_EINVAL;
     if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_deposit: fields and markers must be set first");
-    if (!rhs || flags < 0 || flags > 3 || !(t == t)) return fail(ctx, M3DK_EINVAL, "m3dk_deposit: rhs is NULL, unknown flag or t is NaN");
+    if (!rhs || flags < 0 || flags > 7 || !(t == t)) return fail(ctx, M3DK_EINVAL, "m3dk_deposit: rhs is NULL, unknown flag or t is NaN");
     CU(cudaSetDevice(ctx->device), "cudaSetDevice");
     CU(launch_deposit(ctx, ctx->n, rhs, flags, t), "deposit kernel");
     return M3DK_OK;

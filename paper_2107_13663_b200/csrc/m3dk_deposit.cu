@@ -17,8 +17,9 @@ constexpr int kDepHarmMax = 1 + 2 * M3DK_MAX_MODES;
 // contributions of one marker: amp[0] = w m v_par^2, amp[1] = w mu |B|0; T[h]; xp[i] = xi^i, ep[j] = eta^j
 struct DepMarker { double amp[2], T[kDepHarmMax], xp[6], ep[6]; };
 
-// options of one deposition: with_b1par adds mu B1par (Eq. 16) to the perpendicular moment; cwt / swt = cos / sin(omega_k t)
-struct DepOpts { int with_b1par; double cwt[M3DK_MAX_MODES], swt[M3DK_MAX_MODES]; };
+// options of one deposition: with_b1par adds mu B1par (Eq. 16) to the perpendicular moment; with_bstar replaces w by
+// d = w + B1par / B*par in both moments (reading G25); cwt / swt = cos / sin(omega_k t); q = species charge
+struct DepOpts { int with_b1par, with_bstar; double q; double cwt[M3DK_MAX_MODES], swt[M3DK_MAX_MODES]; };
 
 __device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &o, int e, const Marker &s, double mass,
                                            DepMarker &d) {
@@ -38,10 +39,9 @@ __device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &
     const double binv = m3dk_rsqrt(M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, __dmul_rn(BZ, BZ))));
     const double vR = M3DK_FMA(s.vx, g.cph, __dmul_rn(s.vy, g.sph)), vP = M3DK_FMA(s.vy, g.cph, -__dmul_rn(s.vx, g.sph));
     const double vpar = __dmul_rn(M3DK_FMA(vR, BR, M3DK_FMA(vP, BP, __dmul_rn(s.vz, BZ))), binv);
-    d.amp[0] = __dmul_rn(__dmul_rn(s.w, mass), __dmul_rn(vpar, vpar));
-    d.amp[1] = __dmul_rn(__dmul_rn(s.w, s.mu), v[0][1]);
-    if (o.with_b1par) {   // Eq. (16): mu |B|0 (w + B1par/|B|0); B1par = Re[C e^{i(n phi - omega t)}] from quad 2 of every mode
-        double b1p = 0.0;
+    double b1p = 0.0;     // B1par = Re[C e^{i(n phi - omega t)}] from quad 2 of every mode
+    if (o.with_b1par || o.with_bstar) {
+        const double Bm0 = v[0][1];
         for (int md = 0; md < f.n_modes; ++md) {
             double cth, sth;
             mode_phase(f.n_tor[md], g.cph, g.sph, o.cwt[md], o.swt[md], cth, sth);
@@ -50,8 +50,18 @@ __device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &
             quad_vd<1, false>(pm, pm, ring, xi1, eta1, v, dx, de);
             b1p = __dadd_rn(b1p, re_part(v[0][0], v[0][1], cth, sth));
         }
-        d.amp[1] = M3DK_FMA(s.mu, b1p, d.amp[1]);
+        v[0][1] = Bm0;
     }
+    double dd = s.w;
+    if (o.with_bstar) {   // d = w + B1* / B* with B1* -> B1par and B* = B*par of Eq. (4) at this marker's v_par
+        GcEq ge;
+        gc_eq_fields(tile, g.R, s.z, ge);
+        double Bs[3], bb[3];
+        dd = __dadd_rn(dd, __dmul_rn(b1p, m3dk_rcp(bstar_par(ge, o.q, mass, vpar, Bs, bb))));
+    }
+    d.amp[0] = __dmul_rn(__dmul_rn(dd, mass), __dmul_rn(vpar, vpar));
+    d.amp[1] = __dmul_rn(__dmul_rn(dd, s.mu), v[0][1]);
+    if (o.with_b1par) d.amp[1] = M3DK_FMA(s.mu, b1p, d.amp[1]);   // Eq. (16): mu |B|0 (w + B1par/|B|0)
     d.T[0] = 1.0;     // toroidal factors by complex powers of (cos phi + i sin phi)
 #pragma unroll
     for (int md = 0; md < M3DK_MAX_MODES; ++md)
@@ -260,6 +270,8 @@ __global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constan
 cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t) {
     DepOpts o{};
     o.with_b1par = (flags & 1) && c->f.n_modes > 0;
+    o.with_bstar = (flags & 4) && c->f.n_modes > 0;
+    o.q = c->q;
     for (int k = 0; k < c->f.n_modes; ++k) { o.cwt[k] = cos(c->f.omega[k] * t); o.swt[k] = sin(c->f.omega[k] * t); }
     const size_t bytes = (size_t)c->f.n_elems * 2 * (1 + 2 * c->f.n_modes) * M3DK_NCOEF * sizeof(double);
     cudaError_t e = cudaMemsetAsync(rhs, 0, bytes, c->stream);

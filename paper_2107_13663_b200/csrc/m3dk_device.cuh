@@ -300,6 +300,80 @@ __device__ __forceinline__ void eval_fields(const FieldParams &f, int e, double 
     }
 }
 
+// value, first and second derivatives of the four polynomials of a quad at (xi, eta): nested Horner.  Row j of the
+// triangle is a polynomial in xi (value r, r', r''/2 by the three-term Horner recurrence); the rows are then combined by
+// the same recurrence in eta.  out[s] = {f, f_xi, f_eta, f_xixi, f_xieta, f_etaeta}.
+__device__ __forceinline__ void quad_d2(const double *__restrict__ c, double xi, double eta, double (&out)[4][6]) {
+    constexpr int kRow[6] = {0, 6, 11, 15, 18, 20};
+    double V[4], Ve[4], Vee[4], X[4], Xe[4], XX[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) V[s] = Ve[s] = Vee[s] = X[s] = Xe[s] = XX[s] = 0.0;
+#pragma unroll
+    for (int j = 5; j >= 0; --j) {
+        const int L = 6 - j;
+        double r[4] = {0.0, 0.0, 0.0, 0.0}, r1[4] = {0.0, 0.0, 0.0, 0.0}, r2[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+        for (int i = L - 1; i >= 0; --i) {
+            const Quad u = ldq(c + 4 * (kRow[j] + i));
+            const double uu[4] = {u.a, u.b, u.c, u.d};
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                r2[s] = M3DK_FMA(r2[s], xi, r1[s]);
+                r1[s] = M3DK_FMA(r1[s], xi, r[s]);
+                r[s] = M3DK_FMA(r[s], xi, uu[s]);
+            }
+        }
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            Vee[s] = M3DK_FMA(Vee[s], eta, Ve[s]);
+            Ve[s] = M3DK_FMA(Ve[s], eta, V[s]);
+            V[s] = M3DK_FMA(V[s], eta, r[s]);
+            Xe[s] = M3DK_FMA(Xe[s], eta, X[s]);
+            X[s] = M3DK_FMA(X[s], eta, r1[s]);
+            XX[s] = M3DK_FMA(XX[s], eta, r2[s]);
+        }
+    }
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+        out[s][0] = V[s]; out[s][1] = X[s]; out[s][2] = Ve[s];
+        out[s][3] = __dmul_rn(2.0, XX[s]); out[s][4] = Xe[s]; out[s][5] = __dmul_rn(2.0, Vee[s]);
+    }
+}
+
+// Equilibrium field values of the guiding-centre equations at (R, Z) in the element of `tile` (global memory), with the
+// second derivatives of psi0, and Eqs. (3)-(4): b = B/|B| (|B| from its own table), curl b by the quotient rule
+// (axisymmetric), B* = B + (m v_par/q) curl b, B*par = B* . b (the phase-space Jacobian).
+struct GcEq { double rinv, psi_R, psi_Z, psi_RR, psi_ZZ, Bm, Bm_R, Bm_Z, F, F_R, F_Z; };
+__device__ __forceinline__ void gc_eq_fields(const double *__restrict__ tile, double R, double Z, GcEq &g) {
+    const Quad hd = ldq(tile);
+    const double se = hd.c, xi = (R - hd.a) * se, eta = (Z - hd.b) * se;
+    double d[4][6];
+    quad_d2(tile + kTileHeader, xi, eta, d);                     // slots: psi0, |B|0, F0, kappa
+    const double s2 = se * se;
+    g.rinv = m3dk_rcp(R);
+    g.psi_R = d[0][1] * se; g.psi_Z = d[0][2] * se; g.psi_RR = d[0][3] * s2; g.psi_ZZ = d[0][5] * s2;
+    g.Bm = d[1][0]; g.Bm_R = d[1][1] * se; g.Bm_Z = d[1][2] * se;
+    g.F = d[2][0]; g.F_R = d[2][1] * se; g.F_Z = d[2][2] * se;
+}
+__device__ __forceinline__ double bstar_par(const GcEq &g, double q, double m, double vpar, double (&Bs)[3], double (&b)[3]) {
+    const double rinv = g.rinv, rinv2 = rinv * rinv;
+    const double B[3] = {-g.psi_Z * rinv, g.F * rinv, g.psi_R * rinv};
+    const double BR_Z = -g.psi_ZZ * rinv;
+    const double BP_R = g.F_R * rinv - g.F * rinv2, BP_Z = g.F_Z * rinv;
+    const double BZ_R = g.psi_RR * rinv - g.psi_R * rinv2;
+    const double binv = m3dk_rcp(g.Bm);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) b[k] = B[k] * binv;
+    const double bR_Z = (BR_Z - b[0] * g.Bm_Z) * binv;
+    const double bP_R = (BP_R - b[1] * g.Bm_R) * binv, bP_Z = (BP_Z - b[1] * g.Bm_Z) * binv;
+    const double bZ_R = (BZ_R - b[2] * g.Bm_R) * binv;
+    const double curlb[3] = {-bP_Z, bR_Z - bZ_R, b[1] * rinv + bP_R};
+    const double mvq = m * vpar / q;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) Bs[k] = B[k] + mvq * curlb[k];
+    return Bs[0] * b[0] + Bs[1] * b[1] + Bs[2] * b[2];
+}
+
 // d ln f0 / dE at fixed (P_phi, mu) (G7)
 __device__ __forceinline__ double kappa_E(const PushParams &P, double Ekin, double mu) {
     if (P.f0kind == M3DK_F0_MAXWELLIAN) return -P.f0T_inv;

@@ -9,46 +9,6 @@
 
 namespace m3dk {
 
-// value, first and second derivatives of the four polynomials of a quad at (xi, eta): nested Horner.  Row j of the
-// triangle is a polynomial in xi (value r, r', r''/2 by the three-term Horner recurrence); the rows are then combined by
-// the same recurrence in eta.  out[s] = {f, f_xi, f_eta, f_xixi, f_xieta, f_etaeta}.
-__device__ __forceinline__ void quad_d2(const double *__restrict__ c, double xi, double eta, double (&out)[4][6]) {
-    constexpr int kRow[6] = {0, 6, 11, 15, 18, 20};
-    double V[4], Ve[4], Vee[4], X[4], Xe[4], XX[4];
-#pragma unroll
-    for (int s = 0; s < 4; ++s) V[s] = Ve[s] = Vee[s] = X[s] = Xe[s] = XX[s] = 0.0;
-#pragma unroll
-    for (int j = 5; j >= 0; --j) {
-        const int L = 6 - j;
-        double r[4] = {0.0, 0.0, 0.0, 0.0}, r1[4] = {0.0, 0.0, 0.0, 0.0}, r2[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-        for (int i = L - 1; i >= 0; --i) {
-            const Quad u = ldq(c + 4 * (kRow[j] + i));
-            const double uu[4] = {u.a, u.b, u.c, u.d};
-#pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                r2[s] = M3DK_FMA(r2[s], xi, r1[s]);
-                r1[s] = M3DK_FMA(r1[s], xi, r[s]);
-                r[s] = M3DK_FMA(r[s], xi, uu[s]);
-            }
-        }
-#pragma unroll
-        for (int s = 0; s < 4; ++s) {
-            Vee[s] = M3DK_FMA(Vee[s], eta, Ve[s]);
-            Ve[s] = M3DK_FMA(Ve[s], eta, V[s]);
-            V[s] = M3DK_FMA(V[s], eta, r[s]);
-            Xe[s] = M3DK_FMA(Xe[s], eta, X[s]);
-            X[s] = M3DK_FMA(X[s], eta, r1[s]);
-            XX[s] = M3DK_FMA(XX[s], eta, r2[s]);
-        }
-    }
-#pragma unroll
-    for (int s = 0; s < 4; ++s) {
-        out[s][0] = V[s]; out[s][1] = X[s]; out[s][2] = Ve[s];
-        out[s][3] = __dmul_rn(2.0, XX[s]); out[s][4] = Xe[s]; out[s][5] = __dmul_rn(2.0, Vee[s]);
-    }
-}
-
 // right-hand side of Eqs. (1)-(2) at (R, Z, v_par): dX/dt in cylindrical components, dv_par/dt; false outside the mesh
 __device__ __forceinline__ bool gc_rhs(const FieldParams &f, double q, double m, double R, double Z, double vpar, double mu,
                                        double (&dX)[3], double &dv, int &elem) {
@@ -56,28 +16,11 @@ __device__ __forceinline__ bool gc_rhs(const FieldParams &f, double q, double m,
     elem = e;
     if (e < 0) return false;
     const double *tile = f.tiles + (size_t)e * f.tile_stride;
-    const Quad hd = ldq(tile);
-    const double se = hd.c, xi = (R - hd.a) * se, eta = (Z - hd.b) * se;
-    double d[4][6];
-    quad_d2(tile + kTileHeader, xi, eta, d);                     // slots: psi0, |B|0, F0, kappa
-    const double s2 = se * se, rinv = m3dk_rcp(R), rinv2 = rinv * rinv;
-    const double psi_R = d[0][1] * se, psi_Z = d[0][2] * se, psi_RR = d[0][3] * s2, psi_RZ = d[0][4] * s2, psi_ZZ = d[0][5] * s2;
-    const double Bm = d[1][0], Bm_R = d[1][1] * se, Bm_Z = d[1][2] * se;
-    const double F = d[2][0], F_R = d[2][1] * se, F_Z = d[2][2] * se;
-    const double B[3] = {-psi_Z * rinv, F * rinv, psi_R * rinv};
-    const double BR_Z = -psi_ZZ * rinv;
-    const double BP_R = F_R * rinv - F * rinv2, BP_Z = F_Z * rinv;
-    const double BZ_R = psi_RR * rinv - psi_R * rinv2;
-    (void)psi_RZ;
-    const double binv = m3dk_rcp(Bm);
-    const double b[3] = {B[0] * binv, B[1] * binv, B[2] * binv};
-    const double bR_Z = (BR_Z - b[0] * Bm_Z) * binv;
-    const double bP_R = (BP_R - b[1] * Bm_R) * binv, bP_Z = (BP_Z - b[1] * Bm_Z) * binv;
-    const double bZ_R = (BZ_R - b[2] * Bm_R) * binv;
-    const double curlb[3] = {-bP_Z, bR_Z - bZ_R, b[1] * rinv + bP_R};
-    const double mvq = m * vpar / q;
-    const double Bs[3] = {B[0] + mvq * curlb[0], B[1] + mvq * curlb[1], B[2] + mvq * curlb[2]};
-    const double Bspar = Bs[0] * b[0] + Bs[1] * b[1] + Bs[2] * b[2];
+    GcEq g;
+    gc_eq_fields(tile, R, Z, g);
+    double Bs[3], b[3];
+    const double Bspar = bstar_par(g, q, m, vpar, Bs, b);
+    const double Bm_R = g.Bm_R, Bm_Z = g.Bm_Z;
     const double bsinv = m3dk_rcp(Bspar);
     const double muq = mu / q;
     const double bxg[3] = {b[1] * Bm_Z, b[2] * Bm_R - b[0] * Bm_Z, -b[1] * Bm_R};     // b x grad|B|, grad|B| = (Bm_R, 0, Bm_Z)

@@ -125,3 +125,31 @@ def test_deposit_without_sort_workspace_uses_the_callers_arrays():
         ref, _ = oracle.deposit(mesh, sp, mk, flags=flags, t=1.3)
         got = p.deposit(flags=flags, t=1.3)
         assert np.abs(got - ref).max() <= 1e-11 * np.abs(ref).max(), flags
+
+
+@pytest.mark.parametrize("flags", [4, 5, 6, 7])
+@pytest.mark.parametrize("si", [0, 1])
+def test_deposit_with_the_jacobian_substitution(flags, si):
+    """flags bit 2 (M3DK_DEPOSIT_BSTAR): d = w + B1par/B*par replaces w, alone and together with the B1par
+    term of Eq. (16) and the 4-point FLR deposition; element-ordered (items kernel) and caller order."""
+    w = synth.make_config(3, n_markers=30000 + 11, nx=32, amp=1e-2)
+    rng = np.random.Generator(np.random.PCG64(9))
+    mk = {k: v.copy() for k, v in w.markers.items()}
+    mk["w"] = rng.normal(size=w.n_markers) * 1e-2
+    w = dataclasses.replace(w, markers=mk)
+    p = make_pusher(w, verify=True, sort_interval=si)
+    if si:
+        p.sort()
+    raw, elem, ids = p.state(by_id=False)
+    mesh, sp = oracle_of(w)
+    t = 0.7
+    ref, lost = oracle.deposit(mesh, sp, raw, flags=flags, t=t)
+    absw = dict(raw)
+    absw["w"] = np.abs(raw["w"]) + 2e-2                        # |w| + a bound of |B1par / B*par| (amplitude 1e-2 B0)
+    scale, _ = oracle.deposit(mesh, sp, absw, flags=flags & 2)
+    S = np.abs(scale[:, :, 0, 0])[:, :, None, None] + np.abs(scale).max() * 1e-3
+    got = p.deposit(flags=flags, t=t)
+    err = np.abs(got - ref)
+    assert (err <= 1e-11 * S).all(), float((err / S).max())
+    base, _ = oracle.deposit(mesh, sp, raw, flags=flags & 3, t=t)
+    assert np.abs(ref - base).max() > 1e-4 * np.abs(base).max()          # the substitution does change the table

@@ -188,3 +188,71 @@ def test_d6_four_point_flr_deposition(orc):
         zmom = lambda r: (r[:, mom, 0, 6] / se + cen[:, 1] * r[:, mom, 0, 0]).sum()
         assert abs(zmom(flr) - zmom(plain)) < 1e-10 * scale
     assert np.abs(flr[:, 1, 0, 0] - plain[:, 1, 0, 0]).max() > 1e-3 * np.abs(plain[:, 1, 0, 0]).max()   # but it is spread out
+
+
+# ---- D7: d = w + B1*/B* replaces w (reading G25) ----------------------------------------------------------
+def check_d7_jacobian_substitution(orc):
+    """flags bit 2.  (a) Zero amplitude: the tables of pin D1 with the perturbation switched off give exactly the flags = 0
+    result.  (b) Closed form on hand-made tables: psi0 = A R^2 / 2, F = 0, |B|0 = A is a uniform vertical field (curl b = 0,
+    B*par = |B| = A) and B1par = eps A a uniform compression: d = w + eps, so the unit test function sums to
+    sum_p (w_p + eps) m v_par^2 and sum_p (w_p + eps) mu A.  (c) With curl b: the quintic tables of the analytic equilibrium,
+    B*par = |B| + (m v_par/q) b . curl b computed HERE from the analytic field by central differences; the extra deposit
+    sum_p mu |B| B1par / B*par agrees to the fit error, and fails when the curl b term is dropped (it is 0.1 % of |B|)."""
+    from handmade import HandMade
+    from synth.configs import CHARGE, MASS
+    rng = np.random.Generator(np.random.PCG64(12))
+    # (a)
+    w0 = synth.make_config(1, n_markers=3000, nx=16, amp=0.0)
+    mk = _weights(w0)
+    r0, _ = orc.deposit(orc.Mesh.of(w0), orc.species_of(w0), mk, 0)
+    r4, _ = orc.deposit(orc.Mesh.of(w0), orc.species_of(w0), mk, 4)
+    assert np.array_equal(r0, r4)
+    # (b)
+    A, eps, n = 0.8, 3.0e-3, 4000
+    hm = HandMade(eq=dict(psi=(0.0, 0.0, 0.0, 0.5 * A), Bm=(A,), F=(0.0,), kappa=(0.0,)), pert=dict(B_par=(eps * A,)), n_tor=0)
+    R, phi, Z = rng.uniform(2.0, 4.0, n), rng.uniform(-3, 3, n), rng.uniform(-1.0, 1.0, n)
+    m2 = dict(x=R * np.cos(phi), y=R * np.sin(phi), z=Z, vx=rng.normal(size=n), vy=rng.normal(size=n), vz=rng.normal(size=n),
+              mu=rng.uniform(0, 0.02, n), w=rng.normal(size=n) * 1e-3)
+    sp = orc.species(CHARGE, MASS)
+    rhs, lost = orc.deposit(hm.oracle_mesh(orc), sp, m2, 4)
+    assert lost == 0
+    par = ((m2["w"] + eps) * MASS * m2["vz"] ** 2).sum()           # b0 = +Z: v_par = vz
+    perp = ((m2["w"] + eps) * m2["mu"] * A).sum()
+    assert abs(rhs[:, 0, 0, 0].sum() - par) <= 1e-12 * np.abs((np.abs(m2["w"]) + eps) * MASS * m2["vz"] ** 2).sum()
+    assert abs(rhs[:, 1, 0, 0].sum() - perp) <= 1e-12 * ((np.abs(m2["w"]) + eps) * m2["mu"] * A).sum()
+    # (c)
+    w1 = synth.make_config(3, n_markers=12000, nx=32, amp=1e-2)
+    mesh, sp1 = orc.Mesh.of(w1), orc.species_of(w1)
+    t = 0.4
+    eq = w1.eq
+    h = 2e-4
+
+    def bhat(r, z):
+        B = np.array(eq.B_cyl(r, z))
+        return B / np.sqrt((B ** 2).sum(axis=0))
+
+    def analytic(mk):
+        R = np.hypot(mk["x"], mk["y"])
+        _, fe = mesh.eval(R, np.arctan2(mk["y"], mk["x"]), mk["z"], t)
+        b = bhat(R, mk["z"])
+        dbR, dbZ = (bhat(R + h, mk["z"]) - bhat(R - h, mk["z"])) / (2 * h), (bhat(R, mk["z"] + h) - bhat(R, mk["z"] - h)) / (2 * h)
+        curl = np.array([-dbZ[1], dbZ[0] - dbR[2], b[1] / R + dbR[1]])
+        c, s = mk["x"] / R, mk["y"] / R
+        vpar = (mk["vx"] * c + mk["vy"] * s) * b[0] + (-mk["vx"] * s + mk["vy"] * c) * b[1] + mk["vz"] * b[2]
+        Babs = np.sqrt(sum(x ** 2 for x in eq.B_cyl(R, mk["z"])))
+        return fe[:, 17], fe[:, 2], vpar, Babs, Babs + (w1.mass * vpar / w1.charge) * (b * curl).sum(axis=0)
+    B1p, _, vpar, _, _ = analytic(w1.markers)
+    # the markers on which the curl b correction (proportional to v_par) has one sign, so that it does not cancel in a sum
+    keep = (B1p * vpar > 0) & (np.abs(vpar) > 0.3)
+    mk = {k: v[keep].copy() for k, v in w1.markers.items()}        # w = 0: only the B1par / B*par part deposits
+    B1p, Bm, vpar, Babs, Bstar = analytic(mk)
+    rhs, _ = orc.deposit(mesh, sp1, mk, 4, t)
+    for mom, amp in ((0, w1.mass * vpar ** 2), (1, mk["mu"] * Bm)):
+        want, without_curl = (amp * B1p / Bstar).sum(), (amp * B1p / Babs).sum()
+        got = rhs[:, mom, 0, 0].sum()
+        assert abs(got - want) < 1e-5 * abs(want), (mom, got, want)
+        assert abs(without_curl - want) > 1e-4 * abs(want), (mom, without_curl, want)      # the pin tells the two apart
+
+
+def test_d7_jacobian_substitution(orc):
+    check_d7_jacobian_substitution(orc)

@@ -1,4 +1,5 @@
-"""Mutation checks of the pins M1-M3, N1, Q1, Q2 (tests/test_oracle_magnetic.py) and G5 (tests/test_oracle_gc.py).
+"""Mutation checks of the pins M1-M3, N1, Q1, Q2 (tests/test_oracle_magnetic.py), G5, G6 (tests/test_oracle_gc.py) and D7
+(tests/test_oracle_deposit.py).
 
 Each case compiles a COPY of oracle/m3dk_oracle.c with one plausible mistake (a flipped sign, a dropped factor, a wrong
 index) into a temporary directory, routes the oracle binding to that copy and asserts that the named pin FAILS -- the
@@ -7,9 +8,10 @@ evidence that the pin would catch that mistake.  The oracle itself is never modi
 import pytest
 
 from test_oracle_gc import check_g5_phase_space_volume, check_g6_bootstrap
+from test_oracle_deposit import check_d7_jacobian_substitution
 from test_oracle_magnetic import CHECKS as _MAGNETIC
 
-CHECKS = dict(_MAGNETIC, g5=check_g5_phase_space_volume, g6=check_g6_bootstrap)
+CHECKS = dict(_MAGNETIC, g5=check_g5_phase_space_volume, g6=check_g6_bootstrap, d7=check_d7_jacobian_substitution)
 
 #        pin   tag                      text in the oracle source                         mutated text
 MUTANTS = [
@@ -38,6 +40,8 @@ MUTANTS = [
     ("q2", "curlb_Z_term", "b[1] / R + bP_R};", "bP_R};"),
     ("g5", "curlb_phi_sign", "double curlb[3] = {-bP_Z, bR_Z - bZ_R,", "double curlb[3] = {-bP_Z, bZ_R - bR_Z,"),
     ("g5", "Bstar_par", "Bspar += Bs[k] * b[k]; }", "Bspar += B[k] * b[k]; }"),
+    ("d7", "jacobian_sign", "dd += f.B1p / bstar(&g, sp, R, vpar, Bs, bb);", "dd -= f.B1p / bstar(&g, sp, R, vpar, Bs, bb);"),
+    ("d7", "jacobian_without_curl_b", "dd += f.B1p / bstar(&g, sp, R, vpar, Bs, bb);", "dd += f.B1p / g.Bm;"),
     ("g6", "bootstrap_sign", "vx[i] = (s[0] - x[i]) / dt;", "vx[i] = (x[i] - s[0]) / dt;"),
     ("g6", "bootstrap_keeps_x0", "x[i] = s[0]; y[i] = s[1]; z[i] = s[2];\n    }\n}", "\n    }\n}"),
     ("q1", "psi_ZZ_dropped", "g->psi_ZZ = d * s * s;", "g->psi_ZZ = 0.0 * d;"),
