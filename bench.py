@@ -161,19 +161,21 @@ def oracle_sample_rate(w, sample_stride: int, nsteps: int, nthreads: int = 0):
     return n * nsteps / dt, n, dt, oracle.max_threads() if nthreads == 0 else nthreads
 
 
-def build_workload(args, rank: int):
+def build_workload(args, rank: int, tables: bool = True):
     import synth
     from paper_2107_13663_b200 import shard
-    # every rank draws its own shard (seed offset by rank): independent markers, same tables
+    # every rank draws its own shard (seed offset by rank): independent markers.  Only rank 0 fits
+    # the field tables; the other ranks receive the packed field image from it
     return synth.make_config(args.config, n_markers=args.n_markers, nx=args.nx, dt_gyro=args.dt_gyro,
-                             seed=shard.shard_seed(args.config, rank))
+                             seed=shard.shard_seed(args.config, rank), tables=tables)
 
 
 def config_dict(args, w, sort_interval, world):
     return {"workload": f"BASELINE.json configs[{args.config}] ({w.name})", "n_markers_per_gpu": w.n_markers,
             "mesh": f"{w.nx}x{w.nx} cells, {w.n_elems} triangles", "n_modes": w.n_modes, "dt": w.dt,
             "sort_interval": sort_interval, "mode": ("linear delta-f", "non-linear trajectories", "linear delta-f + FLR 4-point average")[args.mode],
-            "parallelism": f"{world} independent marker shard(s), no collective",
+            "parallelism": (f"{world} independent marker shard(s), no collective in the push" +
+                            ("; field image broadcast from rank 0 (NCCL)" if world > 1 else "")),
             "l2": "inputs larger than L2 (marker state %.0f MB + tables %.0f MB per GPU)" % (
                 w.n_markers * 64 / 1e6, (w.eq_coef.nbytes + w.pert_coef.nbytes) / 1e6)}
 
@@ -206,16 +208,22 @@ def run_ours(args, rank, world, local_rank):
         raise SystemExit("bench.py: no CUDA device (libm3dk has no CPU fallback)")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    m3dk.build_all()
-    w = build_workload(args, rank)
-    # decision D-c: the ordering interval is a tuning knob with bit-identical results; workloads
-    # that sort at all run the fused ordering every step unless --sort-interval says otherwise
+    from paper_2107_13663_b200 import shard
+    if rank == 0:
+        m3dk.build_all()                 # one rank compiles (if the library is stale); the others wait and load it
+    if world > 1:
+        dist.barrier()
+    w = build_workload(args, rank, tables=(rank == 0))
+    # decision D-c: workloads that sort at all run the ordered pipeline, which orders every step
     si = (1 if w.sort_interval > 0 else 0) if args.sort_interval is None else args.sort_interval
     N, K, W = w.n_markers, args.steps, args.warmup
 
     p = m3dk.Pusher(device=local_rank, verify=False)
-    p.fields_create(w.node_RZ, w.tri, w.eq_coef, w.n_tor if w.n_modes else None, w.omega if w.n_modes else None,
-                    w.pert_coef if w.n_modes else None)
+    if rank == 0:
+        p.fields_create(w.node_RZ, w.tri, w.eq_coef, w.n_tor if w.n_modes else None, w.omega if w.n_modes else None,
+                        w.pert_coef if w.n_modes else None)
+    if world > 1:
+        shard.broadcast_fields(p, dist, w.n_elems, w.n_modes, src=0)
     p.particles_init(w.markers, w.charge, w.mass, w.f0)
     p.set_options(sort_interval=si, mode=args.mode, t0=0.0)
     p.set_push_variant(args.push_variant)
@@ -260,8 +268,24 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     ms_e2e = f0.elapsed_time(f1)
 
-    from paper_2107_13663_b200 import shard
     ms, ms_e2e = shard.max_over_ranks([ms, ms_e2e], dist if world > 1 else None, device=dev)
+    dep = None
+    if args.deposit:
+        # row (f)-4 with its exchange step: every rank deposits its shard, the moment tables are summed over the ranks
+        need = p.deposit_bytes()
+        rhs = torch.empty(need // 8, dtype=torch.float64, device=dev)
+        p.deposit_into(rhs, 1, 0.0)
+        shard.allreduce_moments(rhs, dist if world > 1 else None)
+        barrier()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(p.stream)
+        for _ in range(5):
+            p.deposit_into(rhs, 1, 0.0)
+            shard.allreduce_moments(rhs, dist if world > 1 else None)
+        d1.record(p.stream)
+        barrier()
+        dms, = shard.max_over_ranks([d0.elapsed_time(d1) / 5], dist if world > 1 else None, device=dev)
+        dep = (dms, need)
     if rank != 0:
         return
 
@@ -311,23 +335,13 @@ def run_ours(args, rank, world, local_rank):
         gms = g0.elapsed_time(g1) / 10
         line["gc"] = {"ms_per_step": gms, "particle_steps_per_s": N / (gms * 1e-3),
                       "note": "m3dk_gc_push, RK4 on Eqs. (1)-(4), equilibrium fields (SURVEY.md 8(f)-3); 4 field evaluations per step"}
-    if args.deposit:
-        # row (f)-4: one deposition of the pressure moments from the element-ordered arrays the push left behind
-        need = p.deposit_bytes()
-        rhs = torch.empty(need // 8, dtype=torch.float64, device=dev)
-        p.deposit_into(rhs, 1, 0.0)
-        torch.cuda.synchronize(dev)
-        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        d0.record(p.stream)
-        for _ in range(5):
-            p.deposit_into(rhs, 1, 0.0)
-        d1.record(p.stream)
-        torch.cuda.synchronize(dev)
-        dms = d0.elapsed_time(d1) / 5
+    if dep is not None:
+        dms, need = dep
         dbytes = (68.0 * N + need)            # 8 fp64 + element key per marker read, the table cleared and accumulated
-        line["deposit"] = {"ms": dms, "markers_per_s": N / (dms * 1e-3), "table_bytes": need,
+        line["deposit"] = {"ms": dms, "markers_per_s": N * world / (dms * 1e-3), "table_bytes": need,
                            "hbm_bytes": dbytes, "hbm_frac": dbytes / (dms * 1e-3) / (hbm_gbs * 1e9),
-                           "note": "m3dk_deposit with the B1par term of Eq. (16), delta-function shape (SURVEY.md 8(f)-4)"}
+                           "note": "m3dk_deposit with the B1par term of Eq. (16), delta-function shape (SURVEY.md 8(f)-4)" +
+                                   (f", then NCCL all-reduce of the {need} B table over {world} ranks" if world > 1 else "")}
     if world == 1 and not args.no_cpu_baseline:
         rate, n, secs, cores, stride, rsteps = oracle_bounded_sample(w, args.ref_sample)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",

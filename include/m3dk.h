@@ -105,6 +105,13 @@ int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node_RZ, int n_
                        const double *eq_coef, int n_modes, const int *n_tor, const double *omega,
                        const double *pert_coef, void *dev_workspace, size_t workspace_bytes);
 
+/* A fields workspace is self-describing: a byte-for-byte copy of it (on this or another GPU: a peer copy, an NCCL broadcast)
+ * can be bound to a context without the host tables and without repeating the host-side repack.  This is how the whole-mesh
+ * field replica of PAPER.md:235 ("collected and uploaded to every GPU") reaches the other GPUs of a node: rank 0 calls
+ * m3dk_fields_create, the workspace is broadcast, every other rank calls m3dk_fields_attach on its copy.  dev_workspace:
+ * DEVICE, 256-byte aligned, borrowed like the one of m3dk_fields_create.  Synchronises (reads the header in the control block).      */
+int m3dk_fields_attach(m3dk_ctx *ctx, void *dev_workspace, size_t workspace_bytes);
+
 /* ---- markers: SoA fp64 x, v, mu, w; species charge / mass -------------------------------------
  * x..w: DEVICE arrays of n doubles, caller-owned, updated in place by push and permuted by sort.
  * elem: DEVICE int[n], library-managed: the element of each marker's current position (-1 = lost).

@@ -68,6 +68,7 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_last_error": ([vp], C.c_char_p),
         "m3dk_fields_workspace_bytes": ([i, i, i, C.POINTER(sz)], i),
         "m3dk_fields_create": ([vp, i, _c_dp, i, _c_ip, _c_dp, i, _c_ip, _c_dp, _c_dp, vp, sz], i),
+        "m3dk_fields_attach": ([vp, vp, sz], i),
         "m3dk_particles_init": ([vp, lng] + [vp] * 10 + [dbl, dbl, C.POINTER(_F0)], i),
         "m3dk_set_options": ([vp, i, i, dbl], i),
         "m3dk_set_push_variant": ([vp, i], i),
@@ -179,6 +180,17 @@ class Pusher:
         self._keep["fields_ws"] = ws
         self.n_elems, self.n_modes = n_elems, n_modes
         self.fields_bytes = need.value
+
+    def fields_workspace(self):
+        """The device tensor (uint8) that holds the fields image: what a broadcast to the other ranks sends."""
+        return self._keep["fields_ws"]
+
+    def fields_attach(self, ws, n_elems: int, n_modes: int):
+        """m3dk_fields_attach: bind a byte-for-byte copy of another context's fields workspace (a uint8 device tensor)."""
+        self._ck(self.L.m3dk_fields_attach(self.h, self._p(ws), ws.numel()))
+        self._keep["fields_ws"] = ws
+        self.n_elems, self.n_modes = int(n_elems), int(n_modes)
+        self.fields_bytes = ws.numel()
 
     # ---- m3dk_particles_init --------------------------------------------------------------------------------
     def _f0(self, f0) -> _F0:

@@ -91,6 +91,39 @@ extern "C" int m3dk_destroy(m3dk_ctx *ctx) {
 //            [fast grid: first records gf*gf][overflow records: at most one per bucket, gf*gf]
 static constexpr int kCandPerElem = 24;
 
+// Header of a fields workspace, kept in its control block at byte 32 (bytes 0..31 are device scratch): everything
+// m3dk_fields_attach needs to rebuild the context's FieldParams from a byte-for-byte copy of the workspace on another GPU.
+struct FieldsHeader {
+    unsigned long long magic;
+    unsigned long long off_tiles, off_edges, off_bstart, off_bcand, off_ffirst, off_fovf, total_bytes;
+    double Rmin, Rmax, Zmin, Zmax, inv_hx, inv_hz, finv_hx, finv_hz;
+    double omega[M3DK_MAX_MODES];
+    int n_tor[M3DK_MAX_MODES];
+    int n_elems, n_modes, tile_stride, g, gf, pad;
+};
+static_assert(sizeof(FieldsHeader) <= 224, "the header must fit the control block behind the 32 bytes of scratch");
+static constexpr unsigned long long kFieldsMagic = 0x4d33444b46313030ull;   // "M3DKF100"
+
+static void bind_fields(m3dk_ctx *ctx, char *base, const FieldsHeader &h) {
+    FieldParams &f = ctx->f;
+    f = FieldParams{};
+    ctx->d_count = reinterpret_cast<int *>(base);
+    f.tiles = reinterpret_cast<const double *>(base + h.off_tiles);
+    f.tile_stride = h.tile_stride; f.n_elems = h.n_elems; f.n_modes = h.n_modes;
+    for (int k = 0; k < h.n_modes; ++k) { f.n_tor[k] = h.n_tor[k]; f.omega[k] = h.omega[k]; }
+    f.grid.Rmin = h.Rmin; f.grid.Rmax = h.Rmax; f.grid.Zmin = h.Zmin; f.grid.Zmax = h.Zmax;
+    f.grid.inv_hx = h.inv_hx; f.grid.inv_hz = h.inv_hz; f.grid.gx = h.g; f.grid.gz = h.g;
+    f.grid.bstart = reinterpret_cast<const int *>(base + h.off_bstart);
+    f.grid.bcand = reinterpret_cast<const int *>(base + h.off_bcand);
+    f.grid.edges = reinterpret_cast<const double *>(base + h.off_edges);
+    f.fast.Rmin = h.Rmin; f.fast.Zmin = h.Zmin; f.fast.inv_hx = h.finv_hx; f.fast.inv_hz = h.finv_hz;
+    f.fast.gx = h.gf; f.fast.gz = h.gf;
+    f.fast.first = reinterpret_cast<const FastRec *>(base + h.off_ffirst);
+    f.fast.ovf = reinterpret_cast<const FastRec *>(base + h.off_fovf);
+    ctx->have_fields = true;
+    ctx->have_markers = false;   // cached elements refer to the old mesh
+}
+
 static int fast_grid_dim(int n_elems) {
     int g = (int)ceil(sqrt(2.0 * (double)n_elems));
     return g < 1 ? 1 : g;
@@ -327,7 +360,23 @@ extern "C" int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node
     int *d_bcand = reinterpret_cast<int *>(p); p += up256((size_t)kCandPerElem * n_elems * sizeof(int) + 1024);
     FastRec *d_ffirst = reinterpret_cast<FastRec *>(p); p += up256(ffirst.size() * sizeof(FastRec));
     FastRec *d_fovf = reinterpret_cast<FastRec *>(p);
+    FieldsHeader hdr;
+    memset(&hdr, 0, sizeof(hdr));
+    hdr.magic = kFieldsMagic;
+    char *const base = static_cast<char *>(dev_workspace);
+    hdr.off_tiles = (unsigned long long)(reinterpret_cast<char *>(d_tiles) - base);
+    hdr.off_edges = (unsigned long long)(reinterpret_cast<char *>(d_edges) - base);
+    hdr.off_bstart = (unsigned long long)(reinterpret_cast<char *>(d_bstart) - base);
+    hdr.off_bcand = (unsigned long long)(reinterpret_cast<char *>(d_bcand) - base);
+    hdr.off_ffirst = (unsigned long long)(reinterpret_cast<char *>(d_ffirst) - base);
+    hdr.off_fovf = (unsigned long long)(reinterpret_cast<char *>(d_fovf) - base);
+    hdr.total_bytes = need;
+    hdr.Rmin = Rmin; hdr.Rmax = Rmax; hdr.Zmin = Zmin; hdr.Zmax = Zmax;
+    hdr.inv_hx = 1.0 / hx; hdr.inv_hz = 1.0 / hz; hdr.finv_hx = finv_hx; hdr.finv_hz = finv_hz;
+    for (int k = 0; k < n_modes; ++k) { hdr.n_tor[k] = n_tor[k]; hdr.omega[k] = omega[k]; }
+    hdr.n_elems = n_elems; hdr.n_modes = n_modes; hdr.tile_stride = stride; hdr.g = g; hdr.gf = gf;
     CU(cudaMemsetAsync(ctx->d_count, 0, 256, ctx->stream), "memset control block");
+    CU(cudaMemcpyAsync(base + 32, &hdr, sizeof(hdr), cudaMemcpyHostToDevice, ctx->stream), "upload header");
     CU(cudaMemcpyAsync(d_tiles, tiles.data(), tiles.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "upload tiles");
     CU(cudaMemcpyAsync(d_edges, edges.data(), edges.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "upload edge records");
     CU(cudaMemcpyAsync(d_bstart, bstart.data(), bstart.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream), "upload grid");
@@ -335,18 +384,24 @@ extern "C" int m3dk_fields_create(m3dk_ctx *ctx, int n_nodes, const double *node
     CU(cudaMemcpyAsync(d_ffirst, ffirst.data(), ffirst.size() * sizeof(FastRec), cudaMemcpyHostToDevice, ctx->stream), "upload fast grid");
     CU(cudaMemcpyAsync(d_fovf, fovf.data(), fovf.size() * sizeof(FastRec), cudaMemcpyHostToDevice, ctx->stream), "upload fast grid overflow");
     CU(cudaStreamSynchronize(ctx->stream), "fields upload");
+    bind_fields(ctx, base, hdr);
+    return M3DK_OK;
+}
 
-    FieldParams &f = ctx->f;
-    f = FieldParams{};
-    f.tiles = d_tiles; f.tile_stride = stride; f.n_elems = n_elems; f.n_modes = n_modes;
-    for (int k = 0; k < n_modes; ++k) { f.n_tor[k] = n_tor[k]; f.omega[k] = omega[k]; }
-    f.grid.Rmin = Rmin; f.grid.Rmax = Rmax; f.grid.Zmin = Zmin; f.grid.Zmax = Zmax;
-    f.grid.inv_hx = 1.0 / hx; f.grid.inv_hz = 1.0 / hz; f.grid.gx = g; f.grid.gz = g;
-    f.grid.bstart = d_bstart; f.grid.bcand = d_bcand; f.grid.edges = d_edges;
-    f.fast.Rmin = Rmin; f.fast.Zmin = Zmin; f.fast.inv_hx = finv_hx; f.fast.inv_hz = finv_hz;
-    f.fast.gx = gf; f.fast.gz = gf; f.fast.first = d_ffirst; f.fast.ovf = d_fovf;
-    ctx->have_fields = true;
-    ctx->have_markers = false;   // cached elements refer to the old mesh
+extern "C" int m3dk_fields_attach(m3dk_ctx *ctx, void *dev_workspace, size_t workspace_bytes) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!dev_workspace || workspace_bytes < 256 || ((uintptr_t)dev_workspace & 255))
+        return fail(ctx, M3DK_EWORKSPACE, "m3dk_fields_attach: workspace NULL, misaligned or shorter than its control block");
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    FieldsHeader hdr;
+    char *const base = static_cast<char *>(dev_workspace);
+    CU(cudaMemcpyAsync(&hdr, base + 32, sizeof(hdr), cudaMemcpyDeviceToHost, ctx->stream), "read header");
+    CU(cudaStreamSynchronize(ctx->stream), "read header");
+    if (hdr.magic != kFieldsMagic || hdr.total_bytes > workspace_bytes || hdr.n_elems < 1 || hdr.n_modes < 0 ||
+        hdr.n_modes > M3DK_MAX_MODES || hdr.tile_stride != tile_stride_doubles(hdr.n_modes))
+        return fail(ctx, M3DK_EINVAL, "m3dk_fields_attach: the workspace does not hold a fields image of this library version");
+    ctx->have_fields = false;
+    bind_fields(ctx, base, hdr);
     return M3DK_OK;
 }
 

@@ -38,3 +38,44 @@ def max_over_ranks(values, dist=None, device=None):
     if dist is not None and dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return [float(x) for x in t]
+
+
+# ---- the two exchange steps around the push ----------------------------------------------
+# (1) the field image goes from the rank that built it to every other rank once per field update; (2) the deposited
+# moments of the marker shards are summed.  Both are plain collectives on whole buffers (NCCL on device tensors, gloo on
+# CPU tensors in the tests); the push itself exchanges nothing.
+
+def broadcast_bytes(buf, dist, src: int = 0):
+    """Broadcast a uint8 tensor whose length only `src` knows.  `buf` is the tensor on `src` and None (or anything) on the
+    other ranks, which get a fresh tensor on `like_device`.  Returns the tensor every rank now holds."""
+    import torch
+
+    rank = dist.get_rank()
+    dev = buf.device if rank == src else None
+    n = torch.tensor([buf.numel() if rank == src else 0], dtype=torch.int64)
+    backend = dist.get_backend()
+    if backend == "nccl":
+        n = n.cuda()
+    dist.broadcast(n, src)
+    if rank != src:
+        dev = torch.device("cuda", torch.cuda.current_device()) if backend == "nccl" else torch.device("cpu")
+        buf = torch.empty(int(n.item()), dtype=torch.uint8, device=dev)
+    dist.broadcast(buf, src)
+    return buf
+
+
+def broadcast_fields(pusher, dist, n_elems: int, n_modes: int, src: int = 0):
+    """"the fields ... are collected and uploaded to every GPU".  Rank `src` has called fields_create; its
+    self-describing fields workspace is broadcast and every other rank binds its copy with m3dk_fields_attach (no host
+    tables, no second least-squares fit or search-grid build)."""
+    ws = broadcast_bytes(pusher.fields_workspace() if dist.get_rank() == src else None, dist, src)
+    if dist.get_rank() != src:
+        pusher.fields_attach(ws, n_elems, n_modes)
+    return ws.numel()
+
+
+def allreduce_moments(rhs, dist):
+    """Sum of the deposited moment tables of all marker shards, in place on every rank."""
+    if dist is not None and dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(rhs, op=dist.ReduceOp.SUM)
+    return rhs

@@ -111,7 +111,9 @@ def _kappa_fn(eq: CircularTokamak, profile_L: Optional[float]):
 
 
 def make_config(idx: int, n_markers: Optional[int] = None, nx: Optional[int] = None, amp: float = 1.0e-4,
-                dt_gyro: Optional[float] = None, seed: Optional[int] = None) -> Workload:
+                dt_gyro: Optional[float] = None, seed: Optional[int] = None, tables: bool = True) -> Workload:
+    """tables = False: mesh, mode structure and markers only (eq_coef / pert_coef are None): for the ranks that receive
+    the field image from rank 0 instead of fitting the tables themselves."""
     spec = CONFIGS[idx]
     n = spec["n"] if n_markers is None else int(n_markers)
     nx = spec["nx"] if nx is None else int(nx)
@@ -139,18 +141,24 @@ def make_config(idx: int, n_markers: Optional[int] = None, nx: Optional[int] = N
         L = 0.4
 
     key = (idx, nx, amp)
-    if key not in _table_cache:
+    if not tables:
         node_RZ, tri = rect_tri_mesh(nx, BOX)
-        eqc = eq_tables(eq, node_RZ, tri, _kappa_fn(eq, L))
-        if perts:
-            pc, n_tor, omega = pert_tables(perts, node_RZ, tri)
-        else:
-            pc = np.zeros((0, tri.shape[0], 7, 2, 21))
-            n_tor = np.zeros(0, dtype=np.int32)
-            omega = np.zeros(0)
-        _table_cache.clear()  # keep at most one big table set alive
-        _table_cache[key] = (node_RZ, tri, eqc, pc, n_tor, omega)
-    node_RZ, tri, eqc, pc, n_tor, omega = _table_cache[key]
+        eqc, pc = None, None
+        n_tor = np.array([p.n for p in perts], dtype=np.int32)
+        omega = np.array([p.omega for p in perts], dtype=np.float64)
+    else:
+        if key not in _table_cache:
+            node_RZ, tri = rect_tri_mesh(nx, BOX)
+            eqc = eq_tables(eq, node_RZ, tri, _kappa_fn(eq, L))
+            if perts:
+                pc, n_tor, omega = pert_tables(perts, node_RZ, tri)
+            else:
+                pc = np.zeros((0, tri.shape[0], 7, 2, 21))
+                n_tor = np.zeros(0, dtype=np.int32)
+                omega = np.zeros(0)
+            _table_cache.clear()  # keep at most one big table set alive
+            _table_cache[key] = (node_RZ, tri, eqc, pc, n_tor, omega)
+        node_RZ, tri, eqc, pc, n_tor, omega = _table_cache[key]
 
     markers = load_markers(eq, n, seed, CHARGE, MASS, dt, **mk)
     return Workload(name=spec["name"], eq=eq, perts=perts, node_RZ=node_RZ, tri=tri, eq_coef=eqc, pert_coef=pc,

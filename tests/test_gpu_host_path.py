@@ -101,3 +101,26 @@ def test_sort_workspace_is_recarved_on_reinit_with_a_larger_n():
     assert np.array_equal(np.sort(ids), np.arange(w_big.n_markers))
     for k in KEYS:
         assert np.array_equal(got[k], want[k]), k
+
+
+def test_fields_attach_binds_a_copy_of_the_workspace():
+    """m3dk_fields_attach on a byte-for-byte copy of another context's fields workspace (what the NCCL broadcast of
+    bench.py --gpus N delivers): no host tables, same search and field evaluation, same pushed bits."""
+    import paper_2107_13663_b200 as m3dk
+    w = synth.make_config(3, n_markers=4000 + 9, nx=48)
+    a = make_pusher(w, verify=False, sort_interval=1)
+    copy = a.fields_workspace().clone()
+    b = m3dk.Pusher(device=0, verify=False)
+    b.fields_attach(copy, w.n_elems, w.n_modes)
+    b.particles_init(w.markers, w.charge, w.mass, w.f0)
+    b.set_options(sort_interval=1, t0=0.0)
+    a.push(5, w.dt)
+    b.push(5, w.dt)
+    ra, ea, _ = a.state()
+    rb, eb, _ = b.state()
+    assert np.array_equal(ea, eb)
+    for k in KEYS:
+        assert np.array_equal(ra[k], rb[k]), k
+    garbage = torch.zeros(4096, dtype=torch.uint8, device="cuda")
+    with pytest.raises(m3dk.M3DKError):
+        m3dk.Pusher(device=0, verify=False).fields_attach(garbage, 1, 0)

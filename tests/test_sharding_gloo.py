@@ -51,6 +51,55 @@ def test_two_rank_shards_and_max_over_ranks():
     assert (r0[3], r0[4], r1[3], r1[4]) == (0, 501, 501, 1001)   # contiguous, disjoint, complete
 
 
+def _worker_moments(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import oracle
+        import synth
+        w = synth.make_config(1, n_markers=3001, nx=12, tables=(rank == 0))       # only rank 0 fits the tables
+        rng = np.random.Generator(np.random.PCG64(5))
+        w.markers["w"] = rng.normal(size=w.n_markers)
+        # (1) the field tables travel as one byte image from rank 0 (here: the host tables, pickled to bytes)
+        if rank == 0:
+            blob = np.concatenate([w.eq_coef.ravel(), w.pert_coef.ravel()]).view(np.uint8)
+            buf = torch.from_numpy(blob.copy())
+        else:
+            buf = None
+        buf = shard.broadcast_bytes(buf, dist, 0)
+        flat = buf.numpy().view(np.float64)
+        n_eq = w.n_elems * 4 * 21
+        eq_coef = flat[:n_eq].reshape(w.n_elems, 4, 21)
+        pert_coef = flat[n_eq:].reshape(w.n_modes, w.n_elems, 7, 2, 21)
+        mesh = oracle.Mesh(w.node_RZ, w.tri, eq_coef, pert_coef, w.n_tor, w.omega)
+        sp = oracle.species_of(w)
+        # (2) every rank deposits its shard of the SAME global marker set; the tables are summed
+        b, e = shard.shard_range(w.n_markers, rank, world)
+        mine = {k: v[b:e] for k, v in w.markers.items()}
+        rhs, _ = oracle.deposit(mesh, sp, mine, 1, 0.3)
+        t = torch.from_numpy(rhs.copy())
+        shard.allreduce_moments(t, dist)
+        whole, _ = oracle.deposit(mesh, sp, w.markers, 1, 0.3)
+        out[rank] = (float(np.abs(t.numpy() - whole).max()), float(np.abs(whole).max()), int(buf.numel()), e - b)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_field_broadcast_and_moment_allreduce():
+    """The two exchange steps around the push: rank 1 never sees the host tables, it receives rank 0's
+    byte image; the all-reduced moment table of the two marker shards equals the deposition of the whole marker set."""
+    world = 2
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_worker_moments, args=(world, _free_port(), out), nprocs=world, join=True)
+    for r in range(world):
+        err, scale, nbytes, n_mine = out[r]
+        assert err <= 1e-12 * scale and scale > 0
+        assert nbytes == out[0][2] > 0
+    assert out[0][3] + out[1][3] == 3001
+
+
 def test_shard_range_partitions_every_count():
     for n in (0, 1, 7, 64, 1000):
         for world in (1, 2, 3, 8):
