@@ -383,8 +383,10 @@ static double weight_rhs(const orc_fields *f, const orc_species *sp, double R, c
         double v = sqrt(2.0 * Ekin / m), vc = sp->f0par[1];
         kE = -3.0 * v / (m * (v * v * v + vc * vc * vc));
         if (sp->f0kind == 2) {
-            double Lam = mu * sp->f0par[4] / Ekin, L0 = sp->f0par[2], dL = sp->f0par[3];
-            kE += 2.0 * (Lam - L0) * Lam / (dL * dL * Ekin);
+            if (Ekin > 0.0) {                          /* a marker with v = 0 and mu = 0 has no pitch: the term is dropped */
+                double Lam = mu * sp->f0par[4] / Ekin, L0 = sp->f0par[2], dL = sp->f0par[3];
+                kE += 2.0 * (Lam - L0) * Lam / (dL * dL * Ekin);
+            }
         }
     }
     /* Eqs. (8)-(9), (1-w) -> 1:  dw/dt = -[ (kappa/q) dPphi/dt + kE dE/dt ] */
@@ -423,6 +425,9 @@ static void gyro_ring(const double X[3], const double B0c[3], double c, double s
     double b[3] = {B0c[0] / Bn, B0c[1] / Bn, B0c[2] / Bn};
     double rho = sqrt(2.0 * m * mu / Bn) / fabs(q);
     double e1[3] = {1.0 - b[0] * b[0], -b[0] * b[1], -b[0] * b[2]};      /* R-hat - (R-hat . b) b, cylindrical */
+    if (b[0] * b[0] > 0.999999) {                                        /* b (anti)parallel to R-hat: start from Z-hat */
+        e1[0] = -b[2] * b[0]; e1[1] = -b[2] * b[1]; e1[2] = 1.0 - b[2] * b[2];
+    }
     double n1 = sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
     for (int k = 0; k < 3; ++k) e1[k] /= n1;
     double e2[3] = {b[1] * e1[2] - b[2] * e1[1], b[2] * e1[0] - b[0] * e1[2], b[0] * e1[1] - b[1] * e1[0]};

@@ -302,6 +302,9 @@ __device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, 
     const double rho = __dmul_rn(m3dk_sqrt(__dmul_rn(__dmul_rn(__dmul_rn(2.0, P.m), mu), binv)), fabs(P.inv_q));
     // e1 = R-hat - (R-hat . b) b, normalised; e2 = b x e1 (cylindrical components at the marker)
     double e1R = M3DK_FMA(-bR, bR, 1.0), e1P = -__dmul_rn(bR, bP), e1Z = -__dmul_rn(bR, bZ);
+    if (__dmul_rn(bR, bR) > 0.999999) {   // b (anti)parallel to R-hat: start from Z-hat instead (same rule as the oracle)
+        e1R = -__dmul_rn(bZ, bR); e1P = -__dmul_rn(bZ, bP); e1Z = M3DK_FMA(-bZ, bZ, 1.0);
+    }
     const double n1 = m3dk_rsqrt(M3DK_FMA(e1R, e1R, M3DK_FMA(e1P, e1P, __dmul_rn(e1Z, e1Z))));
     e1R = __dmul_rn(e1R, n1); e1P = __dmul_rn(e1P, n1); e1Z = __dmul_rn(e1Z, n1);
     const double e2R = M3DK_FMA(bP, e1Z, -__dmul_rn(bZ, e1P)), e2P = M3DK_FMA(bZ, e1R, -__dmul_rn(bR, e1Z)),

@@ -65,3 +65,31 @@ def test_flr_ordered_pipeline_and_bitwise_order_independence(two_modes):
     for si in (1, 3):
         for k in KEYS:
             assert np.array_equal(res[si][k], res[0][k]), (si, k)
+
+
+def test_flr_where_b_is_parallel_to_the_major_radius():
+    """the ring basis must not divide by zero where b0 is parallel to the major-radius direction.  Hand-made
+    tables with a nearly radial field (psi0 = A Z, a weak F): push (mode 2) and 4-point deposition against the oracle."""
+    import dataclasses
+    import oracle
+    from handmade import HandMade
+    w0 = synth.make_config(1, n_markers=2000 + 3, nx=12)
+    hm = HandMade(eq=dict(psi=(0.0, 0.0, 0.9), Bm=(1.0, 0.0, 0.0), F=(0.0,), kappa=(0.3,)),
+                  pert=dict(E_R=(1e-3,), E_Z=(2e-3 + 1e-3j,), B_Z=(1e-3j,), B_par=(1e-3, 2e-3, -1e-3)), n_tor=2, omega=0.05, nx=12)
+    w = dataclasses.replace(w0, node_RZ=hm.node, tri=hm.tri, eq_coef=hm.eq_coef, pert_coef=hm.pert_coef,
+                            n_tor=hm.n_tor_a, omega=hm.omega_a)
+    mesh, sp = oracle_of(w, mode=2)
+    ref, e_ref, _ = oracle_push(mesh, sp, w.markers, 2, 0.01)
+    p = make_pusher(w, verify=True, sort_interval=1, mode=2)
+    p.push(2, 0.01)
+    got, _, _ = p.state()
+    live = e_ref >= 0
+    assert live.mean() > 0.9 and np.isfinite(got["w"]).all()
+    wrms = np.sqrt(np.mean(ref["w"][live] ** 2))
+    ex, ev, ew = g16_errors(take(got, live), take(ref, live), w_floor=wrms)
+    assert max(ex.max(), ev.max(), ew.max()) <= 3 * TOL_STEP, (ex.max(), ev.max(), ew.max())
+    raw, _, _ = p.state(by_id=False)
+    want, _ = oracle.deposit(mesh, sp, raw, 2, 0.0)
+    rhs = p.deposit(flags=2, t=0.0)
+    assert np.isfinite(rhs).all()
+    assert np.abs(rhs - want).max() <= 1e-10 * max(np.abs(want).max(), 1e-300)

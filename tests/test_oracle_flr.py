@@ -126,3 +126,25 @@ def test_f4_plane_wave_reduction_factor(orc):
         e_theta = -avg[0] * np.sin(th0) + avg[2] * np.cos(th0)
         assert abs(factor) < 0.98                                        # a real reduction at this k rho
         assert abs(e_theta / e_theta0 - factor) < 0.04, (mu, e_theta / e_theta0, factor)
+
+
+def test_f5_ring_where_b_is_parallel_to_the_major_radius(orc):
+    """The construction of reading G23 starts from the major-radius direction made perpendicular to b0; where b0 is
+    (anti)parallel to it (a purely radial field: psi0 = A Z, F = 0) it starts from Z-hat instead.  The ring must still be
+    four finite points at distance rho, perpendicular to b0, 90 degrees apart."""
+    from handmade import HandMade
+    from synth.configs import CHARGE, MASS
+    A, mu = 0.9, 0.004
+    hm = HandMade(eq=dict(psi=(0.0, 0.0, A), Bm=(1.0,), F=(0.0,), kappa=(0.0,)))
+    sp = orc.species(CHARGE, MASS)
+    X = np.array([3.2 * np.cos(0.4), 3.2 * np.sin(0.4), 0.1])
+    pts = orc.gyro_ring(sp, X, mu, mesh=hm.oracle_mesh(orc))
+    assert np.isfinite(pts).all()
+    bx = -np.array([np.cos(0.4), np.sin(0.4), 0.0])                 # B_R = -A / R: b0 = -R-hat
+    rho = np.sqrt(2 * MASS * mu / (A / 3.2)) / abs(CHARGE)
+    d = pts - X
+    assert np.allclose(np.linalg.norm(d, axis=1), rho, rtol=1e-12)
+    assert np.abs(d @ bx).max() < 1e-12 * rho
+    assert np.allclose(d[0], -d[2], atol=1e-15) and np.allclose(d[1], -d[3], atol=1e-15)
+    assert abs(d[0] @ d[1]) < 1e-12 * rho * rho
+    assert np.allclose(np.cross(bx, d[0]), d[1], rtol=1e-12, atol=1e-15)          # e2 = b0 x e1
