@@ -151,6 +151,14 @@ int m3dk_set_push_variant(m3dk_ctx *ctx, int variant);
 int m3dk_sort_workspace_bytes(long n_markers, int n_elems, size_t *bytes);
 int m3dk_set_sort_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes);
 
+/* FLR workspace (DEVICE, 256-byte aligned, borrowed until replaced; optional): with it, the ordered pipeline of mode 2
+ * (sort_interval >= 1) does not let every marker gather the coefficient tiles of its four ring points: the push emits the
+ * 4 n ring points (position, element, the marker's weights), they are ordered by THEIR element like the markers, a warp
+ * evaluates up to 64 ring points of one element with the tile staged in shared memory, and the four contributions are
+ * summed back into w (290 bytes per marker).  Results are bit-identical with and without it.                          */
+int m3dk_flr_workspace_bytes(long n_markers, int n_elems, size_t *bytes);
+int m3dk_set_flr_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes);
+
 /* nsteps slow-manifold Boris steps of size dt with field evaluation and weight update, Eqs. (5), (6), (8)-(13).
  * Asynchronous; t advances by nsteps * dt.  A lost marker is frozen.  On return (stream order) the caller's arrays hold
  * the new state; if sorts ran, slots are permuted and id[] says who is where.                                         */

@@ -74,6 +74,8 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_set_push_variant": ([vp, i], i),
         "m3dk_sort_workspace_bytes": ([lng, i, C.POINTER(sz)], i),
         "m3dk_set_sort_workspace": ([vp, vp, sz], i),
+        "m3dk_flr_workspace_bytes": ([lng, i, C.POINTER(sz)], i),
+        "m3dk_set_flr_workspace": ([vp, vp, sz], i),
         "m3dk_push": ([vp, i, dbl], i),
         "m3dk_sort": ([vp, vp, sz], i),
         "m3dk_stats": ([vp, C.POINTER(_Stats)], i),
@@ -259,6 +261,14 @@ class Pusher:
         ws = self._empty(self.sort_workspace_bytes())
         self._ck(self.L.m3dk_set_sort_workspace(self.h, self._p(ws), ws.numel()))
         self._keep["sort_ws"] = ws
+
+    def set_flr_workspace(self):
+        """Allocate and lend the FLR workspace (ring stream of the ordered mode 2)."""
+        need = C.c_size_t()
+        self._ck(self.L.m3dk_flr_workspace_bytes(self.n, self.n_elems, C.byref(need)))
+        ws = self._empty(need.value)
+        self._ck(self.L.m3dk_set_flr_workspace(self.h, self._p(ws), ws.numel()))
+        self._keep["flr_ws"] = ws
 
     def push(self, nsteps: int, dt: float):
         self._ck(self.L.m3dk_push(self.h, int(nsteps), float(dt)))

@@ -432,6 +432,11 @@ extern "C" int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, 
         ctx->sb.bytes = ctx->sortws_bytes;
         ctx->have_sortws = true;
     }
+    ctx->have_flrws = false;
+    if (ctx->flrws_base && flr_workspace_bytes(n, ctx->f.n_elems) <= ctx->flrws_bytes) {
+        carve_flr_workspace(ctx->flrws_base, n, ctx->f.n_elems, &ctx->fb);
+        ctx->have_flrws = true;
+    }
     CU(launch_locate(ctx, ctx->user, n, true), "locate kernel");
     return M3DK_OK;
 }
@@ -475,6 +480,23 @@ static int bind_sort_ws(m3dk_ctx *ctx, void *ws, size_t bytes, const char *who) 
 extern "C" int m3dk_set_sort_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes) {
     if (!ctx) return M3DK_EINVAL;
     return bind_sort_ws(ctx, dev_workspace, bytes, "m3dk_set_sort_workspace");
+}
+
+extern "C" int m3dk_flr_workspace_bytes(long n_markers, int n_elems, size_t *bytes) {
+    if (!bytes || n_markers < 0 || n_elems < 1) return M3DK_EINVAL;
+    *bytes = flr_workspace_bytes(n_markers, n_elems);
+    return M3DK_OK;
+}
+
+extern "C" int m3dk_set_flr_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes) {
+    if (!ctx) return M3DK_EINVAL;
+    if (!ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_set_flr_workspace: call m3dk_particles_init first");
+    if (!dev_workspace || ((uintptr_t)dev_workspace & 255) || bytes < flr_workspace_bytes(ctx->n, ctx->f.n_elems))
+        return fail(ctx, M3DK_EWORKSPACE, "m3dk_set_flr_workspace: workspace NULL, misaligned or smaller than m3dk_flr_workspace_bytes");
+    carve_flr_workspace(dev_workspace, ctx->n, ctx->f.n_elems, &ctx->fb);
+    ctx->flrws_base = dev_workspace; ctx->flrws_bytes = bytes;
+    ctx->have_flrws = true;
+    return M3DK_OK;
 }
 
 // ---- sort and push ---------------------------------------------------------------------------------------------------
@@ -541,6 +563,12 @@ static int run_steps(m3dk_ctx *ctx, int nsteps, double dt) {
         {
             EvScope ev(ctx, &ctx->ev_push);
             CU(launch_push_rec(ctx, ctx->n, dt, t, reorder_after), "push kernel");
+            if (ctx->mode == 2 && ctx->have_flrws && ctx->f.n_modes > 0) {
+                // the push has emitted the ring stream: order it by the ring points' elements, evaluate, sum back into w
+                CU(launch_flr_ring_stage(ctx, ctx->n), "ring ordering kernels");
+                CU(launch_flr_ring_eval(ctx, ctx->n, dt, t), "ring evaluation kernel");
+                CU(launch_flr_reduce(ctx, ctx->n, dt), "ring reduction kernel");
+            }
         }
         ctx->steps_done++; ctx->steps_at_dt++;
         ctx->steps_since_sort = 1;
@@ -672,6 +700,7 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
         ctx->user = MarkerArrays{all.x + o, all.y + o, all.z + o, all.vx + o, all.vy + o, all.vz + o, all.mu + o, all.w + o,
                                  all.elem + o, all.id + o};
         if (ctx->have_sortws) carve_sort_workspace(ctx->sortws_base, nc, ctx->f.n_elems, &ctx->sb);
+        if (ctx->have_flrws) carve_flr_workspace(ctx->flrws_base, nc, ctx->f.n_elems, &ctx->fb);
         ctx->steps_done = steps0; ctx->steps_at_dt = at0; ctx->t_base = tb0; ctx->last_dt = ldt0;
         cudaError_t e = launch_locate(ctx, ctx->user, nc, true, (int)o);
         if (e != cudaSuccess) { rc = cuda_fail(ctx, e, "locate kernel"); break; }
@@ -687,6 +716,7 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
     // restore the full binding
     ctx->n = n; ctx->user = all;
     if (ctx->have_sortws) carve_sort_workspace(ctx->sortws_base, n, ctx->f.n_elems, &ctx->sb);
+    if (ctx->have_flrws) carve_flr_workspace(ctx->flrws_base, n, ctx->f.n_elems, &ctx->fb);
     ctx->sb.bytes = ctx->sortws_bytes;
     if (rc != M3DK_OK) return rc;
     CU(cudaStreamSynchronize(ctx->s_down), "download stream synchronize (an earlier kernel may have failed)");

@@ -92,10 +92,21 @@ struct RecArrays {            // ordered pipeline, carved from the sort workspac
     int *key;                // [n] element of the NEW position of output slot d (n_elems = lost)
 };
 
+// Ring stream of the ordered FLR mode (mode 2 with an FLR workspace): four ring points per marker slot.
+struct FlrArrays {
+    double *ring;            // [4 n][4] (x, y, z, -) of ring point 4 slot + j
+    double *wts;             // [n][10] the marker's weights of the perturbed fields in dw/dt, Cartesian (FlrW)
+    double *contrib;         // [4 n] c_j of every ring point
+    int *rkey, *rrank;       // [4 n] element of the ring point (n_elems = outside, -1 = the slot holds a lost marker), rank in it
+    int *rorder;             // [4 n] ring points in element order
+    int *rhist;              // [n_elems + 2]
+};
+
 struct PushParams {
     long n;
     MarkerArrays a;          // SoA path (sort_interval = 0)
     RecArrays rc;            // record path (sort_interval >= 1)
+    FlrArrays fl;            // ring stream (mode 2, ordered)
     FieldParams f;
     double dt, h;            // h = q dt / (2 m)
     double q, m, inv_q, inv_m;
@@ -113,6 +124,15 @@ struct PushParams {
 #endif
 constexpr int kItemR = M3DK_ITEM_R;              // markers per lane in the element-ordered push
 constexpr int kItemMarkers = 32 * kItemR;        // markers per work item
+
+struct FlrBuffers {          // carved from the FLR workspace (m3dk_set_flr_workspace)
+    FlrArrays a;
+    int *roffs, *rioffs;     // [n_elems + 2]
+    int4 *ritems;            // [4 n / kItemMarkers + n_elems + 2]
+    int4 *ritems_small;      // [n_elems + 2]
+    unsigned long long *rstate;   // scan state + item tickets, as SortBuffers::scan_state
+    size_t bytes;
+};
 
 struct SortBuffers {         // carved from the sort workspace
     double *rec[2];          // [n][8] record ping-pong
@@ -164,6 +184,10 @@ struct m3dk_ctx {
     // sort workspace
     bool have_sortws = false;
     m3dk::SortBuffers sb{};
+    bool have_flrws = false;
+    m3dk::FlrBuffers fb{};
+    void *flrws_base = nullptr;
+    size_t flrws_bytes = 0;
     int *d_count = nullptr;      // small device scratch inside the fields workspace (lost counter etc.)
     void *sortws_base = nullptr; // the caller's sort workspace as given (re-carved when n or the mesh changes)
     size_t sortws_bytes = 0;
@@ -194,6 +218,11 @@ cudaError_t launch_gc_push(m3dk_ctx *c, long n, double *vpar, int nsteps, double
 cudaError_t launch_gc_bootstrap(m3dk_ctx *c, long n, const double *vpar, double dt);     // (x_1, v_{1/2}) from one such step
 cudaError_t fp64_probe(m3dk_ctx *c, double *tflops);
 
+cudaError_t launch_flr_ring_stage(m3dk_ctx *c, long n);   // ring histogram -> offsets, ring items, ring order
+cudaError_t launch_flr_ring_eval(m3dk_ctx *c, long n, double dt, double t);   // ring_items_kernel (push.cu)
+cudaError_t launch_flr_reduce(m3dk_ctx *c, long n, double dt);   // w += dt * quarter sum of the contributions
+size_t flr_workspace_bytes(long n, int n_elems);
+void carve_flr_workspace(void *ws, long n, int n_elems, FlrBuffers *fb);
 size_t sort_workspace_bytes(long n, int n_elems);
 void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb);
 

@@ -111,12 +111,17 @@ struct RecIO {   // record = (x, y, z, w | vx, vy, vz, mu): two 32-byte sectors,
 // tile: the element's coefficient tile, in global memory (kSmem = false) or staged in shared memory (kSmem = true).
 __device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
                                            const PertW &W);
+__device__ __forceinline__ void flr_emit(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
+                                         const PertW &W, long slot);
 
-// kFlr (mode 2): phase B is replaced by the 4-point gyro-average of the perturbed fields (flr_wdot).
+// kFlr (mode 2): phase B is replaced by the 4-point gyro-average of the perturbed fields.  kFlr = 1: every lane evaluates
+// its four ring points itself, each on its own element's tile read from global memory (flr_wdot).  kFlr = 2: the lane only
+// EMITS the ring points (position, element, weights of the perturbed fields in dw/dt) into the ring stream (flr_emit);
+// they are ordered by THEIR element, evaluated by ring_items_kernel with staged tiles and summed back by flr_reduce_kernel.
 // kPost (asynchronously staged kernel): the step ends with the new (R, Z) in Rn, Zn; search, key, histogram and rank are
 // the caller's (it runs them one item later, on data that was fetched in the meantime); io.stage_next() is called once
 // all of this lane's input has been consumed.
-template <int R, bool kHist, bool kSmem, class IO, bool kFlr = false, bool kPost = false>
+template <int R, bool kHist, bool kSmem, class IO, int kFlr = 0, bool kPost = false>
 __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const double *__restrict__ tile,
                                        const long (&mi)[R], const long (&mo)[R], const bool (&on)[R], double (&Rn)[R],
                                        double (&Zn)[R]) {
@@ -196,8 +201,12 @@ __device__ __forceinline__ void step_R(const PushParams &P, const IO &io, const 
     if (kFlr && P.f.n_modes > 0) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const double wdot = flr_wdot(P, fe[kFlr ? r : 0], g[r], zl[kFlr ? r : 0], s[r].mu, W[r]);
-            if (on[r]) io.store_w(mo[r], M3DK_FMA(P.dt, wdot, s[r].w));
+            if constexpr (kFlr == 2) {
+                if (on[r]) flr_emit(P, fe[kFlr ? r : 0], g[r], zl[kFlr ? r : 0], s[r].mu, W[r], mo[r]);
+            } else {
+                const double wdot = flr_wdot(P, fe[kFlr ? r : 0], g[r], zl[kFlr ? r : 0], s[r].mu, W[r]);
+                if (on[r]) io.store_w(mo[r], M3DK_FMA(P.dt, wdot, s[r].w));
+            }
         }
         locate_and_count();
     } else if (P.f.n_modes > 0) {
@@ -291,15 +300,19 @@ __device__ __forceinline__ void pert_fields(const PushParams &P, const double *_
 // ---- finite Larmor radius (mode 2; Eq. 14; reading G23) ------------------------------------------
 // dw/dt of one marker with the perturbed fields replaced by the quarter sum over the four gyro-ring points
 // X +- rho e1, X +- rho e2 (rho = m v_perp / (|q| B), v_perp = sqrt(2 mu B / m); e1 = the major-radius direction made
-// perpendicular to b0, e2 = b0 x e1).  Each point is searched and evaluated on its own element's tile (global memory:
-// the ring leaves the marker's element), vectors are summed in Cartesian components and returned to the marker's
-// cylindrical frame.  A point outside the mesh contributes zero.  (g, zl) = cylindrical map and z of x_l.
-__device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
-                                           const PertW &W) {
+// perpendicular to b0, e2 = b0 x e1).  dw/dt is linear in the perturbed fields, so the quarter sum is taken of the four
+// scalar contributions c_j = (weights) . (fields at ring point j): the nine weights of PertW are rotated once to Cartesian
+// components (FlrW), the fields of a ring point are rotated from that point's cylindrical frame, and
+//     dw/dt = 0.25 (((c_0 + c_1) + c_2) + c_3),      c_j = 0 for a ring point outside the mesh.
+// Every kernel takes the same route through flr_ring_point / flr_fold, so the bits do not depend on who evaluates a point.
+struct FlrRing { double X, Y, rho, ex[2], ey[2], ez[2]; };
+struct FlrW { double aEx, aEy, aEz, bBx, bBy, bBz, gGx, gGy, gGz, dT; };
+
+__device__ __forceinline__ void flr_ring(const PushParams &P, const EqOut &f, const StepGeom &g, double mu, FlrRing &rg) {
     const double BR = -__dmul_rn(f.psi_Z, g.rinv), BP = __dmul_rn(f.F, g.rinv), BZ = __dmul_rn(f.psi_R, g.rinv);
     const double binv = m3dk_rsqrt(M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, __dmul_rn(BZ, BZ))));
     const double bR = __dmul_rn(BR, binv), bP = __dmul_rn(BP, binv), bZ = __dmul_rn(BZ, binv);
-    const double rho = __dmul_rn(m3dk_sqrt(__dmul_rn(__dmul_rn(__dmul_rn(2.0, P.m), mu), binv)), fabs(P.inv_q));
+    rg.rho = __dmul_rn(m3dk_sqrt(__dmul_rn(__dmul_rn(__dmul_rn(2.0, P.m), mu), binv)), fabs(P.inv_q));
     // e1 = R-hat - (R-hat . b) b, normalised; e2 = b x e1 (cylindrical components at the marker)
     double e1R = M3DK_FMA(-bR, bR, 1.0), e1P = -__dmul_rn(bR, bP), e1Z = -__dmul_rn(bR, bZ);
     if (__dmul_rn(bR, bR) > 0.999999) {   // b (anti)parallel to R-hat: start from Z-hat instead (same rule as the oracle)
@@ -310,46 +323,91 @@ __device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, 
     const double e2R = M3DK_FMA(bP, e1Z, -__dmul_rn(bZ, e1P)), e2P = M3DK_FMA(bZ, e1R, -__dmul_rn(bR, e1Z)),
                  e2Z = M3DK_FMA(bR, e1P, -__dmul_rn(bP, e1R));
     const double c = g.cph, sn = g.sph;
-    const double ex[2] = {M3DK_FMA(e1R, c, -__dmul_rn(e1P, sn)), M3DK_FMA(e2R, c, -__dmul_rn(e2P, sn))};
-    const double ey[2] = {M3DK_FMA(e1R, sn, __dmul_rn(e1P, c)), M3DK_FMA(e2R, sn, __dmul_rn(e2P, c))};
-    const double ez[2] = {e1Z, e2Z};
-    const double X = __dmul_rn(g.R, c), Y = __dmul_rn(g.R, sn);
-    double Ex = 0.0, Ey = 0.0, Ez = 0.0, Bx = 0.0, By = 0.0, Bz = 0.0, Gx = 0.0, Gy = 0.0, Gz = 0.0, dT = 0.0;
+    rg.ex[0] = M3DK_FMA(e1R, c, -__dmul_rn(e1P, sn)); rg.ex[1] = M3DK_FMA(e2R, c, -__dmul_rn(e2P, sn));
+    rg.ey[0] = M3DK_FMA(e1R, sn, __dmul_rn(e1P, c)); rg.ey[1] = M3DK_FMA(e2R, sn, __dmul_rn(e2P, c));
+    rg.ez[0] = e1Z; rg.ez[1] = e2Z;
+    rg.X = __dmul_rn(g.R, c); rg.Y = __dmul_rn(g.R, sn);
+}
+__device__ __forceinline__ void flr_ring_point(const FlrRing &rg, double zl, int j, double &x, double &y, double &z) {
+    const double sg = j < 2 ? rg.rho : -rg.rho;
+    x = M3DK_FMA(sg, rg.ex[j & 1], rg.X); y = M3DK_FMA(sg, rg.ey[j & 1], rg.Y); z = M3DK_FMA(sg, rg.ez[j & 1], zl);
+}
+// the weights of PertW (marker's cylindrical frame; B1_phi does not enter) as Cartesian vectors
+__device__ __forceinline__ void flr_cart_weights(const PertW &W, double c, double sn, FlrW &cw) {
+    cw.aEx = M3DK_FMA(W.aER, c, -__dmul_rn(W.aEP, sn)); cw.aEy = M3DK_FMA(W.aER, sn, __dmul_rn(W.aEP, c)); cw.aEz = W.aEZ;
+    cw.bBx = __dmul_rn(W.bBR, c); cw.bBy = __dmul_rn(W.bBR, sn); cw.bBz = W.bBZ;
+    cw.gGx = M3DK_FMA(W.gR, c, -__dmul_rn(W.gP, sn)); cw.gGy = M3DK_FMA(W.gR, sn, __dmul_rn(W.gP, c)); cw.gGz = W.gZ;
+    cw.dT = W.dT;
+}
+// c_j: the fields pf of a ring point (its own cylindrical frame, cos / sin of its phi = cj, sj) against the weights
+__device__ __forceinline__ double flr_fold(const PertF &pf, double cj, double sj, const FlrW &cw) {
+    const double Ex = M3DK_FMA(pf.ER, cj, -__dmul_rn(pf.EP, sj)), Ey = M3DK_FMA(pf.ER, sj, __dmul_rn(pf.EP, cj));
+    const double Bx = M3DK_FMA(pf.BR, cj, -__dmul_rn(pf.BP, sj)), By = M3DK_FMA(pf.BR, sj, __dmul_rn(pf.BP, cj));
+    const double Gx = M3DK_FMA(pf.gR, cj, -__dmul_rn(pf.gP, sj)), Gy = M3DK_FMA(pf.gR, sj, __dmul_rn(pf.gP, cj));
+    double a = __dmul_rn(cw.aEx, Ex);
+    a = M3DK_FMA(cw.aEy, Ey, a); a = M3DK_FMA(cw.aEz, pf.EZ, a);
+    a = M3DK_FMA(cw.bBx, Bx, a); a = M3DK_FMA(cw.bBy, By, a); a = M3DK_FMA(cw.bBz, pf.BZ, a);
+    a = M3DK_FMA(cw.gGx, Gx, a); a = M3DK_FMA(cw.gGy, Gy, a); a = M3DK_FMA(cw.gGz, pf.gZ, a);
+    return M3DK_FMA(cw.dT, pf.dT, a);
+}
+
+// kFlr = 1: the lane evaluates its four ring points itself, each searched and evaluated on its own element's tile (global
+// memory: the ring leaves the marker's element).  (g, zl) = cylindrical map and z of x_l.
+__device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
+                                           const PertW &W) {
+    FlrRing rg;
+    flr_ring(P, f, g, mu, rg);
+    FlrW cw;
+    flr_cart_weights(W, g.cph, g.sph, cw);
+    double sum = 0.0;
 #pragma unroll 1
     for (int j = 0; j < 4; ++j) {
-        const double sg = j < 2 ? rho : -rho;
-        const double x = M3DK_FMA(sg, ex[j & 1], X), y = M3DK_FMA(sg, ey[j & 1], Y), z = M3DK_FMA(sg, ez[j & 1], zl);
         Marker sp;
-        sp.x = x; sp.y = y; sp.z = z;
+        flr_ring_point(rg, zl, j, sp.x, sp.y, sp.z);
         StepGeom gj[1];
         step_geometry(sp, gj[0]);
-        const int ej = locate_any(P.f, gj[0].R, z);
-        if (ej < 0) continue;
-        const double *tile = P.f.tiles + (size_t)ej * P.f.tile_stride;
-        const Quad hd = ldq(tile);
-        const double se = hd.c;
-        const double xi[1] = {__dmul_rn(__dsub_rn(gj[0].R, hd.a), se)}, eta[1] = {__dmul_rn(__dsub_rn(z, hd.b), se)};
-        PertF pf[1];
-        pf[0].ER = pf[0].EP = pf[0].EZ = pf[0].BR = pf[0].BP = pf[0].BZ = pf[0].gR = pf[0].gP = pf[0].gZ = pf[0].dT = 0.0;
-        pert_fields<1, false>(P, tile, xi, eta, gj, se, pf);
-        const double cj = gj[0].cph, sj = gj[0].sph;
-        Ex = __dadd_rn(Ex, M3DK_FMA(pf[0].ER, cj, -__dmul_rn(pf[0].EP, sj))); Ey = __dadd_rn(Ey, M3DK_FMA(pf[0].ER, sj, __dmul_rn(pf[0].EP, cj)));
-        Ez = __dadd_rn(Ez, pf[0].EZ);
-        Bx = __dadd_rn(Bx, M3DK_FMA(pf[0].BR, cj, -__dmul_rn(pf[0].BP, sj))); By = __dadd_rn(By, M3DK_FMA(pf[0].BR, sj, __dmul_rn(pf[0].BP, cj)));
-        Bz = __dadd_rn(Bz, pf[0].BZ);
-        Gx = __dadd_rn(Gx, M3DK_FMA(pf[0].gR, cj, -__dmul_rn(pf[0].gP, sj))); Gy = __dadd_rn(Gy, M3DK_FMA(pf[0].gR, sj, __dmul_rn(pf[0].gP, cj)));
-        Gz = __dadd_rn(Gz, pf[0].gZ);
-        dT = __dadd_rn(dT, pf[0].dT);
+        const int ej = locate_any(P.f, gj[0].R, sp.z);
+        double cj = 0.0;
+        if (ej >= 0) {
+            const double *tile = P.f.tiles + (size_t)ej * P.f.tile_stride;
+            const Quad hd = ldq(tile);
+            const double se = hd.c;
+            const double xi[1] = {__dmul_rn(__dsub_rn(gj[0].R, hd.a), se)}, eta[1] = {__dmul_rn(__dsub_rn(sp.z, hd.b), se)};
+            PertF pf[1];
+            pf[0].ER = pf[0].EP = pf[0].EZ = pf[0].BR = pf[0].BP = pf[0].BZ = pf[0].gR = pf[0].gP = pf[0].gZ = pf[0].dT = 0.0;
+            pert_fields<1, false>(P, tile, xi, eta, gj, se, pf);
+            cj = flr_fold(pf[0], gj[0].cph, gj[0].sph, cw);
+        }
+        sum = j == 0 ? cj : __dadd_rn(sum, cj);
     }
-    // back to the marker's frame, quarter sum (Eq. 14), then the linear right-hand side of Eqs. (8)-(13)
-    const double ER = __dmul_rn(0.25, M3DK_FMA(Ex, c, __dmul_rn(Ey, sn))), EP = __dmul_rn(0.25, M3DK_FMA(Ey, c, -__dmul_rn(Ex, sn)));
-    const double B1R = __dmul_rn(0.25, M3DK_FMA(Bx, c, __dmul_rn(By, sn)));
-    const double gR = __dmul_rn(0.25, M3DK_FMA(Gx, c, __dmul_rn(Gy, sn))), gP = __dmul_rn(0.25, M3DK_FMA(Gy, c, -__dmul_rn(Gx, sn)));
-    double a = __dmul_rn(W.aER, ER);
-    a = M3DK_FMA(W.aEP, EP, a); a = M3DK_FMA(W.aEZ, __dmul_rn(0.25, Ez), a);
-    a = M3DK_FMA(W.bBR, B1R, a); a = M3DK_FMA(W.bBZ, __dmul_rn(0.25, Bz), a);
-    a = M3DK_FMA(W.gR, gR, a); a = M3DK_FMA(W.gP, gP, a); a = M3DK_FMA(W.gZ, __dmul_rn(0.25, Gz), a);
-    return M3DK_FMA(W.dT, __dmul_rn(0.25, dT), a);
+    return __dmul_rn(0.25, sum);
+}
+
+// kFlr = 2: emit the four ring points of the marker in output slot `slot` into the ring stream: position, element (the
+// key of the ring ordering, n_elems = outside the mesh) with its rank from the ring histogram, and the marker's weights.
+__device__ __forceinline__ void flr_emit(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
+                                         const PertW &W, long slot) {
+    FlrRing rg;
+    flr_ring(P, f, g, mu, rg);
+    FlrW cw;
+    flr_cart_weights(W, g.cph, g.sph, cw);
+    double *wt = P.fl.wts + 10 * slot;
+    wt[0] = cw.aEx; wt[1] = cw.aEy; wt[2] = cw.aEz; wt[3] = cw.bBx; wt[4] = cw.bBy; wt[5] = cw.bBz;
+    wt[6] = cw.gGx; wt[7] = cw.gGy; wt[8] = cw.gGz; wt[9] = cw.dT;
+#pragma unroll 1
+    for (int j = 0; j < 4; ++j) {
+        Marker sp;
+        flr_ring_point(rg, zl, j, sp.x, sp.y, sp.z);
+        StepGeom gj;
+        step_geometry(sp, gj);                            // the same R as the evaluation will see
+        const double x = sp.x, y = sp.y, z = sp.z;
+        const int ej = locate_any(P.f, gj.R, z);
+        const int key = ej < 0 ? P.f.n_elems : ej;
+        const long idx = 4 * slot + j;
+        strec256(P.fl.ring + 4 * idx, x, y, z, 0.0);
+        P.fl.rkey[idx] = key;
+        P.fl.rrank[idx] = atomicAdd(P.fl.rhist + key, 1);
+    }
 }
 
 // ---- the same step in the non-linear trajectory mode (mode 1: PAPER.md:108, :130; reading G21) ------------------------
@@ -436,7 +494,7 @@ __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant
         double Rn[1], Zn[1];
         const SoAIO io{P.a, P.f.n_elems};
         if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on, Rn, Zn);
-        else step_R<1, false, false, SoAIO, kMode == 2>(P, io, tile, m, m, on, Rn, Zn);
+        else step_R<1, false, false, SoAIO, kMode == 2 ? 1 : 0>(P, io, tile, m, m, on, Rn, Zn);
     }
 }
 
@@ -532,6 +590,8 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
                     io.load_pos(mi[r], a0, a1, a2, a3); io.load_vel(mi[r], b0, b1, b2, b3);
                     io.store_pos(mo[r], a0, a1, a2, a3); io.store_vel(mo[r], b0, b1, b2, b3);
                     io.store_key(mo[r], -1);
+                    if (kMode == 3)                      // no ring for a lost marker: its slot is skipped by the ring kernels
+                        for (int j = 0; j < 4; ++j) P.fl.rkey[4 * mo[r] + j] = -1;
                 }
             }
             if (kHist) {
@@ -545,7 +605,7 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
             phase ^= 1u << b;
             double Rn[kR], Zn[kR];
             if (kMode == 1) step_R_nl<kR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
-            else step_R<kR, kHist, true, RecIO, kMode == 2>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
+            else step_R<kR, kHist, true, RecIO, kMode == 2 ? 1 : (kMode == 3 ? 2 : 0)>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
         }
         b ^= 1;
         it = it1; it1 = it2; it2 = 3 * stride + __shfl_sync(0xffffffffu, ticket, 0);
@@ -555,6 +615,87 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
     }
 }
 
+
+// ---- mode 2, ordered: evaluation of the ring stream ---------------------------------------------------------------------
+// The ring points emitted by push_items_kernel<.., 3, ..> are ordered by THEIR element (histogram fused into the emit,
+// scan + work-item cut + placement: the kernels of the marker ordering) and a warp takes a ring item: up to 64 ring points
+// of one element, kR per lane, the element's tile staged in shared memory by a bulk copy (double-buffered, items by
+// ticket: the machinery of push_items_kernel).  A lane gathers its points (32 B) and the weights of the markers that own
+// them (80 B), evaluates all perturbed polynomials at the points (pert_fields with broadcast coefficient reads shared by
+// the lane's points) and stores the scalar contribution c_j of each point.
+template <int kR>
+__global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 1 : M3DK_PUSH_MINBLOCKS) ring_items_kernel(const __grid_constant__ PushParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int kWarps = kPushThreads / 32;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int stride_d = P.f.tile_stride;
+    const unsigned tile_bytes = (unsigned)stride_d * 8u;
+    double *const tbuf = reinterpret_cast<double *>(smem_raw) + (size_t)warp * 2 * stride_d;
+    unsigned long long *const bars = reinterpret_cast<unsigned long long *>(smem_raw + (size_t)kWarps * 2 * tile_bytes) + warp * 2;
+    const unsigned bar0 = smem_u32(bars), buf0 = smem_u32(tbuf);
+    if (lane == 0) {
+        mbar_init(bar0); mbar_init(bar0 + 8);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    const int total = *P.n_items;
+    const int stride = gridDim.x * kWarps;
+    const int4 none = make_int4(P.f.n_elems, 0, 0, 0);
+    int it = blockIdx.x * kWarps + warp, it1 = it + stride, it2 = it + 2 * stride;
+    int4 w0 = it < total ? __ldg(P.items + it) : none;
+    int4 w1 = it1 < total ? __ldg(P.items + it1) : none;
+    unsigned b = 0, phase = 0;
+    if (w0.x < P.f.n_elems && lane == 0) tile_copy_issue(buf0, P.f.tiles + (size_t)w0.x * stride_d, tile_bytes, bar0);
+    while (it < total) {
+        const int e = w0.x, start = w0.y, count = w0.z;
+        const int4 w2 = it2 < total ? __ldg(P.items + it2) : none;
+        int ticket = 0;
+        if (lane == 0) ticket = atomicAdd(P.ticket, 1);
+        __syncwarp();                                  // every lane has finished reading buffer b ^ 1 (previous item)
+        if (w1.x < P.f.n_elems && lane == 0)
+            tile_copy_issue(buf0 + (b ^ 1) * tile_bytes, P.f.tiles + (size_t)w1.x * stride_d, tile_bytes, bar0 + (b ^ 1) * 8);
+        long idx[kR];
+        bool on[kR];
+        Marker sp[kR];
+        FlrW cw[kR];
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            on[r] = 32 * r + lane < count;
+            idx[r] = on[r] ? P.fl.rorder[start + 32 * r + lane] : 0;
+            double pad;
+            if (on[r]) ldrec256(P.fl.ring + 4 * idx[r], sp[r].x, sp[r].y, sp[r].z, pad);
+            else { sp[r].x = 1.0; sp[r].y = 0.0; sp[r].z = 0.0; }
+        }
+        if (e < P.f.n_elems) {                          // (ring points outside the mesh contribute zero: written by the placement)
+            mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
+            phase ^= 1u << b;
+            const double *tile = tbuf + (size_t)b * stride_d;
+            const Quad hd = ldq_t<true>(tile);
+            const double se = hd.c;
+            StepGeom g[kR];
+            double xi[kR], eta[kR];
+            PertF pf[kR];
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                step_geometry(sp[r], g[r]);
+                xi[r] = __dmul_rn(__dsub_rn(g[r].R, hd.a), se); eta[r] = __dmul_rn(__dsub_rn(sp[r].z, hd.b), se);
+                pf[r].ER = pf[r].EP = pf[r].EZ = pf[r].BR = pf[r].BP = pf[r].BZ = pf[r].gR = pf[r].gP = pf[r].gZ = pf[r].dT = 0.0;
+            }
+            pert_fields<kR, true>(P, tile, xi, eta, g, se, pf);
+#pragma unroll
+            for (int r = 0; r < kR; ++r)
+                if (on[r]) {
+                    const double *wt = P.fl.wts + 10 * (idx[r] >> 2);
+                    cw[r].aEx = wt[0]; cw[r].aEy = wt[1]; cw[r].aEz = wt[2]; cw[r].bBx = wt[3]; cw[r].bBy = wt[4];
+                    cw[r].bBz = wt[5]; cw[r].gGx = wt[6]; cw[r].gGy = wt[7]; cw[r].gGz = wt[8]; cw[r].dT = wt[9];
+                    P.fl.contrib[idx[r]] = flr_fold(pf[r], g[r].cph, g[r].sph, cw[r]);
+                }
+        }
+        b ^= 1;
+        it = it1; it1 = it2; it2 = 3 * stride + __shfl_sync(0xffffffffu, ticket, 0);
+        w0 = w1; w1 = w2;
+    }
+}
 
 // ---- element-ordered push with asynchronous staging (modes 0 and 1) ---------------------------------------------------
 // The same work decomposition as push_items_kernel (a warp takes a work item of one element, a lane up to kR of its
@@ -765,7 +906,7 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
             mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
             phase ^= 1u << b;
             if (kMode == 1) step_R_nl<kR, kHist, true, AsyncIO<kR>, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
-            else step_R<kR, kHist, true, AsyncIO<kR>, false, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
+            else step_R<kR, kHist, true, AsyncIO<kR>, 0, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
         }
         cp_async_wait<2>();                            // the search records of item k - 1 have landed
         search_prev(k - 1);
@@ -892,6 +1033,12 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
         cudaError_t e = cudaMemsetAsync(c->sb.hist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
         if (e != cudaSuccess) return e;
     }
+    const bool flr_stream = c->mode == 2 && c->have_flrws && c->f.n_modes > 0;
+    if (flr_stream) {
+        P.fl = c->fb.a;
+        cudaError_t e = cudaMemsetAsync(c->fb.a.rhist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
+        if (e != cudaSuccess) return e;
+    }
     {
         P.rc.out = c->sb.rec[c->cur ^ 1];
         P.items = c->sb.items; P.n_items = c->sb.ioffs + c->f.n_elems + 1;
@@ -922,20 +1069,44 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
                 c->ranks_valid = false;      // this kernel only counts; invert_kernel draws the slots
                 continue;
             }
+            // mode 2: with an FLR workspace the push emits the ring stream (kernel mode 3), else every lane gathers its ring
+            const int km = c->mode == 2 ? (flr_stream ? 3 : (c->f.n_modes > 0 ? 2 : 0)) : c->mode;
             if (small)
-                kern = c->mode == 1   ? (with_hist ? push_items_kernel<true, 1, 1> : push_items_kernel<false, 1, 1>)
-                       : c->mode == 2 ? (with_hist ? push_items_kernel<true, 2, 1> : push_items_kernel<false, 2, 1>)
-                                      : (with_hist ? push_items_kernel<true, 0, 1> : push_items_kernel<false, 0, 1>);
+                kern = km == 1   ? (with_hist ? push_items_kernel<true, 1, 1> : push_items_kernel<false, 1, 1>)
+                       : km == 2 ? (with_hist ? push_items_kernel<true, 2, 1> : push_items_kernel<false, 2, 1>)
+                       : km == 3 ? (with_hist ? push_items_kernel<true, 3, 1> : push_items_kernel<false, 3, 1>)
+                                 : (with_hist ? push_items_kernel<true, 0, 1> : push_items_kernel<false, 0, 1>);
             else
-                kern = c->mode == 1   ? (with_hist ? push_items_kernel<true, 1, 2> : push_items_kernel<false, 1, 2>)
-                       : c->mode == 2 ? (with_hist ? push_items_kernel<true, 2, 2> : push_items_kernel<false, 2, 2>)
-                                      : (with_hist ? push_items_kernel<true, 0, 2> : push_items_kernel<false, 0, 2>);
+                kern = km == 1   ? (with_hist ? push_items_kernel<true, 1, 2> : push_items_kernel<false, 1, 2>)
+                       : km == 2 ? (with_hist ? push_items_kernel<true, 2, 2> : push_items_kernel<false, 2, 2>)
+                       : km == 3 ? (with_hist ? push_items_kernel<true, 3, 2> : push_items_kernel<false, 3, 2>)
+                                 : (with_hist ? push_items_kernel<true, 0, 2> : push_items_kernel<false, 0, 2>);
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
             if (small) c->kernel_launches += 1;
             kern<<<small ? grid / M3DK_PUSH_MINBLOCKS * (M3DK_PUSH_MINBLOCKS + 1) : grid, kPushThreads, smem, c->stream>>>(P);
         }
         c->cur ^= 1;
+    }
+    return cudaGetLastError();
+}
+
+// evaluation of the ordered ring stream (mode 2): the ring items of up to 64 points, then the small ones
+cudaError_t launch_flr_ring_eval(m3dk_ctx *c, long n, double dt, double t) {
+    if (n == 0) return cudaSuccess;
+    PushParams P = make_params(c, c->user, n, dt, t);
+    P.fl = c->fb.a;
+    const size_t smem = (size_t)(kPushThreads / 32) * 2 * (c->f.tile_stride * 8 + 8);
+    const unsigned grid = (unsigned)(c->sm_count * M3DK_PUSH_MINBLOCKS);
+    for (int small = 0; small < 2; ++small) {
+        P.items = small ? c->fb.ritems_small : c->fb.ritems;
+        P.n_items = small ? reinterpret_cast<const int *>(c->fb.rstate + 1) : c->fb.rioffs + c->f.n_elems + 1;
+        P.ticket = reinterpret_cast<int *>(c->fb.rstate + (c->f.n_elems + 1 + 4095) / 4096 + 2) + small;
+        void (*kern)(PushParams) = small ? ring_items_kernel<1> : ring_items_kernel<2>;
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        c->kernel_launches += 1;
+        kern<<<small ? grid / M3DK_PUSH_MINBLOCKS * (M3DK_PUSH_MINBLOCKS + 1) : grid, kPushThreads, smem, c->stream>>>(P);
     }
     return cudaGetLastError();
 }

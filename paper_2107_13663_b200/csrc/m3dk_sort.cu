@@ -216,16 +216,98 @@ __global__ void __launch_bounds__(256) unpack_kernel(MarkerArrays a, long n, int
     a.elem[j] = k >= n_elems ? -1 : k;
 }
 
-static cudaError_t scan_and_cut(m3dk_ctx *c) {
+// scan of a histogram of m = n_elems + 1 bins into segment offsets, work-item cut (shared by the marker ordering and the
+// ring ordering of the FLR mode)
+static cudaError_t scan_and_cut_arrays(m3dk_ctx *c, int *hist, int *offs, int *ioffs, int4 *items, int4 *items_small,
+                                       unsigned long long *state) {
     const int m = c->f.n_elems + 1;
     c->kernel_launches += 2;
     const int nchunks = (m + kScanChunk - 1) / kScanChunk;
     // ticket and per-chunk words cleared together (a few hundred bytes): a word is ready when its tag is set
-    cudaError_t e = cudaMemsetAsync(c->sb.scan_state, 0, (size_t)(nchunks + 3) * sizeof(unsigned long long), c->stream);
+    cudaError_t e = cudaMemsetAsync(state, 0, (size_t)(nchunks + 3) * sizeof(unsigned long long), c->stream);
     if (e != cudaSuccess) return e;
-    scan_kernel<<<nchunks, 1024, 0, c->stream>>>(c->sb.hist, m, c->sb.offs, c->sb.ioffs, c->sb.scan_state, 1u);
-    items_kernel<<<(m + 255) / 256, 256, 0, c->stream>>>(c->sb.offs, c->sb.ioffs, m, c->sb.items, c->sb.items_small,
-                                                        reinterpret_cast<int *>(c->sb.scan_state + 1));
+    scan_kernel<<<nchunks, 1024, 0, c->stream>>>(hist, m, offs, ioffs, state, 1u);
+    items_kernel<<<(m + 255) / 256, 256, 0, c->stream>>>(offs, ioffs, m, items, items_small, reinterpret_cast<int *>(state + 1));
+    return cudaGetLastError();
+}
+static cudaError_t scan_and_cut(m3dk_ctx *c) {
+    return scan_and_cut_arrays(c, c->sb.hist, c->sb.offs, c->sb.ioffs, c->sb.items, c->sb.items_small, c->sb.scan_state);
+}
+
+// ---- ring stream of the ordered FLR mode ----------------------------------------------------------------------------------
+size_t flr_workspace_bytes(long n, int n_elems) {
+    const size_t n4 = 4 * (size_t)n;
+    const size_t nh = up256((size_t)(n_elems + 2) * sizeof(int));
+    return up256(n4 * 4 * sizeof(double)) + up256((size_t)n * 10 * sizeof(double)) + up256(n4 * sizeof(double)) +
+           3 * up256(n4 * sizeof(int)) + 3 * nh + up256((n4 / kItemMarkers + n_elems + 2) * sizeof(int4)) +
+           up256((size_t)(n_elems + 2) * sizeof(int4)) + up256(((size_t)(n_elems + 1) / 4096 + 6) * sizeof(unsigned long long));
+}
+
+void carve_flr_workspace(void *ws, long n, int n_elems, FlrBuffers *fb) {
+    char *p = static_cast<char *>(ws);
+    const size_t n4 = 4 * (size_t)n;
+    const size_t nh = up256((size_t)(n_elems + 2) * sizeof(int));
+    fb->a.ring = reinterpret_cast<double *>(p); p += up256(n4 * 4 * sizeof(double));
+    fb->a.wts = reinterpret_cast<double *>(p); p += up256((size_t)n * 10 * sizeof(double));
+    fb->a.contrib = reinterpret_cast<double *>(p); p += up256(n4 * sizeof(double));
+    fb->a.rkey = reinterpret_cast<int *>(p); p += up256(n4 * sizeof(int));
+    fb->a.rrank = reinterpret_cast<int *>(p); p += up256(n4 * sizeof(int));
+    fb->a.rorder = reinterpret_cast<int *>(p); p += up256(n4 * sizeof(int));
+    fb->a.rhist = reinterpret_cast<int *>(p); p += nh;
+    fb->roffs = reinterpret_cast<int *>(p); p += nh;
+    fb->rioffs = reinterpret_cast<int *>(p); p += nh;
+    fb->ritems = reinterpret_cast<int4 *>(p); p += up256((n4 / kItemMarkers + n_elems + 2) * sizeof(int4));
+    fb->ritems_small = reinterpret_cast<int4 *>(p); p += up256((size_t)(n_elems + 2) * sizeof(int4));
+    fb->rstate = reinterpret_cast<unsigned long long *>(p); p += up256(((size_t)(n_elems + 1) / 4096 + 6) * sizeof(unsigned long long));
+    fb->bytes = (size_t)(p - static_cast<char *>(ws));
+}
+
+// ring point i goes to position offs[key] + rank of the element-ordered ring list; a point outside the mesh contributes
+// zero; points of a lost marker's slot (key -1) are not in the list
+__global__ void __launch_bounds__(256) ring_place_kernel(long n4, int n_elems, const int *__restrict__ rkey,
+                                                         const int *__restrict__ rrank, const int *__restrict__ roffs,
+                                                         int *__restrict__ rorder, double *__restrict__ contrib) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n4) return;
+    const int k = rkey[i];
+    if (k < 0) return;
+    rorder[(long)roffs[k] + rrank[i]] = (int)i;
+    if (k >= n_elems) contrib[i] = 0.0;
+}
+
+// Eq. (14) and the weight update (readings G9, G23): w_{l+1/2} = w_{l-1/2} + dt * 0.25 (((c_0 + c_1) + c_2) + c_3) on the
+// records the push has just written (their w is still the old one)
+__global__ void __launch_bounds__(256) flr_reduce_kernel(long n, double dt, const int *__restrict__ rkey,
+                                                         const double *__restrict__ contrib, double *__restrict__ rec) {
+    const long d = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (d >= n) return;
+    if (rkey[4 * d] < 0) return;                       // the slot holds a marker that was lost before this step
+    const double4 c = *reinterpret_cast<const double4 *>(contrib + 4 * d);
+    const double sum = __dadd_rn(__dadd_rn(__dadd_rn(c.x, c.y), c.z), c.w);
+    double *w = rec + kRecDoubles * d + 3;
+#ifdef M3DK_NO_FMA
+    *w = __dadd_rn(__dmul_rn(dt, __dmul_rn(0.25, sum)), *w);
+#else
+    *w = fma(dt, __dmul_rn(0.25, sum), *w);
+#endif
+}
+
+cudaError_t launch_flr_ring_stage(m3dk_ctx *c, long n) {
+    if (n == 0) return cudaSuccess;
+    FlrBuffers &fb = c->fb;
+    cudaError_t e = scan_and_cut_arrays(c, fb.a.rhist, fb.roffs, fb.rioffs, fb.ritems, fb.ritems_small, fb.rstate);
+    if (e != cudaSuccess) return e;
+    c->kernel_launches += 1;
+    const long n4 = 4 * n;
+    ring_place_kernel<<<(unsigned)((n4 + 255) / 256), 256, 0, c->stream>>>(n4, c->f.n_elems, fb.a.rkey, fb.a.rrank, fb.roffs,
+                                                                          fb.a.rorder, fb.a.contrib);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_flr_reduce(m3dk_ctx *c, long n, double dt) {
+    if (n == 0) return cudaSuccess;
+    c->kernel_launches += 1;
+    flr_reduce_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, dt, c->fb.a.rkey, c->fb.a.contrib, c->sb.rec[c->cur]);
     return cudaGetLastError();
 }
 

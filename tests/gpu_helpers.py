@@ -27,12 +27,15 @@ def take(markers: dict, idx):
     return {k: np.ascontiguousarray(markers[k][idx]) for k in KEYS}
 
 
-def make_pusher(w, verify=True, markers=None, sort_interval=0, t0=0.0, mode=0):
+def make_pusher(w, verify=True, markers=None, sort_interval=0, t0=0.0, mode=0, flr_ws=True):
+    """flr_ws: in mode 2 with the ordered pipeline, also lend the FLR workspace (ring stream); False = every lane gathers."""
     p = m3dk.Pusher(device=0, verify=verify)
     p.fields_create(w.node_RZ, w.tri, w.eq_coef, w.n_tor if w.n_modes else None, w.omega if w.n_modes else None,
                     w.pert_coef if w.n_modes else None)
     p.particles_init(w.markers if markers is None else markers, w.charge, w.mass, w.f0)
     p.set_options(sort_interval=sort_interval, mode=mode, t0=t0)
+    if mode == 2 and sort_interval > 0 and flr_ws:
+        p.set_flr_workspace()
     return p
 
 

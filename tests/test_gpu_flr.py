@@ -52,8 +52,8 @@ def test_flr_ordered_pipeline_and_bitwise_order_independence(two_modes):
     nsteps = 5
     ref, e_ref, _ = oracle_push(mesh, sp, w.markers, nsteps, w.dt)
     res = {}
-    for si in (0, 1, 3):
-        p = make_pusher(w, verify=True, sort_interval=si, mode=2)
+    for si in (0, 1, 3, -1):                       # -1: ordered pipeline WITHOUT the FLR workspace (every lane gathers)
+        p = make_pusher(w, verify=True, sort_interval=abs(si), mode=2, flr_ws=si > 0)
         p.push(nsteps, w.dt)
         got, elem, ids = p.state()
         assert np.array_equal(np.sort(ids), np.arange(w.n_markers))
@@ -62,9 +62,42 @@ def test_flr_ordered_pipeline_and_bitwise_order_independence(two_modes):
         wrms = np.sqrt(np.mean(ref["w"][live] ** 2))
         ex, ev, ew = g16_errors(take(got, live), take(ref, live), w_floor=wrms)
         assert max(ex.max(), ev.max(), ew.max()) <= 5 * TOL_STEP, (si, ex.max(), ev.max(), ew.max())
-    for si in (1, 3):
+    for si in (1, 3, -1):
         for k in KEYS:
             assert np.array_equal(res[si][k], res[0][k]), (si, k)
+
+
+@pytest.mark.parametrize("verify", [True, False])
+def test_flr_ring_stream_per_step_parity_with_lost_markers(verify):
+    """The ordered FLR path (ring points emitted, ordered by their element, evaluated with staged tiles, summed back):
+    one step restarted from the oracle at steps 0 and 7, config 3 shape, with markers outside the mesh from the start and
+    ring points that fall outside it (markers at the edge of the box)."""
+    import dataclasses
+    w0 = synth.make_config(3, n_markers=9000 + 5, nx=64)
+    mk = {k: v.copy() for k, v in w0.markers.items()}
+    mk["x"][:9] = 20.0                                      # lost from the start: no ring
+    mk["z"][9:60] = 1.0995                                  # at the upper edge: part of the ring is outside the mesh
+    w = dataclasses.replace(w0, markers=mk)
+    mesh, sp = oracle_of(w, mode=2)
+    p = make_pusher(w, verify=verify, sort_interval=1, mode=2)
+    state = {k: mk[k].copy() for k in KEYS}
+    done = 0
+    for s in (0, 7):
+        if s > done:
+            state, _, _ = oracle_push(mesh, sp, state, s - done, w.dt, t0=0.0, step0=done)
+            done = s
+        ref, e_ref, _ = oracle_push(mesh, sp, state, 1, w.dt, t0=0.0, step0=s)
+        p.set_state(state)
+        p.set_options(sort_interval=1, mode=2, t0=s * w.dt)
+        p.push(1, w.dt)
+        got, _, ids = p.state()
+        assert np.array_equal(np.sort(ids), np.arange(w.n_markers))
+        live = e_ref >= 0
+        for k in KEYS:
+            assert np.array_equal(got[k][~live], state[k][~live])
+        wrms = np.sqrt(np.mean(ref["w"][live] ** 2))
+        ex, ev, ew = g16_errors(take(got, live), take(ref, live), w_floor=wrms)
+        assert max(ex.max(), ev.max(), ew.max()) <= TOL_STEP, (s, ex.max(), ev.max(), ew.max())
 
 
 def test_flr_where_b_is_parallel_to_the_major_radius():
