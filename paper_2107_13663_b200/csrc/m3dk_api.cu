@@ -565,6 +565,7 @@ static int run_steps(m3dk_ctx *ctx, int nsteps, double dt) {
             CU(launch_push_rec(ctx, ctx->n, dt, t, reorder_after), "push kernel");
             if (ctx->mode == 2 && ctx->have_flrws && ctx->f.n_modes > 0) {
                 // the push has emitted the ring stream: order it by the ring points' elements, evaluate, sum back into w
+                CU(launch_flr_ring_keys(ctx, ctx->n), "ring key kernel");
                 CU(launch_flr_ring_stage(ctx, ctx->n), "ring ordering kernels");
                 CU(launch_flr_ring_eval(ctx, ctx->n, dt, t), "ring evaluation kernel");
                 CU(launch_flr_reduce(ctx, ctx->n, dt), "ring reduction kernel");

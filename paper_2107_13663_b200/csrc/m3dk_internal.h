@@ -218,6 +218,7 @@ cudaError_t launch_gc_push(m3dk_ctx *c, long n, double *vpar, int nsteps, double
 cudaError_t launch_gc_bootstrap(m3dk_ctx *c, long n, const double *vpar, double dt);     // (x_1, v_{1/2}) from one such step
 cudaError_t fp64_probe(m3dk_ctx *c, double *tflops);
 
+cudaError_t launch_flr_ring_keys(m3dk_ctx *c, long n);    // element + rank of every ring point (push.cu)
 cudaError_t launch_flr_ring_stage(m3dk_ctx *c, long n);   // ring histogram -> offsets, ring items, ring order
 cudaError_t launch_flr_ring_eval(m3dk_ctx *c, long n, double dt, double t);   // ring_items_kernel (push.cu)
 cudaError_t launch_flr_reduce(m3dk_ctx *c, long n, double dt);   // w += dt * quarter sum of the contributions

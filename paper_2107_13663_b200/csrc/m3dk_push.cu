@@ -383,8 +383,9 @@ __device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, 
     return __dmul_rn(0.25, sum);
 }
 
-// kFlr = 2: emit the four ring points of the marker in output slot `slot` into the ring stream: position, element (the
-// key of the ring ordering, n_elems = outside the mesh) with its rank from the ring histogram, and the marker's weights.
+// kFlr = 2: emit the four ring points of the marker in output slot `slot` into the ring stream (positions, flagged live)
+// and the marker's weights.  Their elements are found by ring_key_kernel, one thread per ring point: four searches and
+// four returned atomics in a row inside the push would serialise eight L2 round trips per marker.
 __device__ __forceinline__ void flr_emit(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
                                          const PertW &W, long slot) {
     FlrRing rg;
@@ -394,19 +395,45 @@ __device__ __forceinline__ void flr_emit(const PushParams &P, const EqOut &f, co
     double *wt = P.fl.wts + 10 * slot;
     wt[0] = cw.aEx; wt[1] = cw.aEy; wt[2] = cw.aEz; wt[3] = cw.bBx; wt[4] = cw.bBy; wt[5] = cw.bBz;
     wt[6] = cw.gGx; wt[7] = cw.gGy; wt[8] = cw.gGz; wt[9] = cw.dT;
-#pragma unroll 1
+#pragma unroll
     for (int j = 0; j < 4; ++j) {
+        double x, y, z;
+        flr_ring_point(rg, zl, j, x, y, z);
+        strec256(P.fl.ring + 4 * (4 * slot + j), x, y, z, 1.0);
+    }
+}
+
+// element of every ring point (the key of the ring ordering; n_elems = outside the mesh, -1 = the slot of a lost marker)
+// and its rank inside the key, from the ring histogram (warp-aggregated atomics)
+__global__ void __launch_bounds__(256) ring_key_kernel(const __grid_constant__ FieldParams f, long n4,
+                                                       const double *__restrict__ ring, int *__restrict__ rkey,
+                                                       int *__restrict__ rrank, int *__restrict__ rhist, unsigned cstride) {
+    // ring points are in the order of the markers' elements, so neighbouring blocks would hit the same few histogram bins
+    // at the same time: block b takes chunk (b * cstride) mod gridDim.x (cstride coprime with the grid)
+    const long i = (long)(((unsigned long long)blockIdx.x * cstride) % gridDim.x) * blockDim.x + threadIdx.x;
+    bool on = i < n4;
+    int key = 0;
+    if (on) {
         Marker sp;
-        flr_ring_point(rg, zl, j, sp.x, sp.y, sp.z);
-        StepGeom gj;
-        step_geometry(sp, gj);                            // the same R as the evaluation will see
-        const double x = sp.x, y = sp.y, z = sp.z;
-        const int ej = locate_any(P.f, gj.R, z);
-        const int key = ej < 0 ? P.f.n_elems : ej;
-        const long idx = 4 * slot + j;
-        strec256(P.fl.ring + 4 * idx, x, y, z, 0.0);
-        P.fl.rkey[idx] = key;
-        P.fl.rrank[idx] = atomicAdd(P.fl.rhist + key, 1);
+        double live;
+        ldrec256(ring + 4 * i, sp.x, sp.y, sp.z, live);
+        if (live < 0.0) { rkey[i] = -1; on = false; }
+        else {
+            StepGeom gj;
+            step_geometry(sp, gj);                        // the same R as the evaluation will see
+            const int ej = locate_any(f, gj.R, sp.z);
+            key = ej < 0 ? f.n_elems : ej;
+            rkey[i] = key;
+        }
+    }
+    const unsigned live_mask = __ballot_sync(0xffffffffu, on);
+    if (on) {
+        const unsigned peers = __match_any_sync(live_mask, key);
+        const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
+        int base = 0;
+        if (lane == leader) base = atomicAdd(rhist + key, __popc(peers));
+        base = __shfl_sync(peers, base, leader);
+        rrank[i] = base + __popc(peers & ((1u << lane) - 1u));
     }
 }
 
@@ -591,7 +618,7 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
                     io.store_pos(mo[r], a0, a1, a2, a3); io.store_vel(mo[r], b0, b1, b2, b3);
                     io.store_key(mo[r], -1);
                     if (kMode == 3)                      // no ring for a lost marker: its slot is skipped by the ring kernels
-                        for (int j = 0; j < 4; ++j) P.fl.rkey[4 * mo[r] + j] = -1;
+                        for (int j = 0; j < 4; ++j) strec256(P.fl.ring + 4 * (4 * mo[r] + j), 0.0, 0.0, 0.0, -1.0);
                 }
             }
             if (kHist) {
@@ -1088,6 +1115,19 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
         }
         c->cur ^= 1;
     }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_flr_ring_keys(m3dk_ctx *c, long n) {
+    if (n == 0) return cudaSuccess;
+    const long n4 = 4 * n;
+    c->kernel_launches += 1;
+    const unsigned grid = (unsigned)((n4 + 255) / 256);
+    static const unsigned primes[] = {1009u, 1013u, 1019u, 1021u, 1031u};
+    unsigned cs = 1u;
+    for (unsigned p : primes)
+        if (grid % p != 0) { cs = p; break; }
+    ring_key_kernel<<<grid, 256, 0, c->stream>>>(c->f, n4, c->fb.a.ring, c->fb.a.rkey, c->fb.a.rrank, c->fb.a.rhist, cs);
     return cudaGetLastError();
 }
 
