@@ -276,13 +276,15 @@ def run_ours(args, rank, world, local_rank):
         # row (f)-4 with its exchange step: every rank deposits its shard, the moment tables are summed over the ranks
         need = p.deposit_bytes()
         rhs = torch.empty(need // 8, dtype=torch.float64, device=dev)
-        p.deposit_into(rhs, 1, 0.0)
+        if args.deposit_flags & 2:
+            p.set_flr_workspace()       # ordered ring stream of the 4-point deposition
+        p.deposit_into(rhs, args.deposit_flags, 0.0)
         shard.allreduce_moments(rhs, dist if world > 1 else None)
         barrier()
         d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         d0.record(p.stream)
         for _ in range(5):
-            p.deposit_into(rhs, 1, 0.0)
+            p.deposit_into(rhs, args.deposit_flags, 0.0)
             shard.allreduce_moments(rhs, dist if world > 1 else None)
         d1.record(p.stream)
         barrier()
@@ -342,7 +344,9 @@ def run_ours(args, rank, world, local_rank):
         dbytes = (68.0 * N + need)            # 8 fp64 + element key per marker read, the table cleared and accumulated
         line["deposit"] = {"ms": dms, "markers_per_s": N * world / (dms * 1e-3), "table_bytes": need,
                            "hbm_bytes": dbytes, "hbm_frac": dbytes / (dms * 1e-3) / (hbm_gbs * 1e9),
-                           "note": "m3dk_deposit with the B1par term of Eq. (16), delta-function shape (SURVEY.md 8(f)-4)" +
+                           "flags": args.deposit_flags,
+                           "note": "m3dk_deposit (flags: 1 = B1par term of Eq. 16, 2 = 4-point FLR, 4 = d = w + B1par/B*par), "
+                                   "delta-function shape (SURVEY.md 8(f)-4)" +
                                    (f", then NCCL all-reduce of the {need} B table over {world} ranks" if world > 1 else "")}
     if world == 1 and not args.no_cpu_baseline:
         rate, n, secs, cores, stride, rsteps = oracle_bounded_sample(w, args.ref_sample)
@@ -411,6 +415,7 @@ def main():
                          "2: linear delta-f with the 4-point gyro-average (8(f)-2)")
     ap.add_argument("--gc", action="store_true", help="also time m3dk_gc_push (SURVEY.md 8(f)-3) on the final state")
     ap.add_argument("--deposit", action="store_true", help="also time m3dk_deposit (SURVEY.md 8(f)-4) on the final state")
+    ap.add_argument("--deposit-flags", type=int, default=1, help="flags of the timed m3dk_deposit (1 B1par, 2 FLR, 4 Bstar)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-chunks", type=int, default=4, help="marker chunks of the pipelined host-buffer call (e2e leg)")
     ap.add_argument("--push-variant", type=int, default=0, choices=[0, 1],

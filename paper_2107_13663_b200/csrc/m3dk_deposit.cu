@@ -270,6 +270,129 @@ __global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constan
         }
 }
 
+// ---- 4-point FLR deposition through the ordered ring stream (FLR workspace set) ---------------------------------------
+// The ring points of all markers are emitted (position + the marker's two amplitudes), ordered by THEIR element with the
+// ring-ordering kernels of the FLR push (ring_key_kernel, scan, work-item cut, placement), and a warp deposits a ring item
+// (up to 64 ring points of one element) with shuffle reductions and one atomic per table entry.
+__global__ void __launch_bounds__(128) deposit_flr_emit_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
+                                                               const double *__restrict__ rec, const int *__restrict__ key, long n,
+                                                               double q, double mass, double *__restrict__ ring,
+                                                               double *__restrict__ wts) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int e = key[i];
+    if (e >= f.n_elems) e = -1;
+    if (e < 0) {                                     // lost markers deposit nothing: no ring
+        for (int j = 0; j < 4; ++j) {
+            double *r = ring + 4 * (4 * i + j);
+            r[0] = 0.0; r[1] = 0.0; r[2] = 0.0; r[3] = -1.0;
+        }
+        return;
+    }
+    const double *p = rec + (size_t)kRecDoubles * i;
+    Marker s;
+    s.x = p[0]; s.y = p[1]; s.z = p[2]; s.w = p[3]; s.vx = p[4]; s.vy = p[5]; s.vz = p[6]; s.mu = p[7];
+    DepMarker d;
+    dep_marker(f, o, e, s, mass, d);          // amplitudes at the marker itself
+    wts[10 * i] = d.amp[0]; wts[10 * i + 1] = d.amp[1];
+    // the ring: same construction as the FLR push (reading G23)
+    StepGeom g;
+    step_geometry(s, g);
+    const double *tile = f.tiles + (size_t)e * f.tile_stride;
+    const Quad hd = ldq(tile);
+    const double se0 = hd.c;
+    const double xi1[1] = {__dmul_rn(__dsub_rn(g.R, hd.a), se0)}, eta1[1] = {__dmul_rn(__dsub_rn(s.z, hd.b), se0)};
+    double v[1][4], dx[1][4], de[1][4];
+    Ring rg;
+    ring_fill<false>(rg, tile + kTileHeader);
+    quad_vd<1, false>(tile + kTileHeader, tile + kTileHeader, rg, xi1, eta1, v, dx, de);
+    const double BR = -__dmul_rn(__dmul_rn(de[0][0], se0), g.rinv), BP = __dmul_rn(v[0][2], g.rinv),
+                 BZ = __dmul_rn(__dmul_rn(dx[0][0], se0), g.rinv);
+    const double binv = m3dk_rsqrt(M3DK_FMA(BR, BR, M3DK_FMA(BP, BP, __dmul_rn(BZ, BZ))));
+    const double bR = __dmul_rn(BR, binv), bP = __dmul_rn(BP, binv), bZ = __dmul_rn(BZ, binv);
+    const double rho = __dmul_rn(m3dk_sqrt(__dmul_rn(__dmul_rn(__dmul_rn(2.0, mass), s.mu), binv)), fabs(1.0 / q));
+    double e1R = M3DK_FMA(-bR, bR, 1.0), e1P = -__dmul_rn(bR, bP), e1Z = -__dmul_rn(bR, bZ);
+    if (__dmul_rn(bR, bR) > 0.999999) {   // b (anti)parallel to R-hat: start from Z-hat instead (same rule as the oracle)
+        e1R = -__dmul_rn(bZ, bR); e1P = -__dmul_rn(bZ, bP); e1Z = M3DK_FMA(-bZ, bZ, 1.0);
+    }
+    const double n1 = m3dk_rsqrt(M3DK_FMA(e1R, e1R, M3DK_FMA(e1P, e1P, __dmul_rn(e1Z, e1Z))));
+    e1R = __dmul_rn(e1R, n1); e1P = __dmul_rn(e1P, n1); e1Z = __dmul_rn(e1Z, n1);
+    const double e2R = M3DK_FMA(bP, e1Z, -__dmul_rn(bZ, e1P)), e2P = M3DK_FMA(bZ, e1R, -__dmul_rn(bR, e1Z)),
+                 e2Z = M3DK_FMA(bR, e1P, -__dmul_rn(bP, e1R));
+    const double c = g.cph, sn = g.sph;
+    const double ex[2] = {M3DK_FMA(e1R, c, -__dmul_rn(e1P, sn)), M3DK_FMA(e2R, c, -__dmul_rn(e2P, sn))};
+    const double ey[2] = {M3DK_FMA(e1R, sn, __dmul_rn(e1P, c)), M3DK_FMA(e2R, sn, __dmul_rn(e2P, c))};
+    const double ez[2] = {e1Z, e2Z};
+    const double X = __dmul_rn(g.R, c), Y = __dmul_rn(g.R, sn);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const double sg = j < 2 ? rho : -rho;
+        double *r = ring + 4 * (4 * i + j);
+        r[0] = M3DK_FMA(sg, ex[j & 1], X); r[1] = M3DK_FMA(sg, ey[j & 1], Y); r[2] = M3DK_FMA(sg, ez[j & 1], s.z); r[3] = 1.0;
+    }
+}
+
+template <int kR>
+__global__ void __launch_bounds__(128) deposit_ring_items_kernel(const __grid_constant__ FieldParams f, const double *__restrict__ ring,
+                                                                 const double *__restrict__ wts, const int *__restrict__ rorder,
+                                                                 const int4 *__restrict__ items, const int *__restrict__ n_items,
+                                                                 double *__restrict__ rhs) {
+    const int lane = threadIdx.x & 31;
+    const int it = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (it >= *n_items) return;
+    const int4 w = __ldg(items + it);
+    const int e = w.x, start = w.y, count = w.z;
+    if (e >= f.n_elems) return;                      // ring points outside the mesh deposit nothing
+    const int H = 1 + 2 * f.n_modes;
+    const Quad hd = ldq(f.tiles + (size_t)e * f.tile_stride);
+    double amp[kR][2], T[kR][kDepHarmMax], xp[kR][6], ep[kR][6];
+#pragma unroll
+    for (int r = 0; r < kR; ++r) {
+        const bool on = 32 * r + lane < count;
+        Marker sp;
+        sp.x = 1.0; sp.y = 0.0; sp.z = 0.0;
+        amp[r][0] = 0.0; amp[r][1] = 0.0;
+        if (on) {
+            const long idx = rorder[start + 32 * r + lane];
+            const double *p = ring + 4 * idx;
+            sp.x = p[0]; sp.y = p[1]; sp.z = p[2];
+            amp[r][0] = __dmul_rn(0.25, wts[10 * (idx >> 2)]); amp[r][1] = __dmul_rn(0.25, wts[10 * (idx >> 2) + 1]);
+        }
+        StepGeom gj;
+        step_geometry(sp, gj);
+        const double xi = __dmul_rn(__dsub_rn(gj.R, hd.a), hd.c), eta = __dmul_rn(__dsub_rn(sp.z, hd.b), hd.c);
+        xp[r][0] = 1.0; ep[r][0] = 1.0;
+#pragma unroll
+        for (int q = 1; q < 6; ++q) { xp[r][q] = __dmul_rn(xp[r][q - 1], xi); ep[r][q] = __dmul_rn(ep[r][q - 1], eta); }
+        T[r][0] = 1.0;
+#pragma unroll
+        for (int md = 0; md < M3DK_MAX_MODES; ++md)
+            if (md < f.n_modes) mode_phase(f.n_tor[md], gj.cph, gj.sph, 1.0, 0.0, T[r][1 + 2 * md], T[r][2 + 2 * md]);
+    }
+    double *out = rhs + (size_t)e * 2 * H * M3DK_NCOEF;
+    for (int mom = 0; mom < 2; ++mom)
+#pragma unroll
+        for (int h = 0; h < kDepHarmMax; ++h) {
+            if (h >= H) break;
+            double ah[kR];
+#pragma unroll
+            for (int r = 0; r < kR; ++r) ah[r] = __dmul_rn(amp[r][mom], T[r][h]);
+            double *o = out + ((size_t)mom * H + h) * M3DK_NCOEF;
+            int k = 0;
+#pragma unroll
+            for (int j = 0; j < 6; ++j)
+#pragma unroll
+                for (int ii = 0; ii < 6 - j; ++ii, ++k) {
+                    double val = 0.0;
+#pragma unroll
+                    for (int r = 0; r < kR; ++r) val = M3DK_FMA(ah[r], __dmul_rn(xp[r][ii], ep[r][j]), val);
+#pragma unroll
+                    for (int sft = 16; sft > 0; sft >>= 1) val += __shfl_xor_sync(0xffffffffu, val, sft);
+                    if (lane == 0) atomicAdd(o + k, val);
+                }
+        }
+}
+
 cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t) {
     DepOpts o{};
     o.with_b1par = (flags & 1) && c->f.n_modes > 0;
@@ -280,7 +403,27 @@ cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t
     cudaError_t e = cudaMemsetAsync(rhs, 0, bytes, c->stream);
     if (e != cudaSuccess || n == 0) return e;
     if (flags & 2) {   // 4-point FLR deposition: the ring points leave the marker's element, one marker per lane
-        if (c->have_sortws) {
+        if (c->have_sortws && c->have_flrws) {
+            // ordered ring stream: markers into element order, ring points emitted, ordered by their own element, deposited
+            // item by item
+            e = launch_pack_sorted(c, n);
+            if (e != cudaSuccess) return e;
+            e = cudaMemsetAsync(c->fb.a.rhist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
+            if (e != cudaSuccess) return e;
+            c->kernel_launches += 3;
+            deposit_flr_emit_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->sb.rec[c->cur], c->sb.key, n,
+                                                                                       c->q, c->m, c->fb.a.ring, c->fb.a.wts);
+            e = launch_flr_ring_keys(c, n);
+            if (e != cudaSuccess) return e;
+            e = launch_flr_ring_stage(c, n);
+            if (e != cudaSuccess) return e;
+            const long max_items = 4 * n / kItemMarkers + c->f.n_elems + 2, max_small = c->f.n_elems + 2;
+            deposit_ring_items_kernel<2><<<(unsigned)((max_items + 3) / 4), 128, 0, c->stream>>>(
+                c->f, c->fb.a.ring, c->fb.a.wts, c->fb.a.rorder, c->fb.ritems, c->fb.rioffs + c->f.n_elems + 1, rhs);
+            deposit_ring_items_kernel<1><<<(unsigned)((max_small + 3) / 4), 128, 0, c->stream>>>(
+                c->f, c->fb.a.ring, c->fb.a.wts, c->fb.a.rorder, c->fb.ritems_small,
+                reinterpret_cast<const int *>(c->fb.rstate + 1), rhs);
+        } else if (c->have_sortws) {
             e = launch_pack_sorted(c, n);
             if (e != cudaSuccess) return e;
             c->kernel_launches += 1;

@@ -101,11 +101,14 @@ def test_deposit_flr_four_point():
     mk["mu"] = mk["mu"] * 4.0                                   # rings of a few elements; near the edge some points fall outside
     p = make_pusher(dataclasses.replace(w, markers=mk), verify=True)
     mesh, sp = oracle_of(w)
-    for flags in (2, 3):
-        ref, _ = oracle.deposit(mesh, sp, mk, flags=flags, t=2.1)
-        got = p.deposit(flags=flags, t=2.1)
-        S = np.abs(ref).max()
-        assert np.abs(got - ref).max() <= 1e-11 * S, float(np.abs(got - ref).max() / S)
+    for ring_stream in (False, True):               # every lane loops over its ring's elements / ordered ring items
+        if ring_stream:
+            p.set_flr_workspace()
+        for flags in (2, 3, 7):
+            ref, _ = oracle.deposit(mesh, sp, mk, flags=flags, t=2.1)
+            got = p.deposit(flags=flags, t=2.1)
+            S = np.abs(ref).max()
+            assert np.abs(got - ref).max() <= 1e-11 * S, (ring_stream, flags, float(np.abs(got - ref).max() / S))
     plain = p.deposit(flags=0)
     assert np.abs(got[:, 1, 0, 0] - plain[:, 1, 0, 0]).max() > 1e-3 * np.abs(plain[:, 1, 0, 0]).max()
 
