@@ -79,19 +79,53 @@ def measured_peaks():
     return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)", 1965.0
 
 
-def ncu_traffic(config: int, sort_interval: int):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the push kernel, per launch, from the committed ncu --set full
-    capture of this workload (profiles/push_traffic.csv, copied by hand from the capture named in the .md beside it);
-    None when no capture of this configuration is committed."""
-    p = os.path.join(ROOT, "profiles", "push_traffic.csv")
-    if not os.path.exists(p):
-        return None
-    with open(p) as fh:
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "push_traffic.csv")
+
+
+def ncu_traffic(config: int, sort_interval: int, mode: int = 0):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the push kernels, per push, from the committed ncu --set full
+    capture of this workload: profiles/push_traffic.csv, written by `bench.py --traffic-from <ncu raw csv>` together with
+    the commit the capture was taken at.  Returns (bytes, commit) or (None, None) when no capture of this configuration
+    is recorded."""
+    if not os.path.exists(TRAFFIC_CSV):
+        return None, None
+    found = (None, None)
+    with open(TRAFFIC_CSV) as fh:
         for line in fh:
             cols = [c.strip() for c in line.split(",")]
-            if len(cols) >= 3 and cols[0] == f"config{config}" and cols[1] == f"si{sort_interval}":
-                return float(cols[2])
-    return None
+            if len(cols) >= 5 and cols[0] == f"config{config}" and cols[1] == f"si{sort_interval}" and cols[2] == f"mode{mode}":
+                found = (float(cols[3]), cols[4])
+    return found
+
+
+def record_traffic(args):
+    """--traffic-from: read an `ncu -i <rep> --page raw --csv` export of ONE push (its launches of the push kernels) and
+    append its DRAM traffic to profiles/push_traffic.csv with the current commit."""
+    import csv
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    with open(args.traffic_from) as fh:
+        rows = [r for r in csv.reader(fh) if r]
+    hdr, units = rows[0], rows[1]
+    kcol = hdr.index("Kernel Name")
+    total, kernels = 0.0, []
+    for r in rows[2:]:
+        if "push_items_kernel" not in r[kcol] and "push_async_kernel" not in r[kcol]:
+            continue
+        kernels.append(r[kcol].split("(")[0].replace("void ", ""))
+        for name in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            c = hdr.index(name)
+            total += float(r[c].replace(",", "")) * scale[units[c]]
+    if not kernels:
+        raise SystemExit("no push kernel in " + args.traffic_from)
+    commit = subprocess.run(["git", "-C", ROOT, "rev-parse", "--short", "HEAD"], capture_output=True, text=True).stdout.strip()
+    si = 1 if args.sort_interval is None else args.sort_interval
+    new_file = not os.path.exists(TRAFFIC_CSV)
+    with open(TRAFFIC_CSV, "a") as fh:
+        if new_file:
+            fh.write("workload,sort_interval,mode,dram_bytes_per_push,commit,date,kernels\n")
+        fh.write(f"config{args.config},si{si},mode{args.mode},{total:.0f},{commit or 'unknown'},"
+                 f"{time.strftime('%Y-%m-%d')},{'+'.join(kernels)}\n")
+    print(f"recorded {total:.0f} B per push ({'+'.join(kernels)}) at {commit}")
 
 
 class ClockSampler:
@@ -306,8 +340,12 @@ def run_ours(args, rank, world, local_rank):
         roof = {"bound": "hbm", "achieved": bytes_push / (push_ms * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
                 "peak_source": hbm_src}
     roof["frac"] = roof["achieved"] / roof["peak"]
+    traffic, traffic_commit = ncu_traffic(args.config, si, args.mode)
+    if roof["bound"] == "alu":
+        # the measured FP64 peak (register-resident DFMA chains, m3dk_fp64_peak_tflops) beside the nominal one
+        roof["frac_of_measured_peak"] = roof["achieved"] / fp64_meas if fp64_meas > 0 else None
     roof.update({"kernel": "push kernel (a1-a10)", "launch_ms": push_ms, "launches": tm["push_launches"],
-                 "share_of_step": tm["push_ms"] / ms, "traffic": ncu_traffic(args.config, si),
+                 "share_of_step": tm["push_ms"] / ms, "traffic": traffic, "traffic_commit": traffic_commit,
                  "fp64_peak_measured_tflops": fp64_meas,
                  "flops_per_marker_step": algorithmic_flops(w.n_modes, args.mode),
                  "hbm_bytes_per_marker_step": algorithmic_bytes_push(w.n_modes, ordered=si > 0),
@@ -387,12 +425,21 @@ def run_sweep(args):
                 tm = p.timing()
                 t_alu = algorithmic_flops(w.n_modes) * n / (FP64_NOMINAL_TFLOPS * 1e12)
                 t_hbm = (algorithmic_bytes_push(w.n_modes, ordered=si > 0) + algorithmic_bytes_sort() * tm["sort_launches"] / K) * n / (hbm_gbs * 1e9)
-                print(json.dumps({"sweep_point": {"n_markers": n, "dt_gyro": dtg, "sort_interval": si},
-                                  "value": n / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms,
-                                  "push_ms": tm["push_ms"] / max(1, tm["push_launches"]),
-                                  "binding": "alu" if t_alu >= t_hbm else "hbm",
-                                  "frac_of_binding_roofline": max(t_alu, t_hbm) / (ms * 1e-3),
-                                  "n_lost": p.stats()["n_lost"]}), flush=True)
+                row = {"sweep_point": {"n_markers": n, "dt_gyro": dtg, "sort_interval": si},
+                       "value": n / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms,
+                       "push_ms": tm["push_ms"] / max(1, tm["push_launches"]),
+                       "binding": "alu" if t_alu >= t_hbm else "hbm",
+                       "frac_of_binding_roofline": max(t_alu, t_hbm) / (ms * 1e-3),
+                       "n_lost": p.stats()["n_lost"]}
+                print(json.dumps(row), flush=True)
+                if args.sweep_out:
+                    new_file = not os.path.exists(args.sweep_out)
+                    with open(args.sweep_out, "a") as fh:
+                        if new_file:
+                            fh.write("n_markers,dt_gyro,sort_interval,particle_steps_per_s,ms_per_step,push_ms,binding,"
+                                     "frac_of_binding_roofline,n_lost,steps,warmup\n")
+                        fh.write(f"{n},{dtg},{si},{row['value']:.6e},{ms:.5f},{row['push_ms']:.5f},{row['binding']},"
+                                 f"{row['frac_of_binding_roofline']:.4f},{row['n_lost']},{K},{W}\n")
                 p.close()
                 del p
                 torch.cuda.empty_cache()
@@ -420,7 +467,11 @@ def main():
     ap.add_argument("--e2e-chunks", type=int, default=4, help="marker chunks of the pipelined host-buffer call (e2e leg)")
     ap.add_argument("--push-variant", type=int, default=0, choices=[0, 1],
                     help="m3dk_set_push_variant: 0 = default kernel, 1 = asynchronously staged kernel (A/B comparison)")
+    ap.add_argument("--traffic-from", default=None,
+                    help="record the DRAM traffic of the push kernels from an `ncu --page raw --csv` export into "
+                         "profiles/push_traffic.csv (with the current commit) and exit")
     ap.add_argument("--sweep", action="store_true", help="configs[4] sweep: one JSON line per (n, dt, sort interval)")
+    ap.add_argument("--sweep-out", default=None, help="append one CSV row per sweep point to this file")
     ap.add_argument("--sweep-n", type=int, nargs="+", default=[1 << 20, 1 << 22, 1 << 24, 1 << 26])
     ap.add_argument("--sweep-dt", type=float, nargs="+", default=[1.0, 4.0, 16.0])
     ap.add_argument("--sweep-si", type=int, nargs="+", default=[1, 10, 0])
@@ -431,6 +482,9 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.traffic_from:
+        record_traffic(args)
+        return
     if args.impl == "reference":
         run_reference(args, rank, world)
         return
