@@ -200,7 +200,10 @@ int m3dk_eval_fields(m3dk_ctx *ctx, long n, const double *R, const double *phi, 
                      int *elem_out, double *out);
 
 /* RK4 guiding-centre pusher (Eqs. 1-4; reading G24): the paper's comparator
- * (Fig. 1) and the equilibrium guiding-centre motion "(dX/dt)_0" of PAPER.md:130.  Equilibrium fields only (E = 0):
+ * (Fig. 1) and the equilibrium guiding-centre motion "(dX/dt)_0" of PAPER.md:130.  In mode 1 (non-linear trajectories) the
+ * guiding centres move in the total fields to first order (reading G26): E = E1, B1 added to B-star, grad|B| ->
+ * grad(|B|0 + B1par), b and curl b from the equilibrium, all at the context's time, which then advances by nsteps * dt as
+ * in m3dk_push.  In modes 0 and 2 equilibrium fields only (E = 0):
  *   dX/dt = (1/B*par)[v_par B* + (mu/q) b x grad|B|],  m dv_par/dt = -(mu/B*par) B* . grad|B|,
  *   B* = B + (m v_par/q) curl b,  B*par = B* . b;  curl b from the second derivatives of psi0 and the first of F0.
  * The registered arrays x, y, z are read and written as the guiding-centre position X (Cartesian), mu is read, elem is

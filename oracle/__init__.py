@@ -59,8 +59,8 @@ def _configure(L):
     L.orc_flr_fields.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), c_dp, C.c_double, C.c_double, c_dp]
     L.orc_gc_push.restype = C.c_long
     L.orc_gc_push.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5 + [c_ip, C.c_int,
-                              C.c_double, C.c_int]
-    L.orc_gc_rhs.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5
+                              C.c_double, C.c_double, C.c_int]
+    L.orc_gc_rhs.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5 + [C.c_double, c_dp]
     L.orc_gc_bootstrap.argtypes = [C.c_void_p, C.POINTER(Analytic), C.POINTER(Species), C.c_long] + [c_dp] * 5 + [C.c_double] + [c_dp] * 3 + [c_ip]
     L.orc_gc_fields.argtypes = [C.c_void_p, C.POINTER(Analytic), C.c_long, c_dp, c_dp, c_ip, c_dp]
     L.orc_deposit.restype = C.c_long
@@ -233,15 +233,16 @@ def push_analytic(an: Analytic, sp: Species, markers: dict, nsteps: int, dt: flo
     return st
 
 
-def gc_push(sp: Species, x, y, z, vpar, mu, nsteps: int, dt: float, *, mesh=None, an=None, nthreads: int = 0):
-    """RK4 on the guiding-centre equations (Eqs. 1-4, equilibrium fields; reading G24).  Returns (x, y, z, vpar, elem, lost)."""
+def gc_push(sp: Species, x, y, z, vpar, mu, nsteps: int, dt: float, *, mesh=None, an=None, nthreads: int = 0, t0: float = 0.0):
+    """RK4 on the guiding-centre equations (Eqs. 1-4; equilibrium fields, reading G24; sp.mode == 1: total fields, reading
+    G26, from time t0).  Returns (x, y, z, vpar, elem, lost)."""
     arrs = [np.array(a, dtype=np.float64, copy=True, order="C") for a in (x, y, z, vpar)]
     mu = np.ascontiguousarray(mu, dtype=np.float64)
     n = arrs[0].shape[0]
     e = np.zeros(n, dtype=np.int32)
     lost = lib().orc_gc_push(mesh.h if mesh is not None else None, C.byref(an) if an is not None else None, C.byref(sp), n,
                              *[a.ctypes.data_as(c_dp) for a in arrs], mu.ctypes.data_as(c_dp), e.ctypes.data_as(c_ip),
-                             int(nsteps), float(dt), int(nthreads))
+                             int(nsteps), float(dt), float(t0), int(nthreads))
     return arrs[0], arrs[1], arrs[2], arrs[3], e, int(lost)
 
 
@@ -259,13 +260,14 @@ def gc_bootstrap(sp: Species, x, y, z, vpar, mu, dt: float, *, mesh=None, an=Non
     return pos[0], pos[1], pos[2], v[0], v[1], v[2], ok.astype(bool)
 
 
-def gc_rhs(sp: Species, R, Z, vpar, mu, *, mesh=None, an=None):
-    """Right-hand sides of Eqs. (1)-(2): rows (dR/dt, R dphi/dt, dZ/dt, dv_par/dt)."""
+def gc_rhs(sp: Species, R, Z, vpar, mu, *, mesh=None, an=None, phi=None, t: float = 0.0):
+    """Right-hand sides of Eqs. (1)-(2): rows (dR/dt, R dphi/dt, dZ/dt, dv_par/dt); phi and t matter with sp.mode == 1."""
     R, Z, vpar, mu = (np.ascontiguousarray(a, dtype=np.float64) for a in (R, Z, vpar, mu))
+    phi = np.zeros_like(R) if phi is None else np.ascontiguousarray(phi, dtype=np.float64)
     out = np.zeros((R.shape[0], 4))
     lib().orc_gc_rhs(mesh.h if mesh is not None else None, C.byref(an) if an is not None else None, C.byref(sp), R.shape[0],
-                     R.ctypes.data_as(c_dp), Z.ctypes.data_as(c_dp), vpar.ctypes.data_as(c_dp), mu.ctypes.data_as(c_dp),
-                     out.ctypes.data_as(c_dp))
+                     R.ctypes.data_as(c_dp), phi.ctypes.data_as(c_dp), Z.ctypes.data_as(c_dp), vpar.ctypes.data_as(c_dp),
+                     mu.ctypes.data_as(c_dp), float(t), out.ctypes.data_as(c_dp))
     return out
 
 

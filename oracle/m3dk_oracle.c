@@ -800,9 +800,16 @@ static double bstar(const orc_gcf *g, const orc_species *sp, double R, double vp
     return Bspar;
 }
 
-/* right-hand side of Eqs. (1)-(2) at (R, Z, v_par): dX/dt in cylindrical components, dv_par/dt.  Returns -1 outside. */
-static int gc_rhs(const provider *pv, const orc_species *sp, double R, double Z, double vpar, double mu, double dX[3],
-                  double *dvpar)
+/* right-hand side of Eqs. (1)-(2) at (R, phi, Z, v_par, t): dX/dt in cylindrical components, dv_par/dt.  Returns -1 outside.
+ *     dX/dt       = (1/B*par) [ v_par B* - b x (E - (mu/q) grad B) ]          Eq. (1)
+ *     m dv_par/dt = (1/B*par) B* . (q E - mu grad B)                          Eq. (2)
+ * sp->mode != 1: equilibrium fields only, E = 0 (reading G24).  sp->mode == 1 (reading G26): the guiding centre moves in
+ * the total fields to first order in the perturbation: E = E1, B = B0 + B1 in B*, grad B = grad(|B|0 + B1par) as in the
+ * mode-1 push (G21), while b, curl b and B*par = B* . b keep the equilibrium unit vector b0 (the perturbed part of b
+ * needs derivatives of B1 that the field tables do not carry).  Linearised in the amplitude and at lowest order in rho*
+ * the difference to the equilibrium right-hand side is Eq. (12): E1 x B0/B0^2 + v_par B1/B0.                          */
+static int gc_rhs(const provider *pv, const orc_species *sp, double R, double phi, double Z, double vpar, double mu, double t,
+                  double dX[3], double *dvpar)
 {
     orc_gcf g;
     int e = gc_fields(pv, R, Z, &g);
@@ -811,9 +818,19 @@ static int gc_rhs(const provider *pv, const orc_species *sp, double R, double Z,
     double Bs[3], b[3];
     double Bspar = bstar(&g, sp, R, vpar, Bs, b);
     double gB[3] = {g.Bm_R, 0.0, g.Bm_Z};
-    double bxg[3] = {b[1] * gB[2] - b[2] * gB[1], b[2] * gB[0] - b[0] * gB[2], b[0] * gB[1] - b[1] * gB[0]};
-    for (int k = 0; k < 3; ++k) dX[k] = (vpar * Bs[k] + (mu / q) * bxg[k]) / Bspar;
-    *dvpar = -(mu / m) * (Bs[0] * gB[0] + Bs[1] * gB[1] + Bs[2] * gB[2]) / Bspar;
+    double E[3] = {0.0, 0.0, 0.0};
+    if (sp->mode == 1) {
+        orc_fields f;
+        if (pv->kind == 0) fe_fields(pv->mesh, e, R, phi, Z, t, &f);
+        else an_fields(pv->an, R, phi, Z, t, &f);
+        Bspar = 0.0;
+        for (int k = 0; k < 3; ++k) { Bs[k] += f.B1[k]; Bspar += Bs[k] * b[k]; gB[k] += f.gB1p[k]; E[k] = f.E1[k]; }
+    }
+    double Ee[3];                                       /* E - (mu/q) grad B */
+    for (int k = 0; k < 3; ++k) Ee[k] = E[k] - (mu / q) * gB[k];
+    double bxE[3] = {b[1] * Ee[2] - b[2] * Ee[1], b[2] * Ee[0] - b[0] * Ee[2], b[0] * Ee[1] - b[1] * Ee[0]};
+    for (int k = 0; k < 3; ++k) dX[k] = (vpar * Bs[k] - bxE[k]) / Bspar;
+    *dvpar = (q / m) * (Bs[0] * Ee[0] + Bs[1] * Ee[1] + Bs[2] * Ee[2]) / Bspar;
     return e;
 }
 
@@ -821,7 +838,7 @@ static int gc_rhs(const provider *pv, const orc_species *sp, double R, double Z,
  * caller keeps the state of the step before: lost), otherwise the element of the NEW position (FE back-end; 0 for the
  * analytic one), which is -1 as well when the step itself ends outside: then the new state is kept and the guiding centre
  * is lost from there.  *stage_lost tells the two cases apart.                                                          */
-static int gc_step(const provider *pv, const orc_species *sp, double y[4], double mu, double dt, int *stage_lost)
+static int gc_step(const provider *pv, const orc_species *sp, double y[4], double mu, double t, double dt, int *stage_lost)
 {
     double k[4][4], yy[4];
     static const double cs[4] = {0.0, 0.5, 0.5, 1.0};
@@ -830,7 +847,7 @@ static int gc_step(const provider *pv, const orc_species *sp, double y[4], doubl
         for (int i = 0; i < 4; ++i) yy[i] = y[i] + (st ? cs[st] * dt * k[st - 1][i] : 0.0);
         double R = sqrt(yy[0] * yy[0] + yy[1] * yy[1]), c = yy[0] / R, sn = yy[1] / R;
         double dX[3], dv;
-        int e = gc_rhs(pv, sp, R, yy[2], yy[3], mu, dX, &dv);
+        int e = gc_rhs(pv, sp, R, atan2(yy[1], yy[0]), yy[2], yy[3], mu, t + cs[st] * dt, dX, &dv);
         if (e < 0) { *stage_lost = 1; return -1; }
         k[st][0] = dX[0] * c - dX[1] * sn; k[st][1] = dX[0] * sn + dX[1] * c; k[st][2] = dX[2]; k[st][3] = dv;
     }
@@ -843,7 +860,7 @@ static int gc_step(const provider *pv, const orc_species *sp, double y[4], doubl
 /* n guiding centres nsteps RK4 steps; elem (optional out): element of the CURRENT position, -1 = lost (frozen): either a
  * stage of a step left the mesh (state of the step before) or a step ended outside (state after that step)             */
 long orc_gc_push(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, long n, double *x, double *y, double *z,
-                 double *vpar, const double *mu, int *elem, int nsteps, double dt, int nthreads)
+                 double *vpar, const double *mu, int *elem, int nsteps, double dt, double t0, int nthreads)
 {
     provider pv = {m ? 0 : 1, m, a, 0};
     long lost = 0;
@@ -859,7 +876,7 @@ long orc_gc_push(const orc_mesh *m, const orc_analytic *a, const orc_species *sp
         for (int l = 0; l < nsteps && !dead; ++l) {
             double keep[4] = {s[0], s[1], s[2], s[3]};
             int stage_lost;
-            e = gc_step(&pv, sp, s, mu[i], dt, &stage_lost);
+            e = gc_step(&pv, sp, s, mu[i], t0 + (double)l * dt, dt, &stage_lost);
             if (e < 0) { dead = 1; if (stage_lost) for (int q = 0; q < 4; ++q) s[q] = keep[q]; }
         }
         if (dead) { lost++; e = -1; }
@@ -878,10 +895,12 @@ void orc_gc_bootstrap(const orc_mesh *m, const orc_analytic *a, const orc_specie
                       const double *vpar, const double *mu, double dt, double *vx, double *vy, double *vz, int *ok)
 {
     provider pv = {m ? 0 : 1, m, a, 0};
+    orc_species eq = *sp;
+    eq.mode = 0;                                         /* the bootstrap uses the equilibrium fields */
     for (long i = 0; i < n; ++i) {
         double s[4] = {x[i], y[i], z[i], vpar[i]};
         int stage_lost;
-        int e = gc_step(&pv, sp, s, mu[i], dt, &stage_lost);
+        int e = gc_step(&pv, &eq, s, mu[i], 0.0, dt, &stage_lost);
         ok[i] = e >= 0;
         if (e < 0) continue;
         vx[i] = (s[0] - x[i]) / dt; vy[i] = (s[1] - y[i]) / dt; vz[i] = (s[2] - z[i]) / dt;
@@ -905,13 +924,13 @@ void orc_gc_fields(const orc_mesh *m, const orc_analytic *a, long n, const doubl
 }
 
 /* right-hand side at given points, for the pins: out[n][4] = dX/dt (R, phi, Z components), dv_par/dt */
-void orc_gc_rhs(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, long n, const double *R, const double *Z,
-                const double *vpar, const double *mu, double *out)
+void orc_gc_rhs(const orc_mesh *m, const orc_analytic *a, const orc_species *sp, long n, const double *R, const double *phi,
+                const double *Z, const double *vpar, const double *mu, double t, double *out)
 {
     provider pv = {m ? 0 : 1, m, a, 0};
     for (long i = 0; i < n; ++i) {
         double dX[3] = {0, 0, 0}, dv = 0.0;
-        gc_rhs(&pv, sp, R[i], Z[i], vpar[i], mu[i], dX, &dv);
+        gc_rhs(&pv, sp, R[i], phi[i], Z[i], vpar[i], mu[i], t, dX, &dv);
         out[4 * i] = dX[0]; out[4 * i + 1] = dX[1]; out[4 * i + 2] = dX[2]; out[4 * i + 3] = dv;
     }
 }

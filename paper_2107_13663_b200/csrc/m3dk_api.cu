@@ -740,7 +740,11 @@ extern "C" int m3dk_gc_push(m3dk_ctx *ctx, int nsteps, double dt, double *vpar) 
     if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_gc_push: fields and markers must be set first");
     if (nsteps < 0 || !(dt == dt) || (ctx->n > 0 && !vpar)) return fail(ctx, M3DK_EINVAL, "m3dk_gc_push: nsteps < 0, dt is NaN or vpar is NULL");
     CU(cudaSetDevice(ctx->device), "cudaSetDevice");
-    CU(launch_gc_push(ctx, ctx->n, vpar, nsteps, dt), "guiding-centre kernel");
+    // mode 1 (non-linear trajectories): the guiding centres move in the total fields at the context's time, which advances
+    const bool pert = ctx->mode == 1 && ctx->f.n_modes > 0;
+    const double t0 = pert ? step_time(ctx, dt) : 0.0;
+    CU(launch_gc_push(ctx, ctx->n, vpar, nsteps, dt, pert, t0), "guiding-centre kernel");
+    if (pert) { ctx->steps_done += nsteps; ctx->steps_at_dt += nsteps; }
     return M3DK_OK;
 }
 

@@ -9,9 +9,12 @@
 
 namespace m3dk {
 
-// right-hand side of Eqs. (1)-(2) at (R, Z, v_par): dX/dt in cylindrical components, dv_par/dt; false outside the mesh
-__device__ __forceinline__ bool gc_rhs(const FieldParams &f, double q, double m, double R, double Z, double vpar, double mu,
-                                       double (&dX)[3], double &dv, int &elem) {
+// right-hand side of Eqs. (1)-(2) at (R, phi, Z, v_par, t): dX/dt in cylindrical components, dv_par/dt; false outside the mesh
+//     dX/dt = (1/B*par) [v_par B* - b x (E - (mu/q) grad B)],   m dv_par/dt = (1/B*par) B* . (q E - mu grad B)
+// kPert (reading G26): E = E1, B1 added to B*, grad B = grad(|B|0 + B1par); b, curl b and B*par = B* . b keep b0.
+template <bool kPert>
+__device__ __forceinline__ bool gc_rhs(const FieldParams &f, double q, double m, double R, double Z, double cph, double sph,
+                                       double vpar, double mu, double t, double (&dX)[3], double &dv, int &elem) {
     const int e = locate_any(f, R, Z);
     elem = e;
     if (e < 0) return false;
@@ -19,19 +22,30 @@ __device__ __forceinline__ bool gc_rhs(const FieldParams &f, double q, double m,
     GcEq g;
     gc_eq_fields(tile, R, Z, g);
     double Bs[3], b[3];
-    const double Bspar = bstar_par(g, q, m, vpar, Bs, b);
-    const double Bm_R = g.Bm_R, Bm_Z = g.Bm_Z;
+    double Bspar = bstar_par(g, q, m, vpar, Bs, b);
+    double gB[3] = {g.Bm_R, 0.0, g.Bm_Z}, E[3] = {0.0, 0.0, 0.0};
+    if (kPert) {
+        double cwt[M3DK_MAX_MODES], swt[M3DK_MAX_MODES];
+        for (int k = 0; k < f.n_modes; ++k) sincos(f.omega[k] * t, &swt[k], &cwt[k]);
+        Fields o;
+        eval_fields(f, e, R, Z, cph, sph, g.rinv, cwt, swt, o);
+        Bspar = 0.0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { Bs[k] += o.B1[k]; Bspar += Bs[k] * b[k]; gB[k] += o.gB[k]; E[k] = o.E1[k]; }
+    }
     const double bsinv = m3dk_rcp(Bspar);
     const double muq = mu / q;
-    const double bxg[3] = {b[1] * Bm_Z, b[2] * Bm_R - b[0] * Bm_Z, -b[1] * Bm_R};     // b x grad|B|, grad|B| = (Bm_R, 0, Bm_Z)
+    const double Ee[3] = {E[0] - muq * gB[0], E[1] - muq * gB[1], E[2] - muq * gB[2]};
+    const double bxE[3] = {b[1] * Ee[2] - b[2] * Ee[1], b[2] * Ee[0] - b[0] * Ee[2], b[0] * Ee[1] - b[1] * Ee[0]};
 #pragma unroll
-    for (int k = 0; k < 3; ++k) dX[k] = (vpar * Bs[k] + muq * bxg[k]) * bsinv;
-    dv = -(mu / m) * (Bs[0] * Bm_R + Bs[2] * Bm_Z) * bsinv;
+    for (int k = 0; k < 3; ++k) dX[k] = (vpar * Bs[k] - bxE[k]) * bsinv;
+    dv = (q / m) * (Bs[0] * Ee[0] + Bs[1] * Ee[1] + Bs[2] * Ee[2]) * bsinv;
     return true;
 }
 
 // One RK4 step of y = (x, y, z, v_par).  false: one of the four stages lies outside the mesh (y is left untouched).
-__device__ __forceinline__ bool gc_rk4_step(const FieldParams &f, double q, double m, double mu, double dt, double (&y)[4]) {
+template <bool kPert>
+__device__ __forceinline__ bool gc_rk4_step(const FieldParams &f, double q, double m, double mu, double t, double dt, double (&y)[4]) {
     double k[4][4], yy[4];
     bool ok = true;
 #pragma unroll
@@ -43,7 +57,7 @@ __device__ __forceinline__ bool gc_rk4_step(const FieldParams &f, double q, doub
         const double rinv = m3dk_rsqrt(r2), R = r2 * rinv, c = yy[0] * rinv, sn = yy[1] * rinv;
         double dX[3], dv;
         int es;
-        if (ok && !gc_rhs(f, q, m, R, yy[2], yy[3], mu, dX, dv, es)) ok = false;
+        if (ok && !gc_rhs<kPert>(f, q, m, R, yy[2], c, sn, yy[3], mu, t + cs * dt, dX, dv, es)) ok = false;
         if (!ok) { dX[0] = dX[1] = dX[2] = 0.0; dv = 0.0; }
         k[st][0] = dX[0] * c - dX[1] * sn; k[st][1] = dX[0] * sn + dX[1] * c; k[st][2] = dX[2]; k[st][3] = dv;
     }
@@ -56,8 +70,9 @@ __device__ __forceinline__ bool gc_rk4_step(const FieldParams &f, double q, doub
 // nsteps RK4 steps.  elem is kept at the element of the CURRENT position (every other entry point trusts it).  A guiding
 // centre is lost (elem = -1, frozen; reading G12) when a stage of a step leaves the mesh (it keeps the state of the step
 // before) or when a step ends outside (it keeps that state).
+template <bool kPert>
 __global__ void __launch_bounds__(128) gc_push_kernel(const __grid_constant__ FieldParams f, MarkerArrays a, double *vpar,
-                                                      long n, double q, double m, double dt, int nsteps) {
+                                                      long n, double q, double m, double t0, double dt, int nsteps) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int e = a.elem[i];
@@ -65,7 +80,7 @@ __global__ void __launch_bounds__(128) gc_push_kernel(const __grid_constant__ Fi
     double y[4] = {a.x[i], a.y[i], a.z[i], vpar[i]};
     const double mu = a.mu[i];
     for (int l = 0; l < nsteps && e >= 0; ++l) {
-        if (!gc_rk4_step(f, q, m, mu, dt, y)) { e = -1; break; }
+        if (!gc_rk4_step<kPert>(f, q, m, mu, t0 + (double)l * dt, dt, y)) { e = -1; break; }
         e = locate_xyz(f, y[0], y[1], y[2]);
     }
     a.x[i] = y[0]; a.y[i] = y[1]; a.z[i] = y[2]; vpar[i] = y[3];
@@ -83,7 +98,7 @@ __global__ void __launch_bounds__(128) gc_bootstrap_kernel(const __grid_constant
     const double x0 = a.x[i], y0 = a.y[i], z0 = a.z[i];
     double y[4] = {x0, y0, z0, vpar[i]};
     int e = -1;
-    if (gc_rk4_step(f, q, m, a.mu[i], dt, y)) e = locate_xyz(f, y[0], y[1], y[2]);
+    if (gc_rk4_step<false>(f, q, m, a.mu[i], 0.0, dt, y)) e = locate_xyz(f, y[0], y[1], y[2]);
     a.elem[i] = e;
     if (e < 0) return;
     const double rdt = 1.0 / dt;
@@ -91,10 +106,12 @@ __global__ void __launch_bounds__(128) gc_bootstrap_kernel(const __grid_constant
     a.x[i] = y[0]; a.y[i] = y[1]; a.z[i] = y[2];
 }
 
-cudaError_t launch_gc_push(m3dk_ctx *c, long n, double *vpar, int nsteps, double dt) {
+cudaError_t launch_gc_push(m3dk_ctx *c, long n, double *vpar, int nsteps, double dt, bool pert, double t0) {
     if (n == 0 || nsteps == 0) return cudaSuccess;
     c->kernel_launches += 1;
-    gc_push_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, c->user, vpar, n, c->q, c->m, dt, nsteps);
+    const unsigned grid = (unsigned)((n + 127) / 128);
+    if (pert) gc_push_kernel<true><<<grid, 128, 0, c->stream>>>(c->f, c->user, vpar, n, c->q, c->m, t0, dt, nsteps);
+    else gc_push_kernel<false><<<grid, 128, 0, c->stream>>>(c->f, c->user, vpar, n, c->q, c->m, t0, dt, nsteps);
     return cudaGetLastError();
 }
 

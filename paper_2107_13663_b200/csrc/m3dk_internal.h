@@ -214,7 +214,7 @@ cudaError_t launch_pack_sorted(m3dk_ctx *c, long n);     // caller's arrays -> r
 cudaError_t launch_reorder(m3dk_ctx *c, long n);         // histogram of the last push -> offsets, items, next order
 cudaError_t launch_unpack(m3dk_ctx *c, long n);          // records -> caller's arrays (+ elem, id)
 cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t);   // Eqs. (17)-(18) right-hand sides from the caller's arrays
-cudaError_t launch_gc_push(m3dk_ctx *c, long n, double *vpar, int nsteps, double dt);   // RK4 guiding-centre steps
+cudaError_t launch_gc_push(m3dk_ctx *c, long n, double *vpar, int nsteps, double dt, bool pert, double t0);   // RK4 guiding-centre steps
 cudaError_t launch_gc_bootstrap(m3dk_ctx *c, long n, const double *vpar, double dt);     // (x_1, v_{1/2}) from one such step
 cudaError_t fp64_probe(m3dk_ctx *c, double *tflops);
 

@@ -206,3 +206,65 @@ def check_g6_bootstrap(orc):
 
 def test_g6_bootstrap_puts_the_marker_on_the_slow_manifold(orc):
     check_g6_bootstrap(orc)
+
+
+def check_g7_perturbed_guiding_centre_rhs(orc):
+    """Eqs. (1)-(2) with the perturbed fields (sp.mode = 1; reading G26).
+    (a) Closed forms on hand-made tables: psi0 = A R^2/2, F = 0, |B|0 = A is a uniform vertical field (b0 = Z-hat,
+    curl b0 = 0), so B* = B0 + B1 and B*par = A + B1_Z; with one perturbed component at a time
+        B1_R = eps:        dR/dt = v_par eps / A                      (v_par B1/B0 of Eq. 12)
+        E1_phi = eps:      dR/dt = eps / A                            (E x B / B^2:  phi-hat x Z-hat = R-hat)
+        E1_R = eps:        R dphi/dt = -eps / A                       (R-hat x Z-hat = -phi-hat)
+        E1_Z = eps:        dv_par/dt = (q/m) eps                      (Eq. 2)
+        B1par = eps Z:     dv_par/dt = -(mu/m) eps                    (mirror force of the perturbed field strength)
+        B1par = eps R:     R dphi/dt = -(mu/q) eps / A                (grad-B drift: b x grad B / B = Z-hat x R-hat = +phi-hat, sign of -b x (-(mu/q) grad B))
+    (b) An invariant: with a static electrostatic perturbation on the analytic back-end, H = m v_par^2/2 + mu |B| + q Phi is
+    conserved pointwise by Eqs. (1)-(2): m v_par dv_par/dt + (mu grad|B| + q grad Phi) . dX/dt = 0 (gradients by central
+    differences of the analytic fields)."""
+    from handmade import HandMade
+    A, eps = 0.8, 1e-3
+    q, m = CHARGE, MASS
+    R, Z, phi = np.array([3.1]), np.array([0.2]), np.array([0.6])
+    vpar, mu = np.array([0.7]), np.array([0.004])
+    eqd = dict(psi=(0.0, 0.0, 0.0, 0.5 * A), Bm=(A,), F=(0.0,), kappa=(0.0,))
+    sp = orc.species(q, m, mode=1)
+
+    def rhs(pert):
+        hm = HandMade(eq=eqd, pert=pert, n_tor=0)
+        return orc.gc_rhs(sp, R, Z, vpar, mu, mesh=hm.oracle_mesh(orc), phi=phi)[0]
+    base = rhs(dict(B_R=(0.0,)))
+    assert np.allclose(base, [0.0, 0.0, vpar[0], 0.0], atol=1e-15)           # streaming along the uniform field
+    assert np.allclose(rhs(dict(B_R=(eps,))) - base, [vpar[0] * eps / A, 0, 0, 0], rtol=1e-12, atol=1e-18)
+    assert np.allclose(rhs(dict(E_phi=(eps,))) - base, [eps / A, 0, 0, 0], rtol=1e-12, atol=1e-18)
+    assert np.allclose(rhs(dict(E_R=(eps,))) - base, [0, -eps / A, 0, 0], rtol=1e-12, atol=1e-18)
+    assert np.allclose(rhs(dict(E_Z=(eps,))) - base, [0, 0, 0, q / m * eps], rtol=1e-12, atol=1e-18)
+    assert np.allclose(rhs(dict(B_par=(0.0, 0.0, eps))) - base, [0, 0, 0, -mu[0] / m * eps], rtol=1e-12, atol=1e-18)
+    assert np.allclose(rhs(dict(B_par=(0.0, eps, 0.0))) - base, [0, mu[0] / q * eps / A, 0, 0], rtol=1e-12, atol=1e-18)
+    # B1_Z changes the Jacobian B*par = A + eps but not the streaming velocity: v_par (A + eps) / (A + eps)
+    assert np.allclose(rhs(dict(B_Z=(eps,))), base, rtol=1e-12, atol=1e-15)
+    # (b)
+    p = (2e-3, 0.3, 0.1, 0.0, 2, 3)
+    an = orc.analytic_of(EQ, pA=p[0], prc=p[1], pwd=p[2], pomega=p[3], pn=p[4], pm=p[5])
+    rng = np.random.Generator(np.random.PCG64(13))
+    n = 150
+    Rr, Zz, ph = rng.uniform(2.5, 3.5, n), rng.uniform(-0.45, 0.45, n), rng.uniform(-3, 3, n)
+    vp, mm = rng.uniform(-1, 1, n), rng.uniform(0.001, 0.01, n)
+    out = orc.gc_rhs(sp, Rr, Zz, vp, mm, an=an, phi=ph)
+    h = 1e-5
+    Bm = lambda r, z: np.sqrt(sum(b ** 2 for b in EQ.B_cyl(r, z)))
+
+    def Phi(r, f, z):
+        dR = r - EQ.R0
+        rr, th = np.hypot(dR, z), np.arctan2(z, dR)
+        return p[0] * np.exp(-((rr - p[1]) / p[2]) ** 2) * np.cos(p[4] * f - p[5] * th)
+    gB = [(Bm(Rr + h, Zz) - Bm(Rr - h, Zz)) / (2 * h), 0 * Rr, (Bm(Rr, Zz + h) - Bm(Rr, Zz - h)) / (2 * h)]
+    gP = [(Phi(Rr + h, ph, Zz) - Phi(Rr - h, ph, Zz)) / (2 * h), (Phi(Rr, ph + h, Zz) - Phi(Rr, ph - h, Zz)) / (2 * h) / Rr,
+          (Phi(Rr, ph, Zz + h) - Phi(Rr, ph, Zz - h)) / (2 * h)]
+    dH = m * vp * out[:, 3] + sum((mm * gB[k] + q * gP[k]) * out[:, k] for k in range(3))
+    scale = np.abs(m * vp * out[:, 3]) + sum(np.abs((mm * gB[k] + q * gP[k]) * out[:, k]) for k in range(3)) + 1e-12
+    assert (np.abs(dH) / scale).max() < 1e-6, (np.abs(dH) / scale).max()
+    assert np.abs(q * gP[1] * out[:, 1]).max() > 1e-5                        # the potential does take part
+
+
+def test_g7_perturbed_guiding_centre_rhs(orc):
+    check_g7_perturbed_guiding_centre_rhs(orc)

@@ -1,4 +1,4 @@
-"""Mutation checks of the pins M1-M3, N1, Q1, Q2 (tests/test_oracle_magnetic.py), G5, G6 (tests/test_oracle_gc.py) and D7
+"""Mutation checks of the pins M1-M3, N1, Q1, Q2 (tests/test_oracle_magnetic.py), G5, G6, G7 (tests/test_oracle_gc.py) and D7
 (tests/test_oracle_deposit.py).
 
 Each case compiles a COPY of oracle/m3dk_oracle.c with one plausible mistake (a flipped sign, a dropped factor, a wrong
@@ -7,11 +7,12 @@ evidence that the pin would catch that mistake.  The oracle itself is never modi
 """
 import pytest
 
-from test_oracle_gc import check_g5_phase_space_volume, check_g6_bootstrap
+from test_oracle_gc import check_g5_phase_space_volume, check_g6_bootstrap, check_g7_perturbed_guiding_centre_rhs
 from test_oracle_deposit import check_d7_jacobian_substitution
 from test_oracle_magnetic import CHECKS as _MAGNETIC
 
-CHECKS = dict(_MAGNETIC, g5=check_g5_phase_space_volume, g6=check_g6_bootstrap, d7=check_d7_jacobian_substitution)
+CHECKS = dict(_MAGNETIC, g5=check_g5_phase_space_volume, g6=check_g6_bootstrap, g7=check_g7_perturbed_guiding_centre_rhs,
+              d7=check_d7_jacobian_substitution)
 
 #        pin   tag                      text in the oracle source                         mutated text
 MUTANTS = [
@@ -42,6 +43,11 @@ MUTANTS = [
     ("g5", "Bstar_par", "Bspar += Bs[k] * b[k]; }", "Bspar += B[k] * b[k]; }"),
     ("d7", "jacobian_sign", "dd += f.B1p / bstar(&g, sp, R, vpar, Bs, bb);", "dd -= f.B1p / bstar(&g, sp, R, vpar, Bs, bb);"),
     ("d7", "jacobian_without_curl_b", "dd += f.B1p / bstar(&g, sp, R, vpar, Bs, bb);", "dd += f.B1p / g.Bm;"),
+    ("g7", "ExB_sign", "dX[k] = (vpar * Bs[k] - bxE[k]) / Bspar;", "dX[k] = (vpar * Bs[k] + bxE[k]) / Bspar;"),
+    ("g7", "B1_dropped_from_Bstar", "Bs[k] += f.B1[k]; Bspar += Bs[k] * b[k];", "Bspar += Bs[k] * b[k];"),
+    ("g7", "mirror_of_B1par_dropped", "gB[k] += f.gB1p[k]; E[k] = f.E1[k]; }", "E[k] = f.E1[k]; }"),
+    ("g7", "parallel_E_sign", "*dvpar = (q / m) * (Bs[0] * Ee[0] + Bs[1] * Ee[1] + Bs[2] * Ee[2]) / Bspar;",
+     "*dvpar = -(q / m) * (Bs[0] * Ee[0] + Bs[1] * Ee[1] + Bs[2] * Ee[2]) / Bspar;"),
     ("g6", "bootstrap_sign", "vx[i] = (s[0] - x[i]) / dt;", "vx[i] = (x[i] - s[0]) / dt;"),
     ("g6", "bootstrap_keeps_x0", "x[i] = s[0]; y[i] = s[1]; z[i] = s[2];\n    }\n}", "\n    }\n}"),
     ("q1", "psi_ZZ_dropped", "g->psi_ZZ = d * s * s;", "g->psi_ZZ = 0.0 * d;"),
