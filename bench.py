@@ -49,6 +49,8 @@ def algorithmic_flops(n_modes: int, mode: int = 0) -> float:
     weight = 86 + 2                           # coefficients of dw/dt (Eqs. 8-13 incl. kappa_E), w update
     if mode == 1:                             # non-linear trajectories: + B_phi (re, im), total fields, (1 - w)
         return eq + common + weight + 30 + n_modes * (pert + 2 * 2 * 20 + fold + 5)
+    if mode == 3:                             # non-linear trajectories in the gyro-averaged fields: mode 1 + the ring of mode 2
+        return eq + common + weight + 30 + 60 + 4 * (11 + 4 + 30 + n_modes * (pert + 2 * 2 * 20 + fold)) + 30
     if mode == 2:                             # FLR: ring geometry, then 4 x (map, local coordinates, all 14 polynomials, rotation)
         return eq + common + weight + 60 + 4 * (11 + 4 + 30 + n_modes * (pert + 2 * 2 * 20 + fold)) + 30
     return eq + common + weight + n_modes * (pert + fold)
@@ -207,7 +209,8 @@ def build_workload(args, rank: int, tables: bool = True):
 def config_dict(args, w, sort_interval, world):
     return {"workload": f"BASELINE.json configs[{args.config}] ({w.name})", "n_markers_per_gpu": w.n_markers,
             "mesh": f"{w.nx}x{w.nx} cells, {w.n_elems} triangles", "n_modes": w.n_modes, "dt": w.dt,
-            "sort_interval": sort_interval, "mode": ("linear delta-f", "non-linear trajectories", "linear delta-f + FLR 4-point average")[args.mode],
+            "sort_interval": sort_interval, "mode": ("linear delta-f", "non-linear trajectories", "linear delta-f + FLR 4-point average",
+                     "non-linear trajectories + FLR 4-point average")[args.mode],
             "parallelism": (f"{world} independent marker shard(s), no collective in the push" +
                             ("; field image broadcast from rank 0 (NCCL)" if world > 1 else "")),
             "l2": "inputs larger than L2 (marker state %.0f MB + tables %.0f MB per GPU)" % (
@@ -457,7 +460,7 @@ def main():
     ap.add_argument("--dt-gyro", type=float, default=None)
     ap.add_argument("--sort-interval", type=int, default=None)
     ap.add_argument("--ref-sample", type=int, default=65536, help="markers in the oracle's bounded sample")
-    ap.add_argument("--mode", type=int, default=0, choices=[0, 1, 2],
+    ap.add_argument("--mode", type=int, default=0, choices=[0, 1, 2, 3],
                     help="0: linear delta-f (the headline); 1: non-linear trajectories (SURVEY.md 8(f)-1); "
                          "2: linear delta-f with the 4-point gyro-average (8(f)-2)")
     ap.add_argument("--gc", action="store_true", help="also time m3dk_gc_push (SURVEY.md 8(f)-3) on the final state")

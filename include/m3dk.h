@@ -136,6 +136,9 @@ int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, double *z, 
  *           grad B1par and dB1par/dt of the weight equation are replaced by the quarter sum over the four gyro-ring
  *           points x_l +- rho e1, x_l +- rho e2, rho = m v_perp / (|q| B0), v_perp = sqrt(2 mu B0 / m), e1 = the
  *           major-radius direction made perpendicular to b0, e2 = b0 x e1; a ring point outside the mesh contributes 0.
+ *       3 = modes 1 and 2 together ("use orbit-averaged fields in the above equations"): the marker moves in
+ *           B0 + <B1>, E-dagger = <E1> - (mu/q) grad(|B|0 + <B1par>) with the 4-point gyro-averages of mode 2, and the weight
+ *           equation uses the same averages and keeps (1 - w).  Every lane gathers its ring (no ring stream yet).
  * t0: time of the next step's x_l.  Resets steps_done to 0.                                                          */
 int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, double t0);
 

@@ -100,7 +100,8 @@ typedef struct {
     int f0kind;        /* 0 Maxwellian, 1 slowing-down, 2 beam pitch (reading G7) */
     double f0par[5];   /* T, v_c, Lambda0, dLambda, B_axis */
     int mode;          /* 0: linear delta-f; 1: non-linear trajectories, (1 - w) kept (reading G21);
-                          2: linear delta-f with 4-point gyro-averaged perturbed fields (Eq. 14; reading G23) */
+                          2: linear delta-f with 4-point gyro-averaged perturbed fields (Eq. 14; reading G23);
+                          3: non-linear trajectories in the gyro-averaged perturbed fields (modes 1 and 2 together) */
 } orc_species;
 
 /* ------------------------------------------------------------------------------------------------ */
@@ -495,16 +496,19 @@ static int step_marker(const provider *pv, const orc_species *sp, double *s, dou
     double mu = s[6], q = sp->charge, m = sp->mass;
     double BR = -f.psi_Z / R, BP = f.F / R, BZ = f.psi_R / R;
     double ER = -(mu / q) * f.Bm_R, EP = 0.0, EZ = -(mu / q) * f.Bm_Z;
-    if (sp->mode == 1) {
+    const int nonlinear = sp->mode == 1 || sp->mode == 3, flr = sp->mode == 2 || sp->mode == 3;
+    if (flr) {   /* 4-point gyro-average of the perturbed fields (Eq. 14, reading G23): "one can use orbit-averaged fields <E1>,
+                    <B1> in the above equations" -- in the weight equation (mode 2) and, in the non-linear
+                    mode (mode 3), in the trajectory as well.  The ring is built on the EQUILIBRIUM field at x_l.            */
+        double X[3] = {x, y, z}, B0c[3] = {BR, BP, BZ}, pts[4][3];
+        gyro_ring(X, B0c, c, sn, mu, q, m, pts);
+        flr_average(pv, pts, c, sn, t, &f);
+    }
+    if (nonlinear) {
         BR += f.B1[0]; BP += f.B1[1]; BZ += f.B1[2];
         ER = f.E1[0] - (mu / q) * (f.Bm_R + f.gB1p[0]);
         EP = f.E1[1] - (mu / q) * f.gB1p[1];
         EZ = f.E1[2] - (mu / q) * (f.Bm_Z + f.gB1p[2]);
-    }
-    if (sp->mode == 2) {   /* linear delta-f with the 4-point gyro-average of the perturbed fields (Eq. 14, reading G23) */
-        double X[3] = {x, y, z}, B0c[3] = {BR, BP, BZ}, pts[4][3];
-        gyro_ring(X, B0c, c, sn, mu, q, m, pts);
-        flr_average(pv, pts, c, sn, t, &f);
     }
     double B[3] = {BR * c - BP * sn, BR * sn + BP * c, BZ};
     double E[3] = {ER * c - EP * sn, ER * sn + EP * c, EZ};
@@ -518,7 +522,7 @@ static int step_marker(const provider *pv, const orc_species *sp, double *s, dou
     double wdot = weight_rhs(&f, sp, R, vlc, mu);
     /* Eq. (8): dw/dt = -(1 - w) (1/f0) df0/dt; the linear mode takes (1 - w) -> 1, the non-linear mode
      * keeps the factor, explicit in w on the staggered grid (readings G9, G21)                                    */
-    if (sp->mode == 1) wdot *= (1.0 - s[7]);
+    if (nonlinear) wdot *= (1.0 - s[7]);
     s[7] = s[7] + dt * wdot;
     /* 8 */
     s[0] = x + dt * vp[0]; s[1] = y + dt * vp[1]; s[2] = z + dt * vp[2];

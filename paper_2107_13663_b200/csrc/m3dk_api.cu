@@ -444,8 +444,8 @@ extern "C" int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, 
 extern "C" int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, double t0) {
     if (!ctx) return M3DK_EINVAL;
     if (sort_interval < 0) return fail(ctx, M3DK_EINVAL, "m3dk_set_options: sort_interval < 0");
-    if (mode < 0 || mode > 2)
-        return fail(ctx, M3DK_EINVAL, "m3dk_set_options: mode must be 0 (linear delta-f), 1 (non-linear trajectories) or 2 (linear + FLR)");
+    if (mode < 0 || mode > 3)
+        return fail(ctx, M3DK_EINVAL, "m3dk_set_options: mode must be 0 (linear delta-f), 1 (non-linear trajectories), 2 (linear + FLR) or 3 (non-linear + FLR)");
     ctx->sort_interval = sort_interval; ctx->mode = mode; ctx->t0 = t0;
     ctx->t_base = t0; ctx->steps_at_dt = 0;
     ctx->steps_done = 0;
@@ -741,7 +741,7 @@ extern "C" int m3dk_gc_push(m3dk_ctx *ctx, int nsteps, double dt, double *vpar) 
     if (nsteps < 0 || !(dt == dt) || (ctx->n > 0 && !vpar)) return fail(ctx, M3DK_EINVAL, "m3dk_gc_push: nsteps < 0, dt is NaN or vpar is NULL");
     CU(cudaSetDevice(ctx->device), "cudaSetDevice");
     // mode 1 (non-linear trajectories): the guiding centres move in the total fields at the context's time, which advances
-    const bool pert = ctx->mode == 1 && ctx->f.n_modes > 0;
+    const bool pert = (ctx->mode == 1 || ctx->mode == 3) && ctx->f.n_modes > 0;
     const double t0 = pert ? step_time(ctx, dt) : 0.0;
     CU(launch_gc_push(ctx, ctx->n, vpar, nsteps, dt, pert, t0), "guiding-centre kernel");
     if (pert) { ctx->steps_done += nsteps; ctx->steps_at_dt += nsteps; }

@@ -113,6 +113,7 @@ __device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, 
                                            const PertW &W);
 __device__ __forceinline__ void flr_emit(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
                                          const PertW &W, long slot);
+struct PertF;
 
 // kFlr (mode 2): phase B is replaced by the 4-point gyro-average of the perturbed fields.  kFlr = 1: every lane evaluates
 // its four ring points itself, each on its own element's tile read from global memory (flr_wdot).  kFlr = 2: the lane only
@@ -383,6 +384,48 @@ __device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, 
     return __dmul_rn(0.25, sum);
 }
 
+// Gyro-averaged perturbed fields of one marker in its own cylindrical frame (mode 3: non-linear trajectories in the
+// averaged fields): quarter sum over the ring points of the vectors in Cartesian components (Eq. 14), each
+// point searched and evaluated on its own element's tile (global memory); a point outside the mesh contributes zero.
+__device__ __forceinline__ void flr_avg_fields(const PushParams &P, const EqOut &f, const StepGeom &g, double zl, double mu,
+                                               PertF &out) {
+    FlrRing rg;
+    flr_ring(P, f, g, mu, rg);
+    double Ex = 0.0, Ey = 0.0, Ez = 0.0, Bx = 0.0, By = 0.0, Bz = 0.0, Gx = 0.0, Gy = 0.0, Gz = 0.0, dT = 0.0;
+#pragma unroll 1
+    for (int j = 0; j < 4; ++j) {
+        Marker sp;
+        flr_ring_point(rg, zl, j, sp.x, sp.y, sp.z);
+        StepGeom gj[1];
+        step_geometry(sp, gj[0]);
+        const int ej = locate_any(P.f, gj[0].R, sp.z);
+        if (ej < 0) continue;
+        const double *tile = P.f.tiles + (size_t)ej * P.f.tile_stride;
+        const Quad hd = ldq(tile);
+        const double se = hd.c;
+        const double xi[1] = {__dmul_rn(__dsub_rn(gj[0].R, hd.a), se)}, eta[1] = {__dmul_rn(__dsub_rn(sp.z, hd.b), se)};
+        PertF pf[1];
+        pf[0].ER = pf[0].EP = pf[0].EZ = pf[0].BR = pf[0].BP = pf[0].BZ = pf[0].gR = pf[0].gP = pf[0].gZ = pf[0].dT = 0.0;
+        pert_fields<1, false>(P, tile, xi, eta, gj, se, pf);
+        const double cj = gj[0].cph, sj = gj[0].sph;
+        Ex = __dadd_rn(Ex, M3DK_FMA(pf[0].ER, cj, -__dmul_rn(pf[0].EP, sj))); Ey = __dadd_rn(Ey, M3DK_FMA(pf[0].ER, sj, __dmul_rn(pf[0].EP, cj)));
+        Ez = __dadd_rn(Ez, pf[0].EZ);
+        Bx = __dadd_rn(Bx, M3DK_FMA(pf[0].BR, cj, -__dmul_rn(pf[0].BP, sj))); By = __dadd_rn(By, M3DK_FMA(pf[0].BR, sj, __dmul_rn(pf[0].BP, cj)));
+        Bz = __dadd_rn(Bz, pf[0].BZ);
+        Gx = __dadd_rn(Gx, M3DK_FMA(pf[0].gR, cj, -__dmul_rn(pf[0].gP, sj))); Gy = __dadd_rn(Gy, M3DK_FMA(pf[0].gR, sj, __dmul_rn(pf[0].gP, cj)));
+        Gz = __dadd_rn(Gz, pf[0].gZ);
+        dT = __dadd_rn(dT, pf[0].dT);
+    }
+    const double c = g.cph, sn = g.sph;
+    out.ER = __dmul_rn(0.25, M3DK_FMA(Ex, c, __dmul_rn(Ey, sn))); out.EP = __dmul_rn(0.25, M3DK_FMA(Ey, c, -__dmul_rn(Ex, sn)));
+    out.EZ = __dmul_rn(0.25, Ez);
+    out.BR = __dmul_rn(0.25, M3DK_FMA(Bx, c, __dmul_rn(By, sn))); out.BP = __dmul_rn(0.25, M3DK_FMA(By, c, -__dmul_rn(Bx, sn)));
+    out.BZ = __dmul_rn(0.25, Bz);
+    out.gR = __dmul_rn(0.25, M3DK_FMA(Gx, c, __dmul_rn(Gy, sn))); out.gP = __dmul_rn(0.25, M3DK_FMA(Gy, c, -__dmul_rn(Gx, sn)));
+    out.gZ = __dmul_rn(0.25, Gz);
+    out.dT = __dmul_rn(0.25, dT);
+}
+
 // kFlr = 2: emit the four ring points of the marker in output slot `slot` into the ring stream (positions, flagged live)
 // and the marker's weights.  Their elements are found by ring_key_kernel, one thread per ring point: four searches and
 // four returned atomics in a row inside the push would serialise eight L2 round trips per marker.
@@ -440,7 +483,7 @@ __global__ void __launch_bounds__(256) ring_key_kernel(const __grid_constant__ F
 // ---- the same step in the non-linear trajectory mode (mode 1: PAPER.md:108, :130; reading G21) ------------------------
 // All perturbed fields are needed BEFORE the velocity update (the marker moves in the total fields), so they are
 // accumulated per marker (10 values) and the folding trick of the linear mode does not apply; B1_phi (quad 3) enters.
-template <int R, bool kHist, bool kSmem, class IO, bool kPost = false>
+template <int R, bool kHist, bool kSmem, class IO, bool kPost = false, bool kFlr = false>
 __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, const double *__restrict__ tile,
                                           const long (&mi)[R], const long (&mo)[R], const bool (&on)[R], double (&Rn)[R],
                                           double (&Zn)[R]) {
@@ -472,7 +515,13 @@ __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, con
         f[r].F = v[r][2]; f[r].kappa = v[r][3];
         pf[r].ER = pf[r].EP = pf[r].EZ = pf[r].BR = pf[r].BP = pf[r].BZ = pf[r].gR = pf[r].gP = pf[r].gZ = pf[r].dT = 0.0;
     }
-    pert_fields<R, kSmem>(P, tile, xi, eta, g, se, pf);
+    if constexpr (kFlr) {           // mode 3: the gyro-averaged perturbed fields replace the fields at the marker
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (P.f.n_modes > 0) flr_avg_fields(P, f[r], g[r], s[r].z, s[r].mu, pf[r]);
+    } else {
+        pert_fields<R, kSmem>(P, tile, xi, eta, g, se, pf);
+    }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const double w_old = s[r].w;
@@ -520,7 +569,7 @@ __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant
     if (__any_sync(0xffffffffu, on[0])) {
         double Rn[1], Zn[1];
         const SoAIO io{P.a, P.f.n_elems};
-        if (kMode == 1) step_R_nl<1, false, false>(P, io, tile, m, m, on, Rn, Zn);
+        if (kMode == 1 || kMode == 4) step_R_nl<1, false, false, SoAIO, false, kMode == 4>(P, io, tile, m, m, on, Rn, Zn);
         else step_R<1, false, false, SoAIO, kMode == 2 ? 1 : 0>(P, io, tile, m, m, on, Rn, Zn);
     }
 }
@@ -631,7 +680,7 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
             mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
             phase ^= 1u << b;
             double Rn[kR], Zn[kR];
-            if (kMode == 1) step_R_nl<kR, kHist, true>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
+            if (kMode == 1 || kMode == 4) step_R_nl<kR, kHist, true, RecIO, false, kMode == 4>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
             else step_R<kR, kHist, true, RecIO, kMode == 2 ? 1 : (kMode == 3 ? 2 : 0)>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
         }
         b ^= 1;
@@ -1042,6 +1091,7 @@ cudaError_t launch_push_soa(m3dk_ctx *c, long n, double dt, double t) {
     c->kernel_launches += 1;
     if (c->mode == 1) push_generic_kernel<1><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
     else if (c->mode == 2) push_generic_kernel<2><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
+    else if (c->mode == 3) push_generic_kernel<4><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
     else push_generic_kernel<0><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(P);
     return cudaGetLastError();
 }
@@ -1097,16 +1147,18 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
                 continue;
             }
             // mode 2: with an FLR workspace the push emits the ring stream (kernel mode 3), else every lane gathers its ring
-            const int km = c->mode == 2 ? (flr_stream ? 3 : (c->f.n_modes > 0 ? 2 : 0)) : c->mode;
+            const int km = c->mode == 2 ? (flr_stream ? 3 : (c->f.n_modes > 0 ? 2 : 0)) : c->mode == 3 ? 4 : c->mode;
             if (small)
                 kern = km == 1   ? (with_hist ? push_items_kernel<true, 1, 1> : push_items_kernel<false, 1, 1>)
                        : km == 2 ? (with_hist ? push_items_kernel<true, 2, 1> : push_items_kernel<false, 2, 1>)
                        : km == 3 ? (with_hist ? push_items_kernel<true, 3, 1> : push_items_kernel<false, 3, 1>)
+                       : km == 4 ? (with_hist ? push_items_kernel<true, 4, 1> : push_items_kernel<false, 4, 1>)
                                  : (with_hist ? push_items_kernel<true, 0, 1> : push_items_kernel<false, 0, 1>);
             else
                 kern = km == 1   ? (with_hist ? push_items_kernel<true, 1, 2> : push_items_kernel<false, 1, 2>)
                        : km == 2 ? (with_hist ? push_items_kernel<true, 2, 2> : push_items_kernel<false, 2, 2>)
                        : km == 3 ? (with_hist ? push_items_kernel<true, 3, 2> : push_items_kernel<false, 3, 2>)
+                       : km == 4 ? (with_hist ? push_items_kernel<true, 4, 2> : push_items_kernel<false, 4, 2>)
                                  : (with_hist ? push_items_kernel<true, 0, 2> : push_items_kernel<false, 0, 2>);
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;

@@ -126,3 +126,38 @@ def test_flr_where_b_is_parallel_to_the_major_radius():
     rhs = p.deposit(flags=2, t=0.0)
     assert np.isfinite(rhs).all()
     assert np.abs(rhs - want).max() <= 1e-10 * max(np.abs(want).max(), 1e-300)
+
+
+@pytest.mark.parametrize("verify", [True, False])
+def test_nonlinear_mode_with_gyro_average(verify):
+    """Mode 3 (non-linear trajectories in the gyro-averaged perturbed fields; oracle pin F6): one step restarted from the
+    oracle at steps 0 and 9, amplitude 1e-2 so that the perturbation moves the orbits; then the same bits for the SoA path and
+    the ordered pipeline over 6 chained steps."""
+    w = synth.make_config(3, n_markers=5000 + 11, nx=64, amp=1e-2)
+    mesh, sp = oracle_of(w, mode=3)
+    p = make_pusher(w, verify=verify, mode=3)
+    state = {k: w.markers[k].copy() for k in KEYS}
+    done = 0
+    for s in (0, 9):
+        if s > done:
+            state, _, _ = oracle_push(mesh, sp, state, s - done, w.dt, t0=0.0, step0=done)
+            done = s
+        ref, e_ref, _ = oracle_push(mesh, sp, state, 1, w.dt, t0=0.0, step0=s)
+        p.set_state(state)
+        p.set_options(sort_interval=0, mode=3, t0=s * w.dt)
+        p.push(1, w.dt)
+        got, _, _ = p.state()
+        live = e_ref >= 0
+        wrms = np.sqrt(np.mean(ref["w"][live] ** 2))
+        ex, ev, ew = g16_errors(take(got, live), take(ref, live), w_floor=wrms)
+        assert max(ex.max(), ev.max(), ew.max()) <= TOL_STEP, (s, ex.max(), ev.max(), ew.max())
+    lin, _, _ = oracle_push(*oracle_of(w, mode=1), w.markers, 6, w.dt)
+    res = {}
+    for si in (0, 1):
+        q = make_pusher(w, verify=verify, sort_interval=si, mode=3)
+        q.push(6, w.dt)
+        res[si], _, ids = q.state()
+        assert np.array_equal(np.sort(ids), np.arange(w.n_markers))
+    for k in KEYS:
+        assert np.array_equal(res[0][k], res[1][k]), k
+    assert np.abs(res[0]["vx"] - lin["vx"]).max() > 1e-7          # the average changes the orbit itself

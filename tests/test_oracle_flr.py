@@ -148,3 +148,52 @@ def test_f5_ring_where_b_is_parallel_to_the_major_radius(orc):
     assert np.allclose(d[0], -d[2], atol=1e-15) and np.allclose(d[1], -d[3], atol=1e-15)
     assert abs(d[0] @ d[1]) < 1e-12 * rho * rho
     assert np.allclose(np.cross(bx, d[0]), d[1], rtol=1e-12, atol=1e-15)          # e2 = b0 x e1
+
+
+def check_f6_nonlinear_mode_with_gyro_average(orc):
+    """Mode 3 = the non-linear trajectories of mode 1 in the gyro-averaged perturbed fields of mode 2 ("use
+    orbit-averaged fields in the above equations").  (a) mu = 0: the ring collapses onto X, mode 3 is mode 1 up to the
+    rounding of the rotation to Cartesian components and back.  (b) Amplitudes of the Z components (E_Z, B_Z: Cartesian
+    components) that are linear in Z with n = 0 are averaged exactly by the symmetric ring, so the trajectories of modes 3
+    and 1 agree to round-off although rho != 0.  (c) On the config-1 kink (a field that is NOT linear over the ring) the two
+    modes differ by much more: the average does something; and with amplitude 0 mode 3 is the linear mode bit for bit."""
+    from handmade import HandMade
+    from synth.configs import CHARGE, MASS
+    w = synth.make_config(1, n_markers=300, nx=16, amp=1e-2)
+    mesh = orc.Mesh.of(w)
+    mk0 = {k: v.copy() for k, v in w.markers.items()}
+    mk0["mu"][:] = 0.0
+    a, _, _ = orc.push_fe(mesh, orc.species_of(w, mode=1), mk0, 20, w.dt)
+    b, _, _ = orc.push_fe(mesh, orc.species_of(w, mode=3), mk0, 20, w.dt)
+    for k in ("x", "vx", "vz", "w"):
+        scale = np.sqrt(np.mean(a[k] ** 2))
+        assert np.abs(a[k] - b[k]).max() < 1e-11 * scale, k
+    # (b)
+    hm = HandMade(eq=dict(psi=(0.0, 0.0, 0.0, 0.4), Bm=(0.8,), F=(2.4,), kappa=(0.3,)),
+                  pert=dict(E_Z=(1e-3, 0.0, -1e-3), B_Z=(2e-3, 0.0, 3e-3)), n_tor=0, omega=0.0)
+    hmesh = hm.oracle_mesh(orc)
+    rng = np.random.Generator(np.random.PCG64(14))
+    n = 50
+    R, ph, Z = rng.uniform(2.6, 3.4, n), rng.uniform(-3, 3, n), rng.uniform(-0.5, 0.5, n)
+    m2 = dict(x=R * np.cos(ph), y=R * np.sin(ph), z=Z, vx=0.3 * rng.normal(size=n), vy=0.3 * rng.normal(size=n),
+              vz=0.3 * rng.normal(size=n), mu=np.full(n, 0.01), w=np.zeros(n))
+    sp1, sp3 = orc.species(CHARGE, MASS, 0, T=0.5, mode=1), orc.species(CHARGE, MASS, 0, T=0.5, mode=3)
+    a, _, _ = orc.push_fe(hmesh, sp1, m2, 3, 0.01)
+    b, _, _ = orc.push_fe(hmesh, sp3, m2, 3, 0.01)
+    rho = np.sqrt(2 * MASS * 0.01 / 0.8)
+    assert rho > 0.02
+    assert np.abs(a["vz"] - b["vz"]).max() < 1e-14 and np.abs(a["x"] - b["x"]).max() < 1e-14
+    assert np.abs(a["vz"] - m2["vz"]).max() > 1e-5                     # the fields do act
+    # (c)
+    a, _, _ = orc.push_fe(mesh, orc.species_of(w, mode=1), w.markers, 20, w.dt)
+    b, _, _ = orc.push_fe(mesh, orc.species_of(w, mode=3), w.markers, 20, w.dt)
+    assert np.abs(a["w"] - b["w"]).max() > 1e-3 * np.sqrt(np.mean(a["w"] ** 2))
+    w0 = synth.make_config(1, n_markers=100, nx=16, amp=0.0)
+    a, _, _ = orc.push_fe(orc.Mesh.of(w0), orc.species_of(w0, mode=0), w0.markers, 10, w0.dt)
+    b, _, _ = orc.push_fe(orc.Mesh.of(w0), orc.species_of(w0, mode=3), w0.markers, 10, w0.dt)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_f6_nonlinear_mode_with_gyro_average(orc):
+    check_f6_nonlinear_mode_with_gyro_average(orc)

@@ -1,5 +1,5 @@
-"""Mutation checks of the pins M1-M3, N1, Q1, Q2 (tests/test_oracle_magnetic.py), G5, G6, G7 (tests/test_oracle_gc.py) and D7
-(tests/test_oracle_deposit.py).
+"""Mutation checks of the pins M1-M3, N1, Q1, Q2 (tests/test_oracle_magnetic.py), G5, G6, G7 (tests/test_oracle_gc.py) D7
+(tests/test_oracle_deposit.py) and F6 (tests/test_oracle_flr.py).
 
 Each case compiles a COPY of oracle/m3dk_oracle.c with one plausible mistake (a flipped sign, a dropped factor, a wrong
 index) into a temporary directory, routes the oracle binding to that copy and asserts that the named pin FAILS -- the
@@ -9,10 +9,11 @@ import pytest
 
 from test_oracle_gc import check_g5_phase_space_volume, check_g6_bootstrap, check_g7_perturbed_guiding_centre_rhs
 from test_oracle_deposit import check_d7_jacobian_substitution
+from test_oracle_flr import check_f6_nonlinear_mode_with_gyro_average
 from test_oracle_magnetic import CHECKS as _MAGNETIC
 
 CHECKS = dict(_MAGNETIC, g5=check_g5_phase_space_volume, g6=check_g6_bootstrap, g7=check_g7_perturbed_guiding_centre_rhs,
-              d7=check_d7_jacobian_substitution)
+              d7=check_d7_jacobian_substitution, f6=check_f6_nonlinear_mode_with_gyro_average)
 
 #        pin   tag                      text in the oracle source                         mutated text
 MUTANTS = [
@@ -48,6 +49,8 @@ MUTANTS = [
     ("g7", "mirror_of_B1par_dropped", "gB[k] += f.gB1p[k]; E[k] = f.E1[k]; }", "E[k] = f.E1[k]; }"),
     ("g7", "parallel_E_sign", "*dvpar = (q / m) * (Bs[0] * Ee[0] + Bs[1] * Ee[1] + Bs[2] * Ee[2]) / Bspar;",
      "*dvpar = -(q / m) * (Bs[0] * Ee[0] + Bs[1] * Ee[1] + Bs[2] * Ee[2]) / Bspar;"),
+    ("f6", "mode3_without_average", "flr = sp->mode == 2 || sp->mode == 3;", "flr = sp->mode == 2;"),
+    ("f6", "mode3_linear_trajectory", "nonlinear = sp->mode == 1 || sp->mode == 3,", "nonlinear = sp->mode == 1,"),
     ("g6", "bootstrap_sign", "vx[i] = (s[0] - x[i]) / dt;", "vx[i] = (x[i] - s[0]) / dt;"),
     ("g6", "bootstrap_keeps_x0", "x[i] = s[0]; y[i] = s[1]; z[i] = s[2];\n    }\n}", "\n    }\n}"),
     ("q1", "psi_ZZ_dropped", "g->psi_ZZ = d * s * s;", "g->psi_ZZ = 0.0 * d;"),
