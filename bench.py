@@ -292,11 +292,20 @@ def run_ours(args, rank, world, local_rank):
     p.set_profiling(False)
 
     # ---- end-to-end leg: host buffers through the C ABI (m3dk_push_host), copies inside the timed region ------------------
-    # One call = upload + K steps + download of all markers, pipelined by marker chunk.  The buffers are the ones a first
-    # call returned (element order, the steady state of a caller that keeps pushing the same markers): a chunk is then
-    # spatially compact and keeps the full number of markers per element.
-    host = {k: torch.from_numpy(np.ascontiguousarray(w.markers[k])).pin_memory() for k in m3dk.STATE_KEYS}
+    # One call = upload + K steps + download of all markers, pipelined by marker chunk.  A chunk is a range of the host
+    # buffers and stays that set of markers from call to call.  Markers stream around their flux surface, so a chunk that
+    # starts as a range of elements is spread over the whole mesh after some twenty steps (a quarter of the markers per
+    # element: the work items fill badly); a chunk that is a radial shell stays a shell and keeps its markers per element.
+    if args.e2e_order == "shell":
+        # caller's marker order: by minor radius of the loaded position, so that a chunk is a radial shell
+        Rm = np.hypot(w.markers["x"], w.markers["y"])
+        perm = np.argsort(w.eq.rtheta(Rm, w.markers["z"])[0], kind="stable")
+    else:
+        perm = np.arange(N)
+    host = {k: torch.from_numpy(np.ascontiguousarray(w.markers[k][perm])).pin_memory() for k in m3dk.STATE_KEYS}
     Ke, C_e2e = K, args.e2e_chunks
+    if args.e2e_order == "element":
+        p.push_host(host, 1, w.dt, n_chunks=1)
     p.push_host(host, 1, w.dt, n_chunks=C_e2e)
     p.set_options(sort_interval=si, mode=args.mode, t0=0.0)
     barrier()
@@ -309,6 +318,11 @@ def run_ours(args, rank, world, local_rank):
 
     ms, ms_e2e = shard.max_over_ranks([ms, ms_e2e], dist if world > 1 else None, device=dev)
     dep = None
+    if args.deposit or args.gc:
+        # the e2e leg left the device arrays chunk by chunk; the rows below are timed on the state a device-resident
+        # push leaves (all markers in the element order of the step before)
+        p.push(2, w.dt)
+        barrier()
     if args.deposit:
         # row (f)-4 with its exchange step: every rank deposits its shard, the moment tables are summed over the ranks
         need = p.deposit_bytes()
@@ -365,7 +379,7 @@ def run_ours(args, rank, world, local_rank):
             "e2e": {"value": shard.whole_job_rate([N] * world, Ke, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": 64 * N / Ke,
                     "d2h_bytes_per_step": 64 * N / Ke,
                     "note": f"m3dk_push_host: one upload + {Ke} steps + one download per call (PAPER.md:237), pipelined in "
-                            f"{C_e2e} marker chunks; host buffers pinned, in the element order an earlier call returned"},
+                            f"{C_e2e} marker chunks; host buffers pinned, order of the markers: {args.e2e_order}"},
             "roofline": roof, "n_lost": st["n_lost"]}
     if args.gc:
         # row (f)-3: RK4 guiding-centre steps on the same markers (x, y, z as X; v_par = 0.5 for every marker)
@@ -379,7 +393,8 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize(dev)
         gms = g0.elapsed_time(g1) / 10
         line["gc"] = {"ms_per_step": gms, "particle_steps_per_s": N / (gms * 1e-3),
-                      "note": "m3dk_gc_push, RK4 on Eqs. (1)-(4), equilibrium fields (SURVEY.md 8(f)-3); 4 field evaluations per step"}
+                      "fields": "equilibrium + perturbation (reading G26)" if args.mode in (1, 3) and w.n_modes else "equilibrium",
+                      "note": "m3dk_gc_push, RK4 on Eqs. (1)-(4) (SURVEY.md 8(f)-3); 4 field evaluations per step"}
     if dep is not None:
         dms, need = dep
         dbytes = (68.0 * N + need)            # 8 fp64 + element key per marker read, the table cleared and accumulated
@@ -467,6 +482,8 @@ def main():
     ap.add_argument("--deposit", action="store_true", help="also time m3dk_deposit (SURVEY.md 8(f)-4) on the final state")
     ap.add_argument("--deposit-flags", type=int, default=1, help="flags of the timed m3dk_deposit (1 B1par, 2 FLR, 4 Bstar)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-order", choices=("shell", "element", "loaded"), default="shell",
+                    help="order of the host buffers of the e2e leg: radial shells, the element order a one-chunk call returns, as loaded")
     ap.add_argument("--e2e-chunks", type=int, default=4, help="marker chunks of the pipelined host-buffer call (e2e leg)")
     ap.add_argument("--push-variant", type=int, default=0, choices=[0, 1],
                     help="m3dk_set_push_variant: 0 = default kernel, 1 = asynchronously staged kernel (A/B comparison)")

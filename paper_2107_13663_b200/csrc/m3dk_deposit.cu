@@ -21,8 +21,12 @@ struct DepMarker { double amp[2], T[kDepHarmMax], xp[6], ep[6]; };
 // d = w + B1par / B*par in both moments (reading G25); cwt / swt = cos / sin(omega_k t); q = species charge
 struct DepOpts { int with_b1par, with_bstar; double q; double cwt[M3DK_MAX_MODES], swt[M3DK_MAX_MODES]; };
 
+// kF: bit 0 = with_b1par, bit 1 = with_bstar, as compile-time constants (the second-derivative scheme of B*par costs
+// 80 registers, which the plain deposition must not pay for)
+template <int kF>
 __device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &o, int e, const Marker &s, double mass,
                                            DepMarker &d) {
+    constexpr bool kB1 = (kF & 1) != 0, kBs = (kF & 2) != 0;
     StepGeom g;
     step_geometry(s, g);
     // equilibrium quad at the marker: B0 = grad psi0 x grad phi + F0 grad phi (G4), |B|0 from its own table
@@ -40,7 +44,7 @@ __device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &
     const double vR = M3DK_FMA(s.vx, g.cph, __dmul_rn(s.vy, g.sph)), vP = M3DK_FMA(s.vy, g.cph, -__dmul_rn(s.vx, g.sph));
     const double vpar = __dmul_rn(M3DK_FMA(vR, BR, M3DK_FMA(vP, BP, __dmul_rn(s.vz, BZ))), binv);
     double b1p = 0.0;     // B1par = Re[C e^{i(n phi - omega t)}] from quad 2 of every mode
-    if (o.with_b1par || o.with_bstar) {
+    if (kB1 || kBs) {
         const double Bm0 = v[0][1];
         for (int md = 0; md < f.n_modes; ++md) {
             double cth, sth;
@@ -53,7 +57,7 @@ __device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &
         v[0][1] = Bm0;
     }
     double dd = s.w;
-    if (o.with_bstar) {   // d = w + B1* / B* with B1* -> B1par and B* = B*par of Eq. (4) at this marker's v_par
+    if (kBs) {   // d = w + B1* / B* with B1* -> B1par and B* = B*par of Eq. (4) at this marker's v_par
         GcEq ge;
         gc_eq_fields(tile, g.R, s.z, ge);
         double Bs[3], bb[3];
@@ -61,7 +65,7 @@ __device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &
     }
     d.amp[0] = __dmul_rn(__dmul_rn(dd, mass), __dmul_rn(vpar, vpar));
     d.amp[1] = __dmul_rn(__dmul_rn(dd, s.mu), v[0][1]);
-    if (o.with_b1par) d.amp[1] = M3DK_FMA(s.mu, b1p, d.amp[1]);   // Eq. (16): mu |B|0 (w + B1par/|B|0)
+    if (kB1) d.amp[1] = M3DK_FMA(s.mu, b1p, d.amp[1]);   // Eq. (16): mu |B|0 (w + B1par/|B|0)
     d.T[0] = 1.0;     // toroidal factors by complex powers of (cos phi + i sin phi)
 #pragma unroll
     for (int md = 0; md < M3DK_MAX_MODES; ++md)
@@ -72,6 +76,7 @@ __device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &
 }
 
 // any marker order: one marker per lane, the warp loops over its distinct elements
+template <int kF>
 __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
                                                       MarkerArrays a, long n, double mass, double *__restrict__ rhs) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -87,7 +92,7 @@ __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ Fi
         s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
     }
     DepMarker d;
-    dep_marker(f, o, e, s, mass, d);
+    dep_marker<kF>(f, o, e, s, mass, d);
     const size_t stride_e = (size_t)2 * H * M3DK_NCOEF;
     unsigned todo = __ballot_sync(0xffffffffu, active);
     while (todo) {
@@ -120,7 +125,7 @@ __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ Fi
 // finds the point's element and the warp loops over its distinct elements exactly as deposit_kernel does.
 // kRec: the markers are read from the element-ordered records of the sort workspace (a warp's 32 markers then share an
 // element and their rings touch a handful of elements), else from the caller's arrays in whatever order they are.
-template <bool kRec>
+template <bool kRec, int kF>
 __global__ void __launch_bounds__(128) deposit_flr_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
                                                           MarkerArrays a, const double *__restrict__ rec,
                                                           const int *__restrict__ key, long n, double q, double mass,
@@ -142,7 +147,7 @@ __global__ void __launch_bounds__(128) deposit_flr_kernel(const __grid_constant_
         s.x = 1.0; s.y = 0.0; s.z = 0.0; s.vx = s.vy = s.vz = 0.0; s.mu = 0.0; s.w = 0.0;
     }
     DepMarker d;
-    dep_marker(f, o, e, s, mass, d);          // amplitudes at the marker itself
+    dep_marker<kF>(f, o, e, s, mass, d);          // amplitudes at the marker itself
     // the ring: same construction as flr_wdot of the push (reading G23)
     StepGeom g;
     step_geometry(s, g);
@@ -222,6 +227,7 @@ __global__ void __launch_bounds__(128) deposit_flr_kernel(const __grid_constant_
 
 // element-ordered records cut into work items (the ordering kernels of m3dk_sort.cu): a warp takes an item (<= 64
 // markers of ONE element), every lane two of them, one reduction and one atomic per table entry and item
+template <int kF>
 __global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
                                                             const double *__restrict__ rec,
                                                             const int4 *__restrict__ items, const int *__restrict__ n_items,
@@ -243,7 +249,7 @@ __global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constan
             const double *p = rec + (size_t)kRecDoubles * (start + 32 * r + lane);
             s.x = p[0]; s.y = p[1]; s.z = p[2]; s.w = p[3]; s.vx = p[4]; s.vy = p[5]; s.vz = p[6]; s.mu = p[7];
         }
-        dep_marker(f, o, e, s, mass, d[r]);
+        dep_marker<kF>(f, o, e, s, mass, d[r]);
         if (!on) { d[r].amp[0] = 0.0; d[r].amp[1] = 0.0; }
     }
     double *out = rhs + (size_t)e * 2 * H * M3DK_NCOEF;
@@ -274,6 +280,7 @@ __global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constan
 // The ring points of all markers are emitted (position + the marker's two amplitudes), ordered by THEIR element with the
 // ring-ordering kernels of the FLR push (ring_key_kernel, scan, work-item cut, placement), and a warp deposits a ring item
 // (up to 64 ring points of one element) with shuffle reductions and one atomic per table entry.
+template <int kF>
 __global__ void __launch_bounds__(128) deposit_flr_emit_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
                                                                const double *__restrict__ rec, const int *__restrict__ key, long n,
                                                                double q, double mass, double *__restrict__ ring,
@@ -293,7 +300,7 @@ __global__ void __launch_bounds__(128) deposit_flr_emit_kernel(const __grid_cons
     Marker s;
     s.x = p[0]; s.y = p[1]; s.z = p[2]; s.w = p[3]; s.vx = p[4]; s.vy = p[5]; s.vz = p[6]; s.mu = p[7];
     DepMarker d;
-    dep_marker(f, o, e, s, mass, d);          // amplitudes at the marker itself
+    dep_marker<kF>(f, o, e, s, mass, d);          // amplitudes at the marker itself
     wts[10 * i] = d.amp[0]; wts[10 * i + 1] = d.amp[1];
     // the ring: same construction as the FLR push (reading G23)
     StepGeom g;
@@ -393,11 +400,15 @@ __global__ void __launch_bounds__(128) deposit_ring_items_kernel(const __grid_co
         }
 }
 
+// the four instantiations of a kernel template whose LAST parameter is kF (0 .. 3)
+#define M3DK_DEP_PICK(kf, ...) ((kf) == 0 ? __VA_ARGS__ 0> : (kf) == 1 ? __VA_ARGS__ 1> : (kf) == 2 ? __VA_ARGS__ 2> : __VA_ARGS__ 3>)
+
 cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t) {
     DepOpts o{};
     o.with_b1par = (flags & 1) && c->f.n_modes > 0;
     o.with_bstar = (flags & 4) && c->f.n_modes > 0;
     o.q = c->q;
+    const int kf = (o.with_b1par ? 1 : 0) | (o.with_bstar ? 2 : 0);
     for (int k = 0; k < c->f.n_modes; ++k) { o.cwt[k] = cos(c->f.omega[k] * t); o.swt[k] = sin(c->f.omega[k] * t); }
     const size_t bytes = (size_t)c->f.n_elems * 2 * (1 + 2 * c->f.n_modes) * M3DK_NCOEF * sizeof(double);
     cudaError_t e = cudaMemsetAsync(rhs, 0, bytes, c->stream);
@@ -411,8 +422,8 @@ cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t
             e = cudaMemsetAsync(c->fb.a.rhist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
             if (e != cudaSuccess) return e;
             c->kernel_launches += 3;
-            deposit_flr_emit_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->sb.rec[c->cur], c->sb.key, n,
-                                                                                       c->q, c->m, c->fb.a.ring, c->fb.a.wts);
+            M3DK_DEP_PICK(kf, deposit_flr_emit_kernel<)<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(
+                c->f, o, c->sb.rec[c->cur], c->sb.key, n, c->q, c->m, c->fb.a.ring, c->fb.a.wts);
             e = launch_flr_ring_keys(c, n);
             if (e != cudaSuccess) return e;
             e = launch_flr_ring_stage(c, n);
@@ -427,12 +438,12 @@ cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t
             e = launch_pack_sorted(c, n);
             if (e != cudaSuccess) return e;
             c->kernel_launches += 1;
-            deposit_flr_kernel<true><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->user, c->sb.rec[c->cur],
-                                                                                        c->sb.key, n, c->q, c->m, rhs);
+            M3DK_DEP_PICK(kf, deposit_flr_kernel<true,)<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(
+                c->f, o, c->user, c->sb.rec[c->cur], c->sb.key, n, c->q, c->m, rhs);
         } else {
             c->kernel_launches += 1;
-            deposit_flr_kernel<false><<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->user, nullptr, nullptr, n,
-                                                                                         c->q, c->m, rhs);
+            M3DK_DEP_PICK(kf, deposit_flr_kernel<false,)<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(
+                c->f, o, c->user, nullptr, nullptr, n, c->q, c->m, rhs);
         }
         return cudaGetLastError();
     }
@@ -443,14 +454,14 @@ cudaError_t launch_deposit(m3dk_ctx *c, long n, double *rhs, int flags, double t
         if (e != cudaSuccess) return e;
         const long max_items = n / kItemMarkers + c->f.n_elems + 2, max_small = c->f.n_elems + 2;
         c->kernel_launches += 2;
-        deposit_items_kernel<<<(unsigned)((max_items + 3) / 4), 128, 0, c->stream>>>(
+        M3DK_DEP_PICK(kf, deposit_items_kernel<)<<<(unsigned)((max_items + 3) / 4), 128, 0, c->stream>>>(
             c->f, o, c->sb.rec[c->cur], c->sb.items, c->sb.ioffs + c->f.n_elems + 1, c->m, rhs);
-        deposit_items_kernel<<<(unsigned)((max_small + 3) / 4), 128, 0, c->stream>>>(          // the small items
+        M3DK_DEP_PICK(kf, deposit_items_kernel<)<<<(unsigned)((max_small + 3) / 4), 128, 0, c->stream>>>(          // the small items
             c->f, o, c->sb.rec[c->cur], c->sb.items_small, reinterpret_cast<const int *>(c->sb.scan_state + 1), c->m, rhs);
         return cudaGetLastError();
     }
     c->kernel_launches += 1;
-    deposit_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->user, n, c->m, rhs);
+    M3DK_DEP_PICK(kf, deposit_kernel<)<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->f, o, c->user, n, c->m, rhs);
     return cudaGetLastError();
 }
 
