@@ -156,3 +156,57 @@ def test_deposit_with_the_jacobian_substitution(flags, si):
     assert (err <= 1e-11 * S).all(), float((err / S).max())
     base, _ = oracle.deposit(mesh, sp, raw, flags=flags & 3, t=t)
     assert np.abs(ref - base).max() > 1e-4 * np.abs(base).max()          # the substitution does change the table
+
+
+@pytest.mark.parametrize("flags", [0, 1, 5, 3, 7])
+def test_full_size_deposit_on_sampled_elements(flags):
+    """BASELINE.json configs[3] at full size (2^24 markers, 256 x 256 mesh) in the launch configuration
+    `bench.py --deposit --deposit-flags F` times (sort workspace, FLR workspace for the 4-point deposition, timing build).
+    The oracle computes the rows of a sample of elements: it deposits only the markers that can reach a sampled element
+    (position inside the element's bounding box, widened by more than the largest gyro-radius when the ring is
+    deposited), chosen from the INPUT positions; the rows of the sampled elements are then complete and are compared."""
+    from synth.configs import CHARGE, MASS
+    w = synth.make_config(3)
+    assert w.n_markers == 1 << 24 and w.n_elems == 131072
+    rng = np.random.Generator(np.random.PCG64(2024))
+    mk = {k: v.copy() for k, v in w.markers.items()}
+    mk["w"] = rng.normal(size=w.n_markers) * 1e-3
+    R, Z = np.hypot(mk["x"], mk["y"]), mk["z"]
+    flr = bool(flags & 2)
+    margin = 0.0
+    if flr:
+        # textbook gyro-radius m v_perp / (|q| B) with v_perp^2 = 2 mu B / m: only to size the margin generously
+        B = w.eq.Bmag(R, Z)
+        rho = np.sqrt(2.0 * mk["mu"] * B / MASS) * MASS / (abs(CHARGE) * B)
+        margin = 1.5 * float(rho.max()) + 1e-3
+        assert margin < 0.1
+    n_sample = 24 if flr else 192
+    elems = np.linspace(1000, w.n_elems - 1000, n_sample).astype(np.int64)
+    # keep the sampled elements that hold markers at all (the mesh box is larger than the plasma)
+    tri = w.node_RZ[w.tri[elems]]                                # [n_sample][3][2]
+    lo, hi = tri.min(axis=1) - margin, tri.max(axis=1) + margin
+    sel = np.zeros(w.n_markers, dtype=bool)
+    for k in range(n_sample):
+        sel |= (R >= lo[k, 0]) & (R <= hi[k, 0]) & (Z >= lo[k, 1]) & (Z <= hi[k, 1])
+    sub = {k: np.ascontiguousarray(v[sel]) for k, v in mk.items()}
+    assert 10_000 < sub["x"].size < 4_000_000
+    mesh, sp = oracle_of(w)
+    t = 0.9
+    ref, _ = oracle.deposit(mesh, sp, sub, flags=flags, t=t)
+    absw = dict(sub)
+    absw["w"] = np.abs(sub["w"]) + (1e-3 if flags & 4 else 0.0)  # + a bound of |B1par / B*par| (amplitude 1e-4 B0)
+    scale, _ = oracle.deposit(mesh, sp, absw, flags=flags & 2)
+    S = np.abs(scale[:, :, 0, 0])[:, :, None, None] + np.abs(scale).max() * 1e-3
+    p = make_pusher(dataclasses.replace(w, markers=mk), verify=False, sort_interval=1)
+    if flr:
+        p.set_flr_workspace()
+    got = p.deposit(flags=flags, t=t)
+    assert got.shape == (w.n_elems, 2, 3, 21)
+    err = np.abs(got[elems] - ref[elems])
+    assert (err <= 1e-11 * S[elems]).all(), float((err / S[elems]).max())
+    assert (np.abs(ref[elems]).max(axis=(1, 2, 3)) > 0).sum() > n_sample // 3       # the sample does hold markers
+    # nothing is lost or duplicated on the way through the ordering: the unit test function sums to sum(d)
+    if flags == 0:
+        tot = got[:, 1, 0, 0].sum()
+        refsum = float(np.sum(mk["w"] * mk["mu"] * w.eq.Bmag(R, Z)))
+        assert abs(tot - refsum) <= 1e-5 * float(np.sum(np.abs(mk["w"]) * mk["mu"] * w.eq.Bmag(R, Z)))

@@ -124,18 +124,20 @@ def test_all_markers_in_one_element_and_all_lost():
         assert np.array_equal(got[k], lost[k])                   # frozen bit for bit (G12)
 
 
-def test_full_size_bench_configuration_on_sampled_markers():
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
+def test_full_size_bench_configuration_on_sampled_markers(mode):
     """BASELINE.json configs[3] at full size (2^24 markers, 256 x 256 mesh) in the launch configuration bench.py times
-    (sort_interval = 1, timing build): 3 steps, then every 8192-th marker against the oracle (markers are independent,
-    PAPER.md:229, so the oracle can compute the sample alone); ids are a permutation and mu is untouched."""
+    (sort_interval = 1, timing build; `--mode` 0 = the headline, 1 non-linear, 2 FLR through the ordered ring stream,
+    3 non-linear + FLR): 3 steps, then every 8192-th marker against the oracle (markers are independent, so
+    the oracle can compute the sample alone); ids are a permutation and mu is untouched."""
     w = synth.make_config(3)
     assert w.n_markers == 1 << 24 and w.n_elems == 131072
     nsteps = 3
     idx = np.arange(0, w.n_markers, 8192)
     sample = take(w.markers, idx)
-    mesh, sp = oracle_of(w)
+    mesh, sp = oracle_of(w, mode=mode)
     ref, e_ref, _ = oracle_push(mesh, sp, sample, nsteps, w.dt)
-    p = make_pusher(w, verify=False, sort_interval=1)
+    p = make_pusher(w, verify=False, sort_interval=1, mode=mode)
     p.push(nsteps, w.dt)
     got, elem, ids = p.state()
     assert np.array_equal(np.bincount(ids, minlength=w.n_markers), np.ones(w.n_markers, dtype=np.int64))
