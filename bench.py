@@ -484,7 +484,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-order", choices=("shell", "element", "loaded"), default="shell",
                     help="order of the host buffers of the e2e leg: radial shells, the element order a one-chunk call returns, as loaded")
-    ap.add_argument("--e2e-chunks", type=int, default=4, help="marker chunks of the pipelined host-buffer call (e2e leg)")
+    ap.add_argument("--e2e-chunks", type=int, default=8, help="marker chunks of the pipelined host-buffer call (e2e leg)")
     ap.add_argument("--push-variant", type=int, default=0, choices=[0, 1],
                     help="m3dk_set_push_variant: 0 = default kernel, 1 = asynchronously staged kernel (A/B comparison)")
     ap.add_argument("--traffic-from", default=None,

@@ -190,9 +190,14 @@ int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, double *hz, d
  * entry).  host_id / host_elem may be NULL.  Pinned buffers are needed for the copies to overlap.  Every chunk steps from
  * the same time; t advances by nsteps * dt once.  The call needs the device arrays of m3dk_particles_init (n markers) and,
  * for sort_interval >= 1, the sort workspace; it synchronises before returning.  n_chunks = 1 is the unpipelined path.
- * Chunks of a marker stream in random order see a mesh n_chunks times sparser per chunk (fewer markers per element, less
- * sharing of coefficient tiles); buffers that come back from an earlier call are in element order, and their chunks are
- * spatially compact.                                                                                                   */
+ * Two chunks are in flight at a time on two compute streams (the context's and one of the library's own), each with a
+ * chunk-sized carving of the sort (and FLR) workspace, when two carvings fit the registered workspace (they do for
+ * n_chunks >= 2 and the sizes m3dk_sort_workspace_bytes / m3dk_flr_workspace_bytes return for n markers); work enqueued on
+ * the context's stream afterwards is ordered behind both.
+ * A chunk is a range of the buffers and stays that set of markers from call to call.  Chunks of a marker stream in random
+ * order see a mesh n_chunks times sparser per chunk (fewer markers per element, less sharing of coefficient tiles), and a
+ * chunk that starts as a range of elements disperses around its flux surfaces within some twenty steps; markers kept in
+ * the order of their flux surface (radial shells) keep their chunks compact.                                            */
 int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz, double *hvx, double *hvy, double *hvz, double *hmu,
                    double *hw, int *host_id, int *host_elem, int nsteps, double dt, int n_chunks);
 

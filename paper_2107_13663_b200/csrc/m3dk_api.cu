@@ -82,6 +82,7 @@ extern "C" int m3dk_destroy(m3dk_ctx *ctx) {
     for (cudaEvent_t e : ctx->ev_chunk) cudaEventDestroy(e);
     if (ctx->s_up) cudaStreamDestroy(ctx->s_up);
     if (ctx->s_down) cudaStreamDestroy(ctx->s_down);
+    for (cudaStream_t st : ctx->s_c) if (st) cudaStreamDestroy(st);
     delete ctx;
     return M3DK_OK;
 }
@@ -686,27 +687,52 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
     const double tb0 = ctx->t_base, ldt0 = ctx->last_dt;
     double *const hs[8] = {hx, hy, hz, hvx, hvy, hvz, hmu, hw};
     double *const dd[8] = {all.x, all.y, all.z, all.vx, all.vy, all.vz, all.mu, all.w};
-    int rc = M3DK_OK;
     const long per = (n + n_chunks - 1) / n_chunks;
-    for (int c = 0; c < n_chunks && rc == M3DK_OK; ++c) {
+    // Up to host_slots chunks are in flight at a time, each on its own compute stream with its own ordering workspace
+    // (chunk-sized carvings of the caller's workspace): the launch gaps, the small ordering kernels and the tail of the
+    // persistent push kernels of one chunk are filled by the other.
+    const size_t sort_slot = ctx->have_sortws ? sort_workspace_bytes(per, ctx->f.n_elems) : 0;
+    const size_t flr_slot = ctx->have_flrws ? flr_workspace_bytes(per, ctx->f.n_elems) : 0;
+    int slots = std::min(n_chunks, ctx->host_slots);
+    while (slots > 1 && ((ctx->have_sortws && slots * sort_slot > ctx->sortws_bytes) ||
+                         (ctx->have_flrws && slots * flr_slot > ctx->flrws_bytes)))
+        --slots;
+    cudaStream_t const main_stream = ctx->stream;
+    for (int k = 1; k < slots; ++k) {
+        if (!ctx->s_c[k]) CU(cudaStreamCreateWithFlags(&ctx->s_c[k], cudaStreamNonBlocking), "create compute stream");
+        CU(cudaStreamWaitEvent(ctx->s_c[k], ev_start, 0), "compute stream wait");
+    }
+    // whatever happens below, the context leaves this call bound to all markers, its own stream and the whole workspace
+    struct Restore {
+        m3dk_ctx *c; long n; MarkerArrays all; cudaStream_t st;
+        ~Restore() {
+            c->n = n; c->user = all; c->stream = st;
+            if (c->have_sortws) { carve_sort_workspace(c->sortws_base, n, c->f.n_elems, &c->sb); c->sb.bytes = c->sortws_bytes; }
+            if (c->have_flrws) carve_flr_workspace(c->flrws_base, n, c->f.n_elems, &c->fb);
+        }
+    } restore{ctx, n, all, main_stream};
+    for (int c = 0; c < n_chunks; ++c) {
         const long o = (long)c * per, nc = std::min(per, n - o);
         if (nc <= 0) break;
+        const int slot = c % slots;
         const size_t nb = (size_t)nc * sizeof(double);
         for (int k = 0; k < 8; ++k)
             CU(cudaMemcpyAsync(dd[k] + o, hs[k] + o, nb, cudaMemcpyHostToDevice, ctx->s_up), "upload chunk");
         CU(cudaEventRecord(ctx->ev_chunk[2 * c], ctx->s_up), "record upload");
+        ctx->stream = slot ? ctx->s_c[slot] : main_stream;
         CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_chunk[2 * c], 0), "compute waits for upload");
         // bind the chunk: same time and step counter for every chunk
         ctx->n = nc;
         ctx->user = MarkerArrays{all.x + o, all.y + o, all.z + o, all.vx + o, all.vy + o, all.vz + o, all.mu + o, all.w + o,
                                  all.elem + o, all.id + o};
-        if (ctx->have_sortws) carve_sort_workspace(ctx->sortws_base, nc, ctx->f.n_elems, &ctx->sb);
-        if (ctx->have_flrws) carve_flr_workspace(ctx->flrws_base, nc, ctx->f.n_elems, &ctx->fb);
+        if (ctx->have_sortws)
+            carve_sort_workspace(static_cast<char *>(ctx->sortws_base) + slot * sort_slot, nc, ctx->f.n_elems, &ctx->sb);
+        if (ctx->have_flrws)
+            carve_flr_workspace(static_cast<char *>(ctx->flrws_base) + slot * flr_slot, nc, ctx->f.n_elems, &ctx->fb);
         ctx->steps_done = steps0; ctx->steps_at_dt = at0; ctx->t_base = tb0; ctx->last_dt = ldt0;
-        cudaError_t e = launch_locate(ctx, ctx->user, nc, true, (int)o);
-        if (e != cudaSuccess) { rc = cuda_fail(ctx, e, "locate kernel"); break; }
-        rc = run_steps(ctx, nsteps, dt);
-        if (rc != M3DK_OK) break;
+        CU(launch_locate(ctx, ctx->user, nc, true, (int)o), "locate kernel");
+        const int rc = run_steps(ctx, nsteps, dt);
+        if (rc != M3DK_OK) return rc;
         CU(cudaEventRecord(ctx->ev_chunk[2 * c + 1], ctx->stream), "record compute");
         CU(cudaStreamWaitEvent(ctx->s_down, ctx->ev_chunk[2 * c + 1], 0), "download waits for compute");
         for (int k = 0; k < 8; ++k)                     // mu included: it travels with its marker through the sorts
@@ -714,12 +740,11 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
         if (host_id) CU(cudaMemcpyAsync(host_id + o, all.id + o, (size_t)nc * sizeof(int), cudaMemcpyDeviceToHost, ctx->s_down), "download id");
         if (host_elem) CU(cudaMemcpyAsync(host_elem + o, all.elem + o, (size_t)nc * sizeof(int), cudaMemcpyDeviceToHost, ctx->s_down), "download elem");
     }
-    // restore the full binding
-    ctx->n = n; ctx->user = all;
-    if (ctx->have_sortws) carve_sort_workspace(ctx->sortws_base, n, ctx->f.n_elems, &ctx->sb);
-    if (ctx->have_flrws) carve_flr_workspace(ctx->flrws_base, n, ctx->f.n_elems, &ctx->fb);
-    ctx->sb.bytes = ctx->sortws_bytes;
-    if (rc != M3DK_OK) return rc;
+    ctx->stream = main_stream;
+    for (int k = 1; k < slots; ++k) {      // work enqueued on the context's stream after this call sees every stream finished
+        CU(cudaEventRecord(ev_start, ctx->s_c[k]), "record compute stream");
+        CU(cudaStreamWaitEvent(main_stream, ev_start, 0), "join compute stream");
+    }
     CU(cudaStreamSynchronize(ctx->s_down), "download stream synchronize (an earlier kernel may have failed)");
     CU(cudaStreamSynchronize(ctx->stream), "stream synchronize");
     return M3DK_OK;

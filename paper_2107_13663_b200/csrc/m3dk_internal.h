@@ -193,6 +193,8 @@ struct m3dk_ctx {
     size_t sortws_bytes = 0;
     // m3dk_push_host: copy streams and per-chunk events (created on first use)
     cudaStream_t s_up = nullptr, s_down = nullptr;
+    cudaStream_t s_c[4] = {nullptr, nullptr, nullptr, nullptr};   // extra compute streams of the chunk pipeline (s_c[0] unused)
+    int host_slots = 2;                                            // chunks in flight (measured: 2 and 4 within 1 %)
     std::vector<cudaEvent_t> ev_chunk;
     // profiling (m3dk_set_profiling / m3dk_timing)
     bool profiling = false;

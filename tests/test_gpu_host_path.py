@@ -124,3 +124,31 @@ def test_fields_attach_binds_a_copy_of_the_workspace():
     garbage = torch.zeros(4096, dtype=torch.uint8, device="cuda")
     with pytest.raises(m3dk.M3DKError):
         m3dk.Pusher(device=0, verify=False).fields_attach(garbage, 1, 0)
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_push_host_two_chunks_in_flight_in_the_other_modes(mode):
+    """The chunk pipeline keeps two chunks in flight on two compute streams, each with its own carving of the sort and
+    FLR workspaces: non-linear mode and the FLR ring stream (mode 2) against the oracle, 5 chunks (odd: the slots alternate
+    unevenly), and bitwise against the one-chunk call."""
+    w = synth.make_config(3, n_markers=7000 + 13, nx=48)
+    mesh, sp = oracle_of(w, mode=mode)
+    nsteps = 4
+    ref, e_ref, _ = oracle_push(mesh, sp, w.markers, nsteps, w.dt)
+    out = {}
+    for chunks in (1, 5):
+        p = make_pusher(w, verify=True, sort_interval=1, mode=mode)
+        host = _pinned(w.markers)
+        ids = torch.empty(w.n_markers, dtype=torch.int32).pin_memory()
+        p.push_host(host, nsteps, w.dt, n_chunks=chunks, host_id=ids)
+        assert np.array_equal(np.sort(ids.numpy()), np.arange(w.n_markers))
+        r = {k: np.empty(w.n_markers) for k in KEYS}
+        for k in KEYS:
+            r[k][ids.numpy()] = host[k].numpy()
+        out[chunks] = r
+    live = e_ref >= 0
+    wrms = np.sqrt(np.mean(ref["w"][live] ** 2))
+    ex, ev, ew = g16_errors(take(out[5], live), take(ref, live), w_floor=wrms)
+    assert max(ex.max(), ev.max(), ew.max()) <= nsteps * TOL_STEP, (ex.max(), ev.max(), ew.max())
+    for k in KEYS:
+        assert np.array_equal(out[5][k], out[1][k]), k
