@@ -256,6 +256,25 @@ int m3dk_deposit_bytes(const m3dk_ctx *ctx, size_t *bytes);
 #define M3DK_DEPOSIT_BSTAR 4
 int m3dk_deposit(m3dk_ctx *ctx, double *rhs, int flags, double t);
 
+/* m3dk_deposit for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc) and therefore have no sort workspace to lend: the same right-hand sides of
+ * Eqs. (17)-(18), same arguments, same flags, through the element-ordered path (markers ordered by the element of their
+ * current position, a warp reduces up to 64 markers of one element per table update; with M3DK_DEPOSIT_FLR every lane
+ * loops over the elements of its ring points on the ordered records), with the ordering scratch in ONE static device
+ * array of M3DK_NOALLOC_SCRATCH_BYTES inside the library.  Every GPU that loads the library holds that array until the
+ * process exits.  The call allocates nothing (no cudaMalloc, cudaFree or allocating library routine): it enqueues memsets
+ * and kernels on the context's stream; the first call on a device also asks the runtime for the array's device address
+ * (make that call before starting a graph capture).  Whatever sort / FLR workspace the context has registered is neither
+ * used nor touched.  Limit: m3dk_sort_workspace_bytes(n_markers, n_elems) must not exceed M3DK_NOALLOC_SCRATCH_BYTES
+ * (about 48 000 markers on 8 192 elements); beyond it the call fails with M3DK_EWORKSPACE and enqueues nothing.
+ * The array is shared by every context of the process on that device and keeps the last call's contents; what must start
+ * at zero is cleared inside each call.  Calls that overlap on the GPU (two contexts on different streams, or a second call
+ * enqueued on another stream before the first has finished) race on it: serialise them on one stream or with events.
+ * Asynchronous like m3dk_deposit.  m3dk_noalloc_scratch_bytes returns the size of the array.                            */
+#define M3DK_NOALLOC_SCRATCH_BYTES (8u << 20)
+int m3dk_noalloc_scratch_bytes(size_t *bytes);
+int m3dk_deposit_noalloc(m3dk_ctx *ctx, double *rhs, int flags, double t);
+
 /* Measured FP64 FMA throughput of the device (register-resident DFMA chains, all SMs), in TFLOP/s (FMA = 2 flop).
  * Synchronous.  Used as the measured denominator of the FP64 roofline.                                                */
 int m3dk_fp64_peak_tflops(m3dk_ctx *ctx, double *tflops);

@@ -87,6 +87,8 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_gc_bootstrap": ([vp, dbl, vp], i),
         "m3dk_deposit_bytes": ([vp, C.POINTER(sz)], i),
         "m3dk_deposit": ([vp, vp, i, dbl], i),
+        "m3dk_noalloc_scratch_bytes": ([C.POINTER(sz)], i),
+        "m3dk_deposit_noalloc": ([vp, vp, i, dbl], i),
         "m3dk_fp64_peak_tflops": ([vp, _c_dp], i),
         "m3dk_set_profiling": ([vp, i], i),
         "m3dk_timing": ([vp, C.POINTER(_Timing)], i),
@@ -385,6 +387,16 @@ class Pusher:
         self.stats()
         self._keep["rhs"] = rhs
         return rhs.cpu().numpy().reshape(self.n_elems, 2, 1 + 2 * self.n_modes, 21)
+
+    def noalloc_scratch_bytes(self) -> int:
+        need = C.c_size_t()
+        self._ck(self.L.m3dk_noalloc_scratch_bytes(C.byref(need)))
+        return int(need.value)
+
+    def deposit_noalloc_into(self, rhs, flags: int = 0, t: float = 0.0):
+        """m3dk_deposit_noalloc into a caller's device tensor of deposit_bytes() bytes (asynchronous): the ordered
+        deposition with its scratch in the library's static device array; raises M3DKError beyond its size limit."""
+        self._ck(self.L.m3dk_deposit_noalloc(self.h, self._p(rhs), int(flags), float(t)))
 
     def fp64_peak_tflops(self) -> float:
         v = C.c_double()

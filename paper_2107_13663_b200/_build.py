@@ -13,7 +13,7 @@ import sys
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
-SOURCES = ["m3dk_api.cu", "m3dk_push.cu", "m3dk_sort.cu", "m3dk_deposit.cu", "m3dk_gc.cu"]
+SOURCES = ["m3dk_api.cu", "m3dk_push.cu", "m3dk_sort.cu", "m3dk_deposit.cu", "m3dk_gc.cu", "m3dk_noalloc.cu"]
 HEADERS = ["m3dk_internal.h", "m3dk_device.cuh", os.path.join("..", "..", "include", "m3dk.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
