@@ -687,7 +687,25 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
     const double tb0 = ctx->t_base, ldt0 = ctx->last_dt;
     double *const hs[8] = {hx, hy, hz, hvx, hvy, hvz, hmu, hw};
     double *const dd[8] = {all.x, all.y, all.z, all.vx, all.vy, all.vz, all.mu, all.w};
-    const long per = (n + n_chunks - 1) / n_chunks;
+    // Chunk boundaries: with four chunks or more the sizes ramp up and down again (weights 1, 2, .., 2, 1 capped at 4), so
+    // that the first upload and the last download, which nothing overlaps, are short; fewer chunks are equal.
+    std::vector<long> cut(n_chunks + 1, 0);
+    {
+        std::vector<long> wgt(n_chunks, 1);
+        long tot = 0;
+        for (int c = 0; c < n_chunks; ++c) {
+            if (n_chunks >= 4) wgt[c] = std::min<long>(4, 1 + std::min(c, n_chunks - 1 - c));
+            tot += wgt[c];
+        }
+        long acc = 0;
+        for (int c = 0; c < n_chunks; ++c) {
+            acc += wgt[c];
+            cut[c + 1] = std::max(cut[c], std::min(n, (n * acc + tot - 1) / tot));
+        }
+        cut[n_chunks] = n;
+    }
+    long per = 0;                                   // the largest chunk: what a slot of the workspaces must hold
+    for (int c = 0; c < n_chunks; ++c) per = std::max(per, cut[c + 1] - cut[c]);
     // Up to host_slots chunks are in flight at a time, each on its own compute stream with its own ordering workspace
     // (chunk-sized carvings of the caller's workspace): the launch gaps, the small ordering kernels and the tail of the
     // persistent push kernels of one chunk are filled by the other.
@@ -712,8 +730,8 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
         }
     } restore{ctx, n, all, main_stream};
     for (int c = 0; c < n_chunks; ++c) {
-        const long o = (long)c * per, nc = std::min(per, n - o);
-        if (nc <= 0) break;
+        const long o = cut[c], nc = cut[c + 1] - o;
+        if (nc <= 0) continue;
         const int slot = c % slots;
         const size_t nb = (size_t)nc * sizeof(double);
         for (int k = 0; k < 8; ++k)

@@ -75,6 +75,52 @@ __device__ __forceinline__ void dep_marker(const FieldParams &f, const DepOpts &
     for (int q = 1; q < 6; ++q) { d.xp[q] = __dmul_rn(d.xp[q - 1], xi1[0]); d.ep[q] = __dmul_rn(d.ep[q - 1], eta1[0]); }
 }
 
+
+// Sums over the warp of N values per lane by a transposing butterfly: every exchange halves the number of values a lane
+// holds (N/2 + N/4 + .. + 1 shuffles, then one per remaining lane bit), instead of five shuffles per value.  On return
+// lane L holds the total of value (L >> log2(32 / N)) & (N - 1); lanes that share those bits hold the same total.
+template <int N>
+__device__ __forceinline__ double warp_sum_columns(double (&v)[N], int lane) {
+    static_assert(N == 8 || N == 16 || N == 32, "N values per lane, a power of two");
+    int s = 16;
+#pragma unroll
+    for (int cnt = N; cnt > 1; cnt >>= 1, s >>= 1) {
+        const bool up = (lane & s) != 0;
+#pragma unroll
+        for (int i = 0; i < cnt / 2; ++i) {
+            const double send = up ? v[i] : v[i + cnt / 2];
+            const double keep = up ? v[i + cnt / 2] : v[i];
+            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, s);
+        }
+    }
+    double t = v[0];
+#pragma unroll
+    for (; s > 0; s >>= 1) t += __shfl_xor_sync(0xffffffffu, t, s);
+    return t;
+}
+
+// One row (moment, harmonic) of an item's table update: the 21 entries k = (i, j) of o[] each receive the sum over the
+// warp's markers of val(i, j).  Entries 0..15 and 16..20 (padded to 8) are reduced by warp_sum_columns (16 + 9 shuffles of
+// a double for the row against 105 for a butterfly per entry); the totals end up one per lane, so the table is updated by
+// two atomic instructions per row (16 and 5 active lanes).
+template <class F>
+__device__ __forceinline__ void dep_row_add(double *__restrict__ o, int lane, F val) {
+    double va[16], vb[8];
+    int k = 0;
+#pragma unroll
+    for (int j = 0; j < 6; ++j)
+#pragma unroll
+        for (int ii = 0; ii < 6 - j; ++ii, ++k) {
+            const double x = val(ii, j);
+            if (k < 16) va[k] = x; else vb[k - 16] = x;
+        }
+    vb[5] = 0.0; vb[6] = 0.0; vb[7] = 0.0;
+    const double ta = warp_sum_columns<16>(va, lane);       // lane L: entry L >> 1
+    const double tb = warp_sum_columns<8>(vb, lane);        // lane L: entry 16 + (L >> 2)
+    if ((lane & 1) == 0) atomicAdd(o + (lane >> 1), ta);
+    if ((lane & 3) == 0 && (lane >> 2) < 5) atomicAdd(o + 16 + (lane >> 2), tb);
+}
+
 // any marker order: one marker per lane, the warp loops over its distinct elements
 template <int kF>
 __global__ void __launch_bounds__(128) deposit_kernel(const __grid_constant__ FieldParams f, const __grid_constant__ DepOpts o,
@@ -260,19 +306,12 @@ __global__ void __launch_bounds__(128) deposit_items_kernel(const __grid_constan
             double ah[kItemR];
 #pragma unroll
             for (int r = 0; r < kItemR; ++r) ah[r] = __dmul_rn(d[r].amp[mom], d[r].T[h]);
-            double *o = out + ((size_t)mom * H + h) * M3DK_NCOEF;
-            int k = 0;
+            dep_row_add(out + ((size_t)mom * H + h) * M3DK_NCOEF, lane, [&](int ii, int j) {
+                double val = 0.0;
 #pragma unroll
-            for (int j = 0; j < 6; ++j)
-#pragma unroll
-                for (int ii = 0; ii < 6 - j; ++ii, ++k) {
-                    double val = 0.0;
-#pragma unroll
-                    for (int r = 0; r < kItemR; ++r) val = M3DK_FMA(ah[r], __dmul_rn(d[r].xp[ii], d[r].ep[j]), val);
-#pragma unroll
-                    for (int sft = 16; sft > 0; sft >>= 1) val += __shfl_xor_sync(0xffffffffu, val, sft);
-                    if (lane == 0) atomicAdd(o + k, val);
-                }
+                for (int r = 0; r < kItemR; ++r) val = M3DK_FMA(ah[r], __dmul_rn(d[r].xp[ii], d[r].ep[j]), val);
+                return val;
+            });
         }
 }
 
@@ -384,19 +423,12 @@ __global__ void __launch_bounds__(128) deposit_ring_items_kernel(const __grid_co
             double ah[kR];
 #pragma unroll
             for (int r = 0; r < kR; ++r) ah[r] = __dmul_rn(amp[r][mom], T[r][h]);
-            double *o = out + ((size_t)mom * H + h) * M3DK_NCOEF;
-            int k = 0;
+            dep_row_add(out + ((size_t)mom * H + h) * M3DK_NCOEF, lane, [&](int ii, int j) {
+                double val = 0.0;
 #pragma unroll
-            for (int j = 0; j < 6; ++j)
-#pragma unroll
-                for (int ii = 0; ii < 6 - j; ++ii, ++k) {
-                    double val = 0.0;
-#pragma unroll
-                    for (int r = 0; r < kR; ++r) val = M3DK_FMA(ah[r], __dmul_rn(xp[r][ii], ep[r][j]), val);
-#pragma unroll
-                    for (int sft = 16; sft > 0; sft >>= 1) val += __shfl_xor_sync(0xffffffffu, val, sft);
-                    if (lane == 0) atomicAdd(o + k, val);
-                }
+                for (int r = 0; r < kR; ++r) val = M3DK_FMA(ah[r], __dmul_rn(xp[r][ii], ep[r][j]), val);
+                return val;
+            });
         }
 }
 

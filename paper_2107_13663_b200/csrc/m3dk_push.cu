@@ -722,6 +722,14 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
     int4 w1 = it1 < total ? __ldg(P.items + it1) : none;
     unsigned b = 0, phase = 0;
     if (w0.x < P.f.n_elems && lane == 0) tile_copy_issue(buf0, P.f.tiles + (size_t)w0.x * stride_d, tile_bytes, bar0);
+    // the ring points of an item are reached through the order list, and the weights through the point's owner: both
+    // indices are read one item ahead and what they point at is prefetched into L2 while the current item computes
+    int idx0[kR], idx1[kR];
+#pragma unroll
+    for (int r = 0; r < kR; ++r) {
+        idx0[r] = 32 * r + lane < w0.z ? P.fl.rorder[w0.y + 32 * r + lane] : 0;
+        idx1[r] = 32 * r + lane < w1.z ? P.fl.rorder[w1.y + 32 * r + lane] : 0;
+    }
     while (it < total) {
         const int e = w0.x, start = w0.y, count = w0.z;
         const int4 w2 = it2 < total ? __ldg(P.items + it2) : none;
@@ -734,10 +742,21 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
         bool on[kR];
         Marker sp[kR];
         FlrW cw[kR];
+        int idx2[kR];
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            if (32 * r + lane < w1.z) {
+                const double *wp = P.fl.wts + 10 * (size_t)(idx1[r] >> 2);
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(P.fl.ring + 4 * (size_t)idx1[r]));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(wp));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(wp + 9));
+            }
+            idx2[r] = 32 * r + lane < w2.z ? P.fl.rorder[w2.y + 32 * r + lane] : 0;
+        }
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
             on[r] = 32 * r + lane < count;
-            idx[r] = on[r] ? P.fl.rorder[start + 32 * r + lane] : 0;
+            idx[r] = on[r] ? idx0[r] : 0;
             double pad;
             if (on[r]) ldrec256(P.fl.ring + 4 * idx[r], sp[r].x, sp[r].y, sp[r].z, pad);
             else { sp[r].x = 1.0; sp[r].y = 0.0; sp[r].z = 0.0; }
@@ -770,6 +789,8 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
         b ^= 1;
         it = it1; it1 = it2; it2 = 3 * stride + __shfl_sync(0xffffffffu, ticket, 0);
         w0 = w1; w1 = w2;
+#pragma unroll
+        for (int r = 0; r < kR; ++r) { idx0[r] = idx1[r]; idx1[r] = idx2[r]; }
     }
 }
 
