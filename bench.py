@@ -264,8 +264,8 @@ def run_ours(args, rank, world, local_rank):
     p.particles_init(w.markers, w.charge, w.mass, w.f0)
     p.set_options(sort_interval=si, mode=args.mode, t0=0.0)
     p.set_push_variant(args.push_variant)
-    if args.mode == 2 and si > 0:
-        p.set_flr_workspace()           # ring stream of the ordered FLR mode
+    if args.mode in (2, 3) and si > 0:
+        p.set_flr_workspace(nonlinear=(args.mode == 3))           # ring stream of the ordered FLR modes
 
     def barrier():
         if world > 1:

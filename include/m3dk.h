@@ -138,7 +138,8 @@ int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, double *z, 
  *           major-radius direction made perpendicular to b0, e2 = b0 x e1; a ring point outside the mesh contributes 0.
  *       3 = modes 1 and 2 together ("use orbit-averaged fields in the above equations"): the marker moves in
  *           B0 + <B1>, E-dagger = <E1> - (mu/q) grad(|B|0 + <B1par>) with the 4-point gyro-averages of mode 2, and the weight
- *           equation uses the same averages and keeps (1 - w).  Every lane gathers its ring (no ring stream yet).
+ *           equation uses the same averages and keeps (1 - w).  Every lane gathers its ring, unless an FLR workspace of
+ *           m3dk_flr_workspace_bytes_nl bytes is set (ring stream, below).
  * t0: time of the next step's x_l.  Resets steps_done to 0.                                                          */
 int m3dk_set_options(m3dk_ctx *ctx, int sort_interval, int mode, double t0);
 
@@ -158,8 +159,13 @@ int m3dk_set_sort_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes);
  * (sort_interval >= 1) does not let every marker gather the coefficient tiles of its four ring points: the push emits the
  * 4 n ring points (position, element, the marker's weights), they are ordered by THEIR element like the markers, a warp
  * evaluates up to 64 ring points of one element with the tile staged in shared memory, and the four contributions are
- * summed back into w (290 bytes per marker).  Results are bit-identical with and without it.                          */
+ * summed back into w (290 bytes per marker).  Results are bit-identical with and without it.
+ * Mode 3 needs the averaged VECTORS back at the marker before the Boris step, so its ring stream takes two passes over the
+ * markers per step (ring points out; ten Cartesian field components per ring point back, 96 bytes each) and a workspace of
+ * m3dk_flr_workspace_bytes_nl bytes (674 bytes per marker); with the smaller workspace mode 3 keeps its per-lane gathers.
+ * m3dk_set_flr_workspace accepts either size (the larger serves both modes and the FLR deposition).                    */
 int m3dk_flr_workspace_bytes(long n_markers, int n_elems, size_t *bytes);
+int m3dk_flr_workspace_bytes_nl(long n_markers, int n_elems, size_t *bytes);
 int m3dk_set_flr_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes);
 
 /* nsteps slow-manifold Boris steps of size dt with field evaluation and weight update, Eqs. (5), (6), (8)-(13).

@@ -75,6 +75,7 @@ def lib(verify: bool = False) -> C.CDLL:
         "m3dk_sort_workspace_bytes": ([lng, i, C.POINTER(sz)], i),
         "m3dk_set_sort_workspace": ([vp, vp, sz], i),
         "m3dk_flr_workspace_bytes": ([lng, i, C.POINTER(sz)], i),
+        "m3dk_flr_workspace_bytes_nl": ([lng, i, C.POINTER(sz)], i),
         "m3dk_set_flr_workspace": ([vp, vp, sz], i),
         "m3dk_push": ([vp, i, dbl], i),
         "m3dk_sort": ([vp, vp, sz], i),
@@ -264,10 +265,12 @@ class Pusher:
         self._ck(self.L.m3dk_set_sort_workspace(self.h, self._p(ws), ws.numel()))
         self._keep["sort_ws"] = ws
 
-    def set_flr_workspace(self):
-        """Allocate and lend the FLR workspace (ring stream of the ordered mode 2)."""
+    def set_flr_workspace(self, nonlinear: bool = False):
+        """Allocate and lend the FLR workspace (ring stream of the ordered mode 2 and of the FLR deposition; nonlinear:
+        the larger one that also carries the ring stream of mode 3)."""
         need = C.c_size_t()
-        self._ck(self.L.m3dk_flr_workspace_bytes(self.n, self.n_elems, C.byref(need)))
+        fn = self.L.m3dk_flr_workspace_bytes_nl if nonlinear else self.L.m3dk_flr_workspace_bytes
+        self._ck(fn(self.n, self.n_elems, C.byref(need)))
         ws = self._empty(need.value)
         self._ck(self.L.m3dk_set_flr_workspace(self.h, self._p(ws), ws.numel()))
         self._keep["flr_ws"] = ws

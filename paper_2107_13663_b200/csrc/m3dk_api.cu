@@ -434,8 +434,10 @@ extern "C" int m3dk_particles_init(m3dk_ctx *ctx, long n, double *x, double *y, 
         ctx->have_sortws = true;
     }
     ctx->have_flrws = false;
+    ctx->flr_with_avg = false;
     if (ctx->flrws_base && flr_workspace_bytes(n, ctx->f.n_elems) <= ctx->flrws_bytes) {
-        carve_flr_workspace(ctx->flrws_base, n, ctx->f.n_elems, &ctx->fb);
+        ctx->flr_with_avg = flr_workspace_bytes(n, ctx->f.n_elems, true) <= ctx->flrws_bytes;
+        carve_flr_workspace(ctx->flrws_base, n, ctx->f.n_elems, &ctx->fb, ctx->flr_with_avg);
         ctx->have_flrws = true;
     }
     CU(launch_locate(ctx, ctx->user, n, true), "locate kernel");
@@ -489,12 +491,19 @@ extern "C" int m3dk_flr_workspace_bytes(long n_markers, int n_elems, size_t *byt
     return M3DK_OK;
 }
 
+extern "C" int m3dk_flr_workspace_bytes_nl(long n_markers, int n_elems, size_t *bytes) {
+    if (!bytes || n_markers < 0 || n_elems < 1) return M3DK_EINVAL;
+    *bytes = flr_workspace_bytes(n_markers, n_elems, true);
+    return M3DK_OK;
+}
+
 extern "C" int m3dk_set_flr_workspace(m3dk_ctx *ctx, void *dev_workspace, size_t bytes) {
     if (!ctx) return M3DK_EINVAL;
     if (!ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_set_flr_workspace: call m3dk_particles_init first");
     if (!dev_workspace || ((uintptr_t)dev_workspace & 255) || bytes < flr_workspace_bytes(ctx->n, ctx->f.n_elems))
         return fail(ctx, M3DK_EWORKSPACE, "m3dk_set_flr_workspace: workspace NULL, misaligned or smaller than m3dk_flr_workspace_bytes");
-    carve_flr_workspace(dev_workspace, ctx->n, ctx->f.n_elems, &ctx->fb);
+    ctx->flr_with_avg = bytes >= flr_workspace_bytes(ctx->n, ctx->f.n_elems, true);
+    carve_flr_workspace(dev_workspace, ctx->n, ctx->f.n_elems, &ctx->fb, ctx->flr_with_avg);
     ctx->flrws_base = dev_workspace; ctx->flrws_bytes = bytes;
     ctx->have_flrws = true;
     return M3DK_OK;
@@ -563,6 +572,14 @@ static int run_steps(m3dk_ctx *ctx, int nsteps, double dt) {
         const bool reorder_after = l + 1 < nsteps;
         {
             EvScope ev(ctx, &ctx->ev_push);
+            if (flr_nl_stream(ctx)) {
+                // mode 3: ring points of every marker, ordered by their element, fields at the points; the push proper then
+                // reads the four sets of field components of each marker
+                CU(launch_flr_emit_nl(ctx, ctx->n, dt, t), "ring emit kernel");
+                CU(launch_flr_ring_keys(ctx, ctx->n), "ring key kernel");
+                CU(launch_flr_ring_stage(ctx, ctx->n), "ring ordering kernels");
+                CU(launch_flr_ring_eval(ctx, ctx->n, dt, t, true), "ring evaluation kernel");
+            }
             CU(launch_push_rec(ctx, ctx->n, dt, t, reorder_after), "push kernel");
             if (ctx->mode == 2 && ctx->have_flrws && ctx->f.n_modes > 0) {
                 // the push has emitted the ring stream: order it by the ring points' elements, evaluate, sum back into w
@@ -710,7 +727,7 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
     // (chunk-sized carvings of the caller's workspace): the launch gaps, the small ordering kernels and the tail of the
     // persistent push kernels of one chunk are filled by the other.
     const size_t sort_slot = ctx->have_sortws ? sort_workspace_bytes(per, ctx->f.n_elems) : 0;
-    const size_t flr_slot = ctx->have_flrws ? flr_workspace_bytes(per, ctx->f.n_elems) : 0;
+    const size_t flr_slot = ctx->have_flrws ? flr_workspace_bytes(per, ctx->f.n_elems, ctx->flr_with_avg) : 0;
     int slots = std::min(n_chunks, ctx->host_slots);
     while (slots > 1 && ((ctx->have_sortws && slots * sort_slot > ctx->sortws_bytes) ||
                          (ctx->have_flrws && slots * flr_slot > ctx->flrws_bytes)))
@@ -726,7 +743,7 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
         ~Restore() {
             c->n = n; c->user = all; c->stream = st;
             if (c->have_sortws) { carve_sort_workspace(c->sortws_base, n, c->f.n_elems, &c->sb); c->sb.bytes = c->sortws_bytes; }
-            if (c->have_flrws) carve_flr_workspace(c->flrws_base, n, c->f.n_elems, &c->fb);
+            if (c->have_flrws) carve_flr_workspace(c->flrws_base, n, c->f.n_elems, &c->fb, c->flr_with_avg);
         }
     } restore{ctx, n, all, main_stream};
     for (int c = 0; c < n_chunks; ++c) {
@@ -746,7 +763,7 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
         if (ctx->have_sortws)
             carve_sort_workspace(static_cast<char *>(ctx->sortws_base) + slot * sort_slot, nc, ctx->f.n_elems, &ctx->sb);
         if (ctx->have_flrws)
-            carve_flr_workspace(static_cast<char *>(ctx->flrws_base) + slot * flr_slot, nc, ctx->f.n_elems, &ctx->fb);
+            carve_flr_workspace(static_cast<char *>(ctx->flrws_base) + slot * flr_slot, nc, ctx->f.n_elems, &ctx->fb, ctx->flr_with_avg);
         ctx->steps_done = steps0; ctx->steps_at_dt = at0; ctx->t_base = tb0; ctx->last_dt = ldt0;
         CU(launch_locate(ctx, ctx->user, nc, true, (int)o), "locate kernel");
         const int rc = run_steps(ctx, nsteps, dt);

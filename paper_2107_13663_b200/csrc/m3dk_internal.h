@@ -93,6 +93,7 @@ struct RecArrays {            // ordered pipeline, carved from the sort workspac
 };
 
 // Ring stream of the ordered FLR mode (mode 2 with an FLR workspace): four ring points per marker slot.
+constexpr int kAvgDoubles = 12;   // ten components + two of padding: three full 32-byte sectors per ring point
 struct FlrArrays {
     double *ring;            // [4 n][4] (x, y, z, -) of ring point 4 slot + j
     double *wts;             // [n][10] the marker's weights of the perturbed fields in dw/dt, Cartesian (FlrW)
@@ -100,6 +101,7 @@ struct FlrArrays {
     int *rkey, *rrank;       // [4 n] element of the ring point (n_elems = outside, -1 = the slot holds a lost marker), rank in it
     int *rorder;             // [4 n] ring points in element order
     int *rhist;              // [n_elems + 2]
+    double *avg;             // [4 n][kAvgDoubles] mode 3: Cartesian field components at every ring point (NULL: not carved)
 };
 
 struct PushParams {
@@ -185,6 +187,7 @@ struct m3dk_ctx {
     bool have_sortws = false;
     m3dk::SortBuffers sb{};
     bool have_flrws = false;
+    bool flr_with_avg = false;   // the FLR workspace also holds the averages array (mode 3 through the ring stream)
     m3dk::FlrBuffers fb{};
     void *flrws_base = nullptr;
     size_t flrws_bytes = 0;
@@ -222,10 +225,12 @@ cudaError_t fp64_probe(m3dk_ctx *c, double *tflops);
 
 cudaError_t launch_flr_ring_keys(m3dk_ctx *c, long n);    // element + rank of every ring point (push.cu)
 cudaError_t launch_flr_ring_stage(m3dk_ctx *c, long n);   // ring histogram -> offsets, ring items, ring order
-cudaError_t launch_flr_ring_eval(m3dk_ctx *c, long n, double dt, double t);   // ring_items_kernel (push.cu)
+cudaError_t launch_flr_ring_eval(m3dk_ctx *c, long n, double dt, double t, bool avg = false);   // ring_items_kernel (push.cu)
+cudaError_t launch_flr_emit_nl(m3dk_ctx *c, long n, double dt, double t);   // mode 3, first pass: ring points of every marker
+bool flr_nl_stream(const m3dk_ctx *c);   // mode 3 goes through the ring stream (FLR workspace with the averages array)
 cudaError_t launch_flr_reduce(m3dk_ctx *c, long n, double dt);   // w += dt * quarter sum of the contributions
-size_t flr_workspace_bytes(long n, int n_elems);
-void carve_flr_workspace(void *ws, long n, int n_elems, FlrBuffers *fb);
+size_t flr_workspace_bytes(long n, int n_elems, bool with_avg = false);   // with_avg: + the averages array of mode 3
+void carve_flr_workspace(void *ws, long n, int n_elems, FlrBuffers *fb, bool with_avg = false);
 size_t sort_workspace_bytes(long n, int n_elems);
 void carve_sort_workspace(void *ws, long n, int n_elems, SortBuffers *sb);
 

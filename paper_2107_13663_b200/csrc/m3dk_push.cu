@@ -384,6 +384,24 @@ __device__ __forceinline__ double flr_wdot(const PushParams &P, const EqOut &f, 
     return __dmul_rn(0.25, sum);
 }
 
+// The perturbed fields of a ring point (its own cylindrical frame, cos / sin of its phi = cj, sj) as ten Cartesian
+// components (E, B1, grad B1par, dB1par/dt), and the quarter sums of those rotated into the marker's frame (Eq. 14).
+__device__ __forceinline__ void flr_cart_fields(const PertF &pf, double cj, double sj, double (&c)[10]) {
+    c[0] = M3DK_FMA(pf.ER, cj, -__dmul_rn(pf.EP, sj)); c[1] = M3DK_FMA(pf.ER, sj, __dmul_rn(pf.EP, cj)); c[2] = pf.EZ;
+    c[3] = M3DK_FMA(pf.BR, cj, -__dmul_rn(pf.BP, sj)); c[4] = M3DK_FMA(pf.BR, sj, __dmul_rn(pf.BP, cj)); c[5] = pf.BZ;
+    c[6] = M3DK_FMA(pf.gR, cj, -__dmul_rn(pf.gP, sj)); c[7] = M3DK_FMA(pf.gR, sj, __dmul_rn(pf.gP, cj)); c[8] = pf.gZ;
+    c[9] = pf.dT;
+}
+__device__ __forceinline__ void flr_avg_finish(const double (&t)[10], double c, double sn, PertF &out) {
+    out.ER = __dmul_rn(0.25, M3DK_FMA(t[0], c, __dmul_rn(t[1], sn))); out.EP = __dmul_rn(0.25, M3DK_FMA(t[1], c, -__dmul_rn(t[0], sn)));
+    out.EZ = __dmul_rn(0.25, t[2]);
+    out.BR = __dmul_rn(0.25, M3DK_FMA(t[3], c, __dmul_rn(t[4], sn))); out.BP = __dmul_rn(0.25, M3DK_FMA(t[4], c, -__dmul_rn(t[3], sn)));
+    out.BZ = __dmul_rn(0.25, t[5]);
+    out.gR = __dmul_rn(0.25, M3DK_FMA(t[6], c, __dmul_rn(t[7], sn))); out.gP = __dmul_rn(0.25, M3DK_FMA(t[7], c, -__dmul_rn(t[6], sn)));
+    out.gZ = __dmul_rn(0.25, t[8]);
+    out.dT = __dmul_rn(0.25, t[9]);
+}
+
 // Gyro-averaged perturbed fields of one marker in its own cylindrical frame (mode 3: non-linear trajectories in the
 // averaged fields): quarter sum over the ring points of the vectors in Cartesian components (Eq. 14), each
 // point searched and evaluated on its own element's tile (global memory); a point outside the mesh contributes zero.
@@ -407,23 +425,33 @@ __device__ __forceinline__ void flr_avg_fields(const PushParams &P, const EqOut 
         PertF pf[1];
         pf[0].ER = pf[0].EP = pf[0].EZ = pf[0].BR = pf[0].BP = pf[0].BZ = pf[0].gR = pf[0].gP = pf[0].gZ = pf[0].dT = 0.0;
         pert_fields<1, false>(P, tile, xi, eta, gj, se, pf);
-        const double cj = gj[0].cph, sj = gj[0].sph;
-        Ex = __dadd_rn(Ex, M3DK_FMA(pf[0].ER, cj, -__dmul_rn(pf[0].EP, sj))); Ey = __dadd_rn(Ey, M3DK_FMA(pf[0].ER, sj, __dmul_rn(pf[0].EP, cj)));
-        Ez = __dadd_rn(Ez, pf[0].EZ);
-        Bx = __dadd_rn(Bx, M3DK_FMA(pf[0].BR, cj, -__dmul_rn(pf[0].BP, sj))); By = __dadd_rn(By, M3DK_FMA(pf[0].BR, sj, __dmul_rn(pf[0].BP, cj)));
-        Bz = __dadd_rn(Bz, pf[0].BZ);
-        Gx = __dadd_rn(Gx, M3DK_FMA(pf[0].gR, cj, -__dmul_rn(pf[0].gP, sj))); Gy = __dadd_rn(Gy, M3DK_FMA(pf[0].gR, sj, __dmul_rn(pf[0].gP, cj)));
-        Gz = __dadd_rn(Gz, pf[0].gZ);
-        dT = __dadd_rn(dT, pf[0].dT);
+        double c10[10];
+        flr_cart_fields(pf[0], gj[0].cph, gj[0].sph, c10);
+        Ex = __dadd_rn(Ex, c10[0]); Ey = __dadd_rn(Ey, c10[1]); Ez = __dadd_rn(Ez, c10[2]);
+        Bx = __dadd_rn(Bx, c10[3]); By = __dadd_rn(By, c10[4]); Bz = __dadd_rn(Bz, c10[5]);
+        Gx = __dadd_rn(Gx, c10[6]); Gy = __dadd_rn(Gy, c10[7]); Gz = __dadd_rn(Gz, c10[8]);
+        dT = __dadd_rn(dT, c10[9]);
     }
-    const double c = g.cph, sn = g.sph;
-    out.ER = __dmul_rn(0.25, M3DK_FMA(Ex, c, __dmul_rn(Ey, sn))); out.EP = __dmul_rn(0.25, M3DK_FMA(Ey, c, -__dmul_rn(Ex, sn)));
-    out.EZ = __dmul_rn(0.25, Ez);
-    out.BR = __dmul_rn(0.25, M3DK_FMA(Bx, c, __dmul_rn(By, sn))); out.BP = __dmul_rn(0.25, M3DK_FMA(By, c, -__dmul_rn(Bx, sn)));
-    out.BZ = __dmul_rn(0.25, Bz);
-    out.gR = __dmul_rn(0.25, M3DK_FMA(Gx, c, __dmul_rn(Gy, sn))); out.gP = __dmul_rn(0.25, M3DK_FMA(Gy, c, -__dmul_rn(Gx, sn)));
-    out.gZ = __dmul_rn(0.25, Gz);
-    out.dT = __dmul_rn(0.25, dT);
+    const double sum10[10] = {Ex, Ey, Ez, Bx, By, Bz, Gx, Gy, Gz, dT};
+    flr_avg_finish(sum10, g.cph, g.sph, out);
+}
+
+// Mode 3 through the ring stream: the same average from the ten Cartesian components that ring_items_kernel<.., true> has
+// stored for the four ring points of the marker in slot `slot` (zeros for a point outside the mesh), summed in the same
+// order as flr_avg_fields.
+__device__ __forceinline__ void flr_avg_from_stream(const PushParams &P, const StepGeom &g, long slot, PertF &out) {
+    double sum10[10];
+#pragma unroll
+    for (int k = 0; k < 10; ++k) sum10[k] = 0.0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const double *a = P.fl.avg + kAvgDoubles * (4 * slot + j);
+        double c[12];
+        ldrec256(a, c[0], c[1], c[2], c[3]); ldrec256(a + 4, c[4], c[5], c[6], c[7]); ldrec256(a + 8, c[8], c[9], c[10], c[11]);
+#pragma unroll
+        for (int k = 0; k < 10; ++k) sum10[k] = __dadd_rn(sum10[k], c[k]);
+    }
+    flr_avg_finish(sum10, g.cph, g.sph, out);
 }
 
 // kFlr = 2: emit the four ring points of the marker in output slot `slot` into the ring stream (positions, flagged live)
@@ -483,7 +511,9 @@ __global__ void __launch_bounds__(256) ring_key_kernel(const __grid_constant__ F
 // ---- the same step in the non-linear trajectory mode (mode 1: PAPER.md:108, :130; reading G21) ------------------------
 // All perturbed fields are needed BEFORE the velocity update (the marker moves in the total fields), so they are
 // accumulated per marker (10 values) and the folding trick of the linear mode does not apply; B1_phi (quad 3) enters.
-template <int R, bool kHist, bool kSmem, class IO, bool kPost = false, bool kFlr = false>
+// kFlr: 0 fields at the marker; 1 every lane gathers its four ring points (flr_avg_fields); 2 the averages come from the
+// ring stream (flr_avg_from_stream: ring points emitted by flr_emit_nl, evaluated by ring_items_kernel<.., true>)
+template <int R, bool kHist, bool kSmem, class IO, bool kPost = false, int kFlr = 0>
 __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, const double *__restrict__ tile,
                                           const long (&mi)[R], const long (&mo)[R], const bool (&on)[R], double (&Rn)[R],
                                           double (&Zn)[R]) {
@@ -515,7 +545,11 @@ __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, con
         f[r].F = v[r][2]; f[r].kappa = v[r][3];
         pf[r].ER = pf[r].EP = pf[r].EZ = pf[r].BR = pf[r].BP = pf[r].BZ = pf[r].gR = pf[r].gP = pf[r].gZ = pf[r].dT = 0.0;
     }
-    if constexpr (kFlr) {           // mode 3: the gyro-averaged perturbed fields replace the fields at the marker
+    if constexpr (kFlr == 2) {      // mode 3, ordered with a ring stream
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (on[r]) flr_avg_from_stream(P, g[r], mo[r], pf[r]);
+    } else if constexpr (kFlr == 1) {   // mode 3: the gyro-averaged perturbed fields replace the fields at the marker
 #pragma unroll
         for (int r = 0; r < R; ++r)
             if (P.f.n_modes > 0) flr_avg_fields(P, f[r], g[r], s[r].z, s[r].mu, pf[r]);
@@ -556,6 +590,49 @@ __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, con
     }
 }
 
+// Mode 3 through the ring stream, first pass: the equilibrium field at x_l and the four ring points of every marker of the
+// item into the ring stream (slot = the marker's OUTPUT slot, where the second pass, step_R_nl<.., 2>, reads the averages);
+// nothing else is written.
+template <int R, bool kSmem, class IO>
+__device__ __forceinline__ void flr_emit_nl(const PushParams &P, const IO &io, const double *__restrict__ tile,
+                                            const long (&mi)[R], const long (&mo)[R], const bool (&on)[R]) {
+    Marker s[R];
+    StepGeom g[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (on[r]) { io.load_pos(mi[r], s[r].x, s[r].y, s[r].z, s[r].w); io.load_vel(mi[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu); }
+        else { s[r].x = 1.0; s[r].y = 0.0; s[r].z = 0.0; s[r].w = 0.0; s[r].vx = s[r].vy = s[r].vz = 0.0; s[r].mu = 0.0; }
+    }
+    const Quad hd = ldq_t<kSmem>(tile);
+    const double Rc = hd.a, Zc = hd.b, se = hd.c;
+    double xi[R], eta[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        step_geometry(s[r], g[r]);
+        xi[r] = __dmul_rn(__dsub_rn(g[r].R, Rc), se); eta[r] = __dmul_rn(__dsub_rn(s[r].z, Zc), se);
+    }
+    double v[R][4], dx[R][4], de[R][4];
+    Ring ring;
+    ring_fill<kSmem>(ring, tile + kTileHeader);
+    quad_vd<R, kSmem>(tile + kTileHeader, tile + kTileHeader, ring, xi, eta, v, dx, de);   // (psi0, |B|0, F0, kappa)
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (!on[r]) continue;
+        EqOut f;
+        f.psi_R = __dmul_rn(dx[r][0], se); f.psi_Z = __dmul_rn(de[r][0], se);
+        f.Bm = v[r][1]; f.Bm_R = __dmul_rn(dx[r][1], se); f.Bm_Z = __dmul_rn(de[r][1], se);
+        f.F = v[r][2]; f.kappa = v[r][3];
+        FlrRing rg;
+        flr_ring(P, f, g[r], s[r].mu, rg);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            double x, y, z;
+            flr_ring_point(rg, s[r].z, j, x, y, z);
+            strec256(P.fl.ring + 4 * (4 * mo[r] + j), x, y, z, 1.0);
+        }
+    }
+}
+
 // ---- generic push: one marker per thread, any marker order (every thread gathers its own element's tile) ------------
 // The caller's SoA arrays in place: sort_interval = 0, i.e. no sort workspace.
 template <int kMode>
@@ -569,7 +646,7 @@ __global__ void __launch_bounds__(128) push_generic_kernel(const __grid_constant
     if (__any_sync(0xffffffffu, on[0])) {
         double Rn[1], Zn[1];
         const SoAIO io{P.a, P.f.n_elems};
-        if (kMode == 1 || kMode == 4) step_R_nl<1, false, false, SoAIO, false, kMode == 4>(P, io, tile, m, m, on, Rn, Zn);
+        if (kMode == 1 || kMode == 4) step_R_nl<1, false, false, SoAIO, false, kMode == 4 ? 1 : 0>(P, io, tile, m, m, on, Rn, Zn);
         else step_R<1, false, false, SoAIO, kMode == 2 ? 1 : 0>(P, io, tile, m, m, on, Rn, Zn);
     }
 }
@@ -599,6 +676,8 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
 // coefficient read is a broadcast LDS that feeds kItemR markers per lane.  Items are handed out by a ticket counter after
 // a warp's first three.  Items of the pseudo-element n_elems hold the lost markers: frozen, they only enter the histogram.
 // kR = 2: the items of up to 64 markers; kR = 1: the small items (a remainder of 1..32 markers of an element).
+// kMode: 0 linear, 1 non-linear, 2 FLR with per-lane ring gathers, 3 FLR emitting the ring stream, 4 non-linear + FLR with
+// per-lane gathers, 5 / 6 the two passes of non-linear + FLR through the ring stream (emit; step with the stream's averages).
 template <bool kHist, int kMode, int kR>
 __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 1 : M3DK_PUSH_MINBLOCKS) push_items_kernel(const __grid_constant__ PushParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -656,7 +735,12 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
 #pragma unroll
         for (int r = 0; r < kR; ++r) { mo[r] = (long)start + 32 * r + lane; on[r] = 32 * r + lane < count; mi[r] = src0[r]; }
         const RecIO io{P.rc.in, P.rc.out, P.rc.key, P.f.n_elems};
-        if (e >= P.f.n_elems) {                        // lost markers: frozen (G12), moved along and counted for the next sort
+        if (kMode == 5 && e >= P.f.n_elems) {          // emit pass of mode 3: the slots of lost markers carry no ring
+#pragma unroll
+            for (int r = 0; r < kR; ++r)
+                if (on[r])
+                    for (int j = 0; j < 4; ++j) strec256(P.fl.ring + 4 * (4 * mo[r] + j), 0.0, 0.0, 0.0, -1.0);
+        } else if (e >= P.f.n_elems) {                 // lost markers: frozen (G12), moved along and counted for the next sort
             int key[kR];
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
@@ -680,7 +764,9 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
             mbar_wait(bar0 + b * 8, (phase >> b) & 1u);
             phase ^= 1u << b;
             double Rn[kR], Zn[kR];
-            if (kMode == 1 || kMode == 4) step_R_nl<kR, kHist, true, RecIO, false, kMode == 4>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
+            if (kMode == 5) flr_emit_nl<kR, true, RecIO>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on);
+            else if (kMode == 1 || kMode == 4 || kMode == 6)
+                step_R_nl<kR, kHist, true, RecIO, false, kMode == 4 ? 1 : (kMode == 6 ? 2 : 0)>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
             else step_R<kR, kHist, true, RecIO, kMode == 2 ? 1 : (kMode == 3 ? 2 : 0)>(P, io, tbuf + (size_t)b * stride_d, mi, mo, on, Rn, Zn);
         }
         b ^= 1;
@@ -699,7 +785,9 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
 // ticket: the machinery of push_items_kernel).  A lane gathers its points (32 B) and the weights of the markers that own
 // them (80 B), evaluates all perturbed polynomials at the points (pert_fields with broadcast coefficient reads shared by
 // the lane's points) and stores the scalar contribution c_j of each point.
-template <int kR>
+// kAvg (mode 3): no weights; the ten Cartesian components of the fields at the point are stored (12 doubles per point: three
+// full sectors) for the second pass of the push, zeros for a point outside the mesh.
+template <int kR, bool kAvg>
 __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 1 : M3DK_PUSH_MINBLOCKS) ring_items_kernel(const __grid_constant__ PushParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int kWarps = kPushThreads / 32;
@@ -746,10 +834,12 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
             if (32 * r + lane < w1.z) {
-                const double *wp = P.fl.wts + 10 * (size_t)(idx1[r] >> 2);
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(P.fl.ring + 4 * (size_t)idx1[r]));
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(wp));
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(wp + 9));
+                if (!kAvg) {
+                    const double *wp = P.fl.wts + 10 * (size_t)(idx1[r] >> 2);
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(wp));
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(wp + 9));
+                }
             }
             idx2[r] = 32 * r + lane < w2.z ? P.fl.rorder[w2.y + 32 * r + lane] : 0;
         }
@@ -779,11 +869,27 @@ __global__ void __launch_bounds__(kPushThreads, kR == 1 ? M3DK_PUSH_MINBLOCKS + 
             pert_fields<kR, true>(P, tile, xi, eta, g, se, pf);
 #pragma unroll
             for (int r = 0; r < kR; ++r)
-                if (on[r]) {
+                if (kAvg) {
+                    if (on[r]) {
+                        double c10[10];
+                        flr_cart_fields(pf[r], g[r].cph, g[r].sph, c10);
+                        double *a = P.fl.avg + kAvgDoubles * idx[r];
+                        strec256(a, c10[0], c10[1], c10[2], c10[3]); strec256(a + 4, c10[4], c10[5], c10[6], c10[7]);
+                        strec256(a + 8, c10[8], c10[9], 0.0, 0.0);
+                    }
+                } else if (on[r]) {
                     const double *wt = P.fl.wts + 10 * (idx[r] >> 2);
                     cw[r].aEx = wt[0]; cw[r].aEy = wt[1]; cw[r].aEz = wt[2]; cw[r].bBx = wt[3]; cw[r].bBy = wt[4];
                     cw[r].bBz = wt[5]; cw[r].gGx = wt[6]; cw[r].gGy = wt[7]; cw[r].gGz = wt[8]; cw[r].dT = wt[9];
                     P.fl.contrib[idx[r]] = flr_fold(pf[r], g[r].cph, g[r].sph, cw[r]);
+                }
+        }
+        else if (kAvg) {                                // outside the mesh: the point contributes zero to every average
+#pragma unroll
+            for (int r = 0; r < kR; ++r)
+                if (on[r]) {
+                    double *a = P.fl.avg + kAvgDoubles * idx[r];
+                    strec256(a, 0.0, 0.0, 0.0, 0.0); strec256(a + 4, 0.0, 0.0, 0.0, 0.0); strec256(a + 8, 0.0, 0.0, 0.0, 0.0);
                 }
         }
         b ^= 1;
@@ -1117,6 +1223,37 @@ cudaError_t launch_push_soa(m3dk_ctx *c, long n, double dt, double t) {
     return cudaGetLastError();
 }
 
+// mode 3 runs through the ring stream when the FLR workspace holds the averages array
+bool flr_nl_stream(const m3dk_ctx *c) { return c->mode == 3 && c->have_flrws && c->flr_with_avg && c->f.n_modes > 0; }
+
+// Mode 3 through the ring stream, first pass over the current work items: the ring points of every marker into the stream
+// (push_items_kernel<false, 5, .>: nothing but the stream is written).  The item tickets are cleared again afterwards: the
+// second pass (launch_push_rec) walks the same item lists.
+cudaError_t launch_flr_emit_nl(m3dk_ctx *c, long n, double dt, double t) {
+    if (n == 0) return cudaSuccess;
+    PushParams P = make_params(c, c->user, n, dt, t);
+    P.rc.key = c->sb.key; P.rc.order = c->sb.order[c->ocur];
+    P.rc.in = c->sb.rec[c->cur]; P.rc.out = c->sb.rec[c->cur ^ 1];
+    P.fl = c->fb.a;
+    cudaError_t e = cudaMemsetAsync(c->fb.a.rhist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
+    if (e != cudaSuccess) return e;
+    const unsigned grid = (unsigned)(c->sm_count * M3DK_PUSH_MINBLOCKS);
+    const size_t smem = (size_t)(kPushThreads / 32) * 2 * (c->f.tile_stride * 8 + 8);
+    int *const tickets = reinterpret_cast<int *>(c->sb.scan_state + (c->f.n_elems + 1 + 4095) / 4096 + 2);
+    for (int small = 0; small < 2; ++small) {
+        P.items = small ? c->sb.items_small : c->sb.items;
+        P.n_items = small ? reinterpret_cast<const int *>(c->sb.scan_state + 1) : c->sb.ioffs + c->f.n_elems + 1;
+        P.ticket = tickets + small;
+        void (*kern)(PushParams) = small ? push_items_kernel<false, 5, 1> : push_items_kernel<false, 5, 2>;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        c->kernel_launches += 1;
+        kern<<<small ? grid / M3DK_PUSH_MINBLOCKS * (M3DK_PUSH_MINBLOCKS + 1) : grid, kPushThreads, smem, c->stream>>>(P);
+    }
+    e = cudaMemsetAsync(tickets, 0, 2 * sizeof(int), c->stream);
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
 // One element-ordered step on the records: sb.rec[cur] gathered through sb.order[ocur] into sb.rec[cur ^ 1], which becomes
 // current.  with_hist: also histogram the new keys for the reorder that follows.
 cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_hist) {
@@ -1132,11 +1269,13 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
         if (e != cudaSuccess) return e;
     }
     const bool flr_stream = c->mode == 2 && c->have_flrws && c->f.n_modes > 0;
+    const bool nl_stream = flr_nl_stream(c);     // mode 3: the averages are in the ring stream (launch_flr_emit_nl .. ring eval)
     if (flr_stream) {
         P.fl = c->fb.a;
         cudaError_t e = cudaMemsetAsync(c->fb.a.rhist, 0, (size_t)(c->f.n_elems + 1) * sizeof(int), c->stream);
         if (e != cudaSuccess) return e;
     }
+    if (nl_stream) P.fl = c->fb.a;
     {
         P.rc.out = c->sb.rec[c->cur ^ 1];
         P.items = c->sb.items; P.n_items = c->sb.ioffs + c->f.n_elems + 1;
@@ -1149,7 +1288,7 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
             P.ticket = reinterpret_cast<int *>(c->sb.scan_state + (c->f.n_elems + 1 + 4095) / 4096 + 2) + small;
             void (*kern)(PushParams);
             const size_t as_smem = async_smem_bytes(c->f.tile_stride, small ? 1 : 2);
-            if (c->push_variant == 1 && c->mode != 2 && as_smem <= c->smem_optin) {
+            if (c->push_variant == 1 && (c->mode == 0 || c->mode == 1) && as_smem <= c->smem_optin) {
                 if (small)
                     kern = c->mode == 1 ? (with_hist ? push_async_kernel<true, 1, 1> : push_async_kernel<false, 1, 1>)
                                         : (with_hist ? push_async_kernel<true, 0, 1> : push_async_kernel<false, 0, 1>);
@@ -1168,18 +1307,20 @@ cudaError_t launch_push_rec(m3dk_ctx *c, long n, double dt, double t, bool with_
                 continue;
             }
             // mode 2: with an FLR workspace the push emits the ring stream (kernel mode 3), else every lane gathers its ring
-            const int km = c->mode == 2 ? (flr_stream ? 3 : (c->f.n_modes > 0 ? 2 : 0)) : c->mode == 3 ? 4 : c->mode;
+            const int km = c->mode == 2 ? (flr_stream ? 3 : (c->f.n_modes > 0 ? 2 : 0)) : c->mode == 3 ? (nl_stream ? 6 : 4) : c->mode;
             if (small)
                 kern = km == 1   ? (with_hist ? push_items_kernel<true, 1, 1> : push_items_kernel<false, 1, 1>)
                        : km == 2 ? (with_hist ? push_items_kernel<true, 2, 1> : push_items_kernel<false, 2, 1>)
                        : km == 3 ? (with_hist ? push_items_kernel<true, 3, 1> : push_items_kernel<false, 3, 1>)
                        : km == 4 ? (with_hist ? push_items_kernel<true, 4, 1> : push_items_kernel<false, 4, 1>)
+                       : km == 6 ? (with_hist ? push_items_kernel<true, 6, 1> : push_items_kernel<false, 6, 1>)
                                  : (with_hist ? push_items_kernel<true, 0, 1> : push_items_kernel<false, 0, 1>);
             else
                 kern = km == 1   ? (with_hist ? push_items_kernel<true, 1, 2> : push_items_kernel<false, 1, 2>)
                        : km == 2 ? (with_hist ? push_items_kernel<true, 2, 2> : push_items_kernel<false, 2, 2>)
                        : km == 3 ? (with_hist ? push_items_kernel<true, 3, 2> : push_items_kernel<false, 3, 2>)
                        : km == 4 ? (with_hist ? push_items_kernel<true, 4, 2> : push_items_kernel<false, 4, 2>)
+                       : km == 6 ? (with_hist ? push_items_kernel<true, 6, 2> : push_items_kernel<false, 6, 2>)
                                  : (with_hist ? push_items_kernel<true, 0, 2> : push_items_kernel<false, 0, 2>);
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
@@ -1205,7 +1346,7 @@ cudaError_t launch_flr_ring_keys(m3dk_ctx *c, long n) {
 }
 
 // evaluation of the ordered ring stream (mode 2): the ring items of up to 64 points, then the small ones
-cudaError_t launch_flr_ring_eval(m3dk_ctx *c, long n, double dt, double t) {
+cudaError_t launch_flr_ring_eval(m3dk_ctx *c, long n, double dt, double t, bool avg) {
     if (n == 0) return cudaSuccess;
     PushParams P = make_params(c, c->user, n, dt, t);
     P.fl = c->fb.a;
@@ -1215,7 +1356,8 @@ cudaError_t launch_flr_ring_eval(m3dk_ctx *c, long n, double dt, double t) {
         P.items = small ? c->fb.ritems_small : c->fb.ritems;
         P.n_items = small ? reinterpret_cast<const int *>(c->fb.rstate + 1) : c->fb.rioffs + c->f.n_elems + 1;
         P.ticket = reinterpret_cast<int *>(c->fb.rstate + (c->f.n_elems + 1 + 4095) / 4096 + 2) + small;
-        void (*kern)(PushParams) = small ? ring_items_kernel<1> : ring_items_kernel<2>;
+        void (*kern)(PushParams) = avg ? (small ? ring_items_kernel<1, true> : ring_items_kernel<2, true>)
+                                       : (small ? ring_items_kernel<1, false> : ring_items_kernel<2, false>);
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         c->kernel_launches += 1;

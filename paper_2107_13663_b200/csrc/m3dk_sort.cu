@@ -235,15 +235,16 @@ static cudaError_t scan_and_cut(m3dk_ctx *c) {
 }
 
 // ---- ring stream of the ordered FLR mode ----------------------------------------------------------------------------------
-size_t flr_workspace_bytes(long n, int n_elems) {
+size_t flr_workspace_bytes(long n, int n_elems, bool with_avg) {
     const size_t n4 = 4 * (size_t)n;
     const size_t nh = up256((size_t)(n_elems + 2) * sizeof(int));
     return up256(n4 * 4 * sizeof(double)) + up256((size_t)n * 10 * sizeof(double)) + up256(n4 * sizeof(double)) +
            3 * up256(n4 * sizeof(int)) + 3 * nh + up256((n4 / kItemMarkers + n_elems + 2) * sizeof(int4)) +
-           up256((size_t)(n_elems + 2) * sizeof(int4)) + up256(((size_t)(n_elems + 1) / 4096 + 6) * sizeof(unsigned long long));
+           up256((size_t)(n_elems + 2) * sizeof(int4)) + up256(((size_t)(n_elems + 1) / 4096 + 6) * sizeof(unsigned long long)) +
+           (with_avg ? up256(n4 * kAvgDoubles * sizeof(double)) : 0);
 }
 
-void carve_flr_workspace(void *ws, long n, int n_elems, FlrBuffers *fb) {
+void carve_flr_workspace(void *ws, long n, int n_elems, FlrBuffers *fb, bool with_avg) {
     char *p = static_cast<char *>(ws);
     const size_t n4 = 4 * (size_t)n;
     const size_t nh = up256((size_t)(n_elems + 2) * sizeof(int));
@@ -259,6 +260,8 @@ void carve_flr_workspace(void *ws, long n, int n_elems, FlrBuffers *fb) {
     fb->ritems = reinterpret_cast<int4 *>(p); p += up256((n4 / kItemMarkers + n_elems + 2) * sizeof(int4));
     fb->ritems_small = reinterpret_cast<int4 *>(p); p += up256((size_t)(n_elems + 2) * sizeof(int4));
     fb->rstate = reinterpret_cast<unsigned long long *>(p); p += up256(((size_t)(n_elems + 1) / 4096 + 6) * sizeof(unsigned long long));
+    fb->a.avg = nullptr;
+    if (with_avg) { fb->a.avg = reinterpret_cast<double *>(p); p += up256(n4 * kAvgDoubles * sizeof(double)); }
     fb->bytes = (size_t)(p - static_cast<char *>(ws));
 }
 

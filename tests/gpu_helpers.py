@@ -34,8 +34,8 @@ def make_pusher(w, verify=True, markers=None, sort_interval=0, t0=0.0, mode=0, f
                     w.pert_coef if w.n_modes else None)
     p.particles_init(w.markers if markers is None else markers, w.charge, w.mass, w.f0)
     p.set_options(sort_interval=sort_interval, mode=mode, t0=t0)
-    if mode == 2 and sort_interval > 0 and flr_ws:
-        p.set_flr_workspace()
+    if mode in (2, 3) and sort_interval > 0 and flr_ws:
+        p.set_flr_workspace(nonlinear=(mode == 3))
     return p
 
 

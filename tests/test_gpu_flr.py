@@ -1,5 +1,7 @@
 """GPU parity of the finite-Larmor-radius mode (m3dk_set_options mode = 2, Eq. 14,
 reading G23) against the oracle's mode 2 (pinned by tests/test_oracle_flr.py), through the C ABI."""
+import dataclasses
+
 import numpy as np
 import pytest
 
@@ -153,11 +155,40 @@ def test_nonlinear_mode_with_gyro_average(verify):
         assert max(ex.max(), ev.max(), ew.max()) <= TOL_STEP, (s, ex.max(), ev.max(), ew.max())
     lin, _, _ = oracle_push(*oracle_of(w, mode=1), w.markers, 6, w.dt)
     res = {}
-    for si in (0, 1):
-        q = make_pusher(w, verify=verify, sort_interval=si, mode=3)
+    # SoA kernel; ordered pipeline with per-lane ring gathers; ordered pipeline through the ring stream (two passes per step)
+    for name, si, ws in (("soa", 0, False), ("gather", 1, False), ("stream", 1, True)):
+        q = make_pusher(w, verify=verify, sort_interval=si, mode=3, flr_ws=ws)
         q.push(6, w.dt)
-        res[si], _, ids = q.state()
+        res[name], _, ids = q.state()
+        assert np.array_equal(np.sort(ids), np.arange(w.n_markers))
+    for name in ("gather", "stream"):
+        for k in KEYS:
+            assert np.array_equal(res["soa"][k], res[name][k]), (name, k)
+    assert np.abs(res["soa"]["vx"] - lin["vx"]).max() > 1e-7          # the average changes the orbit itself
+
+
+def test_nonlinear_gyro_average_ring_stream_with_lost_markers_and_ring_points_outside():
+    """Mode 3 through the ring stream on markers loaded at the edge of the mesh with large gyro-radii: ring points fall
+    outside the mesh (zero contribution), markers are lost on the way (their slots carry no ring) and the ordering changes
+    every step; chained steps against the oracle, and bit for bit against the per-lane gathers."""
+    from synth.configs import CHARGE, MASS
+    w0 = synth.make_config(3, n_markers=4000 + 9, nx=48, dt_gyro=16.0)
+    mk = synth.load_markers(w0.eq, 4000 + 9, 99, CHARGE, MASS, w0.dt, rmin=0.85, rmax=1.09, profile_L=None,
+                            speed="slowing", v_c=0.3, pitch="uniform")
+    mk["mu"] = mk["mu"] * 3.0
+    w = dataclasses.replace(w0, markers=mk)
+    mesh, sp = oracle_of(w, mode=3)
+    nsteps = 7
+    ref, e_ref, lost = oracle_push(mesh, sp, mk, nsteps, w.dt)
+    assert lost > 100
+    res = {}
+    for name, ws in (("gather", False), ("stream", True)):
+        q = make_pusher(w, verify=True, sort_interval=1, mode=3, flr_ws=ws)
+        q.push(nsteps, w.dt)
+        res[name], _, ids = q.state()
         assert np.array_equal(np.sort(ids), np.arange(w.n_markers))
     for k in KEYS:
-        assert np.array_equal(res[0][k], res[1][k]), k
-    assert np.abs(res[0]["vx"] - lin["vx"]).max() > 1e-7          # the average changes the orbit itself
+        assert np.array_equal(res["gather"][k], res["stream"][k]), k
+    wrms = np.sqrt(np.mean(ref["w"][e_ref >= 0] ** 2))
+    ex, ev, ew = g16_errors(res["stream"], ref, w_floor=wrms)
+    assert max(ex.max(), ev.max(), ew.max()) <= nsteps * TOL_STEP, (ex.max(), ev.max(), ew.max())
