@@ -476,7 +476,7 @@ __device__ __forceinline__ void flr_emit(const PushParams &P, const EqOut &f, co
 
 // element of every ring point (the key of the ring ordering; n_elems = outside the mesh, -1 = the slot of a lost marker)
 // and its rank inside the key, from the ring histogram (warp-aggregated atomics)
-__global__ void __launch_bounds__(256) ring_key_kernel(const __grid_constant__ FieldParams f, long n4,
+__global__ void __launch_bounds__(256, 6) ring_key_kernel(const __grid_constant__ FieldParams f, long n4,
                                                        const double *__restrict__ ring, int *__restrict__ rkey,
                                                        int *__restrict__ rrank, int *__restrict__ rhist, unsigned cstride) {
     // ring points are in the order of the markers' elements, so neighbouring blocks would hit the same few histogram bins
@@ -567,6 +567,11 @@ __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, con
         Zn[r] = s[r].z;
     }
     int key[R];
+    FastRec rec[kPost ? 1 : R];
+    if constexpr (!kPost) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) rec[r] = locate_first(P.f.fast, Rn[r], Zn[r]);   // all first records in flight together
+    }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         int ne = -1;
@@ -575,7 +580,7 @@ __device__ __forceinline__ void step_R_nl(const PushParams &P, const IO &io, con
             io.store_vel(mo[r], s[r].vx, s[r].vy, s[r].vz, s[r].mu);
             if (P.f.n_modes > 0) io.store_w(mo[r], s[r].w);
             if constexpr (!kPost) {
-                ne = locate_any(P.f, Rn[r], Zn[r]);
+                ne = locate_finish(P.f, rec[r], Rn[r], Zn[r]);
                 io.store_key(mo[r], ne);
             }
         }
