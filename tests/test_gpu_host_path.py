@@ -126,10 +126,10 @@ def test_fields_attach_binds_a_copy_of_the_workspace():
         m3dk.Pusher(device=0, verify=False).fields_attach(garbage, 1, 0)
 
 
-@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("mode", [1, 2, 3])
 def test_push_host_two_chunks_in_flight_in_the_other_modes(mode):
     """The chunk pipeline keeps two chunks in flight on two compute streams, each with its own carving of the sort and
-    FLR workspaces: non-linear mode and the FLR ring stream (mode 2) against the oracle, 5 chunks (odd: the slots alternate
+    FLR workspaces: non-linear mode and the FLR ring streams (modes 2 and 3) against the oracle, 5 chunks (odd: the slots alternate
     unevenly), and bitwise against the one-chunk call."""
     w = synth.make_config(3, n_markers=7000 + 13, nx=48)
     mesh, sp = oracle_of(w, mode=mode)
