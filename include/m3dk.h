@@ -190,15 +190,17 @@ int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, double *hz, d
 
 /* The host-buffer path as ONE call, pipelined by marker chunk: equivalent to m3dk_particles_upload -> m3dk_push(nsteps, dt)
  * -> m3dk_particles_download on the same HOST buffers (in place: on return they hold the new state), but the n markers are
- * cut into n_chunks contiguous chunks and chunk c uploads while chunk c - 1 runs its nsteps steps and chunk c - 2
+ * cut into n_chunks contiguous chunks (with four or more, of sizes that ramp up and down again, weights 1, 2, 3, 4, .., 4,
+ * 3, 2, 1: the first upload and the last download, which nothing overlaps, are short) and chunk c uploads while chunk c - 1 runs its nsteps steps and chunk c - 2
  * downloads (markers are independent; the three run on three streams, the two copy directions concurrently).
  * Sorts act inside a chunk: slot i of chunk c holds the marker host_id[i], with ids global (0..n-1 = the caller's order at
  * entry).  host_id / host_elem may be NULL.  Pinned buffers are needed for the copies to overlap.  Every chunk steps from
  * the same time; t advances by nsteps * dt once.  The call needs the device arrays of m3dk_particles_init (n markers) and,
  * for sort_interval >= 1, the sort workspace; it synchronises before returning.  n_chunks = 1 is the unpipelined path.
  * Two chunks are in flight at a time on two compute streams (the context's and one of the library's own), each with a
- * chunk-sized carving of the sort (and FLR) workspace, when two carvings fit the registered workspace (they do for
- * n_chunks >= 2 and the sizes m3dk_sort_workspace_bytes / m3dk_flr_workspace_bytes return for n markers); work enqueued on
+ * carving of the sort (and FLR) workspace sized for the largest chunk, when two carvings fit the registered workspace (they
+ * do for n_chunks >= 3 and the sizes m3dk_sort_workspace_bytes / m3dk_flr_workspace_bytes return for n markers; else one
+ * chunk is in flight at a time); work enqueued on
  * the context's stream afterwards is ordered behind both.
  * A chunk is a range of the buffers and stays that set of markers from call to call.  Chunks of a marker stream in random
  * order see a mesh n_chunks times sparser per chunk (fewer markers per element, less sharing of coefficient tiles), and a
