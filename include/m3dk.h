@@ -191,8 +191,9 @@ int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, double *hz, d
 /* The host-buffer path as ONE call, pipelined by marker chunk: equivalent to m3dk_particles_upload -> m3dk_push(nsteps, dt)
  * -> m3dk_particles_download on the same HOST buffers (in place: on return they hold the new state), but the n markers are
  * cut into n_chunks contiguous chunks (with four or more, of sizes that ramp up and down again, weights 1, 2, 3, 4, .., 4,
- * 3, 2, 1: the first upload and the last download, which nothing overlaps, are short) and chunk c uploads while chunk c - 1 runs its nsteps steps and chunk c - 2
- * downloads (markers are independent; the three run on three streams, the two copy directions concurrently).
+ * 3, 2, 1: the first upload and the last download, which nothing overlaps, are short) and chunk c uploads while chunk
+ * c - 1 runs its nsteps steps and chunk c - 2 downloads (markers are independent; uploads, steps and
+ * downloads run on streams of their own, the two copy directions concurrently).
  * Sorts act inside a chunk: slot i of chunk c holds the marker host_id[i], with ids global (0..n-1 = the caller's order at
  * entry).  host_id / host_elem may be NULL.  Pinned buffers are needed for the copies to overlap.  Every chunk steps from
  * the same time; t advances by nsteps * dt once.  The call needs the device arrays of m3dk_particles_init (n markers) and,
