@@ -379,7 +379,7 @@ def run_ours(args, rank, world, local_rank):
             "e2e": {"value": shard.whole_job_rate([N] * world, Ke, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": 64 * N / Ke,
                     "d2h_bytes_per_step": 64 * N / Ke,
                     "note": f"m3dk_push_host: one upload + {Ke} steps + one download per call (PAPER.md:237), pipelined in "
-                            f"{C_e2e} marker chunks; host buffers pinned, order of the markers: {args.e2e_order}"},
+                            f"{C_e2e if C_e2e else 'an automatic number of'} marker chunks; host buffers pinned, order of the markers: {args.e2e_order}"},
             "roofline": roof, "n_lost": st["n_lost"]}
     if args.gc:
         # row (f)-3: RK4 guiding-centre steps on the same markers (x, y, z as X; v_par = 0.5 for every marker)
@@ -484,7 +484,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-order", choices=("shell", "element", "loaded"), default="shell",
                     help="order of the host buffers of the e2e leg: radial shells, the element order a one-chunk call returns, as loaded")
-    ap.add_argument("--e2e-chunks", type=int, default=8, help="marker chunks of the pipelined host-buffer call (e2e leg)")
+    ap.add_argument("--e2e-chunks", type=int, default=0, help="marker chunks of the pipelined host-buffer call (e2e leg); 0 = the library chooses")
     ap.add_argument("--push-variant", type=int, default=0, choices=[0, 1],
                     help="m3dk_set_push_variant: 0 = default kernel, 1 = asynchronously staged kernel (A/B comparison)")
     ap.add_argument("--traffic-from", default=None,

@@ -197,7 +197,8 @@ int m3dk_particles_download(m3dk_ctx *ctx, double *hx, double *hy, double *hz, d
  * Sorts act inside a chunk: slot i of chunk c holds the marker host_id[i], with ids global (0..n-1 = the caller's order at
  * entry).  host_id / host_elem may be NULL.  Pinned buffers are needed for the copies to overlap.  Every chunk steps from
  * the same time; t advances by nsteps * dt once.  The call needs the device arrays of m3dk_particles_init (n markers) and,
- * for sort_interval >= 1, the sort workspace; it synchronises before returning.  n_chunks = 1 is the unpipelined path.
+ * for sort_interval >= 1, the sort workspace; it synchronises before returning.  n_chunks = 1 is the unpipelined path;
+ * n_chunks = 0 lets the library choose (8, 4 or 3 chunks by the ratio of transfer to compute time; 1 below 2^18 markers).
  * Two chunks are in flight at a time on two compute streams (the context's and one of the library's own), each with a
  * carving of the sort (and FLR) workspace sized for the largest chunk, when two carvings fit the registered workspace (they
  * do for n_chunks >= 3 and the sizes m3dk_sort_workspace_bytes / m3dk_flr_workspace_bytes return for n markers; else one

@@ -677,12 +677,21 @@ extern "C" int m3dk_push_host(m3dk_ctx *ctx, double *hx, double *hy, double *hz,
     if (!ctx) return M3DK_EINVAL;
     if (!ctx->have_fields || !ctx->have_markers) return fail(ctx, M3DK_ESTATE, "m3dk_push_host: fields and markers must be set first");
     if (!hx || !hy || !hz || !hvx || !hvy || !hvz || !hmu || !hw) return fail(ctx, M3DK_EINVAL, "m3dk_push_host: NULL buffer");
-    if (nsteps < 0 || !(dt == dt) || n_chunks < 1) return fail(ctx, M3DK_EINVAL, "m3dk_push_host: nsteps < 0, dt is NaN or n_chunks < 1");
+    if (nsteps < 0 || !(dt == dt) || n_chunks < 0) return fail(ctx, M3DK_EINVAL, "m3dk_push_host: nsteps < 0, dt is NaN or n_chunks < 0");
     if (ctx->sort_interval > 0 && !ctx->have_sortws)
         return fail(ctx, M3DK_ESTATE, "m3dk_push_host: sort_interval > 0 needs m3dk_set_sort_workspace");
     CU(cudaSetDevice(ctx->device), "cudaSetDevice");
     const long n = ctx->n;
     if (n == 0) return M3DK_OK;
+    if (n_chunks == 0) {
+        // automatic: many chunks hide the transfers, few chunks keep the work items full and the fixed cost of a chunk-step
+        // low.  What decides is the ratio of transfer time (64 B per marker and direction at about 50 GB/s) to compute time
+        // (about 80 / 100 / 400 / 420 ps per marker-step in modes 0 .. 3 on a B200); measured at 2^24 markers, mode 0:
+        // 20 steps (ratio 0.8) best with 8 chunks, 50 steps (0.3) with 4, 200 steps (0.08) with 3.
+        static const double kStepCost[4] = {80e-12, 100e-12, 400e-12, 420e-12};
+        const double ratio = nsteps > 0 ? (64.0 / 50e9) / ((double)nsteps * kStepCost[ctx->mode & 3]) : 1.0;
+        n_chunks = n < (1L << 18) ? 1 : ratio >= 0.6 ? 8 : ratio >= 0.15 ? 4 : 3;
+    }
     if ((long)n_chunks > n) n_chunks = (int)n;
     if (!ctx->s_up) {
         CU(cudaStreamCreateWithFlags(&ctx->s_up, cudaStreamNonBlocking), "create upload stream");

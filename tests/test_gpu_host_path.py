@@ -17,7 +17,7 @@ def _pinned(markers):
 
 
 @pytest.mark.parametrize("si", [1, 0])
-@pytest.mark.parametrize("n_chunks", [1, 3, 7])
+@pytest.mark.parametrize("n_chunks", [0, 1, 3, 7])      # 0: the library chooses
 def test_push_host_matches_the_oracle(n_chunks, si):
     """m3dk_push_host in place on pinned host buffers: ids are a permutation of the caller's indices (global across the
     chunks), every marker carries its own mu, and the state is the oracle's after nsteps steps from t0; the context's
